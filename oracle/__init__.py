@@ -1,0 +1,207 @@
+"""fp64 CPU oracle for the sCWatter field-evaluation hot path -- TEST INFRASTRUCTURE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+leg may import this package.  It never imports the CUDA package and shares no code
+with it.  Citations are PAPER.md line numbers (arxiv 2404.07293).
+
+Tier A  (scw_oracle.c)  : the plain definition -- eq. 34 with eq. 10's factor, one
+                          term at a time (sample, mode j, frequency m), long-double sums.
+Tier B  (tier_b_* here) : the paper's own factored algorithm O(M^2 Fz + M F)
+                           in numpy complex128, a separate
+                          statement used to compare *every* sample of the large
+                          configs; it is itself validated against Tier A in
+                          tests/test_oracle_pins.py.
+
+A "layer" is passed as keyword data (numpy arrays, python scalars):
+  U, Vn, X, Y, lam, z_lo, z_hi, V (shape (J, ldV): column-major [ldV x J], complex64 or
+  complex128), c ((J,) complex or None), gamma ((J,) complex128), dir ((J,) int8 or None).
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from .build import build as _build
+
+_LIB = None
+
+
+def lib():
+    global _LIB
+    if _LIB is None:
+        path = _build()
+        L = ctypes.CDLL(path)
+        dp = ctypes.c_void_p
+        L.scwo_threads.restype = ctypes.c_int
+        L.scwo_set_threads.argtypes = [ctypes.c_int]
+        L.scwo_sz.argtypes = [ctypes.c_double] * 4 + [dp]
+        L.scwo_index_map.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp]
+        L.scwo_green.argtypes = [ctypes.c_double] * 5 + [dp]
+        L.scwo_layer_samples.argtypes = [
+            ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+            ctypes.c_double, ctypes.c_double, ctypes.c_int64,
+            dp, ctypes.c_int, ctypes.c_int64, dp, dp, dp, ctypes.c_int64, dp, dp]
+        L.scwo_planewaves.argtypes = [
+            ctypes.c_int64, ctypes.c_double, dp, dp, dp, dp, dp, ctypes.c_int,
+            ctypes.c_int64, dp, dp]
+        _LIB = L
+    return _LIB
+
+
+def threads() -> int:
+    return int(lib().scwo_threads())
+
+
+def set_threads(n: int) -> None:
+    lib().scwo_set_threads(int(n))
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+# ----------------------------------------------------------------------------- small pieces
+def sz(n, sx, sy) -> complex:
+    """eq. 2, branch Im >= 0."""
+    out = np.zeros(2)
+    n = complex(n)
+    lib().scwo_sz(n.real, n.imag, float(sx), float(sy), _ptr(out))
+    return complex(out[0], out[1])
+
+
+def index_map(U: int, Vn: int, m: int):
+    """eq. 6 index map: m -> (u, v)."""
+    u = ctypes.c_int()
+    v = ctypes.c_int()
+    lib().scwo_index_map(U, Vn, m, ctypes.byref(u), ctypes.byref(v))
+    return u.value, v.value
+
+
+def green(A, za, zb, lam) -> complex:
+    """eq. 7: G(A, z_a, z_b) = exp[ik (z_b - z_a) A]."""
+    out = np.zeros(2)
+    A = complex(A)
+    lib().scwo_green(A.real, A.imag, float(za), float(zb), float(lam), _ptr(out))
+    return complex(out[0], out[1])
+
+
+# ----------------------------------------------------------------------------- Tier A
+def _prep_layer(V, c, gamma, dir):
+    assert V.ndim == 2 and V.flags.c_contiguous and V.dtype in (np.complex64, np.complex128)
+    J, ldV = V.shape
+    gamma = np.ascontiguousarray(gamma, dtype=np.complex128)
+    assert gamma.shape == (J,)
+    c128 = None if c is None else np.ascontiguousarray(c, dtype=np.complex128)
+    d8 = None if dir is None else np.ascontiguousarray(dir, dtype=np.int8)
+    return J, ldV, gamma, c128, d8
+
+
+def layer_samples(*, U, Vn, X, Y, lam, z_lo, z_hi, V, gamma, c=None, dir=None, xyz, **_):
+    """Tier A at arbitrary samples xyz [n,3] -> E [n,3] complex128."""
+    J, ldV, gamma, c128, d8 = _prep_layer(V, c, gamma, dir)
+    assert ldV >= 3 * U * Vn
+    xyz = np.ascontiguousarray(xyz, dtype=np.float64)
+    n = xyz.shape[0]
+    E = np.zeros((n, 3), dtype=np.complex128)
+    lib().scwo_layer_samples(U, Vn, X, Y, lam, z_lo, z_hi, J, _ptr(V),
+                             int(V.dtype == np.complex64), ldV, _ptr(c128), _ptr(gamma),
+                             _ptr(d8), n, _ptr(xyz), _ptr(E))
+    return E
+
+
+def grid_points(x, y, z):
+    """xyz [Fz*Ny*Nx, 3] in the planar output order [z][y][x] (x fastest)."""
+    zz, yy, xx = np.meshgrid(z, y, x, indexing="ij")
+    return np.stack([xx.ravel(), yy.ravel(), zz.ravel()], axis=1)
+
+
+def layer_grid(*, x, y, z, **layer):
+    """Tier A on a rectilinear grid -> E [Fz, 3, Ny, Nx] complex128 (planar layout)."""
+    E = layer_samples(xyz=grid_points(x, y, z), **layer)
+    return np.ascontiguousarray(E.reshape(len(z), len(y), len(x), 3).transpose(0, 3, 1, 2))
+
+
+def planewaves(*, lam, sx, sy, gamma, zref, p, xyz, **_):
+    """Plane-wave form (eq. 3 / eq. 9-10): E [n,3] complex128."""
+    sx = np.ascontiguousarray(sx, dtype=np.float64)
+    sy = np.ascontiguousarray(sy, dtype=np.float64)
+    gamma = np.ascontiguousarray(gamma, dtype=np.complex128)
+    zref = np.ascontiguousarray(zref, dtype=np.float64)
+    assert p.dtype in (np.complex64, np.complex128) and p.flags.c_contiguous
+    J = sx.shape[0]
+    assert p.shape == (J, 3)
+    xyz = np.ascontiguousarray(xyz, dtype=np.float64)
+    n = xyz.shape[0]
+    E = np.zeros((n, 3), dtype=np.complex128)
+    lib().scwo_planewaves(J, lam, _ptr(sx), _ptr(sy), _ptr(gamma), _ptr(zref), _ptr(p),
+                          int(p.dtype == np.complex64), n, _ptr(xyz), _ptr(E))
+    return E
+
+
+# ----------------------------------------------------------------------------- Tier B
+def _dirs(gamma, dir):
+    if dir is not None:
+        return np.where(np.asarray(dir) > 0, 1, -1)
+    return np.where((gamma.imag > 0) | ((gamma.imag == 0) & (gamma.real >= 0)), 1, -1)
+
+
+def tier_b_weights(*, lam, z_lo, z_hi, gamma, c=None, dir=None, z, **_):
+    """g(z) of PAPER.md:430-432 times alpha: W[j,i] = c_j G(gamma_j, zref_j, z_i) (eq. 7, 30)."""
+    gamma = np.asarray(gamma, dtype=np.complex128)
+    zref = np.where(_dirs(gamma, dir) > 0, z_lo, z_hi)
+    dz = np.asarray(z, dtype=np.float64)[None, :] - zref[:, None]
+    W = np.exp(2j * np.pi * gamma[:, None] * dz / lam)
+    if c is not None:
+        W = W * np.asarray(c, dtype=np.complex128)[:, None]
+    return W
+
+
+def tier_b_spectra(*, U, Vn, V, z, **layer):
+    """P(z) = [Q diag(alpha)] g(z): [3M, Fz] complex128, library matmul."""
+    R = 3 * U * Vn
+    W = tier_b_weights(z=z, **layer)
+    Vm = V[:, :R].astype(np.complex128, copy=False).T      # [R, J] view of col-major storage
+    return Vm @ W
+
+
+def twiddles(n_freq, coords, period):
+    """exp(i k s_u x) = exp(i 2 pi u x / X), u = -floor(n/2).. (eq. 6, eq. 10)."""
+    u = np.arange(n_freq) - n_freq // 2
+    t = np.outer(np.asarray(coords, dtype=np.float64) / period, u)
+    t = t - np.rint(t)
+    return np.exp(2j * np.pi * t)
+
+
+def tier_b_synthesize(*, U, Vn, X, Y, P, x, y, **_):
+    """eq. 10 on a rectilinear grid, separably: E_comp = F_x P_comp F_y^T -> [Fz,3,Ny,Nx]."""
+    M = U * Vn
+    Fz = P.shape[1]
+    Fx = twiddles(U, x, X)            # [Nx, U]
+    Fy = twiddles(Vn, y, Y)           # [Ny, Vn]
+    E = np.empty((Fz, 3, len(y), len(x)), dtype=np.complex128)
+    for i in range(Fz):
+        for comp in range(3):
+            Pc = P[comp * M:(comp + 1) * M, i].reshape(Vn, U)   # [v, u], u fastest
+            E[i, comp] = Fy @ Pc @ Fx.T                          # [Ny, Nx]
+    return E
+
+
+def tier_b_grid(*, x, y, z, **layer):
+    P = tier_b_spectra(z=z, **layer)
+    return tier_b_synthesize(P=P, x=x, y=y, **layer)
+
+
+def tier_b_points(*, U, Vn, X, Y, xyz, chunk=2048, **layer):
+    """Factored evaluation at scattered points: P(z_p) per point, then the M-term sum."""
+    M = U * Vn
+    xyz = np.asarray(xyz, dtype=np.float64)
+    E = np.empty((xyz.shape[0], 3), dtype=np.complex128)
+    for s in range(0, xyz.shape[0], chunk):
+        q = xyz[s:s + chunk]
+        P = tier_b_spectra(U=U, Vn=Vn, z=q[:, 2], **layer)       # [3M, n]
+        Fx = twiddles(U, q[:, 0], X)                               # [n, U]
+        Fy = twiddles(Vn, q[:, 1], Y)                              # [n, Vn]
+        T = (Fy[:, :, None] * Fx[:, None, :]).reshape(len(q), M)   # [n, m], u fastest
+        for comp in range(3):
+            E[s:s + chunk, comp] = np.einsum("nm,mn->n", T, P[comp * M:(comp + 1) * M])
+    return E
