@@ -1,0 +1,188 @@
+/*
+ * scwatter.h -- C ABI of libscw: B200-native (sm_100a) field evaluation for the coupled-wave
+ * method of arXiv 2404.07293 ("sCWatter").  Citations are PAPER.md line numbers.
+ *
+ * The library evaluates the plane-wave-expanded electric field (discrete eq. 3)
+ *
+ *     E(r) = sum_j sum_m  c_j V[(comp,m), j] exp(i k s_m . (x,y)) G(gamma_j, zref_j, z)
+ *
+ * inside one sample layer (eq. 30/31/34, recomposed with eq. 10,
+ * PAPER.md:119-124, 382) on rectilinear grids and at scattered points.
+ *
+ * CONVENTIONS
+ *  - Every function returns an int32_t status (SCW_OK == 0).  Nothing throws, aborts or prints.
+ *    All validation happens on the host BEFORE anything is enqueued; on error nothing is written.
+ *    scw_last_error() returns a ctx-owned message for the last failing call.
+ *  - Pointers are DEVICE pointers unless the comment says HOST.  Device pointers must be aligned
+ *    to the complex element size (8 B for SCW_C64, 16 B for SCW_C128; 8 B for doubles).
+ *  - Complex numbers are interleaved (re, im).  SCW_C64 = 2 x fp32, SCW_C128 = 2 x fp64.
+ *  - Ownership: the caller owns every input, output and workspace buffer.  The library never
+ *    allocates or frees device memory and keeps no caller pointer past the call, except the
+ *    workspace registered with scw_set_workspace(), which it uses as scratch during calls.
+ *  - Asynchrony: all work is enqueued on the ctx's CUDA stream; no call synchronises.  Outputs
+ *    are valid once the caller has synchronised that stream.  Descriptor structs are HOST memory
+ *    and are copied by value during the call.
+ *  - One ctx per host thread.  There is no CPU fallback: scw_create fails with
+ *    SCW_ERR_UNSUPPORTED on a device that is not compute capability 10.x.
+ *
+ * INDEXING (eq. 6): M = U*Vn spatial frequencies, m = (v + Vn/2)*U + (u + U/2),
+ * u in [-floor(U/2), floor((U-1)/2)], s_m = lambda (u/X, v/Y).  Rows of V and P are comp*M + m with
+ * comp = 0,1,2 for x,y,z (P = [P_x; P_y; P_z], eq. 28).
+ * MODES (eq. 23/30): J columns, normally J = 4M.  A "+" mode
+ * (dir = +1, gamma = +sqrt, Im gamma >= 0) is referenced at z_lo = z_{l-1}; a "-" mode
+ * (dir = -1) at z_hi = z_l, so that every exponential decays inside [z_lo, z_hi].
+ */
+#ifndef SCWATTER_H
+#define SCWATTER_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct scw_ctx scw_ctx;
+
+enum {
+    SCW_OK = 0,
+    SCW_ERR_NULL = 1,        /* a required pointer is NULL */
+    SCW_ERR_SHAPE = 2,       /* non-positive / inconsistent dimension, leading dimension too small */
+    SCW_ERR_DTYPE = 3,       /* dtype is neither SCW_C64 nor SCW_C128 */
+    SCW_ERR_ALIGN = 4,       /* device pointer not aligned to its element size */
+    SCW_ERR_VALUE = 5,       /* lambda <= 0, X <= 0, Y <= 0, z_hi < z_lo, non-finite scalar */
+    SCW_ERR_WORKSPACE = 6,   /* registered workspace too small; see scw_required_workspace() */
+    SCW_ERR_CUDA = 7,        /* a CUDA runtime call failed; see scw_last_cuda_error() */
+    SCW_ERR_UNSUPPORTED = 8  /* device is not sm_100-class, or an option value is unknown */
+};
+
+enum { SCW_C64 = 0, SCW_C128 = 1 };
+
+/* Which kernels implement the two contractions (scw_set_option(ctx, SCW_OPT_PATH, v)). */
+enum { SCW_OPT_PATH = 1 };
+enum {
+    SCW_PATH_AUTO = 0,    /* tcgen05 tensor-core kernels where shape/dtype allow, CUDA-core otherwise */
+    SCW_PATH_SIMT = 1,    /* CUDA-core kernels only (fp32 FMA for C64, fp64 DFMA for C128) */
+    SCW_PATH_TENSOR = 2   /* tensor-core kernels only; SCW_ERR_UNSUPPORTED if they cannot run */
+};
+
+/* ---------------------------------------------------------------- lifecycle */
+
+/* Create a context bound to `device` and to `cuda_stream` (a cudaStream_t, may be 0 = legacy
+ * default stream).  HOST: out.  Errors: NULL, CUDA, UNSUPPORTED. */
+int32_t scw_create(scw_ctx** out, int32_t device, void* cuda_stream);
+int32_t scw_destroy(scw_ctx* ctx);
+int32_t scw_set_stream(scw_ctx* ctx, void* cuda_stream);
+/* Register caller-owned device scratch (256-byte aligned).  May be (NULL, 0). */
+int32_t scw_set_workspace(scw_ctx* ctx, void* dev_ptr, size_t bytes);
+int32_t scw_set_option(scw_ctx* ctx, int32_t option, int64_t value);
+/* Message / raw cudaError_t / required workspace bytes of the last failing call on this ctx. */
+const char* scw_last_error(const scw_ctx* ctx);
+int32_t scw_last_cuda_error(const scw_ctx* ctx);
+size_t scw_required_workspace(const scw_ctx* ctx);
+/* Number of kernels this ctx has launched since creation (monotone counter). */
+int64_t scw_launch_count(const scw_ctx* ctx);
+/* Library version: major*10000 + minor*100 + patch. */
+int32_t scw_version(void);
+
+/* ---------------------------------------------------------------- descriptors (HOST PODs) */
+
+/* One layer at one wavelength. */
+typedef struct {
+    uint32_t struct_size;      /* = sizeof(scw_layer) */
+    int32_t dtype;             /* SCW_C64 | SCW_C128: element type of V, c, P, E */
+    int32_t U, Vn;             /* frequency grid (eq. 6) */
+    double X, Y;               /* patch size, same unit as lambda (eq. 6) */
+    double lambda;             /* vacuum wavelength, k = 2 pi / lambda (eq. 3) */
+    double z_lo, z_hi;         /* z_{l-1}, z_l: the layer's interfaces (eq. 30) */
+    int64_t J;                 /* number of modes (columns of V), normally 4*U*Vn (eq. 23) */
+    const void* V;             /* [ldV x J] column-major complex<dtype>, rows comp*M+m (eq. 28, 34) */
+    int64_t ldV;               /* >= 3*U*Vn */
+    const void* c;             /* [J] complex<dtype> coefficients alpha_j, NULL = ones (eq. 23) */
+    const double* gamma;       /* [J] complex128 signed z-wavenumbers Gamma_jj (eq. 22-23) */
+    const int8_t* dir;         /* [J] +1 / -1 reference face, NULL = derive from the sign of gamma */
+} scw_layer;
+
+enum { SCW_MODES_PLANEWAVE = 0, SCW_MODES_DENSE = 1 };
+
+/* Mode table of the point path. */
+typedef struct {
+    uint32_t struct_size;      /* = sizeof(scw_modes) */
+    int32_t kind;              /* SCW_MODES_PLANEWAVE | SCW_MODES_DENSE */
+    /* SCW_MODES_PLANEWAVE: one plane wave per mode (eq. 3, eq. 9-10; any s_m) */
+    int32_t dtype;             /* type of p and E */
+    int64_t J;
+    double lambda;
+    const double* sx;          /* [J] direction cosines s_x = lambda u / X */
+    const double* sy;          /* [J] */
+    const double* gamma;       /* [J] complex128 s_z, signed */
+    const double* zref;        /* [J] reference plane of each wave */
+    const void* p;             /* [J x 3] complex<dtype> amplitudes, comp fastest */
+    /* SCW_MODES_DENSE: the full eq. 34 of one layer at scattered points */
+    scw_layer layer;
+} scw_modes;
+
+/* ---------------------------------------------------------------- the hot path */
+
+/*
+ * Spectral assembly (eq. 31 with the diag(alpha) factoring of PAPER.md:428-432):
+ *   P[:, i] = V . ( c o g(z_i) ),  g_j(z) = G(gamma_j, zref_j, z) = exp(i k gamma_j (z - zref_j))  (eq. 7)
+ * z: [Fz] doubles (device).  P: [ldP x Fz] column-major complex<dtype>, ldP >= 3*U*Vn.
+ * z outside [z_lo, z_hi] is evaluated as-is.  Workspace: see scw_assemble_workspace().
+ */
+int32_t scw_assemble_spectra(scw_ctx* ctx, const scw_layer* layer, int64_t Fz, const double* z,
+                             void* P, int64_t ldP);
+int32_t scw_assemble_workspace(scw_ctx* ctx, const scw_layer* layer, int64_t Fz, size_t* bytes);
+
+/*
+ * Separable Fourier synthesis (eq. 10 on a rectilinear grid):
+ *   E_comp(x_i, y_k, z_n) = sum_{u,v} P[comp*M + m(u,v), n] exp(i 2 pi (u x_i / X + v y_k / Y))
+ * x: [Nx], y: [Ny] doubles (device).  E: complex<dtype>, element (comp, n, k, i) at offset
+ * comp*strides[0] + n*strides[1] + k*strides[2] + i*strides[3] (in elements); strides == NULL
+ * (HOST pointer) means planar [Fz][3][Ny][Nx], x fastest.
+ */
+int32_t scw_synthesize_grid(scw_ctx* ctx, int32_t dtype, int32_t U, int32_t Vn, double X, double Y,
+                            int64_t Fz, const void* P, int64_t ldP,
+                            int64_t Nx, const double* x, int64_t Ny, const double* y,
+                            void* E, const int64_t* strides);
+int32_t scw_synthesize_workspace(scw_ctx* ctx, int32_t dtype, int32_t U, int32_t Vn, int64_t Fz,
+                                 int64_t Nx, int64_t Ny, size_t* bytes);
+
+/*
+ * Scattered points (eq. 3 / eq. 9-10 for SCW_MODES_PLANEWAVE, eq. 34 for SCW_MODES_DENSE).
+ * r: [N x 3] doubles (x,y,z per point).  E: [N x 3] complex<dtype>, comp fastest.
+ */
+int32_t scw_eval_points(scw_ctx* ctx, const scw_modes* modes, int64_t N, const double* r, void* E);
+int32_t scw_points_workspace(scw_ctx* ctx, const scw_modes* modes, int64_t N, size_t* bytes);
+
+/*
+ * Batched grid evaluation: assembly + synthesis for every (wavelength, layer) instance in one
+ * call (spectroscopy sweep).  All instances share U, Vn, X, Y, dtype and the
+ * x/y grid (the twiddles are wavelength-free: k s_m . r = 2 pi (u x/X + v y/Y), eq. 6).
+ * inst: HOST [n_inst].  Fz: HOST [n_inst].  z: HOST array of device pointers.  E: HOST array of
+ * device pointers, each laid out by `strides` as in scw_synthesize_grid.
+ */
+int32_t scw_sweep_wavelengths(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst,
+                              const int64_t* Fz, const double* const* z,
+                              int64_t Nx, const double* x, int64_t Ny, const double* y,
+                              void* const* E, const int64_t* strides);
+int32_t scw_sweep_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz,
+                            int64_t Nx, int64_t Ny, size_t* bytes);
+
+/*
+ * Same as scw_sweep_wavelengths with every array in HOST memory (V, c, gamma, dir, z[i], x, y, E[i];
+ * pinned memory recommended): inputs are staged host->device into the workspace, evaluated, and E is
+ * copied device->host, all on the ctx stream.  E[i] is planar [Fz][3][Ny][Nx].  h2d_bytes / d2h_bytes
+ * (HOST, may be NULL) receive the bytes copied in each direction.
+ */
+int32_t scw_sweep_wavelengths_host(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst,
+                                   const int64_t* Fz, const double* const* z,
+                                   int64_t Nx, const double* x, int64_t Ny, const double* y,
+                                   void* const* E, int64_t* h2d_bytes, int64_t* d2h_bytes);
+int32_t scw_sweep_host_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst,
+                                 const int64_t* Fz, int64_t Nx, int64_t Ny, size_t* bytes);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SCWATTER_H */

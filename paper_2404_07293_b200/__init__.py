@@ -1,0 +1,12 @@
+"""B200-native (sm_100a) field evaluation for the coupled-wave method of arXiv 2404.07293.
+
+The product is libscw.so (include/scwatter.h); this package is its thin Python binding.
+Build the library in-tree with `python -m paper_2404_07293_b200.build`.
+"""
+from .binding import (SCW_C64, SCW_C128, SCW_PATH_AUTO, SCW_PATH_SIMT, SCW_PATH_TENSOR, Context, Layer,
+                      PlaneWaves, ScwError, lib, scw_assemble_spectra, scw_eval_points, scw_synthesize_grid,
+                      scw_sweep_wavelengths, scw_sweep_wavelengths_host)
+
+__all__ = ["SCW_C64", "SCW_C128", "SCW_PATH_AUTO", "SCW_PATH_SIMT", "SCW_PATH_TENSOR", "Context", "Layer",
+           "PlaneWaves", "ScwError", "lib", "scw_assemble_spectra", "scw_eval_points", "scw_synthesize_grid",
+           "scw_sweep_wavelengths", "scw_sweep_wavelengths_host"]

@@ -1,0 +1,309 @@
+"""Thin ctypes binding over libscw.so (include/scwatter.h): argument marshalling only.
+
+PyTorch supplies device memory and the CUDA stream; every step of the path runs in the
+library's kernels.  There is no CPU fallback: importing is cheap, but any call raises
+ScwError / RuntimeError if libscw.so is missing or the device is not an sm_100 GPU.
+"""
+import ctypes
+import os
+from ctypes import (POINTER, Structure, byref, c_char_p, c_double, c_int8, c_int32, c_int64, c_size_t,
+                    c_uint32, c_void_p)
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libscw.so")
+
+SCW_C64, SCW_C128 = 0, 1
+SCW_MODES_PLANEWAVE, SCW_MODES_DENSE = 0, 1
+SCW_OPT_PATH = 1
+SCW_PATH_AUTO, SCW_PATH_SIMT, SCW_PATH_TENSOR = 0, 1, 2
+STATUS = {0: "SCW_OK", 1: "SCW_ERR_NULL", 2: "SCW_ERR_SHAPE", 3: "SCW_ERR_DTYPE", 4: "SCW_ERR_ALIGN",
+          5: "SCW_ERR_VALUE", 6: "SCW_ERR_WORKSPACE", 7: "SCW_ERR_CUDA", 8: "SCW_ERR_UNSUPPORTED"}
+
+EXPORTS = [
+    "scw_version", "scw_create", "scw_destroy", "scw_set_stream", "scw_set_workspace", "scw_set_option",
+    "scw_last_error", "scw_last_cuda_error", "scw_required_workspace", "scw_launch_count",
+    "scw_assemble_spectra", "scw_assemble_workspace", "scw_synthesize_grid", "scw_synthesize_workspace",
+    "scw_eval_points", "scw_points_workspace", "scw_sweep_wavelengths", "scw_sweep_workspace",
+    "scw_sweep_wavelengths_host", "scw_sweep_host_workspace",
+]
+
+
+class ScwError(RuntimeError):
+    def __init__(self, status, message=""):
+        self.status = status
+        super().__init__(f"{STATUS.get(status, status)}: {message}")
+
+
+class scw_layer(Structure):
+    _fields_ = [("struct_size", c_uint32), ("dtype", c_int32), ("U", c_int32), ("Vn", c_int32),
+                ("X", c_double), ("Y", c_double), ("lambda_", c_double), ("z_lo", c_double), ("z_hi", c_double),
+                ("J", c_int64), ("V", c_void_p), ("ldV", c_int64), ("c", c_void_p), ("gamma", c_void_p),
+                ("dir", c_void_p)]
+
+
+class scw_modes(Structure):
+    _fields_ = [("struct_size", c_uint32), ("kind", c_int32), ("dtype", c_int32), ("J", c_int64),
+                ("lambda_", c_double), ("sx", c_void_p), ("sy", c_void_p), ("gamma", c_void_p),
+                ("zref", c_void_p), ("p", c_void_p), ("layer", scw_layer)]
+
+
+_LIB = None
+
+
+def lib():
+    """Load libscw.so (built in-tree by paper_2404_07293_b200.build); fail loudly if absent."""
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2404_07293_b200.build` "
+                               "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        L.scw_last_error.restype = c_char_p
+        L.scw_required_workspace.restype = c_size_t
+        L.scw_launch_count.restype = c_int64
+        L.scw_create.argtypes = [POINTER(c_void_p), c_int32, c_void_p]
+        L.scw_destroy.argtypes = [c_void_p]
+        L.scw_set_stream.argtypes = [c_void_p, c_void_p]
+        L.scw_set_workspace.argtypes = [c_void_p, c_void_p, c_size_t]
+        L.scw_set_option.argtypes = [c_void_p, c_int32, c_int64]
+        L.scw_last_error.argtypes = [c_void_p]
+        L.scw_last_cuda_error.argtypes = [c_void_p]
+        L.scw_required_workspace.argtypes = [c_void_p]
+        L.scw_launch_count.argtypes = [c_void_p]
+        L.scw_assemble_spectra.argtypes = [c_void_p, POINTER(scw_layer), c_int64, c_void_p, c_void_p, c_int64]
+        L.scw_assemble_workspace.argtypes = [c_void_p, POINTER(scw_layer), c_int64, POINTER(c_size_t)]
+        L.scw_synthesize_grid.argtypes = [c_void_p, c_int32, c_int32, c_int32, c_double, c_double, c_int64,
+                                          c_void_p, c_int64, c_int64, c_void_p, c_int64, c_void_p, c_void_p,
+                                          POINTER(c_int64)]
+        L.scw_synthesize_workspace.argtypes = [c_void_p, c_int32, c_int32, c_int32, c_int64, c_int64, c_int64,
+                                               POINTER(c_size_t)]
+        L.scw_eval_points.argtypes = [c_void_p, POINTER(scw_modes), c_int64, c_void_p, c_void_p]
+        L.scw_points_workspace.argtypes = [c_void_p, POINTER(scw_modes), c_int64, POINTER(c_size_t)]
+        L.scw_sweep_wavelengths.argtypes = [c_void_p, c_int64, POINTER(scw_layer), POINTER(c_int64),
+                                            POINTER(c_void_p), c_int64, c_void_p, c_int64, c_void_p,
+                                            POINTER(c_void_p), POINTER(c_int64)]
+        L.scw_sweep_workspace.argtypes = [c_void_p, c_int64, POINTER(scw_layer), POINTER(c_int64), c_int64,
+                                          c_int64, POINTER(c_size_t)]
+        L.scw_sweep_wavelengths_host.argtypes = [c_void_p, c_int64, POINTER(scw_layer), POINTER(c_int64),
+                                                 POINTER(c_void_p), c_int64, c_void_p, c_int64, c_void_p,
+                                                 POINTER(c_void_p), POINTER(c_int64), POINTER(c_int64)]
+        L.scw_sweep_host_workspace.argtypes = [c_void_p, c_int64, POINTER(scw_layer), POINTER(c_int64), c_int64,
+                                               c_int64, POINTER(c_size_t)]
+        _LIB = L
+    return _LIB
+
+
+def _dt(t):
+    if t.dtype == torch.complex64:
+        return SCW_C64
+    if t.dtype == torch.complex128:
+        return SCW_C128
+    raise ScwError(3, f"unsupported tensor dtype {t.dtype}")
+
+
+def _p(t):
+    return None if t is None else c_void_p(t.data_ptr())
+
+
+class Layer:
+    """Tensors of one layer at one wavelength (device tensors, or host tensors for the *_host call).
+
+    V: (J, ldV) complex (column-major [ldV x J]); c: (J,) complex or None; gamma: (J,) complex128;
+    dir: (J,) int8 or None.
+    """
+
+    def __init__(self, *, U, Vn, X, Y, lam, z_lo, z_hi, V, gamma, c=None, dir=None, **_):
+        self.U, self.Vn, self.X, self.Y, self.lam = int(U), int(Vn), float(X), float(Y), float(lam)
+        self.z_lo, self.z_hi = float(z_lo), float(z_hi)
+        self.V, self.c, self.gamma, self.dir = V, c, gamma, dir
+        assert V.dim() == 2 and V.is_contiguous() and gamma.dtype == torch.complex128
+        assert c is None or c.dtype == V.dtype
+        assert dir is None or dir.dtype == torch.int8
+
+    @property
+    def J(self):
+        return self.V.shape[0]
+
+    @property
+    def R(self):
+        return 3 * self.U * self.Vn
+
+    def struct(self):
+        return scw_layer(ctypes.sizeof(scw_layer), _dt(self.V), self.U, self.Vn, self.X, self.Y, self.lam,
+                         self.z_lo, self.z_hi, self.V.shape[0], self.V.data_ptr(), self.V.shape[1],
+                         None if self.c is None else self.c.data_ptr(), self.gamma.data_ptr(),
+                         None if self.dir is None else self.dir.data_ptr())
+
+    @staticmethod
+    def from_numpy(d, device):
+        """Upload a scw_inputs / oracle-style dict of numpy arrays."""
+        t = lambda a: None if a is None else torch.from_numpy(a).to(device)
+        return Layer(U=d["U"], Vn=d["Vn"], X=d["X"], Y=d["Y"], lam=d["lam"], z_lo=d["z_lo"], z_hi=d["z_hi"],
+                     V=t(d["V"]), gamma=t(d["gamma"]), c=t(d.get("c")), dir=t(d.get("dir")))
+
+
+class PlaneWaves:
+    """Plane-wave mode table of the point path: sx, sy, zref (J,) float64; gamma (J,) complex128; p (J,3)."""
+
+    def __init__(self, *, lam, sx, sy, gamma, zref, p, **_):
+        self.lam, self.sx, self.sy, self.gamma, self.zref, self.p = float(lam), sx, sy, gamma, zref, p
+
+    def struct(self):
+        m = scw_modes()
+        m.struct_size = ctypes.sizeof(scw_modes)
+        m.kind = SCW_MODES_PLANEWAVE
+        m.dtype = _dt(self.p)
+        m.J = self.p.shape[0]
+        m.lambda_ = self.lam
+        m.sx, m.sy, m.gamma = self.sx.data_ptr(), self.sy.data_ptr(), self.gamma.data_ptr()
+        m.zref, m.p = self.zref.data_ptr(), self.p.data_ptr()
+        return m
+
+    @staticmethod
+    def from_numpy(d, device):
+        t = lambda a: torch.from_numpy(a).to(device)
+        return PlaneWaves(lam=d["lam"], sx=t(d["sx"]), sy=t(d["sy"]), gamma=t(d["gamma"]), zref=t(d["zref"]),
+                          p=t(d["p"]))
+
+
+class Context:
+    """scw_ctx bound to a torch device and stream; owns a growable torch workspace buffer."""
+
+    def __init__(self, device=0, stream=None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2404_07293_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.device = torch.device("cuda", device) if isinstance(device, int) else torch.device(device)
+        self.L = lib()
+        self._h = c_void_p()
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.stream = st
+        s = self.L.scw_create(byref(self._h), self.device.index or 0, c_void_p(st.cuda_stream))
+        if s != 0:
+            raise ScwError(s, "scw_create failed (device must be compute capability 10.x)")
+        self._ws = None
+
+    def close(self):
+        if self._h:
+            self.L.scw_destroy(self._h)
+            self._h = c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- helpers
+    def check(self, status):
+        if status != 0:
+            raise ScwError(status, self.L.scw_last_error(self._h).decode())
+
+    def last_error(self):
+        return self.L.scw_last_error(self._h).decode()
+
+    def launch_count(self):
+        return int(self.L.scw_launch_count(self._h))
+
+    def set_path(self, path):
+        self.check(self.L.scw_set_option(self._h, SCW_OPT_PATH, path))
+
+    def reserve(self, nbytes):
+        """Grow the registered workspace to at least nbytes."""
+        if nbytes and (self._ws is None or self._ws.numel() < nbytes):
+            self._ws = None
+            self._ws = torch.empty(int(nbytes), dtype=torch.uint8, device=self.device)
+            self.check(self.L.scw_set_workspace(self._h, c_void_p(self._ws.data_ptr()), self._ws.numel()))
+
+    def workspace_bytes(self):
+        return 0 if self._ws is None else self._ws.numel()
+
+
+# ---------------------------------------------------------------------------------------------
+def scw_assemble_spectra(ctx, layer, z, out=None):
+    """P = V (c o g(z)): returns P as a (Fz, ldP) tensor (column-major [ldP x Fz])."""
+    Fz = z.numel()
+    st = layer.struct()
+    need = c_size_t()
+    ctx.check(ctx.L.scw_assemble_workspace(ctx._h, byref(st), Fz, byref(need)))
+    ctx.reserve(need.value)
+    if out is None:
+        out = torch.empty((Fz, layer.R), dtype=layer.V.dtype, device=ctx.device)
+    ctx.check(ctx.L.scw_assemble_spectra(ctx._h, byref(st), Fz, _p(z), _p(out), out.shape[1] if Fz else layer.R))
+    return out
+
+
+def scw_synthesize_grid(ctx, *, U, Vn, X, Y, P, x, y, out=None, strides=None):
+    """E[n, comp, k, i] = sum_uv P[n, comp*M+m] exp(i 2 pi (u x_i/X + v y_k/Y)); P is (Fz, ldP)."""
+    Fz, Nx, Ny = P.shape[0], x.numel(), y.numel()
+    dt = _dt(P)
+    need = c_size_t()
+    ctx.check(ctx.L.scw_synthesize_workspace(ctx._h, dt, U, Vn, Fz, Nx, Ny, byref(need)))
+    ctx.reserve(need.value)
+    if out is None:
+        out = torch.empty((Fz, 3, Ny, Nx), dtype=P.dtype, device=ctx.device)
+    sarr = None if strides is None else (c_int64 * 4)(*strides)
+    ctx.check(ctx.L.scw_synthesize_grid(ctx._h, dt, U, Vn, X, Y, Fz, _p(P), P.shape[1], Nx, _p(x), Ny, _p(y),
+                                        _p(out), sarr))
+    return out
+
+
+def scw_eval_points(ctx, modes, r, out=None):
+    """E (N, 3) at points r (N, 3) float64; modes is a PlaneWaves table or a Layer (dense eq. 34)."""
+    N = r.shape[0]
+    if isinstance(modes, Layer):
+        m = scw_modes()
+        m.struct_size = ctypes.sizeof(scw_modes)
+        m.kind = SCW_MODES_DENSE
+        m.layer = modes.struct()
+        dtype = modes.V.dtype
+    else:
+        m = modes.struct()
+        dtype = modes.p.dtype
+    need = c_size_t()
+    ctx.check(ctx.L.scw_points_workspace(ctx._h, byref(m), N, byref(need)))
+    ctx.reserve(need.value)
+    if out is None:
+        out = torch.empty((N, 3), dtype=dtype, device=ctx.device)
+    ctx.check(ctx.L.scw_eval_points(ctx._h, byref(m), N, _p(r), _p(out)))
+    return out
+
+
+def _sweep_args(layers, zs):
+    n = len(layers)
+    inst = (scw_layer * max(n, 1))(*[l.struct() for l in layers])
+    Fz = (c_int64 * max(n, 1))(*[z.numel() for z in zs])
+    zp = (c_void_p * max(n, 1))(*[z.data_ptr() for z in zs])
+    return n, inst, Fz, zp
+
+
+def scw_sweep_wavelengths(ctx, layers, zs, x, y, out=None, strides=None):
+    """Assembly + synthesis for every (wavelength, layer) instance; returns a list of E tensors."""
+    n, inst, Fz, zp = _sweep_args(layers, zs)
+    Nx, Ny = x.numel(), y.numel()
+    need = c_size_t()
+    ctx.check(ctx.L.scw_sweep_workspace(ctx._h, n, inst, Fz, Nx, Ny, byref(need)))
+    ctx.reserve(need.value)
+    if out is None:
+        out = [torch.empty((z.numel(), 3, Ny, Nx), dtype=l.V.dtype, device=ctx.device) for l, z in zip(layers, zs)]
+    Ep = (c_void_p * max(n, 1))(*[e.data_ptr() for e in out])
+    sarr = None if strides is None else (c_int64 * 4)(*strides)
+    ctx.check(ctx.L.scw_sweep_wavelengths(ctx._h, n, inst, Fz, zp, Nx, _p(x), Ny, _p(y), Ep, sarr))
+    return out
+
+
+def scw_sweep_wavelengths_host(ctx, layers, zs, x, y, out=None):
+    """Host-buffer variant: every tensor lives in (pinned) host memory; returns (E list, h2d, d2h bytes)."""
+    n, inst, Fz, zp = _sweep_args(layers, zs)
+    Nx, Ny = x.numel(), y.numel()
+    need = c_size_t()
+    ctx.check(ctx.L.scw_sweep_host_workspace(ctx._h, n, inst, Fz, Nx, Ny, byref(need)))
+    ctx.reserve(need.value)
+    if out is None:
+        out = [torch.empty((z.numel(), 3, Ny, Nx), dtype=l.V.dtype).pin_memory() for l, z in zip(layers, zs)]
+    Ep = (c_void_p * max(n, 1))(*[e.data_ptr() for e in out])
+    up, down = c_int64(), c_int64()
+    ctx.check(ctx.L.scw_sweep_wavelengths_host(ctx._h, n, inst, Fz, zp, Nx, _p(x), Ny, _p(y), Ep, byref(up),
+                                               byref(down)))
+    return out, up.value, down.value

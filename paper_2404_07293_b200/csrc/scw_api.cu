@@ -1,0 +1,562 @@
+// C ABI of libscw: argument validation, workspace carving and kernel dispatch.
+// See include/scwatter.h for the contract of every entry point.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "scw_internal.h"
+
+using namespace scw;
+
+namespace {
+
+int32_t fail(scw_ctx* ctx, int32_t code, const char* fmt, ...)
+{
+    if (ctx) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(ctx->msg, sizeof(ctx->msg), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+inline size_t esize(int dtype) { return dtype == SCW_C64 ? 8 : 16; }
+inline bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
+
+constexpr int64_t MAX_FREQ = 4096;        // per-axis frequency count
+constexpr int64_t MAX_GRID = 1 << 20;     // per-axis grid points
+
+int32_t check_ctx(scw_ctx* ctx)
+{
+    if (!ctx) return SCW_ERR_NULL;
+    ctx->msg[0] = 0;
+    ctx->cuda_err = 0;
+    ctx->required_ws = 0;
+    int cur = -1;
+    cudaError_t e = cudaGetDevice(&cur);
+    if (e == cudaSuccess && cur != ctx->device) e = cudaSetDevice(ctx->device);
+    if (e != cudaSuccess) {
+        ctx->cuda_err = (int32_t)e;
+        return fail(ctx, SCW_ERR_CUDA, "cudaSetDevice(%d): %s", ctx->device, cudaGetErrorString(e));
+    }
+    return SCW_OK;
+}
+
+int32_t check_launch(scw_ctx* ctx, const char* what)
+{
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        ctx->cuda_err = (int32_t)e;
+        return fail(ctx, SCW_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+    }
+    return SCW_OK;
+}
+
+int32_t check_layer(scw_ctx* ctx, const scw_layer* L, const char* who)
+{
+    if (!L) return fail(ctx, SCW_ERR_NULL, "%s: layer is NULL", who);
+    if (L->struct_size != sizeof(scw_layer))
+        return fail(ctx, SCW_ERR_SHAPE, "%s: layer.struct_size %u != %zu", who, L->struct_size, sizeof(scw_layer));
+    if (L->dtype != SCW_C64 && L->dtype != SCW_C128) return fail(ctx, SCW_ERR_DTYPE, "%s: bad dtype %d", who, L->dtype);
+    if (L->U <= 0 || L->Vn <= 0 || L->U > MAX_FREQ || L->Vn > MAX_FREQ)
+        return fail(ctx, SCW_ERR_SHAPE, "%s: U=%d Vn=%d out of range", who, L->U, L->Vn);
+    if (L->J <= 0) return fail(ctx, SCW_ERR_SHAPE, "%s: J=%lld must be positive", who, (long long)L->J);
+    const int64_t R = 3LL * L->U * L->Vn;
+    if (L->ldV < R) return fail(ctx, SCW_ERR_SHAPE, "%s: ldV=%lld < 3*U*Vn=%lld", who, (long long)L->ldV, (long long)R);
+    if (!finite_pos(L->X) || !finite_pos(L->Y) || !finite_pos(L->lambda))
+        return fail(ctx, SCW_ERR_VALUE, "%s: X, Y and lambda must be finite and > 0", who);
+    if (!std::isfinite(L->z_lo) || !std::isfinite(L->z_hi) || L->z_hi < L->z_lo)
+        return fail(ctx, SCW_ERR_VALUE, "%s: need finite z_lo <= z_hi", who);
+    if (!L->V || !L->gamma) return fail(ctx, SCW_ERR_NULL, "%s: V and gamma are required", who);
+    const size_t es = esize(L->dtype);
+    if (!aligned(L->V, es) || (L->c && !aligned(L->c, es)) || !aligned(L->gamma, 16))
+        return fail(ctx, SCW_ERR_ALIGN, "%s: V/c/gamma misaligned", who);
+    return SCW_OK;
+}
+
+int32_t need_ws(scw_ctx* ctx, size_t bytes, const char* who)
+{
+    if (bytes == 0) return SCW_OK;
+    if (!ctx->ws || ctx->ws_bytes < bytes) {
+        ctx->required_ws = bytes;
+        return fail(ctx, SCW_ERR_WORKSPACE, "%s: workspace of %zu bytes required, %zu registered", who, bytes,
+                    ctx->ws_bytes);
+    }
+    return SCW_OK;
+}
+
+// ---- assembly -----------------------------------------------------------------------------
+size_t assemble_ws(const scw_ctx* ctx, const scw_layer* L, int64_t Fz)
+{
+    const int64_t R = 3LL * L->U * L->Vn;
+    return align_up((size_t)L->J * Fz * esize(L->dtype)) + simt_assemble_scratch(L->dtype, R, L->J, Fz, ctx->sm_count);
+}
+
+void run_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z, void* P, int64_t ldP, Carver& cv)
+{
+    const int64_t R = 3LL * L->U * L->Vn;
+    void* W = cv.take((size_t)L->J * Fz * esize(L->dtype));
+    void* scratch = cv.take(simt_assemble_scratch(L->dtype, R, L->J, Fz, ctx->sm_count));
+    launch_mode_weights(ctx, L->dtype, L->J, Fz, L->lambda, L->z_lo, L->z_hi, L->c, L->gamma, L->dir, z, W);
+    launch_simt_assemble(ctx, L->dtype, R, L->J, Fz, L->V, L->ldV, W, P, ldP, scratch);
+}
+
+// ---- synthesis ----------------------------------------------------------------------------
+size_t twiddle_ws(int dtype, int U, int Vn, int64_t Nx, int64_t Ny)
+{
+    return align_up((size_t)U * Nx * esize(dtype)) + align_up((size_t)Vn * Ny * esize(dtype));
+}
+
+size_t synth_ws(int dtype, int U, int64_t Fz, int64_t Ny) { return simt_synth_scratch(dtype, U, Fz, Ny); }
+
+int32_t check_grid(scw_ctx* ctx, int32_t dtype, int32_t U, int32_t Vn, double X, double Y, int64_t Nx,
+                   const double* x, int64_t Ny, const double* y, const char* who)
+{
+    if (dtype != SCW_C64 && dtype != SCW_C128) return fail(ctx, SCW_ERR_DTYPE, "%s: bad dtype %d", who, dtype);
+    if (U <= 0 || Vn <= 0 || U > MAX_FREQ || Vn > MAX_FREQ) return fail(ctx, SCW_ERR_SHAPE, "%s: U=%d Vn=%d out of range", who, U, Vn);
+    if (Nx <= 0 || Ny <= 0 || Nx > MAX_GRID || Ny > MAX_GRID)
+        return fail(ctx, SCW_ERR_SHAPE, "%s: Nx=%lld Ny=%lld out of range", who, (long long)Nx, (long long)Ny);
+    if (!finite_pos(X) || !finite_pos(Y)) return fail(ctx, SCW_ERR_VALUE, "%s: X and Y must be finite and > 0", who);
+    if (!x || !y) return fail(ctx, SCW_ERR_NULL, "%s: x and y are required", who);
+    if (!aligned(x, 8) || !aligned(y, 8)) return fail(ctx, SCW_ERR_ALIGN, "%s: x/y misaligned", who);
+    return SCW_OK;
+}
+
+void planar_strides(int64_t Nx, int64_t Ny, int64_t s[4])
+{
+    s[3] = 1;
+    s[2] = Nx;
+    s[0] = Nx * Ny;
+    s[1] = 3 * Nx * Ny;
+}
+
+}  // namespace
+
+extern "C" {
+
+int32_t scw_version(void) { return 100; }
+
+int32_t scw_create(scw_ctx** out, int32_t device, void* cuda_stream)
+{
+    if (!out) return SCW_ERR_NULL;
+    *out = nullptr;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return SCW_ERR_CUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return SCW_ERR_CUDA;
+    if (prop.major != 10) return SCW_ERR_UNSUPPORTED;
+    scw_ctx* ctx = new (std::nothrow) scw_ctx();
+    if (!ctx) return SCW_ERR_CUDA;
+    ctx->device = device;
+    ctx->sm_count = prop.multiProcessorCount;
+    ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+    *out = ctx;
+    return SCW_OK;
+}
+
+int32_t scw_destroy(scw_ctx* ctx)
+{
+    if (!ctx) return SCW_ERR_NULL;
+    delete ctx;
+    return SCW_OK;
+}
+
+int32_t scw_set_stream(scw_ctx* ctx, void* cuda_stream)
+{
+    if (!ctx) return SCW_ERR_NULL;
+    ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+    return SCW_OK;
+}
+
+int32_t scw_set_workspace(scw_ctx* ctx, void* dev_ptr, size_t bytes)
+{
+    if (!ctx) return SCW_ERR_NULL;
+    if ((dev_ptr == nullptr) != (bytes == 0)) return fail(ctx, SCW_ERR_NULL, "workspace pointer/size mismatch");
+    if (!aligned(dev_ptr, 256)) return fail(ctx, SCW_ERR_ALIGN, "workspace must be 256-byte aligned");
+    ctx->ws = dev_ptr;
+    ctx->ws_bytes = bytes;
+    return SCW_OK;
+}
+
+int32_t scw_set_option(scw_ctx* ctx, int32_t option, int64_t value)
+{
+    if (!ctx) return SCW_ERR_NULL;
+    if (option == SCW_OPT_PATH && value >= SCW_PATH_AUTO && value <= SCW_PATH_TENSOR) {
+        ctx->path = value;
+        return SCW_OK;
+    }
+    return fail(ctx, SCW_ERR_UNSUPPORTED, "unknown option %d / value %lld", option, (long long)value);
+}
+
+const char* scw_last_error(const scw_ctx* ctx) { return ctx ? ctx->msg : "ctx is NULL"; }
+int32_t scw_last_cuda_error(const scw_ctx* ctx) { return ctx ? ctx->cuda_err : 0; }
+size_t scw_required_workspace(const scw_ctx* ctx) { return ctx ? ctx->required_ws : 0; }
+int64_t scw_launch_count(const scw_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+// ------------------------------------------------------------------------------------------
+int32_t scw_assemble_workspace(scw_ctx* ctx, const scw_layer* layer, int64_t Fz, size_t* bytes)
+{
+    if (!ctx || !bytes) return SCW_ERR_NULL;
+    ctx->msg[0] = 0;
+    if (int32_t s = check_layer(ctx, layer, "scw_assemble_workspace")) return s;
+    if (Fz < 0) return fail(ctx, SCW_ERR_SHAPE, "Fz=%lld < 0", (long long)Fz);
+    *bytes = Fz ? assemble_ws(ctx, layer, Fz) : 0;
+    return SCW_OK;
+}
+
+int32_t scw_assemble_spectra(scw_ctx* ctx, const scw_layer* layer, int64_t Fz, const double* z, void* P, int64_t ldP)
+{
+    if (int32_t s = check_ctx(ctx)) return s;
+    if (int32_t s = check_layer(ctx, layer, "scw_assemble_spectra")) return s;
+    if (Fz < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_assemble_spectra: Fz=%lld < 0", (long long)Fz);
+    if (Fz == 0) return SCW_OK;
+    if (!z || !P) return fail(ctx, SCW_ERR_NULL, "scw_assemble_spectra: z and P are required");
+    const int64_t R = 3LL * layer->U * layer->Vn;
+    if (ldP < R) return fail(ctx, SCW_ERR_SHAPE, "scw_assemble_spectra: ldP=%lld < 3*U*Vn=%lld", (long long)ldP, (long long)R);
+    if (!aligned(z, 8) || !aligned(P, esize(layer->dtype))) return fail(ctx, SCW_ERR_ALIGN, "scw_assemble_spectra: z/P misaligned");
+    if (int32_t s = need_ws(ctx, assemble_ws(ctx, layer, Fz), "scw_assemble_spectra")) return s;
+    Carver cv(ctx->ws);
+    run_assemble(ctx, layer, Fz, z, P, ldP, cv);
+    return check_launch(ctx, "scw_assemble_spectra");
+}
+
+// ------------------------------------------------------------------------------------------
+int32_t scw_synthesize_workspace(scw_ctx* ctx, int32_t dtype, int32_t U, int32_t Vn, int64_t Fz, int64_t Nx,
+                                 int64_t Ny, size_t* bytes)
+{
+    if (!ctx || !bytes) return SCW_ERR_NULL;
+    ctx->msg[0] = 0;
+    if (dtype != SCW_C64 && dtype != SCW_C128) return fail(ctx, SCW_ERR_DTYPE, "bad dtype %d", dtype);
+    if (U <= 0 || Vn <= 0 || Fz < 0 || Nx <= 0 || Ny <= 0) return fail(ctx, SCW_ERR_SHAPE, "bad dimensions");
+    *bytes = Fz ? twiddle_ws(dtype, U, Vn, Nx, Ny) + synth_ws(dtype, U, Fz, Ny) : 0;
+    return SCW_OK;
+}
+
+int32_t scw_synthesize_grid(scw_ctx* ctx, int32_t dtype, int32_t U, int32_t Vn, double X, double Y, int64_t Fz,
+                            const void* P, int64_t ldP, int64_t Nx, const double* x, int64_t Ny, const double* y,
+                            void* E, const int64_t* strides)
+{
+    if (int32_t s = check_ctx(ctx)) return s;
+    if (int32_t s = check_grid(ctx, dtype, U, Vn, X, Y, Nx, x, Ny, y, "scw_synthesize_grid")) return s;
+    if (Fz < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_synthesize_grid: Fz=%lld < 0", (long long)Fz);
+    if (Fz == 0) return SCW_OK;
+    if (!P || !E) return fail(ctx, SCW_ERR_NULL, "scw_synthesize_grid: P and E are required");
+    if (ldP < 3LL * U * Vn) return fail(ctx, SCW_ERR_SHAPE, "scw_synthesize_grid: ldP=%lld < 3*U*Vn", (long long)ldP);
+    if (!aligned(P, esize(dtype)) || !aligned(E, esize(dtype))) return fail(ctx, SCW_ERR_ALIGN, "scw_synthesize_grid: P/E misaligned");
+    int64_t s4[4];
+    if (strides) memcpy(s4, strides, sizeof(s4)); else planar_strides(Nx, Ny, s4);
+    for (int i = 0; i < 4; ++i)
+        if (s4[i] < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_synthesize_grid: negative stride");
+    if (int32_t s = need_ws(ctx, twiddle_ws(dtype, U, Vn, Nx, Ny) + synth_ws(dtype, U, Fz, Ny), "scw_synthesize_grid")) return s;
+    Carver cv(ctx->ws);
+    void* FxT = cv.take((size_t)U * Nx * esize(dtype));
+    void* FyT = cv.take((size_t)Vn * Ny * esize(dtype));
+    void* scratch = cv.take(synth_ws(dtype, U, Fz, Ny));
+    launch_twiddles(ctx, dtype, U, Nx, x, X, FxT);
+    launch_twiddles(ctx, dtype, Vn, Ny, y, Y, FyT);
+    launch_simt_synth(ctx, dtype, U, Vn, Fz, P, ldP, Nx, FxT, Ny, FyT, E, s4, scratch);
+    return check_launch(ctx, "scw_synthesize_grid");
+}
+
+// ------------------------------------------------------------------------------------------
+static int32_t check_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, int64_t Nx,
+                           int64_t Ny, const char* who, int64_t* fz_max, size_t* asm_max)
+{
+    if (n_inst < 0) return fail(ctx, SCW_ERR_SHAPE, "%s: n_inst=%lld < 0", who, (long long)n_inst);
+    if (n_inst == 0) return SCW_OK;
+    if (!inst || !Fz) return fail(ctx, SCW_ERR_NULL, "%s: inst and Fz are required", who);
+    if (Nx <= 0 || Ny <= 0 || Nx > MAX_GRID || Ny > MAX_GRID) return fail(ctx, SCW_ERR_SHAPE, "%s: bad Nx/Ny", who);
+    *fz_max = 0;
+    *asm_max = 0;
+    for (int64_t i = 0; i < n_inst; ++i) {
+        if (int32_t s = check_layer(ctx, &inst[i], who)) return s;
+        if (inst[i].dtype != inst[0].dtype || inst[i].U != inst[0].U || inst[i].Vn != inst[0].Vn ||
+            inst[i].X != inst[0].X || inst[i].Y != inst[0].Y)
+            return fail(ctx, SCW_ERR_SHAPE, "%s: instance %lld differs in dtype/U/Vn/X/Y", who, (long long)i);
+        if (Fz[i] < 0) return fail(ctx, SCW_ERR_SHAPE, "%s: Fz[%lld] < 0", who, (long long)i);
+        if (Fz[i] > *fz_max) *fz_max = Fz[i];
+        if (Fz[i] > 0) {
+            const size_t a = assemble_ws(ctx, &inst[i], Fz[i]);
+            if (a > *asm_max) *asm_max = a;
+        }
+    }
+    return SCW_OK;
+}
+
+static size_t sweep_ws(const scw_layer* L0, int64_t fz_max, size_t asm_max, int64_t Nx, int64_t Ny)
+{
+    if (fz_max == 0) return 0;
+    const int64_t R = 3LL * L0->U * L0->Vn;
+    return twiddle_ws(L0->dtype, L0->U, L0->Vn, Nx, Ny) + align_up((size_t)R * fz_max * esize(L0->dtype)) + asm_max +
+           synth_ws(L0->dtype, L0->U, fz_max, Ny);
+}
+
+int32_t scw_sweep_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, int64_t Nx,
+                            int64_t Ny, size_t* bytes)
+{
+    if (!ctx || !bytes) return SCW_ERR_NULL;
+    ctx->msg[0] = 0;
+    int64_t fz_max = 0;
+    size_t asm_max = 0;
+    if (int32_t s = check_sweep(ctx, n_inst, inst, Fz, Nx, Ny, "scw_sweep_workspace", &fz_max, &asm_max)) return s;
+    *bytes = n_inst ? sweep_ws(&inst[0], fz_max, asm_max, Nx, Ny) : 0;
+    return SCW_OK;
+}
+
+// Shared by the device- and host-buffer variants: everything after validation.
+static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, const double* const* z,
+                      int64_t Nx, const double* x, int64_t Ny, const double* y, void* const* E, const int64_t s4[4],
+                      int64_t fz_max, size_t asm_max, Carver& cv)
+{
+    const scw_layer& L0 = inst[0];
+    const int64_t R = 3LL * L0.U * L0.Vn;
+    void* FxT = cv.take((size_t)L0.U * Nx * esize(L0.dtype));
+    void* FyT = cv.take((size_t)L0.Vn * Ny * esize(L0.dtype));
+    void* P = cv.take((size_t)R * fz_max * esize(L0.dtype));
+    const size_t asm_off = cv.off;
+    cv.take(asm_max);
+    void* scratch = cv.take(synth_ws(L0.dtype, L0.U, fz_max, Ny));
+    launch_twiddles(ctx, L0.dtype, L0.U, Nx, x, L0.X, FxT);
+    launch_twiddles(ctx, L0.dtype, L0.Vn, Ny, y, L0.Y, FyT);
+    for (int64_t i = 0; i < n_inst; ++i) {
+        if (Fz[i] == 0) continue;
+        Carver sub(cv.base ? cv.base + asm_off : nullptr);
+        run_assemble(ctx, &inst[i], Fz[i], z[i], P, R, sub);
+        launch_simt_synth(ctx, L0.dtype, L0.U, L0.Vn, Fz[i], P, R, Nx, FxT, Ny, FyT, E[i], s4, scratch);
+    }
+}
+
+int32_t scw_sweep_wavelengths(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz,
+                              const double* const* z, int64_t Nx, const double* x, int64_t Ny, const double* y,
+                              void* const* E, const int64_t* strides)
+{
+    if (int32_t s = check_ctx(ctx)) return s;
+    int64_t fz_max = 0;
+    size_t asm_max = 0;
+    if (int32_t s = check_sweep(ctx, n_inst, inst, Fz, Nx, Ny, "scw_sweep_wavelengths", &fz_max, &asm_max)) return s;
+    if (n_inst == 0 || fz_max == 0) return SCW_OK;
+    if (int32_t s = check_grid(ctx, inst[0].dtype, inst[0].U, inst[0].Vn, inst[0].X, inst[0].Y, Nx, x, Ny, y,
+                               "scw_sweep_wavelengths")) return s;
+    if (!z || !E) return fail(ctx, SCW_ERR_NULL, "scw_sweep_wavelengths: z and E are required");
+    for (int64_t i = 0; i < n_inst; ++i) {
+        if (Fz[i] == 0) continue;
+        if (!z[i] || !E[i]) return fail(ctx, SCW_ERR_NULL, "scw_sweep_wavelengths: z[%lld]/E[%lld] is NULL", (long long)i, (long long)i);
+        if (!aligned(z[i], 8) || !aligned(E[i], esize(inst[0].dtype)))
+            return fail(ctx, SCW_ERR_ALIGN, "scw_sweep_wavelengths: z[%lld]/E[%lld] misaligned", (long long)i, (long long)i);
+    }
+    int64_t s4[4];
+    if (strides) memcpy(s4, strides, sizeof(s4)); else planar_strides(Nx, Ny, s4);
+    for (int i = 0; i < 4; ++i)
+        if (s4[i] < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_sweep_wavelengths: negative stride");
+    if (int32_t s = need_ws(ctx, sweep_ws(&inst[0], fz_max, asm_max, Nx, Ny), "scw_sweep_wavelengths")) return s;
+    Carver cv(ctx->ws);
+    run_sweep(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, E, s4, fz_max, asm_max, cv);
+    return check_launch(ctx, "scw_sweep_wavelengths");
+}
+
+// ------------------------------------------------------------------------------------------
+// Host-buffer variant: one staging area for the inputs and one for the output of an instance,
+// reused in stream order.
+static size_t host_stage_bytes(const scw_layer* L, int64_t Fz, int64_t Nx, int64_t Ny, size_t* e_bytes)
+{
+    const size_t es = esize(L->dtype);
+    *e_bytes = align_up((size_t)Fz * 3 * Nx * Ny * es);
+    return align_up((size_t)L->ldV * L->J * es) + align_up((size_t)L->J * es) + align_up((size_t)L->J * 16) +
+           align_up((size_t)L->J) + align_up((size_t)Fz * 8);
+}
+
+static int32_t sweep_host_sizes(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, int64_t Nx,
+                                int64_t Ny, const char* who, int64_t* fz_max, size_t* asm_max, size_t* in_max,
+                                size_t* e_max)
+{
+    if (int32_t s = check_sweep(ctx, n_inst, inst, Fz, Nx, Ny, who, fz_max, asm_max)) return s;
+    *in_max = *e_max = 0;
+    for (int64_t i = 0; i < n_inst; ++i) {
+        size_t eb = 0;
+        const size_t ib = host_stage_bytes(&inst[i], Fz[i], Nx, Ny, &eb);
+        if (ib > *in_max) *in_max = ib;
+        if (eb > *e_max) *e_max = eb;
+    }
+    return SCW_OK;
+}
+
+int32_t scw_sweep_host_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, int64_t Nx,
+                                 int64_t Ny, size_t* bytes)
+{
+    if (!ctx || !bytes) return SCW_ERR_NULL;
+    ctx->msg[0] = 0;
+    int64_t fz_max = 0;
+    size_t asm_max = 0, in_max = 0, e_max = 0;
+    if (int32_t s = sweep_host_sizes(ctx, n_inst, inst, Fz, Nx, Ny, "scw_sweep_host_workspace", &fz_max, &asm_max,
+                                     &in_max, &e_max)) return s;
+    *bytes = n_inst ? align_up((size_t)Nx * 8) + align_up((size_t)Ny * 8) + in_max + e_max +
+                          sweep_ws(&inst[0], fz_max, asm_max, Nx, Ny)
+                    : 0;
+    return SCW_OK;
+}
+
+int32_t scw_sweep_wavelengths_host(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz,
+                                   const double* const* z, int64_t Nx, const double* x, int64_t Ny, const double* y,
+                                   void* const* E, int64_t* h2d_bytes, int64_t* d2h_bytes)
+{
+    if (int32_t s = check_ctx(ctx)) return s;
+    int64_t fz_max = 0;
+    size_t asm_max = 0, in_max = 0, e_max = 0;
+    if (int32_t s = sweep_host_sizes(ctx, n_inst, inst, Fz, Nx, Ny, "scw_sweep_wavelengths_host", &fz_max, &asm_max,
+                                     &in_max, &e_max)) return s;
+    if (h2d_bytes) *h2d_bytes = 0;
+    if (d2h_bytes) *d2h_bytes = 0;
+    if (n_inst == 0 || fz_max == 0) return SCW_OK;
+    if (int32_t s = check_grid(ctx, inst[0].dtype, inst[0].U, inst[0].Vn, inst[0].X, inst[0].Y, Nx, x, Ny, y,
+                               "scw_sweep_wavelengths_host")) return s;
+    if (!z || !E) return fail(ctx, SCW_ERR_NULL, "scw_sweep_wavelengths_host: z and E are required");
+    for (int64_t i = 0; i < n_inst; ++i)
+        if (Fz[i] > 0 && (!z[i] || !E[i])) return fail(ctx, SCW_ERR_NULL, "scw_sweep_wavelengths_host: z[i]/E[i] is NULL");
+    const size_t total = align_up((size_t)Nx * 8) + align_up((size_t)Ny * 8) + in_max + e_max +
+                         sweep_ws(&inst[0], fz_max, asm_max, Nx, Ny);
+    if (int32_t s = need_ws(ctx, total, "scw_sweep_wavelengths_host")) return s;
+
+    Carver cv(ctx->ws);
+    double* dx = (double*)cv.take((size_t)Nx * 8);
+    double* dy = (double*)cv.take((size_t)Ny * 8);
+    char* stage_in = (char*)cv.take(in_max);
+    char* stage_e = (char*)cv.take(e_max);
+    const scw_layer& L0 = inst[0];
+    const size_t es = esize(L0.dtype);
+    const int64_t R = 3LL * L0.U * L0.Vn;
+    int64_t up = 0, down = 0;
+    cudaError_t err = cudaSuccess;
+    auto h2d = [&](void* d, const void* h, size_t n) {
+        if (err == cudaSuccess) err = cudaMemcpyAsync(d, h, n, cudaMemcpyHostToDevice, ctx->stream);
+        up += (int64_t)n;
+    };
+    h2d(dx, x, (size_t)Nx * 8);
+    h2d(dy, y, (size_t)Ny * 8);
+    void* FxT = cv.take((size_t)L0.U * Nx * es);
+    void* FyT = cv.take((size_t)L0.Vn * Ny * es);
+    void* P = cv.take((size_t)R * fz_max * es);
+    const size_t asm_off = cv.off;
+    cv.take(asm_max);
+    void* scratch = cv.take(synth_ws(L0.dtype, L0.U, fz_max, Ny));
+    launch_twiddles(ctx, L0.dtype, L0.U, Nx, dx, L0.X, FxT);
+    launch_twiddles(ctx, L0.dtype, L0.Vn, Ny, dy, L0.Y, FyT);
+    int64_t s4[4];
+    planar_strides(Nx, Ny, s4);
+    for (int64_t i = 0; i < n_inst && err == cudaSuccess; ++i) {
+        if (Fz[i] == 0) continue;
+        scw_layer L = inst[i];
+        Carver st(stage_in);
+        void* dV = st.take((size_t)L.ldV * L.J * es);
+        void* dc = st.take((size_t)L.J * es);
+        void* dg = st.take((size_t)L.J * 16);
+        void* dd = st.take((size_t)L.J);
+        void* dz = st.take((size_t)Fz[i] * 8);
+        h2d(dV, L.V, (size_t)L.ldV * L.J * es);
+        if (L.c) h2d(dc, L.c, (size_t)L.J * es);
+        h2d(dg, L.gamma, (size_t)L.J * 16);
+        if (L.dir) h2d(dd, L.dir, (size_t)L.J);
+        h2d(dz, z[i], (size_t)Fz[i] * 8);
+        L.V = dV;
+        L.c = L.c ? dc : nullptr;
+        L.gamma = (const double*)dg;
+        L.dir = L.dir ? (const int8_t*)dd : nullptr;
+        Carver sub((char*)ctx->ws + asm_off);
+        run_assemble(ctx, &L, Fz[i], (const double*)dz, P, R, sub);
+        launch_simt_synth(ctx, L0.dtype, L0.U, L0.Vn, Fz[i], P, R, Nx, FxT, Ny, FyT, stage_e, s4, scratch);
+        const size_t eb = (size_t)Fz[i] * 3 * Nx * Ny * es;
+        if (err == cudaSuccess) err = cudaMemcpyAsync(E[i], stage_e, eb, cudaMemcpyDeviceToHost, ctx->stream);
+        down += (int64_t)eb;
+    }
+    if (err != cudaSuccess) {
+        ctx->cuda_err = (int32_t)err;
+        return fail(ctx, SCW_ERR_CUDA, "scw_sweep_wavelengths_host: %s", cudaGetErrorString(err));
+    }
+    if (h2d_bytes) *h2d_bytes = up;
+    if (d2h_bytes) *d2h_bytes = down;
+    return check_launch(ctx, "scw_sweep_wavelengths_host");
+}
+
+// ------------------------------------------------------------------------------------------
+static int32_t check_modes(scw_ctx* ctx, const scw_modes* m, const char* who)
+{
+    if (!m) return fail(ctx, SCW_ERR_NULL, "%s: modes is NULL", who);
+    if (m->struct_size != sizeof(scw_modes)) return fail(ctx, SCW_ERR_SHAPE, "%s: modes.struct_size mismatch", who);
+    if (m->kind == SCW_MODES_DENSE) return check_layer(ctx, &m->layer, who);
+    if (m->kind != SCW_MODES_PLANEWAVE) return fail(ctx, SCW_ERR_SHAPE, "%s: unknown modes.kind %d", who, m->kind);
+    if (m->dtype != SCW_C64 && m->dtype != SCW_C128) return fail(ctx, SCW_ERR_DTYPE, "%s: bad dtype %d", who, m->dtype);
+    if (m->J <= 0) return fail(ctx, SCW_ERR_SHAPE, "%s: J must be positive", who);
+    if (!finite_pos(m->lambda)) return fail(ctx, SCW_ERR_VALUE, "%s: lambda must be finite and > 0", who);
+    if (!m->sx || !m->sy || !m->gamma || !m->zref || !m->p) return fail(ctx, SCW_ERR_NULL, "%s: sx, sy, gamma, zref, p are required", who);
+    if (!aligned(m->sx, 8) || !aligned(m->sy, 8) || !aligned(m->gamma, 16) || !aligned(m->zref, 8) ||
+        !aligned(m->p, esize(m->dtype)))
+        return fail(ctx, SCW_ERR_ALIGN, "%s: mode arrays misaligned", who);
+    return SCW_OK;
+}
+
+constexpr int64_t DENSE_CHUNK_MAX = 4096;   // points per pass of the dense point path
+constexpr int64_t DENSE_CHUNK_MIN = 64;
+
+static size_t dense_chunk_ws(const scw_ctx* ctx, const scw_layer* L, int64_t N, int64_t chunk)
+{
+    // the full chunks and the ragged last chunk split the mode index differently: take the larger need
+    const int64_t R = 3LL * L->U * L->Vn;
+    if (chunk > N) chunk = N;
+    const int64_t tail = N % chunk;
+    size_t a = assemble_ws(ctx, L, chunk);
+    if (tail) { const size_t b = assemble_ws(ctx, L, tail); if (b > a) a = b; }
+    return align_up((size_t)chunk * 8) + align_up((size_t)R * chunk * esize(L->dtype)) + a;
+}
+
+int32_t scw_points_workspace(scw_ctx* ctx, const scw_modes* modes, int64_t N, size_t* bytes)
+{
+    if (!ctx || !bytes) return SCW_ERR_NULL;
+    ctx->msg[0] = 0;
+    if (int32_t s = check_modes(ctx, modes, "scw_points_workspace")) return s;
+    if (N < 0) return fail(ctx, SCW_ERR_SHAPE, "N < 0");
+    if (N == 0) { *bytes = 0; return SCW_OK; }
+    if (modes->kind == SCW_MODES_PLANEWAVE) *bytes = points_table_bytes(modes->dtype, modes->J);
+    else *bytes = dense_chunk_ws(ctx, &modes->layer, N, DENSE_CHUNK_MAX);
+    return SCW_OK;
+}
+
+int32_t scw_eval_points(scw_ctx* ctx, const scw_modes* modes, int64_t N, const double* r, void* E)
+{
+    if (int32_t s = check_ctx(ctx)) return s;
+    if (int32_t s = check_modes(ctx, modes, "scw_eval_points")) return s;
+    if (N < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_eval_points: N=%lld < 0", (long long)N);
+    if (N == 0) return SCW_OK;
+    if (!r || !E) return fail(ctx, SCW_ERR_NULL, "scw_eval_points: r and E are required");
+    const int dtype = modes->kind == SCW_MODES_PLANEWAVE ? modes->dtype : modes->layer.dtype;
+    if (!aligned(r, 8) || !aligned(E, esize(dtype))) return fail(ctx, SCW_ERR_ALIGN, "scw_eval_points: r/E misaligned");
+
+    if (modes->kind == SCW_MODES_PLANEWAVE) {
+        if (int32_t s = need_ws(ctx, points_table_bytes(dtype, modes->J), "scw_eval_points")) return s;
+        launch_points_planewave(ctx, modes, N, r, E, ctx->ws);
+        return check_launch(ctx, "scw_eval_points");
+    }
+    // dense: chunks of points sized to the registered workspace
+    const scw_layer* L = &modes->layer;
+    int64_t chunk = N < DENSE_CHUNK_MAX ? N : DENSE_CHUNK_MAX;
+    while (chunk > DENSE_CHUNK_MIN && dense_chunk_ws(ctx, L, N, chunk) > ctx->ws_bytes) chunk = (chunk + 1) / 2;
+    if (chunk > N) chunk = N;
+    if (int32_t s = need_ws(ctx, dense_chunk_ws(ctx, L, N, chunk), "scw_eval_points")) return s;
+    const int64_t R = 3LL * L->U * L->Vn;
+    const size_t es = esize(dtype);
+    for (int64_t p0 = 0; p0 < N; p0 += chunk) {
+        const int64_t n = (N - p0) < chunk ? (N - p0) : chunk;
+        Carver cv(ctx->ws);
+        double* zc = (double*)cv.take((size_t)chunk * 8);
+        void* P = cv.take((size_t)R * chunk * es);
+        launch_extract_z(ctx, n, r + 3 * p0, zc);
+        run_assemble(ctx, L, n, zc, P, R, cv);
+        launch_point_synth(ctx, dtype, L->U, L->Vn, L->X, L->Y, n, r + 3 * p0, P, R, (char*)E + (size_t)p0 * 3 * es);
+    }
+    return check_launch(ctx, "scw_eval_points");
+}
+
+}  // extern "C"

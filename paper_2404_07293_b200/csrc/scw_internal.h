@@ -1,0 +1,66 @@
+// Internal declarations shared by the translation units of libscw (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "scwatter.h"
+
+struct scw_ctx {
+    int device = 0;
+    int sm_count = 148;
+    cudaStream_t stream = nullptr;
+    void* ws = nullptr;
+    size_t ws_bytes = 0;
+    int64_t path = SCW_PATH_AUTO;
+    int64_t launches = 0;
+    int32_t cuda_err = 0;
+    size_t required_ws = 0;
+    char msg[256] = {0};
+};
+
+namespace scw {
+
+inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+// Bump allocator over the caller's workspace.
+struct Carver {
+    char* base;
+    size_t off = 0;
+    explicit Carver(void* p) : base(static_cast<char*>(p)) {}
+    void* take(size_t bytes) {
+        void* p = base ? base + off : nullptr;
+        off += align_up(bytes);
+        return p;
+    }
+};
+
+// ---- kernels_simt.cu ----------------------------------------------------------------------
+// W[j*Fz + i] = c_j * exp(i 2 pi gamma_j (z_i - zref_j) / lambda)  (eq. 7, 30)
+void launch_mode_weights(scw_ctx* ctx, int dtype, int64_t J, int64_t Fz, double lambda, double z_lo,
+                         double z_hi, const void* c, const double* gamma, const int8_t* dir,
+                         const double* z, void* W);
+// Ft[f*N + i] = exp(i 2 pi (f - nfreq/2) coord_i / period)  (eq. 6, 10) -- frequency-major table
+void launch_twiddles(scw_ctx* ctx, int dtype, int nfreq, int64_t N, const double* coord, double period,
+                     void* Ft);
+// P[r + i*ldP] = sum_j V[r + j*ldV] W[j*Fz + i]   (eq. 31)
+size_t simt_assemble_scratch(int dtype, int64_t R, int64_t J, int64_t Fz, int sm_count);
+void launch_simt_assemble(scw_ctx* ctx, int dtype, int64_t R, int64_t J, int64_t Fz, const void* V,
+                          int64_t ldV, const void* W, void* P, int64_t ldP, void* scratch);
+// Two-pass separable synthesis (eq. 10): T = P_comp Fy^T, E = Fx T.
+size_t simt_synth_scratch(int dtype, int U, int64_t Fz, int64_t Ny);
+void launch_simt_synth(scw_ctx* ctx, int dtype, int U, int Vn, int64_t Fz, const void* P, int64_t ldP,
+                       int64_t Nx, const void* FxT, int64_t Ny, const void* FyT, void* E,
+                       const int64_t strides[4], void* scratch);
+
+// ---- points.cu ------------------------------------------------------------------------------
+struct PwTableInfo { size_t bytes; };
+size_t points_table_bytes(int dtype, int64_t J);
+void launch_points_planewave(scw_ctx* ctx, const scw_modes* m, int64_t N, const double* r, void* E,
+                             void* table);
+// dense form, per-point synthesis: E[p,comp] = sum_m P[comp*M+m, p] exp(i 2 pi (u x_p/X + v y_p/Y))
+void launch_point_synth(scw_ctx* ctx, int dtype, int U, int Vn, double X, double Y, int64_t n,
+                        const double* r, const void* P, int64_t ldP, void* E);
+// z[p] = r[3p+2]
+void launch_extract_z(scw_ctx* ctx, int64_t n, const double* r, double* z);
+
+}  // namespace scw

@@ -1,0 +1,191 @@
+"""GPU edge cases and error paths of the C ABI: ragged shapes, padding, strides, empties, bad arguments."""
+import ctypes
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import scw_inputs as si
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def scw():
+    import paper_2404_07293_b200 as m
+    m.lib()
+    return m
+
+
+@pytest.fixture(scope="module")
+def ctx(scw):
+    c = scw.Context(0)
+    yield c
+    c.close()
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def rel_err(got, ref):
+    return float(np.abs(np.asarray(got, dtype=np.complex128) - ref).max() / np.abs(ref).max())
+
+
+def ragged_layer(U, Vn, J, dtype, seed, ldV_pad=0, with_c=True, with_dir=True):
+    g = np.random.default_rng(seed)
+    R = 3 * U * Vn
+    V = np.full((J, R + ldV_pad), 9.0 + 9.0j, dtype=dtype)        # padding rows hold garbage on purpose
+    V[:, :R] = ((g.standard_normal((J, R)) + 1j * g.standard_normal((J, R))) / np.sqrt(2 * U * Vn)).astype(dtype)
+    dirs = np.where(g.uniform(0, 1, J) < 0.5, 1, -1).astype(np.int8)
+    gamma = dirs * (g.uniform(0.0, 1.5, J) + 1j * g.uniform(0.0, 0.8, J))
+    c = ((g.standard_normal(J) + 1j * g.standard_normal(J)) / np.sqrt(2)).astype(dtype) if with_c else None
+    return dict(U=U, Vn=Vn, X=3.0, Y=4.5, lam=0.7, z_lo=-0.4, z_hi=0.9, V=V, gamma=gamma, c=c,
+                dir=dirs if with_dir else None)
+
+
+@pytest.mark.parametrize("dtype,tol", [(np.complex64, 2e-4), (np.complex128, 1e-10)])
+@pytest.mark.parametrize("U,Vn,J,Nx,Ny,Fz", [(5, 3, 17, 37, 21, 3), (1, 1, 4, 5, 130, 1), (4, 6, 96, 129, 7, 35),
+                                             (7, 2, 56, 300, 3, 18)])
+def test_ragged_shapes_padding_and_defaults(scw, ctx, dtype, tol, U, Vn, J, Nx, Ny, Fz):
+    """Odd/even frequency counts, J not 4M, padded ldV/ldP, c = NULL, dir = NULL, non-uniform x/y,
+    z outside the layer: every sample against Tier A."""
+    lay = ragged_layer(U, Vn, J, dtype, seed=U * 100 + J, ldV_pad=3, with_c=(J % 2 == 0), with_dir=(J % 3 == 0))
+    g = np.random.default_rng(5)
+    x = np.sort(g.uniform(-4, 7, Nx))
+    y = np.sort(g.uniform(-4, 7, Ny))
+    z = np.linspace(-0.6, 1.1, Fz)                                  # includes z outside [z_lo, z_hi]
+    ref = oracle.layer_grid(x=x, y=y, z=z, **lay)
+    L = scw.Layer.from_numpy(lay, "cuda")
+    R = 3 * U * Vn
+    Pbuf = torch.full((Fz, R + 5), 7.0, dtype=L.V.dtype, device="cuda")
+    scw.scw_assemble_spectra(ctx, L, dev(z), out=Pbuf)
+    assert torch.all(Pbuf[:, R:] == 7.0)                            # padding of P untouched
+    E = scw.scw_synthesize_grid(ctx, U=U, Vn=Vn, X=lay["X"], Y=lay["Y"], P=Pbuf, x=dev(x), y=dev(y))
+    torch.cuda.synchronize()
+    assert rel_err(E.cpu().numpy(), ref) <= tol
+    E2 = scw.scw_sweep_wavelengths(ctx, [L], [dev(z)], dev(x), dev(y))[0]
+    torch.cuda.synchronize()
+    assert rel_err(E2.cpu().numpy(), ref) <= tol
+    # dense point path on a ragged number of points
+    xyz = oracle.grid_points(x, y, z)[:: max(1, (Nx * Ny * Fz) // 301)]
+    Ep = scw.scw_eval_points(ctx, L, dev(xyz))
+    torch.cuda.synchronize()
+    refp = oracle.layer_samples(xyz=xyz, **lay)
+    assert np.abs(Ep.cpu().numpy() - refp).max() / np.abs(ref).max() <= tol
+
+
+def test_custom_strides_interleaved_output(scw, ctx):
+    """strides = (comp, z, y, x): write E as [Fz][Ny][Nx][3] (component fastest)."""
+    lay = ragged_layer(5, 3, 20, np.complex64, seed=3)
+    x = np.arange(24) * 3.0 / 24
+    y = np.arange(10) * 4.5 / 10
+    z = np.linspace(-0.4, 0.9, 4)
+    L = scw.Layer.from_numpy(lay, "cuda")
+    P = scw.scw_assemble_spectra(ctx, L, dev(z))
+    out = torch.zeros((4, 10, 24, 3), dtype=torch.complex64, device="cuda")
+    scw.scw_synthesize_grid(ctx, U=5, Vn=3, X=3.0, Y=4.5, P=P, x=dev(x), y=dev(y), out=out,
+                            strides=(1, 10 * 24 * 3, 24 * 3, 3))
+    planar = scw.scw_synthesize_grid(ctx, U=5, Vn=3, X=3.0, Y=4.5, P=P, x=dev(x), y=dev(y))
+    torch.cuda.synchronize()
+    assert torch.equal(out.permute(0, 3, 1, 2), planar)
+    assert rel_err(planar.cpu().numpy(), oracle.layer_grid(x=x, y=y, z=z, **lay)) <= 2e-4
+
+
+def test_empty_inputs_are_noops(scw, ctx):
+    lay = ragged_layer(3, 3, 36, np.complex64, seed=1)
+    L = scw.Layer.from_numpy(lay, "cuda")
+    empty = torch.empty(0, dtype=torch.float64, device="cuda")
+    n0 = ctx.launch_count()
+    P = scw.scw_assemble_spectra(ctx, L, empty)
+    assert P.shape == (0, 27)
+    E = scw.scw_synthesize_grid(ctx, U=3, Vn=3, X=3.0, Y=4.5, P=P, x=dev(np.arange(4.0)), y=dev(np.arange(5.0)))
+    assert E.shape == (0, 3, 5, 4)
+    pts = scw.scw_eval_points(ctx, L, torch.empty((0, 3), dtype=torch.float64, device="cuda"))
+    assert pts.shape == (0, 3)
+    assert scw.scw_sweep_wavelengths(ctx, [], [], dev(np.arange(4.0)), dev(np.arange(5.0))) == []
+    assert ctx.launch_count() == n0                                  # nothing was launched
+
+
+def test_error_codes_and_nothing_written(scw, ctx):
+    from paper_2404_07293_b200 import binding as b
+    lay = ragged_layer(3, 3, 36, np.complex64, seed=2)
+    L = scw.Layer.from_numpy(lay, "cuda")
+    z = dev(np.linspace(-0.4, 0.9, 4))
+    P = torch.full((4, 27), 5.0, dtype=torch.complex64, device="cuda")
+    lib = ctx.L
+    need = ctypes.c_size_t()
+
+    def call(st, Fz=4, zp=z, Pp=P, ldP=27):
+        return lib.scw_assemble_spectra(ctx._h, ctypes.byref(st), Fz, b._p(zp), b._p(Pp), ldP)
+
+    ctx.reserve(1 << 20)
+    st = L.struct(); st.lambda_ = 0.0
+    assert call(st) == 5 and "lambda" in ctx.last_error()            # SCW_ERR_VALUE
+    st = L.struct(); st.z_hi = st.z_lo - 1.0
+    assert call(st) == 5
+    st = L.struct(); st.X = float("nan")
+    assert call(st) == 5
+    st = L.struct(); st.dtype = 7
+    assert call(st) == 3                                             # SCW_ERR_DTYPE
+    st = L.struct(); st.ldV = 26
+    assert call(st) == 2                                             # SCW_ERR_SHAPE
+    st = L.struct(); st.J = 0
+    assert call(st) == 2
+    st = L.struct(); st.struct_size = 8
+    assert call(st) == 2
+    st = L.struct(); st.V = None
+    assert call(st) == 1                                             # SCW_ERR_NULL
+    st = L.struct(); st.V = L.V.data_ptr() + 4
+    assert call(st) == 4                                             # SCW_ERR_ALIGN
+    st = L.struct()
+    assert call(st, ldP=26) == 2
+    assert call(st, Fz=-1) == 2
+    assert call(st, zp=None) == 1
+    assert lib.scw_assemble_spectra(None, ctypes.byref(st), 4, b._p(z), b._p(P), 27) == 1
+    # workspace too small: error, required size reported, nothing written
+    lib.scw_assemble_workspace(ctx._h, ctypes.byref(st), 4, ctypes.byref(need))
+    assert need.value > 0
+    small = torch.empty(256, dtype=torch.uint8, device="cuda")
+    assert lib.scw_set_workspace(ctx._h, b._p(small), 256) == 0
+    assert call(st) == 6 and lib.scw_required_workspace(ctx._h) == need.value
+    torch.cuda.synchronize()
+    assert torch.all(P == 5.0)                                       # nothing was written by any failing call
+    ctx._ws = None
+    ctx.reserve(need.value)
+    assert call(st) == 0
+    torch.cuda.synchronize()
+    assert not torch.all(P == 5.0)
+    # misaligned workspace / unknown option
+    assert lib.scw_set_workspace(ctx._h, ctypes.c_void_p(ctx._ws.data_ptr() + 8), 1024) == 4
+    assert lib.scw_set_option(ctx._h, 99, 0) == 8
+    # sweep with mismatching instances
+    lay2 = ragged_layer(5, 3, 20, np.complex64, seed=3)
+    with pytest.raises(scw.ScwError) as e:
+        scw.scw_sweep_wavelengths(ctx, [L, scw.Layer.from_numpy(lay2, "cuda")], [z, z], dev(np.arange(4.0)),
+                                  dev(np.arange(4.0)))
+    assert e.value.status == 2
+    # points: bad kind / N < 0
+    m = b.scw_modes(); m.struct_size = ctypes.sizeof(b.scw_modes); m.kind = 5
+    assert lib.scw_eval_points(ctx._h, ctypes.byref(m), 1, b._p(z), b._p(P)) == 2
+    pw = scw.PlaneWaves.from_numpy(si.make_planewaves(si.CONFIGS[3]), "cuda").struct()
+    assert lib.scw_eval_points(ctx._h, ctypes.byref(pw), -3, b._p(z), b._p(P)) == 2
+    pw.lambda_ = -1.0
+    assert lib.scw_eval_points(ctx._h, ctypes.byref(pw), 1, b._p(z), b._p(P)) == 5
+
+
+def test_stream_and_launch_counter(scw):
+    """Work is enqueued on the stream given at creation; the launch counter advances."""
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        c = scw.Context(0, stream=s)
+        lay = ragged_layer(3, 3, 36, np.complex128, seed=4)
+        z = dev(np.linspace(-0.4, 0.9, 2))
+        x, y = np.arange(6) * 0.5, np.arange(4) * 1.125
+        n0 = c.launch_count()
+        E = scw.scw_sweep_wavelengths(c, [scw.Layer.from_numpy(lay, "cuda")], [z], dev(x), dev(y))[0]
+        assert c.launch_count() > n0
+        s.synchronize()
+    assert rel_err(E.cpu().numpy(), oracle.layer_grid(x=x, y=y, z=np.linspace(-0.4, 0.9, 2), **lay)) <= 1e-10
+    c.close()
