@@ -59,7 +59,7 @@ enum {
 enum { SCW_C64 = 0, SCW_C128 = 1 };
 
 /* Which kernels implement the two contractions (scw_set_option(ctx, SCW_OPT_PATH, v)). */
-enum { SCW_OPT_PATH = 1 };
+enum { SCW_OPT_PATH = 1, SCW_OPT_PROFILE = 2 /* 0/1: record CUDA events around every kernel launch */ };
 enum {
     SCW_PATH_AUTO = 0,    /* tcgen05 tensor-core kernels where shape/dtype allow, CUDA-core otherwise */
     SCW_PATH_SIMT = 1,    /* CUDA-core kernels only (fp32 FMA for C64, fp64 DFMA for C128) */
@@ -84,6 +84,15 @@ size_t scw_required_workspace(const scw_ctx* ctx);
 int64_t scw_launch_count(const scw_ctx* ctx);
 /* Library version: major*10000 + minor*100 + patch. */
 int32_t scw_version(void);
+
+/* Per-kernel device timers (only while SCW_OPT_PROFILE is 1): every launch is bracketed by CUDA events
+ * on the ctx stream.  scw_profile_read synchronises on the recorded events and returns, for one kernel
+ * class in [0, scw_profile_classes()), the accumulated device milliseconds and launch count since the
+ * last scw_profile_reset (HOST out-pointers).  scw_profile_name returns a static string, NULL if out of range. */
+int32_t scw_profile_classes(void);
+const char* scw_profile_name(int32_t kernel_class);
+int32_t scw_profile_read(scw_ctx* ctx, int32_t kernel_class, double* ms_total, int64_t* launches);
+int32_t scw_profile_reset(scw_ctx* ctx);
 
 /* ---------------------------------------------------------------- descriptors (HOST PODs) */
 

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(HERE, "libscw.so")
 
 SCW_C64, SCW_C128 = 0, 1
 SCW_MODES_PLANEWAVE, SCW_MODES_DENSE = 0, 1
-SCW_OPT_PATH = 1
+SCW_OPT_PATH, SCW_OPT_PROFILE = 1, 2
 SCW_PATH_AUTO, SCW_PATH_SIMT, SCW_PATH_TENSOR = 0, 1, 2
 STATUS = {0: "SCW_OK", 1: "SCW_ERR_NULL", 2: "SCW_ERR_SHAPE", 3: "SCW_ERR_DTYPE", 4: "SCW_ERR_ALIGN",
           5: "SCW_ERR_VALUE", 6: "SCW_ERR_WORKSPACE", 7: "SCW_ERR_CUDA", 8: "SCW_ERR_UNSUPPORTED"}
@@ -27,6 +27,7 @@ EXPORTS = [
     "scw_assemble_spectra", "scw_assemble_workspace", "scw_synthesize_grid", "scw_synthesize_workspace",
     "scw_eval_points", "scw_points_workspace", "scw_sweep_wavelengths", "scw_sweep_workspace",
     "scw_sweep_wavelengths_host", "scw_sweep_host_workspace",
+    "scw_profile_classes", "scw_profile_name", "scw_profile_read", "scw_profile_reset",
 ]
 
 
@@ -72,6 +73,10 @@ def lib():
         L.scw_last_cuda_error.argtypes = [c_void_p]
         L.scw_required_workspace.argtypes = [c_void_p]
         L.scw_launch_count.argtypes = [c_void_p]
+        L.scw_profile_name.restype = c_char_p
+        L.scw_profile_name.argtypes = [c_int32]
+        L.scw_profile_read.argtypes = [c_void_p, c_int32, POINTER(c_double), POINTER(c_int64)]
+        L.scw_profile_reset.argtypes = [c_void_p]
         L.scw_assemble_spectra.argtypes = [c_void_p, POINTER(scw_layer), c_int64, c_void_p, c_void_p, c_int64]
         L.scw_assemble_workspace.argtypes = [c_void_p, POINTER(scw_layer), c_int64, POINTER(c_size_t)]
         L.scw_synthesize_grid.argtypes = [c_void_p, c_int32, c_int32, c_int32, c_double, c_double, c_int64,
@@ -208,6 +213,20 @@ class Context:
 
     def set_path(self, path):
         self.check(self.L.scw_set_option(self._h, SCW_OPT_PATH, path))
+
+    def set_profile(self, on):
+        self.check(self.L.scw_set_option(self._h, SCW_OPT_PROFILE, 1 if on else 0))
+        self.check(self.L.scw_profile_reset(self._h))
+
+    def profile(self):
+        """{kernel name: (device ms, launches)} accumulated since set_profile(True) / the last reset."""
+        out = {}
+        for kc in range(self.L.scw_profile_classes()):
+            ms, n = c_double(), c_int64()
+            self.check(self.L.scw_profile_read(self._h, kc, byref(ms), byref(n)))
+            if n.value:
+                out[self.L.scw_profile_name(kc).decode()] = (ms.value, n.value)
+        return out
 
     def reserve(self, nbytes):
         """Grow the registered workspace to at least nbytes."""

@@ -162,6 +162,7 @@ int32_t scw_create(scw_ctx** out, int32_t device, void* cuda_stream)
 int32_t scw_destroy(scw_ctx* ctx)
 {
     if (!ctx) return SCW_ERR_NULL;
+    for (ProfRec& r : ctx->recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     delete ctx;
     return SCW_OK;
 }
@@ -190,7 +191,53 @@ int32_t scw_set_option(scw_ctx* ctx, int32_t option, int64_t value)
         ctx->path = value;
         return SCW_OK;
     }
+    if (option == SCW_OPT_PROFILE && (value == 0 || value == 1)) {
+        ctx->profile = value != 0;
+        return SCW_OK;
+    }
     return fail(ctx, SCW_ERR_UNSUPPORTED, "unknown option %d / value %lld", option, (long long)value);
+}
+
+int32_t scw_profile_classes(void) { return KC_COUNT; }
+
+const char* scw_profile_name(int32_t kc)
+{
+    static const char* names[KC_COUNT] = {"mode_weights", "twiddles", "simt_assemble", "reduce_splits", "simt_synth_a",
+                                          "simt_synth_b", "points_table", "points_planewave", "point_synth", "misc",
+                                          "tc_assemble", "tc_synth"};
+    return (kc >= 0 && kc < KC_COUNT) ? names[kc] : nullptr;
+}
+
+static void profile_drain(scw_ctx* ctx)
+{
+    for (ProfRec& r : ctx->recs) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(r.b) == cudaSuccess && cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess) {
+            ctx->prof_ms[r.kc] += (double)ms;
+            ctx->prof_n[r.kc] += 1;
+        }
+        cudaEventDestroy(r.a);
+        cudaEventDestroy(r.b);
+    }
+    ctx->recs.clear();
+}
+
+int32_t scw_profile_read(scw_ctx* ctx, int32_t kc, double* ms_total, int64_t* launches)
+{
+    if (!ctx) return SCW_ERR_NULL;
+    if (kc < 0 || kc >= KC_COUNT) return fail(ctx, SCW_ERR_SHAPE, "kernel class %d out of range", kc);
+    profile_drain(ctx);
+    if (ms_total) *ms_total = ctx->prof_ms[kc];
+    if (launches) *launches = ctx->prof_n[kc];
+    return SCW_OK;
+}
+
+int32_t scw_profile_reset(scw_ctx* ctx)
+{
+    if (!ctx) return SCW_ERR_NULL;
+    profile_drain(ctx);
+    for (int i = 0; i < KC_COUNT; ++i) { ctx->prof_ms[i] = 0; ctx->prof_n[i] = 0; }
+    return SCW_OK;
 }
 
 const char* scw_last_error(const scw_ctx* ctx) { return ctx ? ctx->msg : "ctx is NULL"; }

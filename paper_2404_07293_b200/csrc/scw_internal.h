@@ -3,7 +3,17 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stddef.h>
+#include <vector>
 #include "scwatter.h"
+
+namespace scw {
+// Kernel classes for launch accounting and the optional per-kernel CUDA-event timers.
+enum KernelClass {
+    KC_WEIGHTS = 0, KC_TWIDDLES, KC_ASSEMBLE, KC_REDUCE, KC_SYNTH_A, KC_SYNTH_B, KC_POINTS_TABLE, KC_POINTS,
+    KC_POINT_SYNTH, KC_MISC, KC_ASSEMBLE_TC, KC_SYNTH_TC, KC_COUNT
+};
+struct ProfRec { cudaEvent_t a, b; int kc; };
+}  // namespace scw
 
 struct scw_ctx {
     int device = 0;
@@ -16,11 +26,40 @@ struct scw_ctx {
     int32_t cuda_err = 0;
     size_t required_ws = 0;
     char msg[256] = {0};
+    bool profile = false;
+    std::vector<scw::ProfRec> recs;
+    double prof_ms[scw::KC_COUNT] = {0};
+    int64_t prof_n[scw::KC_COUNT] = {0};
 };
 
 namespace scw {
 
 inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+// Brackets one kernel launch: counts it and, when profiling is on, records CUDA events around it
+// on the ctx stream (read back by scw_profile_read).
+struct KernelScope {
+    scw_ctx* ctx;
+    ProfRec rec;
+    bool on;
+    KernelScope(scw_ctx* c, int kc) : ctx(c), on(c->profile)
+    {
+        ctx->launches++;
+        rec.kc = kc;
+        if (on) {
+            cudaEventCreate(&rec.a);
+            cudaEventCreate(&rec.b);
+            cudaEventRecord(rec.a, ctx->stream);
+        }
+    }
+    ~KernelScope()
+    {
+        if (on) {
+            cudaEventRecord(rec.b, ctx->stream);
+            ctx->recs.push_back(rec);
+        }
+    }
+};
 
 // Bump allocator over the caller's workspace.
 struct Carver {

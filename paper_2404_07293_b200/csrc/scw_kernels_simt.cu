@@ -61,13 +61,13 @@ void launch_mode_weights(scw_ctx* ctx, int dtype, int64_t J, int64_t Fz, double 
     const int64_t n = J * Fz;
     const int threads = 256;
     const unsigned blocks = (unsigned)((n + threads - 1) / threads);
+    KernelScope ks(ctx, KC_WEIGHTS);
     if (dtype == SCW_C64)
         k_mode_weights<float><<<blocks, threads, 0, ctx->stream>>>(
             J, Fz, 1.0 / lambda, z_lo, z_hi, (const float2*)c, (const double2*)gamma, dir, z, (float2*)W);
     else
         k_mode_weights<double><<<blocks, threads, 0, ctx->stream>>>(
             J, Fz, 1.0 / lambda, z_lo, z_hi, (const double2*)c, (const double2*)gamma, dir, z, (double2*)W);
-    ctx->launches++;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -93,11 +93,11 @@ void launch_twiddles(scw_ctx* ctx, int dtype, int nfreq, int64_t N, const double
     const int64_t n = (int64_t)nfreq * N;
     const int threads = 256;
     const unsigned blocks = (unsigned)((n + threads - 1) / threads);
+    KernelScope ks(ctx, KC_TWIDDLES);
     if (dtype == SCW_C64)
         k_twiddles<float><<<blocks, threads, 0, ctx->stream>>>(nfreq, N, coord, 1.0 / period, (float2*)Ft);
     else
         k_twiddles<double><<<blocks, threads, 0, ctx->stream>>>(nfreq, N, coord, 1.0 / period, (double2*)Ft);
-    ctx->launches++;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -201,16 +201,19 @@ static void run_simt_assemble(scw_ctx* ctx, int64_t R, int64_t J, int64_t Fz, co
     ns = (int)((J + kchunk - 1) / kchunk);
     dim3 grid((unsigned)((R + ASM_THREADS - 1) / ASM_THREADS), (unsigned)((Fz + TN - 1) / TN), (unsigned)ns);
     if (ns == 1) {
+        KernelScope ks(ctx, KC_ASSEMBLE);
         k_simt_assemble<T, TN><<<grid, ASM_THREADS, 0, ctx->stream>>>(R, J, Fz, (const T2*)V, ldV, (const T2*)W,
                                                                       (T2*)P, ldP, 0, kchunk);
-        ctx->launches++;
     } else {
-        k_simt_assemble<T, TN><<<grid, ASM_THREADS, 0, ctx->stream>>>(R, J, Fz, (const T2*)V, ldV, (const T2*)W,
-                                                                      (T2*)scratch, R, R * Fz, kchunk);
+        {
+            KernelScope ks(ctx, KC_ASSEMBLE);
+            k_simt_assemble<T, TN><<<grid, ASM_THREADS, 0, ctx->stream>>>(R, J, Fz, (const T2*)V, ldV, (const T2*)W,
+                                                                          (T2*)scratch, R, R * Fz, kchunk);
+        }
         const int64_t n = R * Fz;
+        KernelScope ks(ctx, KC_REDUCE);
         k_reduce_splits<T><<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(R, Fz, ns, (const T2*)scratch,
                                                                                  (T2*)P, ldP);
-        ctx->launches += 2;
     }
 }
 
@@ -322,12 +325,15 @@ static void run_simt_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* 
     const int64_t planes = Fz * 3;
     // gridDim.x carries the plane index (up to 2^31-1)
     dim3 ga((unsigned)planes, (unsigned)((Ny + SYN_THREADS - 1) / SYN_THREADS), (unsigned)((U + TU - 1) / TU));
-    k_simt_synth_a<T, TU><<<ga, SYN_THREADS, (size_t)Vn * TU * sizeof(T2), ctx->stream>>>(
-        U, Vn, (const T2*)P, ldP, Ny, (const T2*)FyT, (T2*)scratch);
+    {
+        KernelScope ks(ctx, KC_SYNTH_A);
+        k_simt_synth_a<T, TU><<<ga, SYN_THREADS, (size_t)Vn * TU * sizeof(T2), ctx->stream>>>(
+            U, Vn, (const T2*)P, ldP, Ny, (const T2*)FyT, (T2*)scratch);
+    }
     dim3 gb((unsigned)planes, (unsigned)((Nx + SYN_THREADS - 1) / SYN_THREADS), (unsigned)((Ny + TK - 1) / TK));
+    KernelScope ks(ctx, KC_SYNTH_B);
     k_simt_synth_b<T, TK><<<gb, SYN_THREADS, (size_t)U * TK * sizeof(T2), ctx->stream>>>(
         U, Nx, Ny, (const T2*)FxT, (const T2*)scratch, (T2*)E, s[0], s[1], s[2], s[3]);
-    ctx->launches += 2;
 }
 
 void launch_simt_synth(scw_ctx* ctx, int dtype, int U, int Vn, int64_t Fz, const void* P, int64_t ldP,

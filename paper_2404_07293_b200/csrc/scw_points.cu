@@ -176,18 +176,21 @@ void launch_points_planewave(scw_ctx* ctx, const scw_modes* m, int64_t N, const 
                              void* table)
 {
     if (m->dtype == SCW_C64) {
-        k_points_table<float2><<<(unsigned)((m->J + 127) / 128), 128, 0, ctx->stream>>>(
+        {
+            KernelScope ks(ctx, KC_POINTS_TABLE);
+            k_points_table<float2><<<(unsigned)((m->J + 127) / 128), 128, 0, ctx->stream>>>(
             m->J, 1.0 / m->lambda, m->sx, m->sy, (const double2*)m->gamma, m->zref, (const float2*)m->p,
-            (PwMode*)table);
+                (PwMode*)table);
+        }
         const int64_t per_block = PW_THREADS * PW_PPT;
+        KernelScope ks(ctx, KC_POINTS);
         k_points_pw_c64<<<(unsigned)((N + per_block - 1) / per_block), PW_THREADS, 0, ctx->stream>>>(
             m->J, N, r, (const PwMode*)table, m->zref, (float2*)E);
-        ctx->launches += 2;
     } else {
+        KernelScope ks(ctx, KC_POINTS);
         k_points_pw_c128<<<(unsigned)((N + 127) / 128), 128, 0, ctx->stream>>>(
             m->J, N, 1.0 / m->lambda, r, m->sx, m->sy, (const double2*)m->gamma, m->zref,
             (const double2*)m->p, (double2*)E);
-        ctx->launches += 1;
     }
 }
 
@@ -240,13 +243,13 @@ void launch_point_synth(scw_ctx* ctx, int dtype, int U, int Vn, double X, double
                         const double* r, const void* P, int64_t ldP, void* E)
 {
     const unsigned blocks = (unsigned)((n + 3) / 4);
+    KernelScope ks(ctx, KC_POINT_SYNTH);
     if (dtype == SCW_C64)
         k_point_synth<float, float2><<<blocks, 128, 4 * (U + Vn) * sizeof(float2), ctx->stream>>>(
             U, Vn, 1.0 / X, 1.0 / Y, n, r, (const float2*)P, ldP, (float2*)E);
     else
         k_point_synth<double, double2><<<blocks, 128, 4 * (U + Vn) * sizeof(double2), ctx->stream>>>(
             U, Vn, 1.0 / X, 1.0 / Y, n, r, (const double2*)P, ldP, (double2*)E);
-    ctx->launches++;
 }
 
 __global__ void k_extract_z(int64_t n, const double* __restrict__ r, double* __restrict__ z)
@@ -257,8 +260,8 @@ __global__ void k_extract_z(int64_t n, const double* __restrict__ r, double* __r
 
 void launch_extract_z(scw_ctx* ctx, int64_t n, const double* r, double* z)
 {
+    KernelScope ks(ctx, KC_MISC);
     k_extract_z<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(n, r, z);
-    ctx->launches++;
 }
 
 }  // namespace scw
