@@ -63,6 +63,8 @@ int32_t check_layer(scw_ctx* ctx, const scw_layer* L, const char* who)
     if (L->struct_size != sizeof(scw_layer))
         return fail(ctx, SCW_ERR_SHAPE, "%s: layer.struct_size %u != %zu", who, L->struct_size, sizeof(scw_layer));
     if (L->dtype != SCW_C64 && L->dtype != SCW_C128) return fail(ctx, SCW_ERR_DTYPE, "%s: bad dtype %d", who, L->dtype);
+    if (ctx && ctx->path == SCW_PATH_TENSOR && L->dtype != SCW_C64)
+        return fail(ctx, SCW_ERR_UNSUPPORTED, "%s: SCW_PATH_TENSOR has no complex128 kernels", who);
     if (L->U <= 0 || L->Vn <= 0 || L->U > MAX_FREQ || L->Vn > MAX_FREQ)
         return fail(ctx, SCW_ERR_SHAPE, "%s: U=%d Vn=%d out of range", who, L->U, L->Vn);
     if (L->J <= 0) return fail(ctx, SCW_ERR_SHAPE, "%s: J=%lld must be positive", who, (long long)L->J);
@@ -91,15 +93,31 @@ int32_t need_ws(scw_ctx* ctx, size_t bytes, const char* who)
 }
 
 // ---- assembly -----------------------------------------------------------------------------
+// Tensor-core assembly is used for complex64 unless the ctx is pinned to the CUDA-core path; tiny
+// problems (less than one 128 x 64 tile) stay on CUDA cores in AUTO mode.
+bool use_tc_assemble(const scw_ctx* ctx, const scw_layer* L, int64_t Fz)
+{
+    const int64_t R = 3LL * L->U * L->Vn;
+    if (ctx->path == SCW_PATH_SIMT || !tc_assemble_supported(L->dtype, R, L->J, Fz)) return false;
+    if (ctx->path == SCW_PATH_TENSOR) return true;
+    return 2 * R >= 128 && L->J >= 64;
+}
+
 size_t assemble_ws(const scw_ctx* ctx, const scw_layer* L, int64_t Fz)
 {
     const int64_t R = 3LL * L->U * L->Vn;
+    if (use_tc_assemble(ctx, L, Fz)) return tc_assemble_scratch(R, L->J, Fz, ctx->sm_count);
     return align_up((size_t)L->J * Fz * esize(L->dtype)) + simt_assemble_scratch(L->dtype, R, L->J, Fz, ctx->sm_count);
 }
 
 void run_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z, void* P, int64_t ldP, Carver& cv)
 {
     const int64_t R = 3LL * L->U * L->Vn;
+    if (use_tc_assemble(ctx, L, Fz)) {
+        void* scratch = cv.take(tc_assemble_scratch(R, L->J, Fz, ctx->sm_count));
+        launch_tc_assemble(ctx, L, Fz, z, P, ldP, scratch);
+        return;
+    }
     void* W = cv.take((size_t)L->J * Fz * esize(L->dtype));
     void* scratch = cv.take(simt_assemble_scratch(L->dtype, R, L->J, Fz, ctx->sm_count));
     launch_mode_weights(ctx, L->dtype, L->J, Fz, L->lambda, L->z_lo, L->z_hi, L->c, L->gamma, L->dir, z, W);

@@ -91,6 +91,13 @@ void launch_simt_synth(scw_ctx* ctx, int dtype, int U, int Vn, int64_t Fz, const
                        int64_t Nx, const void* FxT, int64_t Ny, const void* FyT, void* E,
                        const int64_t strides[4], void* scratch);
 
+// ---- scw_tc_assemble.cu: tcgen05 BF16x3 spectral assembly (complex64) ----------------------------
+bool tc_assemble_supported(int dtype, int64_t R, int64_t J, int64_t Fz);
+size_t tc_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int sm_count);
+// weights (a-1) + P = V W (a-2) + segment reduce; scratch from tc_assemble_scratch
+void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z, void* P, int64_t ldP,
+                        void* scratch);
+
 // ---- points.cu ------------------------------------------------------------------------------
 struct PwTableInfo { size_t bytes; };
 size_t points_table_bytes(int dtype, int64_t J);

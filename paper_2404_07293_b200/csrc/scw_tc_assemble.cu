@@ -1,0 +1,397 @@
+// Spectral assembly P = V . W on the 5th-gen tensor cores (tcgen05, accumulators in TMEM), complex64.
+//
+//   P[:, i] = V . (c o g(z_i))     (eq. 31 with the diag(alpha) factoring)
+//
+// Precision: fp32 operands are split in software into bf16 hi + lo (round to nearest) and three
+// products hi*hi + hi*lo + lo*hi are accumulated in fp32 ("BF16x3", error ~1e-5 relative), because a
+// single TF32/BF16 pass misses the 2e-4 bar.
+// Complex on a real MMA: V (column-major interleaved complex) is viewed as a real matrix with 2R rows
+// (rows 2r / 2r+1 = Re / Im of complex row r); the small operand is laid out as [W_r | W_i] so that one
+// real GEMM yields all four real products, combined between adjacent TMEM lanes in the epilogue.
+//
+// Work decomposition ("stream-K"): the iteration space (n_tile, m_tile, k_block) is cut into equal
+// contiguous spans, one per persistent CTA (one CTA per SM); every (CTA, tile) segment writes an fp32
+// partial tile, k_tc_reduce sums the segments of each tile in a fixed order (deterministic).
+//
+// Warp roles (448 threads): warps 0-7 stream V from HBM (coalesced 8-byte loads kept in flight in
+// registers), split to bf16 hi/lo and store K-major UMMA tiles; warp 8 fetches the pre-formatted W tiles
+// with bulk async copies; warp 9 issues tcgen05.mma; warps 10-13 drain TMEM (tcgen05.ld), combine
+// lanes with one shuffle per element and store the partial tile.
+#include "scw_internal.h"
+#include "scw_tc_common.cuh"
+
+namespace scw {
+
+using namespace tc;
+
+constexpr int TA_BM = 128;                 // real rows per tile (= 64 complex rows)
+constexpr int TA_BK = 64;                  // modes per pipeline stage
+constexpr int TA_PROD_WARPS = 8;
+constexpr int TA_THREADS = (TA_PROD_WARPS + 2 + 4) * 32;
+constexpr int TA_A_SBO = 144;              // bytes between 8-row groups (144 instead of 128: conflict-free stores)
+constexpr int TA_A_LBO = 16 * TA_A_SBO;    // bytes between 8-mode chunks
+constexpr int TA_A_TILE = 8 * TA_A_LBO;    // one bf16 tile (hi or lo): 18432 bytes
+constexpr int TA_TMEM_COLS = 512;
+constexpr int TA_SMEM_LIMIT = 225 * 1024;
+
+struct TaParams {
+    const float2* V;
+    int64_t ldV, R2, J;
+    const uint8_t* Wt;      // [n_tile][k_block][hi | lo] K-major UMMA images of [W_r | W_i]
+    float* part;            // [slot][Fzt][128] fp32 partial tiles
+    int N2, Fzt, n_tiles, m_tiles, kblocks, S, stages;
+};
+
+// ---- W~ in UMMA image form -----------------------------------------------------------------------
+// a-1 mode weights (eq. 7, 30) evaluated in fp64, split to bf16 hi/lo, written as the K-major no-swizzle
+// shared-memory image of every (n_tile, k_block) B tile: element (n, kk) at
+//   (kk/8)*(N2*16) + (n/8)*128 + (n%8)*16 + (kk%8)*2,  n < Fzt: Re W[j, i], n >= Fzt: Im W[j, i].
+__global__ void k_tc_weights(int64_t J, int64_t Fz, int Fzt, int n_tiles, int kblocks, double inv_lambda, double z_lo,
+                             double z_hi, const float2* __restrict__ c, const double2* __restrict__ gamma,
+                             const int8_t* __restrict__ dir, const double* __restrict__ z, uint8_t* __restrict__ Wt)
+{
+    const int64_t Jp = (int64_t)kblocks * TA_BK;
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= Jp * n_tiles * Fzt) return;
+    const int64_t i = idx / Jp, j = idx - i * Jp;
+    float wr = 0.f, wi = 0.f;
+    if (j < J && i < Fz) {
+        const double2 g = gamma[j];
+        const int d = dir ? (dir[j] > 0 ? 1 : -1) : ((g.y > 0.0 || (g.y == 0.0 && g.x >= 0.0)) ? 1 : -1);
+        const double dz = z[i] - (d > 0 ? z_lo : z_hi);
+        double t = g.x * dz * inv_lambda;
+        t -= rint(t);
+        double s, co;
+        sincospi(2.0 * t, &s, &co);
+        const double a = exp(-6.283185307179586476925 * g.y * dz * inv_lambda);
+        double cr = 1.0, ci = 0.0;
+        if (c) { cr = (double)c[j].x; ci = (double)c[j].y; }
+        wr = (float)(cr * a * co - ci * a * s);
+        wi = (float)(cr * a * s + ci * a * co);
+    }
+    const int N2 = 2 * Fzt;
+    const int nt = (int)(i / Fzt), n = (int)(i - (int64_t)nt * Fzt);
+    const int kb = (int)(j / TA_BK), kk = (int)(j - (int64_t)kb * TA_BK);
+    uint8_t* tile = Wt + ((size_t)nt * kblocks + kb) * (size_t)N2 * 256;
+    const size_t off_r = (size_t)(kk >> 3) * (N2 * 16) + (size_t)(n >> 3) * 128 + (n & 7) * 16 + (kk & 7) * 2;
+    const int n2 = n + Fzt;
+    const size_t off_i = (size_t)(kk >> 3) * (N2 * 16) + (size_t)(n2 >> 3) * 128 + (n2 & 7) * 16 + (kk & 7) * 2;
+    const __nv_bfloat16 rh = __float2bfloat16_rn(wr), ih = __float2bfloat16_rn(wi);
+    const __nv_bfloat16 rl = __float2bfloat16_rn(wr - __bfloat162float(rh));
+    const __nv_bfloat16 il = __float2bfloat16_rn(wi - __bfloat162float(ih));
+    const size_t lo = (size_t)N2 * 128;
+    *reinterpret_cast<__nv_bfloat16*>(tile + off_r) = rh;
+    *reinterpret_cast<__nv_bfloat16*>(tile + off_i) = ih;
+    *reinterpret_cast<__nv_bfloat16*>(tile + lo + off_r) = rl;
+    *reinterpret_cast<__nv_bfloat16*>(tile + lo + off_i) = il;
+}
+
+// ---- main kernel -----------------------------------------------------------------------------------
+__device__ __forceinline__ void ta_load(const TaParams& p, int64_t it, int warp, int lane, float2 (&v)[2][8])
+{
+    const int64_t tile = it / p.kblocks;
+    const int kb = (int)(it - tile * p.kblocks);
+    const int mt = (int)(tile % p.m_tiles);
+    const int64_t k0 = (int64_t)kb * TA_BK + warp * 8;
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const int64_t row = (int64_t)mt * TA_BM + 2 * (lane + 32 * h);       // even real row = complex row * 2
+        const bool row_ok = row < p.R2;
+        const float2* src = p.V + (row >> 1) + k0 * p.ldV;
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk) {
+            float2 t = make_float2(0.f, 0.f);
+            if (row_ok && k0 + kk < p.J) t = __ldg(src + kk * p.ldV);
+            v[h][kk] = t;
+        }
+    }
+}
+
+__device__ __forceinline__ void ta_store(uint8_t* a_hi, int warp, int lane, const float2 (&v)[2][8])
+{
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const int r = 2 * (lane + 32 * h);                                   // even row in tile; r+1 is its Im row
+        uint8_t* dst = a_hi + warp * TA_A_LBO + (r >> 3) * TA_A_SBO + (r & 7) * 16;
+        uint4 eh, el, oh, ol;
+        split_bf16x2(v[h][0].x, v[h][1].x, eh.x, el.x);
+        split_bf16x2(v[h][2].x, v[h][3].x, eh.y, el.y);
+        split_bf16x2(v[h][4].x, v[h][5].x, eh.z, el.z);
+        split_bf16x2(v[h][6].x, v[h][7].x, eh.w, el.w);
+        split_bf16x2(v[h][0].y, v[h][1].y, oh.x, ol.x);
+        split_bf16x2(v[h][2].y, v[h][3].y, oh.y, ol.y);
+        split_bf16x2(v[h][4].y, v[h][5].y, oh.z, ol.z);
+        split_bf16x2(v[h][6].y, v[h][7].y, oh.w, ol.w);
+        *reinterpret_cast<uint4*>(dst) = eh;
+        *reinterpret_cast<uint4*>(dst + 16) = oh;
+        *reinterpret_cast<uint4*>(dst + TA_A_TILE) = el;
+        *reinterpret_cast<uint4*>(dst + TA_A_TILE + 16) = ol;
+    }
+}
+
+__global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const TaParams p)
+{
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int stage_bytes = 2 * TA_A_TILE + p.N2 * 256;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)p.stages * stage_bytes);
+    uint64_t* full_a = bars;
+    uint64_t* full_b = bars + p.stages;
+    uint64_t* empty = bars + 2 * p.stages;
+    uint64_t* acc_full = bars + 3 * p.stages;
+    uint64_t* acc_empty = acc_full + 2;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
+
+    if (tid == 0) {
+        for (int s = 0; s < p.stages; ++s) {
+            mbar_init(&full_a[s], TA_PROD_WARPS * 32);
+            mbar_init(&full_b[s], 1);
+            mbar_init(&empty[s], 1);
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(&acc_full[b], 1);
+            mbar_init(&acc_empty[b], 4);
+        }
+        mbar_fence_init();
+    }
+    if (warp == 9) tmem_alloc(tmem_slot, TA_TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    const int64_t T = (int64_t)p.n_tiles * p.m_tiles * p.kblocks;
+    const int64_t it0 = (int64_t)blockIdx.x * T / gridDim.x;
+    const int64_t it1 = (int64_t)(blockIdx.x + 1) * T / gridDim.x;
+
+    if (warp < TA_PROD_WARPS) {
+        // ===== V producers: HBM -> registers -> bf16 hi/lo -> shared memory =====
+        float2 cur[2][8], nxt[2][8];
+        int stage = 0;
+        uint32_t phase = 0;
+        if (it0 < it1) ta_load(p, it0, warp, lane, cur);
+        for (int64_t it = it0; it < it1; ++it) {
+            if (it + 1 < it1) ta_load(p, it + 1, warp, lane, nxt);
+            mbar_wait(&empty[stage], phase ^ 1);
+            ta_store(smem + (size_t)stage * stage_bytes, warp, lane, cur);
+            fence_proxy_async();
+            mbar_arrive(&full_a[stage]);
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int kk = 0; kk < 8; ++kk) cur[h][kk] = nxt[h][kk];
+            if (++stage == p.stages) { stage = 0; phase ^= 1; }
+        }
+    } else if (warp == 8) {
+        // ===== W tile loader (bulk async copy, completes on full_b) =====
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            const uint32_t bytes = (uint32_t)p.N2 * 256;
+            for (int64_t it = it0; it < it1; ++it) {
+                const int64_t tile = it / p.kblocks;
+                const int kb = (int)(it - tile * p.kblocks);
+                const int nt = (int)(tile / p.m_tiles);
+                mbar_wait(&empty[stage], phase ^ 1);
+                mbar_expect_tx(&full_b[stage], bytes);
+                bulk_g2s(smem + (size_t)stage * stage_bytes + 2 * TA_A_TILE,
+                         p.Wt + ((size_t)nt * p.kblocks + kb) * bytes, bytes, &full_b[stage]);
+                if (++stage == p.stages) { stage = 0; phase ^= 1; }
+            }
+        }
+    } else if (warp == 9) {
+        // ===== MMA issuer (one thread) =====
+        if (lane == 0) {
+            const uint32_t idesc = umma_idesc_bf16(TA_BM, p.N2);
+            const uint32_t b_lbo = (uint32_t)p.N2 * 16;
+            int stage = 0, buf = 0;
+            uint32_t phase = 0, use[2] = {0, 0};
+            int64_t it = it0;
+            while (it < it1) {
+                const int64_t tile = it / p.kblocks;
+                const int64_t seg_end = min(it1, (tile + 1) * p.kblocks);
+                mbar_wait(&acc_empty[buf], (use[buf] & 1) ^ 1);
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + (uint32_t)(buf * p.N2);
+                uint32_t acc = 0;
+                for (; it < seg_end; ++it) {
+                    mbar_wait(&full_a[stage], phase);
+                    mbar_wait(&full_b[stage], phase);
+                    tc_fence_after();
+                    const uint32_t a_hi = smem_u32(smem + (size_t)stage * stage_bytes);
+                    const uint32_t a_lo = a_hi + TA_A_TILE;
+                    const uint32_t b_hi = a_hi + 2 * TA_A_TILE;
+                    const uint32_t b_lo = b_hi + (uint32_t)p.N2 * 128;
+#pragma unroll
+                    for (int s = 0; s < TA_BK / 16; ++s) {
+                        const uint64_t da_hi = umma_desc(a_hi + s * 2 * TA_A_LBO, TA_A_LBO, TA_A_SBO);
+                        const uint64_t da_lo = umma_desc(a_lo + s * 2 * TA_A_LBO, TA_A_LBO, TA_A_SBO);
+                        const uint64_t db_hi = umma_desc(b_hi + s * 2 * b_lbo, b_lbo, 128);
+                        const uint64_t db_lo = umma_desc(b_lo + s * 2 * b_lbo, b_lbo, 128);
+                        umma_bf16(d_tmem, da_lo, db_hi, idesc, acc);
+                        acc = 1;
+                        umma_bf16(d_tmem, da_hi, db_lo, idesc, 1);
+                        umma_bf16(d_tmem, da_hi, db_hi, idesc, 1);
+                    }
+                    umma_commit(&empty[stage]);
+                    if (++stage == p.stages) { stage = 0; phase ^= 1; }
+                }
+                umma_commit(&acc_full[buf]);
+                use[buf]++;
+                buf ^= 1;
+            }
+        }
+    } else {
+        // ===== epilogue: TMEM -> registers -> lane-pair combine -> partial tile =====
+        const int q = warp & 3;                                   // TMEM lane quarter this warp may access
+        int buf = 0, seg = 0;
+        uint32_t use[2] = {0, 0};
+        int64_t it = it0;
+        while (it < it1) {
+            const int64_t tile = it / p.kblocks;
+            const int64_t seg_end = min(it1, (tile + 1) * p.kblocks);
+            mbar_wait(&acc_full[buf], use[buf] & 1);
+            tc_fence_after();
+            float* out = p.part + ((size_t)blockIdx.x * p.S + seg) * ((size_t)p.Fzt * TA_BM) + 32 * q + lane;
+            const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(buf * p.N2);
+            for (int i0 = 0; i0 < p.Fzt; i0 += 8) {
+                float a[8], b[8];
+                tmem_ld8(taddr + i0, a);
+                tmem_ld8(taddr + p.Fzt + i0, b);
+                tmem_ld_wait();
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const float recv = __shfl_xor_sync(0xffffffffu, b[e], 1);
+                    // even lane: Re = D[2r,i] - D[2r+1,Fzt+i];  odd lane: Im = D[2r+1,i] + D[2r,Fzt+i]
+                    out[(size_t)(i0 + e) * TA_BM] = (lane & 1) ? a[e] + recv : a[e] - recv;
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&acc_empty[buf]);
+            use[buf]++;
+            buf ^= 1;
+            ++seg;
+            it = seg_end;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 9) tmem_dealloc(tmem_base, TA_TMEM_COLS);
+}
+
+// Sum the segments of every tile in CTA order: P[mt*64 + r, nt*Fzt + n] = sum_seg part[seg][n][2r..2r+1].
+__global__ void k_tc_reduce(int64_t R, int64_t Fz, int Fzt, int m_tiles, int kblocks, int64_t T, int G, int S,
+                            const float* __restrict__ part, float2* __restrict__ P, int64_t ldP)
+{
+    const int tile = blockIdx.x;
+    const int n = blockIdx.y * blockDim.y + threadIdx.y;
+    const int r = threadIdx.x;                                   // complex row in tile, 0..63
+    const int nt = tile / m_tiles, mt = tile - nt * m_tiles;
+    const int64_t row = (int64_t)mt * 64 + r, col = (int64_t)nt * Fzt + n;
+    if (n >= Fzt || row >= R || col >= Fz) return;
+    const int64_t a = (int64_t)tile * kblocks, b = a + kblocks;
+    const int c_first = (int)(((a + 1) * G + T - 1) / T) - 1;
+    const int c_last = (int)((b * G + T - 1) / T) - 1;
+    float2 acc = make_float2(0.f, 0.f);
+    for (int c = c_first; c <= c_last; ++c) {
+        const int64_t start = (int64_t)c * T / G;
+        const int seg = tile - (int)(start / kblocks);
+        const float2 v = *reinterpret_cast<const float2*>(part + ((size_t)c * S + seg) * ((size_t)Fzt * TA_BM) +
+                                                          (size_t)n * TA_BM + 2 * r);
+        acc.x += v.x;
+        acc.y += v.y;
+    }
+    P[row + col * ldP] = acc;
+}
+
+// ---- host side -------------------------------------------------------------------------------------
+struct TaPlan {
+    int Fzt, N2, n_tiles, m_tiles, kblocks, G, S, stages;
+    int64_t T;
+    size_t wt_bytes, part_bytes, smem_bytes;
+};
+
+static TaPlan ta_plan(int64_t R, int64_t J, int64_t Fz, int sm_count)
+{
+    TaPlan pl;
+    int64_t fzt = (Fz + 7) / 8 * 8;
+    if (fzt > 128) fzt = 128;
+    pl.Fzt = (int)fzt;
+    pl.N2 = 2 * pl.Fzt;
+    pl.n_tiles = (int)((Fz + pl.Fzt - 1) / pl.Fzt);
+    pl.m_tiles = (int)((2 * R + TA_BM - 1) / TA_BM);
+    pl.kblocks = (int)((J + TA_BK - 1) / TA_BK);
+    pl.T = (int64_t)pl.n_tiles * pl.m_tiles * pl.kblocks;
+    pl.G = (int)(pl.T < sm_count ? pl.T : sm_count);
+    pl.S = 1;
+    for (int c = 0; c < pl.G; ++c) {
+        const int64_t s = (int64_t)c * pl.T / pl.G, e = (int64_t)(c + 1) * pl.T / pl.G;
+        if (e > s) {
+            const int span = (int)((e - 1) / pl.kblocks - s / pl.kblocks) + 1;
+            if (span > pl.S) pl.S = span;
+        }
+    }
+    const int stage_bytes = 2 * TA_A_TILE + pl.N2 * 256;
+    pl.stages = (TA_SMEM_LIMIT - 256) / stage_bytes;
+    if (pl.stages > 4) pl.stages = 4;
+    pl.smem_bytes = (size_t)pl.stages * stage_bytes + 256;
+    pl.wt_bytes = align_up((size_t)pl.n_tiles * pl.kblocks * pl.N2 * 256);
+    pl.part_bytes = align_up((size_t)pl.G * pl.S * pl.Fzt * TA_BM * sizeof(float));
+    return pl;
+}
+
+bool tc_assemble_supported(int dtype, int64_t R, int64_t J, int64_t Fz)
+{
+    return dtype == SCW_C64 && R >= 1 && J >= 1 && Fz >= 1;
+}
+
+size_t tc_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int sm_count)
+{
+    const TaPlan pl = ta_plan(R, J, Fz, sm_count);
+    return pl.wt_bytes + pl.part_bytes;
+}
+
+void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z, void* P, int64_t ldP,
+                        void* scratch)
+{
+    const int64_t R = 3LL * L->U * L->Vn;
+    const TaPlan pl = ta_plan(R, L->J, Fz, ctx->sm_count);
+    uint8_t* Wt = static_cast<uint8_t*>(scratch);
+    float* part = reinterpret_cast<float*>(Wt + pl.wt_bytes);
+    {
+        KernelScope ks(ctx, KC_WEIGHTS);
+        const int64_t n = (int64_t)pl.kblocks * TA_BK * pl.n_tiles * pl.Fzt;
+        k_tc_weights<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(
+            L->J, Fz, pl.Fzt, pl.n_tiles, pl.kblocks, 1.0 / L->lambda, L->z_lo, L->z_hi, (const float2*)L->c,
+            (const double2*)L->gamma, L->dir, z, Wt);
+    }
+    TaParams p;
+    p.V = (const float2*)L->V;
+    p.ldV = L->ldV;
+    p.R2 = 2 * R;
+    p.J = L->J;
+    p.Wt = Wt;
+    p.part = part;
+    p.N2 = pl.N2;
+    p.Fzt = pl.Fzt;
+    p.n_tiles = pl.n_tiles;
+    p.m_tiles = pl.m_tiles;
+    p.kblocks = pl.kblocks;
+    p.S = pl.S;
+    p.stages = pl.stages;
+    {
+        KernelScope ks(ctx, KC_ASSEMBLE_TC);
+        cudaFuncSetAttribute(k_tc_assemble, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes);
+        k_tc_assemble<<<pl.G, TA_THREADS, pl.smem_bytes, ctx->stream>>>(p);
+    }
+    {
+        KernelScope ks(ctx, KC_REDUCE);
+        dim3 block(64, 4);
+        dim3 grid((unsigned)(pl.n_tiles * pl.m_tiles), (unsigned)((pl.Fzt + 3) / 4));
+        k_tc_reduce<<<grid, block, 0, ctx->stream>>>(R, Fz, pl.Fzt, pl.m_tiles, pl.kblocks, pl.T, pl.G, pl.S, part,
+                                                     (float2*)P, ldP);
+    }
+}
+
+}  // namespace scw
