@@ -13,8 +13,9 @@
 // contiguous spans, one per persistent CTA (one CTA per SM); every (CTA, tile) segment writes an fp32
 // partial tile, k_tc_reduce sums the segments of each tile in a fixed order (deterministic).
 //
-// Warp roles (448 threads): warps 0-7 stream V from HBM (coalesced 8-byte loads kept in flight in
-// registers), split to bf16 hi/lo and store K-major UMMA tiles; warp 8 fetches the pre-formatted W tiles
+// Warp roles (448 threads): warps 0-7 stream V from HBM with bulk async copies (cp.async.bulk, one per
+// 512-byte column segment) into an fp32 staging ring that keeps 64-128 KB in flight per SM, split the
+// staged fp32 into bf16 hi/lo and store K-major UMMA tiles; warp 8 fetches the pre-formatted W tiles
 // with bulk async copies; warp 9 issues tcgen05.mma; warps 10-13 drain TMEM (tcgen05.ld), combine
 // lanes with one shuffle per element and store the partial tile.
 #include "scw_internal.h"
@@ -26,20 +27,24 @@ using namespace tc;
 
 constexpr int TA_BM = 128;                 // real rows per tile (= 64 complex rows)
 constexpr int TA_BK = 64;                  // modes per pipeline stage
-constexpr int TA_PROD_WARPS = 8;
-constexpr int TA_THREADS = (TA_PROD_WARPS + 2 + 4) * 32;
+constexpr int TA_CONV_WARPS = 8;
+constexpr int TA_THREADS = (TA_CONV_WARPS + 2 + 4) * 32;
 constexpr int TA_A_SBO = 144;              // bytes between 8-row groups (144 instead of 128: conflict-free stores)
 constexpr int TA_A_LBO = 16 * TA_A_SBO;    // bytes between 8-mode chunks
 constexpr int TA_A_TILE = 8 * TA_A_LBO;    // one bf16 tile (hi or lo): 18432 bytes
+constexpr int TA_COL_PITCH = 528;          // fp32 staging: 512 B of a V column segment + 16 B alignment slack
+constexpr int TA_STG_BYTES = TA_BK * TA_COL_PITCH;
+constexpr int TA_MMA_STAGES = 2;
 constexpr int TA_TMEM_COLS = 512;
-constexpr int TA_SMEM_LIMIT = 225 * 1024;
+constexpr int TA_SMEM_LIMIT = 226 * 1024;
+constexpr int TA_W_LOADER = TA_CONV_WARPS, TA_MMA_WARP = TA_CONV_WARPS + 1;
 
 struct TaParams {
     const float2* V;
-    int64_t ldV, R2, J;
+    int64_t ldV, R, J;      // R complex rows
     const uint8_t* Wt;      // [n_tile][k_block][hi | lo] K-major UMMA images of [W_r | W_i]
     float* part;            // [slot][Fzt][128] fp32 partial tiles
-    int N2, Fzt, n_tiles, m_tiles, kblocks, S, stages;
+    int N2, Fzt, n_tiles, m_tiles, kblocks, S, stg_stages;
 };
 
 // ---- W~ in UMMA image form -----------------------------------------------------------------------
@@ -87,45 +92,118 @@ __global__ void k_tc_weights(int64_t J, int64_t Fz, int Fzt, int n_tiles, int kb
 }
 
 // ---- main kernel -----------------------------------------------------------------------------------
-__device__ __forceinline__ void ta_load(const TaParams& p, int64_t it, int warp, int lane, float2 (&v)[2][8])
+struct TaPos { int kb, mt; };                      // k-block and m-tile of one iteration (all the V path needs)
+
+__device__ __forceinline__ TaPos ta_pos(const TaParams& p, int64_t it)
 {
     const int64_t tile = it / p.kblocks;
-    const int kb = (int)(it - tile * p.kblocks);
-    const int mt = (int)(tile % p.m_tiles);
-    const int64_t k0 = (int64_t)kb * TA_BK + warp * 8;
-#pragma unroll
-    for (int h = 0; h < 2; ++h) {
-        const int64_t row = (int64_t)mt * TA_BM + 2 * (lane + 32 * h);       // even real row = complex row * 2
-        const bool row_ok = row < p.R2;
-        const float2* src = p.V + (row >> 1) + k0 * p.ldV;
-#pragma unroll
-        for (int kk = 0; kk < 8; ++kk) {
-            float2 t = make_float2(0.f, 0.f);
-            if (row_ok && k0 + kk < p.J) t = __ldg(src + kk * p.ldV);
-            v[h][kk] = t;
-        }
+    TaPos q;
+    q.kb = (int)(it - tile * p.kblocks);
+    q.mt = (int)(tile % p.m_tiles);
+    return q;
+}
+__device__ __forceinline__ void ta_next(const TaParams& p, TaPos& q)
+{
+    if (++q.kb == p.kblocks) {
+        q.kb = 0;
+        if (++q.mt == p.m_tiles) q.mt = 0;
     }
 }
 
-__device__ __forceinline__ void ta_store(uint8_t* a_hi, int warp, int lane, const float2 (&v)[2][8])
+// A V column segment (64 complex rows = 512 B) starts at a 16-byte boundary only when (V/8 + k*ldV) is even;
+// otherwise the bulk copy starts 8 bytes early ("shift" = 8).  The shift depends on the parity of k only.
+__device__ __forceinline__ uint32_t ta_shift(const TaParams& p, int k_parity)
 {
+    return (uint32_t)(((reinterpret_cast<uintptr_t>(p.V) >> 3) + (uint64_t)(k_parity & (int)(p.ldV & 1))) & 1) * 8u;
+}
+// Copies move whole 16-byte granules: the window [shift + nvalid*8) is rounded UP (reading one neighbouring
+// element of V) unless that would leave the V allocation, in which case it is rounded DOWN and the cut-off
+// last row of that column ("tail") is read directly by its converter thread.
+__device__ __forceinline__ bool ta_tail_cut(const TaParams& p, int64_t k, int64_t row0, int nvalid, uint32_t sh)
+{
+    return ((sh + (uint32_t)nvalid * 8u) & 15u) && (k * p.ldV + row0 + nvalid + 1 > p.ldV * p.J);
+}
+
+// Lanes 0-7 of converter warp w copy columns 8w..8w+7 of the iteration at `q` into the staging slot; lane 0
+// posts the warp's byte count on the slot's barrier (one of TA_CONV_WARPS arrivals).
+__device__ __forceinline__ void ta_issue_columns(const TaParams& p, const TaPos q, uint8_t* stg, uint64_t* bar,
+                                                 int warp, int lane)
+{
+    const int64_t row0 = (int64_t)q.mt * (TA_BM / 2);
+    const int nvalid = (int)min((int64_t)(TA_BM / 2), p.R - row0);
+    const int kl = warp * 8 + (lane & 7);
+    const int64_t k = (int64_t)q.kb * TA_BK + kl;
+    const uint32_t sh = ta_shift(p, lane & 1);
+    uint32_t bytes = 0;
+    if (lane < 8 && k < p.J) {
+        const uint32_t need = sh + (uint32_t)nvalid * 8u;
+        bytes = ta_tail_cut(p, k, row0, nvalid, sh) ? (need & ~15u) : ((need + 15u) & ~15u);
+    }
+    uint32_t total = bytes;
+    total += __shfl_xor_sync(0xffffffffu, total, 1);
+    total += __shfl_xor_sync(0xffffffffu, total, 2);
+    total += __shfl_xor_sync(0xffffffffu, total, 4);
+    if (lane == 0) mbar_expect_tx(bar, total);
+    __syncwarp();
+    if (bytes)
+        bulk_g2s(stg + kl * TA_COL_PITCH, reinterpret_cast<const uint8_t*>(p.V + k * p.ldV + row0) - sh, bytes, bar);
+}
+
+__device__ __forceinline__ void ta_split_store(uint8_t* dst, const float2 (&v)[8])
+{
+    uint4 eh, el, oh, ol;
+    split_bf16x2(v[0].x, v[1].x, eh.x, el.x);
+    split_bf16x2(v[2].x, v[3].x, eh.y, el.y);
+    split_bf16x2(v[4].x, v[5].x, eh.z, el.z);
+    split_bf16x2(v[6].x, v[7].x, eh.w, el.w);
+    split_bf16x2(v[0].y, v[1].y, oh.x, ol.x);
+    split_bf16x2(v[2].y, v[3].y, oh.y, ol.y);
+    split_bf16x2(v[4].y, v[5].y, oh.z, ol.z);
+    split_bf16x2(v[6].y, v[7].y, oh.w, ol.w);
+    *reinterpret_cast<uint4*>(dst) = eh;                       // even real row (Re)
+    *reinterpret_cast<uint4*>(dst + 16) = oh;                  // odd real row (Im)
+    *reinterpret_cast<uint4*>(dst + TA_A_TILE) = el;
+    *reinterpret_cast<uint4*>(dst + TA_A_TILE + 16) = ol;
+}
+
+// Converter warp w: staging columns 8w..8w+7 (fp32, [k][row]) -> bf16 hi/lo K-major tiles, k-chunk w.
+// lane l handles complex rows l and l+32 (real rows 2l, 2l+1 and 2l+64, 2l+65).
+__device__ __forceinline__ void ta_convert(const TaParams& p, const uint8_t* stg, uint8_t* a_hi, const TaPos q,
+                                           int warp, int lane)
+{
+    const int64_t row0 = (int64_t)q.mt * (TA_BM / 2);
+    const int nvalid = (int)min((int64_t)(TA_BM / 2), p.R - row0);
+    const uint32_t sh0 = ta_shift(p, 0), sh1 = ta_shift(p, 1);
+    const uint8_t* src0 = stg + warp * 8 * TA_COL_PITCH + lane * 8 + sh0;      // even columns
+    const uint8_t* src1 = stg + warp * 8 * TA_COL_PITCH + lane * 8 + sh1;      // odd columns
+    uint8_t* dst = a_hi + warp * TA_A_LBO + (lane >> 2) * TA_A_SBO + (lane & 3) * 32;
+    const bool slow = nvalid < TA_BM / 2 || (int64_t)(q.kb + 1) * TA_BK > p.J ||
+                      (q.kb == p.kblocks - 1 && row0 + nvalid == p.ldV);
+    if (!slow) {
 #pragma unroll
-    for (int h = 0; h < 2; ++h) {
-        const int r = 2 * (lane + 32 * h);                                   // even row in tile; r+1 is its Im row
-        uint8_t* dst = a_hi + warp * TA_A_LBO + (r >> 3) * TA_A_SBO + (r & 7) * 16;
-        uint4 eh, el, oh, ol;
-        split_bf16x2(v[h][0].x, v[h][1].x, eh.x, el.x);
-        split_bf16x2(v[h][2].x, v[h][3].x, eh.y, el.y);
-        split_bf16x2(v[h][4].x, v[h][5].x, eh.z, el.z);
-        split_bf16x2(v[h][6].x, v[h][7].x, eh.w, el.w);
-        split_bf16x2(v[h][0].y, v[h][1].y, oh.x, ol.x);
-        split_bf16x2(v[h][2].y, v[h][3].y, oh.y, ol.y);
-        split_bf16x2(v[h][4].y, v[h][5].y, oh.z, ol.z);
-        split_bf16x2(v[h][6].y, v[h][7].y, oh.w, ol.w);
-        *reinterpret_cast<uint4*>(dst) = eh;
-        *reinterpret_cast<uint4*>(dst + 16) = oh;
-        *reinterpret_cast<uint4*>(dst + TA_A_TILE) = el;
-        *reinterpret_cast<uint4*>(dst + TA_A_TILE + 16) = ol;
+        for (int h = 0; h < 2; ++h) {
+            float2 v[8];
+#pragma unroll
+            for (int kk = 0; kk < 8; ++kk)
+                v[kk] = *reinterpret_cast<const float2*>(((kk & 1) ? src1 : src0) + kk * TA_COL_PITCH + h * 256);
+            ta_split_store(dst + h * 8 * TA_A_SBO, v);
+        }
+    } else {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int rp = lane + 32 * h;
+            float2 v[8];
+#pragma unroll
+            for (int kk = 0; kk < 8; ++kk) {
+                const int64_t k = (int64_t)q.kb * TA_BK + warp * 8 + kk;
+                float2 t = *reinterpret_cast<const float2*>(((kk & 1) ? src1 : src0) + kk * TA_COL_PITCH + h * 256);
+                const bool valid = rp < nvalid && k < p.J;
+                if (valid && rp == nvalid - 1 && ta_tail_cut(p, k, row0, nvalid, (kk & 1) ? sh1 : sh0))
+                    t = __ldg(p.V + k * p.ldV + row0 + rp);
+                v[kk] = valid ? t : make_float2(0.f, 0.f);
+            }
+            ta_split_store(dst + h * 8 * TA_A_SBO, v);
+        }
     }
 }
 
@@ -133,18 +211,20 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const TaParams p)
 {
     extern __shared__ __align__(1024) uint8_t smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int stage_bytes = 2 * TA_A_TILE + p.N2 * 256;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)p.stages * stage_bytes);
-    uint64_t* full_a = bars;
-    uint64_t* full_b = bars + p.stages;
-    uint64_t* empty = bars + 2 * p.stages;
-    uint64_t* acc_full = bars + 3 * p.stages;
-    uint64_t* acc_empty = acc_full + 2;
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
+    const int mma_stage_bytes = 2 * TA_A_TILE + p.N2 * 256;
+    uint8_t* stg_base = smem + (size_t)TA_MMA_STAGES * mma_stage_bytes;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(stg_base + (size_t)p.stg_stages * TA_STG_BYTES);
+    uint64_t* full_a = bars;                          // converters -> MMA           [TA_MMA_STAGES]
+    uint64_t* full_b = full_a + TA_MMA_STAGES;        // W bulk copy -> MMA          [TA_MMA_STAGES]
+    uint64_t* empty = full_b + TA_MMA_STAGES;         // MMA commit -> converters, W [TA_MMA_STAGES]
+    uint64_t* acc_full = empty + TA_MMA_STAGES;       // MMA commit -> epilogue      [2]
+    uint64_t* acc_empty = acc_full + 2;               // epilogue -> MMA             [2]
+    uint64_t* stg_full = acc_empty + 2;               // V bulk copies -> converters [stg_stages]
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(stg_full + p.stg_stages);
 
     if (tid == 0) {
-        for (int s = 0; s < p.stages; ++s) {
-            mbar_init(&full_a[s], TA_PROD_WARPS * 32);
+        for (int s = 0; s < TA_MMA_STAGES; ++s) {
+            mbar_init(&full_a[s], TA_CONV_WARPS * 32);
             mbar_init(&full_b[s], 1);
             mbar_init(&empty[s], 1);
         }
@@ -152,9 +232,10 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const TaParams p)
             mbar_init(&acc_full[b], 1);
             mbar_init(&acc_empty[b], 4);
         }
+        for (int s = 0; s < p.stg_stages; ++s) mbar_init(&stg_full[s], TA_CONV_WARPS);
         mbar_fence_init();
     }
-    if (warp == 9) tmem_alloc(tmem_slot, TA_TMEM_COLS);
+    if (warp == TA_MMA_WARP) tmem_alloc(tmem_slot, TA_TMEM_COLS);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -164,25 +245,36 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const TaParams p)
     const int64_t it0 = (int64_t)blockIdx.x * T / gridDim.x;
     const int64_t it1 = (int64_t)(blockIdx.x + 1) * T / gridDim.x;
 
-    if (warp < TA_PROD_WARPS) {
-        // ===== V producers: HBM -> registers -> bf16 hi/lo -> shared memory =====
-        float2 cur[2][8], nxt[2][8];
-        int stage = 0;
-        uint32_t phase = 0;
-        if (it0 < it1) ta_load(p, it0, warp, lane, cur);
-        for (int64_t it = it0; it < it1; ++it) {
-            if (it + 1 < it1) ta_load(p, it + 1, warp, lane, nxt);
-            mbar_wait(&empty[stage], phase ^ 1);
-            ta_store(smem + (size_t)stage * stage_bytes, warp, lane, cur);
-            fence_proxy_async();
-            mbar_arrive(&full_a[stage]);
-#pragma unroll
-            for (int h = 0; h < 2; ++h)
-#pragma unroll
-                for (int kk = 0; kk < 8; ++kk) cur[h][kk] = nxt[h][kk];
-            if (++stage == p.stages) { stage = 0; phase ^= 1; }
+    if (warp < TA_CONV_WARPS) {
+        // ===== converters: fp32 staging -> bf16 hi/lo UMMA tiles.  Warp w owns staging columns 8w..8w+7 of
+        // every stage: it converts them and then refills the same columns for iteration it + stg_stages
+        // (lanes 0-7 issue one bulk copy each), so no "staging empty" barrier is needed.
+        int sa = 0, ss = 0;
+        uint32_t pa = 0, ps = 0;
+        TaPos cur = ta_pos(p, it0), ahead = cur;
+        int64_t it_ahead = it0;
+        for (int pre = 0; pre < p.stg_stages; ++pre, ++it_ahead) {
+            if (it_ahead < it1) ta_issue_columns(p, ahead, stg_base + (size_t)pre * TA_STG_BYTES, &stg_full[pre], warp, lane);
+            ta_next(p, ahead);
         }
-    } else if (warp == 8) {
+        for (int64_t it = it0; it < it1; ++it, ++it_ahead) {
+            if (warp == 0) {                       // one warp polls, the other seven sleep on a named barrier
+                mbar_wait(&stg_full[ss], ps);
+                mbar_wait(&empty[sa], pa ^ 1);
+            }
+            named_bar_sync(1, TA_CONV_WARPS * 32);
+            uint8_t* stg = stg_base + (size_t)ss * TA_STG_BYTES;
+            ta_convert(p, stg, smem + (size_t)sa * mma_stage_bytes, cur, warp, lane);
+            fence_proxy_async();
+            mbar_arrive(&full_a[sa]);
+            __syncwarp();
+            if (it_ahead < it1) ta_issue_columns(p, ahead, stg, &stg_full[ss], warp, lane);
+            ta_next(p, cur);
+            ta_next(p, ahead);
+            if (++sa == TA_MMA_STAGES) { sa = 0; pa ^= 1; }
+            if (++ss == p.stg_stages) { ss = 0; ps ^= 1; }
+        }
+    } else if (warp == TA_W_LOADER) {
         // ===== W tile loader (bulk async copy, completes on full_b) =====
         if (lane == 0) {
             int stage = 0;
@@ -194,23 +286,24 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const TaParams p)
                 const int nt = (int)(tile / p.m_tiles);
                 mbar_wait(&empty[stage], phase ^ 1);
                 mbar_expect_tx(&full_b[stage], bytes);
-                bulk_g2s(smem + (size_t)stage * stage_bytes + 2 * TA_A_TILE,
+                bulk_g2s(smem + (size_t)stage * mma_stage_bytes + 2 * TA_A_TILE,
                          p.Wt + ((size_t)nt * p.kblocks + kb) * bytes, bytes, &full_b[stage]);
-                if (++stage == p.stages) { stage = 0; phase ^= 1; }
+                if (++stage == TA_MMA_STAGES) { stage = 0; phase ^= 1; }
             }
         }
-    } else if (warp == 9) {
+    } else if (warp == TA_MMA_WARP) {
         // ===== MMA issuer (one thread) =====
         if (lane == 0) {
             const uint32_t idesc = umma_idesc_bf16(TA_BM, p.N2);
             const uint32_t b_lbo = (uint32_t)p.N2 * 16;
             int stage = 0, buf = 0;
-            uint32_t phase = 0, use[2] = {0, 0};
+            uint32_t phase = 0, use0 = 0, use1 = 0;
             int64_t it = it0;
             while (it < it1) {
                 const int64_t tile = it / p.kblocks;
                 const int64_t seg_end = min(it1, (tile + 1) * p.kblocks);
-                mbar_wait(&acc_empty[buf], (use[buf] & 1) ^ 1);
+                const uint32_t use = buf ? use1 : use0;
+                mbar_wait(&acc_empty[buf], (use & 1) ^ 1);
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + (uint32_t)(buf * p.N2);
                 uint32_t acc = 0;
@@ -218,7 +311,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const TaParams p)
                     mbar_wait(&full_a[stage], phase);
                     mbar_wait(&full_b[stage], phase);
                     tc_fence_after();
-                    const uint32_t a_hi = smem_u32(smem + (size_t)stage * stage_bytes);
+                    const uint32_t a_hi = smem_u32(smem + (size_t)stage * mma_stage_bytes);
                     const uint32_t a_lo = a_hi + TA_A_TILE;
                     const uint32_t b_hi = a_hi + 2 * TA_A_TILE;
                     const uint32_t b_lo = b_hi + (uint32_t)p.N2 * 128;
@@ -234,10 +327,10 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const TaParams p)
                         umma_bf16(d_tmem, da_hi, db_hi, idesc, 1);
                     }
                     umma_commit(&empty[stage]);
-                    if (++stage == p.stages) { stage = 0; phase ^= 1; }
+                    if (++stage == TA_MMA_STAGES) { stage = 0; phase ^= 1; }
                 }
                 umma_commit(&acc_full[buf]);
-                use[buf]++;
+                if (buf) ++use1; else ++use0;
                 buf ^= 1;
             }
         }
@@ -245,12 +338,13 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const TaParams p)
         // ===== epilogue: TMEM -> registers -> lane-pair combine -> partial tile =====
         const int q = warp & 3;                                   // TMEM lane quarter this warp may access
         int buf = 0, seg = 0;
-        uint32_t use[2] = {0, 0};
+        uint32_t use0 = 0, use1 = 0;
         int64_t it = it0;
         while (it < it1) {
             const int64_t tile = it / p.kblocks;
             const int64_t seg_end = min(it1, (tile + 1) * p.kblocks);
-            mbar_wait(&acc_full[buf], use[buf] & 1);
+            if (q == 0) mbar_wait(&acc_full[buf], (buf ? use1 : use0) & 1);
+            named_bar_sync(2, 128);
             tc_fence_after();
             float* out = p.part + ((size_t)blockIdx.x * p.S + seg) * ((size_t)p.Fzt * TA_BM) + 32 * q + lane;
             const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(buf * p.N2);
@@ -269,7 +363,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const TaParams p)
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(&acc_empty[buf]);
-            use[buf]++;
+            if (buf) ++use1; else ++use0;
             buf ^= 1;
             ++seg;
             it = seg_end;
@@ -277,7 +371,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const TaParams p)
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 9) tmem_dealloc(tmem_base, TA_TMEM_COLS);
+    if (warp == TA_MMA_WARP) tmem_dealloc(tmem_base, TA_TMEM_COLS);
 }
 
 // Sum the segments of every tile in CTA order: P[mt*64 + r, nt*Fzt + n] = sum_seg part[seg][n][2r..2r+1].
@@ -307,7 +401,7 @@ __global__ void k_tc_reduce(int64_t R, int64_t Fz, int Fzt, int m_tiles, int kbl
 
 // ---- host side -------------------------------------------------------------------------------------
 struct TaPlan {
-    int Fzt, N2, n_tiles, m_tiles, kblocks, G, S, stages;
+    int Fzt, N2, n_tiles, m_tiles, kblocks, G, S, stg_stages;
     int64_t T;
     size_t wt_bytes, part_bytes, smem_bytes;
 };
@@ -316,7 +410,7 @@ static TaPlan ta_plan(int64_t R, int64_t J, int64_t Fz, int sm_count)
 {
     TaPlan pl;
     int64_t fzt = (Fz + 7) / 8 * 8;
-    if (fzt > 128) fzt = 128;
+    if (fzt > 64) fzt = 64;
     pl.Fzt = (int)fzt;
     pl.N2 = 2 * pl.Fzt;
     pl.n_tiles = (int)((Fz + pl.Fzt - 1) / pl.Fzt);
@@ -332,10 +426,10 @@ static TaPlan ta_plan(int64_t R, int64_t J, int64_t Fz, int sm_count)
             if (span > pl.S) pl.S = span;
         }
     }
-    const int stage_bytes = 2 * TA_A_TILE + pl.N2 * 256;
-    pl.stages = (TA_SMEM_LIMIT - 256) / stage_bytes;
-    if (pl.stages > 4) pl.stages = 4;
-    pl.smem_bytes = (size_t)pl.stages * stage_bytes + 256;
+    const int mma_bytes = TA_MMA_STAGES * (2 * TA_A_TILE + pl.N2 * 256);
+    pl.stg_stages = (TA_SMEM_LIMIT - 256 - mma_bytes) / TA_STG_BYTES;
+    if (pl.stg_stages > 4) pl.stg_stages = 4;
+    pl.smem_bytes = (size_t)mma_bytes + (size_t)pl.stg_stages * TA_STG_BYTES + 256;
     pl.wt_bytes = align_up((size_t)pl.n_tiles * pl.kblocks * pl.N2 * 256);
     pl.part_bytes = align_up((size_t)pl.G * pl.S * pl.Fzt * TA_BM * sizeof(float));
     return pl;
@@ -369,7 +463,7 @@ void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const doub
     TaParams p;
     p.V = (const float2*)L->V;
     p.ldV = L->ldV;
-    p.R2 = 2 * R;
+    p.R = R;
     p.J = L->J;
     p.Wt = Wt;
     p.part = part;
@@ -379,7 +473,7 @@ void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const doub
     p.m_tiles = pl.m_tiles;
     p.kblocks = pl.kblocks;
     p.S = pl.S;
-    p.stages = pl.stages;
+    p.stg_stages = pl.stg_stages;
     {
         KernelScope ks(ctx, KC_ASSEMBLE_TC);
         cudaFuncSetAttribute(k_tc_assemble, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes);
