@@ -125,12 +125,54 @@ void run_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z,
 }
 
 // ---- synthesis ----------------------------------------------------------------------------
-size_t twiddle_ws(int dtype, int U, int Vn, int64_t Nx, int64_t Ny)
+// ---- synthesis: tensor-core kernel for complex64 with 2U, 2V <= 80, CUDA-core kernels otherwise ----
+bool use_tc_synth(const scw_ctx* ctx, int dtype, int U, int Vn)
 {
+    return ctx->path != SCW_PATH_SIMT && tc_synth_supported(dtype, U, Vn);
+}
+
+struct Twiddles {
+    bool tc;
+    void* a;     // CUDA-core: FxT [U x Nx];  tensor-core: image blob (A1 | A2)
+    void* b;     // CUDA-core: FyT [Vn x Ny]
+};
+
+size_t twiddle_ws(const scw_ctx* ctx, int dtype, int U, int Vn, int64_t Nx, int64_t Ny)
+{
+    if (use_tc_synth(ctx, dtype, U, Vn)) return align_up(tc_synth_twiddle_bytes(U, Vn, Nx, Ny));
     return align_up((size_t)U * Nx * esize(dtype)) + align_up((size_t)Vn * Ny * esize(dtype));
 }
 
-size_t synth_ws(int dtype, int U, int64_t Fz, int64_t Ny) { return simt_synth_scratch(dtype, U, Fz, Ny); }
+size_t synth_ws(const scw_ctx* ctx, int dtype, int U, int Vn, int64_t Fz, int64_t Ny)
+{
+    if (use_tc_synth(ctx, dtype, U, Vn)) return align_up(tc_synth_scratch(U, Vn, Fz));
+    return simt_synth_scratch(dtype, U, Fz, Ny);
+}
+
+Twiddles run_twiddles(scw_ctx* ctx, int dtype, int U, int Vn, double X, double Y, int64_t Nx, const double* x,
+                      int64_t Ny, const double* y, Carver& cv)
+{
+    Twiddles t;
+    t.tc = use_tc_synth(ctx, dtype, U, Vn);
+    if (t.tc) {
+        t.a = cv.take(tc_synth_twiddle_bytes(U, Vn, Nx, Ny));
+        t.b = nullptr;
+        launch_tc_synth_twiddles(ctx, U, Vn, X, Y, Nx, x, Ny, y, t.a);
+    } else {
+        t.a = cv.take((size_t)U * Nx * esize(dtype));
+        t.b = cv.take((size_t)Vn * Ny * esize(dtype));
+        launch_twiddles(ctx, dtype, U, Nx, x, X, t.a);
+        launch_twiddles(ctx, dtype, Vn, Ny, y, Y, t.b);
+    }
+    return t;
+}
+
+void run_synth(scw_ctx* ctx, const Twiddles& t, int dtype, int U, int Vn, int64_t Fz, const void* P, int64_t ldP,
+               int64_t Nx, int64_t Ny, void* E, const int64_t s4[4], void* scratch)
+{
+    if (t.tc) launch_tc_synth(ctx, U, Vn, Fz, P, ldP, Nx, Ny, t.a, E, s4, scratch);
+    else launch_simt_synth(ctx, dtype, U, Vn, Fz, P, ldP, Nx, t.a, Ny, t.b, E, s4, scratch);
+}
 
 int32_t check_grid(scw_ctx* ctx, int32_t dtype, int32_t U, int32_t Vn, double X, double Y, int64_t Nx,
                    const double* x, int64_t Ny, const double* y, const char* who)
@@ -298,7 +340,7 @@ int32_t scw_synthesize_workspace(scw_ctx* ctx, int32_t dtype, int32_t U, int32_t
     ctx->msg[0] = 0;
     if (dtype != SCW_C64 && dtype != SCW_C128) return fail(ctx, SCW_ERR_DTYPE, "bad dtype %d", dtype);
     if (U <= 0 || Vn <= 0 || Fz < 0 || Nx <= 0 || Ny <= 0) return fail(ctx, SCW_ERR_SHAPE, "bad dimensions");
-    *bytes = Fz ? twiddle_ws(dtype, U, Vn, Nx, Ny) + synth_ws(dtype, U, Fz, Ny) : 0;
+    *bytes = Fz ? twiddle_ws(ctx, dtype, U, Vn, Nx, Ny) + synth_ws(ctx, dtype, U, Vn, Fz, Ny) : 0;
     return SCW_OK;
 }
 
@@ -317,14 +359,13 @@ int32_t scw_synthesize_grid(scw_ctx* ctx, int32_t dtype, int32_t U, int32_t Vn, 
     if (strides) memcpy(s4, strides, sizeof(s4)); else planar_strides(Nx, Ny, s4);
     for (int i = 0; i < 4; ++i)
         if (s4[i] < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_synthesize_grid: negative stride");
-    if (int32_t s = need_ws(ctx, twiddle_ws(dtype, U, Vn, Nx, Ny) + synth_ws(dtype, U, Fz, Ny), "scw_synthesize_grid")) return s;
+    if (ctx->path == SCW_PATH_TENSOR && !tc_synth_supported(dtype, U, Vn))
+        return fail(ctx, SCW_ERR_UNSUPPORTED, "scw_synthesize_grid: no tensor-core synthesis for this dtype / frequency count");
+    if (int32_t s = need_ws(ctx, twiddle_ws(ctx, dtype, U, Vn, Nx, Ny) + synth_ws(ctx, dtype, U, Vn, Fz, Ny), "scw_synthesize_grid")) return s;
     Carver cv(ctx->ws);
-    void* FxT = cv.take((size_t)U * Nx * esize(dtype));
-    void* FyT = cv.take((size_t)Vn * Ny * esize(dtype));
-    void* scratch = cv.take(synth_ws(dtype, U, Fz, Ny));
-    launch_twiddles(ctx, dtype, U, Nx, x, X, FxT);
-    launch_twiddles(ctx, dtype, Vn, Ny, y, Y, FyT);
-    launch_simt_synth(ctx, dtype, U, Vn, Fz, P, ldP, Nx, FxT, Ny, FyT, E, s4, scratch);
+    const Twiddles tw = run_twiddles(ctx, dtype, U, Vn, X, Y, Nx, x, Ny, y, cv);
+    void* scratch = cv.take(synth_ws(ctx, dtype, U, Vn, Fz, Ny));
+    run_synth(ctx, tw, dtype, U, Vn, Fz, P, ldP, Nx, Ny, E, s4, scratch);
     return check_launch(ctx, "scw_synthesize_grid");
 }
 
@@ -353,12 +394,12 @@ static int32_t check_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, 
     return SCW_OK;
 }
 
-static size_t sweep_ws(const scw_layer* L0, int64_t fz_max, size_t asm_max, int64_t Nx, int64_t Ny)
+static size_t sweep_ws(const scw_ctx* ctx, const scw_layer* L0, int64_t fz_max, size_t asm_max, int64_t Nx, int64_t Ny)
 {
     if (fz_max == 0) return 0;
     const int64_t R = 3LL * L0->U * L0->Vn;
-    return twiddle_ws(L0->dtype, L0->U, L0->Vn, Nx, Ny) + align_up((size_t)R * fz_max * esize(L0->dtype)) + asm_max +
-           synth_ws(L0->dtype, L0->U, fz_max, Ny);
+    return twiddle_ws(ctx, L0->dtype, L0->U, L0->Vn, Nx, Ny) + align_up((size_t)R * fz_max * esize(L0->dtype)) + asm_max +
+           synth_ws(ctx, L0->dtype, L0->U, L0->Vn, fz_max, Ny);
 }
 
 int32_t scw_sweep_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, int64_t Nx,
@@ -369,7 +410,7 @@ int32_t scw_sweep_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst,
     int64_t fz_max = 0;
     size_t asm_max = 0;
     if (int32_t s = check_sweep(ctx, n_inst, inst, Fz, Nx, Ny, "scw_sweep_workspace", &fz_max, &asm_max)) return s;
-    *bytes = n_inst ? sweep_ws(&inst[0], fz_max, asm_max, Nx, Ny) : 0;
+    *bytes = n_inst ? sweep_ws(ctx, &inst[0], fz_max, asm_max, Nx, Ny) : 0;
     return SCW_OK;
 }
 
@@ -380,19 +421,16 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
 {
     const scw_layer& L0 = inst[0];
     const int64_t R = 3LL * L0.U * L0.Vn;
-    void* FxT = cv.take((size_t)L0.U * Nx * esize(L0.dtype));
-    void* FyT = cv.take((size_t)L0.Vn * Ny * esize(L0.dtype));
+    const Twiddles tw = run_twiddles(ctx, L0.dtype, L0.U, L0.Vn, L0.X, L0.Y, Nx, x, Ny, y, cv);
     void* P = cv.take((size_t)R * fz_max * esize(L0.dtype));
     const size_t asm_off = cv.off;
     cv.take(asm_max);
-    void* scratch = cv.take(synth_ws(L0.dtype, L0.U, fz_max, Ny));
-    launch_twiddles(ctx, L0.dtype, L0.U, Nx, x, L0.X, FxT);
-    launch_twiddles(ctx, L0.dtype, L0.Vn, Ny, y, L0.Y, FyT);
+    void* scratch = cv.take(synth_ws(ctx, L0.dtype, L0.U, L0.Vn, fz_max, Ny));
     for (int64_t i = 0; i < n_inst; ++i) {
         if (Fz[i] == 0) continue;
         Carver sub(cv.base ? cv.base + asm_off : nullptr);
         run_assemble(ctx, &inst[i], Fz[i], z[i], P, R, sub);
-        launch_simt_synth(ctx, L0.dtype, L0.U, L0.Vn, Fz[i], P, R, Nx, FxT, Ny, FyT, E[i], s4, scratch);
+        run_synth(ctx, tw, L0.dtype, L0.U, L0.Vn, Fz[i], P, R, Nx, Ny, E[i], s4, scratch);
     }
 }
 
@@ -418,7 +456,7 @@ int32_t scw_sweep_wavelengths(scw_ctx* ctx, int64_t n_inst, const scw_layer* ins
     if (strides) memcpy(s4, strides, sizeof(s4)); else planar_strides(Nx, Ny, s4);
     for (int i = 0; i < 4; ++i)
         if (s4[i] < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_sweep_wavelengths: negative stride");
-    if (int32_t s = need_ws(ctx, sweep_ws(&inst[0], fz_max, asm_max, Nx, Ny), "scw_sweep_wavelengths")) return s;
+    if (int32_t s = need_ws(ctx, sweep_ws(ctx, &inst[0], fz_max, asm_max, Nx, Ny), "scw_sweep_wavelengths")) return s;
     Carver cv(ctx->ws);
     run_sweep(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, E, s4, fz_max, asm_max, cv);
     return check_launch(ctx, "scw_sweep_wavelengths");
@@ -460,7 +498,7 @@ int32_t scw_sweep_host_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* 
     if (int32_t s = sweep_host_sizes(ctx, n_inst, inst, Fz, Nx, Ny, "scw_sweep_host_workspace", &fz_max, &asm_max,
                                      &in_max, &e_max)) return s;
     *bytes = n_inst ? align_up((size_t)Nx * 8) + align_up((size_t)Ny * 8) + in_max + e_max +
-                          sweep_ws(&inst[0], fz_max, asm_max, Nx, Ny)
+                          sweep_ws(ctx, &inst[0], fz_max, asm_max, Nx, Ny)
                     : 0;
     return SCW_OK;
 }
@@ -483,7 +521,7 @@ int32_t scw_sweep_wavelengths_host(scw_ctx* ctx, int64_t n_inst, const scw_layer
     for (int64_t i = 0; i < n_inst; ++i)
         if (Fz[i] > 0 && (!z[i] || !E[i])) return fail(ctx, SCW_ERR_NULL, "scw_sweep_wavelengths_host: z[i]/E[i] is NULL");
     const size_t total = align_up((size_t)Nx * 8) + align_up((size_t)Ny * 8) + in_max + e_max +
-                         sweep_ws(&inst[0], fz_max, asm_max, Nx, Ny);
+                         sweep_ws(ctx, &inst[0], fz_max, asm_max, Nx, Ny);
     if (int32_t s = need_ws(ctx, total, "scw_sweep_wavelengths_host")) return s;
 
     Carver cv(ctx->ws);
@@ -502,14 +540,11 @@ int32_t scw_sweep_wavelengths_host(scw_ctx* ctx, int64_t n_inst, const scw_layer
     };
     h2d(dx, x, (size_t)Nx * 8);
     h2d(dy, y, (size_t)Ny * 8);
-    void* FxT = cv.take((size_t)L0.U * Nx * es);
-    void* FyT = cv.take((size_t)L0.Vn * Ny * es);
+    const Twiddles tw = run_twiddles(ctx, L0.dtype, L0.U, L0.Vn, L0.X, L0.Y, Nx, dx, Ny, dy, cv);
     void* P = cv.take((size_t)R * fz_max * es);
     const size_t asm_off = cv.off;
     cv.take(asm_max);
-    void* scratch = cv.take(synth_ws(L0.dtype, L0.U, fz_max, Ny));
-    launch_twiddles(ctx, L0.dtype, L0.U, Nx, dx, L0.X, FxT);
-    launch_twiddles(ctx, L0.dtype, L0.Vn, Ny, dy, L0.Y, FyT);
+    void* scratch = cv.take(synth_ws(ctx, L0.dtype, L0.U, L0.Vn, fz_max, Ny));
     int64_t s4[4];
     planar_strides(Nx, Ny, s4);
     for (int64_t i = 0; i < n_inst && err == cudaSuccess; ++i) {
@@ -532,7 +567,7 @@ int32_t scw_sweep_wavelengths_host(scw_ctx* ctx, int64_t n_inst, const scw_layer
         L.dir = L.dir ? (const int8_t*)dd : nullptr;
         Carver sub((char*)ctx->ws + asm_off);
         run_assemble(ctx, &L, Fz[i], (const double*)dz, P, R, sub);
-        launch_simt_synth(ctx, L0.dtype, L0.U, L0.Vn, Fz[i], P, R, Nx, FxT, Ny, FyT, stage_e, s4, scratch);
+        run_synth(ctx, tw, L0.dtype, L0.U, L0.Vn, Fz[i], P, R, Nx, Ny, stage_e, s4, scratch);
         const size_t eb = (size_t)Fz[i] * 3 * Nx * Ny * es;
         if (err == cudaSuccess) err = cudaMemcpyAsync(E[i], stage_e, eb, cudaMemcpyDeviceToHost, ctx->stream);
         down += (int64_t)eb;

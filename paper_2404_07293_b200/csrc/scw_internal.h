@@ -98,6 +98,15 @@ size_t tc_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int sm_count);
 void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z, void* P, int64_t ldP,
                         void* scratch);
 
+// ---- scw_tc_synth.cu: tcgen05 BF16x3 separable synthesis (complex64, 2U and 2V <= 80) ---------------
+bool tc_synth_supported(int dtype, int U, int Vn);
+size_t tc_synth_twiddle_bytes(int U, int Vn, int64_t Nx, int64_t Ny);
+size_t tc_synth_scratch(int U, int Vn, int64_t Fz);
+void launch_tc_synth_twiddles(scw_ctx* ctx, int U, int Vn, double X, double Y, int64_t Nx, const double* x, int64_t Ny,
+                              const double* y, void* tw);
+void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,
+                     const void* tw, void* E, const int64_t strides[4], void* scratch);
+
 // ---- points.cu ------------------------------------------------------------------------------
 struct PwTableInfo { size_t bytes; };
 size_t points_table_bytes(int dtype, int64_t J);

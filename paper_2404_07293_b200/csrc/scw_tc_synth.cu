@@ -1,0 +1,391 @@
+// Separable Fourier synthesis E_comp(z) = F_x . P_comp(z) . F_y^T on the 5th-gen tensor cores, complex64.
+//   E_comp(x_i, y_k, z_n) = sum_{u,v} P[comp*M + m(u,v), n] exp(i 2 pi (u x_i/X + v y_k/Y))     (eq. 10)
+// exact because the spatial frequencies lie on a rectangular (u,v) grid (eq. 6).
+//
+// One persistent CTA owns a 128(x) x 128(y) output tile and walks the (z, comp) planes.  Per plane two chained
+// real GEMMs run on tcgen05 with fp32 accumulators in TMEM, each as three bf16 products (hi*hi + hi*lo + lo*hi):
+//   GEMM1  D1[y, 2u+c]        = sum_k A1[y, k] B1[2u+c, k]        A1 = (Fy_r, Fy_i) interleaved over k = 2v+c''
+//                                                                  B1 = the plane's spectrum in "complex as real" form
+//          -> D1 row y holds T[u, y] = sum_v P[u,v] Fy[y,v] as (Re, Im) pairs
+//   GEMM2  D2[x, 2y+c]        = sum_k A2[x, k] B2[2y+c, k]        A2 = (Fx_r, Fx_i), B2 built from D1 in-kernel
+// The 128 converter threads read their own D1 row from TMEM (tcgen05.ld), split it to bf16 hi/lo and write the two
+// B2 rows (y,Re), (y,Im) of the K-major UMMA image; the 128 epilogue threads read D2 (lane = x) and store
+// (Re, Im) pairs straight to E: a warp writes 256 contiguous bytes per y.  Twiddle and spectrum images are
+// produced by two small pre-kernels in fp64 / fp32 and fetched with bulk async copies.
+#include "scw_internal.h"
+#include "scw_tc_common.cuh"
+
+namespace scw {
+
+using namespace tc;
+
+constexpr int TS_TILE = 128;               // output tile edge (x and y)
+constexpr int TS_KMAX = 80;                // max padded K (= 2U, 2V rounded up to 16)
+constexpr int TS_THREADS = 10 * 32;        // loader, MMA, 4 converter warps, 4 epilogue warps
+constexpr int TS_TMEM_COLS = 512;
+constexpr int TS_D2_COL = 0;               // D2[h] at columns h*128
+constexpr int TS_D1_COL = 256;             // D1 at columns 256..256+N1
+
+struct TsParams {
+    const uint8_t* A1;     // [ty][hi|lo] images of (Fy_r, Fy_i): 128 rows x K1p, K-major, LBO = 2048, SBO = 128
+    const uint8_t* A2;     // [tx][hi|lo] images of (Fx_r, Fx_i): 128 rows x K2p
+    const uint8_t* B1;     // [plane][hi|lo] images: N1 rows x K1p, LBO = N1*16, SBO = 128
+    float2* E;
+    int64_t s_comp, s_z, s_y, s_x;
+    int64_t Nx, Ny;
+    int planes;            // Fz * 3
+    int K1p, K2p;          // padded 2V, 2U  (N1 == K2p)
+    int tiles_x, tiles_y, pair0, npairs;   // this launch covers tile pairs [pair0, pair0 + npairs)
+};
+
+__host__ __device__ inline int ts_pad16(int v) { return (v + 15) / 16 * 16; }
+
+// ---- pre-kernels ------------------------------------------------------------------------------------
+// Twiddle images (a-3): for tile t, row r (coordinate index t*128 + r), k = 2f + c: c = 0 -> cos, c = 1 -> sin of
+// 2 pi (f - nfreq/2) coord / period; rows past N and k past 2*nfreq are zero.  hi image then lo image per tile.
+__global__ void k_tc_synth_twiddles(int nfreq, int Kp, int64_t N, int tiles, const double* __restrict__ coord,
+                                    double inv_period, uint8_t* __restrict__ img)
+{
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;      // (tile, r, kpair)
+    const int kpairs = Kp / 2;
+    if (idx >= (int64_t)tiles * TS_TILE * kpairs) return;
+    const int f = (int)(idx % kpairs);
+    const int64_t tr = idx / kpairs;
+    const int r = (int)(tr % TS_TILE);
+    const int t = (int)(tr / TS_TILE);
+    const int64_t i = (int64_t)t * TS_TILE + r;
+    float co = 0.f, si = 0.f;
+    if (f < nfreq && i < N) {
+        double ph = (double)(f - nfreq / 2) * (coord[i] * inv_period);
+        ph -= rint(ph);
+        double s, c;
+        sincospi(2.0 * ph, &s, &c);
+        co = (float)c;
+        si = (float)s;
+    }
+    uint32_t hi, lo;
+    split_bf16x2(co, si, hi, lo);
+    const int k = 2 * f;
+    const size_t img_bytes = (size_t)TS_TILE * Kp * 2;
+    uint8_t* base = img + (size_t)t * 2 * img_bytes;
+    const size_t off = (size_t)(k >> 3) * 2048 + (size_t)(r >> 3) * 128 + (r & 7) * 16 + (k & 7) * 2;
+    *reinterpret_cast<uint32_t*>(base + off) = hi;
+    *reinterpret_cast<uint32_t*>(base + img_bytes + off) = lo;
+}
+
+// Spectrum images: plane = n*3 + comp, row = 2u + c, k = 2v + c'':
+//   row (u,Re): (P_r, -P_i);  row (u,Im): (P_i, P_r)   so that  D1[y, (u,c)] = sum_v Fy[y,v] P[u,v]  in real arithmetic.
+__global__ void k_tc_synth_pimage(int U, int Vn, int K1p, int N1, int planes, const float2* __restrict__ P, int64_t ldP,
+                                  uint8_t* __restrict__ img)
+{
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;      // (plane, row, kpair)
+    const int kpairs = K1p / 2;
+    if (idx >= (int64_t)planes * N1 * kpairs) return;
+    const int v = (int)(idx % kpairs);
+    const int64_t pr = idx / kpairs;
+    const int row = (int)(pr % N1);
+    const int64_t plane = pr / N1;
+    const int u = row >> 1, c = row & 1;
+    float a = 0.f, b = 0.f;
+    if (u < U && v < Vn) {
+        const int64_t n = plane / 3;
+        const int comp = (int)(plane - n * 3);
+        const float2 p = P[n * ldP + (int64_t)comp * U * Vn + (int64_t)v * U + u];
+        a = c ? p.y : p.x;
+        b = c ? p.x : -p.y;
+    }
+    uint32_t hi, lo;
+    split_bf16x2(a, b, hi, lo);
+    const int k = 2 * v;
+    const size_t img_bytes = (size_t)N1 * K1p * 2;
+    uint8_t* base = img + (size_t)plane * 2 * img_bytes;
+    const size_t off = (size_t)(k >> 3) * (N1 * 16) + (size_t)(row >> 3) * 128 + (row & 7) * 16 + (k & 7) * 2;
+    *reinterpret_cast<uint32_t*>(base + off) = hi;
+    *reinterpret_cast<uint32_t*>(base + img_bytes + off) = lo;
+}
+
+// ---- main kernel ------------------------------------------------------------------------------------
+// Three-product bf16 GEMM step over K = Kp: D (+)= Ahi*Bhi + Ahi*Blo + Alo*Bhi.
+__device__ __forceinline__ void ts_mma3(uint32_t d_tmem, uint32_t a_hi, uint32_t a_lo, uint32_t a_lbo, uint32_t b_hi,
+                                        uint32_t b_lo, uint32_t b_lbo, int Kp, uint32_t idesc)
+{
+    uint32_t acc = 0;
+    for (int s = 0; s < Kp / 16; ++s) {
+        const uint64_t da_hi = umma_desc(a_hi + s * 2 * a_lbo, a_lbo, 128);
+        const uint64_t da_lo = umma_desc(a_lo + s * 2 * a_lbo, a_lbo, 128);
+        const uint64_t db_hi = umma_desc(b_hi + s * 2 * b_lbo, b_lbo, 128);
+        const uint64_t db_lo = umma_desc(b_lo + s * 2 * b_lbo, b_lbo, 128);
+        umma_bf16(d_tmem, da_lo, db_hi, idesc, acc);
+        acc = 1;
+        umma_bf16(d_tmem, da_hi, db_lo, idesc, 1);
+        umma_bf16(d_tmem, da_hi, db_hi, idesc, 1);
+    }
+}
+
+__global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const TsParams p)
+{
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int K1p = p.K1p, K2p = p.K2p, N1 = p.K2p;
+    const uint32_t a1_img = TS_TILE * K1p * 2, a2_img = TS_TILE * K2p * 2;     // bytes of one (hi or lo) image
+    const uint32_t b1_img = (uint32_t)N1 * K1p * 2, b2_img = TS_TILE * K2p * 2;
+    uint8_t* sA1 = smem;                              // hi | lo
+    uint8_t* sA2 = sA1 + 2 * a1_img;
+    uint8_t* sB1 = sA2 + 2 * a2_img;                  // 2 stages x (hi | lo)
+    uint8_t* sB2 = sB1 + 4 * b1_img;                  // 2 halves x (hi | lo)
+    uint64_t* bars = reinterpret_cast<uint64_t*>(sB2 + 4 * b2_img);
+    uint64_t* tw_full = bars;            // [1]
+    uint64_t* b1_full = bars + 1;        // [2]
+    uint64_t* b1_empty = bars + 3;       // [2]
+    uint64_t* d1_full = bars + 5;        // [1]
+    uint64_t* d1_empty = bars + 6;       // [1]
+    uint64_t* b2_full = bars + 7;        // [2]
+    uint64_t* b2_empty = bars + 9;       // [2]
+    uint64_t* d2_full = bars + 11;       // [2]
+    uint64_t* d2_empty = bars + 13;      // [2]
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 15);
+
+    if (tid == 0) {
+        mbar_init(tw_full, 1);
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(&b1_full[s], 1);
+            mbar_init(&b1_empty[s], 1);
+            mbar_init(&b2_full[s], 2);
+            mbar_init(&b2_empty[s], 1);
+            mbar_init(&d2_full[s], 1);
+            mbar_init(&d2_empty[s], 4);
+        }
+        mbar_init(d1_full, 1);
+        mbar_init(d1_empty, 4);
+        mbar_fence_init();
+    }
+    if (warp == 1) tmem_alloc(tmem_slot, TS_TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    // this CTA's tile pair and plane sequence
+    const int per_pair = gridDim.x / p.npairs;                 // CTAs per pair (gridDim.x is a multiple of npairs)
+    const int pair = p.pair0 + (int)blockIdx.x % p.npairs;
+    const int first_plane = (int)blockIdx.x / p.npairs;
+    const int tx = pair % p.tiles_x, ty = pair / p.tiles_x;
+    const int n_items = first_plane < p.planes ? (p.planes - first_plane + per_pair - 1) / per_pair : 0;
+
+    if (warp == 0) {
+        // ===== loader: twiddle images once, then one spectrum image per plane =====
+        if (lane == 0 && n_items > 0) {
+            mbar_expect_tx(tw_full, 2 * a1_img + 2 * a2_img);
+            bulk_g2s(sA1, p.A1 + (size_t)ty * 2 * a1_img, 2 * a1_img, tw_full);
+            bulk_g2s(sA2, p.A2 + (size_t)tx * 2 * a2_img, 2 * a2_img, tw_full);
+            for (int n = 0; n < n_items; ++n) {
+                const int s = n & 1;
+                const int plane = first_plane + n * per_pair;
+                mbar_wait(&b1_empty[s], ((n >> 1) & 1) ^ 1);
+                mbar_expect_tx(&b1_full[s], 2 * b1_img);
+                bulk_g2s(sB1 + (size_t)s * 2 * b1_img, p.B1 + (size_t)plane * 2 * b1_img, 2 * b1_img, &b1_full[s]);
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer =====
+        if (lane == 0 && n_items > 0) {
+            const uint32_t idesc1 = umma_idesc_bf16(TS_TILE, N1);
+            const uint32_t idesc2 = umma_idesc_bf16(TS_TILE, TS_TILE);
+            const uint32_t a1 = smem_u32(sA1), a2 = smem_u32(sA2), b1 = smem_u32(sB1), b2 = smem_u32(sB2);
+            const uint32_t d1 = tmem_base + TS_D1_COL;
+            mbar_wait(tw_full, 0);
+            auto issue_gemm1 = [&](int n) {
+                const int s = n & 1;
+                mbar_wait(&b1_full[s], (n >> 1) & 1);
+                if (n > 0) mbar_wait(d1_empty, (n - 1) & 1);
+                tc_fence_after();
+                ts_mma3(d1, a1, a1 + a1_img, 2048, b1 + s * 2 * b1_img, b1 + s * 2 * b1_img + b1_img, (uint32_t)N1 * 16, K1p,
+                        idesc1);
+                umma_commit(d1_full);
+                umma_commit(&b1_empty[s]);
+            };
+            auto issue_gemm2 = [&](int n, int h) {
+                mbar_wait(&b2_full[h], n & 1);
+                mbar_wait(&d2_empty[h], (n & 1) ^ 1);
+                tc_fence_after();
+                ts_mma3(tmem_base + TS_D2_COL + h * TS_TILE, a2, a2 + a2_img, 2048, b2 + h * 2 * b2_img,
+                        b2 + h * 2 * b2_img + b2_img, 2048, K2p, idesc2);
+                umma_commit(&d2_full[h]);
+                umma_commit(&b2_empty[h]);
+            };
+            issue_gemm1(0);
+            for (int n = 0; n < n_items; ++n) {
+                issue_gemm2(n, 0);
+                if (n + 1 < n_items) issue_gemm1(n + 1);
+                issue_gemm2(n, 1);
+            }
+        }
+    } else if (warp < 6) {
+        // ===== converters: D1 row y (TMEM) -> B2 rows (y,Re), (y,Im) as bf16 hi/lo =====
+        const int q = warp & 3;                      // TMEM lane quarter: y = 32q + lane
+        const int h = q >> 1;                        // which half of the tile this y belongs to
+        const int yy = 32 * (q & 1) + lane;          // y within the half
+        uint8_t* row = sB2 + (size_t)h * 2 * b2_img + yy * 32;
+        const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + TS_D1_COL;
+        for (int n = 0; n < n_items; ++n) {
+            mbar_wait(d1_full, n & 1);
+            mbar_wait(&b2_empty[h], (n & 1) ^ 1);
+            tc_fence_after();
+            for (int c = 0; c < K2p / 8; ++c) {
+                float t[8];
+                tmem_ld8(taddr + 8 * c, t);          // (Tr0, Ti0, Tr1, Ti1, Tr2, Ti2, Tr3, Ti3)
+                tmem_ld_wait();
+                uint4 re_hi, re_lo, im_hi, im_lo;
+                split_bf16x2(t[0], -t[1], re_hi.x, re_lo.x);
+                split_bf16x2(t[2], -t[3], re_hi.y, re_lo.y);
+                split_bf16x2(t[4], -t[5], re_hi.z, re_lo.z);
+                split_bf16x2(t[6], -t[7], re_hi.w, re_lo.w);
+                split_bf16x2(t[1], t[0], im_hi.x, im_lo.x);
+                split_bf16x2(t[3], t[2], im_hi.y, im_lo.y);
+                split_bf16x2(t[5], t[4], im_hi.z, im_lo.z);
+                split_bf16x2(t[7], t[6], im_hi.w, im_lo.w);
+                uint8_t* dst = row + (size_t)c * 2048;
+                *reinterpret_cast<uint4*>(dst) = re_hi;
+                *reinterpret_cast<uint4*>(dst + 16) = im_hi;
+                *reinterpret_cast<uint4*>(dst + b2_img) = re_lo;
+                *reinterpret_cast<uint4*>(dst + b2_img + 16) = im_lo;
+            }
+            tc_fence_before();
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(d1_empty);
+                mbar_arrive(&b2_full[h]);
+            }
+        }
+    } else {
+        // ===== epilogue: D2 (lane = x, columns = (y, Re/Im)) -> E =====
+        const int q = warp & 3;
+        const int64_t x = (int64_t)tx * TS_TILE + 32 * q + lane;
+        const bool x_ok = x < p.Nx;
+        for (int n = 0; n < n_items; ++n) {
+            const int plane = first_plane + n * per_pair;
+            const int64_t zi = plane / 3;
+            const int comp = plane - (int)zi * 3;
+            float2* out = p.E + comp * p.s_comp + zi * p.s_z + x * p.s_x;
+#pragma unroll 1
+            for (int h = 0; h < 2; ++h) {
+                mbar_wait(&d2_full[h], n & 1);
+                tc_fence_after();
+                const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + TS_D2_COL + h * TS_TILE;
+                const int64_t y0 = (int64_t)ty * TS_TILE + 64 * h;
+#pragma unroll 2
+                for (int c = 0; c < 8; ++c) {
+                    float v[16];
+                    tmem_ld16(taddr + 16 * c, v);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const int64_t y = y0 + 8 * c + e;
+                        if (x_ok && y < p.Ny) out[y * p.s_y] = make_float2(v[2 * e], v[2 * e + 1]);
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&d2_empty[h]);
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc(tmem_base, TS_TMEM_COLS);
+}
+
+// ---- host side -------------------------------------------------------------------------------------
+bool tc_synth_supported(int dtype, int U, int Vn)
+{
+    return dtype == SCW_C64 && ts_pad16(2 * U) <= TS_KMAX && ts_pad16(2 * Vn) <= TS_KMAX;
+}
+
+struct TsPlan {
+    int K1p, K2p, tiles_x, tiles_y;
+    size_t a1_bytes, a2_bytes, b1_bytes, smem_bytes;
+};
+
+static TsPlan ts_plan(int U, int Vn, int64_t Fz, int64_t Nx, int64_t Ny)
+{
+    TsPlan pl;
+    pl.K1p = ts_pad16(2 * Vn);
+    pl.K2p = ts_pad16(2 * U);
+    pl.tiles_x = (int)((Nx + TS_TILE - 1) / TS_TILE);
+    pl.tiles_y = (int)((Ny + TS_TILE - 1) / TS_TILE);
+    pl.a1_bytes = align_up((size_t)pl.tiles_y * 2 * TS_TILE * pl.K1p * 2);
+    pl.a2_bytes = align_up((size_t)pl.tiles_x * 2 * TS_TILE * pl.K2p * 2);
+    pl.b1_bytes = align_up((size_t)Fz * 3 * 2 * pl.K2p * pl.K1p * 2);
+    pl.smem_bytes = (size_t)2 * TS_TILE * pl.K1p * 2 + (size_t)2 * TS_TILE * pl.K2p * 2 +
+                    (size_t)4 * pl.K2p * pl.K1p * 2 + (size_t)4 * TS_TILE * pl.K2p * 2 + 256;
+    return pl;
+}
+
+size_t tc_synth_twiddle_bytes(int U, int Vn, int64_t Nx, int64_t Ny)
+{
+    const TsPlan pl = ts_plan(U, Vn, 1, Nx, Ny);
+    return pl.a1_bytes + pl.a2_bytes;
+}
+
+size_t tc_synth_scratch(int U, int Vn, int64_t Fz) { return ts_plan(U, Vn, Fz, 1, 1).b1_bytes; }
+
+void launch_tc_synth_twiddles(scw_ctx* ctx, int U, int Vn, double X, double Y, int64_t Nx, const double* x, int64_t Ny,
+                              const double* y, void* tw)
+{
+    const TsPlan pl = ts_plan(U, Vn, 1, Nx, Ny);
+    uint8_t* A1 = static_cast<uint8_t*>(tw);
+    uint8_t* A2 = A1 + pl.a1_bytes;
+    {
+        KernelScope ks(ctx, KC_TWIDDLES);
+        const int64_t n = (int64_t)pl.tiles_y * TS_TILE * (pl.K1p / 2);
+        k_tc_synth_twiddles<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(Vn, pl.K1p, Ny, pl.tiles_y, y, 1.0 / Y, A1);
+    }
+    {
+        KernelScope ks(ctx, KC_TWIDDLES);
+        const int64_t n = (int64_t)pl.tiles_x * TS_TILE * (pl.K2p / 2);
+        k_tc_synth_twiddles<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(U, pl.K2p, Nx, pl.tiles_x, x, 1.0 / X, A2);
+    }
+}
+
+void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,
+                     const void* tw, void* E, const int64_t strides[4], void* scratch)
+{
+    const TsPlan pl = ts_plan(U, Vn, Fz, Nx, Ny);
+    const int planes = (int)(Fz * 3);
+    uint8_t* B1 = static_cast<uint8_t*>(scratch);
+    {
+        KernelScope ks(ctx, KC_SYNTH_A);
+        const int64_t n = (int64_t)planes * pl.K2p * (pl.K1p / 2);
+        k_tc_synth_pimage<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(U, Vn, pl.K1p, pl.K2p, planes,
+                                                                                (const float2*)P, ldP, B1);
+    }
+    TsParams p;
+    p.A1 = static_cast<const uint8_t*>(tw);
+    p.A2 = p.A1 + pl.a1_bytes;
+    p.B1 = B1;
+    p.E = static_cast<float2*>(E);
+    p.s_comp = strides[0];
+    p.s_z = strides[1];
+    p.s_y = strides[2];
+    p.s_x = strides[3];
+    p.Nx = Nx;
+    p.Ny = Ny;
+    p.planes = planes;
+    p.K1p = pl.K1p;
+    p.K2p = pl.K2p;
+    p.tiles_x = pl.tiles_x;
+    p.tiles_y = pl.tiles_y;
+    const int total_pairs = pl.tiles_x * pl.tiles_y;
+    cudaFuncSetAttribute(k_tc_synth, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes);
+    for (int pair0 = 0; pair0 < total_pairs; pair0 += ctx->sm_count) {
+        p.pair0 = pair0;
+        p.npairs = total_pairs - pair0 < ctx->sm_count ? total_pairs - pair0 : ctx->sm_count;
+        int per_pair = ctx->sm_count / p.npairs;
+        if (per_pair > planes) per_pair = planes;
+        KernelScope ks(ctx, KC_SYNTH_TC);
+        k_tc_synth<<<p.npairs * per_pair, TS_THREADS, pl.smem_bytes, ctx->stream>>>(p);
+    }
+}
+
+}  // namespace scw
