@@ -106,7 +106,7 @@ bool use_tc_assemble(const scw_ctx* ctx, const scw_layer* L, int64_t Fz)
 size_t assemble_ws(const scw_ctx* ctx, const scw_layer* L, int64_t Fz)
 {
     const int64_t R = 3LL * L->U * L->Vn;
-    if (use_tc_assemble(ctx, L, Fz)) return tc_assemble_scratch(R, L->J, Fz, ctx->sm_count);
+    if (use_tc_assemble(ctx, L, Fz)) return tc_assemble_scratch(R, L->J, Fz, 1, ctx->sm_count);
     return align_up((size_t)L->J * Fz * esize(L->dtype)) + simt_assemble_scratch(L->dtype, R, L->J, Fz, ctx->sm_count);
 }
 
@@ -114,7 +114,7 @@ void run_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z,
 {
     const int64_t R = 3LL * L->U * L->Vn;
     if (use_tc_assemble(ctx, L, Fz)) {
-        void* scratch = cv.take(tc_assemble_scratch(R, L->J, Fz, ctx->sm_count));
+        void* scratch = cv.take(tc_assemble_scratch(R, L->J, Fz, 1, ctx->sm_count));
         launch_tc_assemble(ctx, L, Fz, z, P, ldP, scratch);
         return;
     }
@@ -394,6 +394,25 @@ static int32_t check_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, 
     return SCW_OK;
 }
 
+// Grouped (batched) sweep: every instance on the tensor-core kernels with the same J and Fz.
+static int sweep_group_size(const scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz)
+{
+    if (n_inst < 2 || Fz[0] <= 0) return 0;
+    if (!use_tc_assemble(ctx, &inst[0], Fz[0]) || !use_tc_synth(ctx, inst[0].dtype, inst[0].U, inst[0].Vn)) return 0;
+    for (int64_t i = 1; i < n_inst; ++i)
+        if (inst[i].J != inst[0].J || Fz[i] != Fz[0]) return 0;
+    int g = tc_assemble_max_group() < tc_synth_max_group() ? tc_assemble_max_group() : tc_synth_max_group();
+    return (int)(n_inst < g ? n_inst : g);
+}
+
+static size_t sweep_group_ws(const scw_ctx* ctx, const scw_layer* L0, int64_t Fz, int group, int64_t Nx, int64_t Ny)
+{
+    const int64_t R = 3LL * L0->U * L0->Vn;
+    return twiddle_ws(ctx, L0->dtype, L0->U, L0->Vn, Nx, Ny) + align_up((size_t)R * Fz * group * esize(L0->dtype)) +
+           align_up(tc_assemble_scratch(R, L0->J, Fz, group, ctx->sm_count)) +
+           align_up(tc_synth_scratch(L0->U, L0->Vn, Fz * group));
+}
+
 static size_t sweep_ws(const scw_ctx* ctx, const scw_layer* L0, int64_t fz_max, size_t asm_max, int64_t Nx, int64_t Ny)
 {
     if (fz_max == 0) return 0;
@@ -410,7 +429,9 @@ int32_t scw_sweep_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst,
     int64_t fz_max = 0;
     size_t asm_max = 0;
     if (int32_t s = check_sweep(ctx, n_inst, inst, Fz, Nx, Ny, "scw_sweep_workspace", &fz_max, &asm_max)) return s;
-    *bytes = n_inst ? sweep_ws(ctx, &inst[0], fz_max, asm_max, Nx, Ny) : 0;
+    const int group = n_inst ? sweep_group_size(ctx, n_inst, inst, Fz) : 0;
+    *bytes = !n_inst ? 0 : group ? sweep_group_ws(ctx, &inst[0], Fz[0], group, Nx, Ny)
+                                 : sweep_ws(ctx, &inst[0], fz_max, asm_max, Nx, Ny);
     return SCW_OK;
 }
 
@@ -422,6 +443,19 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
     const scw_layer& L0 = inst[0];
     const int64_t R = 3LL * L0.U * L0.Vn;
     const Twiddles tw = run_twiddles(ctx, L0.dtype, L0.U, L0.Vn, L0.X, L0.Y, Nx, x, Ny, y, cv);
+    const int group = sweep_group_size(ctx, n_inst, inst, Fz);
+    if (group) {
+        // batched: all instances of a group share three assembly launches and two synthesis launches
+        void* P_all = cv.take((size_t)R * Fz[0] * group * esize(L0.dtype));
+        void* a_scr = cv.take(tc_assemble_scratch(R, L0.J, Fz[0], group, ctx->sm_count));
+        void* s_scr = cv.take(tc_synth_scratch(L0.U, L0.Vn, Fz[0] * group));
+        for (int64_t i0 = 0; i0 < n_inst; i0 += group) {
+            const int g = (int)(n_inst - i0 < group ? n_inst - i0 : group);
+            launch_tc_assemble_group(ctx, g, inst + i0, Fz[0], z + i0, P_all, R, R * Fz[0], a_scr);
+            launch_tc_synth_group(ctx, L0.U, L0.Vn, Fz[0], g, P_all, R, Nx, Ny, tw.a, E + i0, s4, s_scr);
+        }
+        return;
+    }
     void* P = cv.take((size_t)R * fz_max * esize(L0.dtype));
     const size_t asm_off = cv.off;
     cv.take(asm_max);
@@ -456,7 +490,12 @@ int32_t scw_sweep_wavelengths(scw_ctx* ctx, int64_t n_inst, const scw_layer* ins
     if (strides) memcpy(s4, strides, sizeof(s4)); else planar_strides(Nx, Ny, s4);
     for (int i = 0; i < 4; ++i)
         if (s4[i] < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_sweep_wavelengths: negative stride");
-    if (int32_t s = need_ws(ctx, sweep_ws(ctx, &inst[0], fz_max, asm_max, Nx, Ny), "scw_sweep_wavelengths")) return s;
+    {
+        const int group = sweep_group_size(ctx, n_inst, inst, Fz);
+        const size_t need = group ? sweep_group_ws(ctx, &inst[0], Fz[0], group, Nx, Ny)
+                                  : sweep_ws(ctx, &inst[0], fz_max, asm_max, Nx, Ny);
+        if (int32_t s = need_ws(ctx, need, "scw_sweep_wavelengths")) return s;
+    }
     Carver cv(ctx->ws);
     run_sweep(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, E, s4, fz_max, asm_max, cv);
     return check_launch(ctx, "scw_sweep_wavelengths");

@@ -93,7 +93,11 @@ void launch_simt_synth(scw_ctx* ctx, int dtype, int U, int Vn, int64_t Fz, const
 
 // ---- scw_tc_assemble.cu: tcgen05 BF16x3 spectral assembly (complex64) ----------------------------
 bool tc_assemble_supported(int dtype, int64_t R, int64_t J, int64_t Fz);
-size_t tc_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int sm_count);
+int tc_assemble_max_group();
+size_t tc_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int n_inst, int sm_count);
+// n_inst <= tc_assemble_max_group() instances with equal U, Vn, J, Fz in three launches; instance i -> P_all + i*inst_stride
+void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
+                              void* P_all, int64_t ldP, int64_t inst_stride, void* scratch);
 // weights (a-1) + P = V W (a-2) + segment reduce; scratch from tc_assemble_scratch
 void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z, void* P, int64_t ldP,
                         void* scratch);
@@ -104,6 +108,11 @@ size_t tc_synth_twiddle_bytes(int U, int Vn, int64_t Nx, int64_t Ny);
 size_t tc_synth_scratch(int U, int Vn, int64_t Fz);
 void launch_tc_synth_twiddles(scw_ctx* ctx, int U, int Vn, double X, double Y, int64_t Nx, const double* x, int64_t Ny,
                               const double* y, void* tw);
+int tc_synth_max_group();
+// n_inst instances with equal Fz, spectra back to back in P_all ([ldP x n_inst*Fz]); scratch = tc_synth_scratch(U, Vn, Fz*n_inst)
+void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const void* P_all, int64_t ldP,
+                           int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
+                           void* scratch);
 void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,
                      const void* tw, void* E, const int64_t strides[4], void* scratch);
 

@@ -39,9 +39,13 @@ constexpr int TA_TMEM_COLS = 512;
 constexpr int TA_SMEM_LIMIT = 226 * 1024;
 constexpr int TA_W_LOADER = TA_CONV_WARPS, TA_MMA_WARP = TA_CONV_WARPS + 1;
 
+constexpr int TA_MAX_INST = 64;            // instances (layers x wavelengths) per grouped launch
+
 struct TaParams {
-    const float2* V;
-    int64_t ldV, R, J;      // R complex rows
+    const float2* V[TA_MAX_INST];
+    int64_t ldV[TA_MAX_INST];
+    int n_inst;
+    int64_t R, J;           // R complex rows, J modes (same for every instance of a group)
     const uint8_t* Wt;      // [n_tile][k_block][hi | lo] K-major UMMA images of [W_r | W_i]
     float* part;            // [slot][Fzt][128] fp32 partial tiles
     int N2, Fzt, n_tiles, m_tiles, kblocks, S, stg_stages;
@@ -51,13 +55,29 @@ struct TaParams {
 // a-1 mode weights (eq. 7, 30) evaluated in fp64, split to bf16 hi/lo, written as the K-major no-swizzle
 // shared-memory image of every (n_tile, k_block) B tile: element (n, kk) at
 //   (kk/8)*(N2*16) + (n/8)*128 + (n%8)*16 + (kk%8)*2,  n < Fzt: Re W[j, i], n >= Fzt: Im W[j, i].
-__global__ void k_tc_weights(int64_t J, int64_t Fz, int Fzt, int n_tiles, int kblocks, double inv_lambda, double z_lo,
-                             double z_hi, const float2* __restrict__ c, const double2* __restrict__ gamma,
-                             const int8_t* __restrict__ dir, const double* __restrict__ z, uint8_t* __restrict__ Wt)
+struct TwGroup {
+    const float2* c[TA_MAX_INST];
+    const double2* gamma[TA_MAX_INST];
+    const int8_t* dir[TA_MAX_INST];
+    const double* z[TA_MAX_INST];
+    double inv_lambda[TA_MAX_INST], z_lo[TA_MAX_INST], z_hi[TA_MAX_INST];
+};
+
+__global__ void k_tc_weights(int n_inst, int64_t J, int64_t Fz, int Fzt, int n_tiles, int kblocks,
+                             const __grid_constant__ TwGroup g_, uint8_t* __restrict__ Wt_all)
 {
     const int64_t Jp = (int64_t)kblocks * TA_BK;
-    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= Jp * n_tiles * Fzt) return;
+    const int64_t per_inst = Jp * n_tiles * Fzt;
+    const int64_t gidx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gidx >= per_inst * n_inst) return;
+    const int inst = (int)(gidx / per_inst);
+    const int64_t idx = gidx - inst * per_inst;
+    const float2* __restrict__ c = g_.c[inst];
+    const double2* __restrict__ gamma = g_.gamma[inst];
+    const int8_t* __restrict__ dir = g_.dir[inst];
+    const double* __restrict__ z = g_.z[inst];
+    const double inv_lambda = g_.inv_lambda[inst], z_lo = g_.z_lo[inst], z_hi = g_.z_hi[inst];
+    uint8_t* Wt = Wt_all + (size_t)inst * n_tiles * kblocks * (size_t)(2 * Fzt) * 256;
     const int64_t i = idx / Jp, j = idx - i * Jp;
     float wr = 0.f, wi = 0.f;
     if (j < J && i < Fz) {
@@ -92,36 +112,42 @@ __global__ void k_tc_weights(int64_t J, int64_t Fz, int Fzt, int n_tiles, int kb
 }
 
 // ---- main kernel -----------------------------------------------------------------------------------
-struct TaPos { int kb, mt; };                      // k-block and m-tile of one iteration (all the V path needs)
+struct TaPos { int kb, mt, nt, inst; };            // iteration order: instance, n-tile, m-tile, k-block (fastest)
 
 __device__ __forceinline__ TaPos ta_pos(const TaParams& p, int64_t it)
 {
     const int64_t tile = it / p.kblocks;
+    const int64_t g = tile / p.m_tiles;
     TaPos q;
     q.kb = (int)(it - tile * p.kblocks);
-    q.mt = (int)(tile % p.m_tiles);
+    q.mt = (int)(tile - g * p.m_tiles);
+    q.inst = (int)(g / p.n_tiles);
+    q.nt = (int)(g - (int64_t)q.inst * p.n_tiles);
     return q;
 }
 __device__ __forceinline__ void ta_next(const TaParams& p, TaPos& q)
 {
     if (++q.kb == p.kblocks) {
         q.kb = 0;
-        if (++q.mt == p.m_tiles) q.mt = 0;
+        if (++q.mt == p.m_tiles) {
+            q.mt = 0;
+            if (++q.nt == p.n_tiles) { q.nt = 0; ++q.inst; }
+        }
     }
 }
 
 // A V column segment (64 complex rows = 512 B) starts at a 16-byte boundary only when (V/8 + k*ldV) is even;
 // otherwise the bulk copy starts 8 bytes early ("shift" = 8).  The shift depends on the parity of k only.
-__device__ __forceinline__ uint32_t ta_shift(const TaParams& p, int k_parity)
+__device__ __forceinline__ uint32_t ta_shift(const float2* V, int64_t ldV, int k_parity)
 {
-    return (uint32_t)(((reinterpret_cast<uintptr_t>(p.V) >> 3) + (uint64_t)(k_parity & (int)(p.ldV & 1))) & 1) * 8u;
+    return (uint32_t)(((reinterpret_cast<uintptr_t>(V) >> 3) + (uint64_t)(k_parity & (int)(ldV & 1))) & 1) * 8u;
 }
 // Copies move whole 16-byte granules: the window [shift + nvalid*8) is rounded UP (reading one neighbouring
 // element of V) unless that would leave the V allocation, in which case it is rounded DOWN and the cut-off
 // last row of that column ("tail") is read directly by its converter thread.
-__device__ __forceinline__ bool ta_tail_cut(const TaParams& p, int64_t k, int64_t row0, int nvalid, uint32_t sh)
+__device__ __forceinline__ bool ta_tail_cut(int64_t ldV, int64_t J, int64_t k, int64_t row0, int nvalid, uint32_t sh)
 {
-    return ((sh + (uint32_t)nvalid * 8u) & 15u) && (k * p.ldV + row0 + nvalid + 1 > p.ldV * p.J);
+    return ((sh + (uint32_t)nvalid * 8u) & 15u) && (k * ldV + row0 + nvalid + 1 > ldV * J);
 }
 
 // Lanes 0-7 of converter warp w copy columns 8w..8w+7 of the iteration at `q` into the staging slot; lane 0
@@ -129,15 +155,17 @@ __device__ __forceinline__ bool ta_tail_cut(const TaParams& p, int64_t k, int64_
 __device__ __forceinline__ void ta_issue_columns(const TaParams& p, const TaPos q, uint8_t* stg, uint64_t* bar,
                                                  int warp, int lane)
 {
+    const float2* V = p.V[q.inst];
+    const int64_t ldV = p.ldV[q.inst];
     const int64_t row0 = (int64_t)q.mt * (TA_BM / 2);
     const int nvalid = (int)min((int64_t)(TA_BM / 2), p.R - row0);
     const int kl = warp * 8 + (lane & 7);
     const int64_t k = (int64_t)q.kb * TA_BK + kl;
-    const uint32_t sh = ta_shift(p, lane & 1);
+    const uint32_t sh = ta_shift(V, ldV, lane & 1);
     uint32_t bytes = 0;
     if (lane < 8 && k < p.J) {
         const uint32_t need = sh + (uint32_t)nvalid * 8u;
-        bytes = ta_tail_cut(p, k, row0, nvalid, sh) ? (need & ~15u) : ((need + 15u) & ~15u);
+        bytes = ta_tail_cut(ldV, p.J, k, row0, nvalid, sh) ? (need & ~15u) : ((need + 15u) & ~15u);
     }
     uint32_t total = bytes;
     total += __shfl_xor_sync(0xffffffffu, total, 1);
@@ -146,7 +174,7 @@ __device__ __forceinline__ void ta_issue_columns(const TaParams& p, const TaPos 
     if (lane == 0) mbar_expect_tx(bar, total);
     __syncwarp();
     if (bytes)
-        bulk_g2s(stg + kl * TA_COL_PITCH, reinterpret_cast<const uint8_t*>(p.V + k * p.ldV + row0) - sh, bytes, bar);
+        bulk_g2s(stg + kl * TA_COL_PITCH, reinterpret_cast<const uint8_t*>(V + k * ldV + row0) - sh, bytes, bar);
 }
 
 __device__ __forceinline__ void ta_split_store(uint8_t* dst, const float2 (&v)[8])
@@ -171,14 +199,16 @@ __device__ __forceinline__ void ta_split_store(uint8_t* dst, const float2 (&v)[8
 __device__ __forceinline__ void ta_convert(const TaParams& p, const uint8_t* stg, uint8_t* a_hi, const TaPos q,
                                            int warp, int lane)
 {
+    const float2* V = p.V[q.inst];
+    const int64_t ldV = p.ldV[q.inst];
     const int64_t row0 = (int64_t)q.mt * (TA_BM / 2);
     const int nvalid = (int)min((int64_t)(TA_BM / 2), p.R - row0);
-    const uint32_t sh0 = ta_shift(p, 0), sh1 = ta_shift(p, 1);
+    const uint32_t sh0 = ta_shift(V, ldV, 0), sh1 = ta_shift(V, ldV, 1);
     const uint8_t* src0 = stg + warp * 8 * TA_COL_PITCH + lane * 8 + sh0;      // even columns
     const uint8_t* src1 = stg + warp * 8 * TA_COL_PITCH + lane * 8 + sh1;      // odd columns
     uint8_t* dst = a_hi + warp * TA_A_LBO + (lane >> 2) * TA_A_SBO + (lane & 3) * 32;
     const bool slow = nvalid < TA_BM / 2 || (int64_t)(q.kb + 1) * TA_BK > p.J ||
-                      (q.kb == p.kblocks - 1 && row0 + nvalid == p.ldV);
+                      (q.kb == p.kblocks - 1 && row0 + nvalid == ldV);
     if (!slow) {
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
@@ -198,8 +228,8 @@ __device__ __forceinline__ void ta_convert(const TaParams& p, const uint8_t* stg
                 const int64_t k = (int64_t)q.kb * TA_BK + warp * 8 + kk;
                 float2 t = *reinterpret_cast<const float2*>(((kk & 1) ? src1 : src0) + kk * TA_COL_PITCH + h * 256);
                 const bool valid = rp < nvalid && k < p.J;
-                if (valid && rp == nvalid - 1 && ta_tail_cut(p, k, row0, nvalid, (kk & 1) ? sh1 : sh0))
-                    t = __ldg(p.V + k * p.ldV + row0 + rp);
+                if (valid && rp == nvalid - 1 && ta_tail_cut(ldV, p.J, k, row0, nvalid, (kk & 1) ? sh1 : sh0))
+                    t = __ldg(V + k * ldV + row0 + rp);
                 v[kk] = valid ? t : make_float2(0.f, 0.f);
             }
             ta_split_store(dst + h * 8 * TA_A_SBO, v);
@@ -207,7 +237,7 @@ __device__ __forceinline__ void ta_convert(const TaParams& p, const uint8_t* stg
     }
 }
 
-__global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const TaParams p)
+__global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_constant__ TaParams p)
 {
     extern __shared__ __align__(1024) uint8_t smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -241,7 +271,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const TaParams p)
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
-    const int64_t T = (int64_t)p.n_tiles * p.m_tiles * p.kblocks;
+    const int64_t T = (int64_t)p.n_inst * p.n_tiles * p.m_tiles * p.kblocks;
     const int64_t it0 = (int64_t)blockIdx.x * T / gridDim.x;
     const int64_t it1 = (int64_t)(blockIdx.x + 1) * T / gridDim.x;
 
@@ -375,13 +405,15 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const TaParams p)
 }
 
 // Sum the segments of every tile in CTA order: P[mt*64 + r, nt*Fzt + n] = sum_seg part[seg][n][2r..2r+1].
-__global__ void k_tc_reduce(int64_t R, int64_t Fz, int Fzt, int m_tiles, int kblocks, int64_t T, int G, int S,
-                            const float* __restrict__ part, float2* __restrict__ P, int64_t ldP)
+__global__ void k_tc_reduce(int64_t R, int64_t Fz, int Fzt, int n_tiles, int m_tiles, int kblocks, int64_t T, int G, int S,
+                            const float* __restrict__ part, float2* __restrict__ P_all, int64_t ldP, int64_t inst_stride)
 {
-    const int tile = blockIdx.x;
+    const int tile = blockIdx.x;                                 // global tile id: (inst, n_tile, m_tile)
     const int n = blockIdx.y * blockDim.y + threadIdx.y;
     const int r = threadIdx.x;                                   // complex row in tile, 0..63
-    const int nt = tile / m_tiles, mt = tile - nt * m_tiles;
+    const int gnt = tile / m_tiles, mt = tile - gnt * m_tiles;
+    const int inst = gnt / n_tiles, nt = gnt - inst * n_tiles;
+    float2* __restrict__ P = P_all + (int64_t)inst * inst_stride;
     const int64_t row = (int64_t)mt * 64 + r, col = (int64_t)nt * Fzt + n;
     if (n >= Fzt || row >= R || col >= Fz) return;
     const int64_t a = (int64_t)tile * kblocks, b = a + kblocks;
@@ -403,10 +435,10 @@ __global__ void k_tc_reduce(int64_t R, int64_t Fz, int Fzt, int m_tiles, int kbl
 struct TaPlan {
     int Fzt, N2, n_tiles, m_tiles, kblocks, G, S, stg_stages;
     int64_t T;
-    size_t wt_bytes, part_bytes, smem_bytes;
+    size_t wt_bytes, part_bytes, smem_bytes;      // wt_bytes: W~ images of ONE instance
 };
 
-static TaPlan ta_plan(int64_t R, int64_t J, int64_t Fz, int sm_count)
+static TaPlan ta_plan(int64_t R, int64_t J, int64_t Fz, int n_inst, int sm_count)
 {
     TaPlan pl;
     int64_t fzt = (Fz + 7) / 8 * 8;
@@ -416,7 +448,7 @@ static TaPlan ta_plan(int64_t R, int64_t J, int64_t Fz, int sm_count)
     pl.n_tiles = (int)((Fz + pl.Fzt - 1) / pl.Fzt);
     pl.m_tiles = (int)((2 * R + TA_BM - 1) / TA_BM);
     pl.kblocks = (int)((J + TA_BK - 1) / TA_BK);
-    pl.T = (int64_t)pl.n_tiles * pl.m_tiles * pl.kblocks;
+    pl.T = (int64_t)n_inst * pl.n_tiles * pl.m_tiles * pl.kblocks;
     pl.G = (int)(pl.T < sm_count ? pl.T : sm_count);
     pl.S = 1;
     for (int c = 0; c < pl.G; ++c) {
@@ -430,7 +462,7 @@ static TaPlan ta_plan(int64_t R, int64_t J, int64_t Fz, int sm_count)
     pl.stg_stages = (TA_SMEM_LIMIT - 256 - mma_bytes) / TA_STG_BYTES;
     if (pl.stg_stages > 4) pl.stg_stages = 4;
     pl.smem_bytes = (size_t)mma_bytes + (size_t)pl.stg_stages * TA_STG_BYTES + 256;
-    pl.wt_bytes = align_up((size_t)pl.n_tiles * pl.kblocks * pl.N2 * 256);
+    pl.wt_bytes = (size_t)pl.n_tiles * pl.kblocks * pl.N2 * 256;
     pl.part_bytes = align_up((size_t)pl.G * pl.S * pl.Fzt * TA_BM * sizeof(float));
     return pl;
 }
@@ -440,31 +472,47 @@ bool tc_assemble_supported(int dtype, int64_t R, int64_t J, int64_t Fz)
     return dtype == SCW_C64 && R >= 1 && J >= 1 && Fz >= 1;
 }
 
-size_t tc_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int sm_count)
+int tc_assemble_max_group() { return TA_MAX_INST; }
+
+size_t tc_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int n_inst, int sm_count)
 {
-    const TaPlan pl = ta_plan(R, J, Fz, sm_count);
-    return pl.wt_bytes + pl.part_bytes;
+    const TaPlan pl = ta_plan(R, J, Fz, n_inst, sm_count);
+    return align_up(pl.wt_bytes * n_inst) + pl.part_bytes;
 }
 
-void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z, void* P, int64_t ldP,
-                        void* scratch)
+// A group of n_inst <= TA_MAX_INST instances with the same U, Vn, J and Fz in three launches:
+// weights (a-1), P = V W over the concatenated iteration space (a-2), segment reduce.
+// Instance i writes P_all + i * inst_stride (column-major [ldP x Fz]).
+void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
+                              void* P_all, int64_t ldP, int64_t inst_stride, void* scratch)
 {
-    const int64_t R = 3LL * L->U * L->Vn;
-    const TaPlan pl = ta_plan(R, L->J, Fz, ctx->sm_count);
+    const scw_layer& L0 = inst[0];
+    const int64_t R = 3LL * L0.U * L0.Vn;
+    const TaPlan pl = ta_plan(R, L0.J, Fz, n_inst, ctx->sm_count);
     uint8_t* Wt = static_cast<uint8_t*>(scratch);
-    float* part = reinterpret_cast<float*>(Wt + pl.wt_bytes);
+    float* part = reinterpret_cast<float*>(Wt + align_up(pl.wt_bytes * n_inst));
+    TwGroup g;
+    TaParams p;
+    for (int i = 0; i < n_inst; ++i) {
+        g.c[i] = (const float2*)inst[i].c;
+        g.gamma[i] = (const double2*)inst[i].gamma;
+        g.dir[i] = inst[i].dir;
+        g.z[i] = z[i];
+        g.inv_lambda[i] = 1.0 / inst[i].lambda;
+        g.z_lo[i] = inst[i].z_lo;
+        g.z_hi[i] = inst[i].z_hi;
+        p.V[i] = (const float2*)inst[i].V;
+        p.ldV[i] = inst[i].ldV;
+    }
     {
         KernelScope ks(ctx, KC_WEIGHTS);
-        const int64_t n = (int64_t)pl.kblocks * TA_BK * pl.n_tiles * pl.Fzt;
-        k_tc_weights<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(
-            L->J, Fz, pl.Fzt, pl.n_tiles, pl.kblocks, 1.0 / L->lambda, L->z_lo, L->z_hi, (const float2*)L->c,
-            (const double2*)L->gamma, L->dir, z, Wt);
+        const int64_t n = (int64_t)pl.kblocks * TA_BK * pl.n_tiles * pl.Fzt * n_inst;
+        k_tc_weights<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(n_inst, L0.J, Fz, pl.Fzt, pl.n_tiles,
+                                                                           pl.kblocks, g, Wt);
     }
-    TaParams p;
-    p.V = (const float2*)L->V;
-    p.ldV = L->ldV;
+    p.n_inst = n_inst;
     p.R = R;
-    p.J = L->J;
+    p.J = L0.J;
     p.Wt = Wt;
     p.part = part;
     p.N2 = pl.N2;
@@ -482,10 +530,16 @@ void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const doub
     {
         KernelScope ks(ctx, KC_REDUCE);
         dim3 block(64, 4);
-        dim3 grid((unsigned)(pl.n_tiles * pl.m_tiles), (unsigned)((pl.Fzt + 3) / 4));
-        k_tc_reduce<<<grid, block, 0, ctx->stream>>>(R, Fz, pl.Fzt, pl.m_tiles, pl.kblocks, pl.T, pl.G, pl.S, part,
-                                                     (float2*)P, ldP);
+        dim3 grid((unsigned)(n_inst * pl.n_tiles * pl.m_tiles), (unsigned)((pl.Fzt + 3) / 4));
+        k_tc_reduce<<<grid, block, 0, ctx->stream>>>(R, Fz, pl.Fzt, pl.n_tiles, pl.m_tiles, pl.kblocks, pl.T, pl.G, pl.S,
+                                                     part, (float2*)P_all, ldP, inst_stride);
     }
+}
+
+void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z, void* P, int64_t ldP,
+                        void* scratch)
+{
+    launch_tc_assemble_group(ctx, 1, L, Fz, &z, P, ldP, 0, scratch);
 }
 
 }  // namespace scw

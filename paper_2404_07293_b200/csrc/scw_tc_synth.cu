@@ -21,19 +21,28 @@ using namespace tc;
 
 constexpr int TS_TILE = 128;               // output tile edge (x and y)
 constexpr int TS_KMAX = 80;                // max padded K (= 2U, 2V rounded up to 16)
-constexpr int TS_THREADS = 10 * 32;        // loader, MMA, 4 converter warps, 4 epilogue warps
+constexpr int TS_THREADS = 18 * 32;        // loader, MMA, 8 converter warps, 8 epilogue warps
 constexpr int TS_TMEM_COLS = 512;
 constexpr int TS_D2_COL = 0;               // D2[h] at columns h*128
 constexpr int TS_D1_COL = 256;             // D1 at columns 256..256+N1
+constexpr int TS_MAX_INST = 64;            // instances per grouped launch
+
+#ifdef SCW_TS_DEBUG
+__device__ long long g_ts_dbg[4096];
+#define TS_MARK(slot) do { if (blockIdx.x == 0) g_ts_dbg[(slot)] = clock64(); } while (0)
+#else
+#define TS_MARK(slot) do { } while (0)
+#endif
 
 struct TsParams {
     const uint8_t* A1;     // [ty][hi|lo] images of (Fy_r, Fy_i): 128 rows x K1p, K-major, LBO = 2048, SBO = 128
     const uint8_t* A2;     // [tx][hi|lo] images of (Fx_r, Fx_i): 128 rows x K2p
     const uint8_t* B1;     // [plane][hi|lo] images: N1 rows x K1p, LBO = N1*16, SBO = 128
-    float2* E;
+    float2* E[TS_MAX_INST];   // output of every instance of the group
     int64_t s_comp, s_z, s_y, s_x;
     int64_t Nx, Ny;
-    int planes;            // Fz * 3
+    int planes;            // n_inst * Fz * 3 (global plane id = inst * planes_per_inst + n*3 + comp)
+    int planes_per_inst;
     int K1p, K2p;          // padded 2V, 2U  (N1 == K2p)
     int tiles_x, tiles_y, pair0, npairs;   // this launch covers tile pairs [pair0, pair0 + npairs)
 };
@@ -122,7 +131,7 @@ __device__ __forceinline__ void ts_mma3(uint32_t d_tmem, uint32_t a_hi, uint32_t
     }
 }
 
-__global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const TsParams p)
+__global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constant__ TsParams p)
 {
     extern __shared__ __align__(1024) uint8_t smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -150,13 +159,13 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const TsParams p)
         for (int s = 0; s < 2; ++s) {
             mbar_init(&b1_full[s], 1);
             mbar_init(&b1_empty[s], 1);
-            mbar_init(&b2_full[s], 2);
+            mbar_init(&b2_full[s], 4);
             mbar_init(&b2_empty[s], 1);
             mbar_init(&d2_full[s], 1);
-            mbar_init(&d2_empty[s], 4);
+            mbar_init(&d2_empty[s], 8);
         }
         mbar_init(d1_full, 1);
-        mbar_init(d1_empty, 4);
+        mbar_init(d1_empty, 8);
         mbar_fence_init();
     }
     if (warp == 1) tmem_alloc(tmem_slot, TS_TMEM_COLS);
@@ -199,19 +208,24 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const TsParams p)
                 mbar_wait(&b1_full[s], (n >> 1) & 1);
                 if (n > 0) mbar_wait(d1_empty, (n - 1) & 1);
                 tc_fence_after();
+                TS_MARK(n * 32 + 0);
                 ts_mma3(d1, a1, a1 + a1_img, 2048, b1 + s * 2 * b1_img, b1 + s * 2 * b1_img + b1_img, (uint32_t)N1 * 16, K1p,
                         idesc1);
                 umma_commit(d1_full);
                 umma_commit(&b1_empty[s]);
+                TS_MARK(n * 32 + 1);
             };
             auto issue_gemm2 = [&](int n, int h) {
                 mbar_wait(&b2_full[h], n & 1);
+                TS_MARK(n * 32 + 2 + 4 * h);
                 mbar_wait(&d2_empty[h], (n & 1) ^ 1);
                 tc_fence_after();
+                TS_MARK(n * 32 + 3 + 4 * h);
                 ts_mma3(tmem_base + TS_D2_COL + h * TS_TILE, a2, a2 + a2_img, 2048, b2 + h * 2 * b2_img,
                         b2 + h * 2 * b2_img + b2_img, 2048, K2p, idesc2);
                 umma_commit(&d2_full[h]);
                 umma_commit(&b2_empty[h]);
+                TS_MARK(n * 32 + 4 + 4 * h);
             };
             issue_gemm1(0);
             for (int n = 0; n < n_items; ++n) {
@@ -220,74 +234,99 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const TsParams p)
                 issue_gemm2(n, 1);
             }
         }
-    } else if (warp < 6) {
-        // ===== converters: D1 row y (TMEM) -> B2 rows (y,Re), (y,Im) as bf16 hi/lo =====
+    } else if (warp < 10) {
+        // ===== converters: D1 row y (TMEM) -> B2 rows (y,Re), (y,Im) as bf16 hi/lo.  Two warps per TMEM lane
+        // quarter: warp kg = 0/1 takes the even/odd 8-column chunks of the row. =====
         const int q = warp & 3;                      // TMEM lane quarter: y = 32q + lane
+        const int kg = (warp - 2) >> 2;              // chunk parity handled by this warp
         const int h = q >> 1;                        // which half of the tile this y belongs to
         const int yy = 32 * (q & 1) + lane;          // y within the half
         uint8_t* row = sB2 + (size_t)h * 2 * b2_img + yy * 32;
         const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + TS_D1_COL;
+        const int nchunks = K2p / 8;                 // <= 10
         for (int n = 0; n < n_items; ++n) {
             mbar_wait(d1_full, n & 1);
-            mbar_wait(&b2_empty[h], (n & 1) ^ 1);
             tc_fence_after();
-            for (int c = 0; c < K2p / 8; ++c) {
-                float t[8];
-                tmem_ld8(taddr + 8 * c, t);          // (Tr0, Ti0, Tr1, Ti1, Tr2, Ti2, Tr3, Ti3)
-                tmem_ld_wait();
-                uint4 re_hi, re_lo, im_hi, im_lo;
-                split_bf16x2(t[0], -t[1], re_hi.x, re_lo.x);
-                split_bf16x2(t[2], -t[3], re_hi.y, re_lo.y);
-                split_bf16x2(t[4], -t[5], re_hi.z, re_lo.z);
-                split_bf16x2(t[6], -t[7], re_hi.w, re_lo.w);
-                split_bf16x2(t[1], t[0], im_hi.x, im_lo.x);
-                split_bf16x2(t[3], t[2], im_hi.y, im_lo.y);
-                split_bf16x2(t[5], t[4], im_hi.z, im_lo.z);
-                split_bf16x2(t[7], t[6], im_hi.w, im_lo.w);
-                uint8_t* dst = row + (size_t)c * 2048;
-                *reinterpret_cast<uint4*>(dst) = re_hi;
-                *reinterpret_cast<uint4*>(dst + 16) = im_hi;
-                *reinterpret_cast<uint4*>(dst + b2_img) = re_lo;
-                *reinterpret_cast<uint4*>(dst + b2_img + 16) = im_lo;
-            }
+            if (warp == 4 && lane == 0) TS_MARK(n * 32 + 10);
+            uint32_t t[5][8];
+#pragma unroll
+            for (int i = 0; i < 5; ++i)
+                if (2 * i + kg < nchunks) tmem_ld8_raw(taddr + 8 * (2 * i + kg), t[i]);
+            tmem_ld_wait();
             tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(d1_empty);    // D1 may be overwritten by the next plane's GEMM1
+            if (warp == 4 && lane == 0) TS_MARK(n * 32 + 11);
+            mbar_wait(&b2_empty[h], (n & 1) ^ 1);
+            if (warp == 4 && lane == 0) TS_MARK(n * 32 + 12);
+#pragma unroll
+            for (int i = 0; i < 5; ++i) {
+                const int c = 2 * i + kg;
+                if (c < nchunks) {
+                    float f[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(t[i][e]);   // (Tr0, Ti0, ..., Tr3, Ti3)
+                    uint4 re_hi, re_lo, im_hi, im_lo;
+                    split_bf16x2(f[0], -f[1], re_hi.x, re_lo.x);
+                    split_bf16x2(f[2], -f[3], re_hi.y, re_lo.y);
+                    split_bf16x2(f[4], -f[5], re_hi.z, re_lo.z);
+                    split_bf16x2(f[6], -f[7], re_hi.w, re_lo.w);
+                    split_bf16x2(f[1], f[0], im_hi.x, im_lo.x);
+                    split_bf16x2(f[3], f[2], im_hi.y, im_lo.y);
+                    split_bf16x2(f[5], f[4], im_hi.z, im_lo.z);
+                    split_bf16x2(f[7], f[6], im_hi.w, im_lo.w);
+                    uint8_t* dst = row + (size_t)c * 2048;
+                    *reinterpret_cast<uint4*>(dst) = re_hi;
+                    *reinterpret_cast<uint4*>(dst + 16) = im_hi;
+                    *reinterpret_cast<uint4*>(dst + b2_img) = re_lo;
+                    *reinterpret_cast<uint4*>(dst + b2_img + 16) = im_lo;
+                }
+            }
+            if (warp == 4 && lane == 0) TS_MARK(n * 32 + 13);
             fence_proxy_async();
             __syncwarp();
-            if (lane == 0) {
-                mbar_arrive(d1_empty);
-                mbar_arrive(&b2_full[h]);
-            }
+            if (lane == 0) mbar_arrive(&b2_full[h]);
+            if (warp == 4 && lane == 0) TS_MARK(n * 32 + 14);
         }
     } else {
-        // ===== epilogue: D2 (lane = x, columns = (y, Re/Im)) -> E =====
+        // ===== epilogue: D2 (lane = x, columns = (y, Re/Im)) -> E.  Two warps per lane quarter, 32 y each. =====
         const int q = warp & 3;
+        const int cg = (warp - 10) >> 2;             // which 32-y group of the half
         const int64_t x = (int64_t)tx * TS_TILE + 32 * q + lane;
         const bool x_ok = x < p.Nx;
         for (int n = 0; n < n_items; ++n) {
-            const int plane = first_plane + n * per_pair;
+            const int gplane = first_plane + n * per_pair;
+            const int inst = gplane / p.planes_per_inst;
+            const int plane = gplane - inst * p.planes_per_inst;
             const int64_t zi = plane / 3;
             const int comp = plane - (int)zi * 3;
-            float2* out = p.E + comp * p.s_comp + zi * p.s_z + x * p.s_x;
+            float2* const Einst = p.E[inst];
 #pragma unroll 1
             for (int h = 0; h < 2; ++h) {
                 mbar_wait(&d2_full[h], n & 1);
                 tc_fence_after();
-                const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + TS_D2_COL + h * TS_TILE;
-                const int64_t y0 = (int64_t)ty * TS_TILE + 64 * h;
-#pragma unroll 2
-                for (int c = 0; c < 8; ++c) {
-                    float v[16];
-                    tmem_ld16(taddr + 16 * c, v);
-                    tmem_ld_wait();
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) {
-                        const int64_t y = y0 + 8 * c + e;
-                        if (x_ok && y < p.Ny) out[y * p.s_y] = make_float2(v[2 * e], v[2 * e + 1]);
-                    }
-                }
+                if (warp == 12 && lane == 0) TS_MARK(n * 32 + 16 + 4 * h);
+                const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + TS_D2_COL + h * TS_TILE + 64 * cg;
+                uint32_t v[2][32];
+                tmem_ld32_raw(taddr, v[0]);
+                tmem_ld32_raw(taddr + 32, v[1]);
+                tmem_ld_wait();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&d2_empty[h]);
+                if (lane == 0) mbar_arrive(&d2_empty[h]);          // D2[h] is in registers now
+                if (warp == 12 && lane == 0) TS_MARK(n * 32 + 17 + 4 * h);
+                const int64_t y0 = (int64_t)ty * TS_TILE + 64 * h + 32 * cg;
+                const int ny = (int)min((int64_t)32, p.Ny - y0);   // may be <= 0
+                float2* out = Einst + comp * p.s_comp + zi * p.s_z + x * p.s_x + y0 * p.s_y;
+                if (x_ok) {
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) {
+                        if (e < ny)
+                            out[e * p.s_y] = make_float2(__uint_as_float(v[e >> 4][(2 * e) & 31]),
+                                                         __uint_as_float(v[e >> 4][(2 * e + 1) & 31]));
+                    }
+                }
+                if (warp == 12 && lane == 0) TS_MARK(n * 32 + 18 + 4 * h);
             }
         }
     }
@@ -348,23 +387,32 @@ void launch_tc_synth_twiddles(scw_ctx* ctx, int U, int Vn, double X, double Y, i
     }
 }
 
-void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,
-                     const void* tw, void* E, const int64_t strides[4], void* scratch)
+#ifdef SCW_TS_DEBUG
+extern "C" void scw_debug_ts_read(long long* out) { cudaMemcpyFromSymbol(out, g_ts_dbg, sizeof(long long) * 4096); }
+#endif
+
+int tc_synth_max_group() { return TS_MAX_INST; }
+
+// n_inst <= TS_MAX_INST instances with the same Fz whose spectra are stored back to back
+// (P_all is one column-major [ldP x n_inst*Fz] matrix): one image pre-kernel + one synthesis launch.
+void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const void* P_all, int64_t ldP,
+                           int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
+                           void* scratch)
 {
-    const TsPlan pl = ts_plan(U, Vn, Fz, Nx, Ny);
-    const int planes = (int)(Fz * 3);
+    const TsPlan pl = ts_plan(U, Vn, Fz * n_inst, Nx, Ny);
+    const int planes = (int)(Fz * 3 * n_inst);
     uint8_t* B1 = static_cast<uint8_t*>(scratch);
     {
         KernelScope ks(ctx, KC_SYNTH_A);
         const int64_t n = (int64_t)planes * pl.K2p * (pl.K1p / 2);
         k_tc_synth_pimage<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(U, Vn, pl.K1p, pl.K2p, planes,
-                                                                                (const float2*)P, ldP, B1);
+                                                                                (const float2*)P_all, ldP, B1);
     }
     TsParams p;
     p.A1 = static_cast<const uint8_t*>(tw);
     p.A2 = p.A1 + pl.a1_bytes;
     p.B1 = B1;
-    p.E = static_cast<float2*>(E);
+    for (int i = 0; i < n_inst; ++i) p.E[i] = static_cast<float2*>(E[i]);
     p.s_comp = strides[0];
     p.s_z = strides[1];
     p.s_y = strides[2];
@@ -372,6 +420,7 @@ void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int
     p.Nx = Nx;
     p.Ny = Ny;
     p.planes = planes;
+    p.planes_per_inst = (int)(Fz * 3);
     p.K1p = pl.K1p;
     p.K2p = pl.K2p;
     p.tiles_x = pl.tiles_x;
@@ -386,6 +435,12 @@ void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int
         KernelScope ks(ctx, KC_SYNTH_TC);
         k_tc_synth<<<p.npairs * per_pair, TS_THREADS, pl.smem_bytes, ctx->stream>>>(p);
     }
+}
+
+void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,
+                     const void* tw, void* E, const int64_t strides[4], void* scratch)
+{
+    launch_tc_synth_group(ctx, U, Vn, Fz, 1, P, ldP, Nx, Ny, tw, &E, strides, scratch);
 }
 
 }  // namespace scw

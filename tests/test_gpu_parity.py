@@ -212,7 +212,10 @@ def test_config4_sweep_full_size(scw, ctx):
         assert rel_err(Es[i].cpu().numpy(), ref_b) <= 2e-4
         one = scw.scw_sweep_wavelengths(ctx, [Ls[i]], [dz[i]], dev(x), dev(y))[0]
         torch.cuda.synchronize()
-        assert rel_err(one.cpu().numpy(), Es[i].cpu().numpy().astype(np.complex128)) <= 1e-6
+        # batched and single-instance calls cut the mode sum into different stream-K segments: they agree to
+        # the BF16x3 rounding level (each is ~1e-5 from the oracle), not bit for bit
+        err_one = rel_err(one.cpu().numpy(), Es[i].cpu().numpy().astype(np.complex128))
+        assert err_one <= 5e-5, err_one
     for i in range(0, 64, 7):
         idx = si.sample_subset(cfg, 16 * 256 * 256, 32, lam_index=i // 2, layer=i % 2)
         iz, iy, ix = np.unravel_index(idx, (16, 256, 256))
@@ -235,4 +238,5 @@ def test_sweep_host_buffers_match_device_call(scw, ctx):
     torch.cuda.synchronize()
     assert down == sum(e.numel() * 8 for e in Eh) and up > sum(d["V"].nbytes for d in insts)
     for a, b in zip(Ed, Eh):
-        assert torch.equal(a.cpu(), b)
+        err = float((a.cpu() - b).abs().max() / b.abs().max())
+        assert err <= 5e-5, err          # batched device call vs per-instance host call: BF16x3 rounding level
