@@ -13,11 +13,11 @@
 // contiguous spans, one per persistent CTA (one CTA per SM); every (CTA, tile) segment writes an fp32
 // partial tile, k_tc_reduce sums the segments of each tile in a fixed order (deterministic).
 //
-// Warp roles (448 threads): warps 0-7 stream V from HBM with bulk async copies (cp.async.bulk, one per
-// 512-byte column segment) into an fp32 staging ring that keeps 64-128 KB in flight per SM, split the
-// staged fp32 into bf16 hi/lo and store K-major UMMA tiles; warp 8 fetches the pre-formatted W tiles
-// with bulk async copies; warp 9 issues tcgen05.mma; warps 10-13 drain TMEM (tcgen05.ld), combine
-// lanes with one shuffle per element and store the partial tile.
+// Warp roles (704 threads): warps 8-15 stream V from HBM with bulk async copies (cp.async.bulk, one per
+// 512-byte column segment) into an fp32 staging ring that keeps 64-128 KB in flight per SM; warps 0-7
+// split the staged fp32 into bf16 hi/lo and store K-major UMMA tiles; warp 16 fetches the pre-formatted
+// W tiles with bulk async copies; warp 17 issues tcgen05.mma; warps 18-21 drain TMEM (tcgen05.ld),
+// combine lanes with one shuffle per element and store the partial tile.
 #include "scw_internal.h"
 #include "scw_tc_common.cuh"
 
@@ -27,19 +27,32 @@ using namespace tc;
 
 constexpr int TA_BM = 128;                 // real rows per tile (= 64 complex rows)
 constexpr int TA_BK = 64;                  // modes per pipeline stage
-constexpr int TA_CONV_WARPS = 8;
-constexpr int TA_THREADS = (TA_CONV_WARPS + 2 + 4) * 32;
-constexpr int TA_A_SBO = 144;              // bytes between 8-row groups (144 instead of 128: conflict-free stores)
-constexpr int TA_A_LBO = 16 * TA_A_SBO;    // bytes between 8-mode chunks
-constexpr int TA_A_TILE = 8 * TA_A_LBO;    // one bf16 tile (hi or lo): 18432 bytes
+constexpr int TA_CONV_WARPS = 8;           // warp w converts k-chunk w (8 modes) of every stage
+constexpr int TA_LOAD_WARPS = 8;           // V loader warps: 8 column copies each per stage
+constexpr int TA_THREADS = (TA_CONV_WARPS + TA_LOAD_WARPS + 2 + 4) * 32;
+constexpr int TA_D_COLS = 256;             // TMEM: two accumulators of N2 <= 128 columns
+constexpr int TA_A_COL = TA_D_COLS;        // TMEM: A operand, per MMA stage 32 columns hi + 32 columns lo (bf16 pairs)
 constexpr int TA_COL_PITCH = 528;          // fp32 staging: 512 B of a V column segment + 16 B alignment slack
 constexpr int TA_STG_BYTES = TA_BK * TA_COL_PITCH;
 constexpr int TA_MMA_STAGES = 2;
 constexpr int TA_TMEM_COLS = 512;
 constexpr int TA_SMEM_LIMIT = 226 * 1024;
-constexpr int TA_W_LOADER = TA_CONV_WARPS, TA_MMA_WARP = TA_CONV_WARPS + 1;
+constexpr int TA_V_LOADER = TA_CONV_WARPS, TA_W_LOADER = TA_V_LOADER + TA_LOAD_WARPS, TA_MMA_WARP = TA_W_LOADER + 1;
 
 constexpr int TA_MAX_INST = 64;            // instances (layers x wavelengths) per grouped launch
+
+#ifdef SCW_TS_DEBUG
+__device__ long long g_ta_dbg[8192];
+#define TA_MARK(slot) do { if (blockIdx.x == 0 && (slot) < 8192) g_ta_dbg[(slot)] = clock64(); } while (0)
+__device__ long long g_ta_blk[4 * 256];
+__device__ __forceinline__ long long ta_gtime() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define TA_BLK(i) do { if (threadIdx.x == 0) { g_ta_blk[blockIdx.x * 4 + (i)] = clock64(); g_ta_blk[blockIdx.x * 4 + (i) + 2] = ta_gtime(); } } while (0)
+extern "C" void scw_debug_ta_read(long long* out) { cudaMemcpyFromSymbol(out, g_ta_dbg, sizeof(long long) * 8192); }
+extern "C" void scw_debug_ta_blk(long long* out) { cudaMemcpyFromSymbol(out, g_ta_blk, sizeof(long long) * 1024); }
+#else
+#define TA_MARK(slot) do { } while (0)
+#define TA_BLK(i) do { } while (0)
+#endif
 
 struct TaParams {
     const float2* V[TA_MAX_INST];
@@ -150,16 +163,17 @@ __device__ __forceinline__ bool ta_tail_cut(int64_t ldV, int64_t J, int64_t k, i
     return ((sh + (uint32_t)nvalid * 8u) & 15u) && (k * ldV + row0 + nvalid + 1 > ldV * J);
 }
 
-// Lanes 0-7 of converter warp w copy columns 8w..8w+7 of the iteration at `q` into the staging slot; lane 0
-// posts the warp's byte count on the slot's barrier (one of TA_CONV_WARPS arrivals).
-__device__ __forceinline__ void ta_issue_columns(const TaParams& p, const TaPos q, uint8_t* stg, uint64_t* bar,
-                                                 int warp, int lane)
+// V-loader warp w copies column segments 8w..8w+7 of the iteration at `q` into a staging slot (lanes 0-7, one
+// bulk copy each; a single warp issues only ~1 copy per 80 clk, eight warps together reach ~1 per 16 clk);
+// lane 0 posts the warp's byte count on the slot's barrier (one of TA_LOAD_WARPS arrivals).
+__device__ __forceinline__ void ta_issue_columns(const TaParams& p, const TaPos q, uint8_t* stg, uint64_t* bar, int w,
+                                                 int lane)
 {
     const float2* V = p.V[q.inst];
     const int64_t ldV = p.ldV[q.inst];
     const int64_t row0 = (int64_t)q.mt * (TA_BM / 2);
     const int nvalid = (int)min((int64_t)(TA_BM / 2), p.R - row0);
-    const int kl = warp * 8 + (lane & 7);
+    const int kl = w * 8 + (lane & 7);
     const int64_t k = (int64_t)q.kb * TA_BK + kl;
     const uint32_t sh = ta_shift(V, ldV, lane & 1);
     uint32_t bytes = 0;
@@ -177,26 +191,12 @@ __device__ __forceinline__ void ta_issue_columns(const TaParams& p, const TaPos 
         bulk_g2s(stg + kl * TA_COL_PITCH, reinterpret_cast<const uint8_t*>(V + k * ldV + row0) - sh, bytes, bar);
 }
 
-__device__ __forceinline__ void ta_split_store(uint8_t* dst, const float2 (&v)[8])
-{
-    uint4 eh, el, oh, ol;
-    split_bf16x2(v[0].x, v[1].x, eh.x, el.x);
-    split_bf16x2(v[2].x, v[3].x, eh.y, el.y);
-    split_bf16x2(v[4].x, v[5].x, eh.z, el.z);
-    split_bf16x2(v[6].x, v[7].x, eh.w, el.w);
-    split_bf16x2(v[0].y, v[1].y, oh.x, ol.x);
-    split_bf16x2(v[2].y, v[3].y, oh.y, ol.y);
-    split_bf16x2(v[4].y, v[5].y, oh.z, ol.z);
-    split_bf16x2(v[6].y, v[7].y, oh.w, ol.w);
-    *reinterpret_cast<uint4*>(dst) = eh;                       // even real row (Re)
-    *reinterpret_cast<uint4*>(dst + 16) = oh;                  // odd real row (Im)
-    *reinterpret_cast<uint4*>(dst + TA_A_TILE) = el;
-    *reinterpret_cast<uint4*>(dst + TA_A_TILE + 16) = ol;
-}
-
-// Converter warp w: staging columns 8w..8w+7 (fp32, [k][row]) -> bf16 hi/lo K-major tiles, k-chunk w.
-// lane l handles complex rows l and l+32 (real rows 2l, 2l+1 and 2l+64, 2l+65).
-__device__ __forceinline__ void ta_convert(const TaParams& p, const uint8_t* stg, uint8_t* a_hi, const TaPos q,
+// Converter warp w: TMEM lane quarter q = w & 3 (real rows 32q..32q+31 of the tile), mode half kh = w >> 2
+// (modes 32kh..32kh+31 of the stage).  A thread reads its row's 32 fp32 values from the staging slot ([k][row],
+// conflict-free 4-byte loads), splits them to bf16 hi/lo pairs and writes them to the A operand block in TMEM
+// (lane = row, 32-bit column c holds modes 2c, 2c+1): the tensor core then reads A from TMEM (no shared-memory
+// round trip for the converted tile).
+__device__ __forceinline__ void ta_convert(const TaParams& p, const uint8_t* stg, uint32_t tmem_a, const TaPos q,
                                            int warp, int lane)
 {
     const float2* V = p.V[q.inst];
@@ -204,44 +204,45 @@ __device__ __forceinline__ void ta_convert(const TaParams& p, const uint8_t* stg
     const int64_t row0 = (int64_t)q.mt * (TA_BM / 2);
     const int nvalid = (int)min((int64_t)(TA_BM / 2), p.R - row0);
     const uint32_t sh0 = ta_shift(V, ldV, 0), sh1 = ta_shift(V, ldV, 1);
-    const uint8_t* src0 = stg + warp * 8 * TA_COL_PITCH + lane * 8 + sh0;      // even columns
-    const uint8_t* src1 = stg + warp * 8 * TA_COL_PITCH + lane * 8 + sh1;      // odd columns
-    uint8_t* dst = a_hi + warp * TA_A_LBO + (lane >> 2) * TA_A_SBO + (lane & 3) * 32;
-    const bool slow = nvalid < TA_BM / 2 || (int64_t)(q.kb + 1) * TA_BK > p.J ||
-                      (q.kb == p.kblocks - 1 && row0 + nvalid == ldV);
-    if (!slow) {
+    const int q4 = warp & 3, kh = warp >> 2;
+    const int r = 32 * q4 + lane;                                 // real row in tile: complex row r/2, part r&1
+    const uint8_t* src0 = stg + kh * 32 * TA_COL_PITCH + r * 4 + sh0;     // even modes
+    const uint8_t* src1 = stg + kh * 32 * TA_COL_PITCH + r * 4 + sh1;     // odd modes
+    float v[32];
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            float2 v[8];
+    for (int kk = 0; kk < 32; ++kk) v[kk] = *reinterpret_cast<const float*>(((kk & 1) ? src1 : src0) + kk * TA_COL_PITCH);
+    // ragged edges: rows past R and modes past J read as zero (the staging slot holds stale data there)
+    const int rc = r >> 1;
+    const int klim = (int)min((int64_t)32, p.J - ((int64_t)q.kb * TA_BK + kh * 32));      // warp-uniform
+    if (rc >= nvalid || klim < 32) {
 #pragma unroll
-            for (int kk = 0; kk < 8; ++kk)
-                v[kk] = *reinterpret_cast<const float2*>(((kk & 1) ? src1 : src0) + kk * TA_COL_PITCH + h * 256);
-            ta_split_store(dst + h * 8 * TA_A_SBO, v);
-        }
-    } else {
+        for (int kk = 0; kk < 32; ++kk)
+            if (rc >= nvalid || kk >= klim) v[kk] = 0.f;
+    }
+    // the one element a rounded-down copy can cut off: last row of the last column when V has no padding rows
+    if (q.kb == p.kblocks - 1 && row0 + nvalid == ldV && rc == nvalid - 1) {
+        const int kk = (int)(p.J - 1 - ((int64_t)q.kb * TA_BK + kh * 32));
+        if (kk >= 0 && kk < 32 && ta_tail_cut(ldV, p.J, p.J - 1, row0, nvalid, (kk & 1) ? sh1 : sh0)) {
+            const float t = __ldg(reinterpret_cast<const float*>(V + (p.J - 1) * ldV + row0 + rc) + (r & 1));
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int rp = lane + 32 * h;
-            float2 v[8];
-#pragma unroll
-            for (int kk = 0; kk < 8; ++kk) {
-                const int64_t k = (int64_t)q.kb * TA_BK + warp * 8 + kk;
-                float2 t = *reinterpret_cast<const float2*>(((kk & 1) ? src1 : src0) + kk * TA_COL_PITCH + h * 256);
-                const bool valid = rp < nvalid && k < p.J;
-                if (valid && rp == nvalid - 1 && ta_tail_cut(ldV, p.J, k, row0, nvalid, (kk & 1) ? sh1 : sh0))
-                    t = __ldg(V + k * ldV + row0 + rp);
-                v[kk] = valid ? t : make_float2(0.f, 0.f);
-            }
-            ta_split_store(dst + h * 8 * TA_A_SBO, v);
+            for (int i = 0; i < 32; ++i)
+                if (i == kk) v[i] = t;
         }
     }
+    uint32_t hi[16], lo[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) split_bf16x2(v[2 * i], v[2 * i + 1], hi[i], lo[i]);
+    const uint32_t taddr = tmem_a + ((uint32_t)(32 * q4) << 16) + 16 * kh;
+    tmem_st16(taddr, hi);
+    tmem_st16(taddr + 32, lo);
+    tmem_st_wait();
 }
 
 __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_constant__ TaParams p)
 {
     extern __shared__ __align__(1024) uint8_t smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int mma_stage_bytes = 2 * TA_A_TILE + p.N2 * 256;
+    const int mma_stage_bytes = p.N2 * 256;             // W~ tile (hi | lo); the A operand lives in TMEM
     uint8_t* stg_base = smem + (size_t)TA_MMA_STAGES * mma_stage_bytes;
     uint64_t* bars = reinterpret_cast<uint64_t*>(stg_base + (size_t)p.stg_stages * TA_STG_BYTES);
     uint64_t* full_a = bars;                          // converters -> MMA           [TA_MMA_STAGES]
@@ -250,7 +251,8 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
     uint64_t* acc_full = empty + TA_MMA_STAGES;       // MMA commit -> epilogue      [2]
     uint64_t* acc_empty = acc_full + 2;               // epilogue -> MMA             [2]
     uint64_t* stg_full = acc_empty + 2;               // V bulk copies -> converters [stg_stages]
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(stg_full + p.stg_stages);
+    uint64_t* stg_empty = stg_full + p.stg_stages;    // converters -> V loader      [stg_stages]
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(stg_empty + p.stg_stages);
 
     if (tid == 0) {
         for (int s = 0; s < TA_MMA_STAGES; ++s) {
@@ -262,7 +264,10 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
             mbar_init(&acc_full[b], 1);
             mbar_init(&acc_empty[b], 4);
         }
-        for (int s = 0; s < p.stg_stages; ++s) mbar_init(&stg_full[s], TA_CONV_WARPS);
+        for (int s = 0; s < p.stg_stages; ++s) {
+            mbar_init(&stg_full[s], TA_LOAD_WARPS);
+            mbar_init(&stg_empty[s], TA_CONV_WARPS);
+        }
         mbar_fence_init();
     }
     if (warp == TA_MMA_WARP) tmem_alloc(tmem_slot, TA_TMEM_COLS);
@@ -271,37 +276,48 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
+    TA_BLK(0);
     const int64_t T = (int64_t)p.n_inst * p.n_tiles * p.m_tiles * p.kblocks;
     const int64_t it0 = (int64_t)blockIdx.x * T / gridDim.x;
     const int64_t it1 = (int64_t)(blockIdx.x + 1) * T / gridDim.x;
 
     if (warp < TA_CONV_WARPS) {
-        // ===== converters: fp32 staging -> bf16 hi/lo UMMA tiles.  Warp w owns staging columns 8w..8w+7 of
-        // every stage: it converts them and then refills the same columns for iteration it + stg_stages
-        // (lanes 0-7 issue one bulk copy each), so no "staging empty" barrier is needed.
+        // ===== converters: fp32 staging -> bf16 hi/lo UMMA tiles =====
         int sa = 0, ss = 0;
         uint32_t pa = 0, ps = 0;
-        TaPos cur = ta_pos(p, it0), ahead = cur;
-        int64_t it_ahead = it0;
-        for (int pre = 0; pre < p.stg_stages; ++pre, ++it_ahead) {
-            if (it_ahead < it1) ta_issue_columns(p, ahead, stg_base + (size_t)pre * TA_STG_BYTES, &stg_full[pre], warp, lane);
-            ta_next(p, ahead);
-        }
-        for (int64_t it = it0; it < it1; ++it, ++it_ahead) {
+        TaPos cur = ta_pos(p, it0);
+        for (int64_t it = it0; it < it1; ++it) {
+            const int dn = (int)(it - it0);
             if (warp == 0) {                       // one warp polls, the other seven sleep on a named barrier
+                if (lane == 0) TA_MARK(dn * 16 + 0);
                 mbar_wait(&stg_full[ss], ps);
+                if (lane == 0) TA_MARK(dn * 16 + 1);
                 mbar_wait(&empty[sa], pa ^ 1);
+                if (lane == 0) TA_MARK(dn * 16 + 2);
             }
             named_bar_sync(1, TA_CONV_WARPS * 32);
-            uint8_t* stg = stg_base + (size_t)ss * TA_STG_BYTES;
-            ta_convert(p, stg, smem + (size_t)sa * mma_stage_bytes, cur, warp, lane);
-            fence_proxy_async();
+            tc_fence_after();
+            if (warp == 0 && lane == 0) TA_MARK(dn * 16 + 3);
+            ta_convert(p, stg_base + (size_t)ss * TA_STG_BYTES, tmem_base + TA_A_COL + sa * 64, cur, warp, lane);
+            if (warp == 0 && lane == 0) TA_MARK(dn * 16 + 4);
+            tc_fence_before();
             mbar_arrive(&full_a[sa]);
             __syncwarp();
-            if (it_ahead < it1) ta_issue_columns(p, ahead, stg, &stg_full[ss], warp, lane);
+            if (lane == 0) mbar_arrive(&stg_empty[ss]);
+            if (warp == 0 && lane == 0) TA_MARK(dn * 16 + 5);
             ta_next(p, cur);
-            ta_next(p, ahead);
             if (++sa == TA_MMA_STAGES) { sa = 0; pa ^= 1; }
+            if (++ss == p.stg_stages) { ss = 0; ps ^= 1; }
+        }
+    } else if (warp < TA_W_LOADER) {
+        // ===== V loaders: keep stg_stages x 32 KB of bulk copies in flight =====
+        int ss = 0;
+        uint32_t ps = 0;
+        TaPos q = ta_pos(p, it0);
+        for (int64_t it = it0; it < it1; ++it) {
+            mbar_wait(&stg_empty[ss], ps ^ 1);
+            ta_issue_columns(p, q, stg_base + (size_t)ss * TA_STG_BYTES, &stg_full[ss], warp - TA_V_LOADER, lane);
+            ta_next(p, q);
             if (++ss == p.stg_stages) { ss = 0; ps ^= 1; }
         }
     } else if (warp == TA_W_LOADER) {
@@ -316,53 +332,59 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
                 const int nt = (int)(tile / p.m_tiles);
                 mbar_wait(&empty[stage], phase ^ 1);
                 mbar_expect_tx(&full_b[stage], bytes);
-                bulk_g2s(smem + (size_t)stage * mma_stage_bytes + 2 * TA_A_TILE,
+                bulk_g2s(smem + (size_t)stage * mma_stage_bytes,
                          p.Wt + ((size_t)nt * p.kblocks + kb) * bytes, bytes, &full_b[stage]);
                 if (++stage == TA_MMA_STAGES) { stage = 0; phase ^= 1; }
             }
         }
     } else if (warp == TA_MMA_WARP) {
-        // ===== MMA issuer (one thread) =====
-        if (lane == 0) {
-            const uint32_t idesc = umma_idesc_bf16(TA_BM, p.N2);
-            const uint32_t b_lbo = (uint32_t)p.N2 * 16;
-            int stage = 0, buf = 0;
-            uint32_t phase = 0, use0 = 0, use1 = 0;
-            int64_t it = it0;
-            while (it < it1) {
-                const int64_t tile = it / p.kblocks;
-                const int64_t seg_end = min(it1, (tile + 1) * p.kblocks);
-                const uint32_t use = buf ? use1 : use0;
-                mbar_wait(&acc_empty[buf], (use & 1) ^ 1);
+        // ===== MMA issuer: the whole warp runs the loop (warp-uniform descriptors), one elected lane issues =====
+        const uint32_t idesc = umma_idesc_bf16(TA_BM, p.N2);
+        const uint32_t b_lbo = (uint32_t)p.N2 * 16;
+        const uint32_t smem0 = smem_u32(smem);
+        int stage = 0, buf = 0;
+        uint32_t phase = 0, use0 = 0, use1 = 0;
+        int64_t it = it0;
+        while (it < it1) {
+            const int64_t tile = it / p.kblocks;
+            const int64_t seg_end = min(it1, (tile + 1) * p.kblocks);
+            const uint32_t use = buf ? use1 : use0;
+            mbar_wait(&acc_empty[buf], (use & 1) ^ 1);
+            tc_fence_after();
+            const uint32_t d_tmem = tmem_base + (uint32_t)(buf * p.N2);
+            uint32_t acc = 0;
+            for (; it < seg_end; ++it) {
+                TA_MARK((int)(it - it0) * 16 + 8);
+                mbar_wait(&full_a[stage], phase);
+                TA_MARK((int)(it - it0) * 16 + 9);
+                mbar_wait(&full_b[stage], phase);
                 tc_fence_after();
-                const uint32_t d_tmem = tmem_base + (uint32_t)(buf * p.N2);
-                uint32_t acc = 0;
-                for (; it < seg_end; ++it) {
-                    mbar_wait(&full_a[stage], phase);
-                    mbar_wait(&full_b[stage], phase);
-                    tc_fence_after();
-                    const uint32_t a_hi = smem_u32(smem + (size_t)stage * mma_stage_bytes);
-                    const uint32_t a_lo = a_hi + TA_A_TILE;
-                    const uint32_t b_hi = a_hi + 2 * TA_A_TILE;
-                    const uint32_t b_lo = b_hi + (uint32_t)p.N2 * 128;
+                TA_MARK((int)(it - it0) * 16 + 10);
+                const uint32_t a_hi = tmem_base + TA_A_COL + (uint32_t)stage * 64;     // TMEM columns
+                const uint32_t a_lo = a_hi + 32;
+                const uint32_t b_hi = smem0 + (uint32_t)stage * (uint32_t)mma_stage_bytes;
+                const uint32_t b_lo = b_hi + (uint32_t)p.N2 * 128;
+                const uint64_t db_hi0 = umma_desc(b_hi, b_lbo, 128), db_lo0 = umma_desc(b_lo, b_lbo, 128);
+                if (elect_one()) {
 #pragma unroll
                     for (int s = 0; s < TA_BK / 16; ++s) {
-                        const uint64_t da_hi = umma_desc(a_hi + s * 2 * TA_A_LBO, TA_A_LBO, TA_A_SBO);
-                        const uint64_t da_lo = umma_desc(a_lo + s * 2 * TA_A_LBO, TA_A_LBO, TA_A_SBO);
-                        const uint64_t db_hi = umma_desc(b_hi + s * 2 * b_lbo, b_lbo, 128);
-                        const uint64_t db_lo = umma_desc(b_lo + s * 2 * b_lbo, b_lbo, 128);
-                        umma_bf16(d_tmem, da_lo, db_hi, idesc, acc);
+                        const uint64_t kb = (uint64_t)((s * 2 * b_lbo) >> 4);
+                        umma_bf16_ts(d_tmem, a_lo + 8 * s, db_hi0 + kb, idesc, acc);
                         acc = 1;
-                        umma_bf16(d_tmem, da_hi, db_lo, idesc, 1);
-                        umma_bf16(d_tmem, da_hi, db_hi, idesc, 1);
+                        umma_bf16_ts(d_tmem, a_hi + 8 * s, db_lo0 + kb, idesc, 1);
+                        umma_bf16_ts(d_tmem, a_hi + 8 * s, db_hi0 + kb, idesc, 1);
                     }
                     umma_commit(&empty[stage]);
-                    if (++stage == TA_MMA_STAGES) { stage = 0; phase ^= 1; }
                 }
-                umma_commit(&acc_full[buf]);
-                if (buf) ++use1; else ++use0;
-                buf ^= 1;
+                __syncwarp();
+                acc = 1;
+                TA_MARK((int)(it - it0) * 16 + 11);
+                if (++stage == TA_MMA_STAGES) { stage = 0; phase ^= 1; }
             }
+            if (elect_one()) umma_commit(&acc_full[buf]);
+            __syncwarp();
+            if (buf) ++use1; else ++use0;
+            buf ^= 1;
         }
     } else {
         // ===== epilogue: TMEM -> registers -> lane-pair combine -> partial tile =====
@@ -374,7 +396,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
             const int64_t tile = it / p.kblocks;
             const int64_t seg_end = min(it1, (tile + 1) * p.kblocks);
             if (q == 0) mbar_wait(&acc_full[buf], (buf ? use1 : use0) & 1);
-            named_bar_sync(2, 128);
+            named_bar_sync(10, 128);
             tc_fence_after();
             float* out = p.part + ((size_t)blockIdx.x * p.S + seg) * ((size_t)p.Fzt * TA_BM) + 32 * q + lane;
             const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(buf * p.N2);
@@ -401,6 +423,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
     }
     tc_fence_before();
     __syncthreads();
+    TA_BLK(1);
     if (warp == TA_MMA_WARP) tmem_dealloc(tmem_base, TA_TMEM_COLS);
 }
 
@@ -458,9 +481,9 @@ static TaPlan ta_plan(int64_t R, int64_t J, int64_t Fz, int n_inst, int sm_count
             if (span > pl.S) pl.S = span;
         }
     }
-    const int mma_bytes = TA_MMA_STAGES * (2 * TA_A_TILE + pl.N2 * 256);
+    const int mma_bytes = TA_MMA_STAGES * (pl.N2 * 256);
     pl.stg_stages = (TA_SMEM_LIMIT - 256 - mma_bytes) / TA_STG_BYTES;
-    if (pl.stg_stages > 4) pl.stg_stages = 4;
+    if (pl.stg_stages > 5) pl.stg_stages = 5;
     pl.smem_bytes = (size_t)mma_bytes + (size_t)pl.stg_stages * TA_STG_BYTES + 256;
     pl.wt_bytes = (size_t)pl.n_tiles * pl.kblocks * pl.N2 * 256;
     pl.part_bytes = align_up((size_t)pl.G * pl.S * pl.Fzt * TA_BM * sizeof(float));
