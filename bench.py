@@ -159,10 +159,17 @@ def kernel_rooflines(prof, steps, cfg, dtype_bytes, peaks):
         per = ms / n
         k = dict(ms_per_launch=per, launches_per_step=n / steps, share=ms / total)
         if name in alg:
-            gbs = alg[name]["bytes"] / (per * 1e-3) / 1e9
+            # a grouped launch covers several layers: units per launch = layers per step / launches per step
+            units = cfg.n_layers / (n / steps)
+            nbytes, flops = alg[name]["bytes"] * units, alg[name]["flops"] * units
+            gbs = nbytes / (per * 1e-3) / 1e9
             k.update(bound="hbm", achieved=gbs, peak=peaks["hbm_gbs"], unit="GB/s", frac=gbs / peaks["hbm_gbs"],
-                     traffic=traffic.get(name), alg_bytes=alg[name]["bytes"],
-                     useful_tflops=alg[name]["flops"] / (per * 1e-3) / 1e12)
+                     traffic=traffic.get(name), layers_per_launch=units, alg_bytes=nbytes,
+                     useful_tflops=flops / (per * 1e-3) / 1e12)
+            if name.startswith("tc_"):
+                # BF16x3: three bf16 products per real product; sustained measured bf16 peak (kernel inside a step)
+                ex = 3 * flops / (per * 1e-3) / 1e12
+                k.update(executed_bf16_tflops=ex, tensor_frac=ex / peaks["bf16_tflops_sustained"])
         out[name] = k
     return out
 
