@@ -37,6 +37,7 @@ int32_t check_ctx(scw_ctx* ctx)
     ctx->msg[0] = 0;
     ctx->cuda_err = 0;
     ctx->required_ws = 0;
+    ctx->tc_error = false;
     int cur = -1;
     cudaError_t e = cudaGetDevice(&cur);
     if (e == cudaSuccess && cur != ctx->device) e = cudaSetDevice(ctx->device);
@@ -49,6 +50,7 @@ int32_t check_ctx(scw_ctx* ctx)
 
 int32_t check_launch(scw_ctx* ctx, const char* what)
 {
+    if (ctx->tc_error) return fail(ctx, SCW_ERR_CUDA, "%s: cuTensorMapEncodeTiled failed", what);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) {
         ctx->cuda_err = (int32_t)e;
@@ -98,7 +100,7 @@ int32_t need_ws(scw_ctx* ctx, size_t bytes, const char* who)
 bool use_tc_assemble(const scw_ctx* ctx, const scw_layer* L, int64_t Fz)
 {
     const int64_t R = 3LL * L->U * L->Vn;
-    if (ctx->path == SCW_PATH_SIMT || !tc_assemble_supported(L->dtype, R, L->J, Fz)) return false;
+    if (ctx->path == SCW_PATH_SIMT || !tc_assemble_supported(L->dtype, R, L->J, Fz, L->V, L->ldV)) return false;
     if (ctx->path == SCW_PATH_TENSOR) return true;
     return 2 * R >= 128 && L->J >= 64;
 }

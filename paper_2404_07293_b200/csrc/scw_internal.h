@@ -27,6 +27,7 @@ struct scw_ctx {
     size_t required_ws = 0;
     char msg[256] = {0};
     bool profile = false;
+    bool tc_error = false;          // a tensor map could not be encoded (reported by the entry point)
     std::vector<scw::ProfRec> recs;
     double prof_ms[scw::KC_COUNT] = {0};
     int64_t prof_n[scw::KC_COUNT] = {0};
@@ -92,7 +93,7 @@ void launch_simt_synth(scw_ctx* ctx, int dtype, int U, int Vn, int64_t Fz, const
                        const int64_t strides[4], void* scratch);
 
 // ---- scw_tc_assemble.cu: tcgen05 BF16x3 spectral assembly (complex64) ----------------------------
-bool tc_assemble_supported(int dtype, int64_t R, int64_t J, int64_t Fz);
+bool tc_assemble_supported(int dtype, int64_t R, int64_t J, int64_t Fz, const void* V, int64_t ldV);
 int tc_assemble_max_group();
 size_t tc_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int n_inst, int sm_count);
 // n_inst <= tc_assemble_max_group() instances with equal U, Vn, J, Fz in three launches; instance i -> P_all + i*inst_stride

@@ -76,6 +76,36 @@ def test_ragged_shapes_padding_and_defaults(scw, ctx, dtype, tol, U, Vn, J, Nx, 
     assert np.abs(Ep.cpu().numpy() - refp).max() / np.abs(ref).max() <= tol
 
 
+@pytest.mark.parametrize("U,Vn,J,Fz,pad,n_inst", [(5, 3, 17, 3, 0, 1), (5, 3, 33, 9, 1, 2), (7, 9, 250, 20, 2, 3),
+                                                   (9, 11, 131, 70, 3, 1), (3, 1, 2, 1, 0, 1)])
+def test_forced_tensor_path_ragged(scw, U, Vn, J, Fz, pad, n_inst):
+    """SCW_PATH_TENSOR on shapes that are not multiples of any tile: odd and even ldV (the two TMA column maps),
+    rows not a multiple of 128, J not a multiple of 32 (zero-filled boxes), Fz not a multiple of 8 and above one
+    n tile, grouped instances; every sample of every instance against Tier A."""
+    c = scw.Context(0)
+    c.set_path(scw.SCW_PATH_TENSOR)
+    try:
+        g = np.random.default_rng(11)
+        x = np.sort(g.uniform(-2, 5, 19))
+        y = np.sort(g.uniform(-2, 5, 150))
+        lays = [ragged_layer(U, Vn, J, np.complex64, seed=40 + i + J, ldV_pad=pad, with_c=(i % 2 == 0), with_dir=(i != 1))
+                for i in range(n_inst)]
+        zs = [np.linspace(-0.5 + 0.1 * i, 1.0, Fz) for i in range(n_inst)]
+        Ls = [scw.Layer.from_numpy(l, "cuda") for l in lays]
+        n0 = c.launch_count()
+        Es = scw.scw_sweep_wavelengths(c, Ls, [dev(z) for z in zs], dev(x), dev(y))
+        torch.cuda.synchronize()
+        assert c.launch_count() - n0 <= 2 + 3 + 2                       # twiddles, assembly group, synthesis group
+        for lay, z, E in zip(lays, zs, Es):
+            assert rel_err(E.cpu().numpy(), oracle.layer_grid(x=x, y=y, z=z, **lay)) <= 2e-4
+        P = scw.scw_assemble_spectra(c, Ls[0], dev(zs[0]))
+        E1 = scw.scw_synthesize_grid(c, U=U, Vn=Vn, X=lays[0]["X"], Y=lays[0]["Y"], P=P, x=dev(x), y=dev(y))
+        torch.cuda.synchronize()
+        assert float((E1 - Es[0]).abs().max() / Es[0].abs().max()) <= 2e-5   # other stream-K split, same values
+    finally:
+        c.close()
+
+
 def test_custom_strides_interleaved_output(scw, ctx):
     """strides = (comp, z, y, x): write E as [Fz][Ny][Nx][3] (component fastest)."""
     lay = ragged_layer(5, 3, 20, np.complex64, seed=3)
