@@ -266,7 +266,7 @@ const char* scw_profile_name(int32_t kc)
 {
     static const char* names[KC_COUNT] = {"mode_weights", "twiddles", "simt_assemble", "reduce_splits", "simt_synth_a",
                                           "simt_synth_b", "points_table", "points_planewave", "point_synth", "misc",
-                                          "tc_assemble", "tc_synth"};
+                                          "tc_assemble", "tc_synth", "tc_synth_images"};
     return (kc >= 0 && kc < KC_COUNT) ? names[kc] : nullptr;
 }
 
@@ -399,7 +399,7 @@ static int32_t check_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, 
 // Grouped (batched) sweep: every instance on the tensor-core kernels with the same J and Fz.
 static int sweep_group_size(const scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz)
 {
-    if (n_inst < 2 || Fz[0] <= 0) return 0;
+    if (n_inst < 1 || Fz[0] <= 0) return 0;
     if (!use_tc_assemble(ctx, &inst[0], Fz[0]) || !use_tc_synth(ctx, inst[0].dtype, inst[0].U, inst[0].Vn)) return 0;
     for (int64_t i = 1; i < n_inst; ++i)
         if (inst[i].J != inst[0].J || Fz[i] != Fz[0]) return 0;
@@ -447,14 +447,22 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
     const Twiddles tw = run_twiddles(ctx, L0.dtype, L0.U, L0.Vn, L0.X, L0.Y, Nx, x, Ny, y, cv);
     const int group = sweep_group_size(ctx, n_inst, inst, Fz);
     if (group) {
-        // batched: all instances of a group share three assembly launches and two synthesis launches
+        // batched: all instances of a group share two assembly launches and two synthesis launches
         void* P_all = cv.take((size_t)R * Fz[0] * group * esize(L0.dtype));
         void* a_scr = cv.take(tc_assemble_scratch(R, L0.J, Fz[0], group, ctx->sm_count));
         void* s_scr = cv.take(tc_synth_scratch(L0.U, L0.Vn, Fz[0] * group));
         for (int64_t i0 = 0; i0 < n_inst; i0 += group) {
             const int g = (int)(n_inst - i0 < group ? n_inst - i0 : group);
-            launch_tc_assemble_group(ctx, g, inst + i0, Fz[0], z + i0, P_all, R, R * Fz[0], a_scr);
-            launch_tc_synth_group(ctx, L0.U, L0.Vn, Fz[0], g, P_all, R, Nx, Ny, tw.a, E + i0, s4, s_scr);
+            // the spectra go from the assembly's stream-K partial tiles straight into the synthesis images
+            TcPartials parts;
+            launch_tc_assemble_group_partials(ctx, g, inst + i0, Fz[0], z + i0, a_scr, &parts);
+            if (ctx->tc_error) return;
+            if (tc_synth_partials_supported(L0.U, L0.Vn, parts)) {
+                launch_tc_synth_group_partials(ctx, L0.U, L0.Vn, Fz[0], g, parts, Nx, Ny, tw.a, E + i0, s4, s_scr);
+            } else {
+                launch_tc_assemble_group(ctx, g, inst + i0, Fz[0], z + i0, P_all, R, R * Fz[0], a_scr);
+                launch_tc_synth_group(ctx, L0.U, L0.Vn, Fz[0], g, P_all, R, Nx, Ny, tw.a, E + i0, s4, s_scr);
+            }
         }
         return;
     }

@@ -10,7 +10,7 @@ namespace scw {
 // Kernel classes for launch accounting and the optional per-kernel CUDA-event timers.
 enum KernelClass {
     KC_WEIGHTS = 0, KC_TWIDDLES, KC_ASSEMBLE, KC_REDUCE, KC_SYNTH_A, KC_SYNTH_B, KC_POINTS_TABLE, KC_POINTS,
-    KC_POINT_SYNTH, KC_MISC, KC_ASSEMBLE_TC, KC_SYNTH_TC, KC_COUNT
+    KC_POINT_SYNTH, KC_MISC, KC_ASSEMBLE_TC, KC_SYNTH_TC, KC_SYNTH_IMG, KC_COUNT
 };
 struct ProfRec { cudaEvent_t a, b; int kc; };
 }  // namespace scw
@@ -99,6 +99,18 @@ size_t tc_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int n_inst, int sm_
 // n_inst <= tc_assemble_max_group() instances with equal U, Vn, J, Fz in three launches; instance i -> P_all + i*inst_stride
 void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
                               void* P_all, int64_t ldP, int64_t inst_stride, void* scratch);
+// Where the stream-K partial tiles of a grouped assembly are: tile (inst, n_tile, m_tile) = rows_per_tile complex
+// rows x Fzt planes, fp32 [plane][2*rows_per_tile]; the segments of a tile are the CTAs c_first..c_last whose
+// iteration span [c*T/G, (c+1)*T/G) meets [tile*kblocks, (tile+1)*kblocks), slot (c*S + tile - (c*T/G)/kblocks).
+struct TcPartials {
+    const float* part;
+    int Fzt, n_tiles, m_tiles, kblocks, G, S, rows_per_tile;
+    int64_t T;
+};
+// weights (a-1) + stream-K partial tiles of P = V W (a-2), WITHOUT the segment reduce: the consumer sums the segments
+// (launch_tc_synth_group_partials folds that into its spectrum-image pass, so P never goes to memory).
+void launch_tc_assemble_group_partials(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
+                                       void* scratch, TcPartials* out);
 // weights (a-1) + P = V W (a-2) + segment reduce; scratch from tc_assemble_scratch
 void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z, void* P, int64_t ldP,
                         void* scratch);
@@ -114,6 +126,11 @@ int tc_synth_max_group();
 void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const void* P_all, int64_t ldP,
                            int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
                            void* scratch);
+// Same, reading the spectra as stream-K partial tiles (segment reduce fused into the image pass).
+bool tc_synth_partials_supported(int U, int Vn, const TcPartials& parts);
+void launch_tc_synth_group_partials(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const TcPartials& parts,
+                                    int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
+                                    void* scratch);
 void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,
                      const void* tw, void* E, const int64_t strides[4], void* scratch);
 

@@ -242,7 +242,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
         if (grp == 1) advance();
         const uint32_t a_lane = tmem_base + TA_A_COL + (uint32_t)((w >> 2) * 32) + ((uint32_t)(32 * (w & 3)) << 16);
         for (int64_t it = it0 + grp; it < it1; it += TA_CONV_GROUPS) {
-            const int dn = (int)(it - it0);
+            [[maybe_unused]] const int dn = (int)(it - it0);
             if (w == 0) {                          // one warp polls, the other seven sleep on a named barrier
                 if (lane == 0) TA_MARK(dn * 16 + 0);
                 mbar_wait(&stg_full[ss], ps);
@@ -418,19 +418,28 @@ __global__ void k_tc_reduce(int64_t R, int64_t Fz, int Fzt, int n_tiles, int m_t
     const int tile = blockIdx.x;                                 // global tile id: (inst, n_tile, m_tile)
     const int n = blockIdx.y * blockDim.y + threadIdx.y;
     const int r = threadIdx.x;                                   // complex row in tile, 0..127
+    __shared__ int s_count;                                      // segments of this tile and their slots (64-bit
+    __shared__ int s_slot[256];                                  // divisions done once per block; G <= 256 CTAs)
+    const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+    {
+        const int64_t a = (int64_t)tile * kblocks, b = a + kblocks;
+        const int c_first = (int)(((a + 1) * G + T - 1) / T) - 1;
+        const int c_last = (int)((b * G + T - 1) / T) - 1;
+        if (tid == 0) s_count = c_last - c_first + 1;
+        if (tid <= c_last - c_first) {
+            const int c = c_first + tid;
+            s_slot[tid] = c * S + tile - (int)(((int64_t)c * T / G) / kblocks);
+        }
+    }
+    __syncthreads();
     const int gnt = tile / m_tiles, mt = tile - gnt * m_tiles;
     const int inst = gnt / n_tiles, nt = gnt - inst * n_tiles;
     float2* __restrict__ P = P_all + (int64_t)inst * inst_stride;
     const int64_t row = (int64_t)mt * TA_ROWS + r, col = (int64_t)nt * Fzt + n;
     if (n >= Fzt || row >= R || col >= Fz) return;
-    const int64_t a = (int64_t)tile * kblocks, b = a + kblocks;
-    const int c_first = (int)(((a + 1) * G + T - 1) / T) - 1;
-    const int c_last = (int)((b * G + T - 1) / T) - 1;
     float2 acc = make_float2(0.f, 0.f);
-    for (int c = c_first; c <= c_last; ++c) {
-        const int64_t start = (int64_t)c * T / G;
-        const int seg = tile - (int)(start / kblocks);
-        const float2 v = *reinterpret_cast<const float2*>(part + ((size_t)c * S + seg) * ((size_t)Fzt * 2 * TA_ROWS) +
+    for (int i = 0; i < s_count; ++i) {
+        const float2 v = *reinterpret_cast<const float2*>(part + (size_t)s_slot[i] * ((size_t)Fzt * 2 * TA_ROWS) +
                                                           (size_t)n * (2 * TA_ROWS) + 2 * r);
         acc.x += v.x;
         acc.y += v.y;
@@ -531,17 +540,15 @@ size_t tc_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int n_inst, int sm_
     return align_up(pl.wt_bytes * n_inst) + pl.part_bytes;
 }
 
-// A group of n_inst <= TA_MAX_INST instances with the same U, Vn, J and Fz in three launches:
-// weights (a-1), P = V W over the concatenated iteration space (a-2), segment reduce.
-// Instance i writes P_all + i * inst_stride (column-major [ldP x Fz]).
-void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
-                              void* P_all, int64_t ldP, int64_t inst_stride, void* scratch)
+// weights (a-1) + the stream-K assembly kernel (a-2) of a group; the partial tiles end up in `part`.
+static bool ta_run(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z, void* scratch,
+                   TaPlan& pl, float*& part)
 {
     const scw_layer& L0 = inst[0];
     const int64_t R = 3LL * L0.U * L0.Vn;
-    const TaPlan pl = ta_plan(R, L0.J, Fz, n_inst, ctx->sm_count);
+    pl = ta_plan(R, L0.J, Fz, n_inst, ctx->sm_count);
     uint8_t* Wt = static_cast<uint8_t*>(scratch);
-    float* part = reinterpret_cast<float*>(Wt + align_up(pl.wt_bytes * n_inst));
+    part = reinterpret_cast<float*>(Wt + align_up(pl.wt_bytes * n_inst));
     TwGroup g;
     static thread_local TaParams p;                 // 17 KB of kernel parameters: kept off the stack
     bool maps_ok = true;
@@ -556,9 +563,9 @@ void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, i
         maps_ok = maps_ok && ta_make_map(&p.tmap[i][0], inst[i].V, inst[i].ldV, R, L0.J, 0, nullptr) &&
                   ta_make_map(&p.tmap[i][1], inst[i].V, inst[i].ldV, R, L0.J, 1, &p.xoff1[i]);
     }
-    if (!maps_ok) {                                 // reported by the caller's check_launch as a CUDA error
+    if (!maps_ok) {                                 // reported by the entry point's check_launch
         ctx->tc_error = true;
-        return;
+        return false;
     }
     {
         KernelScope ks(ctx, KC_WEIGHTS);
@@ -582,13 +589,42 @@ void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, i
         cudaFuncSetAttribute(k_tc_assemble, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes);
         k_tc_assemble<<<pl.G, TA_THREADS, pl.smem_bytes, ctx->stream>>>(p);
     }
-    {
-        KernelScope ks(ctx, KC_REDUCE);
-        dim3 block(TA_ROWS, 2);
-        dim3 grid((unsigned)(n_inst * pl.n_tiles * pl.m_tiles), (unsigned)((pl.Fzt + 1) / 2));
-        k_tc_reduce<<<grid, block, 0, ctx->stream>>>(R, Fz, pl.Fzt, pl.n_tiles, pl.m_tiles, pl.kblocks, pl.T, pl.G, pl.S,
-                                                     part, (float2*)P_all, ldP, inst_stride);
-    }
+    return true;
+}
+
+void launch_tc_assemble_group_partials(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
+                                       void* scratch, TcPartials* out)
+{
+    TaPlan pl;
+    float* part = nullptr;
+    out->part = nullptr;
+    if (!ta_run(ctx, n_inst, inst, Fz, z, scratch, pl, part)) return;
+    out->part = part;
+    out->Fzt = pl.Fzt;
+    out->n_tiles = pl.n_tiles;
+    out->m_tiles = pl.m_tiles;
+    out->kblocks = pl.kblocks;
+    out->G = pl.G;
+    out->S = pl.S;
+    out->rows_per_tile = TA_ROWS;
+    out->T = pl.T;
+}
+
+// A group of n_inst <= TA_MAX_INST instances with the same U, Vn, J and Fz in three launches:
+// weights (a-1), P = V W over the concatenated iteration space (a-2), segment reduce.
+// Instance i writes P_all + i * inst_stride (column-major [ldP x Fz]).
+void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
+                              void* P_all, int64_t ldP, int64_t inst_stride, void* scratch)
+{
+    TaPlan pl;
+    float* part = nullptr;
+    if (!ta_run(ctx, n_inst, inst, Fz, z, scratch, pl, part)) return;
+    const int64_t R = 3LL * inst[0].U * inst[0].Vn;
+    KernelScope ks(ctx, KC_REDUCE);
+    dim3 block(TA_ROWS, 2);
+    dim3 grid((unsigned)(n_inst * pl.n_tiles * pl.m_tiles), (unsigned)((pl.Fzt + 1) / 2));
+    k_tc_reduce<<<grid, block, 0, ctx->stream>>>(R, Fz, pl.Fzt, pl.n_tiles, pl.m_tiles, pl.kblocks, pl.T, pl.G, pl.S,
+                                                 part, (float2*)P_all, ldP, inst_stride);
 }
 
 void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z, void* P, int64_t ldP,

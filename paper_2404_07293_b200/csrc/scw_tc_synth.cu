@@ -52,31 +52,31 @@ __host__ __device__ inline int ts_pad16(int v) { return (v + 15) / 16 * 16; }
 // ---- pre-kernels ------------------------------------------------------------------------------------
 // Twiddle images (a-3): for tile t, row r (coordinate index t*128 + r), k = 2f + c: c = 0 -> cos, c = 1 -> sin of
 // 2 pi (f - nfreq/2) coord / period; rows past N and k past 2*nfreq are zero.  hi image then lo image per tile.
-__global__ void k_tc_synth_twiddles(int nfreq, int Kp, int64_t N, int tiles, const double* __restrict__ coord,
-                                    double inv_period, uint8_t* __restrict__ img)
+struct TwAxis { int nfreq, Kp, tiles; int64_t N; const double* coord; double inv_period; uint8_t* img; };
+
+__global__ void k_tc_synth_twiddles(const TwAxis ay, const TwAxis ax, int blocks_y)
 {
-    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;      // (tile, r, kpair)
-    const int kpairs = Kp / 2;
-    if (idx >= (int64_t)tiles * TS_TILE * kpairs) return;
+    const bool is_y = (int)blockIdx.x < blocks_y;                            // one launch covers both axes
+    const TwAxis& a = is_y ? ay : ax;
+    const int64_t idx = (int64_t)(blockIdx.x - (is_y ? 0 : blocks_y)) * blockDim.x + threadIdx.x;      // (tile, r, kpair)
+    const int kpairs = a.Kp / 2;
+    if (idx >= (int64_t)a.tiles * TS_TILE * kpairs) return;
     const int f = (int)(idx % kpairs);
     const int64_t tr = idx / kpairs;
     const int r = (int)(tr % TS_TILE);
     const int t = (int)(tr / TS_TILE);
     const int64_t i = (int64_t)t * TS_TILE + r;
     float co = 0.f, si = 0.f;
-    if (f < nfreq && i < N) {
-        double ph = (double)(f - nfreq / 2) * (coord[i] * inv_period);
-        ph -= rint(ph);
-        double s, c;
-        sincospi(2.0 * ph, &s, &c);
-        co = (float)c;
-        si = (float)s;
+    if (f < a.nfreq && i < a.N) {
+        double ph = (double)(f - a.nfreq / 2) * (a.coord[i] * a.inv_period);   // turns, reduced in fp64; the bf16 hi/lo
+        ph -= rint(ph);                                                         // split below keeps 2^-17: fp32 sincospi
+        sincospif((float)(2.0 * ph), &si, &co);
     }
     uint32_t hi, lo;
     split_bf16x2(co, si, hi, lo);
     const int k = 2 * f;
-    const size_t img_bytes = (size_t)TS_TILE * Kp * 2;
-    uint8_t* base = img + (size_t)t * 2 * img_bytes;
+    const size_t img_bytes = (size_t)TS_TILE * a.Kp * 2;
+    uint8_t* base = a.img + (size_t)t * 2 * img_bytes;
     const size_t off = (size_t)(k >> 3) * 2048 + (size_t)(r >> 3) * 128 + (r & 7) * 16 + (k & 7) * 2;
     *reinterpret_cast<uint32_t*>(base + off) = hi;
     *reinterpret_cast<uint32_t*>(base + img_bytes + off) = lo;
@@ -111,6 +111,80 @@ __global__ void k_tc_synth_pimage(int U, int Vn, int K1p, int N1, int planes, co
     const size_t off = (size_t)(k >> 3) * (N1 * 16) + (size_t)(row >> 3) * 128 + (row & 7) * 16 + (k & 7) * 2;
     *reinterpret_cast<uint32_t*>(base + off) = hi;
     *reinterpret_cast<uint32_t*>(base + img_bytes + off) = lo;
+}
+
+// Spectrum images straight from the stream-K partial tiles of the assembly (TcPartials): one block per plane
+// (inst, z, comp) sums the segments of the M rows it needs into shared memory (fixed CTA order: deterministic)
+// and writes the hi and lo images with 16-byte stores -- P itself never goes to memory.
+constexpr int TS_MAX_PTILES = 64;          // m tiles one plane may touch (M <= 40*40 rows, 128 rows per tile)
+constexpr int TS_MAX_SEGS = 256;           // stream-K segments of one tile (<= number of CTAs)
+
+__global__ void __launch_bounds__(256) k_tc_synth_pimage_partials(int U, int Vn, int K1p, int N1, int64_t Fz,
+                                                                  const __grid_constant__ TcPartials tp,
+                                                                  uint8_t* __restrict__ img)
+{
+    extern __shared__ float2 s_P[];                               // [M] spectrum of this plane, m = v*U + u
+    __shared__ int s_cfirst[TS_MAX_PTILES], s_count[TS_MAX_PTILES], s_seg0[TS_MAX_PTILES];
+    const int plane = blockIdx.x;                                 // inst*Fz*3 + n*3 + comp
+    const int M = U * Vn;
+    const int64_t pz = plane / 3;
+    const int comp = plane - (int)pz * 3;
+    const int inst = (int)(pz / Fz);
+    const int n = (int)(pz - (int64_t)inst * Fz);
+    const int nt = n / tp.Fzt, nn = n - nt * tp.Fzt;
+    const int rpt = tp.rows_per_tile;
+    const int mt0 = (comp * M) / rpt, mt1 = (comp * M + M - 1) / rpt;
+    const int tile_base = (inst * tp.n_tiles + nt) * tp.m_tiles;
+    if ((int)threadIdx.x <= mt1 - mt0) {                          // segment range of each tile: 64-bit divisions once
+        const int tile = tile_base + mt0 + threadIdx.x;
+        const int64_t a = (int64_t)tile * tp.kblocks, b = a + tp.kblocks;
+        const int c_first = (int)(((a + 1) * tp.G + tp.T - 1) / tp.T) - 1;
+        const int c_last = (int)((b * tp.G + tp.T - 1) / tp.T) - 1;
+        s_cfirst[threadIdx.x] = c_first;
+        s_count[threadIdx.x] = c_last - c_first + 1;
+        s_seg0[threadIdx.x] = tile - (int)(((int64_t)c_first * tp.T / tp.G) / tp.kblocks);   // slot of the first segment
+    }
+    __syncthreads();
+    const size_t tile_floats = (size_t)tp.Fzt * 2 * rpt;
+    for (int m = threadIdx.x; m < M; m += blockDim.x) {
+        const int row = comp * M + m;
+        const int ti = row / rpt - mt0, r = row - (row / rpt) * rpt;
+        // a CTA after the first starts inside or at the start of this tile: its segment index is tile - start_tile,
+        // which is 0 for every CTA but the first one of the tile
+        float2 acc = make_float2(0.f, 0.f);
+        const int c0 = s_cfirst[ti], cnt = s_count[ti];
+        for (int i = 0; i < cnt; ++i) {
+            const int seg = i == 0 ? s_seg0[ti] : 0;
+            const float2 v = *reinterpret_cast<const float2*>(tp.part + ((size_t)(c0 + i) * tp.S + seg) * tile_floats +
+                                                              (size_t)nn * (2 * rpt) + 2 * r);
+            acc.x += v.x;
+            acc.y += v.y;
+        }
+        s_P[m] = acc;
+    }
+    __syncthreads();
+    const int kchunks = K1p / 8;
+    const size_t img_bytes = (size_t)N1 * K1p * 2;
+    uint8_t* base = img + (size_t)plane * 2 * img_bytes;
+    for (int idx = threadIdx.x; idx < kchunks * N1; idx += blockDim.x) {
+        const int kc = idx / N1, row = idx - kc * N1;
+        const int u = row >> 1, c = row & 1;
+        uint32_t hi[4], lo[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int v = 4 * kc + e;
+            float a = 0.f, b = 0.f;
+            if (u < U && v < Vn) {
+                const float2 pv = s_P[v * U + u];
+                a = c ? pv.y : pv.x;
+                b = c ? pv.x : -pv.y;
+            }
+            split_bf16x2(a, b, hi[e], lo[e]);
+        }
+        const size_t off = (size_t)kc * (N1 * 16) + (size_t)(row >> 3) * 128 + (row & 7) * 16;
+        *reinterpret_cast<uint4*>(base + off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+        *reinterpret_cast<uint4*>(base + img_bytes + off) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+    }
 }
 
 // ---- main kernel ------------------------------------------------------------------------------------
@@ -375,16 +449,12 @@ void launch_tc_synth_twiddles(scw_ctx* ctx, int U, int Vn, double X, double Y, i
     const TsPlan pl = ts_plan(U, Vn, 1, Nx, Ny);
     uint8_t* A1 = static_cast<uint8_t*>(tw);
     uint8_t* A2 = A1 + pl.a1_bytes;
-    {
-        KernelScope ks(ctx, KC_TWIDDLES);
-        const int64_t n = (int64_t)pl.tiles_y * TS_TILE * (pl.K1p / 2);
-        k_tc_synth_twiddles<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(Vn, pl.K1p, Ny, pl.tiles_y, y, 1.0 / Y, A1);
-    }
-    {
-        KernelScope ks(ctx, KC_TWIDDLES);
-        const int64_t n = (int64_t)pl.tiles_x * TS_TILE * (pl.K2p / 2);
-        k_tc_synth_twiddles<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(U, pl.K2p, Nx, pl.tiles_x, x, 1.0 / X, A2);
-    }
+    const TwAxis ay{Vn, pl.K1p, pl.tiles_y, Ny, y, 1.0 / Y, A1};
+    const TwAxis ax{U, pl.K2p, pl.tiles_x, Nx, x, 1.0 / X, A2};
+    const int64_t ny = (int64_t)pl.tiles_y * TS_TILE * (pl.K1p / 2), nx = (int64_t)pl.tiles_x * TS_TILE * (pl.K2p / 2);
+    const int by = (int)((ny + 255) / 256), bx = (int)((nx + 255) / 256);
+    KernelScope ks(ctx, KC_TWIDDLES);
+    k_tc_synth_twiddles<<<by + bx, 256, 0, ctx->stream>>>(ay, ax, by);
 }
 
 #ifdef SCW_TS_DEBUG
@@ -393,22 +463,12 @@ extern "C" void scw_debug_ts_read(long long* out) { cudaMemcpyFromSymbol(out, g_
 
 int tc_synth_max_group() { return TS_MAX_INST; }
 
-// n_inst <= TS_MAX_INST instances with the same Fz whose spectra are stored back to back
-// (P_all is one column-major [ldP x n_inst*Fz] matrix): one image pre-kernel + one synthesis launch.
-void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const void* P_all, int64_t ldP,
-                           int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
-                           void* scratch)
+// The synthesis launches proper: B1 holds the spectrum images of all n_inst*Fz*3 planes.
+static void ts_launch_main(scw_ctx* ctx, const TsPlan& pl, int64_t Fz, int n_inst, const uint8_t* B1, int64_t Nx,
+                           int64_t Ny, const void* tw, void* const* E, const int64_t strides[4])
 {
-    const TsPlan pl = ts_plan(U, Vn, Fz * n_inst, Nx, Ny);
+    static thread_local TsParams p;
     const int planes = (int)(Fz * 3 * n_inst);
-    uint8_t* B1 = static_cast<uint8_t*>(scratch);
-    {
-        KernelScope ks(ctx, KC_SYNTH_A);
-        const int64_t n = (int64_t)planes * pl.K2p * (pl.K1p / 2);
-        k_tc_synth_pimage<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(U, Vn, pl.K1p, pl.K2p, planes,
-                                                                                (const float2*)P_all, ldP, B1);
-    }
-    TsParams p;
     p.A1 = static_cast<const uint8_t*>(tw);
     p.A2 = p.A1 + pl.a1_bytes;
     p.B1 = B1;
@@ -435,6 +495,45 @@ void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, 
         KernelScope ks(ctx, KC_SYNTH_TC);
         k_tc_synth<<<p.npairs * per_pair, TS_THREADS, pl.smem_bytes, ctx->stream>>>(p);
     }
+}
+
+// n_inst <= TS_MAX_INST instances with the same Fz whose spectra are stored back to back
+// (P_all is one column-major [ldP x n_inst*Fz] matrix): one image pre-kernel + one synthesis launch.
+void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const void* P_all, int64_t ldP,
+                           int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
+                           void* scratch)
+{
+    const TsPlan pl = ts_plan(U, Vn, Fz * n_inst, Nx, Ny);
+    const int planes = (int)(Fz * 3 * n_inst);
+    uint8_t* B1 = static_cast<uint8_t*>(scratch);
+    {
+        KernelScope ks(ctx, KC_SYNTH_IMG);
+        const int64_t n = (int64_t)planes * pl.K2p * (pl.K1p / 2);
+        k_tc_synth_pimage<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(U, Vn, pl.K1p, pl.K2p, planes,
+                                                                                (const float2*)P_all, ldP, B1);
+    }
+    ts_launch_main(ctx, pl, Fz, n_inst, B1, Nx, Ny, tw, E, strides);
+}
+
+bool tc_synth_partials_supported(int U, int Vn, const TcPartials& parts)
+{
+    const int M = U * Vn;
+    return parts.part && (M + parts.rows_per_tile - 1) / parts.rows_per_tile + 1 <= TS_MAX_PTILES && parts.G <= TS_MAX_SEGS;
+}
+
+void launch_tc_synth_group_partials(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const TcPartials& parts,
+                                    int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
+                                    void* scratch)
+{
+    const TsPlan pl = ts_plan(U, Vn, Fz * n_inst, Nx, Ny);
+    const int planes = (int)(Fz * 3 * n_inst);
+    uint8_t* B1 = static_cast<uint8_t*>(scratch);
+    {
+        KernelScope ks(ctx, KC_SYNTH_IMG);
+        k_tc_synth_pimage_partials<<<planes, 256, (size_t)U * Vn * sizeof(float2), ctx->stream>>>(U, Vn, pl.K1p, pl.K2p, Fz,
+                                                                                                 parts, B1);
+    }
+    ts_launch_main(ctx, pl, Fz, n_inst, B1, Nx, Ny, tw, E, strides);
 }
 
 void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,
