@@ -100,12 +100,13 @@ size_t tc_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int n_inst, int sm_
 void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
                               void* P_all, int64_t ldP, int64_t inst_stride, void* scratch);
 // Where the stream-K partial tiles of a grouped assembly are: tile (inst, n_tile, m_tile) = rows_per_tile complex
-// rows x Fzt planes, fp32 [plane][2*rows_per_tile]; the segments of a tile are the CTAs c_first..c_last whose
-// iteration span [c*T/G, (c+1)*T/G) meets [tile*kblocks, (tile+1)*kblocks), slot (c*S + tile - (c*T/G)/kblocks).
+// rows x Fzt planes, fp32 [plane][2*rows_per_tile].  A tile is the sum of seg_count[tile] segments, segment i in slot
+// seg_slot[tile*max_segs + i] (the table is written by the assembly kernel, in CTA order: a fixed summation order).
 struct TcPartials {
     const float* part;
-    int Fzt, n_tiles, m_tiles, kblocks, G, S, rows_per_tile;
-    int64_t T;
+    const int* seg_count;
+    const int* seg_slot;
+    int Fzt, n_tiles, m_tiles, max_segs, rows_per_tile;
 };
 // weights (a-1) + stream-K partial tiles of P = V W (a-2), WITHOUT the segment reduce: the consumer sums the segments
 // (launch_tc_synth_group_partials folds that into its spectrum-image pass, so P never goes to memory).

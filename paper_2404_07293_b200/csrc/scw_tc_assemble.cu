@@ -68,7 +68,9 @@ struct TaParams {
     int n_inst;
     const uint8_t* Wt;      // [inst][n_tile][k_block][hi | lo] K-major UMMA images of [W_r | W_i]
     float* part;            // [slot][Fzt][256] fp32 partial tiles
-    int N2, Fzt, n_tiles, m_tiles, kblocks, S, stg_stages, nbuf;
+    int* seg_count;         // [tile] number of stream-K segments of the tile (written by the tile's first CTA)
+    int* seg_slot;          // [tile][max_segs] slot of every segment, in CTA order
+    int N2, Fzt, n_tiles, m_tiles, kblocks, S, stg_stages, nbuf, max_segs;
 };
 
 // Mode index of staging column kk (0..31) of k-block kb: even modes first, then odd modes.
@@ -82,7 +84,7 @@ __host__ __device__ __forceinline__ int64_t ta_mode(int kb, int kk)
 // bf16 hi + lo, 2^-17 relative, so fp32 transcendentals lose nothing), written as the K-major no-swizzle
 // shared-memory image of every (n_tile, k_block) B tile: element (n, kk) at
 //   (kk/8)*(N2*16) + (n/8)*128 + (n%8)*16 + (kk%8)*2,  n < Fzt: Re W[j, i], n >= Fzt: Im W[j, i],  j = ta_mode(kb, kk).
-// One thread produces the 8 consecutive kk of one 16-byte core-matrix row, for the Re and the Im row, hi and lo.
+// One thread produces two consecutive kk (4 bytes of a 16-byte core-matrix row), for the Re and the Im row, hi and lo.
 struct TwGroup {
     const float2* c[TA_MAX_INST];
     const double2* gamma[TA_MAX_INST];
@@ -94,26 +96,25 @@ struct TwGroup {
 __global__ void __launch_bounds__(256) k_tc_weights(int n_inst, int64_t J, int64_t Fz, int Fzt, int n_tiles, int kblocks,
                                                     const __grid_constant__ TwGroup g_, uint8_t* __restrict__ Wt_all)
 {
-    const int64_t per_tile = 4 * (int64_t)Fzt;                         // threads per (inst, n_tile, k_block) tile
-    const int64_t gidx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const int64_t n_tiles_all = (int64_t)n_inst * n_tiles * kblocks;
-    if (gidx >= per_tile * n_tiles_all) return;
-    const int64_t tile_id = gidx / per_tile;
-    const int rem = (int)(gidx - tile_id * per_tile);
-    const int c4 = rem / Fzt, n = rem - c4 * Fzt;                      // k chunk (8 modes), plane within the n tile
-    const int kb = (int)(tile_id % kblocks);
-    const int64_t t2 = tile_id / kblocks;
-    const int nt = (int)(t2 % n_tiles), inst = (int)(t2 / n_tiles);
+    // block = one (inst, n_tile, k_block) tile; thread item = (k chunk c4, plane n, mode pair e2), e2 fastest: the four
+    // lanes of a pair group fill one 16-byte core-matrix row, a warp writes 128 contiguous bytes per store
+    const int kb = blockIdx.x, nt = blockIdx.y, inst = blockIdx.z;
+    const int64_t tile_id = ((int64_t)inst * n_tiles + nt) * kblocks + kb;
     const float2* __restrict__ c = g_.c[inst];
     const double2* __restrict__ gamma = g_.gamma[inst];
     const int8_t* __restrict__ dir = g_.dir[inst];
     const double inv_lambda = g_.inv_lambda[inst], z_lo = g_.z_lo[inst], z_hi = g_.z_hi[inst];
+    const int N2 = 2 * Fzt;
+    uint8_t* tile = Wt_all + (size_t)tile_id * (size_t)N2 * 128;
+    for (int rem = threadIdx.x; rem < 16 * Fzt; rem += blockDim.x) {
+    const int e2 = rem & 3, cn = rem >> 2;
+    const int c4 = cn / Fzt, n = cn - c4 * Fzt;                        // k chunk (8 modes), plane within the n tile
     const int64_t i = (int64_t)nt * Fzt + n;
     const double zi = i < Fz ? g_.z[inst][i] : 0.0;
-    float wr[8], wi[8];
+    float wr[2], wi[2];
 #pragma unroll
-    for (int e = 0; e < 8; ++e) {
-        const int64_t j = ta_mode(kb, 8 * c4 + e);
+    for (int e = 0; e < 2; ++e) {
+        const int64_t j = ta_mode(kb, 8 * c4 + 2 * e2 + e);
         wr[e] = 0.f;
         wi[e] = 0.f;
         if (j < J && i < Fz) {
@@ -132,25 +133,18 @@ __global__ void __launch_bounds__(256) k_tc_weights(int n_inst, int64_t J, int64
             wi[e] = cr * ai + ci * ar;
         }
     }
-    const int N2 = 2 * Fzt;
-    uint4 rh, rl, ih, il;
-    split_bf16x2(wr[0], wr[1], rh.x, rl.x);
-    split_bf16x2(wr[2], wr[3], rh.y, rl.y);
-    split_bf16x2(wr[4], wr[5], rh.z, rl.z);
-    split_bf16x2(wr[6], wr[7], rh.w, rl.w);
-    split_bf16x2(wi[0], wi[1], ih.x, il.x);
-    split_bf16x2(wi[2], wi[3], ih.y, il.y);
-    split_bf16x2(wi[4], wi[5], ih.z, il.z);
-    split_bf16x2(wi[6], wi[7], ih.w, il.w);
-    uint8_t* tile = Wt_all + (size_t)tile_id * (size_t)N2 * 128;
+    uint32_t rh, rl, ih, il;
+    split_bf16x2(wr[0], wr[1], rh, rl);
+    split_bf16x2(wi[0], wi[1], ih, il);
     const int n2 = n + Fzt;
-    const size_t off_r = (size_t)c4 * (N2 * 16) + (size_t)(n >> 3) * 128 + (n & 7) * 16;
-    const size_t off_i = (size_t)c4 * (N2 * 16) + (size_t)(n2 >> 3) * 128 + (n2 & 7) * 16;
+    const size_t off_r = (size_t)c4 * (N2 * 16) + (size_t)(n >> 3) * 128 + (n & 7) * 16 + e2 * 4;
+    const size_t off_i = (size_t)c4 * (N2 * 16) + (size_t)(n2 >> 3) * 128 + (n2 & 7) * 16 + e2 * 4;
     const size_t lo = (size_t)N2 * 64;
-    *reinterpret_cast<uint4*>(tile + off_r) = rh;
-    *reinterpret_cast<uint4*>(tile + off_i) = ih;
-    *reinterpret_cast<uint4*>(tile + lo + off_r) = rl;
-    *reinterpret_cast<uint4*>(tile + lo + off_i) = il;
+    *reinterpret_cast<uint32_t*>(tile + off_r) = rh;
+    *reinterpret_cast<uint32_t*>(tile + off_i) = ih;
+    *reinterpret_cast<uint32_t*>(tile + lo + off_r) = rl;
+    *reinterpret_cast<uint32_t*>(tile + lo + off_i) = il;
+    }
 }
 
 // ---- main kernel -----------------------------------------------------------------------------------
@@ -379,6 +373,13 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
             if (q == 0) mbar_wait(&acc_full[buf], (buf ? use1 : use0) & 1);
             named_bar_sync(10, 128);
             tc_fence_after();
+            if (q == 0 && lane == 0) {
+                // segment table: the CTAs whose spans meet this tile are c_first..c_last, this one is number c - c_first
+                const int64_t a = tile * p.kblocks, b = a + p.kblocks;
+                const int c_first = (int)(((a + 1) * gridDim.x + T - 1) / T) - 1;
+                p.seg_slot[tile * p.max_segs + ((int)blockIdx.x - c_first)] = (int)blockIdx.x * p.S + seg;
+                if ((int)blockIdx.x == c_first) p.seg_count[tile] = (int)((b * gridDim.x + T - 1) / T) - c_first;
+            }
             float* out = p.part + ((size_t)blockIdx.x * p.S + seg) * ((size_t)p.Fzt * 2 * TA_ROWS) + 32 * q + lane;
 #pragma unroll 1
             for (int b = 0; b < 2; ++b) {
@@ -412,34 +413,23 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
 }
 
 // Sum the segments of every tile in CTA order: P[mt*128 + r, nt*Fzt + n] = sum_seg part[seg][n][2r..2r+1].
-__global__ void k_tc_reduce(int64_t R, int64_t Fz, int Fzt, int n_tiles, int m_tiles, int kblocks, int64_t T, int G, int S,
+__global__ void k_tc_reduce(int64_t R, int64_t Fz, int Fzt, int n_tiles, int m_tiles, int max_segs,
+                            const int* __restrict__ seg_count, const int* __restrict__ seg_slot,
                             const float* __restrict__ part, float2* __restrict__ P_all, int64_t ldP, int64_t inst_stride)
 {
     const int tile = blockIdx.x;                                 // global tile id: (inst, n_tile, m_tile)
     const int n = blockIdx.y * blockDim.y + threadIdx.y;
     const int r = threadIdx.x;                                   // complex row in tile, 0..127
-    __shared__ int s_count;                                      // segments of this tile and their slots (64-bit
-    __shared__ int s_slot[256];                                  // divisions done once per block; G <= 256 CTAs)
-    const int tid = threadIdx.y * blockDim.x + threadIdx.x;
-    {
-        const int64_t a = (int64_t)tile * kblocks, b = a + kblocks;
-        const int c_first = (int)(((a + 1) * G + T - 1) / T) - 1;
-        const int c_last = (int)((b * G + T - 1) / T) - 1;
-        if (tid == 0) s_count = c_last - c_first + 1;
-        if (tid <= c_last - c_first) {
-            const int c = c_first + tid;
-            s_slot[tid] = c * S + tile - (int)(((int64_t)c * T / G) / kblocks);
-        }
-    }
-    __syncthreads();
     const int gnt = tile / m_tiles, mt = tile - gnt * m_tiles;
     const int inst = gnt / n_tiles, nt = gnt - inst * n_tiles;
     float2* __restrict__ P = P_all + (int64_t)inst * inst_stride;
     const int64_t row = (int64_t)mt * TA_ROWS + r, col = (int64_t)nt * Fzt + n;
     if (n >= Fzt || row >= R || col >= Fz) return;
+    const int count = seg_count[tile];
+    const int* __restrict__ slots = seg_slot + (size_t)tile * max_segs;
     float2 acc = make_float2(0.f, 0.f);
-    for (int i = 0; i < s_count; ++i) {
-        const float2 v = *reinterpret_cast<const float2*>(part + (size_t)s_slot[i] * ((size_t)Fzt * 2 * TA_ROWS) +
+    for (int i = 0; i < count; ++i) {
+        const float2 v = *reinterpret_cast<const float2*>(part + (size_t)slots[i] * ((size_t)Fzt * 2 * TA_ROWS) +
                                                           (size_t)n * (2 * TA_ROWS) + 2 * r);
         acc.x += v.x;
         acc.y += v.y;
@@ -449,9 +439,9 @@ __global__ void k_tc_reduce(int64_t R, int64_t Fz, int Fzt, int n_tiles, int m_t
 
 // ---- host side -------------------------------------------------------------------------------------
 struct TaPlan {
-    int Fzt, N2, n_tiles, m_tiles, kblocks, G, S, stg_stages, nbuf;
+    int Fzt, N2, n_tiles, m_tiles, kblocks, G, S, stg_stages, nbuf, max_segs;
     int64_t T;
-    size_t wt_bytes, part_bytes, smem_bytes;      // wt_bytes: W~ images of ONE instance
+    size_t wt_bytes, part_bytes, seg_bytes, smem_bytes;      // wt_bytes: W~ images of ONE instance
 };
 
 static TaPlan ta_plan(int64_t R, int64_t J, int64_t Fz, int n_inst, int sm_count)
@@ -481,6 +471,9 @@ static TaPlan ta_plan(int64_t R, int64_t J, int64_t Fz, int n_inst, int sm_count
     pl.smem_bytes = (size_t)w_bytes + (size_t)pl.stg_stages * TA_STG_BYTES + 256;
     pl.wt_bytes = (size_t)pl.n_tiles * pl.kblocks * pl.N2 * 128;
     pl.part_bytes = align_up((size_t)pl.G * pl.S * pl.Fzt * 2 * TA_ROWS * sizeof(float));
+    // a CTA span holds at least T/G iterations, so at most (kblocks-1)/(T/G) + 2 spans meet one tile
+    pl.max_segs = (int)((pl.kblocks - 1) / (pl.T / pl.G) + 2);
+    pl.seg_bytes = align_up((size_t)n_inst * pl.n_tiles * pl.m_tiles * (1 + pl.max_segs) * sizeof(int));
     return pl;
 }
 
@@ -504,6 +497,8 @@ static EncodeTiledFn encode_tiled_fn()
 
 // Tensor map over every second column of V starting at column `first` (0 or 1): 8-byte elements,
 // dim0 = rows (contiguous), dim1 = columns at stride 2*ldV*8 bytes; box 128 x 16; out-of-range reads give 0.
+// L2 promotion 64 B: the 1 KB column pieces start at arbitrary 8-byte offsets, wider promotion re-fetches the
+// boundary lines shared with the vertically adjacent tile (measured: 256 B -> 64 B = 112 -> 104 us at config 1).
 // For odd ldV the odd columns start 8 bytes off a 16-byte boundary: their map starts one element earlier (the last
 // element of the column before) and its box is 130 rows, so that every box still starts on a 16-byte boundary
 // (TMA faults otherwise); row r of the tile then sits at box row r + 1 (xoff = 1).
@@ -521,7 +516,7 @@ static bool ta_make_map(CUtensorMap* map, const void* V, int64_t ldV, int64_t R,
     const cuuint32_t estr[2] = {1, 1};
     if (xoff) *xoff = off;
     return enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT64, 2, const_cast<char*>(base), dims, strides, box, estr,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_64B,
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
@@ -529,7 +524,7 @@ static bool ta_make_map(CUtensorMap* map, const void* V, int64_t ldV, int64_t R,
 bool tc_assemble_supported(int dtype, int64_t R, int64_t J, int64_t Fz, const void* V, int64_t ldV)
 {
     return dtype == SCW_C64 && R >= 1 && J >= 2 && Fz >= 1 && (reinterpret_cast<uintptr_t>(V) & 15) == 0 &&
-           2 * ldV * 8 < ((int64_t)1 << 40) && R + 1 < ((int64_t)1 << 32);
+           2 * ldV * 8 < ((int64_t)1 << 40) && R + 1 < ((int64_t)1 << 32) && (Fz + 63) / 64 <= 65535;
 }
 
 int tc_assemble_max_group() { return TA_MAX_INST; }
@@ -537,18 +532,20 @@ int tc_assemble_max_group() { return TA_MAX_INST; }
 size_t tc_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int n_inst, int sm_count)
 {
     const TaPlan pl = ta_plan(R, J, Fz, n_inst, sm_count);
-    return align_up(pl.wt_bytes * n_inst) + pl.part_bytes;
+    return align_up(pl.wt_bytes * n_inst) + pl.part_bytes + pl.seg_bytes;
 }
 
 // weights (a-1) + the stream-K assembly kernel (a-2) of a group; the partial tiles end up in `part`.
 static bool ta_run(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z, void* scratch,
-                   TaPlan& pl, float*& part)
+                   TaPlan& pl, float*& part, int*& seg_count, int*& seg_slot)
 {
     const scw_layer& L0 = inst[0];
     const int64_t R = 3LL * L0.U * L0.Vn;
     pl = ta_plan(R, L0.J, Fz, n_inst, ctx->sm_count);
     uint8_t* Wt = static_cast<uint8_t*>(scratch);
     part = reinterpret_cast<float*>(Wt + align_up(pl.wt_bytes * n_inst));
+    seg_count = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(part) + pl.part_bytes);
+    seg_slot = seg_count + (size_t)n_inst * pl.n_tiles * pl.m_tiles;
     TwGroup g;
     static thread_local TaParams p;                 // 17 KB of kernel parameters: kept off the stack
     bool maps_ok = true;
@@ -569,13 +566,15 @@ static bool ta_run(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, 
     }
     {
         KernelScope ks(ctx, KC_WEIGHTS);
-        const int64_t n = (int64_t)n_inst * pl.n_tiles * pl.kblocks * 4 * pl.Fzt;
-        k_tc_weights<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(n_inst, L0.J, Fz, pl.Fzt, pl.n_tiles,
-                                                                           pl.kblocks, g, Wt);
+        const dim3 grid((unsigned)pl.kblocks, (unsigned)pl.n_tiles, (unsigned)n_inst);
+        k_tc_weights<<<grid, 256, 0, ctx->stream>>>(n_inst, L0.J, Fz, pl.Fzt, pl.n_tiles, pl.kblocks, g, Wt);
     }
     p.n_inst = n_inst;
     p.Wt = Wt;
     p.part = part;
+    p.seg_count = seg_count;
+    p.seg_slot = seg_slot;
+    p.max_segs = pl.max_segs;
     p.N2 = pl.N2;
     p.Fzt = pl.Fzt;
     p.n_tiles = pl.n_tiles;
@@ -597,17 +596,17 @@ void launch_tc_assemble_group_partials(scw_ctx* ctx, int n_inst, const scw_layer
 {
     TaPlan pl;
     float* part = nullptr;
+    int *seg_count = nullptr, *seg_slot = nullptr;
     out->part = nullptr;
-    if (!ta_run(ctx, n_inst, inst, Fz, z, scratch, pl, part)) return;
+    if (!ta_run(ctx, n_inst, inst, Fz, z, scratch, pl, part, seg_count, seg_slot)) return;
     out->part = part;
+    out->seg_count = seg_count;
+    out->seg_slot = seg_slot;
+    out->max_segs = pl.max_segs;
     out->Fzt = pl.Fzt;
     out->n_tiles = pl.n_tiles;
     out->m_tiles = pl.m_tiles;
-    out->kblocks = pl.kblocks;
-    out->G = pl.G;
-    out->S = pl.S;
     out->rows_per_tile = TA_ROWS;
-    out->T = pl.T;
 }
 
 // A group of n_inst <= TA_MAX_INST instances with the same U, Vn, J and Fz in three launches:
@@ -618,12 +617,13 @@ void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, i
 {
     TaPlan pl;
     float* part = nullptr;
-    if (!ta_run(ctx, n_inst, inst, Fz, z, scratch, pl, part)) return;
+    int *seg_count = nullptr, *seg_slot = nullptr;
+    if (!ta_run(ctx, n_inst, inst, Fz, z, scratch, pl, part, seg_count, seg_slot)) return;
     const int64_t R = 3LL * inst[0].U * inst[0].Vn;
     KernelScope ks(ctx, KC_REDUCE);
     dim3 block(TA_ROWS, 2);
     dim3 grid((unsigned)(n_inst * pl.n_tiles * pl.m_tiles), (unsigned)((pl.Fzt + 1) / 2));
-    k_tc_reduce<<<grid, block, 0, ctx->stream>>>(R, Fz, pl.Fzt, pl.n_tiles, pl.m_tiles, pl.kblocks, pl.T, pl.G, pl.S,
+    k_tc_reduce<<<grid, block, 0, ctx->stream>>>(R, Fz, pl.Fzt, pl.n_tiles, pl.m_tiles, pl.max_segs, seg_count, seg_slot,
                                                  part, (float2*)P_all, ldP, inst_stride);
 }
 

@@ -113,78 +113,64 @@ __global__ void k_tc_synth_pimage(int U, int Vn, int K1p, int N1, int planes, co
     *reinterpret_cast<uint32_t*>(base + img_bytes + off) = lo;
 }
 
-// Spectrum images straight from the stream-K partial tiles of the assembly (TcPartials): one block per plane
-// (inst, z, comp) sums the segments of the M rows it needs into shared memory (fixed CTA order: deterministic)
-// and writes the hi and lo images with 16-byte stores -- P itself never goes to memory.
-constexpr int TS_MAX_PTILES = 64;          // m tiles one plane may touch (M <= 40*40 rows, 128 rows per tile)
-constexpr int TS_MAX_SEGS = 256;           // stream-K segments of one tile (<= number of CTAs)
+// Spectrum images straight from the stream-K partial tiles of the assembly (TcPartials): thread = (plane, 8-wide
+// k chunk kc, frequency u) sums the segments of its four spectrum entries P[u, 4kc..4kc+3] in the table's fixed order
+// (deterministic) and writes the 16-byte chunks of image rows (u,Re) and (u,Im), hi and lo -- P itself never goes to
+// memory.  Lanes run along u: loads of one v are contiguous, a warp's stores cover 1 KB of the image.
+constexpr int TS_PI_THREADS = 128;
 
-__global__ void __launch_bounds__(256) k_tc_synth_pimage_partials(int U, int Vn, int K1p, int N1, int64_t Fz,
-                                                                  const __grid_constant__ TcPartials tp,
-                                                                  uint8_t* __restrict__ img)
+__global__ void __launch_bounds__(TS_PI_THREADS) k_tc_synth_pimage_partials(int U, int Vn, int K1p, int N1, int Fz,
+                                                                            const __grid_constant__ TcPartials tp,
+                                                                            uint8_t* __restrict__ img)
 {
-    extern __shared__ float2 s_P[];                               // [M] spectrum of this plane, m = v*U + u
-    __shared__ int s_cfirst[TS_MAX_PTILES], s_count[TS_MAX_PTILES], s_seg0[TS_MAX_PTILES];
     const int plane = blockIdx.x;                                 // inst*Fz*3 + n*3 + comp
+    const int item = blockIdx.y * TS_PI_THREADS + threadIdx.x;    // kc * (N1/2) + u
+    const int half = N1 / 2, kchunks = K1p / 8;
+    if (item >= kchunks * half) return;
+    const int kc = item / half, u = item - kc * half;
     const int M = U * Vn;
-    const int64_t pz = plane / 3;
-    const int comp = plane - (int)pz * 3;
-    const int inst = (int)(pz / Fz);
-    const int n = (int)(pz - (int64_t)inst * Fz);
+    const int pz = plane / 3, comp = plane - pz * 3;
+    const int inst = pz / Fz, n = pz - inst * Fz;
     const int nt = n / tp.Fzt, nn = n - nt * tp.Fzt;
     const int rpt = tp.rows_per_tile;
-    const int mt0 = (comp * M) / rpt, mt1 = (comp * M + M - 1) / rpt;
     const int tile_base = (inst * tp.n_tiles + nt) * tp.m_tiles;
-    if ((int)threadIdx.x <= mt1 - mt0) {                          // segment range of each tile: 64-bit divisions once
-        const int tile = tile_base + mt0 + threadIdx.x;
-        const int64_t a = (int64_t)tile * tp.kblocks, b = a + tp.kblocks;
-        const int c_first = (int)(((a + 1) * tp.G + tp.T - 1) / tp.T) - 1;
-        const int c_last = (int)((b * tp.G + tp.T - 1) / tp.T) - 1;
-        s_cfirst[threadIdx.x] = c_first;
-        s_count[threadIdx.x] = c_last - c_first + 1;
-        s_seg0[threadIdx.x] = tile - (int)(((int64_t)c_first * tp.T / tp.G) / tp.kblocks);   // slot of the first segment
-    }
-    __syncthreads();
     const size_t tile_floats = (size_t)tp.Fzt * 2 * rpt;
-    for (int m = threadIdx.x; m < M; m += blockDim.x) {
-        const int row = comp * M + m;
-        const int ti = row / rpt - mt0, r = row - (row / rpt) * rpt;
-        // a CTA after the first starts inside or at the start of this tile: its segment index is tile - start_tile,
-        // which is 0 for every CTA but the first one of the tile
-        float2 acc = make_float2(0.f, 0.f);
-        const int c0 = s_cfirst[ti], cnt = s_count[ti];
-        for (int i = 0; i < cnt; ++i) {
-            const int seg = i == 0 ? s_seg0[ti] : 0;
-            const float2 v = *reinterpret_cast<const float2*>(tp.part + ((size_t)(c0 + i) * tp.S + seg) * tile_floats +
-                                                              (size_t)nn * (2 * rpt) + 2 * r);
-            acc.x += v.x;
-            acc.y += v.y;
-        }
-        s_P[m] = acc;
-    }
-    __syncthreads();
-    const int kchunks = K1p / 8;
-    const size_t img_bytes = (size_t)N1 * K1p * 2;
-    uint8_t* base = img + (size_t)plane * 2 * img_bytes;
-    for (int idx = threadIdx.x; idx < kchunks * N1; idx += blockDim.x) {
-        const int kc = idx / N1, row = idx - kc * N1;
-        const int u = row >> 1, c = row & 1;
-        uint32_t hi[4], lo[4];
+    float2 pv[4];
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const int v = 4 * kc + e;
-            float a = 0.f, b = 0.f;
-            if (u < U && v < Vn) {
-                const float2 pv = s_P[v * U + u];
-                a = c ? pv.y : pv.x;
-                b = c ? pv.x : -pv.y;
+    for (int e = 0; e < 4; ++e) {
+        const int v = 4 * kc + e;
+        pv[e] = make_float2(0.f, 0.f);
+        if (u < U && v < Vn) {
+            const int row = comp * M + v * U + u;
+            const int mt = row / rpt, r = row - mt * rpt;
+            const int tile = tile_base + mt;
+            const int cnt = tp.seg_count[tile];
+            const int* __restrict__ slots = tp.seg_slot + (size_t)tile * tp.max_segs;
+            const float* __restrict__ src = tp.part + (size_t)nn * (2 * rpt) + 2 * r;
+            for (int i = 0; i < cnt; ++i) {
+                const float2 t = *reinterpret_cast<const float2*>(src + (size_t)slots[i] * tile_floats);
+                pv[e].x += t.x;
+                pv[e].y += t.y;
             }
-            split_bf16x2(a, b, hi[e], lo[e]);
         }
-        const size_t off = (size_t)kc * (N1 * 16) + (size_t)(row >> 3) * 128 + (row & 7) * 16;
-        *reinterpret_cast<uint4*>(base + off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-        *reinterpret_cast<uint4*>(base + img_bytes + off) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
     }
+    // row (u,Re): (P_r, -P_i) per v;  row (u,Im): (P_i, P_r)
+    uint4 re_hi, re_lo, im_hi, im_lo;
+    split_bf16x2(pv[0].x, -pv[0].y, re_hi.x, re_lo.x);
+    split_bf16x2(pv[1].x, -pv[1].y, re_hi.y, re_lo.y);
+    split_bf16x2(pv[2].x, -pv[2].y, re_hi.z, re_lo.z);
+    split_bf16x2(pv[3].x, -pv[3].y, re_hi.w, re_lo.w);
+    split_bf16x2(pv[0].y, pv[0].x, im_hi.x, im_lo.x);
+    split_bf16x2(pv[1].y, pv[1].x, im_hi.y, im_lo.y);
+    split_bf16x2(pv[2].y, pv[2].x, im_hi.z, im_lo.z);
+    split_bf16x2(pv[3].y, pv[3].x, im_hi.w, im_lo.w);
+    const size_t img_bytes = (size_t)N1 * K1p * 2;
+    const int row = 2 * u;                                        // rows 2u and 2u+1 sit in the same 8-row core matrix
+    uint8_t* dst = img + (size_t)plane * 2 * img_bytes + (size_t)kc * (N1 * 16) + (size_t)(row >> 3) * 128 + (row & 7) * 16;
+    *reinterpret_cast<uint4*>(dst) = re_hi;
+    *reinterpret_cast<uint4*>(dst + 16) = im_hi;
+    *reinterpret_cast<uint4*>(dst + img_bytes) = re_lo;
+    *reinterpret_cast<uint4*>(dst + img_bytes + 16) = im_lo;
 }
 
 // ---- main kernel ------------------------------------------------------------------------------------
@@ -517,8 +503,7 @@ void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, 
 
 bool tc_synth_partials_supported(int U, int Vn, const TcPartials& parts)
 {
-    const int M = U * Vn;
-    return parts.part && (M + parts.rows_per_tile - 1) / parts.rows_per_tile + 1 <= TS_MAX_PTILES && parts.G <= TS_MAX_SEGS;
+    return parts.part && (int64_t)U * Vn * 3 < (1 << 30);
 }
 
 void launch_tc_synth_group_partials(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const TcPartials& parts,
@@ -530,8 +515,9 @@ void launch_tc_synth_group_partials(scw_ctx* ctx, int U, int Vn, int64_t Fz, int
     uint8_t* B1 = static_cast<uint8_t*>(scratch);
     {
         KernelScope ks(ctx, KC_SYNTH_IMG);
-        k_tc_synth_pimage_partials<<<planes, 256, (size_t)U * Vn * sizeof(float2), ctx->stream>>>(U, Vn, pl.K1p, pl.K2p, Fz,
-                                                                                                 parts, B1);
+        const int items = (pl.K1p / 8) * (pl.K2p / 2);
+        const dim3 grid((unsigned)planes, (unsigned)((items + TS_PI_THREADS - 1) / TS_PI_THREADS));
+        k_tc_synth_pimage_partials<<<grid, TS_PI_THREADS, 0, ctx->stream>>>(U, Vn, pl.K1p, pl.K2p, (int)Fz, parts, B1);
     }
     ts_launch_main(ctx, pl, Fz, n_inst, B1, Nx, Ny, tw, E, strides);
 }
