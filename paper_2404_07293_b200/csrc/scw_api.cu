@@ -65,8 +65,6 @@ int32_t check_layer(scw_ctx* ctx, const scw_layer* L, const char* who)
     if (L->struct_size != sizeof(scw_layer))
         return fail(ctx, SCW_ERR_SHAPE, "%s: layer.struct_size %u != %zu", who, L->struct_size, sizeof(scw_layer));
     if (L->dtype != SCW_C64 && L->dtype != SCW_C128) return fail(ctx, SCW_ERR_DTYPE, "%s: bad dtype %d", who, L->dtype);
-    if (ctx && ctx->path == SCW_PATH_TENSOR && L->dtype != SCW_C64)
-        return fail(ctx, SCW_ERR_UNSUPPORTED, "%s: SCW_PATH_TENSOR has no complex128 kernels", who);
     if (L->U <= 0 || L->Vn <= 0 || L->U > MAX_FREQ || L->Vn > MAX_FREQ)
         return fail(ctx, SCW_ERR_SHAPE, "%s: U=%d Vn=%d out of range", who, L->U, L->Vn);
     if (L->J <= 0) return fail(ctx, SCW_ERR_SHAPE, "%s: J=%lld must be positive", who, (long long)L->J);
@@ -105,10 +103,15 @@ bool use_tc_assemble(const scw_ctx* ctx, const scw_layer* L, int64_t Fz)
     return 2 * R >= 128 && L->J >= 64;
 }
 
+// complex128 runs on the FP64 tensor cores (DMMA) unless the ctx is pinned to the CUDA-core path
+bool use_dmma(const scw_ctx* ctx, int dtype) { return ctx->path != SCW_PATH_SIMT && dmma_supported(dtype); }
+
 size_t assemble_ws(const scw_ctx* ctx, const scw_layer* L, int64_t Fz)
 {
     const int64_t R = 3LL * L->U * L->Vn;
     if (use_tc_assemble(ctx, L, Fz)) return tc_assemble_scratch(R, L->J, Fz, 1, ctx->sm_count);
+    if (use_dmma(ctx, L->dtype))
+        return align_up((size_t)L->J * Fz * esize(L->dtype)) + dmma_assemble_scratch(R, L->J, Fz, ctx->sm_count);
     return align_up((size_t)L->J * Fz * esize(L->dtype)) + simt_assemble_scratch(L->dtype, R, L->J, Fz, ctx->sm_count);
 }
 
@@ -121,6 +124,12 @@ void run_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z,
         return;
     }
     void* W = cv.take((size_t)L->J * Fz * esize(L->dtype));
+    if (use_dmma(ctx, L->dtype)) {
+        void* scratch = cv.take(dmma_assemble_scratch(R, L->J, Fz, ctx->sm_count));
+        launch_mode_weights(ctx, L->dtype, L->J, Fz, L->lambda, L->z_lo, L->z_hi, L->c, L->gamma, L->dir, z, W);
+        launch_dmma_assemble(ctx, R, L->J, Fz, L->V, L->ldV, W, P, ldP, scratch);
+        return;
+    }
     void* scratch = cv.take(simt_assemble_scratch(L->dtype, R, L->J, Fz, ctx->sm_count));
     launch_mode_weights(ctx, L->dtype, L->J, Fz, L->lambda, L->z_lo, L->z_hi, L->c, L->gamma, L->dir, z, W);
     launch_simt_assemble(ctx, L->dtype, R, L->J, Fz, L->V, L->ldV, W, P, ldP, scratch);
@@ -173,6 +182,7 @@ void run_synth(scw_ctx* ctx, const Twiddles& t, int dtype, int U, int Vn, int64_
                int64_t Nx, int64_t Ny, void* E, const int64_t s4[4], void* scratch)
 {
     if (t.tc) launch_tc_synth(ctx, U, Vn, Fz, P, ldP, Nx, Ny, t.a, E, s4, scratch);
+    else if (use_dmma(ctx, dtype)) launch_dmma_synth(ctx, U, Vn, Fz, P, ldP, Nx, t.a, Ny, t.b, E, s4, scratch);
     else launch_simt_synth(ctx, dtype, U, Vn, Fz, P, ldP, Nx, t.a, Ny, t.b, E, s4, scratch);
 }
 
@@ -266,7 +276,8 @@ const char* scw_profile_name(int32_t kc)
 {
     static const char* names[KC_COUNT] = {"mode_weights", "twiddles", "simt_assemble", "reduce_splits", "simt_synth_a",
                                           "simt_synth_b", "points_table", "points_planewave", "point_synth", "misc",
-                                          "tc_assemble", "tc_synth", "tc_synth_images"};
+                                          "tc_assemble", "tc_synth", "tc_synth_images", "dmma_assemble", "dmma_synth_a",
+                                          "dmma_synth_b"};
     return (kc >= 0 && kc < KC_COUNT) ? names[kc] : nullptr;
 }
 
@@ -361,7 +372,7 @@ int32_t scw_synthesize_grid(scw_ctx* ctx, int32_t dtype, int32_t U, int32_t Vn, 
     if (strides) memcpy(s4, strides, sizeof(s4)); else planar_strides(Nx, Ny, s4);
     for (int i = 0; i < 4; ++i)
         if (s4[i] < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_synthesize_grid: negative stride");
-    if (ctx->path == SCW_PATH_TENSOR && !tc_synth_supported(dtype, U, Vn))
+    if (ctx->path == SCW_PATH_TENSOR && !tc_synth_supported(dtype, U, Vn) && !dmma_supported(dtype))
         return fail(ctx, SCW_ERR_UNSUPPORTED, "scw_synthesize_grid: no tensor-core synthesis for this dtype / frequency count");
     if (int32_t s = need_ws(ctx, twiddle_ws(ctx, dtype, U, Vn, Nx, Ny) + synth_ws(ctx, dtype, U, Vn, Fz, Ny), "scw_synthesize_grid")) return s;
     Carver cv(ctx->ws);

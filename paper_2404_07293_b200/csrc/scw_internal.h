@@ -10,7 +10,7 @@ namespace scw {
 // Kernel classes for launch accounting and the optional per-kernel CUDA-event timers.
 enum KernelClass {
     KC_WEIGHTS = 0, KC_TWIDDLES, KC_ASSEMBLE, KC_REDUCE, KC_SYNTH_A, KC_SYNTH_B, KC_POINTS_TABLE, KC_POINTS,
-    KC_POINT_SYNTH, KC_MISC, KC_ASSEMBLE_TC, KC_SYNTH_TC, KC_SYNTH_IMG, KC_COUNT
+    KC_POINT_SYNTH, KC_MISC, KC_ASSEMBLE_TC, KC_SYNTH_TC, KC_SYNTH_IMG, KC_ASSEMBLE_DMMA, KC_SYNTH_A_DMMA, KC_SYNTH_B_DMMA, KC_COUNT
 };
 struct ProfRec { cudaEvent_t a, b; int kc; };
 }  // namespace scw
@@ -134,6 +134,16 @@ void launch_tc_synth_group_partials(scw_ctx* ctx, int U, int Vn, int64_t Fz, int
                                     void* scratch);
 void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,
                      const void* tw, void* E, const int64_t strides[4], void* scratch);
+
+// ---- scw_dmma.cu: FP64 tensor-core (DMMA mma.sync) batched complex GEMM for the complex128 contractions -----------
+bool dmma_supported(int dtype);
+size_t dmma_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int sm_count);
+// P = V W with W[j*Fz + i] from launch_mode_weights; scratch from dmma_assemble_scratch
+void launch_dmma_assemble(scw_ctx* ctx, int64_t R, int64_t J, int64_t Fz, const void* V, int64_t ldV, const void* W,
+                          void* P, int64_t ldP, void* scratch);
+// two-pass synthesis with the frequency-major tables of launch_twiddles; scratch = simt_synth_scratch(SCW_C128, ...)
+void launch_dmma_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, const void* FxT,
+                       int64_t Ny, const void* FyT, void* E, const int64_t strides[4], void* scratch);
 
 // ---- points.cu ------------------------------------------------------------------------------
 struct PwTableInfo { size_t bytes; };

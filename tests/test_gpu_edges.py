@@ -45,12 +45,23 @@ def ragged_layer(U, Vn, J, dtype, seed, ldV_pad=0, with_c=True, with_dir=True):
                 dir=dirs if with_dir else None)
 
 
+@pytest.fixture(scope="module")
+def ctx_simt(scw):
+    c = scw.Context(0)
+    c.set_path(scw.SCW_PATH_SIMT)
+    yield c
+    c.close()
+
+
+@pytest.mark.parametrize("path", ["auto", "simt"])
 @pytest.mark.parametrize("dtype,tol", [(np.complex64, 2e-4), (np.complex128, 1e-10)])
 @pytest.mark.parametrize("U,Vn,J,Nx,Ny,Fz", [(5, 3, 17, 37, 21, 3), (1, 1, 4, 5, 130, 1), (4, 6, 96, 129, 7, 35),
                                              (7, 2, 56, 300, 3, 18)])
-def test_ragged_shapes_padding_and_defaults(scw, ctx, dtype, tol, U, Vn, J, Nx, Ny, Fz):
+def test_ragged_shapes_padding_and_defaults(scw, ctx, ctx_simt, path, dtype, tol, U, Vn, J, Nx, Ny, Fz):
     """Odd/even frequency counts, J not 4M, padded ldV/ldP, c = NULL, dir = NULL, non-uniform x/y,
-    z outside the layer: every sample against Tier A."""
+    z outside the layer: every sample against Tier A.  path "auto": complex128 on the DMMA kernels, complex64 on
+    tcgen05 where a tile fits; "simt": the CUDA-core kernels for both."""
+    ctx = ctx if path == "auto" else ctx_simt
     lay = ragged_layer(U, Vn, J, dtype, seed=U * 100 + J, ldV_pad=3, with_c=(J % 2 == 0), with_dir=(J % 3 == 0))
     g = np.random.default_rng(5)
     x = np.sort(g.uniform(-4, 7, Nx))
