@@ -8,10 +8,14 @@
 //                                                                  B1 = the plane's spectrum in "complex as real" form
 //          -> D1 row y holds T[u, y] = sum_v P[u,v] Fy[y,v] as (Re, Im) pairs
 //   GEMM2  D2[x, 2y+c]        = sum_k A2[x, k] B2[2y+c, k]        A2 = (Fx_r, Fx_i), B2 built from D1 in-kernel
+// The frequencies are cut into chunks of at most 40 (K <= 80 per GEMM): GEMM1 accumulates the v chunks into D1,
+// GEMM2 accumulates the u chunks into D2, so up to 80 x 80 frequencies run in one pass over the output.
+// A1 (all v chunks) sits in shared memory; A2 (all u chunks) is written ONCE into TMEM and GEMM2 runs in TS mode
+// (A from TMEM, B from shared memory), which halves the shared-memory operand traffic of the dominant GEMM.
 // The 128 converter threads read their own D1 row from TMEM (tcgen05.ld), split it to bf16 hi/lo and write the two
 // B2 rows (y,Re), (y,Im) of the K-major UMMA image; the 128 epilogue threads read D2 (lane = x) and store
 // (Re, Im) pairs straight to E: a warp writes 256 contiguous bytes per y.  Twiddle and spectrum images are
-// produced by two small pre-kernels in fp64 / fp32 and fetched with bulk async copies.
+// produced by two small pre-kernels and fetched with bulk async copies.
 #include "scw_internal.h"
 #include "scw_tc_common.cuh"
 
@@ -20,83 +24,111 @@ namespace scw {
 using namespace tc;
 
 constexpr int TS_TILE = 128;               // output tile edge (x and y)
-constexpr int TS_KMAX = 80;                // max padded K (= 2U, 2V rounded up to 16)
+constexpr int TS_KMAX = 80;                // max padded K per chunk (= 2*chunk rounded up to 16)
+constexpr int TS_FMAX = 80;                // max frequencies per axis (two chunks)
 constexpr int TS_THREADS = 18 * 32;        // loader, MMA, 8 converter warps, 8 epilogue warps
 constexpr int TS_TMEM_COLS = 512;
 constexpr int TS_D2_COL = 0;               // D2[h] at columns h*128
-constexpr int TS_D1_COL = 256;             // D1 at columns 256..256+N1
+constexpr int TS_D1_COL = 256;             // D1 at columns 256..256+N1, then A2 (per u chunk: hi K2p/2 | lo K2p/2 columns)
 constexpr int TS_MAX_INST = 64;            // instances per grouped launch
 
 #ifdef SCW_TS_DEBUG
 __device__ long long g_ts_dbg[4096];
-#define TS_MARK(slot) do { if (blockIdx.x == 0) g_ts_dbg[(slot)] = clock64(); } while (0)
+#define TS_MARK(slot) do { if (blockIdx.x == 0 && (slot) < 4096) g_ts_dbg[(slot)] = clock64(); } while (0)
 #else
 #define TS_MARK(slot) do { } while (0)
 #endif
 
 struct TsParams {
-    const uint8_t* A1;     // [ty][hi|lo] images of (Fy_r, Fy_i): 128 rows x K1p, K-major, LBO = 2048, SBO = 128
-    const uint8_t* A2;     // [tx][hi|lo] images of (Fx_r, Fx_i): 128 rows x K2p
-    const uint8_t* B1;     // [plane][hi|lo] images: N1 rows x K1p, LBO = N1*16, SBO = 128
+    const uint8_t* A1;     // [ty][vc][hi|lo] images of (Fy_r, Fy_i): 128 rows x K1p, K-major, LBO = 2048, SBO = 128
+    const uint32_t* A2;    // [tx][uc][row][hi K2p/2 | lo K2p/2] packed bf16 pairs (cos, sin) of Fx: TMEM A-operand rows
+    const uint8_t* B1;     // [plane][uc][vc][hi|lo] images: N1 rows x K1p, LBO = N1*16, SBO = 128
     float2* E[TS_MAX_INST];   // output of every instance of the group
     int64_t s_comp, s_z, s_y, s_x;
     int64_t Nx, Ny;
     int planes;            // n_inst * Fz * 3 (global plane id = inst * planes_per_inst + n*3 + comp)
     int planes_per_inst;
-    int K1p, K2p;          // padded 2V, 2U  (N1 == K2p)
+    int K1p, K2p;          // padded 2*Vc, 2*Uc  (N1 == K2p)
+    int nuc, nvc;          // frequency chunks along u and v
     int tiles_x, tiles_y, pair0, npairs;   // this launch covers tile pairs [pair0, pair0 + npairs)
 };
 
 __host__ __device__ inline int ts_pad16(int v) { return (v + 15) / 16 * 16; }
 
+// Chunking of one frequency axis: n chunks of `len` frequencies (the last may be shorter), padded K = Kp.
+struct TsChunks { int n, len, Kp; };
+__host__ __device__ inline TsChunks ts_chunks(int nfreq)
+{
+    TsChunks c;
+    c.n = (2 * nfreq + TS_KMAX - 1) / TS_KMAX;
+    c.len = (nfreq + c.n - 1) / c.n;
+    c.Kp = ts_pad16(2 * c.len);
+    return c;
+}
+
 // ---- pre-kernels ------------------------------------------------------------------------------------
-// Twiddle images (a-3): for tile t, row r (coordinate index t*128 + r), k = 2f + c: c = 0 -> cos, c = 1 -> sin of
-// 2 pi (f - nfreq/2) coord / period; rows past N and k past 2*nfreq are zero.  hi image then lo image per tile.
-struct TwAxis { int nfreq, Kp, tiles; int64_t N; const double* coord; double inv_period; uint8_t* img; };
+// Twiddle operands (a-3) in one launch.  y axis: K-major UMMA images, for tile t, chunk ch, row r (coordinate index
+// t*128 + r), k = 2f + c: c = 0 -> cos, c = 1 -> sin of 2 pi (ch*len + f - nfreq/2) coord / period; rows past N and
+// frequencies past the axis are zero; hi image then lo image.  x axis: the same values as TMEM A-operand rows,
+// row = [hi: Kp/2 words | lo: Kp/2 words], word f = bf16 pair (cos, sin).
+struct TwAxis { int nfreq, nch, len, Kp, tiles; int64_t N; const double* coord; double inv_period; void* out; };
 
 __global__ void k_tc_synth_twiddles(const TwAxis ay, const TwAxis ax, int blocks_y)
 {
     const bool is_y = (int)blockIdx.x < blocks_y;                            // one launch covers both axes
     const TwAxis& a = is_y ? ay : ax;
-    const int64_t idx = (int64_t)(blockIdx.x - (is_y ? 0 : blocks_y)) * blockDim.x + threadIdx.x;      // (tile, r, kpair)
+    const int64_t idx = (int64_t)(blockIdx.x - (is_y ? 0 : blocks_y)) * blockDim.x + threadIdx.x;   // (tile, chunk, r, f)
     const int kpairs = a.Kp / 2;
-    if (idx >= (int64_t)a.tiles * TS_TILE * kpairs) return;
+    if (idx >= (int64_t)a.tiles * a.nch * TS_TILE * kpairs) return;
     const int f = (int)(idx % kpairs);
     const int64_t tr = idx / kpairs;
     const int r = (int)(tr % TS_TILE);
-    const int t = (int)(tr / TS_TILE);
+    const int tc_ = (int)(tr / TS_TILE);                                      // tile * nch + chunk
+    const int ch = tc_ % a.nch, t = tc_ / a.nch;
     const int64_t i = (int64_t)t * TS_TILE + r;
+    const int fg = ch * a.len + f;
     float co = 0.f, si = 0.f;
-    if (f < a.nfreq && i < a.N) {
-        double ph = (double)(f - a.nfreq / 2) * (a.coord[i] * a.inv_period);   // turns, reduced in fp64; the bf16 hi/lo
+    if (f < a.len && fg < a.nfreq && i < a.N) {
+        double ph = (double)(fg - a.nfreq / 2) * (a.coord[i] * a.inv_period);  // turns, reduced in fp64; the bf16 hi/lo
         ph -= rint(ph);                                                         // split below keeps 2^-17: fp32 sincospi
         sincospif((float)(2.0 * ph), &si, &co);
     }
     uint32_t hi, lo;
     split_bf16x2(co, si, hi, lo);
-    const int k = 2 * f;
-    const size_t img_bytes = (size_t)TS_TILE * a.Kp * 2;
-    uint8_t* base = a.img + (size_t)t * 2 * img_bytes;
-    const size_t off = (size_t)(k >> 3) * 2048 + (size_t)(r >> 3) * 128 + (r & 7) * 16 + (k & 7) * 2;
-    *reinterpret_cast<uint32_t*>(base + off) = hi;
-    *reinterpret_cast<uint32_t*>(base + img_bytes + off) = lo;
+    if (is_y) {
+        const int k = 2 * f;
+        const size_t img_bytes = (size_t)TS_TILE * a.Kp * 2;
+        uint8_t* base = static_cast<uint8_t*>(a.out) + (size_t)tc_ * 2 * img_bytes;
+        const size_t off = (size_t)(k >> 3) * 2048 + (size_t)(r >> 3) * 128 + (r & 7) * 16 + (k & 7) * 2;
+        *reinterpret_cast<uint32_t*>(base + off) = hi;
+        *reinterpret_cast<uint32_t*>(base + img_bytes + off) = lo;
+    } else {
+        uint32_t* row = static_cast<uint32_t*>(a.out) + ((size_t)tc_ * TS_TILE + r) * a.Kp;
+        row[f] = hi;
+        row[kpairs + f] = lo;
+    }
 }
 
-// Spectrum images: plane = n*3 + comp, row = 2u + c, k = 2v + c'':
-//   row (u,Re): (P_r, -P_i);  row (u,Im): (P_i, P_r)   so that  D1[y, (u,c)] = sum_v Fy[y,v] P[u,v]  in real arithmetic.
-__global__ void k_tc_synth_pimage(int U, int Vn, int K1p, int N1, int planes, const float2* __restrict__ P, int64_t ldP,
-                                  uint8_t* __restrict__ img)
+// Spectrum images: image (plane, uc, vc), plane = n*3 + comp, row = 2ul + c, k = 2vl + c'' with u = uc*Uc + ul,
+// v = vc*Vc + vl:   row (u,Re): (P_r, -P_i);  row (u,Im): (P_i, P_r)
+// so that  D1[y, (u,c)] = sum_v Fy[y,v] P[u,v]  in real arithmetic.
+__global__ void k_tc_synth_pimage(int U, int Vn, int Uc, int Vc, int nuc, int nvc, int K1p, int N1, int planes,
+                                  const float2* __restrict__ P, int64_t ldP, uint8_t* __restrict__ img)
 {
-    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;      // (plane, row, kpair)
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;      // (image, row, kpair)
     const int kpairs = K1p / 2;
-    if (idx >= (int64_t)planes * N1 * kpairs) return;
-    const int v = (int)(idx % kpairs);
+    if (idx >= (int64_t)planes * nuc * nvc * N1 * kpairs) return;
+    const int vl = (int)(idx % kpairs);
     const int64_t pr = idx / kpairs;
     const int row = (int)(pr % N1);
-    const int64_t plane = pr / N1;
-    const int u = row >> 1, c = row & 1;
+    const int64_t image = pr / N1;
+    const int vc = (int)(image % nvc);
+    const int uc = (int)((image / nvc) % nuc);
+    const int64_t plane = image / (nvc * nuc);
+    const int ul = row >> 1, c = row & 1;
+    const int u = uc * Uc + ul, v = vc * Vc + vl;
     float a = 0.f, b = 0.f;
-    if (u < U && v < Vn) {
+    if (ul < Uc && vl < Vc && u < U && v < Vn) {
         const int64_t n = plane / 3;
         const int comp = (int)(plane - n * 3);
         const float2 p = P[n * ldP + (int64_t)comp * U * Vn + (int64_t)v * U + u];
@@ -105,29 +137,33 @@ __global__ void k_tc_synth_pimage(int U, int Vn, int K1p, int N1, int planes, co
     }
     uint32_t hi, lo;
     split_bf16x2(a, b, hi, lo);
-    const int k = 2 * v;
+    const int k = 2 * vl;
     const size_t img_bytes = (size_t)N1 * K1p * 2;
-    uint8_t* base = img + (size_t)plane * 2 * img_bytes;
+    uint8_t* base = img + (size_t)image * 2 * img_bytes;
     const size_t off = (size_t)(k >> 3) * (N1 * 16) + (size_t)(row >> 3) * 128 + (row & 7) * 16 + (k & 7) * 2;
     *reinterpret_cast<uint32_t*>(base + off) = hi;
     *reinterpret_cast<uint32_t*>(base + img_bytes + off) = lo;
 }
 
-// Spectrum images straight from the stream-K partial tiles of the assembly (TcPartials): thread = (plane, 8-wide
-// k chunk kc, frequency u) sums the segments of its four spectrum entries P[u, 4kc..4kc+3] in the table's fixed order
-// (deterministic) and writes the 16-byte chunks of image rows (u,Re) and (u,Im), hi and lo -- P itself never goes to
-// memory.  Lanes run along u: loads of one v are contiguous, a warp's stores cover 1 KB of the image.
+// Spectrum images straight from the stream-K partial tiles of the assembly (TcPartials): thread = (image (plane, uc,
+// vc), 8-wide k chunk kc, local frequency ul) sums the segments of its four spectrum entries P[u, v0..v0+3] in the
+// table's fixed order (deterministic) and writes the 16-byte chunks of image rows (ul,Re) and (ul,Im), hi and lo --
+// P itself never goes to memory.  Lanes run along u: loads of one v are contiguous, a warp's stores cover 1 KB.
 constexpr int TS_PI_THREADS = 128;
 
-__global__ void __launch_bounds__(TS_PI_THREADS) k_tc_synth_pimage_partials(int U, int Vn, int K1p, int N1, int Fz,
+__global__ void __launch_bounds__(TS_PI_THREADS) k_tc_synth_pimage_partials(int U, int Vn, int Uc, int Vc, int nuc, int nvc,
+                                                                            int K1p, int N1, int Fz,
                                                                             const __grid_constant__ TcPartials tp,
                                                                             uint8_t* __restrict__ img)
 {
-    const int plane = blockIdx.x;                                 // inst*Fz*3 + n*3 + comp
-    const int item = blockIdx.y * TS_PI_THREADS + threadIdx.x;    // kc * (N1/2) + u
+    const int image = blockIdx.x;                                 // (plane * nuc + uc) * nvc + vc
+    const int item = blockIdx.y * TS_PI_THREADS + threadIdx.x;    // kc * (N1/2) + ul
     const int half = N1 / 2, kchunks = K1p / 8;
     if (item >= kchunks * half) return;
-    const int kc = item / half, u = item - kc * half;
+    const int kc = item / half, ul = item - kc * half;
+    const int vc = image % nvc, puc = image / nvc;
+    const int uc = puc % nuc, plane = puc / nuc;                  // plane = inst*Fz*3 + n*3 + comp
+    const int u = uc * Uc + ul;
     const int M = U * Vn;
     const int pz = plane / 3, comp = plane - pz * 3;
     const int inst = pz / Fz, n = pz - inst * Fz;
@@ -138,9 +174,9 @@ __global__ void __launch_bounds__(TS_PI_THREADS) k_tc_synth_pimage_partials(int 
     float2 pv[4];
 #pragma unroll
     for (int e = 0; e < 4; ++e) {
-        const int v = 4 * kc + e;
+        const int vl = 4 * kc + e, v = vc * Vc + vl;
         pv[e] = make_float2(0.f, 0.f);
-        if (u < U && v < Vn) {
+        if (ul < Uc && vl < Vc && u < U && v < Vn) {
             const int row = comp * M + v * U + u;
             const int mt = row / rpt, r = row - mt * rpt;
             const int tile = tile_base + mt;
@@ -165,8 +201,8 @@ __global__ void __launch_bounds__(TS_PI_THREADS) k_tc_synth_pimage_partials(int 
     split_bf16x2(pv[2].y, pv[2].x, im_hi.z, im_lo.z);
     split_bf16x2(pv[3].y, pv[3].x, im_hi.w, im_lo.w);
     const size_t img_bytes = (size_t)N1 * K1p * 2;
-    const int row = 2 * u;                                        // rows 2u and 2u+1 sit in the same 8-row core matrix
-    uint8_t* dst = img + (size_t)plane * 2 * img_bytes + (size_t)kc * (N1 * 16) + (size_t)(row >> 3) * 128 + (row & 7) * 16;
+    const int row = 2 * ul;                                       // rows 2ul and 2ul+1 sit in the same 8-row core matrix
+    uint8_t* dst = img + (size_t)image * 2 * img_bytes + (size_t)kc * (N1 * 16) + (size_t)(row >> 3) * 128 + (row & 7) * 16;
     *reinterpret_cast<uint4*>(dst) = re_hi;
     *reinterpret_cast<uint4*>(dst + 16) = im_hi;
     *reinterpret_cast<uint4*>(dst + img_bytes) = re_lo;
@@ -174,11 +210,11 @@ __global__ void __launch_bounds__(TS_PI_THREADS) k_tc_synth_pimage_partials(int 
 }
 
 // ---- main kernel ------------------------------------------------------------------------------------
-// Three-product bf16 GEMM step over K = Kp: D (+)= Ahi*Bhi + Ahi*Blo + Alo*Bhi.
-__device__ __forceinline__ void ts_mma3(uint32_t d_tmem, uint32_t a_hi, uint32_t a_lo, uint32_t a_lbo, uint32_t b_hi,
-                                        uint32_t b_lo, uint32_t b_lbo, int Kp, uint32_t idesc)
+// Three-product bf16 GEMM step over K = Kp: D (+)= Ahi*Bhi + Ahi*Blo + Alo*Bhi.  `acc` = accumulate onto D.
+// SS form: both operands are K-major shared-memory images.
+__device__ __forceinline__ void ts_mma3_ss(uint32_t d_tmem, uint32_t a_hi, uint32_t a_lo, uint32_t a_lbo, uint32_t b_hi,
+                                           uint32_t b_lo, uint32_t b_lbo, int Kp, uint32_t idesc, uint32_t acc)
 {
-    uint32_t acc = 0;
     for (int s = 0; s < Kp / 16; ++s) {
         const uint64_t da_hi = umma_desc(a_hi + s * 2 * a_lbo, a_lbo, 128);
         const uint64_t da_lo = umma_desc(a_lo + s * 2 * a_lbo, a_lbo, 128);
@@ -190,17 +226,29 @@ __device__ __forceinline__ void ts_mma3(uint32_t d_tmem, uint32_t a_hi, uint32_t
         umma_bf16(d_tmem, da_hi, db_hi, idesc, 1);
     }
 }
+// TS form: A is a TMEM block (column c = bf16 pair k = 2c, 2c+1; hi at ta_hi, lo at ta_lo), B a shared-memory image.
+__device__ __forceinline__ void ts_mma3_ts(uint32_t d_tmem, uint32_t ta_hi, uint32_t ta_lo, uint32_t b_hi, uint32_t b_lo,
+                                           uint32_t b_lbo, int Kp, uint32_t idesc, uint32_t acc)
+{
+    for (int s = 0; s < Kp / 16; ++s) {
+        const uint64_t db_hi = umma_desc(b_hi + s * 2 * b_lbo, b_lbo, 128);
+        const uint64_t db_lo = umma_desc(b_lo + s * 2 * b_lbo, b_lbo, 128);
+        umma_bf16_ts(d_tmem, ta_lo + 8 * s, db_hi, idesc, acc);
+        acc = 1;
+        umma_bf16_ts(d_tmem, ta_hi + 8 * s, db_lo, idesc, 1);
+        umma_bf16_ts(d_tmem, ta_hi + 8 * s, db_hi, idesc, 1);
+    }
+}
 
 __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constant__ TsParams p)
 {
     extern __shared__ __align__(1024) uint8_t smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int K1p = p.K1p, K2p = p.K2p, N1 = p.K2p;
-    const uint32_t a1_img = TS_TILE * K1p * 2, a2_img = TS_TILE * K2p * 2;     // bytes of one (hi or lo) image
+    const int K1p = p.K1p, K2p = p.K2p, N1 = p.K2p, nuc = p.nuc, nvc = p.nvc;
+    const uint32_t a1_img = TS_TILE * K1p * 2;                                 // bytes of one (hi or lo) image
     const uint32_t b1_img = (uint32_t)N1 * K1p * 2, b2_img = TS_TILE * K2p * 2;
-    uint8_t* sA1 = smem;                              // hi | lo
-    uint8_t* sA2 = sA1 + 2 * a1_img;
-    uint8_t* sB1 = sA2 + 2 * a2_img;                  // 2 stages x (hi | lo)
+    uint8_t* sA1 = smem;                              // nvc x (hi | lo)
+    uint8_t* sB1 = sA1 + (size_t)nvc * 2 * a1_img;    // 2 stages x (hi | lo)
     uint8_t* sB2 = sB1 + 4 * b1_img;                  // 2 halves x (hi | lo)
     uint64_t* bars = reinterpret_cast<uint64_t*>(sB2 + 4 * b2_img);
     uint64_t* tw_full = bars;            // [1]
@@ -233,26 +281,53 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
+    const uint32_t a2_col = TS_D1_COL + N1;                    // A2 chunk uc: hi at a2_col + uc*K2p, lo K2p/2 columns on
 
     // this CTA's tile pair and plane sequence
     const int per_pair = gridDim.x / p.npairs;                 // CTAs per pair (gridDim.x is a multiple of npairs)
     const int pair = p.pair0 + (int)blockIdx.x % p.npairs;
     const int first_plane = (int)blockIdx.x / p.npairs;
     const int tx = pair % p.tiles_x, ty = pair / p.tiles_x;
-    const int n_items = first_plane < p.planes ? (p.planes - first_plane + per_pair - 1) / per_pair : 0;
+    const int n_planes = first_plane < p.planes ? (p.planes - first_plane + per_pair - 1) / per_pair : 0;
+    const int n_items = n_planes * nuc;                        // item = (plane, u chunk)
+
+    // A2 (the x twiddles of this tile, every u chunk) goes to TMEM once: the converter warp pair of lane quarter q
+    // writes rows 32q..32q+31, warp kg = 0 the hi words, kg = 1 the lo words
+    if (warp >= 2 && warp < 10 && n_items > 0) {
+        const int q = warp & 3, kg = (warp - 2) >> 2;
+        const int half = K2p / 2;
+        for (int uc = 0; uc < nuc; ++uc) {
+            const uint4* src = reinterpret_cast<const uint4*>(p.A2 + (((size_t)tx * nuc + uc) * TS_TILE + 32 * q + lane) * K2p +
+                                                              kg * half);
+            const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + a2_col + uc * K2p + kg * half;
+            for (int c8 = 0; c8 < half / 8; ++c8) {
+                const uint4 v0 = src[2 * c8], v1 = src[2 * c8 + 1];
+                const uint32_t r[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
+                tmem_st8(taddr + 8 * c8, r);
+            }
+        }
+        tmem_st_wait();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
 
     if (warp == 0) {
-        // ===== loader: twiddle images once, then one spectrum image per plane =====
+        // ===== loader: y twiddle images once, then the nvc spectrum images of every item =====
         if (lane == 0 && n_items > 0) {
-            mbar_expect_tx(tw_full, 2 * a1_img + 2 * a2_img);
-            bulk_g2s(sA1, p.A1 + (size_t)ty * 2 * a1_img, 2 * a1_img, tw_full);
-            bulk_g2s(sA2, p.A2 + (size_t)tx * 2 * a2_img, 2 * a2_img, tw_full);
-            for (int n = 0; n < n_items; ++n) {
-                const int s = n & 1;
-                const int plane = first_plane + n * per_pair;
-                mbar_wait(&b1_empty[s], ((n >> 1) & 1) ^ 1);
-                mbar_expect_tx(&b1_full[s], 2 * b1_img);
-                bulk_g2s(sB1 + (size_t)s * 2 * b1_img, p.B1 + (size_t)plane * 2 * b1_img, 2 * b1_img, &b1_full[s]);
+            mbar_expect_tx(tw_full, nvc * 2 * a1_img);
+            bulk_g2s(sA1, p.A1 + (size_t)ty * nvc * 2 * a1_img, nvc * 2 * a1_img, tw_full);
+            int q = 0;
+            for (int i = 0; i < n_items; ++i) {
+                const int n = i / nuc, uc = i - n * nuc;
+                const size_t plane = (size_t)first_plane + (size_t)n * per_pair;
+                for (int vc = 0; vc < nvc; ++vc, ++q) {
+                    const int s = q & 1;
+                    mbar_wait(&b1_empty[s], ((q >> 1) & 1) ^ 1);
+                    mbar_expect_tx(&b1_full[s], 2 * b1_img);
+                    bulk_g2s(sB1 + (size_t)s * 2 * b1_img, p.B1 + ((plane * nuc + uc) * nvc + vc) * 2 * b1_img, 2 * b1_img,
+                             &b1_full[s]);
+                }
             }
         }
     } else if (warp == 1) {
@@ -260,38 +335,42 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
         if (lane == 0 && n_items > 0) {
             const uint32_t idesc1 = umma_idesc_bf16(TS_TILE, N1);
             const uint32_t idesc2 = umma_idesc_bf16(TS_TILE, TS_TILE);
-            const uint32_t a1 = smem_u32(sA1), a2 = smem_u32(sA2), b1 = smem_u32(sB1), b2 = smem_u32(sB2);
+            const uint32_t a1 = smem_u32(sA1), b1 = smem_u32(sB1), b2 = smem_u32(sB2);
             const uint32_t d1 = tmem_base + TS_D1_COL;
             mbar_wait(tw_full, 0);
-            auto issue_gemm1 = [&](int n) {
-                const int s = n & 1;
-                mbar_wait(&b1_full[s], (n >> 1) & 1);
-                if (n > 0) mbar_wait(d1_empty, (n - 1) & 1);
-                tc_fence_after();
-                TS_MARK(n * 32 + 0);
-                ts_mma3(d1, a1, a1 + a1_img, 2048, b1 + s * 2 * b1_img, b1 + s * 2 * b1_img + b1_img, (uint32_t)N1 * 16, K1p,
-                        idesc1);
+            auto issue_gemm1 = [&](int i) {            // D1 = sum over the v chunks of item i
+                for (int vc = 0; vc < nvc; ++vc) {
+                    const int q = i * nvc + vc, s = q & 1;
+                    mbar_wait(&b1_full[s], (q >> 1) & 1);
+                    if (vc == 0 && i > 0) mbar_wait(d1_empty, (i - 1) & 1);
+                    tc_fence_after();
+                    TS_MARK(i * 32 + 0);
+                    ts_mma3_ss(d1, a1 + vc * 2 * a1_img, a1 + vc * 2 * a1_img + a1_img, 2048, b1 + s * 2 * b1_img,
+                               b1 + s * 2 * b1_img + b1_img, (uint32_t)N1 * 16, K1p, idesc1, vc > 0 ? 1u : 0u);
+                    umma_commit(&b1_empty[s]);
+                }
                 umma_commit(d1_full);
-                umma_commit(&b1_empty[s]);
-                TS_MARK(n * 32 + 1);
+                TS_MARK(i * 32 + 1);
             };
-            auto issue_gemm2 = [&](int n, int h) {
-                mbar_wait(&b2_full[h], n & 1);
-                TS_MARK(n * 32 + 2 + 4 * h);
-                mbar_wait(&d2_empty[h], (n & 1) ^ 1);
+            auto issue_gemm2 = [&](int i, int h) {     // D2[h] (+)= A2[uc] B2[h]; complete after the last u chunk
+                const int n = i / nuc, uc = i - n * nuc;
+                mbar_wait(&b2_full[h], i & 1);
+                TS_MARK(i * 32 + 2 + 4 * h);
+                if (uc == 0) mbar_wait(&d2_empty[h], (n & 1) ^ 1);
                 tc_fence_after();
-                TS_MARK(n * 32 + 3 + 4 * h);
-                ts_mma3(tmem_base + TS_D2_COL + h * TS_TILE, a2, a2 + a2_img, 2048, b2 + h * 2 * b2_img,
-                        b2 + h * 2 * b2_img + b2_img, 2048, K2p, idesc2);
-                umma_commit(&d2_full[h]);
+                TS_MARK(i * 32 + 3 + 4 * h);
+                const uint32_t ta = tmem_base + a2_col + uc * K2p;
+                ts_mma3_ts(tmem_base + TS_D2_COL + h * TS_TILE, ta, ta + K2p / 2, b2 + h * 2 * b2_img,
+                           b2 + h * 2 * b2_img + b2_img, 2048, K2p, idesc2, uc > 0 ? 1u : 0u);
                 umma_commit(&b2_empty[h]);
-                TS_MARK(n * 32 + 4 + 4 * h);
+                if (uc == nuc - 1) umma_commit(&d2_full[h]);
+                TS_MARK(i * 32 + 4 + 4 * h);
             };
             issue_gemm1(0);
-            for (int n = 0; n < n_items; ++n) {
-                issue_gemm2(n, 0);
-                if (n + 1 < n_items) issue_gemm1(n + 1);
-                issue_gemm2(n, 1);
+            for (int i = 0; i < n_items; ++i) {
+                issue_gemm2(i, 0);
+                if (i + 1 < n_items) issue_gemm1(i + 1);
+                issue_gemm2(i, 1);
             }
         }
     } else if (warp < 10) {
@@ -304,7 +383,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
         uint8_t* row = sB2 + (size_t)h * 2 * b2_img + yy * 32;
         const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + TS_D1_COL;
         const int nchunks = K2p / 8;                 // <= 10
-        for (int n = 0; n < n_items; ++n) {
+        for (int n = 0; n < n_items; ++n) {          // n = item (plane, u chunk)
             mbar_wait(d1_full, n & 1);
             tc_fence_after();
             if (warp == 4 && lane == 0) TS_MARK(n * 32 + 10);
@@ -354,7 +433,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
         const int cg = (warp - 10) >> 2;             // which 32-y group of the half
         const int64_t x = (int64_t)tx * TS_TILE + 32 * q + lane;
         const bool x_ok = x < p.Nx;
-        for (int n = 0; n < n_items; ++n) {
+        for (int n = 0; n < n_planes; ++n) {
             const int gplane = first_plane + n * per_pair;
             const int inst = gplane / p.planes_per_inst;
             const int plane = gplane - inst * p.planes_per_inst;
@@ -396,12 +475,8 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
 }
 
 // ---- host side -------------------------------------------------------------------------------------
-bool tc_synth_supported(int dtype, int U, int Vn)
-{
-    return dtype == SCW_C64 && ts_pad16(2 * U) <= TS_KMAX && ts_pad16(2 * Vn) <= TS_KMAX;
-}
-
 struct TsPlan {
+    TsChunks cu, cv;          // frequency chunks along u (GEMM2's K) and v (GEMM1's K)
     int K1p, K2p, tiles_x, tiles_y;
     size_t a1_bytes, a2_bytes, b1_bytes, smem_bytes;
 };
@@ -409,16 +484,26 @@ struct TsPlan {
 static TsPlan ts_plan(int U, int Vn, int64_t Fz, int64_t Nx, int64_t Ny)
 {
     TsPlan pl;
-    pl.K1p = ts_pad16(2 * Vn);
-    pl.K2p = ts_pad16(2 * U);
+    pl.cu = ts_chunks(U);
+    pl.cv = ts_chunks(Vn);
+    pl.K1p = pl.cv.Kp;
+    pl.K2p = pl.cu.Kp;
     pl.tiles_x = (int)((Nx + TS_TILE - 1) / TS_TILE);
     pl.tiles_y = (int)((Ny + TS_TILE - 1) / TS_TILE);
-    pl.a1_bytes = align_up((size_t)pl.tiles_y * 2 * TS_TILE * pl.K1p * 2);
-    pl.a2_bytes = align_up((size_t)pl.tiles_x * 2 * TS_TILE * pl.K2p * 2);
-    pl.b1_bytes = align_up((size_t)Fz * 3 * 2 * pl.K2p * pl.K1p * 2);
-    pl.smem_bytes = (size_t)2 * TS_TILE * pl.K1p * 2 + (size_t)2 * TS_TILE * pl.K2p * 2 +
-                    (size_t)4 * pl.K2p * pl.K1p * 2 + (size_t)4 * TS_TILE * pl.K2p * 2 + 256;
+    pl.a1_bytes = align_up((size_t)pl.tiles_y * pl.cv.n * 2 * TS_TILE * pl.K1p * 2);
+    pl.a2_bytes = align_up((size_t)pl.tiles_x * pl.cu.n * TS_TILE * pl.K2p * 4);
+    pl.b1_bytes = align_up((size_t)Fz * 3 * pl.cu.n * pl.cv.n * 2 * pl.K2p * pl.K1p * 2);
+    pl.smem_bytes = (size_t)pl.cv.n * 2 * TS_TILE * pl.K1p * 2 + (size_t)4 * pl.K2p * pl.K1p * 2 +
+                    (size_t)4 * TS_TILE * pl.K2p * 2 + 256;
     return pl;
+}
+
+// up to TS_FMAX frequencies per axis: TMEM holds D2 (256 columns), D1 (K2p) and A2 (K2p per u chunk)
+bool tc_synth_supported(int dtype, int U, int Vn)
+{
+    if (dtype != SCW_C64 || U > TS_FMAX || Vn > TS_FMAX) return false;
+    const TsPlan pl = ts_plan(U, Vn, 1, 1, 1);
+    return TS_D1_COL + pl.K2p * (1 + pl.cu.n) <= TS_TMEM_COLS && pl.smem_bytes <= 227 * 1024;
 }
 
 size_t tc_synth_twiddle_bytes(int U, int Vn, int64_t Nx, int64_t Ny)
@@ -435,9 +520,10 @@ void launch_tc_synth_twiddles(scw_ctx* ctx, int U, int Vn, double X, double Y, i
     const TsPlan pl = ts_plan(U, Vn, 1, Nx, Ny);
     uint8_t* A1 = static_cast<uint8_t*>(tw);
     uint8_t* A2 = A1 + pl.a1_bytes;
-    const TwAxis ay{Vn, pl.K1p, pl.tiles_y, Ny, y, 1.0 / Y, A1};
-    const TwAxis ax{U, pl.K2p, pl.tiles_x, Nx, x, 1.0 / X, A2};
-    const int64_t ny = (int64_t)pl.tiles_y * TS_TILE * (pl.K1p / 2), nx = (int64_t)pl.tiles_x * TS_TILE * (pl.K2p / 2);
+    const TwAxis ay{Vn, pl.cv.n, pl.cv.len, pl.K1p, pl.tiles_y, Ny, y, 1.0 / Y, A1};
+    const TwAxis ax{U, pl.cu.n, pl.cu.len, pl.K2p, pl.tiles_x, Nx, x, 1.0 / X, A2};
+    const int64_t ny = (int64_t)pl.tiles_y * pl.cv.n * TS_TILE * (pl.K1p / 2);
+    const int64_t nx = (int64_t)pl.tiles_x * pl.cu.n * TS_TILE * (pl.K2p / 2);
     const int by = (int)((ny + 255) / 256), bx = (int)((nx + 255) / 256);
     KernelScope ks(ctx, KC_TWIDDLES);
     k_tc_synth_twiddles<<<by + bx, 256, 0, ctx->stream>>>(ay, ax, by);
@@ -456,7 +542,7 @@ static void ts_launch_main(scw_ctx* ctx, const TsPlan& pl, int64_t Fz, int n_ins
     static thread_local TsParams p;
     const int planes = (int)(Fz * 3 * n_inst);
     p.A1 = static_cast<const uint8_t*>(tw);
-    p.A2 = p.A1 + pl.a1_bytes;
+    p.A2 = reinterpret_cast<const uint32_t*>(p.A1 + pl.a1_bytes);
     p.B1 = B1;
     for (int i = 0; i < n_inst; ++i) p.E[i] = static_cast<float2*>(E[i]);
     p.s_comp = strides[0];
@@ -469,6 +555,8 @@ static void ts_launch_main(scw_ctx* ctx, const TsPlan& pl, int64_t Fz, int n_ins
     p.planes_per_inst = (int)(Fz * 3);
     p.K1p = pl.K1p;
     p.K2p = pl.K2p;
+    p.nuc = pl.cu.n;
+    p.nvc = pl.cv.n;
     p.tiles_x = pl.tiles_x;
     p.tiles_y = pl.tiles_y;
     const int total_pairs = pl.tiles_x * pl.tiles_y;
@@ -494,9 +582,10 @@ void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, 
     uint8_t* B1 = static_cast<uint8_t*>(scratch);
     {
         KernelScope ks(ctx, KC_SYNTH_IMG);
-        const int64_t n = (int64_t)planes * pl.K2p * (pl.K1p / 2);
-        k_tc_synth_pimage<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(U, Vn, pl.K1p, pl.K2p, planes,
-                                                                                (const float2*)P_all, ldP, B1);
+        const int64_t n = (int64_t)planes * pl.cu.n * pl.cv.n * pl.K2p * (pl.K1p / 2);
+        k_tc_synth_pimage<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(U, Vn, pl.cu.len, pl.cv.len, pl.cu.n, pl.cv.n,
+                                                                                pl.K1p, pl.K2p, planes, (const float2*)P_all,
+                                                                                ldP, B1);
     }
     ts_launch_main(ctx, pl, Fz, n_inst, B1, Nx, Ny, tw, E, strides);
 }
@@ -516,8 +605,9 @@ void launch_tc_synth_group_partials(scw_ctx* ctx, int U, int Vn, int64_t Fz, int
     {
         KernelScope ks(ctx, KC_SYNTH_IMG);
         const int items = (pl.K1p / 8) * (pl.K2p / 2);
-        const dim3 grid((unsigned)planes, (unsigned)((items + TS_PI_THREADS - 1) / TS_PI_THREADS));
-        k_tc_synth_pimage_partials<<<grid, TS_PI_THREADS, 0, ctx->stream>>>(U, Vn, pl.K1p, pl.K2p, (int)Fz, parts, B1);
+        const dim3 grid((unsigned)(planes * pl.cu.n * pl.cv.n), (unsigned)((items + TS_PI_THREADS - 1) / TS_PI_THREADS));
+        k_tc_synth_pimage_partials<<<grid, TS_PI_THREADS, 0, ctx->stream>>>(U, Vn, pl.cu.len, pl.cv.len, pl.cu.n, pl.cv.n,
+                                                                            pl.K1p, pl.K2p, (int)Fz, parts, B1);
     }
     ts_launch_main(ctx, pl, Fz, n_inst, B1, Nx, Ny, tw, E, strides);
 }

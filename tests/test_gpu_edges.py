@@ -88,11 +88,13 @@ def test_ragged_shapes_padding_and_defaults(scw, ctx, ctx_simt, path, dtype, tol
 
 
 @pytest.mark.parametrize("U,Vn,J,Fz,pad,n_inst", [(5, 3, 17, 3, 0, 1), (5, 3, 33, 9, 1, 2), (7, 9, 250, 20, 2, 3),
-                                                   (9, 11, 131, 70, 3, 1), (3, 1, 2, 1, 0, 1)])
+                                                   (9, 11, 131, 70, 3, 1), (3, 1, 2, 1, 0, 1),
+                                                   (45, 50, 64, 4, 1, 1), (65, 41, 40, 3, 0, 2), (80, 80, 36, 2, 0, 1)])
 def test_forced_tensor_path_ragged(scw, U, Vn, J, Fz, pad, n_inst):
     """SCW_PATH_TENSOR on shapes that are not multiples of any tile: odd and even ldV (the two TMA column maps),
     rows not a multiple of 128, J not a multiple of 32 (zero-filled boxes), Fz not a multiple of 8 and above one
-    n tile, grouped instances; every sample of every instance against Tier A."""
+    n tile, grouped instances, more than 40 frequencies per axis (two frequency chunks accumulated in TMEM, up to the
+    80 x 80 limit); every sample of every instance against Tier A."""
     c = scw.Context(0)
     c.set_path(scw.SCW_PATH_TENSOR)
     try:
