@@ -35,8 +35,13 @@ constexpr int TS_MAX_INST = 64;            // instances per grouped launch
 #ifdef SCW_TS_DEBUG
 __device__ long long g_ts_dbg[4096];
 #define TS_MARK(slot) do { if (blockIdx.x == 0 && (slot) < 4096) g_ts_dbg[(slot)] = clock64(); } while (0)
+__device__ long long g_ts_blk[4 * 256];
+__device__ __forceinline__ long long ts_gtime() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define TS_BLK(i) do { if (threadIdx.x == 0 && blockIdx.x < 256) g_ts_blk[blockIdx.x * 4 + (i)] = ts_gtime(); } while (0)
+extern "C" void scw_debug_ts_blk(long long* out) { cudaMemcpyFromSymbol(out, g_ts_blk, sizeof(long long) * 1024); }
 #else
 #define TS_MARK(slot) do { } while (0)
+#define TS_BLK(i) do { } while (0)
 #endif
 
 struct TsParams {
@@ -210,33 +215,36 @@ __global__ void __launch_bounds__(TS_PI_THREADS) k_tc_synth_pimage_partials(int 
 }
 
 // ---- main kernel ------------------------------------------------------------------------------------
-// Three-product bf16 GEMM step over K = Kp: D (+)= Ahi*Bhi + Ahi*Blo + Alo*Bhi.  `acc` = accumulate onto D.
-// SS form: both operands are K-major shared-memory images.
+// Three-product bf16 GEMM over K = Kp: D (+)= Ahi*Bhi + Ahi*Blo + Alo*Bhi.  `acc` = accumulate onto D.  The descriptors of
+// k step s are the step-0 descriptors plus a constant (the address field is in 16-byte units), so the issuing
+// thread spends two 64-bit adds per MMA instead of rebuilding descriptors.
+// SS form: both operands are K-major shared-memory images (LBO a_lbo / b_lbo bytes between the 8-wide k chunks).
 __device__ __forceinline__ void ts_mma3_ss(uint32_t d_tmem, uint32_t a_hi, uint32_t a_lo, uint32_t a_lbo, uint32_t b_hi,
                                            uint32_t b_lo, uint32_t b_lbo, int Kp, uint32_t idesc, uint32_t acc)
 {
+    uint64_t da_hi = umma_desc(a_hi, a_lbo, 128), da_lo = umma_desc(a_lo, a_lbo, 128);
+    uint64_t db_hi = umma_desc(b_hi, b_lbo, 128), db_lo = umma_desc(b_lo, b_lbo, 128);
+    const uint64_t a_step = (uint64_t)((2 * a_lbo) >> 4), b_step = (uint64_t)((2 * b_lbo) >> 4);
     for (int s = 0; s < Kp / 16; ++s) {
-        const uint64_t da_hi = umma_desc(a_hi + s * 2 * a_lbo, a_lbo, 128);
-        const uint64_t da_lo = umma_desc(a_lo + s * 2 * a_lbo, a_lbo, 128);
-        const uint64_t db_hi = umma_desc(b_hi + s * 2 * b_lbo, b_lbo, 128);
-        const uint64_t db_lo = umma_desc(b_lo + s * 2 * b_lbo, b_lbo, 128);
         umma_bf16(d_tmem, da_lo, db_hi, idesc, acc);
         acc = 1;
         umma_bf16(d_tmem, da_hi, db_lo, idesc, 1);
         umma_bf16(d_tmem, da_hi, db_hi, idesc, 1);
+        da_hi += a_step; da_lo += a_step; db_hi += b_step; db_lo += b_step;
     }
 }
 // TS form: A is a TMEM block (column c = bf16 pair k = 2c, 2c+1; hi at ta_hi, lo at ta_lo), B a shared-memory image.
 __device__ __forceinline__ void ts_mma3_ts(uint32_t d_tmem, uint32_t ta_hi, uint32_t ta_lo, uint32_t b_hi, uint32_t b_lo,
                                            uint32_t b_lbo, int Kp, uint32_t idesc, uint32_t acc)
 {
+    uint64_t db_hi = umma_desc(b_hi, b_lbo, 128), db_lo = umma_desc(b_lo, b_lbo, 128);
+    const uint64_t b_step = (uint64_t)((2 * b_lbo) >> 4);
     for (int s = 0; s < Kp / 16; ++s) {
-        const uint64_t db_hi = umma_desc(b_hi + s * 2 * b_lbo, b_lbo, 128);
-        const uint64_t db_lo = umma_desc(b_lo + s * 2 * b_lbo, b_lbo, 128);
-        umma_bf16_ts(d_tmem, ta_lo + 8 * s, db_hi, idesc, acc);
+        umma_bf16_ts(d_tmem, ta_lo, db_hi, idesc, acc);
         acc = 1;
-        umma_bf16_ts(d_tmem, ta_hi + 8 * s, db_lo, idesc, 1);
-        umma_bf16_ts(d_tmem, ta_hi + 8 * s, db_hi, idesc, 1);
+        umma_bf16_ts(d_tmem, ta_hi, db_lo, idesc, 1);
+        umma_bf16_ts(d_tmem, ta_hi, db_hi, idesc, 1);
+        ta_hi += 8; ta_lo += 8; db_hi += b_step; db_lo += b_step;
     }
 }
 
@@ -244,6 +252,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
 {
     extern __shared__ __align__(1024) uint8_t smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    TS_BLK(0);
     const int K1p = p.K1p, K2p = p.K2p, N1 = p.K2p, nuc = p.nuc, nvc = p.nvc;
     const uint32_t a1_img = TS_TILE * K1p * 2;                                 // bytes of one (hi or lo) image
     const uint32_t b1_img = (uint32_t)N1 * K1p * 2, b2_img = TS_TILE * K2p * 2;
@@ -311,6 +320,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
+    TS_BLK(1);
 
     if (warp == 0) {
         // ===== loader: y twiddle images once, then the nvc spectrum images of every item =====
@@ -331,8 +341,8 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer =====
-        if (lane == 0 && n_items > 0) {
+        // ===== MMA issuer: the whole warp runs the loop (warp-uniform control flow), one elected lane issues =====
+        if (n_items > 0) {
             const uint32_t idesc1 = umma_idesc_bf16(TS_TILE, N1);
             const uint32_t idesc2 = umma_idesc_bf16(TS_TILE, TS_TILE);
             const uint32_t a1 = smem_u32(sA1), b1 = smem_u32(sB1), b2 = smem_u32(sB2);
@@ -345,11 +355,14 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                     if (vc == 0 && i > 0) mbar_wait(d1_empty, (i - 1) & 1);
                     tc_fence_after();
                     TS_MARK(i * 32 + 0);
-                    ts_mma3_ss(d1, a1 + vc * 2 * a1_img, a1 + vc * 2 * a1_img + a1_img, 2048, b1 + s * 2 * b1_img,
-                               b1 + s * 2 * b1_img + b1_img, (uint32_t)N1 * 16, K1p, idesc1, vc > 0 ? 1u : 0u);
-                    umma_commit(&b1_empty[s]);
+                    if (elect_one()) {
+                        ts_mma3_ss(d1, a1 + vc * 2 * a1_img, a1 + vc * 2 * a1_img + a1_img, 2048, b1 + s * 2 * b1_img,
+                                   b1 + s * 2 * b1_img + b1_img, (uint32_t)N1 * 16, K1p, idesc1, vc > 0 ? 1u : 0u);
+                        umma_commit(&b1_empty[s]);
+                        if (vc == nvc - 1) umma_commit(d1_full);
+                    }
+                    __syncwarp();
                 }
-                umma_commit(d1_full);
                 TS_MARK(i * 32 + 1);
             };
             auto issue_gemm2 = [&](int i, int h) {     // D2[h] (+)= A2[uc] B2[h]; complete after the last u chunk
@@ -360,12 +373,17 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                 tc_fence_after();
                 TS_MARK(i * 32 + 3 + 4 * h);
                 const uint32_t ta = tmem_base + a2_col + uc * K2p;
-                ts_mma3_ts(tmem_base + TS_D2_COL + h * TS_TILE, ta, ta + K2p / 2, b2 + h * 2 * b2_img,
-                           b2 + h * 2 * b2_img + b2_img, 2048, K2p, idesc2, uc > 0 ? 1u : 0u);
-                umma_commit(&b2_empty[h]);
-                if (uc == nuc - 1) umma_commit(&d2_full[h]);
+                if (elect_one()) {
+                    ts_mma3_ts(tmem_base + TS_D2_COL + h * TS_TILE, ta, ta + K2p / 2, b2 + h * 2 * b2_img,
+                               b2 + h * 2 * b2_img + b2_img, 2048, K2p, idesc2, uc > 0 ? 1u : 0u);
+                    umma_commit(&b2_empty[h]);
+                    if (uc == nuc - 1) umma_commit(&d2_full[h]);
+                }
+                __syncwarp();
                 TS_MARK(i * 32 + 4 + 4 * h);
             };
+            // order GEMM2(h=0), GEMM1(next), GEMM2(h=1): measured best -- issuing GEMM1 of the next item first shortens
+            // one CTA's period but widens the spread of CTA finishing times on the HBM-write-bound kernel (77 vs 83 us)
             issue_gemm1(0);
             for (int i = 0; i < n_items; ++i) {
                 issue_gemm2(i, 0);
@@ -471,6 +489,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
     }
     tc_fence_before();
     __syncthreads();
+    TS_BLK(2);
     if (warp == 1) tmem_dealloc(tmem_base, TS_TMEM_COLS);
 }
 
