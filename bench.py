@@ -32,6 +32,7 @@ import scw_inputs as si  # noqa: E402
 METRIC = "field samples/s (complex E 3-vectors)"
 UNIT = "samples/s"
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # CUDA-core FFMA peak at max clock (context only)
+FP64_DMMA_PEAK_TFLOPS = 37.1                           # measured on this pool's B200 (DMMA microbenchmark)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -310,7 +311,13 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
         out = [torch.empty((c1.planes, 3, c1.Ny, c1.Nx), dtype=torch.complex128, device=device) for _ in Ls]
         dz, dx, dy = [dev(z) for z in zs1], dev(x1), dev(y1)
         ms = time_steps(torch, lambda: scw.scw_sweep_wavelengths(ctx, Ls, dz, dx, dy, out=out), max(2, args.steps // 2), 2)
-        extra["config1_c128"] = dict(ms_per_call=ms, samples_per_s=c1.n_layers * c1.planes * c1.Nx * c1.Ny / (ms * 1e-3))
+        M1 = c1.U * c1.Vn
+        gf = c1.n_layers * (8 * 3 * M1 * 4 * M1 * c1.planes + 8 * 3 * c1.planes * (M1 * c1.Ny + c1.Nx * c1.U * c1.Ny)) / 1e9
+        extra["config1_c128"] = dict(ms_per_call=ms, samples_per_s=c1.n_layers * c1.planes * c1.Nx * c1.Ny / (ms * 1e-3),
+                                     roofline=dict(bound="tensor", achieved=gf / ms, peak=FP64_DMMA_PEAK_TFLOPS,
+                                                   unit="TFLOP/s (useful fp64, 8 per complex MAC; peak = measured "
+                                                        "mma.sync m8n8k4 f64 rate, DESIGN.md 5)",
+                                                   frac=gf / ms / FP64_DMMA_PEAK_TFLOPS, traffic=None))
         del Ls, out, layers
         torch.cuda.empty_cache()
         c2 = si.CONFIGS[2]
