@@ -161,19 +161,21 @@ __global__ void __launch_bounds__(TS_PI_THREADS) k_tc_synth_pimage_partials(int 
                                                                             const __grid_constant__ TcPartials tp,
                                                                             uint8_t* __restrict__ img)
 {
-    const int image = blockIdx.x;                                 // (plane * nuc + uc) * nvc + vc
+    // grid: x = (instance, z plane), y = item chunk, z = (u chunk, v chunk, component): few divisions, all but one uniform
+    constexpr int rpt = 128;                                      // rows per assembly tile (checked on the host)
+    const int pz = blockIdx.x;                                    // inst*Fz + n
     const int item = blockIdx.y * TS_PI_THREADS + threadIdx.x;    // kc * (N1/2) + ul
     const int half = N1 / 2, kchunks = K1p / 8;
     if (item >= kchunks * half) return;
     const int kc = item / half, ul = item - kc * half;
-    const int vc = image % nvc, puc = image / nvc;
-    const int uc = puc % nuc, plane = puc / nuc;                  // plane = inst*Fz*3 + n*3 + comp
+    const int comp = blockIdx.z % 3, cc = blockIdx.z / 3;
+    const int vc = cc % nvc, uc = cc / nvc;
+    const int plane = pz * 3 + comp;
+    const int image = (plane * nuc + uc) * nvc + vc;
     const int u = uc * Uc + ul;
     const int M = U * Vn;
-    const int pz = plane / 3, comp = plane - pz * 3;
     const int inst = pz / Fz, n = pz - inst * Fz;
     const int nt = n / tp.Fzt, nn = n - nt * tp.Fzt;
-    const int rpt = tp.rows_per_tile;
     const int tile_base = (inst * tp.n_tiles + nt) * tp.m_tiles;
     const size_t tile_floats = (size_t)tp.Fzt * 2 * rpt;
     float2 pv[4];
@@ -183,7 +185,7 @@ __global__ void __launch_bounds__(TS_PI_THREADS) k_tc_synth_pimage_partials(int 
         pv[e] = make_float2(0.f, 0.f);
         if (ul < Uc && vl < Vc && u < U && v < Vn) {
             const int row = comp * M + v * U + u;
-            const int mt = row / rpt, r = row - mt * rpt;
+            const int mt = row / rpt, r = row % rpt;
             const int tile = tile_base + mt;
             const int cnt = tp.seg_count[tile];
             const int* __restrict__ slots = tp.seg_slot + (size_t)tile * tp.max_segs;
@@ -611,7 +613,7 @@ void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, 
 
 bool tc_synth_partials_supported(int U, int Vn, const TcPartials& parts)
 {
-    return parts.part && (int64_t)U * Vn * 3 < (1 << 30);
+    return parts.part && parts.rows_per_tile == 128 && (int64_t)U * Vn * 3 < (1 << 30);
 }
 
 void launch_tc_synth_group_partials(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const TcPartials& parts,
@@ -624,7 +626,8 @@ void launch_tc_synth_group_partials(scw_ctx* ctx, int U, int Vn, int64_t Fz, int
     {
         KernelScope ks(ctx, KC_SYNTH_IMG);
         const int items = (pl.K1p / 8) * (pl.K2p / 2);
-        const dim3 grid((unsigned)(planes * pl.cu.n * pl.cv.n), (unsigned)((items + TS_PI_THREADS - 1) / TS_PI_THREADS));
+        const dim3 grid((unsigned)(planes / 3), (unsigned)((items + TS_PI_THREADS - 1) / TS_PI_THREADS),
+                        (unsigned)(pl.cu.n * pl.cv.n * 3));
         k_tc_synth_pimage_partials<<<grid, TS_PI_THREADS, 0, ctx->stream>>>(U, Vn, pl.cu.len, pl.cv.len, pl.cu.n, pl.cv.n,
                                                                             pl.K1p, pl.K2p, (int)Fz, parts, B1);
     }
