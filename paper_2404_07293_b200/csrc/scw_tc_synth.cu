@@ -31,6 +31,9 @@ constexpr int TS_TMEM_COLS = 512;
 constexpr int TS_D2_COL = 0;               // D2[h] at columns h*128
 constexpr int TS_D1_COL = 256;             // D1 at columns 256..256+N1, then A2 (per u chunk: hi K2p/2 | lo K2p/2 columns)
 constexpr int TS_MAX_INST = 64;            // instances per grouped launch
+#ifndef SCW_TS_ORDER
+#define SCW_TS_ORDER 0                     // 0: GEMM1(next item) before GEMM2 of this item (measured best with dynamic planes)
+#endif
 
 #ifdef SCW_TS_DEBUG
 __device__ long long g_ts_dbg[4096];
@@ -56,6 +59,7 @@ struct TsParams {
     int K1p, K2p;          // padded 2*Vc, 2*Uc  (N1 == K2p)
     int nuc, nvc;          // frequency chunks along u and v
     int tiles_x, tiles_y, pair0, npairs;   // this launch covers tile pairs [pair0, pair0 + npairs)
+    int* sched;            // [tile pair] next plane to hand out (zeroed by the spectrum-image kernel)
 };
 
 __host__ __device__ inline int ts_pad16(int v) { return (v + 15) / 16 * 16; }
@@ -118,9 +122,11 @@ __global__ void k_tc_synth_twiddles(const TwAxis ay, const TwAxis ax, int blocks
 // v = vc*Vc + vl:   row (u,Re): (P_r, -P_i);  row (u,Im): (P_i, P_r)
 // so that  D1[y, (u,c)] = sum_v Fy[y,v] P[u,v]  in real arithmetic.
 __global__ void k_tc_synth_pimage(int U, int Vn, int Uc, int Vc, int nuc, int nvc, int K1p, int N1, int planes,
-                                  const float2* __restrict__ P, int64_t ldP, uint8_t* __restrict__ img)
+                                  const float2* __restrict__ P, int64_t ldP, uint8_t* __restrict__ img,
+                                  int* __restrict__ sched, int n_sched)
 {
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;      // (image, row, kpair)
+    if (idx < n_sched) sched[idx] = 0;                                       // plane counters of the synthesis that follows
     const int kpairs = K1p / 2;
     if (idx >= (int64_t)planes * nuc * nvc * N1 * kpairs) return;
     const int vl = (int)(idx % kpairs);
@@ -159,8 +165,11 @@ constexpr int TS_PI_THREADS = 128;
 __global__ void __launch_bounds__(TS_PI_THREADS) k_tc_synth_pimage_partials(int U, int Vn, int Uc, int Vc, int nuc, int nvc,
                                                                             int K1p, int N1, int Fz,
                                                                             const __grid_constant__ TcPartials tp,
-                                                                            uint8_t* __restrict__ img)
+                                                                            uint8_t* __restrict__ img,
+                                                                            int* __restrict__ sched, int n_sched)
 {
+    if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0)              // plane counters of the synthesis that follows
+        for (int i = threadIdx.x; i < n_sched; i += TS_PI_THREADS) sched[i] = 0;
     // grid: x = (instance, z plane), y = item chunk, z = (u chunk, v chunk, component): few divisions, all but one uniform
     constexpr int rpt = 128;                                      // rows per assembly tile (checked on the host)
     const int pz = blockIdx.x;                                    // inst*Fz + n
@@ -271,10 +280,13 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
     uint64_t* b2_empty = bars + 9;       // [2]
     uint64_t* d2_full = bars + 11;       // [2]
     uint64_t* d2_empty = bars + 13;      // [2]
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 15);
+    uint64_t* sched_full = bars + 15;    // [8] plane ids handed from the loader to the other roles
+    int* s_plane = reinterpret_cast<int*>(bars + 23);               // [8]
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 27);
 
     if (tid == 0) {
         mbar_init(tw_full, 1);
+        for (int s = 0; s < 8; ++s) mbar_init(&sched_full[s], 1);
         for (int s = 0; s < 2; ++s) {
             mbar_init(&b1_full[s], 1);
             mbar_init(&b1_empty[s], 1);
@@ -294,17 +306,20 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
     const uint32_t tmem_base = *tmem_slot;
     const uint32_t a2_col = TS_D1_COL + N1;                    // A2 chunk uc: hi at a2_col + uc*K2p, lo K2p/2 columns on
 
-    // this CTA's tile pair and plane sequence
-    const int per_pair = gridDim.x / p.npairs;                 // CTAs per pair (gridDim.x is a multiple of npairs)
+    // This CTA's tile pair.  Its planes are handed out dynamically: the CTAs of a pair draw plane ids from a shared
+    // counter (the kernel is HBM-write-bound and the SMs do not all run at the same pace, a static split leaves a tail).
+    // The loader draws the id and publishes it through an 8-deep ring (the loader is never more than 6 planes ahead of
+    // the epilogue); id -1 ends every role.  Item = (plane, u chunk).
     const int pair = p.pair0 + (int)blockIdx.x % p.npairs;
-    const int first_plane = (int)blockIdx.x / p.npairs;
     const int tx = pair % p.tiles_x, ty = pair / p.tiles_x;
-    const int n_planes = first_plane < p.planes ? (p.planes - first_plane + per_pair - 1) / per_pair : 0;
-    const int n_items = n_planes * nuc;                        // item = (plane, u chunk)
+    auto sched_get = [&](int nl) -> int {
+        mbar_wait(&sched_full[nl & 7], (nl >> 3) & 1);
+        return *reinterpret_cast<volatile int*>(&s_plane[nl & 7]);
+    };
 
     // A2 (the x twiddles of this tile, every u chunk) goes to TMEM once: the converter warp pair of lane quarter q
     // writes rows 32q..32q+31, warp kg = 0 the hi words, kg = 1 the lo words
-    if (warp >= 2 && warp < 10 && n_items > 0) {
+    if (warp >= 2 && warp < 10) {
         const int q = warp & 3, kg = (warp - 2) >> 2;
         const int half = K2p / 2;
         for (int uc = 0; uc < nuc; ++uc) {
@@ -325,26 +340,32 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
     TS_BLK(1);
 
     if (warp == 0) {
-        // ===== loader: y twiddle images once, then the nvc spectrum images of every item =====
-        if (lane == 0 && n_items > 0) {
-            mbar_expect_tx(tw_full, nvc * 2 * a1_img);
-            bulk_g2s(sA1, p.A1 + (size_t)ty * nvc * 2 * a1_img, nvc * 2 * a1_img, tw_full);
+        // ===== loader: draws the planes; y twiddle images once, then the nuc*nvc spectrum images of every plane =====
+        if (lane == 0) {
             int q = 0;
-            for (int i = 0; i < n_items; ++i) {
-                const int n = i / nuc, uc = i - n * nuc;
-                const size_t plane = (size_t)first_plane + (size_t)n * per_pair;
-                for (int vc = 0; vc < nvc; ++vc, ++q) {
-                    const int s = q & 1;
-                    mbar_wait(&b1_empty[s], ((q >> 1) & 1) ^ 1);
-                    mbar_expect_tx(&b1_full[s], 2 * b1_img);
-                    bulk_g2s(sB1 + (size_t)s * 2 * b1_img, p.B1 + ((plane * nuc + uc) * nvc + vc) * 2 * b1_img, 2 * b1_img,
-                             &b1_full[s]);
+            for (int nl = 0;; ++nl) {
+                int plane = atomicAdd(&p.sched[pair], 1);
+                if (plane >= p.planes) plane = -1;
+                *reinterpret_cast<volatile int*>(&s_plane[nl & 7]) = plane;
+                mbar_arrive(&sched_full[nl & 7]);
+                if (plane < 0) break;
+                if (nl == 0) {
+                    mbar_expect_tx(tw_full, nvc * 2 * a1_img);
+                    bulk_g2s(sA1, p.A1 + (size_t)ty * nvc * 2 * a1_img, nvc * 2 * a1_img, tw_full);
                 }
+                for (int uc = 0; uc < nuc; ++uc)
+                    for (int vc = 0; vc < nvc; ++vc, ++q) {
+                        const int s = q & 1;
+                        mbar_wait(&b1_empty[s], ((q >> 1) & 1) ^ 1);
+                        mbar_expect_tx(&b1_full[s], 2 * b1_img);
+                        bulk_g2s(sB1 + (size_t)s * 2 * b1_img, p.B1 + (((size_t)plane * nuc + uc) * nvc + vc) * 2 * b1_img,
+                                 2 * b1_img, &b1_full[s]);
+                    }
             }
         }
     } else if (warp == 1) {
         // ===== MMA issuer: the whole warp runs the loop (warp-uniform control flow), one elected lane issues =====
-        if (n_items > 0) {
+        if (sched_get(0) >= 0) {
             const uint32_t idesc1 = umma_idesc_bf16(TS_TILE, N1);
             const uint32_t idesc2 = umma_idesc_bf16(TS_TILE, TS_TILE);
             const uint32_t a1 = smem_u32(sA1), b1 = smem_u32(sB1), b2 = smem_u32(sB2);
@@ -384,13 +405,21 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                 __syncwarp();
                 TS_MARK(i * 32 + 4 + 4 * h);
             };
-            // order GEMM2(h=0), GEMM1(next), GEMM2(h=1): measured best -- issuing GEMM1 of the next item first shortens
-            // one CTA's period but widens the spread of CTA finishing times on the HBM-write-bound kernel (77 vs 83 us)
+            // GEMM1 of the next item goes first: it only needs D1 back from the converters (a TMEM load after d1_full) and
+            // then runs on the tensor pipe while they split and store this item's B2
             issue_gemm1(0);
-            for (int i = 0; i < n_items; ++i) {
+            for (int i = 0;; ++i) {
+                const int n = i / nuc, uc = i - n * nuc;
+                const bool next = (uc + 1 < nuc) || sched_get(n + 1) >= 0;
+#if SCW_TS_ORDER == 0
+                if (next) issue_gemm1(i + 1);
                 issue_gemm2(i, 0);
-                if (i + 1 < n_items) issue_gemm1(i + 1);
+#else
+                issue_gemm2(i, 0);
+                if (next) issue_gemm1(i + 1);
+#endif
                 issue_gemm2(i, 1);
+                if (!next) break;
             }
         }
     } else if (warp < 10) {
@@ -403,7 +432,8 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
         uint8_t* row = sB2 + (size_t)h * 2 * b2_img + yy * 32;
         const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + TS_D1_COL;
         const int nchunks = K2p / 8;                 // <= 10
-        for (int n = 0; n < n_items; ++n) {          // n = item (plane, u chunk)
+        for (int n = 0;; ++n) {                      // n = item (plane, u chunk)
+            if (n % nuc == 0 && sched_get(n / nuc) < 0) break;
             mbar_wait(d1_full, n & 1);
             tc_fence_after();
             if (warp == 4 && lane == 0) TS_MARK(n * 32 + 10);
@@ -453,8 +483,9 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
         const int cg = (warp - 10) >> 2;             // which 32-y group of the half
         const int64_t x = (int64_t)tx * TS_TILE + 32 * q + lane;
         const bool x_ok = x < p.Nx;
-        for (int n = 0; n < n_planes; ++n) {
-            const int gplane = first_plane + n * per_pair;
+        for (int n = 0;; ++n) {
+            const int gplane = sched_get(n);
+            if (gplane < 0) break;
             const int inst = gplane / p.planes_per_inst;
             const int plane = gplane - inst * p.planes_per_inst;
             const int64_t zi = plane / 3;
@@ -499,7 +530,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
 struct TsPlan {
     TsChunks cu, cv;          // frequency chunks along u (GEMM2's K) and v (GEMM1's K)
     int K1p, K2p, tiles_x, tiles_y;
-    size_t a1_bytes, a2_bytes, b1_bytes, smem_bytes;
+    size_t a1_bytes, a2_bytes, sched_bytes, b1_bytes, smem_bytes;
 };
 
 static TsPlan ts_plan(int U, int Vn, int64_t Fz, int64_t Nx, int64_t Ny)
@@ -513,6 +544,7 @@ static TsPlan ts_plan(int U, int Vn, int64_t Fz, int64_t Nx, int64_t Ny)
     pl.tiles_y = (int)((Ny + TS_TILE - 1) / TS_TILE);
     pl.a1_bytes = align_up((size_t)pl.tiles_y * pl.cv.n * 2 * TS_TILE * pl.K1p * 2);
     pl.a2_bytes = align_up((size_t)pl.tiles_x * pl.cu.n * TS_TILE * pl.K2p * 4);
+    pl.sched_bytes = align_up((size_t)pl.tiles_x * pl.tiles_y * sizeof(int));
     pl.b1_bytes = align_up((size_t)Fz * 3 * pl.cu.n * pl.cv.n * 2 * pl.K2p * pl.K1p * 2);
     pl.smem_bytes = (size_t)pl.cv.n * 2 * TS_TILE * pl.K1p * 2 + (size_t)4 * pl.K2p * pl.K1p * 2 +
                     (size_t)4 * TS_TILE * pl.K2p * 2 + 256;
@@ -530,7 +562,7 @@ bool tc_synth_supported(int dtype, int U, int Vn)
 size_t tc_synth_twiddle_bytes(int U, int Vn, int64_t Nx, int64_t Ny)
 {
     const TsPlan pl = ts_plan(U, Vn, 1, Nx, Ny);
-    return pl.a1_bytes + pl.a2_bytes;
+    return pl.a1_bytes + pl.a2_bytes + pl.sched_bytes;      // y images | x operand rows | plane counters
 }
 
 size_t tc_synth_scratch(int U, int Vn, int64_t Fz) { return ts_plan(U, Vn, Fz, 1, 1).b1_bytes; }
@@ -556,6 +588,11 @@ extern "C" void scw_debug_ts_read(long long* out) { cudaMemcpyFromSymbol(out, g_
 
 int tc_synth_max_group() { return TS_MAX_INST; }
 
+static int* ts_sched(const TsPlan& pl, const void* tw)
+{
+    return reinterpret_cast<int*>(static_cast<uint8_t*>(const_cast<void*>(tw)) + pl.a1_bytes + pl.a2_bytes);
+}
+
 // The synthesis launches proper: B1 holds the spectrum images of all n_inst*Fz*3 planes.
 static void ts_launch_main(scw_ctx* ctx, const TsPlan& pl, int64_t Fz, int n_inst, const uint8_t* B1, int64_t Nx,
                            int64_t Ny, const void* tw, void* const* E, const int64_t strides[4])
@@ -565,6 +602,7 @@ static void ts_launch_main(scw_ctx* ctx, const TsPlan& pl, int64_t Fz, int n_ins
     p.A1 = static_cast<const uint8_t*>(tw);
     p.A2 = reinterpret_cast<const uint32_t*>(p.A1 + pl.a1_bytes);
     p.B1 = B1;
+    p.sched = ts_sched(pl, tw);
     for (int i = 0; i < n_inst; ++i) p.E[i] = static_cast<float2*>(E[i]);
     p.s_comp = strides[0];
     p.s_z = strides[1];
@@ -606,7 +644,8 @@ void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, 
         const int64_t n = (int64_t)planes * pl.cu.n * pl.cv.n * pl.K2p * (pl.K1p / 2);
         k_tc_synth_pimage<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(U, Vn, pl.cu.len, pl.cv.len, pl.cu.n, pl.cv.n,
                                                                                 pl.K1p, pl.K2p, planes, (const float2*)P_all,
-                                                                                ldP, B1);
+                                                                                ldP, B1, ts_sched(pl, tw),
+                                                                                pl.tiles_x * pl.tiles_y);
     }
     ts_launch_main(ctx, pl, Fz, n_inst, B1, Nx, Ny, tw, E, strides);
 }
@@ -629,7 +668,8 @@ void launch_tc_synth_group_partials(scw_ctx* ctx, int U, int Vn, int64_t Fz, int
         const dim3 grid((unsigned)(planes / 3), (unsigned)((items + TS_PI_THREADS - 1) / TS_PI_THREADS),
                         (unsigned)(pl.cu.n * pl.cv.n * 3));
         k_tc_synth_pimage_partials<<<grid, TS_PI_THREADS, 0, ctx->stream>>>(U, Vn, pl.cu.len, pl.cv.len, pl.cu.n, pl.cv.n,
-                                                                            pl.K1p, pl.K2p, (int)Fz, parts, B1);
+                                                                            pl.K1p, pl.K2p, (int)Fz, parts, B1,
+                                                                            ts_sched(pl, tw), pl.tiles_x * pl.tiles_y);
     }
     ts_launch_main(ctx, pl, Fz, n_inst, B1, Nx, Ny, tw, E, strides);
 }
