@@ -305,6 +305,28 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
                                   hbm_write_frac=ebytes / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
     del Ls, zs, out
     torch.cuda.empty_cache()
+    # NEXT-1 exterior field (eq. 9-10): the paper's Table 2 shape (M = 2500 orders, one 256 x 256 plane below the
+    # sample; 142 s on one i9 core, 0.29 s on an RTX 3090) and a config-1-shaped volume above it
+    for name, cfgx, side, planes in (("exterior_table2_plane", si.Config(5, "table 2 exterior", 50, 50, 32.0, (1.0,), 1, 1,
+                                                                          256, 256, (np.complex64,)), 1, 1),
+                                     ("exterior_volume_33x33", si.CONFIGS[1], 0, 64)):
+        ext = si.make_exterior(cfgx, side, dtype=np.complex64)
+        X = scw.Exterior.from_numpy(ext, device)
+        xg, yg, _ = si.grid_coords(cfgx, 0)
+        d = np.linspace(0.0, 3.0, planes)
+        zg = dev(ext["z_face"] - d if side == 0 else ext["z_face"] + d)
+        dxg, dyg = dev(xg), dev(yg)
+        Pbuf = torch.empty((planes, 3 * cfgx.U * cfgx.Vn), dtype=torch.complex64, device=device)
+        Eo = torch.empty((planes, 3, cfgx.Ny, cfgx.Nx), dtype=torch.complex64, device=device)
+
+        def ext_step():
+            scw.scw_exterior_spectra(ctx, X, zg, out=Pbuf)
+            scw.scw_synthesize_grid(ctx, U=cfgx.U, Vn=cfgx.Vn, X=ext["X"], Y=ext["Y"], P=Pbuf, x=dxg, y=dyg, out=Eo)
+
+        ms = time_steps(torch, ext_step, args.steps, args.warmup)
+        ns = planes * cfgx.Nx * cfgx.Ny
+        extra[name] = dict(ms_per_call=ms, samples_per_s=ns / (ms * 1e-3), orders=cfgx.U * cfgx.Vn, planes=planes,
+                           hbm_write_frac=ns * 24 / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
     if args.all:
         c1, layers, zs1, x1, y1 = config1_inputs(np.complex128)
         Ls = [scw.Layer.from_numpy(d, device) for d in layers]

@@ -191,6 +191,41 @@ int32_t scw_sweep_wavelengths_host(scw_ctx* ctx, int64_t n_inst, const scw_layer
 int32_t scw_sweep_host_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst,
                                  const int64_t* Fz, int64_t Nx, int64_t Ny, size_t* bytes);
 
+/* ---------------------------------------------------------------- exterior field
+ *
+ * Field in the homogeneous half-spaces above (z <= z_0) and below (z >= z_L) the sample, eq. 9:
+ *   above:  p(s_m, z) = p_inc_m  G[ s_z(n), z_inc,  z]  +  p_face_m G[-s_z(n), z_face, z]     (incident + reflected)
+ *   below:  p(s_m, z) = p_face_m G[ s_z(n), z_face, z]                                         (transmitted)
+ * with s_z(n) = sqrt(n^2 - |s_m|^2), Im >= 0 (eq. 2), s_m = lambda (u/X, v/Y) (eq. 6), G of eq. 7, followed by
+ * eq. 10, E(r, z) = sum_m p(s_m, z) exp(i k s_m . r).  The reflected wave travels toward -z: its z-wavenumber is
+ * -s_z(n), so that it decays away from the interface it is referenced at (reading c-17).
+ * Amplitudes are [M x 3] complex<dtype>, component fastest, m as in eq. 6's index map (u fastest).
+ */
+enum { SCW_SIDE_ABOVE = 0, SCW_SIDE_BELOW = 1 };
+typedef struct {
+    uint32_t struct_size;      /* = sizeof(scw_exterior) */
+    int32_t dtype;             /* SCW_C64 | SCW_C128: element type of the amplitudes, P and E */
+    int32_t side;              /* SCW_SIDE_ABOVE | SCW_SIDE_BELOW */
+    int32_t U, Vn;             /* frequency grid (eq. 6) */
+    double X, Y;               /* patch size */
+    double lambda;             /* vacuum wavelength */
+    double n_re, n_im;         /* refractive index of the half-space (real above, complex below) */
+    double z_face;             /* z_0 (above) or z_L (below): reference plane of p_face */
+    double z_inc;              /* z-bar: reference plane of the incident wave (above only) */
+    const void* p_face;        /* [M x 3] reflected (above) / transmitted (below) amplitudes, device */
+    const void* p_inc;         /* [M x 3] incident amplitudes (above only), device; NULL = no incident wave */
+} scw_exterior;
+
+/* eq. 9 on Fz planes: P[comp*M + m, i] = p_comp(s_m, z_i), column-major [ldP x Fz], ldP >= 3*U*Vn; feed P to
+ * scw_synthesize_grid for eq. 10 on a rectilinear grid.  z: [Fz] doubles (device), evaluated as-is on either side.
+ * No workspace.  Errors: NULL, SHAPE, DTYPE, ALIGN, VALUE, CUDA. */
+int32_t scw_exterior_spectra(scw_ctx* ctx, const scw_exterior* ext, int64_t Fz, const double* z, void* P, int64_t ldP);
+
+/* eq. 9-10 at scattered points: the M (below) or 2M (above) plane waves are tabulated in the workspace and summed by
+ * the direct plane-wave kernels of scw_eval_points.  r: [N x 3] doubles, E: [N x 3] complex<dtype>, comp fastest. */
+int32_t scw_exterior_points(scw_ctx* ctx, const scw_exterior* ext, int64_t N, const double* r, void* E);
+int32_t scw_exterior_points_workspace(scw_ctx* ctx, const scw_exterior* ext, int64_t N, size_t* bytes);
+
 #ifdef __cplusplus
 }
 #endif

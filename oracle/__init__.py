@@ -205,3 +205,43 @@ def tier_b_points(*, U, Vn, X, Y, xyz, chunk=2048, **layer):
         for comp in range(3):
             E[s:s + chunk, comp] = np.einsum("nm,mn->n", T, P[comp * M:(comp + 1) * M])
     return E
+
+
+# ----------------------------------------------------------------------------- exterior field (NEXT-1)
+SIDE_ABOVE, SIDE_BELOW = 0, 1
+
+
+def exterior_samples(*, side, U, Vn, X, Y, lam, n, z_face, p_face, z_inc=0.0, p_inc=None, xyz, **_):
+    """Field outside the sample, eq. 9 then eq. 10, one frequency at a time -> E [n,3] complex128.
+
+    above (z <= z_0):  p(s_m, z) = p_inc_m G[s_z(n), z_inc, z] + p_face_m G[-s_z(n), z_0, z]
+    below (z >= z_L):  p(s_m, z) = p_face_m G[s_z(n), z_L, z]
+    s_z by eq. 2 (Im >= 0), s_m = lam (u/X, v/Y) by eq. 6, G by eq. 7.  The reflected wave travels toward -z, hence
+    -s_z (reading c-17).  p_face, p_inc: [M,3] complex.
+    """
+    xyz = np.asarray(xyz, dtype=np.float64)
+    x, y, z = xyz[:, 0], xyz[:, 1], xyz[:, 2]
+    k = 2.0 * np.pi / lam
+    M = U * Vn
+    p_face = np.asarray(p_face, dtype=np.complex128)
+    p_inc = None if p_inc is None else np.asarray(p_inc, dtype=np.complex128)
+    assert p_face.shape == (M, 3)
+    E = np.zeros((xyz.shape[0], 3), dtype=np.complex128)
+    for m in range(M):
+        u, v = index_map(U, Vn, m)
+        sx, sy = lam * u / X, lam * v / Y                                   # eq. 6
+        s_z = sz(n, sx, sy)                                                 # eq. 2
+        if side == SIDE_ABOVE:
+            pz = p_face[m][None, :] * np.exp(1j * k * (z - z_face) * (-s_z))[:, None]       # reflected, eq. 7
+            if p_inc is not None:
+                pz = pz + p_inc[m][None, :] * np.exp(1j * k * (z - z_inc) * s_z)[:, None]  # incident
+        else:
+            pz = p_face[m][None, :] * np.exp(1j * k * (z - z_face) * s_z)[:, None]          # transmitted
+        E += pz * np.exp(1j * k * (sx * x + sy * y))[:, None]               # eq. 10
+    return E
+
+
+def exterior_grid(*, x, y, z, **ext):
+    """exterior_samples on a rectilinear grid -> E [Fz, 3, Ny, Nx] complex128 (planar layout)."""
+    E = exterior_samples(xyz=grid_points(x, y, z), **ext)
+    return np.ascontiguousarray(E.reshape(len(z), len(y), len(x), 3).transpose(0, 3, 1, 2))

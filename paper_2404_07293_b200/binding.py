@@ -28,7 +28,15 @@ EXPORTS = [
     "scw_eval_points", "scw_points_workspace", "scw_sweep_wavelengths", "scw_sweep_workspace",
     "scw_sweep_wavelengths_host", "scw_sweep_host_workspace",
     "scw_profile_classes", "scw_profile_name", "scw_profile_read", "scw_profile_reset",
+    "scw_exterior_spectra", "scw_exterior_points", "scw_exterior_points_workspace",
 ]
+SCW_SIDE_ABOVE, SCW_SIDE_BELOW = 0, 1
+
+
+class scw_exterior(Structure):
+    _fields_ = [("struct_size", c_uint32), ("dtype", c_int32), ("side", c_int32), ("U", c_int32), ("Vn", c_int32),
+                ("X", c_double), ("Y", c_double), ("lambda_", c_double), ("n_re", c_double), ("n_im", c_double),
+                ("z_face", c_double), ("z_inc", c_double), ("p_face", c_void_p), ("p_inc", c_void_p)]
 
 
 class ScwError(RuntimeError):
@@ -96,6 +104,9 @@ def lib():
                                                  POINTER(c_void_p), POINTER(c_int64), POINTER(c_int64)]
         L.scw_sweep_host_workspace.argtypes = [c_void_p, c_int64, POINTER(scw_layer), POINTER(c_int64), c_int64,
                                                c_int64, POINTER(c_size_t)]
+        L.scw_exterior_spectra.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, c_void_p, c_void_p, c_int64]
+        L.scw_exterior_points.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, c_void_p, c_void_p]
+        L.scw_exterior_points_workspace.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, POINTER(c_size_t)]
         _LIB = L
     return _LIB
 
@@ -171,6 +182,30 @@ class PlaneWaves:
         t = lambda a: torch.from_numpy(a).to(device)
         return PlaneWaves(lam=d["lam"], sx=t(d["sx"]), sy=t(d["sy"]), gamma=t(d["gamma"]), zref=t(d["zref"]),
                           p=t(d["p"]))
+
+
+class Exterior:
+    """Half-space above (side=SCW_SIDE_ABOVE: incident + reflected) or below (transmitted) the sample, eq. 9.
+
+    p_face, p_inc: (M, 3) complex device tensors (component fastest), p_inc None below / when there is no incident wave.
+    """
+
+    def __init__(self, *, side, U, Vn, X, Y, lam, n, z_face, p_face, z_inc=0.0, p_inc=None, **_):
+        self.side, self.U, self.Vn, self.X, self.Y, self.lam = int(side), int(U), int(Vn), float(X), float(Y), float(lam)
+        self.n, self.z_face, self.z_inc, self.p_face, self.p_inc = complex(n), float(z_face), float(z_inc), p_face, p_inc
+        assert p_face.shape == (self.U * self.Vn, 3) and p_face.is_contiguous()
+        assert p_inc is None or (p_inc.shape == p_face.shape and p_inc.dtype == p_face.dtype and p_inc.is_contiguous())
+
+    def struct(self):
+        return scw_exterior(ctypes.sizeof(scw_exterior), _dt(self.p_face), self.side, self.U, self.Vn, self.X, self.Y,
+                            self.lam, self.n.real, self.n.imag, self.z_face, self.z_inc, self.p_face.data_ptr(),
+                            None if self.p_inc is None else self.p_inc.data_ptr())
+
+    @staticmethod
+    def from_numpy(d, device):
+        t = lambda a: None if a is None else torch.from_numpy(a).to(device)
+        return Exterior(side=d["side"], U=d["U"], Vn=d["Vn"], X=d["X"], Y=d["Y"], lam=d["lam"], n=d["n"],
+                        z_face=d["z_face"], z_inc=d.get("z_inc", 0.0), p_face=t(d["p_face"]), p_inc=t(d.get("p_inc")))
 
 
 class Context:
@@ -286,6 +321,29 @@ def scw_eval_points(ctx, modes, r, out=None):
     if out is None:
         out = torch.empty((N, 3), dtype=dtype, device=ctx.device)
     ctx.check(ctx.L.scw_eval_points(ctx._h, byref(m), N, _p(r), _p(out)))
+    return out
+
+
+def scw_exterior_spectra(ctx, ext, z, out=None):
+    """eq. 9 on the planes z: P as a (Fz, 3M) tensor (column-major [3M x Fz]); feed it to scw_synthesize_grid."""
+    Fz, R = z.numel(), 3 * ext.U * ext.Vn
+    st = ext.struct()
+    if out is None:
+        out = torch.empty((Fz, R), dtype=ext.p_face.dtype, device=ctx.device)
+    ctx.check(ctx.L.scw_exterior_spectra(ctx._h, byref(st), Fz, _p(z), _p(out), out.shape[1] if Fz else R))
+    return out
+
+
+def scw_exterior_points(ctx, ext, r, out=None):
+    """eq. 9-10 at scattered points r (N, 3) float64 -> E (N, 3)."""
+    N = r.shape[0]
+    st = ext.struct()
+    need = c_size_t()
+    ctx.check(ctx.L.scw_exterior_points_workspace(ctx._h, byref(st), N, byref(need)))
+    ctx.reserve(need.value)
+    if out is None:
+        out = torch.empty((N, 3), dtype=ext.p_face.dtype, device=ctx.device)
+    ctx.check(ctx.L.scw_exterior_points(ctx._h, byref(st), N, _p(r), _p(out)))
     return out
 
 

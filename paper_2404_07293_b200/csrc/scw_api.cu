@@ -277,7 +277,7 @@ const char* scw_profile_name(int32_t kc)
     static const char* names[KC_COUNT] = {"mode_weights", "twiddles", "simt_assemble", "reduce_splits", "simt_synth_a",
                                           "simt_synth_b", "points_table", "points_planewave", "point_synth", "misc",
                                           "tc_assemble", "tc_synth", "tc_synth_images", "dmma_assemble", "dmma_synth_a",
-                                          "dmma_synth_b"};
+                                          "dmma_synth_b", "exterior"};
     return (kc >= 0 && kc < KC_COUNT) ? names[kc] : nullptr;
 }
 
@@ -717,6 +717,63 @@ int32_t scw_eval_points(scw_ctx* ctx, const scw_modes* modes, int64_t N, const d
         launch_point_synth(ctx, dtype, L->U, L->Vn, L->X, L->Y, n, r + 3 * p0, P, R, (char*)E + (size_t)p0 * 3 * es);
     }
     return check_launch(ctx, "scw_eval_points");
+}
+
+// ------------------------------------------------------------------------------------------
+static int32_t check_exterior(scw_ctx* ctx, const scw_exterior* e, const char* who)
+{
+    if (!e) return fail(ctx, SCW_ERR_NULL, "%s: exterior descriptor is NULL", who);
+    if (e->struct_size != sizeof(scw_exterior)) return fail(ctx, SCW_ERR_SHAPE, "%s: exterior.struct_size mismatch", who);
+    if (e->dtype != SCW_C64 && e->dtype != SCW_C128) return fail(ctx, SCW_ERR_DTYPE, "%s: bad dtype %d", who, e->dtype);
+    if (e->side != SCW_SIDE_ABOVE && e->side != SCW_SIDE_BELOW) return fail(ctx, SCW_ERR_VALUE, "%s: bad side %d", who, e->side);
+    if (e->U <= 0 || e->Vn <= 0 || e->U > MAX_FREQ || e->Vn > MAX_FREQ)
+        return fail(ctx, SCW_ERR_SHAPE, "%s: U=%d Vn=%d out of range", who, e->U, e->Vn);
+    if (!finite_pos(e->X) || !finite_pos(e->Y) || !finite_pos(e->lambda))
+        return fail(ctx, SCW_ERR_VALUE, "%s: X, Y and lambda must be finite and > 0", who);
+    if (!std::isfinite(e->n_re) || !std::isfinite(e->n_im) || !std::isfinite(e->z_face) ||
+        (e->side == SCW_SIDE_ABOVE && e->p_inc && !std::isfinite(e->z_inc)))
+        return fail(ctx, SCW_ERR_VALUE, "%s: n, z_face and z_inc must be finite", who);
+    if (!e->p_face) return fail(ctx, SCW_ERR_NULL, "%s: p_face is required", who);
+    if (e->side == SCW_SIDE_BELOW && e->p_inc) return fail(ctx, SCW_ERR_VALUE, "%s: p_inc is only defined above the sample", who);
+    const size_t es = esize(e->dtype);
+    if (!aligned(e->p_face, es) || (e->p_inc && !aligned(e->p_inc, es))) return fail(ctx, SCW_ERR_ALIGN, "%s: amplitudes misaligned", who);
+    return SCW_OK;
+}
+
+int32_t scw_exterior_spectra(scw_ctx* ctx, const scw_exterior* ext, int64_t Fz, const double* z, void* P, int64_t ldP)
+{
+    if (int32_t s = check_ctx(ctx)) return s;
+    if (int32_t s = check_exterior(ctx, ext, "scw_exterior_spectra")) return s;
+    if (Fz < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_exterior_spectra: Fz=%lld < 0", (long long)Fz);
+    if (Fz == 0) return SCW_OK;
+    if (!z || !P) return fail(ctx, SCW_ERR_NULL, "scw_exterior_spectra: z and P are required");
+    if (ldP < 3LL * ext->U * ext->Vn) return fail(ctx, SCW_ERR_SHAPE, "scw_exterior_spectra: ldP=%lld < 3*U*Vn", (long long)ldP);
+    if (!aligned(z, 8) || !aligned(P, esize(ext->dtype))) return fail(ctx, SCW_ERR_ALIGN, "scw_exterior_spectra: z/P misaligned");
+    launch_exterior_spectra(ctx, ext, Fz, z, P, ldP);
+    return check_launch(ctx, "scw_exterior_spectra");
+}
+
+int32_t scw_exterior_points_workspace(scw_ctx* ctx, const scw_exterior* ext, int64_t N, size_t* bytes)
+{
+    if (!ctx || !bytes) return SCW_ERR_NULL;
+    ctx->msg[0] = 0;
+    if (int32_t s = check_exterior(ctx, ext, "scw_exterior_points_workspace")) return s;
+    if (N < 0) return fail(ctx, SCW_ERR_SHAPE, "N < 0");
+    *bytes = N ? exterior_points_bytes(ext) : 0;
+    return SCW_OK;
+}
+
+int32_t scw_exterior_points(scw_ctx* ctx, const scw_exterior* ext, int64_t N, const double* r, void* E)
+{
+    if (int32_t s = check_ctx(ctx)) return s;
+    if (int32_t s = check_exterior(ctx, ext, "scw_exterior_points")) return s;
+    if (N < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_exterior_points: N=%lld < 0", (long long)N);
+    if (N == 0) return SCW_OK;
+    if (!r || !E) return fail(ctx, SCW_ERR_NULL, "scw_exterior_points: r and E are required");
+    if (!aligned(r, 8) || !aligned(E, esize(ext->dtype))) return fail(ctx, SCW_ERR_ALIGN, "scw_exterior_points: r/E misaligned");
+    if (int32_t s = need_ws(ctx, exterior_points_bytes(ext), "scw_exterior_points")) return s;
+    launch_exterior_points(ctx, ext, N, r, E, ctx->ws);
+    return check_launch(ctx, "scw_exterior_points");
 }
 
 }  // extern "C"

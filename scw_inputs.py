@@ -11,13 +11,13 @@ The paper's own sample images are not available; these inputs stand in for them.
 
 RNG: numpy Generator(Philox(key=[7293, id])),
 id = config*2^20 + lambda_index*2^8 + layer*2^3 + array,
-array: 0 n_j, 1 V, 2 c, 3 thickness, 4 points, 5 oracle subset, 6 evanescent mask/sigma.
+array: 0 n_j, 1 V, 2 c, 3 thickness, 4 points, 5 oracle subset, 6 evanescent mask/sigma, 7 exterior amplitudes.
 """
 from dataclasses import dataclass
 
 import numpy as np
 
-A_N, A_V, A_C, A_T, A_PTS, A_SUB, A_EVAN = range(7)
+A_N, A_V, A_C, A_T, A_PTS, A_SUB, A_EVAN, A_EXT = range(8)
 
 
 def rng(config: int, array: int, lam_index: int = 0, layer: int = 0) -> np.random.Generator:
@@ -157,6 +157,27 @@ def make_planewaves(cfg: Config, layer: int = 0, lam_index: int = 0, dtype=np.co
     zref = np.where(lay["dir"] > 0, lay["z_lo"], lay["z_hi"]).astype(np.float64)
     return dict(lam=lam, sx=sx, sy=sy, gamma=lay["gamma"], zref=zref, p=p, J=J,
                 z_lo=lay["z_lo"], z_hi=lay["z_hi"])
+
+
+N_ABOVE, N_BELOW = 1.0, 1.5          # config 0's half-spaces (BASELINE.json configs[0]); used for every config
+
+
+def make_exterior(cfg: Config, side: int, lam_index: int = 0, dtype=np.complex64, z_inc=None):
+    """Exterior-field inputs (eq. 9): side 0 = above the stack (incident + reflected amplitudes, n = 1.0),
+    side 1 = below (transmitted amplitudes, n = 1.5).  Amplitudes are complex normals / sqrt(M) per component;
+    the incident wave is referenced one wavelength above z_0 unless z_inc is given."""
+    U, Vn = cfg.U, cfg.Vn
+    M = U * Vn
+    lam = cfg.lams[lam_index]
+    zi = stack_interfaces(cfg)
+    g = rng(cfg.cid, A_EXT, lam_index, side)
+    draw = lambda: ((g.standard_normal((M, 3)) + 1j * g.standard_normal((M, 3))) / np.sqrt(2.0 * M)).astype(dtype)
+    d = dict(side=side, U=U, Vn=Vn, X=cfg.L, Y=cfg.L, lam=lam, p_face=draw())
+    if side == 0:
+        d.update(n=complex(N_ABOVE), z_face=float(zi[0]), z_inc=float(zi[0] - lam if z_inc is None else z_inc), p_inc=draw())
+    else:
+        d.update(n=complex(N_BELOW), z_face=float(zi[-1]))
+    return d
 
 
 def make_points(cfg: Config, n=None, layer: int = 0):

@@ -44,8 +44,9 @@ def test_binding_structs_match_header_layout(libscw, tmp_path):
     from paper_2404_07293_b200 import binding
     src = tmp_path / "sz.c"
     src.write_text('#include "scwatter.h"\n#include <stdio.h>\n#include <stddef.h>\n'
-                   'int main(void){printf("%zu %zu %zu %zu %zu\\n", sizeof(scw_layer), sizeof(scw_modes),'
-                   ' offsetof(scw_layer, gamma), offsetof(scw_modes, p), offsetof(scw_modes, layer));return 0;}\n')
+                   'int main(void){printf("%zu %zu %zu %zu %zu %zu %zu %zu\\n", sizeof(scw_layer), sizeof(scw_modes),'
+                   ' offsetof(scw_layer, gamma), offsetof(scw_modes, p), offsetof(scw_modes, layer),'
+                   ' sizeof(scw_exterior), offsetof(scw_exterior, n_re), offsetof(scw_exterior, p_inc));return 0;}\n')
     exe = tmp_path / "sz"
     subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
     out = subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()
@@ -54,6 +55,9 @@ def test_binding_structs_match_header_layout(libscw, tmp_path):
     assert int(out[2]) == binding.scw_layer.gamma.offset
     assert int(out[3]) == binding.scw_modes.p.offset
     assert int(out[4]) == binding.scw_modes.layer.offset
+    assert int(out[5]) == ctypes.sizeof(binding.scw_exterior)
+    assert int(out[6]) == binding.scw_exterior.n_re.offset
+    assert int(out[7]) == binding.scw_exterior.p_inc.offset
     assert set(binding.EXPORTS) == set(declared_symbols())
 
 
