@@ -303,7 +303,12 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
     ebytes = n4 * 24
     extra["config4_sweep"] = dict(ms_per_call=ms, samples_per_s=n4 / (ms * 1e-3),
                                   hbm_write_frac=ebytes / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
-    del Ls, zs, out
+    # NEXT-3 detector: the same sweep with I = sum_comp |E_comp|^2 reduced in the synthesis epilogue (E never written)
+    outI = [torch.empty((c4.planes, c4.Ny, c4.Nx), dtype=torch.float32, device=device) for _ in Ls]
+    ms = time_steps(torch, lambda: scw.scw_sweep_intensity(ctx, Ls, zs, dx, dy, out=outI), args.steps, args.warmup)
+    extra["config4_sweep_intensity"] = dict(ms_per_call=ms, samples_per_s=n4 / (ms * 1e-3),
+                                            speedup_vs_complex_field=extra["config4_sweep"]["ms_per_call"] / ms)
+    del Ls, zs, out, outI
     torch.cuda.empty_cache()
     # NEXT-1 exterior field (eq. 9-10): the paper's Table 2 shape (M = 2500 orders, one 256 x 256 plane below the
     # sample; 142 s on one i9 core, 0.29 s on an RTX 3090) and a config-1-shaped volume above it

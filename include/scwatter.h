@@ -226,6 +226,21 @@ int32_t scw_exterior_spectra(scw_ctx* ctx, const scw_exterior* ext, int64_t Fz, 
 int32_t scw_exterior_points(scw_ctx* ctx, const scw_exterior* ext, int64_t N, const double* r, void* E);
 int32_t scw_exterior_points_workspace(scw_ctx* ctx, const scw_exterior* ext, int64_t N, size_t* bytes);
 
+/* ---------------------------------------------------------------- detector intensity
+ *
+ * scw_sweep_wavelengths followed by the detector reduction I(x, y, z) = sum_comp |E_comp(x, y, z)|^2 (the light intensity
+ * the paper collects on a plane; reading c-18), with the complex field never written:
+ * on the tensor-core path the reduction runs in the synthesis epilogue (4 bytes per sample leave the SM instead of 24).
+ * I: HOST array of device pointers, real (float for SCW_C64, double for SCW_C128), element (n, k, i) at
+ * n*strides[0] + k*strides[1] + i*strides[2] elements; strides == NULL means [Fz][Ny][Nx], x fastest.
+ */
+int32_t scw_sweep_intensity(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst,
+                            const int64_t* Fz, const double* const* z,
+                            int64_t Nx, const double* x, int64_t Ny, const double* y,
+                            void* const* I, const int64_t* strides);
+int32_t scw_sweep_intensity_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz,
+                                      int64_t Nx, int64_t Ny, size_t* bytes);
+
 #ifdef __cplusplus
 }
 #endif

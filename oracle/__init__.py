@@ -245,3 +245,11 @@ def exterior_grid(*, x, y, z, **ext):
     """exterior_samples on a rectilinear grid -> E [Fz, 3, Ny, Nx] complex128 (planar layout)."""
     E = exterior_samples(xyz=grid_points(x, y, z), **ext)
     return np.ascontiguousarray(E.reshape(len(z), len(y), len(x), 3).transpose(0, 3, 1, 2))
+
+
+# ----------------------------------------------------------------------------- detector intensity (NEXT-3)
+def intensity(E):
+    """I = |E_x|^2 + |E_y|^2 + |E_z|^2 from a planar field E [..., 3, Ny, Nx] -> [..., Ny, Nx] (the light intensity
+    collected on a plane; reading c-18)."""
+    E = np.asarray(E)
+    return (E.real ** 2 + E.imag ** 2).sum(axis=-3)

@@ -29,6 +29,7 @@ EXPORTS = [
     "scw_sweep_wavelengths_host", "scw_sweep_host_workspace",
     "scw_profile_classes", "scw_profile_name", "scw_profile_read", "scw_profile_reset",
     "scw_exterior_spectra", "scw_exterior_points", "scw_exterior_points_workspace",
+    "scw_sweep_intensity", "scw_sweep_intensity_workspace",
 ]
 SCW_SIDE_ABOVE, SCW_SIDE_BELOW = 0, 1
 
@@ -104,6 +105,8 @@ def lib():
                                                  POINTER(c_void_p), POINTER(c_int64), POINTER(c_int64)]
         L.scw_sweep_host_workspace.argtypes = [c_void_p, c_int64, POINTER(scw_layer), POINTER(c_int64), c_int64,
                                                c_int64, POINTER(c_size_t)]
+        L.scw_sweep_intensity.argtypes = L.scw_sweep_wavelengths.argtypes
+        L.scw_sweep_intensity_workspace.argtypes = L.scw_sweep_workspace.argtypes
         L.scw_exterior_spectra.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, c_void_p, c_void_p, c_int64]
         L.scw_exterior_points.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, c_void_p, c_void_p]
         L.scw_exterior_points_workspace.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, POINTER(c_size_t)]
@@ -367,6 +370,22 @@ def scw_sweep_wavelengths(ctx, layers, zs, x, y, out=None, strides=None):
     Ep = (c_void_p * max(n, 1))(*[e.data_ptr() for e in out])
     sarr = None if strides is None else (c_int64 * 4)(*strides)
     ctx.check(ctx.L.scw_sweep_wavelengths(ctx._h, n, inst, Fz, zp, Nx, _p(x), Ny, _p(y), Ep, sarr))
+    return out
+
+
+def scw_sweep_intensity(ctx, layers, zs, x, y, out=None, strides=None):
+    """Detector intensity I = sum_comp |E_comp|^2 of every instance (real tensors [Fz, Ny, Nx]); E is never stored."""
+    n, inst, Fz, zp = _sweep_args(layers, zs)
+    Nx, Ny = x.numel(), y.numel()
+    need = c_size_t()
+    ctx.check(ctx.L.scw_sweep_intensity_workspace(ctx._h, n, inst, Fz, Nx, Ny, byref(need)))
+    ctx.reserve(need.value)
+    if out is None:
+        real = {torch.complex64: torch.float32, torch.complex128: torch.float64}
+        out = [torch.empty((z.numel(), Ny, Nx), dtype=real[l.V.dtype], device=ctx.device) for l, z in zip(layers, zs)]
+    Ip = (c_void_p * max(n, 1))(*[e.data_ptr() for e in out])
+    sarr = None if strides is None else (c_int64 * 3)(*strides)
+    ctx.check(ctx.L.scw_sweep_intensity(ctx._h, n, inst, Fz, zp, Nx, _p(x), Ny, _p(y), Ip, sarr))
     return out
 
 

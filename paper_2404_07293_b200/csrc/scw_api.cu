@@ -434,25 +434,47 @@ static size_t sweep_ws(const scw_ctx* ctx, const scw_layer* L0, int64_t fz_max, 
            synth_ws(ctx, L0->dtype, L0->U, L0->Vn, fz_max, Ny);
 }
 
-int32_t scw_sweep_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, int64_t Nx,
-                            int64_t Ny, size_t* bytes)
+// workspace of a sweep; the general (non-grouped) detector path adds a planar E buffer for one instance
+static size_t sweep_need(const scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, int64_t fz_max,
+                         size_t asm_max, int64_t Nx, int64_t Ny, bool intensity)
+{
+    if (!n_inst || fz_max == 0) return 0;
+    const int group = sweep_group_size(ctx, n_inst, inst, Fz);
+    if (group) return sweep_group_ws(ctx, &inst[0], Fz[0], group, Nx, Ny);
+    return sweep_ws(ctx, &inst[0], fz_max, asm_max, Nx, Ny) +
+           (intensity ? align_up((size_t)fz_max * 3 * Nx * Ny * esize(inst[0].dtype)) : 0);
+}
+
+static int32_t sweep_workspace_impl(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, int64_t Nx,
+                                    int64_t Ny, size_t* bytes, bool intensity, const char* who)
 {
     if (!ctx || !bytes) return SCW_ERR_NULL;
     ctx->msg[0] = 0;
     int64_t fz_max = 0;
     size_t asm_max = 0;
-    if (int32_t s = check_sweep(ctx, n_inst, inst, Fz, Nx, Ny, "scw_sweep_workspace", &fz_max, &asm_max)) return s;
-    const int group = n_inst ? sweep_group_size(ctx, n_inst, inst, Fz) : 0;
-    *bytes = !n_inst ? 0 : group ? sweep_group_ws(ctx, &inst[0], Fz[0], group, Nx, Ny)
-                                 : sweep_ws(ctx, &inst[0], fz_max, asm_max, Nx, Ny);
+    if (int32_t s = check_sweep(ctx, n_inst, inst, Fz, Nx, Ny, who, &fz_max, &asm_max)) return s;
+    *bytes = sweep_need(ctx, n_inst, inst, Fz, fz_max, asm_max, Nx, Ny, intensity);
     return SCW_OK;
+}
+
+int32_t scw_sweep_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, int64_t Nx,
+                            int64_t Ny, size_t* bytes)
+{
+    return sweep_workspace_impl(ctx, n_inst, inst, Fz, Nx, Ny, bytes, false, "scw_sweep_workspace");
+}
+
+int32_t scw_sweep_intensity_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, int64_t Nx,
+                                      int64_t Ny, size_t* bytes)
+{
+    return sweep_workspace_impl(ctx, n_inst, inst, Fz, Nx, Ny, bytes, true, "scw_sweep_intensity_workspace");
 }
 
 // Shared by the device- and host-buffer variants: everything after validation.
 static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, const double* const* z,
                       int64_t Nx, const double* x, int64_t Ny, const double* y, void* const* E, const int64_t s4[4],
-                      int64_t fz_max, size_t asm_max, Carver& cv)
+                      int64_t fz_max, size_t asm_max, Carver& cv, bool intensity = false)
 {
+    // intensity: E[i] are real buffers receiving sum_comp |E_comp|^2 at n*s4[1] + k*s4[2] + i*s4[3] (NEXT-3)
     const scw_layer& L0 = inst[0];
     const int64_t R = 3LL * L0.U * L0.Vn;
     const Twiddles tw = run_twiddles(ctx, L0.dtype, L0.U, L0.Vn, L0.X, L0.Y, Nx, x, Ny, y, cv);
@@ -469,10 +491,10 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
             launch_tc_assemble_group_partials(ctx, g, inst + i0, Fz[0], z + i0, a_scr, &parts);
             if (ctx->tc_error) return;
             if (tc_synth_partials_supported(L0.U, L0.Vn, parts)) {
-                launch_tc_synth_group_partials(ctx, L0.U, L0.Vn, Fz[0], g, parts, Nx, Ny, tw.a, E + i0, s4, s_scr);
+                launch_tc_synth_group_partials(ctx, L0.U, L0.Vn, Fz[0], g, parts, Nx, Ny, tw.a, E + i0, s4, s_scr, intensity);
             } else {
                 launch_tc_assemble_group(ctx, g, inst + i0, Fz[0], z + i0, P_all, R, R * Fz[0], a_scr);
-                launch_tc_synth_group(ctx, L0.U, L0.Vn, Fz[0], g, P_all, R, Nx, Ny, tw.a, E + i0, s4, s_scr);
+                launch_tc_synth_group(ctx, L0.U, L0.Vn, Fz[0], g, P_all, R, Nx, Ny, tw.a, E + i0, s4, s_scr, intensity);
             }
         }
         return;
@@ -481,45 +503,70 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
     const size_t asm_off = cv.off;
     cv.take(asm_max);
     void* scratch = cv.take(synth_ws(ctx, L0.dtype, L0.U, L0.Vn, fz_max, Ny));
+    void* E_tmp = intensity ? cv.take((size_t)fz_max * 3 * Nx * Ny * esize(L0.dtype)) : nullptr;   // general detector path
+    int64_t planar[4];
+    planar_strides(Nx, Ny, planar);
     for (int64_t i = 0; i < n_inst; ++i) {
         if (Fz[i] == 0) continue;
         Carver sub(cv.base ? cv.base + asm_off : nullptr);
         run_assemble(ctx, &inst[i], Fz[i], z[i], P, R, sub);
-        run_synth(ctx, tw, L0.dtype, L0.U, L0.Vn, Fz[i], P, R, Nx, Ny, E[i], s4, scratch);
+        if (intensity) {
+            run_synth(ctx, tw, L0.dtype, L0.U, L0.Vn, Fz[i], P, R, Nx, Ny, E_tmp, planar, scratch);
+            launch_intensity(ctx, L0.dtype, Fz[i], Ny, Nx, E_tmp, E[i], s4 + 1);
+        } else {
+            run_synth(ctx, tw, L0.dtype, L0.U, L0.Vn, Fz[i], P, R, Nx, Ny, E[i], s4, scratch);
+        }
     }
+}
+
+static int32_t sweep_impl(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, const double* const* z,
+                          int64_t Nx, const double* x, int64_t Ny, const double* y, void* const* E, const int64_t* strides,
+                          bool intensity, const char* who)
+{
+    if (int32_t s = check_ctx(ctx)) return s;
+    int64_t fz_max = 0;
+    size_t asm_max = 0;
+    if (int32_t s = check_sweep(ctx, n_inst, inst, Fz, Nx, Ny, who, &fz_max, &asm_max)) return s;
+    if (n_inst == 0 || fz_max == 0) return SCW_OK;
+    if (int32_t s = check_grid(ctx, inst[0].dtype, inst[0].U, inst[0].Vn, inst[0].X, inst[0].Y, Nx, x, Ny, y, who)) return s;
+    if (!z || !E) return fail(ctx, SCW_ERR_NULL, "%s: z and the output array are required", who);
+    const size_t out_es = intensity ? esize(inst[0].dtype) / 2 : esize(inst[0].dtype);
+    for (int64_t i = 0; i < n_inst; ++i) {
+        if (Fz[i] == 0) continue;
+        if (!z[i] || !E[i]) return fail(ctx, SCW_ERR_NULL, "%s: z[%lld] / output[%lld] is NULL", who, (long long)i, (long long)i);
+        if (!aligned(z[i], 8) || !aligned(E[i], out_es))
+            return fail(ctx, SCW_ERR_ALIGN, "%s: z[%lld] / output[%lld] misaligned", who, (long long)i, (long long)i);
+    }
+    int64_t s4[4];
+    if (intensity) {                                   // (z, y, x) strides in s4[1..3]; the component slot is unused
+        s4[0] = 0;
+        if (strides) memcpy(s4 + 1, strides, 3 * sizeof(int64_t));
+        else { s4[1] = Nx * Ny; s4[2] = Nx; s4[3] = 1; }
+    } else if (strides) {
+        memcpy(s4, strides, sizeof(s4));
+    } else {
+        planar_strides(Nx, Ny, s4);
+    }
+    for (int i = 0; i < 4; ++i)
+        if (s4[i] < 0) return fail(ctx, SCW_ERR_SHAPE, "%s: negative stride", who);
+    if (int32_t s = need_ws(ctx, sweep_need(ctx, n_inst, inst, Fz, fz_max, asm_max, Nx, Ny, intensity), who)) return s;
+    Carver cv(ctx->ws);
+    run_sweep(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, E, s4, fz_max, asm_max, cv, intensity);
+    return check_launch(ctx, who);
 }
 
 int32_t scw_sweep_wavelengths(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz,
                               const double* const* z, int64_t Nx, const double* x, int64_t Ny, const double* y,
                               void* const* E, const int64_t* strides)
 {
-    if (int32_t s = check_ctx(ctx)) return s;
-    int64_t fz_max = 0;
-    size_t asm_max = 0;
-    if (int32_t s = check_sweep(ctx, n_inst, inst, Fz, Nx, Ny, "scw_sweep_wavelengths", &fz_max, &asm_max)) return s;
-    if (n_inst == 0 || fz_max == 0) return SCW_OK;
-    if (int32_t s = check_grid(ctx, inst[0].dtype, inst[0].U, inst[0].Vn, inst[0].X, inst[0].Y, Nx, x, Ny, y,
-                               "scw_sweep_wavelengths")) return s;
-    if (!z || !E) return fail(ctx, SCW_ERR_NULL, "scw_sweep_wavelengths: z and E are required");
-    for (int64_t i = 0; i < n_inst; ++i) {
-        if (Fz[i] == 0) continue;
-        if (!z[i] || !E[i]) return fail(ctx, SCW_ERR_NULL, "scw_sweep_wavelengths: z[%lld]/E[%lld] is NULL", (long long)i, (long long)i);
-        if (!aligned(z[i], 8) || !aligned(E[i], esize(inst[0].dtype)))
-            return fail(ctx, SCW_ERR_ALIGN, "scw_sweep_wavelengths: z[%lld]/E[%lld] misaligned", (long long)i, (long long)i);
-    }
-    int64_t s4[4];
-    if (strides) memcpy(s4, strides, sizeof(s4)); else planar_strides(Nx, Ny, s4);
-    for (int i = 0; i < 4; ++i)
-        if (s4[i] < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_sweep_wavelengths: negative stride");
-    {
-        const int group = sweep_group_size(ctx, n_inst, inst, Fz);
-        const size_t need = group ? sweep_group_ws(ctx, &inst[0], Fz[0], group, Nx, Ny)
-                                  : sweep_ws(ctx, &inst[0], fz_max, asm_max, Nx, Ny);
-        if (int32_t s = need_ws(ctx, need, "scw_sweep_wavelengths")) return s;
-    }
-    Carver cv(ctx->ws);
-    run_sweep(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, E, s4, fz_max, asm_max, cv);
-    return check_launch(ctx, "scw_sweep_wavelengths");
+    return sweep_impl(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, E, strides, false, "scw_sweep_wavelengths");
+}
+
+int32_t scw_sweep_intensity(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz,
+                            const double* const* z, int64_t Nx, const double* x, int64_t Ny, const double* y,
+                            void* const* I, const int64_t* strides)
+{
+    return sweep_impl(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, I, strides, true, "scw_sweep_intensity");
 }
 
 // ------------------------------------------------------------------------------------------

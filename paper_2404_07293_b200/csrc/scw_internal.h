@@ -92,6 +92,10 @@ void launch_simt_synth(scw_ctx* ctx, int dtype, int U, int Vn, int64_t Fz, const
                        int64_t Nx, const void* FxT, int64_t Ny, const void* FyT, void* E,
                        const int64_t strides[4], void* scratch);
 
+// I[n][k][i] = sum_comp |E[n][comp][k][i]|^2, E planar, I at n*s3[0] + k*s3[1] + i*s3[2]
+void launch_intensity(scw_ctx* ctx, int dtype, int64_t Fz, int64_t Ny, int64_t Nx, const void* E, void* I,
+                      const int64_t s3[3]);
+
 // ---- scw_tc_assemble.cu: tcgen05 BF16x3 spectral assembly (complex64) ----------------------------
 bool tc_assemble_supported(int dtype, int64_t R, int64_t J, int64_t Fz, const void* V, int64_t ldV);
 int tc_assemble_max_group();
@@ -124,14 +128,15 @@ void launch_tc_synth_twiddles(scw_ctx* ctx, int U, int Vn, double X, double Y, i
                               const double* y, void* tw);
 int tc_synth_max_group();
 // n_inst instances with equal Fz, spectra back to back in P_all ([ldP x n_inst*Fz]); scratch = tc_synth_scratch(U, Vn, Fz*n_inst)
+// intensity: E[i] are float buffers receiving I = sum_comp |E_comp|^2 at z*strides[1] + y*strides[2] + x*strides[3]
 void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const void* P_all, int64_t ldP,
                            int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
-                           void* scratch);
+                           void* scratch, bool intensity = false);
 // Same, reading the spectra as stream-K partial tiles (segment reduce fused into the image pass).
 bool tc_synth_partials_supported(int U, int Vn, const TcPartials& parts);
 void launch_tc_synth_group_partials(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const TcPartials& parts,
                                     int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
-                                    void* scratch);
+                                    void* scratch, bool intensity = false);
 void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,
                      const void* tw, void* E, const int64_t strides[4], void* scratch);
 

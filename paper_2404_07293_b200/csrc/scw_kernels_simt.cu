@@ -344,4 +344,38 @@ void launch_simt_synth(scw_ctx* ctx, int dtype, int U, int Vn, int64_t Fz, const
     else run_simt_synth<double>(ctx, U, Vn, Fz, P, ldP, Nx, FxT, Ny, FyT, E, strides, scratch);
 }
 
+// ------------------------------------------------------------------------------------------
+// NEXT-3 detector, general path: I[n][k][i] = sum_comp |E[n][comp][k][i]|^2 from a planar E (the tensor-core synthesis
+// fuses this into its epilogue instead).
+template <typename T>
+__global__ void k_intensity(int64_t Fz, int64_t Ny, int64_t Nx, const typename C2<T>::type* __restrict__ E,
+                            T* __restrict__ I, int64_t s_z, int64_t s_y, int64_t s_x)
+{
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t plane = Nx * Ny;
+    if (idx >= Fz * plane) return;
+    const int64_t n = idx / plane, rem = idx - n * plane;
+    const int64_t k = rem / Nx, i = rem - k * Nx;
+    T acc = 0;
+#pragma unroll
+    for (int comp = 0; comp < 3; ++comp) {
+        const typename C2<T>::type e = E[(n * 3 + comp) * plane + rem];
+        acc += e.x * e.x + e.y * e.y;
+    }
+    I[n * s_z + k * s_y + i * s_x] = acc;
+}
+
+void launch_intensity(scw_ctx* ctx, int dtype, int64_t Fz, int64_t Ny, int64_t Nx, const void* E, void* I,
+                      const int64_t s3[3])
+{
+    const int64_t n = Fz * Ny * Nx;
+    KernelScope ks(ctx, KC_MISC);
+    if (dtype == SCW_C64)
+        k_intensity<float><<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(Fz, Ny, Nx, (const float2*)E, (float*)I,
+                                                                                   s3[0], s3[1], s3[2]);
+    else
+        k_intensity<double><<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(Fz, Ny, Nx, (const double2*)E, (double*)I,
+                                                                                    s3[0], s3[1], s3[2]);
+}
+
 }  // namespace scw

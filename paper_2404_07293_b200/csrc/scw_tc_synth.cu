@@ -59,7 +59,10 @@ struct TsParams {
     int K1p, K2p;          // padded 2*Vc, 2*Uc  (N1 == K2p)
     int nuc, nvc;          // frequency chunks along u and v
     int tiles_x, tiles_y, pair0, npairs;   // this launch covers tile pairs [pair0, pair0 + npairs)
-    int* sched;            // [tile pair] next plane to hand out (zeroed by the spectrum-image kernel)
+    int* sched;            // [tile pair] next plane group to hand out (zeroed by the spectrum-image kernel)
+    int group;             // planes per drawn unit: 1, or 3 (the components of one z) in intensity mode
+    int intensity;         // 1: E[] point to float outputs I = sum_comp |E_comp|^2 (NEXT-3 detector), no complex field stored
+    int acc_col;           // detector: first of 128 TMEM columns holding the running sum, 0 = none (sum kept in the output)
 };
 
 __host__ __device__ inline int ts_pad16(int v) { return (v + 15) / 16 * 16; }
@@ -259,6 +262,7 @@ __device__ __forceinline__ void ts_mma3_ts(uint32_t d_tmem, uint32_t ta_hi, uint
     }
 }
 
+template <bool INTENSITY>
 __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constant__ TsParams p)
 {
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -342,9 +346,11 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
     if (warp == 0) {
         // ===== loader: draws the planes; y twiddle images once, then the nuc*nvc spectrum images of every plane =====
         if (lane == 0) {
-            int q = 0;
+            int q = 0, g = 0;
             for (int nl = 0;; ++nl) {
-                int plane = atomicAdd(&p.sched[pair], 1);
+                const int c = nl % p.group;                 // a drawn unit is `group` consecutive planes
+                if (c == 0) g = atomicAdd(&p.sched[pair], 1);
+                int plane = g * p.group + c;
                 if (plane >= p.planes) plane = -1;
                 *reinterpret_cast<volatile int*>(&s_plane[nl & 7]) = plane;
                 mbar_arrive(&sched_full[nl & 7]);
@@ -455,15 +461,18 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                     float f[8];
 #pragma unroll
                     for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(t[i][e]);   // (Tr0, Ti0, ..., Tr3, Ti3)
-                    uint4 re_hi, re_lo, im_hi, im_lo;
-                    split_bf16x2(f[0], -f[1], re_hi.x, re_lo.x);
-                    split_bf16x2(f[2], -f[3], re_hi.y, re_lo.y);
-                    split_bf16x2(f[4], -f[5], re_hi.z, re_lo.z);
-                    split_bf16x2(f[6], -f[7], re_hi.w, re_lo.w);
-                    split_bf16x2(f[1], f[0], im_hi.x, im_lo.x);
-                    split_bf16x2(f[3], f[2], im_hi.y, im_lo.y);
-                    split_bf16x2(f[5], f[4], im_hi.z, im_lo.z);
-                    split_bf16x2(f[7], f[6], im_hi.w, im_lo.w);
+                    // one split per (T_r, T_i) pair; row (y,Re) holds (T_r, -T_i): sign flip of the upper half (round to
+                    // nearest is odd, so hi/lo of -t are -hi/-lo of t); row (y,Im) holds (T_i, T_r): the halves swapped.
+                    // The conversion instruction is the converters' scarce resource (16 lanes/clk/SM).
+                    uint32_t H[4], Lw[4];
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) split_bf16x2(f[2 * k], f[2 * k + 1], H[k], Lw[k]);
+                    const uint4 re_hi = make_uint4(H[0] ^ 0x80000000u, H[1] ^ 0x80000000u, H[2] ^ 0x80000000u, H[3] ^ 0x80000000u);
+                    const uint4 re_lo = make_uint4(Lw[0] ^ 0x80000000u, Lw[1] ^ 0x80000000u, Lw[2] ^ 0x80000000u, Lw[3] ^ 0x80000000u);
+                    const uint4 im_hi = make_uint4(__byte_perm(H[0], 0, 0x1032), __byte_perm(H[1], 0, 0x1032),
+                                                   __byte_perm(H[2], 0, 0x1032), __byte_perm(H[3], 0, 0x1032));
+                    const uint4 im_lo = make_uint4(__byte_perm(Lw[0], 0, 0x1032), __byte_perm(Lw[1], 0, 0x1032),
+                                                   __byte_perm(Lw[2], 0, 0x1032), __byte_perm(Lw[3], 0, 0x1032));
                     uint8_t* dst = row + (size_t)c * 2048;
                     *reinterpret_cast<uint4*>(dst) = re_hi;
                     *reinterpret_cast<uint4*>(dst + 16) = im_hi;
@@ -493,27 +502,65 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
             float2* const Einst = p.E[inst];
 #pragma unroll 1
             for (int h = 0; h < 2; ++h) {
+                const int64_t y0 = (int64_t)ty * TS_TILE + 64 * h + 32 * cg;
+                const int ny = (int)min((int64_t)32, p.Ny - y0);   // may be <= 0
                 mbar_wait(&d2_full[h], n & 1);
                 tc_fence_after();
                 if (warp == 12 && lane == 0) TS_MARK(n * 32 + 16 + 4 * h);
                 const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + TS_D2_COL + h * TS_TILE + 64 * cg;
-                uint32_t v[2][32];
-                tmem_ld32_raw(taddr, v[0]);
-                tmem_ld32_raw(taddr + 32, v[1]);
-                tmem_ld_wait();
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&d2_empty[h]);          // D2[h] is in registers now
-                if (warp == 12 && lane == 0) TS_MARK(n * 32 + 17 + 4 * h);
-                const int64_t y0 = (int64_t)ty * TS_TILE + 64 * h + 32 * cg;
-                const int ny = (int)min((int64_t)32, p.Ny - y0);   // may be <= 0
-                float2* out = Einst + comp * p.s_comp + zi * p.s_z + x * p.s_x + y0 * p.s_y;
-                if (x_ok) {
+                if (INTENSITY) {
+                    // detector: I = |E_x|^2 + |E_y|^2 + |E_z|^2.  The three components of a z plane come to this CTA in
+                    // order (group = 3) and every (x, y) belongs to one thread.  The running sum lives in TMEM (128 spare
+                    // columns, lane = x, column = y) when they exist (p.acc_col; then only the third component writes the
+                    // output), else in the output itself (read-modify-write through L2).
+                    float* io = reinterpret_cast<float*>(Einst) + zi * p.s_z + x * p.s_x + y0 * p.s_y;
+                    const uint32_t acc = tmem_base + ((uint32_t)(32 * q) << 16) + p.acc_col + h * 64 + 32 * cg;
+                    if (p.acc_col && comp > 0) tmem_st_wait();     // the previous component's sums have landed
 #pragma unroll
-                    for (int e = 0; e < 32; ++e) {
-                        if (e < ny)
-                            out[e * p.s_y] = make_float2(__uint_as_float(v[e >> 4][(2 * e) & 31]),
-                                                         __uint_as_float(v[e >> 4][(2 * e + 1) & 31]));
+                    for (int j = 0; j < 2; ++j) {                  // 16 y at a time
+                        uint32_t v[32];
+                        float a[16];
+                        tmem_ld32_raw(taddr + 32 * j, v);
+                        if (p.acc_col && comp > 0) tmem_ld16(acc + 16 * j, a);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int e = 0; e < 16; ++e) {
+                            const float re = __uint_as_float(v[2 * e]), im = __uint_as_float(v[2 * e + 1]);
+                            const float m2 = re * re + im * im;
+                            if (!p.acc_col && comp > 0 && x_ok && 16 * j + e < ny) a[e] = __ldcg(io + (16 * j + e) * p.s_y);
+                            a[e] = comp > 0 ? a[e] + m2 : m2;
+                        }
+                        if (p.acc_col && comp < 2) {
+                            uint32_t w[16];
+#pragma unroll
+                            for (int e = 0; e < 16; ++e) w[e] = __float_as_uint(a[e]);
+                            tmem_st16(acc + 16 * j, w);
+                        } else if (x_ok) {
+#pragma unroll
+                            for (int e = 0; e < 16; ++e)
+                                if (16 * j + e < ny) __stcg(io + (16 * j + e) * p.s_y, a[e]);
+                        }
+                    }
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&d2_empty[h]);      // D2[h] has been consumed
+                } else {
+                    uint32_t v[2][32];
+                    tmem_ld32_raw(taddr, v[0]);
+                    tmem_ld32_raw(taddr + 32, v[1]);
+                    tmem_ld_wait();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&d2_empty[h]);      // D2[h] is in registers now
+                    if (warp == 12 && lane == 0) TS_MARK(n * 32 + 17 + 4 * h);
+                    float2* out = Einst + comp * p.s_comp + zi * p.s_z + x * p.s_x + y0 * p.s_y;
+                    if (x_ok) {
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) {
+                            if (e < ny)
+                                out[e * p.s_y] = make_float2(__uint_as_float(v[e >> 4][(2 * e) & 31]),
+                                                             __uint_as_float(v[e >> 4][(2 * e + 1) & 31]));
+                        }
                     }
                 }
                 if (warp == 12 && lane == 0) TS_MARK(n * 32 + 18 + 4 * h);
@@ -595,7 +642,7 @@ static int* ts_sched(const TsPlan& pl, const void* tw)
 
 // The synthesis launches proper: B1 holds the spectrum images of all n_inst*Fz*3 planes.
 static void ts_launch_main(scw_ctx* ctx, const TsPlan& pl, int64_t Fz, int n_inst, const uint8_t* B1, int64_t Nx,
-                           int64_t Ny, const void* tw, void* const* E, const int64_t strides[4])
+                           int64_t Ny, const void* tw, void* const* E, const int64_t strides[4], bool intensity)
 {
     static thread_local TsParams p;
     const int planes = (int)(Fz * 3 * n_inst);
@@ -616,17 +663,26 @@ static void ts_launch_main(scw_ctx* ctx, const TsPlan& pl, int64_t Fz, int n_ins
     p.K2p = pl.K2p;
     p.nuc = pl.cu.n;
     p.nvc = pl.cv.n;
+    p.intensity = intensity ? 1 : 0;
+    p.group = intensity ? 3 : 1;
+    {   // detector accumulators go behind D2 | D1 | A2 when 128 TMEM columns are left (U <= 32)
+        const int used = TS_D1_COL + pl.K2p * (1 + pl.cu.n);
+        p.acc_col = (intensity && used + 128 <= TS_TMEM_COLS) ? used : 0;
+    }
+    const size_t smem_bytes = pl.smem_bytes;
     p.tiles_x = pl.tiles_x;
     p.tiles_y = pl.tiles_y;
     const int total_pairs = pl.tiles_x * pl.tiles_y;
-    cudaFuncSetAttribute(k_tc_synth, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes);
+    if (intensity) cudaFuncSetAttribute(k_tc_synth<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    else cudaFuncSetAttribute(k_tc_synth<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     for (int pair0 = 0; pair0 < total_pairs; pair0 += ctx->sm_count) {
         p.pair0 = pair0;
         p.npairs = total_pairs - pair0 < ctx->sm_count ? total_pairs - pair0 : ctx->sm_count;
         int per_pair = ctx->sm_count / p.npairs;
         if (per_pair > planes) per_pair = planes;
         KernelScope ks(ctx, KC_SYNTH_TC);
-        k_tc_synth<<<p.npairs * per_pair, TS_THREADS, pl.smem_bytes, ctx->stream>>>(p);
+        if (intensity) k_tc_synth<true><<<p.npairs * per_pair, TS_THREADS, smem_bytes, ctx->stream>>>(p);
+        else k_tc_synth<false><<<p.npairs * per_pair, TS_THREADS, smem_bytes, ctx->stream>>>(p);
     }
 }
 
@@ -634,7 +690,7 @@ static void ts_launch_main(scw_ctx* ctx, const TsPlan& pl, int64_t Fz, int n_ins
 // (P_all is one column-major [ldP x n_inst*Fz] matrix): one image pre-kernel + one synthesis launch.
 void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const void* P_all, int64_t ldP,
                            int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
-                           void* scratch)
+                           void* scratch, bool intensity)
 {
     const TsPlan pl = ts_plan(U, Vn, Fz * n_inst, Nx, Ny);
     const int planes = (int)(Fz * 3 * n_inst);
@@ -647,7 +703,7 @@ void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, 
                                                                                 ldP, B1, ts_sched(pl, tw),
                                                                                 pl.tiles_x * pl.tiles_y);
     }
-    ts_launch_main(ctx, pl, Fz, n_inst, B1, Nx, Ny, tw, E, strides);
+    ts_launch_main(ctx, pl, Fz, n_inst, B1, Nx, Ny, tw, E, strides, intensity);
 }
 
 bool tc_synth_partials_supported(int U, int Vn, const TcPartials& parts)
@@ -657,7 +713,7 @@ bool tc_synth_partials_supported(int U, int Vn, const TcPartials& parts)
 
 void launch_tc_synth_group_partials(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const TcPartials& parts,
                                     int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
-                                    void* scratch)
+                                    void* scratch, bool intensity)
 {
     const TsPlan pl = ts_plan(U, Vn, Fz * n_inst, Nx, Ny);
     const int planes = (int)(Fz * 3 * n_inst);
@@ -671,13 +727,13 @@ void launch_tc_synth_group_partials(scw_ctx* ctx, int U, int Vn, int64_t Fz, int
                                                                             pl.K1p, pl.K2p, (int)Fz, parts, B1,
                                                                             ts_sched(pl, tw), pl.tiles_x * pl.tiles_y);
     }
-    ts_launch_main(ctx, pl, Fz, n_inst, B1, Nx, Ny, tw, E, strides);
+    ts_launch_main(ctx, pl, Fz, n_inst, B1, Nx, Ny, tw, E, strides, intensity);
 }
 
 void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,
                      const void* tw, void* E, const int64_t strides[4], void* scratch)
 {
-    launch_tc_synth_group(ctx, U, Vn, Fz, 1, P, ldP, Nx, Ny, tw, &E, strides, scratch);
+    launch_tc_synth_group(ctx, U, Vn, Fz, 1, P, ldP, Nx, Ny, tw, &E, strides, scratch, false);
 }
 
 }  // namespace scw
