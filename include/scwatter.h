@@ -180,8 +180,10 @@ int32_t scw_sweep_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst,
 
 /*
  * Same as scw_sweep_wavelengths with every array in HOST memory (V, c, gamma, dir, z[i], x, y, E[i];
- * pinned memory recommended): inputs are staged host->device into the workspace, evaluated, and E is
- * copied device->host, all on the ctx stream.  E[i] is planar [Fz][3][Ny][Nx].  h2d_bytes / d2h_bytes
+ * pinned memory required for overlap): inputs are staged host->device into the workspace, evaluated, and E is
+ * copied device->host.  Two staging buffers each way and two internal copy streams pipeline the instances (the upload of
+ * instance i+1 and the download of instance i-1 run beside the kernels of instance i); the pipeline is forked from and
+ * joined back into the ctx stream with events, so results are complete in ctx-stream order.  E[i] is planar [Fz][3][Ny][Nx].  h2d_bytes / d2h_bytes
  * (HOST, may be NULL) receive the bytes copied in each direction.
  */
 int32_t scw_sweep_wavelengths_host(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst,

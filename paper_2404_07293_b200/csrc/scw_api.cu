@@ -235,6 +235,14 @@ int32_t scw_destroy(scw_ctx* ctx)
 {
     if (!ctx) return SCW_ERR_NULL;
     for (ProfRec& r : ctx->recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    if (ctx->h2d_stream) cudaStreamDestroy(ctx->h2d_stream);
+    if (ctx->d2h_stream) cudaStreamDestroy(ctx->d2h_stream);
+    if (ctx->ev_start) cudaEventDestroy(ctx->ev_start);
+    for (int b = 0; b < 2; ++b) {
+        if (ctx->ev_in[b]) cudaEventDestroy(ctx->ev_in[b]);
+        if (ctx->ev_done[b]) cudaEventDestroy(ctx->ev_done[b]);
+        if (ctx->ev_out[b]) cudaEventDestroy(ctx->ev_out[b]);
+    }
     delete ctx;
     return SCW_OK;
 }
@@ -604,7 +612,7 @@ int32_t scw_sweep_host_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* 
     size_t asm_max = 0, in_max = 0, e_max = 0;
     if (int32_t s = sweep_host_sizes(ctx, n_inst, inst, Fz, Nx, Ny, "scw_sweep_host_workspace", &fz_max, &asm_max,
                                      &in_max, &e_max)) return s;
-    *bytes = n_inst ? align_up((size_t)Nx * 8) + align_up((size_t)Ny * 8) + in_max + e_max +
+    *bytes = n_inst ? align_up((size_t)Nx * 8) + align_up((size_t)Ny * 8) + 2 * in_max + 2 * e_max +
                           sweep_ws(ctx, &inst[0], fz_max, asm_max, Nx, Ny)
                     : 0;
     return SCW_OK;
@@ -627,26 +635,40 @@ int32_t scw_sweep_wavelengths_host(scw_ctx* ctx, int64_t n_inst, const scw_layer
     if (!z || !E) return fail(ctx, SCW_ERR_NULL, "scw_sweep_wavelengths_host: z and E are required");
     for (int64_t i = 0; i < n_inst; ++i)
         if (Fz[i] > 0 && (!z[i] || !E[i])) return fail(ctx, SCW_ERR_NULL, "scw_sweep_wavelengths_host: z[i]/E[i] is NULL");
-    const size_t total = align_up((size_t)Nx * 8) + align_up((size_t)Ny * 8) + in_max + e_max +
+    const size_t total = align_up((size_t)Nx * 8) + align_up((size_t)Ny * 8) + 2 * in_max + 2 * e_max +
                          sweep_ws(ctx, &inst[0], fz_max, asm_max, Nx, Ny);
     if (int32_t s = need_ws(ctx, total, "scw_sweep_wavelengths_host")) return s;
+
+    // copy streams and events are created on first use
+    cudaError_t err = cudaSuccess;
+    auto ok = [&](cudaError_t e) { if (err == cudaSuccess) err = e; };
+    if (!ctx->h2d_stream) {
+        ok(cudaStreamCreateWithFlags(&ctx->h2d_stream, cudaStreamNonBlocking));
+        ok(cudaStreamCreateWithFlags(&ctx->d2h_stream, cudaStreamNonBlocking));
+        ok(cudaEventCreateWithFlags(&ctx->ev_start, cudaEventDisableTiming));
+        for (int b = 0; b < 2; ++b) {
+            ok(cudaEventCreateWithFlags(&ctx->ev_in[b], cudaEventDisableTiming));
+            ok(cudaEventCreateWithFlags(&ctx->ev_done[b], cudaEventDisableTiming));
+            ok(cudaEventCreateWithFlags(&ctx->ev_out[b], cudaEventDisableTiming));
+        }
+    }
 
     Carver cv(ctx->ws);
     double* dx = (double*)cv.take((size_t)Nx * 8);
     double* dy = (double*)cv.take((size_t)Ny * 8);
-    char* stage_in = (char*)cv.take(in_max);
-    char* stage_e = (char*)cv.take(e_max);
+    char* stage_in[2], *stage_e[2];
+    for (int b = 0; b < 2; ++b) stage_in[b] = (char*)cv.take(in_max);
+    for (int b = 0; b < 2; ++b) stage_e[b] = (char*)cv.take(e_max);
     const scw_layer& L0 = inst[0];
     const size_t es = esize(L0.dtype);
     const int64_t R = 3LL * L0.U * L0.Vn;
     int64_t up = 0, down = 0;
-    cudaError_t err = cudaSuccess;
-    auto h2d = [&](void* d, const void* h, size_t n) {
-        if (err == cudaSuccess) err = cudaMemcpyAsync(d, h, n, cudaMemcpyHostToDevice, ctx->stream);
+    auto h2d = [&](void* d, const void* h, size_t n, cudaStream_t st) {
+        ok(cudaMemcpyAsync(d, h, n, cudaMemcpyHostToDevice, st));
         up += (int64_t)n;
     };
-    h2d(dx, x, (size_t)Nx * 8);
-    h2d(dy, y, (size_t)Ny * 8);
+    h2d(dx, x, (size_t)Nx * 8, ctx->stream);
+    h2d(dy, y, (size_t)Ny * 8, ctx->stream);
     const Twiddles tw = run_twiddles(ctx, L0.dtype, L0.U, L0.Vn, L0.X, L0.Y, Nx, dx, Ny, dy, cv);
     void* P = cv.take((size_t)R * fz_max * es);
     const size_t asm_off = cv.off;
@@ -654,31 +676,52 @@ int32_t scw_sweep_wavelengths_host(scw_ctx* ctx, int64_t n_inst, const scw_layer
     void* scratch = cv.take(synth_ws(ctx, L0.dtype, L0.U, L0.Vn, fz_max, Ny));
     int64_t s4[4];
     planar_strides(Nx, Ny, s4);
+    // Pipeline over instances, two staging buffers each way: the host->device copy of instance i+1 and the device->host
+    // copy of instance i-1 run on their own streams beside the kernels of instance i (full-duplex PCIe).  Everything is
+    // ordered after the work already on the ctx stream (ev_start) and joined back into it at the end.
+    ok(cudaEventRecord(ctx->ev_start, ctx->stream));
+    ok(cudaStreamWaitEvent(ctx->h2d_stream, ctx->ev_start, 0));
+    ok(cudaStreamWaitEvent(ctx->d2h_stream, ctx->ev_start, 0));
+    int64_t used[2] = {0, 0};                          // how many instances went through buffer b so far
+    int64_t k = 0;
     for (int64_t i = 0; i < n_inst && err == cudaSuccess; ++i) {
         if (Fz[i] == 0) continue;
+        const int b = (int)(k++ & 1);
         scw_layer L = inst[i];
-        Carver st(stage_in);
+        Carver st(stage_in[b]);
         void* dV = st.take((size_t)L.ldV * L.J * es);
         void* dc = st.take((size_t)L.J * es);
         void* dg = st.take((size_t)L.J * 16);
         void* dd = st.take((size_t)L.J);
         void* dz = st.take((size_t)Fz[i] * 8);
-        h2d(dV, L.V, (size_t)L.ldV * L.J * es);
-        if (L.c) h2d(dc, L.c, (size_t)L.J * es);
-        h2d(dg, L.gamma, (size_t)L.J * 16);
-        if (L.dir) h2d(dd, L.dir, (size_t)L.J);
-        h2d(dz, z[i], (size_t)Fz[i] * 8);
+        // inputs of buffer b may be overwritten once the kernels of its previous user are done
+        if (used[b]) ok(cudaStreamWaitEvent(ctx->h2d_stream, ctx->ev_done[b], 0));
+        h2d(dV, L.V, (size_t)L.ldV * L.J * es, ctx->h2d_stream);
+        if (L.c) h2d(dc, L.c, (size_t)L.J * es, ctx->h2d_stream);
+        h2d(dg, L.gamma, (size_t)L.J * 16, ctx->h2d_stream);
+        if (L.dir) h2d(dd, L.dir, (size_t)L.J, ctx->h2d_stream);
+        h2d(dz, z[i], (size_t)Fz[i] * 8, ctx->h2d_stream);
+        ok(cudaEventRecord(ctx->ev_in[b], ctx->h2d_stream));
         L.V = dV;
         L.c = L.c ? dc : nullptr;
         L.gamma = (const double*)dg;
         L.dir = L.dir ? (const int8_t*)dd : nullptr;
+        // kernels: need this instance's inputs, and the output buffer back from the copy of its previous user
+        ok(cudaStreamWaitEvent(ctx->stream, ctx->ev_in[b], 0));
+        if (used[b]) ok(cudaStreamWaitEvent(ctx->stream, ctx->ev_out[b], 0));
         Carver sub((char*)ctx->ws + asm_off);
         run_assemble(ctx, &L, Fz[i], (const double*)dz, P, R, sub);
-        run_synth(ctx, tw, L0.dtype, L0.U, L0.Vn, Fz[i], P, R, Nx, Ny, stage_e, s4, scratch);
+        run_synth(ctx, tw, L0.dtype, L0.U, L0.Vn, Fz[i], P, R, Nx, Ny, stage_e[b], s4, scratch);
+        ok(cudaEventRecord(ctx->ev_done[b], ctx->stream));
         const size_t eb = (size_t)Fz[i] * 3 * Nx * Ny * es;
-        if (err == cudaSuccess) err = cudaMemcpyAsync(E[i], stage_e, eb, cudaMemcpyDeviceToHost, ctx->stream);
+        ok(cudaStreamWaitEvent(ctx->d2h_stream, ctx->ev_done[b], 0));
+        ok(cudaMemcpyAsync(E[i], stage_e[b], eb, cudaMemcpyDeviceToHost, ctx->d2h_stream));
+        ok(cudaEventRecord(ctx->ev_out[b], ctx->d2h_stream));
         down += (int64_t)eb;
+        used[b]++;
     }
+    for (int b = 0; b < 2; ++b)                        // join: results are complete in ctx-stream order
+        if (used[b]) ok(cudaStreamWaitEvent(ctx->stream, ctx->ev_out[b], 0));
     if (err != cudaSuccess) {
         ctx->cuda_err = (int32_t)err;
         return fail(ctx, SCW_ERR_CUDA, "scw_sweep_wavelengths_host: %s", cudaGetErrorString(err));

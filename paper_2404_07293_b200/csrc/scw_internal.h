@@ -19,6 +19,11 @@ struct scw_ctx {
     int device = 0;
     int sm_count = 148;
     cudaStream_t stream = nullptr;
+    // host-buffer sweep only: copy streams and events of the double-buffered staging pipeline (forked from and joined
+    // back into `stream`, so the caller still sees plain stream order)
+    cudaStream_t h2d_stream = nullptr, d2h_stream = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_in[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr},
+                ev_out[2] = {nullptr, nullptr};
     void* ws = nullptr;
     size_t ws_bytes = 0;
     int64_t path = SCW_PATH_AUTO;
