@@ -232,3 +232,33 @@ def test_stream_and_launch_counter(scw):
         s.synchronize()
     assert rel_err(E.cpu().numpy(), oracle.layer_grid(x=x, y=y, z=np.linspace(-0.4, 0.9, 2), **lay)) <= 1e-10
     c.close()
+
+
+def test_more_tiles_than_sms_and_more_instances_than_a_group(scw):
+    """Tensor path at its scheduling edges: 14 x 11 = 154 output tiles (two synthesis launches over the tile pairs, each
+    pair's planes handed out dynamically), and 70 instances (two groups of the grouped sweep); every sample against the
+    factored fp64 reference (Tier B, itself pinned to Tier A)."""
+    c = scw.Context(0)
+    c.set_path(scw.SCW_PATH_TENSOR)
+    try:
+        g = np.random.default_rng(23)
+        lay = ragged_layer(6, 5, 64, np.complex64, seed=77)
+        x = np.sort(g.uniform(-3, 9, 1700))
+        y = np.sort(g.uniform(-3, 9, 1300))
+        z = np.array([0.1, 0.7])
+        E = scw.scw_sweep_wavelengths(c, [scw.Layer.from_numpy(lay, "cuda")], [dev(z)], dev(x), dev(y))[0]
+        torch.cuda.synchronize()
+        assert rel_err(E.cpu().numpy(), oracle.tier_b_grid(x=x, y=y, z=z, **lay)) <= 2e-4
+        lays = [ragged_layer(4, 3, 40, np.complex64, seed=200 + i, with_c=(i % 3 != 0)) for i in range(70)]
+        xs, ys = np.linspace(0, 3, 33), np.linspace(0, 4.5, 140)
+        zs = [np.array([0.0, 0.3 + 0.01 * i, 0.9]) for i in range(70)]
+        Es = scw.scw_sweep_wavelengths(c, [scw.Layer.from_numpy(l, "cuda") for l in lays], [dev(v) for v in zs], dev(xs), dev(ys))
+        I = scw.scw_sweep_intensity(c, [scw.Layer.from_numpy(l, "cuda") for l in lays], [dev(v) for v in zs], dev(xs), dev(ys))
+        torch.cuda.synchronize()
+        for i in (0, 1, 63, 64, 69):
+            ref = oracle.tier_b_grid(x=xs, y=ys, z=zs[i], **lays[i])
+            assert rel_err(Es[i].cpu().numpy(), ref) <= 2e-4
+            Iref = oracle.intensity(ref)
+            assert np.abs(I[i].cpu().numpy() - Iref).max() / Iref.max() <= 4e-4
+    finally:
+        c.close()
