@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- field samples/s of the sCWatter hot path on B200.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--all]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--skip-large]
 
 A step is one pass of the grid hot path (mode weights -> spectral assembly -> twiddles -> separable
 synthesis, batched over layers by scw_sweep_wavelengths = a-7) over
@@ -272,7 +272,7 @@ def run_ours(args):
 
 
 def extra_workloads(torch, scw, ctx, device, args, peaks):
-    """Config 3 (point path) and config 4 (sweep) at full size; config 2 / config 1 c128 / config 3' with --all."""
+    """Configs 3 (point path), 4 (sweep, detector), exterior field, 2, 1 complex128 and 3' at full size."""
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(device)
     extra = {}
     # config 3: 4e6 scattered points x 4356 plane waves
@@ -332,7 +332,7 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
         ns = planes * cfgx.Nx * cfgx.Ny
         extra[name] = dict(ms_per_call=ms, samples_per_s=ns / (ms * 1e-3), orders=cfgx.U * cfgx.Vn, planes=planes,
                            hbm_write_frac=ns * 24 / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
-    if args.all:
+    if not args.skip_large:
         c1, layers, zs1, x1, y1 = config1_inputs(np.complex128)
         Ls = [scw.Layer.from_numpy(d, device) for d in layers]
         out = [torch.empty((c1.planes, 3, c1.Ny, c1.Nx), dtype=torch.complex128, device=device) for _ in Ls]
@@ -425,7 +425,8 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--all", action="store_true", help="also time config 2, config 1 complex128 and config 3'")
+    ap.add_argument("--all", action="store_true", help="(default now) also time config 2, config 1 complex128, config 3'")
+    ap.add_argument("--skip-large", action="store_true", help="skip config 2, config 1 complex128 and config 3' (extra)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--quick", action="store_true", help="only the resident-input step (for ncu captures)")
     args = ap.parse_args()
