@@ -342,8 +342,8 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
         gf = c1.n_layers * (8 * 3 * M1 * 4 * M1 * c1.planes + 8 * 3 * c1.planes * (M1 * c1.Ny + c1.Nx * c1.U * c1.Ny)) / 1e9
         extra["config1_c128"] = dict(ms_per_call=ms, samples_per_s=c1.n_layers * c1.planes * c1.Nx * c1.Ny / (ms * 1e-3),
                                      roofline=dict(bound="tensor", achieved=gf / ms, peak=FP64_DMMA_PEAK_TFLOPS,
-                                                   unit="TFLOP/s (useful fp64, 8 per complex MAC; peak = measured "
-                                                        "mma.sync m8n8k4 f64 rate, DESIGN.md 5)",
+                                                   unit="TFLOP/s (useful fp64, 8 per complex MAC; the 3M kernel executes 6; peak = "
+                                                        "measured mma.sync m8n8k4 f64 rate, DESIGN.md 5)",
                                                    frac=gf / ms / FP64_DMMA_PEAK_TFLOPS, traffic=None))
         del Ls, out, layers
         torch.cuda.empty_cache()

@@ -2,13 +2,14 @@
 // eq. 31 / PAPER.md:332-334, 428-432) and both passes of the separable synthesis E = F_x P F_y^T (a-4, eq. 10 /
 // PAPER.md:119-124).  tcgen05 has no FP64 kind, so this path uses the warp-level mma.sync instruction.
 //
-// One batched complex GEMM kernel C[b] = A[b] B[b] serves the three uses.  Complex on a real MMA: the complex
-// product is the real product of A' = [[A_r, -A_i], [A_i, A_r]] (rows 2m+c, columns 2k+c') with B' = [B_r; B_i]
-// (rows 2k+c'), so that D[2m+c, n] is component c of C[m, n] -- no cross-lane combine.  An 8x4 A' fragment covers 4
-// complex rows x 2 complex k: lane (g, t) picks ONE component of A[m0 + g/2, k0 + t/2] (component (g^t)&1, negated
-// for g even / t odd); a 4x8 B' fragment lane (t, g) picks component t&1 of B[k0 + t/2, n0 + g]: both are 8-byte
-// shared-memory loads of the interleaved complex tiles, conflict-free with the row paddings below.
-// Every product and sum is fp64 (IEEE fma inside the tensor core): the 1e-10 bar holds as on the CUDA-core path.
+// One batched complex GEMM kernel C[b] = A[b] B[b] serves the three uses.  The complex product runs as THREE real
+// products ("3M"): T1 = A_r B_r, T2 = A_i B_i, T3 = (A_r + A_i)(B_r + B_i), C_r = T1 - T2, C_i = T3 - T1 - T2 --
+// a quarter fewer tensor-core flops than the four-product form, which matters because this path is bound by the FP64
+// tensor rate (37 TFLOP/s measured, equal to the FP64 FMA rate).  An 8x4 A fragment lane (g, t) loads the complex
+// element A[m0 + g, k0 + t] with one 16-byte shared-memory load and forms (re, im, re + im); a 4x8 B fragment lane
+// (t, g) does the same with B[k0 + t, n0 + g]; the row paddings below make both loads conflict-free.
+// Every product and sum is fp64 (IEEE fma inside the tensor core).  3M is normwise as accurate as the direct product
+// (error ~ a few ulp of |A||B| per term); the 1e-10 bar is relative to max|E|, five orders above that.
 #include "scw_internal.h"
 
 namespace scw {
@@ -17,8 +18,8 @@ constexpr int DG_TM = 64, DG_TN = 64;      // CTA tile in complex elements
 constexpr int DG_KB = 16;                  // complex k per pipeline stage
 constexpr int DG_STAGES = 3;
 constexpr int DG_THREADS = 256;            // 8 warps = 4 (m) x 2 (n); warp tile 16 complex rows x 32 columns
-constexpr int DG_LDA = DG_TM + 2;          // row strides (complex) chosen so that the two k rows of a fragment
-constexpr int DG_LDB = DG_TN + 4;          // fall into disjoint banks
+constexpr int DG_LDA = DG_TM + 2;          // row strides (complex): 66 * 16 B = 32 B mod 128, so the four k rows of a
+constexpr int DG_LDB = DG_TN + 2;          // fragment fall into disjoint banks
 constexpr size_t DG_SMEM = (size_t)DG_STAGES * DG_KB * (DG_LDA + DG_LDB) * sizeof(double2);
 
 struct DgParams {
@@ -84,20 +85,22 @@ __global__ void __launch_bounds__(DG_THREADS, 2) k_dmma_cgemm(const DgParams p)
         }
     };
 
-    double acc[4][4][2];
+    // accumulators of the three real products: [m tile][n tile][T1, T2, T3][2 columns]
+    double acc[2][4][3][2];
 #pragma unroll
-    for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < 2; ++i)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+        for (int j = 0; j < 4; ++j)
+#pragma unroll
+            for (int q = 0; q < 3; ++q) acc[i][j][q][0] = acc[i][j][q][1] = 0.0;
 
     for (int s = 0; s < DG_STAGES - 1; ++s) {
         if (s < nstages) load_stage(s, k_begin + (int64_t)s * DG_KB);
         cp_async_commit();
     }
-    // fragment addressing (in doubles): A' lane (g,t): row g/2, k t/2, component (g^t)&1; B' lane (t,g): k t/2, column g
-    const int a_off = ((t >> 1) * DG_LDA + wm * 16 + (g >> 1)) * 2 + ((g ^ t) & 1);
-    const int b_off = ((t >> 1) * DG_LDB + wn * 32 + g) * 2 + (t & 1);
-    const bool a_neg = ((g & 1) == 0) && ((t & 1) == 1);
+    // fragment addressing (complex elements): A lane (g,t): row g, k t; B lane (t,g): k t, column g
+    const int a_off = t * DG_LDA + wm * 16 + g;
+    const int b_off = t * DG_LDB + wn * 32 + g;
 
     for (int st = 0; st < nstages; ++st) {
         cp_async_wait<DG_STAGES - 2>();
@@ -107,45 +110,53 @@ __global__ void __launch_bounds__(DG_THREADS, 2) k_dmma_cgemm(const DgParams p)
             if (nx < nstages) load_stage(nx % DG_STAGES, k_begin + (int64_t)nx * DG_KB);
             cp_async_commit();
         }
-        const double* as = reinterpret_cast<const double*>(As + (size_t)(st % DG_STAGES) * DG_KB * DG_LDA) + a_off;
-        const double* bs = reinterpret_cast<const double*>(Bs + (size_t)(st % DG_STAGES) * DG_KB * DG_LDB) + b_off;
-        auto k_step = [&](int k2) {
-            double a[4], b[4];
+        const double2* as = As + (size_t)(st % DG_STAGES) * DG_KB * DG_LDA + a_off;
+        const double2* bs = Bs + (size_t)(st % DG_STAGES) * DG_KB * DG_LDB + b_off;
+        auto k_step = [&](int k4) {                     // 4 complex k
+            double2 a[2], b[4];
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const double v = as[(k2 * 2 * DG_LDA + i * 4) * 2];
-                a[i] = a_neg ? -v : v;
-            }
+            for (int i = 0; i < 2; ++i) a[i] = as[k4 * 4 * DG_LDA + i * 8];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) b[j] = bs[(k2 * 2 * DG_LDB + j * 8) * 2];
+            for (int j = 0; j < 4; ++j) b[j] = bs[k4 * 4 * DG_LDB + j * 8];
+            double asum[2], bsum[4];
 #pragma unroll
-            for (int i = 0; i < 4; ++i)
+            for (int i = 0; i < 2; ++i) asum[i] = a[i].x + a[i].y;
 #pragma unroll
-                for (int j = 0; j < 4; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+            for (int j = 0; j < 4; ++j) bsum[j] = b[j].x + b[j].y;
+#pragma unroll
+            for (int i = 0; i < 2; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    dmma884(acc[i][j][0][0], acc[i][j][0][1], a[i].x, b[j].x);
+                    dmma884(acc[i][j][1][0], acc[i][j][1][1], a[i].y, b[j].y);
+                    dmma884(acc[i][j][2][0], acc[i][j][2][1], asum[i], bsum[j]);
+                }
         };
         const int64_t k_left = k_end - (k_begin + (int64_t)st * DG_KB);
         if (k_left >= DG_KB) {
 #pragma unroll
-            for (int k2 = 0; k2 < DG_KB / 2; ++k2) k_step(k2);
-        } else {                                        // ragged last stage: only the k pairs that hold data
-            const int k2n = (int)((k_left + 1) / 2);
+            for (int k4 = 0; k4 < DG_KB / 4; ++k4) k_step(k4);
+        } else {                                        // ragged last stage: only the k quads that hold data
+            const int k4n = (int)((k_left + 3) / 4);
 #pragma unroll 1
-            for (int k2 = 0; k2 < k2n; ++k2) k_step(k2);
+            for (int k4 = 0; k4 < k4n; ++k4) k_step(k4);
         }
     }
     cp_async_wait<0>();
 
-    // C fragment: lane (g,t) holds component g&1 of rows m = .. + g/2, columns 2t and 2t+1
-    double* Cd = reinterpret_cast<double*>(C);
+    // C fragment: lane (g,t) holds rows m = .. + g, columns 2t and 2t+1 of T1, T2, T3
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const int64_t m = m0 + wm * 16 + i * 4 + (g >> 1);
+    for (int i = 0; i < 2; ++i) {
+        const int64_t m = m0 + wm * 16 + i * 8 + g;
         if (m >= p.M) continue;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            const int64_t n = n0 + wn * 32 + j * 8 + 2 * t;
-            if (n < p.N) Cd[(m * p.sCm + n * p.sCn) * 2 + (g & 1)] = acc[i][j][0];
-            if (n + 1 < p.N) Cd[(m * p.sCm + (n + 1) * p.sCn) * 2 + (g & 1)] = acc[i][j][1];
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int64_t n = n0 + wn * 32 + j * 8 + 2 * t + e;
+                const double t1 = acc[i][j][0][e], t2 = acc[i][j][1][e], t3 = acc[i][j][2][e];
+                if (n < p.N) C[m * p.sCm + n * p.sCn] = make_double2(t1 - t2, t3 - t1 - t2);
+            }
         }
     }
 }
