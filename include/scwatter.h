@@ -106,7 +106,7 @@ typedef struct {
     double z_lo, z_hi;         /* z_{l-1}, z_l: the layer's interfaces (eq. 30) */
     int64_t J;                 /* number of modes (columns of V), normally 4*U*Vn (eq. 23) */
     const void* V;             /* [ldV x J] column-major complex<dtype>, rows comp*M+m (eq. 28, 34) */
-    int64_t ldV;               /* >= 3*U*Vn */
+    int64_t ldV;               /* >= 3*U*Vn; any value works, 64-byte aligned columns (ldV % 8 == 0 for C64) save ~3 % */
     const void* c;             /* [J] complex<dtype> coefficients alpha_j, NULL = ones (eq. 23) */
     const double* gamma;       /* [J] complex128 signed z-wavenumbers Gamma_jj (eq. 22-23) */
     const int8_t* dir;         /* [J] +1 / -1 reference face, NULL = derive from the sign of gamma */
