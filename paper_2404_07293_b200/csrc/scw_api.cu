@@ -38,6 +38,7 @@ int32_t check_ctx(scw_ctx* ctx)
     ctx->cuda_err = 0;
     ctx->required_ws = 0;
     ctx->tc_error = false;
+    ctx->prof_last = nullptr;       // per-kernel timers: the first kernel of this call gets its own start event
     int cur = -1;
     cudaError_t e = cudaGetDevice(&cur);
     if (e == cudaSuccess && cur != ctx->device) e = cudaSetDevice(ctx->device);
@@ -234,7 +235,7 @@ int32_t scw_create(scw_ctx** out, int32_t device, void* cuda_stream)
 int32_t scw_destroy(scw_ctx* ctx)
 {
     if (!ctx) return SCW_ERR_NULL;
-    for (ProfRec& r : ctx->recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (ProfRec& r : ctx->recs) { if (r.owns_a) cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     if (ctx->h2d_stream) cudaStreamDestroy(ctx->h2d_stream);
     if (ctx->d2h_stream) cudaStreamDestroy(ctx->d2h_stream);
     if (ctx->ev_start) cudaEventDestroy(ctx->ev_start);
@@ -297,10 +298,13 @@ static void profile_drain(scw_ctx* ctx)
             ctx->prof_ms[r.kc] += (double)ms;
             ctx->prof_n[r.kc] += 1;
         }
-        cudaEventDestroy(r.a);
+    }
+    for (ProfRec& r : ctx->recs) {                     // a record's start event may be its predecessor's end event
+        if (r.owns_a) cudaEventDestroy(r.a);
         cudaEventDestroy(r.b);
     }
     ctx->recs.clear();
+    ctx->prof_last = nullptr;
 }
 
 int32_t scw_profile_read(scw_ctx* ctx, int32_t kc, double* ms_total, int64_t* launches)

@@ -12,7 +12,7 @@ enum KernelClass {
     KC_WEIGHTS = 0, KC_TWIDDLES, KC_ASSEMBLE, KC_REDUCE, KC_SYNTH_A, KC_SYNTH_B, KC_POINTS_TABLE, KC_POINTS,
     KC_POINT_SYNTH, KC_MISC, KC_ASSEMBLE_TC, KC_SYNTH_TC, KC_SYNTH_IMG, KC_ASSEMBLE_DMMA, KC_SYNTH_A_DMMA, KC_SYNTH_B_DMMA, KC_EXTERIOR, KC_COUNT
 };
-struct ProfRec { cudaEvent_t a, b; int kc; };
+struct ProfRec { cudaEvent_t a, b; int kc; bool owns_a; };
 }  // namespace scw
 
 struct scw_ctx {
@@ -33,6 +33,7 @@ struct scw_ctx {
     char msg[256] = {0};
     bool profile = false;
     bool tc_error = false;          // a tensor map could not be encoded (reported by the entry point)
+    cudaEvent_t prof_last = nullptr;   // profiling: end event of the previous kernel of this API call
     std::vector<scw::ProfRec> recs;
     double prof_ms[scw::KC_COUNT] = {0};
     int64_t prof_n[scw::KC_COUNT] = {0};
@@ -42,8 +43,10 @@ namespace scw {
 
 inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
-// Brackets one kernel launch: counts it and, when profiling is on, records CUDA events around it
-// on the ctx stream (read back by scw_profile_read).
+// Brackets one kernel launch: counts it and, when profiling is on, times it with CUDA events on the ctx stream (read
+// back by scw_profile_read).  A kernel's interval runs from the end event of the previous kernel of the same API call
+// (a fresh start event for the first one) to its own end event: one event between consecutive kernels, and the
+// intervals of a call add up to the call's span on the device, dependency gaps included.
 struct KernelScope {
     scw_ctx* ctx;
     ProfRec rec;
@@ -53,15 +56,21 @@ struct KernelScope {
         ctx->launches++;
         rec.kc = kc;
         if (on) {
-            cudaEventCreate(&rec.a);
+            rec.owns_a = ctx->prof_last == nullptr;
+            if (rec.owns_a) {
+                cudaEventCreate(&rec.a);
+                cudaEventRecord(rec.a, ctx->stream);
+            } else {
+                rec.a = ctx->prof_last;
+            }
             cudaEventCreate(&rec.b);
-            cudaEventRecord(rec.a, ctx->stream);
         }
     }
     ~KernelScope()
     {
         if (on) {
             cudaEventRecord(rec.b, ctx->stream);
+            ctx->prof_last = rec.b;
             ctx->recs.push_back(rec);
         }
     }
