@@ -209,16 +209,16 @@ __global__ void __launch_bounds__(TS_PI_THREADS) k_tc_synth_pimage_partials(int 
             }
         }
     }
-    // row (u,Re): (P_r, -P_i) per v;  row (u,Im): (P_i, P_r)
-    uint4 re_hi, re_lo, im_hi, im_lo;
-    split_bf16x2(pv[0].x, -pv[0].y, re_hi.x, re_lo.x);
-    split_bf16x2(pv[1].x, -pv[1].y, re_hi.y, re_lo.y);
-    split_bf16x2(pv[2].x, -pv[2].y, re_hi.z, re_lo.z);
-    split_bf16x2(pv[3].x, -pv[3].y, re_hi.w, re_lo.w);
-    split_bf16x2(pv[0].y, pv[0].x, im_hi.x, im_lo.x);
-    split_bf16x2(pv[1].y, pv[1].x, im_hi.y, im_lo.y);
-    split_bf16x2(pv[2].y, pv[2].x, im_hi.z, im_lo.z);
-    split_bf16x2(pv[3].y, pv[3].x, im_hi.w, im_lo.w);
+    // row (u,Re): (P_r, -P_i) per v;  row (u,Im): (P_i, P_r): one split per entry, the two rows by sign flip / half swap
+    uint32_t H[4], Lw[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) split_bf16x2(pv[e].x, pv[e].y, H[e], Lw[e]);
+    const uint4 re_hi = make_uint4(H[0] ^ 0x80000000u, H[1] ^ 0x80000000u, H[2] ^ 0x80000000u, H[3] ^ 0x80000000u);
+    const uint4 re_lo = make_uint4(Lw[0] ^ 0x80000000u, Lw[1] ^ 0x80000000u, Lw[2] ^ 0x80000000u, Lw[3] ^ 0x80000000u);
+    const uint4 im_hi = make_uint4(__byte_perm(H[0], 0, 0x1032), __byte_perm(H[1], 0, 0x1032), __byte_perm(H[2], 0, 0x1032),
+                                   __byte_perm(H[3], 0, 0x1032));
+    const uint4 im_lo = make_uint4(__byte_perm(Lw[0], 0, 0x1032), __byte_perm(Lw[1], 0, 0x1032), __byte_perm(Lw[2], 0, 0x1032),
+                                   __byte_perm(Lw[3], 0, 0x1032));
     const size_t img_bytes = (size_t)N1 * K1p * 2;
     const int row = 2 * ul;                                       // rows 2ul and 2ul+1 sit in the same 8-row core matrix
     uint8_t* dst = img + (size_t)image * 2 * img_bytes + (size_t)kc * (N1 * 16) + (size_t)(row >> 3) * 128 + (row & 7) * 16;
