@@ -287,9 +287,11 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
     uint64_t* sched_full = bars + 15;    // [8] plane ids handed from the loader to the other roles
     int* s_plane = reinterpret_cast<int*>(bars + 23);               // [8]
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 27);
+    uint64_t* a2_full = bars + 28;       // [1] x twiddles are in TMEM (converter warps -> MMA warp)
 
     if (tid == 0) {
         mbar_init(tw_full, 1);
+        mbar_init(a2_full, 8);
         for (int s = 0; s < 8; ++s) mbar_init(&sched_full[s], 1);
         for (int s = 0; s < 2; ++s) {
             mbar_init(&b1_full[s], 1);
@@ -337,10 +339,10 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
             }
         }
         tmem_st_wait();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(a2_full);           // only GEMM2 needs A2: the other roles do not wait for it
     }
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
     TS_BLK(1);
 
     if (warp == 0) {
@@ -396,6 +398,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
             };
             auto issue_gemm2 = [&](int i, int h) {     // D2[h] (+)= A2[uc] B2[h]; complete after the last u chunk
                 const int n = i / nuc, uc = i - n * nuc;
+                if (i == 0 && h == 0) mbar_wait(a2_full, 0);
                 mbar_wait(&b2_full[h], i & 1);
                 TS_MARK(i * 32 + 2 + 4 * h);
                 if (uc == 0) mbar_wait(&d2_empty[h], (n & 1) ^ 1);
