@@ -386,7 +386,20 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
 #pragma unroll 1
             for (int b = 0; b < 2; ++b) {
                 const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(buf * 2 * p.N2 + b * p.N2);
-                for (int i0 = 0; i0 < p.Fzt; i0 += 8) {
+                int i0 = 0;
+                for (; i0 + 16 <= p.Fzt; i0 += 16) {              // 16 planes per TMEM round trip
+                    float a[16], bb[16];
+                    tmem_ld16(taddr + i0, a);
+                    tmem_ld16(taddr + p.Fzt + i0, bb);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) {
+                        const float recv = __shfl_xor_sync(0xffffffffu, bb[e], 1);
+                        // even lane: Re = D[2r,i] - D[2r+1,Fzt+i];  odd lane: Im = D[2r+1,i] + D[2r,Fzt+i]
+                        out[(size_t)(i0 + e) * (2 * TA_ROWS) + b * 128] = (lane & 1) ? a[e] + recv : a[e] - recv;
+                    }
+                }
+                for (; i0 < p.Fzt; i0 += 8) {                     // Fzt is a multiple of 8
                     float a[8], bb[8];
                     tmem_ld8(taddr + i0, a);
                     tmem_ld8(taddr + p.Fzt + i0, bb);
@@ -394,7 +407,6 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
 #pragma unroll
                     for (int e = 0; e < 8; ++e) {
                         const float recv = __shfl_xor_sync(0xffffffffu, bb[e], 1);
-                        // even lane: Re = D[2r,i] - D[2r+1,Fzt+i];  odd lane: Im = D[2r+1,i] + D[2r,Fzt+i]
                         out[(size_t)(i0 + e) * (2 * TA_ROWS) + b * 128] = (lane & 1) ? a[e] + recv : a[e] - recv;
                     }
                 }
