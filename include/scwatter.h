@@ -138,6 +138,9 @@ typedef struct {
  *   P[:, i] = V . ( c o g(z_i) ),  g_j(z) = G(gamma_j, zref_j, z) = exp(i k gamma_j (z - zref_j))  (eq. 7)
  * z: [Fz] doubles (device).  P: [ldP x Fz] column-major complex<dtype>, ldP >= 3*U*Vn.
  * z outside [z_lo, z_hi] is evaluated as-is.  Workspace: see scw_assemble_workspace().
+ * Domain: every phase gamma_j (z - zref_j) / lambda is reduced to a fraction of a turn in fp64 (rint) before the
+ * trigonometric functions, for both dtypes: any finite z gives the correctly reduced phase (the fp64 product itself
+ * carries 2^-53 |phase| turns of rounding, which is what limits complex128 beyond ~1e5 turns).
  */
 int32_t scw_assemble_spectra(scw_ctx* ctx, const scw_layer* layer, int64_t Fz, const double* z,
                              void* P, int64_t ldP);
@@ -160,6 +163,12 @@ int32_t scw_synthesize_workspace(scw_ctx* ctx, int32_t dtype, int32_t U, int32_t
 /*
  * Scattered points (eq. 3 / eq. 9-10 for SCW_MODES_PLANEWAVE, eq. 34 for SCW_MODES_DENSE).
  * r: [N x 3] doubles (x,y,z per point).  E: [N x 3] complex<dtype>, comp fastest.
+ * Domain: any finite coordinates.  The phase k s . r is range-reduced in fp64: SCW_C128 reduces every term with rint;
+ * SCW_C64 takes phases relative to the first point r_0 of the call (the per-wave phase at r_0 is reduced with rint)
+ * and sums the three fp64 products onto the constant 1.5 * 2^20, exact while the phase relative to r_0 stays below
+ * 2^19 turns; a block of 512 points that holds a point beyond that bound (|s|_max |r - r_0| / lambda >= 524 000)
+ * reduces every term with rint as well, at ~1.3x the time for that block.  The amplitude exponent
+ * -k Im(gamma) (z - zref) is evaluated in fp32 relative to z_0: its error grows as 2^-24 k |Im gamma| |z - z_0|.
  */
 int32_t scw_eval_points(scw_ctx* ctx, const scw_modes* modes, int64_t N, const double* r, void* E);
 int32_t scw_points_workspace(scw_ctx* ctx, const scw_modes* modes, int64_t N, size_t* bytes);
@@ -242,6 +251,20 @@ int32_t scw_sweep_intensity(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst,
                             void* const* I, const int64_t* strides);
 int32_t scw_sweep_intensity_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz,
                                       int64_t Nx, int64_t Ny, size_t* bytes);
+
+/* ---------------------------------------------------------------- roofline denominators (measurement helper)
+ *
+ * Runs a small microbenchmark of one hardware unit on the ctx stream and returns its measured rate (best of `reps`
+ * launches, CUDA events).  Unlike every other call this one SYNCHRONISES the stream.  buf: device scratch of `bytes`
+ * bytes (contents destroyed); the HBM units stream through all of it -- pass >= 1 GiB so that it exceeds the L2;
+ * the arithmetic units need 256 bytes.  value (HOST): TFLOP/s for FP64_DMMA (mma.sync.m8n8k4.f64, the complex128
+ * contractions) and FP32_FMA, Gop/s for MUFU (ex2.approx: the pipe of the point path's sin / cos / ex2), GB/s for
+ * HBM_READ (16-byte loads), HBM_WRITE (16-byte st.global) and HBM_WRITE_TMA (16 KB cp.async.bulk shared -> global).
+ * Errors: NULL, VALUE (unknown unit, reps < 1), CUDA.
+ */
+enum { SCW_PEAK_FP64_DMMA = 0, SCW_PEAK_FP32_FMA = 1, SCW_PEAK_MUFU = 2, SCW_PEAK_HBM_READ = 3, SCW_PEAK_HBM_WRITE = 4,
+       SCW_PEAK_HBM_WRITE_TMA = 5 };
+int32_t scw_measure_peak(scw_ctx* ctx, int32_t which, void* buf, size_t bytes, int32_t reps, double* value);
 
 #ifdef __cplusplus
 }

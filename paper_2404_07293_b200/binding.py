@@ -30,7 +30,10 @@ EXPORTS = [
     "scw_profile_classes", "scw_profile_name", "scw_profile_read", "scw_profile_reset",
     "scw_exterior_spectra", "scw_exterior_points", "scw_exterior_points_workspace",
     "scw_sweep_intensity", "scw_sweep_intensity_workspace",
+    "scw_measure_peak",
 ]
+SCW_PEAKS = {"fp64_dmma_tflops": 0, "fp32_fma_tflops": 1, "mufu_gops": 2, "hbm_read_gbs": 3, "hbm_write_gbs": 4,
+             "hbm_write_tma_gbs": 5}
 SCW_SIDE_ABOVE, SCW_SIDE_BELOW = 0, 1
 
 
@@ -110,6 +113,7 @@ def lib():
         L.scw_exterior_spectra.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, c_void_p, c_void_p, c_int64]
         L.scw_exterior_points.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, c_void_p, c_void_p]
         L.scw_exterior_points_workspace.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, POINTER(c_size_t)]
+        L.scw_measure_peak.argtypes = [c_void_p, c_int32, c_void_p, c_size_t, c_int32, POINTER(c_double)]
         _LIB = L
     return _LIB
 
@@ -264,6 +268,16 @@ class Context:
             self.check(self.L.scw_profile_read(self._h, kc, byref(ms), byref(n)))
             if n.value:
                 out[self.L.scw_profile_name(kc).decode()] = (ms.value, n.value)
+        return out
+
+    def measure_peaks(self, reps=5, hbm_bytes=1 << 30):
+        """{unit: measured rate} from the library's microbenchmarks (scw_measure_peak); synchronises the stream."""
+        buf = torch.empty(int(hbm_bytes), dtype=torch.uint8, device=self.device)
+        out = {}
+        for name, which in SCW_PEAKS.items():
+            v = c_double()
+            self.check(self.L.scw_measure_peak(self._h, which, c_void_p(buf.data_ptr()), buf.numel(), reps, byref(v)))
+            out[name] = v.value
         return out
 
     def reserve(self, nbytes):

@@ -424,8 +424,8 @@ static int sweep_group_size(const scw_ctx* ctx, int64_t n_inst, const scw_layer*
 {
     if (n_inst < 1 || Fz[0] <= 0) return 0;
     if (!use_tc_assemble(ctx, &inst[0], Fz[0]) || !use_tc_synth(ctx, inst[0].dtype, inst[0].U, inst[0].Vn)) return 0;
-    for (int64_t i = 1; i < n_inst; ++i)
-        if (inst[i].J != inst[0].J || Fz[i] != Fz[0]) return 0;
+    for (int64_t i = 1; i < n_inst; ++i)        // every instance must be able to take the TMA path (16-byte aligned V, ...)
+        if (inst[i].J != inst[0].J || Fz[i] != Fz[0] || !use_tc_assemble(ctx, &inst[i], Fz[i])) return 0;
     int g = tc_assemble_max_group() < tc_synth_max_group() ? tc_assemble_max_group() : tc_synth_max_group();
     return (int)(n_inst < g ? n_inst : g);
 }

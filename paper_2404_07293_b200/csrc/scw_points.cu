@@ -7,42 +7,67 @@
 // without a rint); sin/cos/exp2 run on the MUFU pipe, the three complex MACs as packed fp32
 // FMAs (FFMA2).  Every thread carries PPT points so that one broadcast read of a mode entry
 // from shared memory feeds PPT term evaluations.
+// Domain: the magic-constant reduction is exact only while |phase| < 2^19 turns.  Phases are therefore taken relative
+// to the first point r_0 of the call (the per-mode part a_j . r_0 is reduced with rint in fp64 by the table kernel
+// and folded into c0), so the limit applies to the EXTENT of the point cloud, not to its distance from the origin;
+// a block that holds a point whose bound |a|_max . |r - r_0| reaches 2^19 turns takes a second loop that reduces every
+// term with rint first (any finite coordinate is then evaluated correctly, at ~1.3x the cost for that block).
 #include "scw_internal.h"
 
 namespace scw {
 
 constexpr double PW_MAGIC = 1572864.0;             // 1.5 * 2^20: ulp = 2^-32 turn
+constexpr double PW_FAST_LIMIT = 524000.0;         // < 2^19 - 1: |phase relative to r_0| up to here takes the fast loop
+#ifndef SCW_PW_PPT
+#define SCW_PW_PPT 4
+#endif
+#ifndef SCW_PW_MINBLOCKS
+#define SCW_PW_MINBLOCKS 1
+#endif
 constexpr int PW_THREADS = 128;
-constexpr int PW_PPT = 4;                          // points per thread
+constexpr int PW_PPT = SCW_PW_PPT;                 // points per thread
 constexpr int PW_CHUNK = 256;                      // modes staged per shared-memory chunk
 
 struct __align__(16) PwMode {                      // 96 bytes
-    double ax, ay, az, c0;                         // turns per unit length; c0 = MAGIC - az*zref
-    float nkap, ke0, pad0, pad1;                   // log2-amplitude = nkap*z32 + ke0
+    double ax, ay, az, c0;                         // turns per unit length; c0 = MAGIC + frac(a . r_0 - az*zref)
+    float nkap, ke0, pad0, pad1;                   // log2-amplitude = nkap*(z - z_0) + ke0
     float prr[3][2];                               // (p_re, p_re) per component
     float pii[3][2];                               // (p_im, p_im) per component
 };
 static_assert(sizeof(PwMode) == 96, "PwMode layout");
 
+// Table header (first 256 bytes of the table buffer, zeroed before k_points_table): max_j |ax|, |ay|, |az| as the bit
+// patterns of non-negative doubles (monotone under unsigned compare, so atomicMax works).
+struct PwHeader { unsigned long long max_a[3]; };
+constexpr size_t PW_HEADER_BYTES = 256;
+
 template <typename T2>
 __global__ void k_points_table(int64_t J, double inv_lambda, const double* __restrict__ sx,
                                const double* __restrict__ sy, const double2* __restrict__ gamma,
                                const double* __restrict__ zref, const T2* __restrict__ p,
-                               PwMode* __restrict__ table)
+                               const double* __restrict__ r, PwHeader* __restrict__ hdr, PwMode* __restrict__ table)
 {
     const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= J) return;
-    const double origin = zref[0];
+    const double x0 = r[0], y0 = r[1], z0 = r[2];                 // phase origin: the first point of the call
     const double2 g = gamma[j];
     PwMode m;
     m.ax = sx[j] * inv_lambda;
     m.ay = sy[j] * inv_lambda;
     m.az = g.x * inv_lambda;
-    m.c0 = fma(-m.az, zref[j], PW_MAGIC);
+    // phase of the mode at r_0 in turns, each product reduced on its own (|a x_0| may be 1e5 turns and more)
+    double t0 = m.ax * x0;
+    t0 -= rint(t0);
+    double t1 = m.ay * y0;
+    t1 -= rint(t1);
+    double t2 = m.az * (z0 - zref[j]);
+    t2 -= rint(t2);
+    double f = t0 + t1 + t2;
+    f -= rint(f);
+    m.c0 = PW_MAGIC + f;
     const double kap = 6.283185307179586476925 * 1.4426950408889634074 * g.y * inv_lambda;
-    const float zr32 = (float)(zref[j] - origin);
     m.nkap = (float)(-kap);
-    m.ke0 = (float)(kap * (double)zr32);
+    m.ke0 = (float)(kap * (zref[j] - z0));
     m.pad0 = m.pad1 = 0.f;
     for (int c = 0; c < 3; ++c) {
         const T2 v = p[3 * j + c];
@@ -50,6 +75,18 @@ __global__ void k_points_table(int64_t J, double inv_lambda, const double* __res
         m.pii[c][0] = m.pii[c][1] = (float)v.y;
     }
     table[j] = m;
+    // per-axis maxima for the domain check of the fast loop: one atomic per warp and axis
+    double a3[3] = {fabs(m.ax), fabs(m.ay), fabs(m.az)};
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        unsigned long long b = (unsigned long long)__double_as_longlong(a3[k]);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const unsigned long long other = __shfl_xor_sync(__activemask(), b, o);
+            b = other > b ? other : b;
+        }
+        if ((threadIdx.x & 31) == 0) atomicMax(&hdr->max_a[k], b);
+    }
 }
 
 __device__ __forceinline__ float ex2_approx(float x)
@@ -59,32 +96,81 @@ __device__ __forceinline__ float ex2_approx(float x)
     return r;
 }
 
-__global__ void __launch_bounds__(PW_THREADS)
-k_points_pw_c64(int64_t J, int64_t N, const double* __restrict__ r, const PwMode* __restrict__ table,
-                const double* __restrict__ zref, float2* __restrict__ E)
+// One chunk of modes against the PPT points of the thread.  REDUCE: every term is first reduced with rint (phases of
+// any size); otherwise the three FMAs land directly on the magic constant (|phase| < 2^19 turns).
+template <bool REDUCE>
+__device__ __forceinline__ void pw_chunk(const PwMode* __restrict__ sm, int nj, const double (&x)[PW_PPT],
+                                         const double (&y)[PW_PPT], const double (&z)[PW_PPT], const float (&z32)[PW_PPT],
+                                         float2 (&A)[PW_PPT][3], float2 (&B)[PW_PPT][3])
+{
+#pragma unroll 1
+    for (int jj = 0; jj < nj; ++jj) {
+        const double2 a01 = *reinterpret_cast<const double2*>(&sm[jj].ax);
+        const double2 a23 = *reinterpret_cast<const double2*>(&sm[jj].az);
+        const float4 kk = *reinterpret_cast<const float4*>(&sm[jj].nkap);
+        const float4 p0 = *reinterpret_cast<const float4*>(&sm[jj].prr[0][0]);
+        const float4 p1 = *reinterpret_cast<const float4*>(&sm[jj].prr[2][0]);
+        const float4 p2 = *reinterpret_cast<const float4*>(&sm[jj].pii[1][0]);
+        const float2 prr0 = make_float2(p0.x, p0.y), prr1 = make_float2(p0.z, p0.w);
+        const float2 prr2 = make_float2(p1.x, p1.y), pii0 = make_float2(p1.z, p1.w);
+        const float2 pii1 = make_float2(p2.x, p2.y), pii2 = make_float2(p2.z, p2.w);
+#pragma unroll
+        for (int q = 0; q < PW_PPT; ++q) {
+            double t;
+            if (REDUCE) {
+                t = fma(a01.x, x[q], fma(a01.y, y[q], fma(a23.x, z[q], a23.y - PW_MAGIC)));
+                t = (t - rint(t)) + PW_MAGIC;
+            } else {
+                t = fma(a01.x, x[q], fma(a01.y, y[q], fma(a23.x, z[q], a23.y)));
+            }
+            const int ph = __double2loint(t);                 // frac(turns) * 2^32, signed
+            const float ang = __int2float_rn(ph) * 1.4629180792671596e-9f;   // 2 pi / 2^32
+            const float sn = __sinf(ang), cs = __cosf(ang);
+            const float amp = ex2_approx(fmaf(kk.x, z32[q], kk.y));
+            const float2 w = make_float2(amp * cs, amp * sn);
+            A[q][0] = __ffma2_rn(prr0, w, A[q][0]);
+            B[q][0] = __ffma2_rn(pii0, w, B[q][0]);
+            A[q][1] = __ffma2_rn(prr1, w, A[q][1]);
+            B[q][1] = __ffma2_rn(pii1, w, B[q][1]);
+            A[q][2] = __ffma2_rn(prr2, w, A[q][2]);
+            B[q][2] = __ffma2_rn(pii2, w, B[q][2]);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(PW_THREADS, SCW_PW_MINBLOCKS)
+k_points_pw_c64(int64_t J, int64_t N, const double* __restrict__ r, const PwHeader* __restrict__ hdr,
+                const PwMode* __restrict__ table, float2* __restrict__ E)
 {
     __shared__ PwMode sm[PW_CHUNK];
     const int tid = threadIdx.x;
     const int64_t base = (int64_t)blockIdx.x * (PW_THREADS * PW_PPT);
-    const double origin = zref[0];
+    const double x0 = r[0], y0 = r[1], z0 = r[2];
+    const double max_ax = __longlong_as_double((long long)hdr->max_a[0]);
+    const double max_ay = __longlong_as_double((long long)hdr->max_a[1]);
+    const double max_az = __longlong_as_double((long long)hdr->max_a[2]);
 
     double x[PW_PPT], y[PW_PPT], z[PW_PPT];
     float z32[PW_PPT];
     float2 A[PW_PPT][3], B[PW_PPT][3];
+    bool far = false;
 #pragma unroll
     for (int q = 0; q < PW_PPT; ++q) {
         int64_t ip = base + q * PW_THREADS + tid;
         if (ip >= N) ip = N - 1;
-        x[q] = r[3 * ip + 0];
-        y[q] = r[3 * ip + 1];
-        z[q] = r[3 * ip + 2];
-        z32[q] = (float)(z[q] - origin);
+        x[q] = r[3 * ip + 0] - x0;                  // coordinates relative to the first point
+        y[q] = r[3 * ip + 1] - y0;
+        z[q] = r[3 * ip + 2] - z0;
+        z32[q] = (float)z[q];
+        const double bound = fabs(x[q]) * max_ax + fabs(y[q]) * max_ay + fabs(z[q]) * max_az;
+        far = far || !(bound < PW_FAST_LIMIT);      // NaN / inf coordinates go to the reducing loop too
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             A[q][c] = make_float2(0.f, 0.f);
             B[q][c] = make_float2(0.f, 0.f);
         }
     }
+    const bool reduce = __syncthreads_or(far ? 1 : 0) != 0;    // block-uniform choice of the loop
 
     for (int64_t j0 = 0; j0 < J; j0 += PW_CHUNK) {
         const int nj = (int)min((int64_t)PW_CHUNK, J - j0);
@@ -96,33 +182,8 @@ k_points_pw_c64(int64_t J, int64_t N, const double* __restrict__ r, const PwMode
             for (int i = tid; i < n16; i += PW_THREADS) dst[i] = src[i];
         }
         __syncthreads();
-#pragma unroll 1
-        for (int jj = 0; jj < nj; ++jj) {
-            const double2 a01 = *reinterpret_cast<const double2*>(&sm[jj].ax);
-            const double2 a23 = *reinterpret_cast<const double2*>(&sm[jj].az);
-            const float4 kk = *reinterpret_cast<const float4*>(&sm[jj].nkap);
-            const float4 p0 = *reinterpret_cast<const float4*>(&sm[jj].prr[0][0]);
-            const float4 p1 = *reinterpret_cast<const float4*>(&sm[jj].prr[2][0]);
-            const float4 p2 = *reinterpret_cast<const float4*>(&sm[jj].pii[1][0]);
-            const float2 prr0 = make_float2(p0.x, p0.y), prr1 = make_float2(p0.z, p0.w);
-            const float2 prr2 = make_float2(p1.x, p1.y), pii0 = make_float2(p1.z, p1.w);
-            const float2 pii1 = make_float2(p2.x, p2.y), pii2 = make_float2(p2.z, p2.w);
-#pragma unroll
-            for (int q = 0; q < PW_PPT; ++q) {
-                const double t = fma(a01.x, x[q], fma(a01.y, y[q], fma(a23.x, z[q], a23.y)));
-                const int ph = __double2loint(t);                 // frac(turns) * 2^32, signed
-                const float ang = __int2float_rn(ph) * 1.4629180792671596e-9f;   // 2 pi / 2^32
-                const float sn = __sinf(ang), cs = __cosf(ang);
-                const float amp = ex2_approx(fmaf(kk.x, z32[q], kk.y));
-                const float2 w = make_float2(amp * cs, amp * sn);
-                A[q][0] = __ffma2_rn(prr0, w, A[q][0]);
-                B[q][0] = __ffma2_rn(pii0, w, B[q][0]);
-                A[q][1] = __ffma2_rn(prr1, w, A[q][1]);
-                B[q][1] = __ffma2_rn(pii1, w, B[q][1]);
-                A[q][2] = __ffma2_rn(prr2, w, A[q][2]);
-                B[q][2] = __ffma2_rn(pii2, w, B[q][2]);
-            }
-        }
+        if (reduce) pw_chunk<true>(sm, nj, x, y, z, z32, A, B);
+        else pw_chunk<false>(sm, nj, x, y, z, z32, A, B);
     }
     // E = (A.x - B.y, A.y + B.x): sum p_re*w + i p_im*w
 #pragma unroll
@@ -169,23 +230,25 @@ k_points_pw_c128(int64_t J, int64_t N, double inv_lambda, const double* __restri
 
 size_t points_table_bytes(int dtype, int64_t J)
 {
-    return dtype == SCW_C64 ? align_up((size_t)J * sizeof(PwMode)) : 0;
+    return dtype == SCW_C64 ? PW_HEADER_BYTES + align_up((size_t)J * sizeof(PwMode)) : 0;
 }
 
 void launch_points_planewave(scw_ctx* ctx, const scw_modes* m, int64_t N, const double* r, void* E,
                              void* table)
 {
     if (m->dtype == SCW_C64) {
+        PwHeader* hdr = static_cast<PwHeader*>(table);
+        PwMode* modes = reinterpret_cast<PwMode*>(static_cast<char*>(table) + PW_HEADER_BYTES);
+        cudaMemsetAsync(hdr, 0, sizeof(PwHeader), ctx->stream);
         {
             KernelScope ks(ctx, KC_POINTS_TABLE);
             k_points_table<float2><<<(unsigned)((m->J + 127) / 128), 128, 0, ctx->stream>>>(
-            m->J, 1.0 / m->lambda, m->sx, m->sy, (const double2*)m->gamma, m->zref, (const float2*)m->p,
-                (PwMode*)table);
+                m->J, 1.0 / m->lambda, m->sx, m->sy, (const double2*)m->gamma, m->zref, (const float2*)m->p, r, hdr, modes);
         }
         const int64_t per_block = PW_THREADS * PW_PPT;
         KernelScope ks(ctx, KC_POINTS);
         k_points_pw_c64<<<(unsigned)((N + per_block - 1) / per_block), PW_THREADS, 0, ctx->stream>>>(
-            m->J, N, r, (const PwMode*)table, m->zref, (float2*)E);
+            m->J, N, r, hdr, modes, (float2*)E);
     } else {
         KernelScope ks(ctx, KC_POINTS);
         k_points_pw_c128<<<(unsigned)((N + 127) / 128), 128, 0, ctx->stream>>>(

@@ -49,18 +49,6 @@ constexpr int TA_MAX_STG = 5;
 
 constexpr int TA_MAX_INST = 64;            // instances (layers x wavelengths) per grouped launch
 
-#ifdef SCW_TS_DEBUG
-__device__ long long g_ta_dbg[8192];
-#define TA_MARK(slot) do { if (blockIdx.x == 0 && (slot) < 8192) g_ta_dbg[(slot)] = clock64(); } while (0)
-__device__ long long g_ta_blk[4 * 256];
-__device__ __forceinline__ long long ta_gtime() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define TA_BLK(i) do { if (threadIdx.x == 0) { g_ta_blk[blockIdx.x * 4 + (i)] = clock64(); g_ta_blk[blockIdx.x * 4 + (i) + 2] = ta_gtime(); } } while (0)
-extern "C" void scw_debug_ta_read(long long* out) { cudaMemcpyFromSymbol(out, g_ta_dbg, sizeof(long long) * 8192); }
-extern "C" void scw_debug_ta_blk(long long* out) { cudaMemcpyFromSymbol(out, g_ta_blk, sizeof(long long) * 1024); }
-#else
-#define TA_MARK(slot) do { } while (0)
-#define TA_BLK(i) do { } while (0)
-#endif
 
 struct TaParams {
     CUtensorMap tmap[TA_MAX_INST][2];   // [0]: even columns of V, [1]: odd columns; box = 128 rows x 16 columns of 8 bytes
@@ -124,7 +112,9 @@ __global__ void __launch_bounds__(256) k_tc_weights(int n_inst, int64_t J, int64
             // phase in turns, reduced in fp64 by the magic-constant trick: the low word of t + 1.5*2^20 is
             // frac(t) * 2^32 (two's complement: an angle in [-pi, pi) after scaling), then the MUFU sin / cos / ex2
             // (abs. error ~5e-7, below the 2^-17 of the bf16 hi/lo split that follows)
-            const int ph = __double2loint(fma(g.x, dz, 1572864.0));
+            // (the product is reduced with rint first, so a thick layer with |gamma dz / lambda| >= 2^19 turns is fine)
+            const double tt = g.x * dz;
+            const int ph = __double2loint((tt - rint(tt)) + 1572864.0);
             const float ang = __int2float_rn(ph) * 1.4629180792671596e-9f;           // 2 pi / 2^32
             const float s = __sinf(ang), co = __cosf(ang);
             const float a = exp2f((float)(-9.0647202836543876194 * g.y * dz));        // exp(-2 pi x) = 2^(-2 pi log2(e) x)
@@ -214,7 +204,6 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
-    TA_BLK(0);
     const int64_t T = (int64_t)p.n_inst * p.n_tiles * p.m_tiles * p.kblocks;
     const int64_t it0 = (int64_t)blockIdx.x * T / gridDim.x;
     const int64_t it1 = (int64_t)(blockIdx.x + 1) * T / gridDim.x;
@@ -238,17 +227,12 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
         if (grp == 1) advance();
         const uint32_t a_lane = tmem_base + TA_A_COL + (uint32_t)((w >> 2) * 32) + ((uint32_t)(32 * (w & 3)) << 16);
         for (int64_t it = it0 + grp; it < it1; it += TA_CONV_GROUPS) {
-            [[maybe_unused]] const int dn = (int)(it - it0);
             if (w == 0) {                          // one warp polls, the other seven sleep on a named barrier
-                if (lane == 0) TA_MARK(dn * 16 + 0);
                 mbar_wait(&stg_full[ss], ps);
-                if (lane == 0) TA_MARK(dn * 16 + 1);
                 mbar_wait(&empty[sa], pa ^ 1);
-                if (lane == 0) TA_MARK(dn * 16 + 2);
             }
             named_bar_sync(1 + grp, TA_CONV_WARPS * 32);
             tc_fence_after();
-            if (w == 0 && lane == 0) TA_MARK(dn * 16 + 3);
             const uint8_t* src = stg_base + (size_t)ss * TA_STG_BYTES + (32 * w + lane) * 4;
             float v[32];
 #pragma unroll
@@ -271,10 +255,8 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
             __syncwarp();
             if (lane == 0) mbar_arrive(&stg_empty[ss]);        // staging slot is in registers now
             tmem_st_wait();
-            if (w == 0 && lane == 0) TA_MARK(dn * 16 + 4);
             tc_fence_before();
             mbar_arrive(&full_a[sa]);
-            if (w == 0 && lane == 0) TA_MARK(dn * 16 + 5);
             advance();
             advance();
         }
@@ -328,12 +310,9 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
             const uint32_t d_tmem = tmem_base + (uint32_t)(buf * 2 * p.N2);
             uint32_t acc = 0;
             for (; it < seg_end; ++it) {
-                TA_MARK((int)(it - it0) * 16 + 8);
                 mbar_wait(&full_a[stage], phase);
-                TA_MARK((int)(it - it0) * 16 + 9);
                 mbar_wait(&full_b[stage], phase);
                 tc_fence_after();
-                TA_MARK((int)(it - it0) * 16 + 10);
                 const uint32_t a0 = tmem_base + TA_A_COL + (uint32_t)stage * 64;       // TMEM columns: block b at +32b, lo at +16
                 const uint32_t b_hi = w0 + (uint32_t)stage * (uint32_t)w_stage_bytes;
                 const uint32_t b_lo = b_hi + (uint32_t)p.N2 * 64;
@@ -355,7 +334,6 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
                 }
                 __syncwarp();
                 acc = 1;
-                TA_MARK((int)(it - it0) * 16 + 11);
                 if (++stage == TA_MMA_STAGES) { stage = 0; phase ^= 1; }
             }
             if (elect_one()) umma_commit(&acc_full[buf]);
@@ -422,7 +400,6 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
     }
     tc_fence_before();
     __syncthreads();
-    TA_BLK(1);
     if (warp == TA_MMA_WARP) tmem_dealloc(tmem_base, TA_TMEM_COLS);
 }
 

@@ -35,17 +35,6 @@ constexpr int TS_MAX_INST = 64;            // instances per grouped launch
 #define SCW_TS_ORDER 0                     // 0: GEMM1(next item) before GEMM2 of this item (measured best with dynamic planes)
 #endif
 
-#ifdef SCW_TS_DEBUG
-__device__ long long g_ts_dbg[4096];
-#define TS_MARK(slot) do { if (blockIdx.x == 0 && (slot) < 4096) g_ts_dbg[(slot)] = clock64(); } while (0)
-__device__ long long g_ts_blk[4 * 256];
-__device__ __forceinline__ long long ts_gtime() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define TS_BLK(i) do { if (threadIdx.x == 0 && blockIdx.x < 256) g_ts_blk[blockIdx.x * 4 + (i)] = ts_gtime(); } while (0)
-extern "C" void scw_debug_ts_blk(long long* out) { cudaMemcpyFromSymbol(out, g_ts_blk, sizeof(long long) * 1024); }
-#else
-#define TS_MARK(slot) do { } while (0)
-#define TS_BLK(i) do { } while (0)
-#endif
 
 struct TsParams {
     const uint8_t* A1;     // [ty][vc][hi|lo] images of (Fy_r, Fy_i): 128 rows x K1p, K-major, LBO = 2048, SBO = 128
@@ -129,7 +118,7 @@ __global__ void k_tc_synth_pimage(int U, int Vn, int Uc, int Vc, int nuc, int nv
                                   int* __restrict__ sched, int n_sched)
 {
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;      // (image, row, kpair)
-    if (idx < n_sched) sched[idx] = 0;                                       // plane counters of the synthesis that follows
+    for (int64_t i = idx; i < n_sched; i += (int64_t)gridDim.x * blockDim.x) sched[i] = 0;   // plane counters of the synthesis that follows
     const int kpairs = K1p / 2;
     if (idx >= (int64_t)planes * nuc * nvc * N1 * kpairs) return;
     const int vl = (int)(idx % kpairs);
@@ -267,7 +256,6 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
 {
     extern __shared__ __align__(1024) uint8_t smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    TS_BLK(0);
     const int K1p = p.K1p, K2p = p.K2p, N1 = p.K2p, nuc = p.nuc, nvc = p.nvc;
     const uint32_t a1_img = TS_TILE * K1p * 2;                                 // bytes of one (hi or lo) image
     const uint32_t b1_img = (uint32_t)N1 * K1p * 2, b2_img = TS_TILE * K2p * 2;
@@ -343,7 +331,6 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
         __syncwarp();
         if (lane == 0) mbar_arrive(a2_full);           // only GEMM2 needs A2: the other roles do not wait for it
     }
-    TS_BLK(1);
 
     if (warp == 0) {
         // ===== loader: draws the planes; y twiddle images once, then the nuc*nvc spectrum images of every plane =====
@@ -385,7 +372,6 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                     mbar_wait(&b1_full[s], (q >> 1) & 1);
                     if (vc == 0 && i > 0) mbar_wait(d1_empty, (i - 1) & 1);
                     tc_fence_after();
-                    TS_MARK(i * 32 + 0);
                     if (elect_one()) {
                         ts_mma3_ss(d1, a1 + vc * 2 * a1_img, a1 + vc * 2 * a1_img + a1_img, 2048, b1 + s * 2 * b1_img,
                                    b1 + s * 2 * b1_img + b1_img, (uint32_t)N1 * 16, K1p, idesc1, vc > 0 ? 1u : 0u);
@@ -394,16 +380,13 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                     }
                     __syncwarp();
                 }
-                TS_MARK(i * 32 + 1);
             };
             auto issue_gemm2 = [&](int i, int h) {     // D2[h] (+)= A2[uc] B2[h]; complete after the last u chunk
                 const int n = i / nuc, uc = i - n * nuc;
                 if (i == 0 && h == 0) mbar_wait(a2_full, 0);
                 mbar_wait(&b2_full[h], i & 1);
-                TS_MARK(i * 32 + 2 + 4 * h);
                 if (uc == 0) mbar_wait(&d2_empty[h], (n & 1) ^ 1);
                 tc_fence_after();
-                TS_MARK(i * 32 + 3 + 4 * h);
                 const uint32_t ta = tmem_base + a2_col + uc * K2p;
                 if (elect_one()) {
                     ts_mma3_ts(tmem_base + TS_D2_COL + h * TS_TILE, ta, ta + K2p / 2, b2 + h * 2 * b2_img,
@@ -412,7 +395,6 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                     if (uc == nuc - 1) umma_commit(&d2_full[h]);
                 }
                 __syncwarp();
-                TS_MARK(i * 32 + 4 + 4 * h);
             };
             // GEMM1 of the next item goes first: it only needs D1 back from the converters (a TMEM load after d1_full) and
             // then runs on the tensor pipe while they split and store this item's B2
@@ -445,7 +427,6 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
             if (n % nuc == 0 && sched_get(n / nuc) < 0) break;
             mbar_wait(d1_full, n & 1);
             tc_fence_after();
-            if (warp == 4 && lane == 0) TS_MARK(n * 32 + 10);
             uint32_t t[5][8];
 #pragma unroll
             for (int i = 0; i < 5; ++i)
@@ -454,9 +435,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(d1_empty);    // D1 may be overwritten by the next plane's GEMM1
-            if (warp == 4 && lane == 0) TS_MARK(n * 32 + 11);
             mbar_wait(&b2_empty[h], (n & 1) ^ 1);
-            if (warp == 4 && lane == 0) TS_MARK(n * 32 + 12);
 #pragma unroll
             for (int i = 0; i < 5; ++i) {
                 const int c = 2 * i + kg;
@@ -483,11 +462,9 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                     *reinterpret_cast<uint4*>(dst + b2_img + 16) = im_lo;
                 }
             }
-            if (warp == 4 && lane == 0) TS_MARK(n * 32 + 13);
             fence_proxy_async();
             __syncwarp();
             if (lane == 0) mbar_arrive(&b2_full[h]);
-            if (warp == 4 && lane == 0) TS_MARK(n * 32 + 14);
         }
     } else {
         // ===== epilogue: D2 (lane = x, columns = (y, Re/Im)) -> E.  Two warps per lane quarter, 32 y each. =====
@@ -509,7 +486,6 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                 const int ny = (int)min((int64_t)32, p.Ny - y0);   // may be <= 0
                 mbar_wait(&d2_full[h], n & 1);
                 tc_fence_after();
-                if (warp == 12 && lane == 0) TS_MARK(n * 32 + 16 + 4 * h);
                 const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + TS_D2_COL + h * TS_TILE + 64 * cg;
                 if (INTENSITY) {
                     // detector: I = |E_x|^2 + |E_y|^2 + |E_z|^2.  The three components of a z plane come to this CTA in
@@ -555,7 +531,6 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&d2_empty[h]);      // D2[h] is in registers now
-                    if (warp == 12 && lane == 0) TS_MARK(n * 32 + 17 + 4 * h);
                     float2* out = Einst + comp * p.s_comp + zi * p.s_z + x * p.s_x + y0 * p.s_y;
                     if (x_ok) {
 #pragma unroll
@@ -566,13 +541,11 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                         }
                     }
                 }
-                if (warp == 12 && lane == 0) TS_MARK(n * 32 + 18 + 4 * h);
             }
         }
     }
     tc_fence_before();
     __syncthreads();
-    TS_BLK(2);
     if (warp == 1) tmem_dealloc(tmem_base, TS_TMEM_COLS);
 }
 
@@ -632,9 +605,6 @@ void launch_tc_synth_twiddles(scw_ctx* ctx, int U, int Vn, double X, double Y, i
     k_tc_synth_twiddles<<<by + bx, 256, 0, ctx->stream>>>(ay, ax, by);
 }
 
-#ifdef SCW_TS_DEBUG
-extern "C" void scw_debug_ts_read(long long* out) { cudaMemcpyFromSymbol(out, g_ts_dbg, sizeof(long long) * 4096); }
-#endif
 
 int tc_synth_max_group() { return TS_MAX_INST; }
 

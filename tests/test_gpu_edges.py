@@ -262,3 +262,49 @@ def test_more_tiles_than_sms_and_more_instances_than_a_group(scw):
             assert np.abs(I[i].cpu().numpy() - Iref).max() / Iref.max() <= 4e-4
     finally:
         c.close()
+
+
+def test_many_tiles_few_planes_twice_into_one_workspace(scw, ctx):
+    """3 x 3 frequencies, one z plane, 3072 x 3072 grid = 576 output tiles: more plane counters than threads of the
+    spectrum-image kernel (they must all be reset), run twice into the same workspace; NaN sentinels must all be
+    overwritten and a seeded subset must match Tier A."""
+    lay = ragged_layer(3, 3, 36, np.complex64, seed=77)
+    N = 3072
+    x = np.arange(N) * (3.0 / N)
+    y = np.arange(N) * (4.5 / N)
+    z = np.array([0.2])
+    L = scw.Layer.from_numpy(lay, "cuda")
+    P = scw.scw_assemble_spectra(ctx, L, dev(z))
+    dx, dy = dev(x), dev(y)
+    g = np.random.default_rng(9)
+    iy, ix = g.integers(0, N, 400), g.integers(0, N, 400)
+    xyz = np.column_stack([x[ix], y[iy], np.full(400, z[0])])
+    ref = oracle.layer_samples(xyz=xyz, **lay)
+    for _ in range(2):
+        E = torch.full((1, 3, N, N), float("nan"), dtype=torch.complex64, device="cuda")
+        scw.scw_synthesize_grid(ctx, U=3, Vn=3, X=lay["X"], Y=lay["Y"], P=P, x=dx, y=dy, out=E)
+        torch.cuda.synchronize()
+        assert not bool(torch.isnan(E.real).any())
+        got = E[0][:, torch.from_numpy(iy).cuda(), torch.from_numpy(ix).cuda()].T.cpu().numpy()
+        assert np.abs(got - ref).max() / np.abs(ref).max() <= 2e-4
+        del E
+
+
+def test_grouped_sweep_with_an_8_byte_aligned_V(scw, ctx):
+    """Instance 1 of a sweep holds V at an address that is only 8-byte aligned (a view one element into a buffer): the
+    TMA assembly cannot take it, so the whole sweep must drop to the per-instance path (CUDA-core assembly for that
+    instance) instead of failing in cuTensorMapEncodeTiled."""
+    lays = [ragged_layer(5, 5, 100, np.complex64, seed=90 + i) for i in range(3)]
+    x = np.arange(20) * 3.0 / 20
+    y = np.arange(18) * 4.5 / 18
+    z = np.linspace(-0.3, 0.8, 4)
+    Ls = [scw.Layer.from_numpy(l, "cuda") for l in lays]
+    J, ld = Ls[1].V.shape
+    buf = torch.zeros(J * ld + 1, dtype=torch.complex64, device="cuda")
+    buf[1:] = Ls[1].V.reshape(-1)
+    Ls[1].V = buf[1:].view(J, ld)
+    assert Ls[1].V.data_ptr() % 16 == 8
+    Es = scw.scw_sweep_wavelengths(ctx, Ls, [dev(z)] * 3, dev(x), dev(y))
+    torch.cuda.synchronize()
+    for lay, E in zip(lays, Es):
+        assert rel_err(E.cpu().numpy(), oracle.layer_grid(x=x, y=y, z=z, **lay)) <= 2e-4

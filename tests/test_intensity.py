@@ -105,3 +105,42 @@ def test_config4_intensity_full_size_fused(scw):
         assert float((out[1].permute(2, 0, 1) - I[1]).abs().max()) <= 5e-5 * float(I[1].max())   # other stream-K split
     finally:
         ctx.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("U,Vn", [(33, 33), (45, 50)])
+def test_intensity_wide_frequency_grids(scw, U, Vn):
+    """Fused detector with more than 32 frequencies along u (no 128 spare TMEM columns for the running sum: the other
+    accumulation mode of the epilogue), ragged Nx / Ny, custom strides, two instances: against oracle.intensity of
+    Tier B and against sum |E|^2 of the complex sweep."""
+    import torch
+    g = np.random.default_rng(U)
+    M, J, R = U * Vn, 96, 3 * U * Vn
+    lays = []
+    for i in range(2):
+        V = ((g.standard_normal((J, R)) + 1j * g.standard_normal((J, R))) / np.sqrt(2 * M)).astype(np.complex64)
+        dirs = np.where(np.arange(J) % 2 == 0, 1, -1).astype(np.int8)
+        gamma = dirs * (g.uniform(0.2, 1.4, J) + 1j * g.uniform(0.0, 0.2, J))
+        c = ((g.standard_normal(J) + 1j * g.standard_normal(J)) / np.sqrt(2)).astype(np.complex64)
+        lays.append(dict(U=U, Vn=Vn, X=30.0, Y=28.0, lam=0.9, z_lo=0.0, z_hi=1.3, V=V, c=c, gamma=gamma, dir=dirs))
+    Nx, Ny, Fz = 150, 131, 3
+    x = np.sort(g.uniform(0, 30, Nx))
+    y = np.sort(g.uniform(0, 28, Ny))
+    zs = [np.linspace(0.1, 1.2, Fz), np.linspace(0.0, 1.3, Fz)]
+    ctx = scw.Context(0)
+    try:
+        ctx.set_path(scw.SCW_PATH_TENSOR)
+        Ls = [scw.Layer.from_numpy(d, "cuda") for d in lays]
+        dz, dx, dy = [dev(z) for z in zs], dev(x), dev(y)
+        out = [torch.full((Ny, Nx, Fz), float("nan"), dtype=torch.float32, device="cuda") for _ in Ls]   # [y][x][z]
+        scw.scw_sweep_intensity(ctx, Ls, dz, dx, dy, out=out, strides=(1, Nx * Fz, Fz))
+        E = scw.scw_sweep_wavelengths(ctx, Ls, dz, dx, dy)
+        torch.cuda.synchronize()
+        for i in range(2):
+            I = out[i].permute(2, 0, 1)
+            ref = oracle.intensity(oracle.tier_b_grid(x=x, y=y, z=zs[i], **lays[i]))
+            assert np.abs(I.cpu().numpy() - ref).max() / ref.max() <= 4e-4
+            Ie = (E[i].real ** 2 + E[i].imag ** 2).sum(dim=1)
+            assert float((I - Ie).abs().max() / Ie.max()) <= 5e-6
+    finally:
+        ctx.close()

@@ -124,6 +124,51 @@ def test_reference_plane_invariant():
     assert np.array_equal(oracle.tier_b_weights(z=z, **auto), W)
 
 
+def test_reference_face_derived_from_gamma_in_tier_a(golden_dir):
+    """dir = NULL in Tier A (the C branch scwo_dir): the face of every mode against the hand-derived table
+    tests/golden/dir_cases.txt (readings c-1, c-3), through the single-mode closed form
+    E = c V exp(i 2 pi (u x/X + v y/Y)) exp(i k gamma (z - zref)); then dir = None must equal the explicit dir on the
+    whole toy, and |E| / |c V| <= 1 inside the layer with the derived faces (= 1 on the mode's own face)."""
+    rows = _read_table(os.path.join(golden_dir, "dir_cases.txt"))
+    J = len(rows)
+    U = Vn = 3
+    M = 9
+    g = np.random.default_rng(21)
+    z_lo, z_hi, lam, X, Y = 0.3, 1.7, 0.9, 4.0, 5.0
+    gamma = np.array([complex(r[0], r[1]) for r in rows])
+    face = np.array([int(r[2]) for r in rows])
+    V = (g.standard_normal((J, 3 * M)) + 1j * g.standard_normal((J, 3 * M)))
+    c = g.standard_normal(J) + 1j * g.standard_normal(J)
+    base = dict(U=U, Vn=Vn, X=X, Y=Y, lam=lam, z_lo=z_lo, z_hi=z_hi, gamma=gamma)
+    k = 2 * math.pi / lam
+    xyz = np.column_stack([g.uniform(0, 4, 9), g.uniform(0, 5, 9), np.linspace(z_lo, z_hi, 9)])
+    for j in range(J):                      # one mode, one frequency at a time: closed form with the table's face
+        m, comp = j % M, j % 3
+        V1 = np.zeros_like(V)
+        V1[j, comp * M + m] = V[j, comp * M + m]
+        E = oracle.layer_samples(xyz=xyz, V=V1, c=c, dir=None, **base)
+        u, v = m % 3 - 1, m // 3 - 1
+        zref = z_lo if face[j] == 0 else z_hi
+        for s, (x, y, z) in enumerate(xyz):
+            ref = (c[j] * V1[j, comp * M + m] * cmath.exp(2j * math.pi * (u * x / X + v * y / Y))
+                   * cmath.exp(1j * k * gamma[j] * (z - zref)))
+            assert abs(E[s, comp] - ref) < 1e-13 * abs(ref), (j, gamma[j])
+        ratio = np.abs(E[:, comp]) / abs(c[j] * V1[j, comp * M + m])
+        assert ratio.max() <= 1.0 + 1e-13                       # decays inside the layer (eq. 30)
+        own = 0 if face[j] == 0 else -1                          # xyz[0] is on z_lo, xyz[-1] on z_hi
+        assert abs(ratio[own] - 1.0) < 1e-13
+    dirs = np.where(face == 0, 1, -1).astype(np.int8)
+    E_auto = oracle.layer_samples(xyz=xyz, V=V, c=c, dir=None, **base)
+    E_expl = oracle.layer_samples(xyz=xyz, V=V, c=c, dir=dirs, **base)
+    assert np.array_equal(E_auto, E_expl)
+    E_flip = oracle.layer_samples(xyz=xyz, V=V, c=c, dir=(-dirs).astype(np.int8), **base)
+    assert np.abs(E_flip - E_expl).max() > 1e-3 * np.abs(E_expl).max()       # the faces matter
+    # Tier B's python mirror takes the same decisions
+    W_auto = oracle.tier_b_weights(z=xyz[:, 2], c=c, dir=None, **base)
+    W_expl = oracle.tier_b_weights(z=xyz[:, 2], c=c, dir=dirs, **base)
+    assert np.array_equal(W_auto, W_expl)
+
+
 # --------------------------------------------------------------------------- Tier A closed forms
 @pytest.mark.parametrize("j,m,comp", [(0, 0, 0), (5, 7, 1), (22, 4, 2), (35, 8, 2)])
 def test_single_mode_single_frequency_closed_form(j, m, comp):
