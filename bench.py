@@ -31,18 +31,23 @@ import scw_inputs as si  # noqa: E402
 
 METRIC = "field samples/s (complex E 3-vectors)"
 UNIT = "samples/s"
-FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # CUDA-core FFMA peak at max clock (context only)
-FP64_DMMA_PEAK_TFLOPS = 37.1                           # measured on this pool's B200 (DMMA microbenchmark)
 
 
 # ------------------------------------------------------------------------------------------------
-def measured_peaks():
+def measured_peaks(ctx=None):
+    """Roofline denominators: MEASURED_PEAKS.json (driver-written: HBM copy, dense bf16) plus the library's own
+    microbenchmarks run on this device right now (scw_measure_peak: FP64 DMMA, FP32 FMA, MUFU, HBM read / write streams)."""
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
         d = json.load(open(path))
-        return dict(hbm_gbs=d["hbm_gbs"], bf16_tflops=d["bf16_tflops"],
-                    bf16_tflops_sustained=d.get("bf16_tflops_sustained", d["bf16_tflops"]), source="measured")
-    return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback")
+        out = dict(hbm_gbs=d["hbm_gbs"], bf16_tflops=d["bf16_tflops"],
+                   bf16_tflops_sustained=d.get("bf16_tflops_sustained", d["bf16_tflops"]), source="measured")
+    else:
+        out = dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback")
+    if ctx is not None:
+        out.update(ctx.measure_peaks(reps=5))
+        out["microbenchmarks"] = "scw_measure_peak (csrc/scw_peaks.cu), best of 5 launches each, run before the timed step"
+    return out
 
 
 class ClockSampler:
@@ -138,41 +143,98 @@ def time_steps(torch, fn, steps, warmup, dist=None):
     return max_over_ranks(e0.elapsed_time(e1) / steps, dist)
 
 
-def kernel_rooflines(prof, steps, cfg, dtype_bytes, peaks):
-    """Per-kernel algorithmic bytes / flops per launch for config 1 (one launch = one layer), DESIGN.md table."""
+def time_each(torch, fn, n=20):
+    """n individually timed calls (an event pair each, back to back): best and median, SURVEY 8(d) "Timing"."""
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+    for a, b in ev:
+        a.record()
+        fn()
+        b.record()
+    torch.cuda.synchronize()
+    t = sorted(a.elapsed_time(b) for a, b in ev)
+    return dict(best_ms=t[0], median_ms=t[len(t) // 2], n=n)
+
+
+def sweep_shape(cfg, n_inst):
+    """Sizes of one grouped sweep: n_inst (wavelength, layer) instances of cfg's shape."""
     M = cfg.U * cfg.Vn
-    R, J, Fz, Nx, Ny = 3 * M, 4 * M, cfg.planes, cfg.Nx, cfg.Ny
-    es = dtype_bytes
+    pad16 = lambda v: (v + 15) // 16 * 16
+    chunks = lambda nf: (2 * nf + 79) // 80                          # frequency chunks of the synthesis (K <= 80)
+    nuc, nvc = chunks(cfg.U), chunks(cfg.Vn)
+    K2p, K1p = pad16(2 * -(-cfg.U // nuc)), pad16(2 * -(-cfg.Vn // nvc))
+    tiles = -(-cfg.Nx // 128) * -(-cfg.Ny // 128)
+    return dict(M=M, R=3 * M, J=4 * M, Fz=cfg.planes, Nx=cfg.Nx, Ny=cfg.Ny, U=cfg.U, Vn=cfg.Vn, n_inst=n_inst,
+                # executed tensor flops of the synthesis per plane and 128 x 128 tile: GEMM1 (M = 128, N = K2p, K = K1p per
+                # v chunk) for every u chunk, GEMM2 (two 64-y halves, N = 128, K = K2p) per u chunk; three bf16 products each
+                synth_exec_per_plane_tile=3 * 2 * 128 * (nuc * nvc * K2p * K1p + nuc * 128 * K2p), tiles=tiles)
+
+
+def kernel_rooflines(prof, steps, sh, peaks, traffic=None):
+    """Per-kernel algorithmic bytes / flops per launch of a grouped complex64 sweep (bytes per unit), against
+    BOTH rooflines: HBM (measured copy peak) and bf16 tensor (sustained measured peak; useful and executed flops)."""
+    es = 8
+    R, J, Fz, Nx, Ny, M, U, n = sh["R"], sh["J"], sh["Fz"], sh["Nx"], sh["Ny"], sh["M"], sh["U"], sh["n_inst"]
     alg = {
-        "simt_assemble": dict(bytes=R * J * es + J * Fz * es + R * Fz * es, flops=8 * R * J * Fz),
-        "tc_assemble": dict(bytes=R * J * es + J * Fz * es + R * Fz * es, flops=8 * R * J * Fz),
-        "simt_synth_a": dict(bytes=R * Fz * es + 3 * Fz * cfg.U * Ny * es, flops=8 * 3 * Fz * M * Ny),
-        "simt_synth_b": dict(bytes=3 * Fz * Nx * Ny * es + 3 * Fz * cfg.U * Ny * es, flops=8 * 3 * Fz * Nx * cfg.U * Ny),
-        "tc_synth": dict(bytes=3 * Fz * Nx * Ny * es + R * Fz * es, flops=8 * 3 * Fz * (M * Ny + Nx * cfg.U * Ny)),
+        # fused a-1 + a-2 (+ fix-up into the synthesis images): read V once, read c / gamma / z, spectra stay on chip / in L2
+        "tc_assemble": dict(bytes=n * (R * J * es + J * (es + 17) + Fz * 8), flops=n * 8 * R * J * Fz,
+                            executed=n * 3 * 8 * R * J * Fz),
+        "simt_assemble": dict(bytes=n * (R * J * es + J * Fz * es + R * Fz * es), flops=n * 8 * R * J * Fz, executed=None),
+        # a-4: write E once (the spectrum images are L2-resident)
+        "tc_synth": dict(bytes=n * 3 * Fz * Nx * Ny * es, flops=n * 8 * 3 * Fz * (M * Ny + Nx * U * Ny),
+                         executed=n * 3 * Fz * sh["tiles"] * sh["synth_exec_per_plane_tile"]),
     }
-    traffic = {}
-    tpath = os.path.join(ROOT, "profiles", "dram_traffic.json")
-    if os.path.exists(tpath):
-        traffic = json.load(open(tpath))
+    traffic = traffic or {}
     out = {}
     total = sum(ms for ms, _ in prof.values()) or 1.0
-    for name, (ms, n) in prof.items():
-        per = ms / n
-        k = dict(ms_per_launch=per, launches_per_step=n / steps, share=ms / total)
+    for name, (ms, cnt) in prof.items():
+        per = ms / cnt
+        launches = cnt / steps
+        k = dict(ms_per_launch=per, launches_per_step=launches, share=ms / total)
         if name in alg:
-            # a grouped launch covers several layers: units per launch = layers per step / launches per step
-            units = cfg.n_layers / (n / steps)
-            nbytes, flops = alg[name]["bytes"] * units, alg[name]["flops"] * units
+            a = alg[name]
+            nbytes, flops = a["bytes"] / launches, a["flops"] / launches
             gbs = nbytes / (per * 1e-3) / 1e9
-            k.update(bound="hbm", achieved=gbs, peak=peaks["hbm_gbs"], unit="GB/s", frac=gbs / peaks["hbm_gbs"],
-                     traffic=traffic.get(name), layers_per_launch=units, alg_bytes=nbytes,
-                     useful_tflops=flops / (per * 1e-3) / 1e12)
-            if name.startswith("tc_"):
-                # BF16x3: three bf16 products per real product; sustained measured bf16 peak (kernel inside a step)
-                ex = 3 * flops / (per * 1e-3) / 1e12
-                k.update(executed_bf16_tflops=ex, tensor_frac=ex / peaks["bf16_tflops_sustained"])
+            k.update(alg_bytes=nbytes, hbm_gbs=gbs, hbm_frac=gbs / peaks["hbm_gbs"],
+                     useful_tflops=flops / (per * 1e-3) / 1e12, traffic=traffic.get(name))
+            if a["executed"]:
+                ex = a["executed"] / launches / (per * 1e-3) / 1e12
+                k.update(executed_bf16_tflops=ex, tensor_frac_executed=ex / peaks["bf16_tflops_sustained"],
+                         tensor_frac_useful=k["useful_tflops"] / peaks["bf16_tflops_sustained"])
+                k["binding"] = "hbm" if k["hbm_frac"] >= k["tensor_frac_executed"] else "tensor"
+            else:
+                k["binding"] = "hbm"
         out[name] = k
     return out
+
+
+def dominant_roofline(kernels, peaks):
+    """The `roofline` object of the JSON line for the kernel with the largest share of the step."""
+    dom = max((k for k in kernels if "hbm_frac" in kernels[k]), key=lambda k: kernels[k]["share"])
+    k = kernels[dom]
+    if k["binding"] == "tensor":
+        roof = dict(bound="tensor", achieved=k["executed_bf16_tflops"], peak=peaks["bf16_tflops_sustained"], unit="TFLOP/s",
+                    frac=k["tensor_frac_executed"])
+    else:
+        roof = dict(bound="hbm", achieved=k["hbm_gbs"], peak=peaks["hbm_gbs"], unit="GB/s", frac=k["hbm_frac"])
+    roof.update(traffic=k.get("traffic"), kernel=dom, share_of_step=k["share"], alg_bytes_per_launch=k["alg_bytes"],
+                ms_per_launch=k["ms_per_launch"], peak_source=peaks["source"])
+    return roof
+
+
+def profile_sweep(torch, ctx, step, steps):
+    """Per-kernel device milliseconds over `steps` further calls (the library's CUDA-event timers)."""
+    ctx.set_profile(True)
+    for _ in range(steps):
+        step()
+    torch.cuda.synchronize()
+    prof = ctx.profile()
+    ctx.set_profile(False)
+    return prof
+
+
+def load_traffic():
+    path = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    return json.load(open(path)) if os.path.exists(path) else {}
 
 
 def run_ours(args):
@@ -185,16 +247,21 @@ def run_ours(args):
     torch.cuda.set_device(local_rank)
     device = torch.device("cuda", local_rank)
     scw.lib()
-    peaks = measured_peaks()
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(device)
 
     cfg, layers, zs, x, y = config1_inputs(np.complex64)
     ctx = scw.Context(local_rank)
+    peaks = measured_peaks(None if args.quick else ctx)
     Ls = [scw.Layer.from_numpy(d, device) for d in layers]
     dz, dx, dy = [dev(z) for z in zs], dev(x), dev(y)
     out = [torch.empty((cfg.planes, 3, cfg.Ny, cfg.Nx), dtype=torch.complex64, device=device) for _ in Ls]
     samples = cfg.n_layers * cfg.planes * cfg.Nx * cfg.Ny
     step = lambda: scw.scw_sweep_wavelengths(ctx, Ls, dz, dx, dy, out=out)
+
+    # ---- set-up (untimed, once per context): twiddle cache on (x, y do not change between steps) and the stream-K split
+    # of the assembly calibrated on this very sweep (scw_calibrate: 3 rounds of 6 sweeps)
+    ctx.set_cache(True)
+    scw.scw_calibrate(ctx, Ls, dz, dx, dy, out=out, reps=5)
 
     # ---- value: inputs resident in HBM
     step()
@@ -207,6 +274,7 @@ def run_ours(args):
         time.sleep(0.05)
     ms = time_steps(torch, step, args.steps, args.warmup, dist)
     launches = (ctx.launch_count() - n0) // (args.steps + args.warmup)
+    each = time_each(torch, step, max(20, args.steps))
     # the timed region lasts a few ms: keep the identical step running ~0.7 s so the 100 ms sampler sees it
     t_hold = time.perf_counter()
     while time.perf_counter() - t_hold < 0.7:
@@ -217,36 +285,32 @@ def run_ours(args):
     value = world * samples / (ms * 1e-3)
 
     # ---- per-kernel device timers over a second pass of the same K steps
-    ctx.set_profile(True)
-    for _ in range(args.steps):
-        step()
-    torch.cuda.synchronize()
-    prof = ctx.profile()
-    ctx.set_profile(False)
-    kernels = kernel_rooflines(prof, args.steps, cfg, 8, peaks)
-    dominant = max((k for k in kernels if "frac" in kernels[k]), key=lambda k: kernels[k]["share"])
-    roof = {k: kernels[dominant][k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")}
-    roof.update(kernel=dominant, share_of_step=kernels[dominant]["share"], peak_source=peaks["source"],
-                alg_bytes_per_launch=kernels[dominant]["alg_bytes"])
+    prof = profile_sweep(torch, ctx, step, args.steps)
+    kernels = kernel_rooflines(prof, args.steps, sweep_shape(cfg, cfg.n_layers), peaks, load_traffic())
+    roof = dominant_roofline(kernels, peaks)
+    vbytes = sum(l.V.numel() * 8 for l in Ls)
+    whole = dict(alg_bytes=vbytes + samples * 24, hbm_frac=(vbytes + samples * 24) / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                 note="V read once + E written once per step, over the step time: the step's HBM floor fraction")
 
     # ---- e2e: the same step through the host-buffer C-ABI call (pinned host memory, H2D + D2H inside)
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    Lh = [scw.Layer(U=d["U"], Vn=d["Vn"], X=d["X"], Y=d["Y"], lam=d["lam"], z_lo=d["z_lo"], z_hi=d["z_hi"],
-                    V=pin(d["V"]), gamma=pin(d["gamma"]), c=pin(d["c"]), dir=pin(d["dir"])) for d in layers]
-    hz, hx, hy = [pin(z) for z in zs], pin(x), pin(y)
-    hout = [torch.empty((cfg.planes, 3, cfg.Ny, cfg.Nx), dtype=torch.complex64).pin_memory() for _ in Lh]
-    io = {}
-
-    def host_step():
-        _, io["up"], io["down"] = scw.scw_sweep_wavelengths_host(ctx, Lh, hz, hx, hy, out=hout)
-
     e2e = None
     if not args.quick:
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        Lh = [scw.Layer(U=d["U"], Vn=d["Vn"], X=d["X"], Y=d["Y"], lam=d["lam"], z_lo=d["z_lo"], z_hi=d["z_hi"],
+                        V=pin(d["V"]), gamma=pin(d["gamma"]), c=pin(d["c"]), dir=pin(d["dir"])) for d in layers]
+        hz, hx, hy = [pin(z) for z in zs], pin(x), pin(y)
+        hout = [torch.empty((cfg.planes, 3, cfg.Ny, cfg.Nx), dtype=torch.complex64).pin_memory() for _ in Lh]
+        io = {}
+
+        def host_step():
+            _, io["up"], io["down"] = scw.scw_sweep_wavelengths_host(ctx, Lh, hz, hx, hy, out=hout)
+
         ms_e2e = time_steps(torch, host_step, max(2, args.steps // 2), 1, dist)
         e2e = dict(value=world * samples / (ms_e2e * 1e-3), unit=UNIT, ms_per_step=ms_e2e,
                    h2d_bytes_per_step=io["up"], d2h_bytes_per_step=io["down"])
         dev_host = float((hout[0] - out[0].cpu()).abs().max() / hout[0].abs().max())
         assert dev_host <= 5e-5, f"host-buffer path disagrees with the device path: {dev_host:.3e}"
+        del Lh, hout
 
     extra = {}
     if rank == 0 and not args.quick:
@@ -258,22 +322,32 @@ def run_ours(args):
 
     if rank == 0:
         line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
-                    ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="c64 (fp32)",
-                    data="synthetic",
+                    ms_per_step=ms, step_ms_best=each["best_ms"], step_ms_median=each["median_ms"],
+                    value_at_median=world * samples / (each["median_ms"] * 1e-3), individually_timed_steps=each["n"],
+                    higher_is_better=True, scaling="weak", vs_baseline=None, dtype="c64 (fp32)", data="synthetic",
                     config=dict(workload="BASELINE.json configs[1]: 33x33 frequencies (M=1089, J=4356), 4 layers x 64 "
                                 "planes, 256x256 grid, complex64, one scw_sweep_wavelengths call per step",
                                 samples_per_step=samples, parallelism=f"replicas x{world}",
-                                cache="inputs (457 MB of V) + outputs (403 MB) per step exceed the 126 MB L2"),
+                                cache="inputs (457 MB of V) + outputs (403 MB) per step exceed the 126 MB L2",
+                                setup="untimed, once: SCW_OPT_CACHE=1 (twiddle tables kept between steps, step a-3 'cached in ctx') "
+                                      "and scw_calibrate (per-SM stream-K split of the assembly)",
+                                why_config1="configs[1] is the largest config that runs in BOTH dtypes and the only one "
+                                            "whose assembly is balanced between HBM and tensor work (Fz = 64); configs[2], [4] "
+                                            "(HBM-bound, Fz = 16), [3], [3'] and configs[1] complex128 are under `extra`, "
+                                            "each with its own roofline"),
                     clocks=clocks, e2e=e2e, gpu_launches=int(launches) * args.steps, gpu_launches_per_step=int(launches),
-                    roofline=roof, kernels=kernels, cpu_baseline=cpu, extra=extra, peaks=peaks)
+                    roofline=roof, whole_step=whole, kernels=kernels, cpu_baseline=cpu, extra=extra, peaks=peaks)
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
 
 
 def extra_workloads(torch, scw, ctx, device, args, peaks):
-    """Configs 3 (point path), 4 (sweep, detector), exterior field, 2, 1 complex128 and 3' at full size."""
+    """Configs 3 (point path), 4 (sweep, detector), exterior field, 2, 1 complex128 and 3' at full size, each with the
+    rooflines SURVEY 8(d) asks for (tensor useful / executed, HBM, which one binds)."""
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(device)
+    traffic = load_traffic()
+    mufu = peaks.get("mufu_gops", 148 * 16 * 1.965)           # Gop/s, measured by scw_measure_peak
     extra = {}
     # config 3: 4e6 scattered points x 4356 plane waves
     c3 = si.CONFIGS[3]
@@ -282,11 +356,12 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
     outp = torch.empty((pts.shape[0], 3), dtype=torch.complex64, device=device)
     ms = time_steps(torch, lambda: scw.scw_eval_points(ctx, pw, pts, out=outp), args.steps, args.warmup)
     terms = pts.shape[0] * 4356
-    sfu_peak = 148 * 16 * 1.965e9 / 3                      # terms/s if 3 MUFU ops per term saturate the XU pipe
-    extra["config3_points"] = dict(ms_per_call=ms, points_per_s=pts.shape[0] / (ms * 1e-3), terms_per_s=terms / (ms * 1e-3),
-                                   roofline=dict(bound="alu", achieved=terms / (ms * 1e-3) / 1e9, peak=sfu_peak / 1e9,
-                                                 unit="Gterm/s (3 MUFU/term at 16/clk/SM, 148 SMs, 1965 MHz)",
-                                                 frac=terms / (ms * 1e-3) / sfu_peak, traffic=None))
+    gterm = terms / (ms * 1e-3) / 1e9
+    extra["config3_points"] = dict(ms_per_call=ms, points_per_s=pts.shape[0] / (ms * 1e-3), terms_per_s=gterm * 1e9,
+                                   roofline=dict(bound="alu", achieved=gterm, peak=mufu / 3,
+                                                 unit="Gterm/s (3 MUFU per term: sin, cos, ex2; peak = measured MUFU rate / 3)",
+                                                 frac=gterm / (mufu / 3), traffic=None,
+                                                 fp32_fma_frac=gterm * 28 / 1e3 / peaks.get("fp32_fma_tflops", 70.7)))
     del pts, outp
     # config 4: 32 wavelengths x 2 layers, one call
     c4 = si.CONFIGS[4]
@@ -298,16 +373,26 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
             zs.append(dev(si.grid_coords(c4, l)[2]))
     out = [torch.empty((c4.planes, 3, c4.Ny, c4.Nx), dtype=torch.complex64, device=device) for _ in Ls]
     dx, dy = dev(x), dev(y)
-    ms = time_steps(torch, lambda: scw.scw_sweep_wavelengths(ctx, Ls, zs, dx, dy, out=out), args.steps, args.warmup)
+    sweep4 = lambda: scw.scw_sweep_wavelengths(ctx, Ls, zs, dx, dy, out=out)
+    scw.scw_calibrate(ctx, Ls, zs, dx, dy, out=out, reps=3)
+    ms = time_steps(torch, sweep4, args.steps, args.warmup)
     n4 = len(Ls) * c4.planes * c4.Nx * c4.Ny
-    ebytes = n4 * 24
-    extra["config4_sweep"] = dict(ms_per_call=ms, samples_per_s=n4 / (ms * 1e-3),
-                                  hbm_write_frac=ebytes / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
+    vbytes = sum(l.V.numel() * 8 for l in Ls)
+    k4 = kernel_rooflines(profile_sweep(torch, ctx, sweep4, args.steps), args.steps, sweep_shape(c4, len(Ls)), peaks)
+    extra["config4_sweep"] = dict(ms_per_call=ms, samples_per_s=n4 / (ms * 1e-3), kernels=k4,
+                                  hbm_frac_V_plus_E=(vbytes + n4 * 24) / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
     # NEXT-3 detector: the same sweep with I = sum_comp |E_comp|^2 reduced in the synthesis epilogue (E never written)
     outI = [torch.empty((c4.planes, c4.Ny, c4.Nx), dtype=torch.float32, device=device) for _ in Ls]
-    ms = time_steps(torch, lambda: scw.scw_sweep_intensity(ctx, Ls, zs, dx, dy, out=outI), args.steps, args.warmup)
-    extra["config4_sweep_intensity"] = dict(ms_per_call=ms, samples_per_s=n4 / (ms * 1e-3),
-                                            speedup_vs_complex_field=extra["config4_sweep"]["ms_per_call"] / ms)
+    det4 = lambda: scw.scw_sweep_intensity(ctx, Ls, zs, dx, dy, out=outI)
+    ms_i = time_steps(torch, det4, args.steps, args.warmup)
+    kI = kernel_rooflines(profile_sweep(torch, ctx, det4, args.steps), args.steps, sweep_shape(c4, len(Ls)), peaks)
+    if "tc_synth" in kI:                                     # detector: 4 bytes per sample leave the SM instead of 24
+        kI["tc_synth"]["alg_bytes"] = n4 * 4
+        kI["tc_synth"]["hbm_gbs"] = n4 * 4 / (kI["tc_synth"]["ms_per_launch"] * 1e-3) / 1e9
+        kI["tc_synth"]["hbm_frac"] = kI["tc_synth"]["hbm_gbs"] / peaks["hbm_gbs"]
+        kI["tc_synth"]["binding"] = "tensor"
+    extra["config4_sweep_intensity"] = dict(ms_per_call=ms_i, samples_per_s=n4 / (ms_i * 1e-3), kernels=kI,
+                                            speedup_vs_complex_field=ms / ms_i)
     del Ls, zs, out, outI
     torch.cuda.empty_cache()
     # NEXT-1 exterior field (eq. 9-10): the paper's Table 2 shape (M = 2500 orders, one 256 x 256 plane below the
@@ -340,11 +425,13 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
         ms = time_steps(torch, lambda: scw.scw_sweep_wavelengths(ctx, Ls, dz, dx, dy, out=out), max(2, args.steps // 2), 2)
         M1 = c1.U * c1.Vn
         gf = c1.n_layers * (8 * 3 * M1 * 4 * M1 * c1.planes + 8 * 3 * c1.planes * (M1 * c1.Ny + c1.Nx * c1.U * c1.Ny)) / 1e9
+        dmma = peaks.get("fp64_dmma_tflops")
         extra["config1_c128"] = dict(ms_per_call=ms, samples_per_s=c1.n_layers * c1.planes * c1.Nx * c1.Ny / (ms * 1e-3),
-                                     roofline=dict(bound="tensor", achieved=gf / ms, peak=FP64_DMMA_PEAK_TFLOPS,
+                                     roofline=dict(bound="tensor", achieved=gf / ms, peak=dmma,
                                                    unit="TFLOP/s (useful fp64, 8 per complex MAC; the 3M kernel executes 6; peak = "
-                                                        "measured mma.sync m8n8k4 f64 rate, DESIGN.md 5)",
-                                                   frac=gf / ms / FP64_DMMA_PEAK_TFLOPS, traffic=None))
+                                                        "mma.sync m8n8k4 f64 rate measured by scw_measure_peak in this run)",
+                                                   frac=gf / ms / dmma if dmma else None,
+                                                   frac_executed=0.75 * gf / ms / dmma if dmma else None, traffic=None))
         del Ls, out, layers
         torch.cuda.empty_cache()
         c2 = si.CONFIGS[2]
@@ -353,42 +440,96 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
         dz = [dev(si.grid_coords(c2, l)[2]) for l in range(c2.n_layers)]
         out = [torch.empty((c2.planes, 3, c2.Ny, c2.Nx), dtype=torch.complex64, device=device) for _ in Ls]
         dx, dy = dev(x2), dev(y2)
-        ms = time_steps(torch, lambda: scw.scw_sweep_wavelengths(ctx, Ls, dz, dx, dy, out=out), max(2, args.steps // 2), 2)
+        sweep2 = lambda: scw.scw_sweep_wavelengths(ctx, Ls, dz, dx, dy, out=out)
+        scw.scw_calibrate(ctx, Ls, dz, dx, dy, out=out, reps=2)
+        ms = time_steps(torch, sweep2, max(2, args.steps // 2), 2)
         n2 = c2.n_layers * c2.planes * c2.Nx * c2.Ny
         vbytes = sum(l.V.numel() * 8 for l in Ls)
-        extra["config2_large"] = dict(ms_per_call=ms, samples_per_s=n2 / (ms * 1e-3),
+        k2 = kernel_rooflines(profile_sweep(torch, ctx, sweep2, 4), 4, sweep_shape(c2, len(Ls)), peaks, traffic.get("config2"))
+        extra["config2_large"] = dict(ms_per_call=ms, samples_per_s=n2 / (ms * 1e-3), kernels=k2,
                                       hbm_frac_V_plus_E=(vbytes + n2 * 24) / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
         del Ls, out
         torch.cuda.empty_cache()
+        # config 3': dense eq. 34 at 65 536 scattered points: per point 3*M*J complex MACs on the tensor cores (a-1/a-2 with
+        # one column per point, BF16x3) + an M-term sum per point
         lay = scw.Layer.from_numpy(si.make_layer(c3, dtype=np.complex64), device)
         pts = dev(si.make_points(c3, n=65536))
         ms = time_steps(torch, lambda: scw.scw_eval_points(ctx, lay, pts), 2, 1)
-        extra["config3_dense_points"] = dict(ms_per_call=ms, points_per_s=65536 / (ms * 1e-3))
+        M3 = c3.U * c3.Vn
+        useful = 65536 * 8 * 3 * M3 * 4 * M3 / (ms * 1e-3) / 1e12
+        extra["config3_dense_points"] = dict(
+            ms_per_call=ms, points_per_s=65536 / (ms * 1e-3),
+            roofline=dict(bound="tensor", achieved=3 * useful, peak=peaks["bf16_tflops_sustained"],
+                          unit="TFLOP/s executed (BF16x3; useful = achieved / 3)", frac=3 * useful / peaks["bf16_tflops_sustained"],
+                          useful_tflops=useful, hbm_frac=(65536 / 4096) * lay.V.numel() * 8 / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                          traffic=None, note="V is re-read once per chunk of 4096 points (16 chunks): hbm_frac counts those reads"))
     return extra
 
 
-def cpu_baseline(layer, x, y, z, cfg, budget_s=15.0):
-    """The oracle as it stands (Tier A triple loop) on a bounded seeded sample of config 1, host cores."""
+def blas_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [p.get("num_threads", 1) for p in threadpool_info() if p.get("user_api") == "blas"]
+        return max(n) if n else (os.cpu_count() or 1)
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def time_tier_b(layer, x, y, z, repeats=1):
+    """Tier B of the oracle (the paper's own factored algorithm O(M^2 Fz + M F), numpy complex128 / BLAS) on
+    the full grid of one config-1 layer; returns (samples, seconds)."""
+    import oracle
+    best = None
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        oracle.tier_b_grid(x=x, y=y, z=z, **layer)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    return len(z) * len(y) * len(x), best
+
+
+def time_tier_a(layer, xyz, threads, budget_s):
+    """Tier A (the plain definition, triple loop) on as many of the seeded samples as fit the budget."""
+    import oracle
+    oracle.set_threads(threads)
+    t0 = time.perf_counter()
+    oracle.layer_samples(xyz=xyz[:threads], **layer)
+    probe = time.perf_counter() - t0
+    n = int(max(threads, min(len(xyz), budget_s / max(probe, 1e-6) * threads)))
+    n -= n % threads
+    t0 = time.perf_counter()
+    oracle.layer_samples(xyz=xyz[:n], **layer)
+    return n, time.perf_counter() - t0
+
+
+def cpu_baseline(layer, x, y, z, cfg):
+    """The oracle as it stands on the box's host cores, on config 1 layer 0 (~25 s in all).  Headline: Tier B, the paper's
+    own factored algorithm, on the full 256 x 256 x 64 grid of the layer with all cores (the "fair" CPU baseline of SURVEY
+    8(d)); beside it Tier A, the plain triple loop, on a bounded seeded sample with all cores and with one thread."""
     import oracle
     n_total = cfg.planes * cfg.Ny * cfg.Nx
     idx = si.sample_subset(cfg, n_total, 4096)
     iz, iy, ix = np.unravel_index(idx, (cfg.planes, cfg.Ny, cfg.Nx))
     xyz = np.column_stack([x[ix], y[iy], z[iz]])
     cores = oracle.threads()
-    t0 = time.perf_counter()
-    oracle.layer_samples(xyz=xyz[:cores], **layer)
-    probe = time.perf_counter() - t0
-    n = int(max(cores, min(len(xyz), budget_s / max(probe, 1e-6) * cores)))
-    n -= n % cores
-    t0 = time.perf_counter()
-    oracle.layer_samples(xyz=xyz[:n], **layer)
-    dt = time.perf_counter() - t0
-    return dict(value=n / dt, unit=UNIT, cores=cores, kind="oracle",
-                sample=f"{n} seeded samples of config 1 layer 0 (Tier A: 3*M*J = 14.2e6 complex terms per sample), {dt:.1f} s")
+    nb, tb = time_tier_b(layer, x, y, z, repeats=2)
+    na, ta = time_tier_a(layer, xyz, cores, 10.0)
+    n1, t1 = time_tier_a(layer, xyz, 1, 5.0)
+    oracle.set_threads(cores)
+    return dict(value=nb / tb, unit=UNIT, cores=blas_threads(), kind="oracle",
+                tier="B (factored, O(M^2 Fz + M F), PAPER.md:418; numpy complex128 + BLAS)",
+                sample=f"all {nb} samples of config 1 layer 0 (256 x 256 x 64), best of 2, {tb:.2f} s",
+                definition=dict(value=na / ta, unit=UNIT, cores=cores, kind="oracle",
+                                tier="A (the plain definition: 3*M*J = 14.2e6 complex terms per sample, OpenMP over samples)",
+                                sample=f"{na} seeded samples of config 1 layer 0, {ta:.1f} s"),
+                definition_1thread=dict(value=n1 / t1, unit=UNIT, cores=1, kind="oracle", tier="A, one thread",
+                                        sample=f"{n1} seeded samples of config 1 layer 0, {t1:.1f} s"))
 
 
 def run_reference(args):
-    """--impl reference: the oracle timed on the host cores; each step is a bounded sample of config 1."""
+    """--impl reference: the oracle timed on the host cores.  Each step evaluates ONE full layer of config 1 (4 194 304
+    samples) with Tier B, the factored CPU algorithm the GPU path also runs; Tier A (the plain definition,
+    O(M J) per sample) is reported beside it on a bounded sample."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
@@ -396,25 +537,28 @@ def run_reference(args):
     cfg = si.CONFIGS[1]
     layer = si.make_layer(cfg, 0, dtype=np.complex64)
     x, y, z = si.grid_coords(cfg, 0)
-    cores = oracle.threads()
-    per_step = 2 * cores
-    idx = si.sample_subset(cfg, cfg.planes * cfg.Ny * cfg.Nx, per_step * (args.steps + args.warmup))
-    iz, iy, ix = np.unravel_index(idx, (cfg.planes, cfg.Ny, cfg.Nx))
-    xyz = np.column_stack([x[ix], y[iy], z[iz]])
-    for w in range(args.warmup):
-        oracle.layer_samples(xyz=xyz[w * per_step:(w + 1) * per_step], **layer)
+    per_step = cfg.planes * cfg.Ny * cfg.Nx
+    for _ in range(args.warmup):
+        oracle.tier_b_grid(x=x, y=y, z=z, **layer)
     t0 = time.perf_counter()
-    for s in range(args.warmup, args.warmup + args.steps):
-        oracle.layer_samples(xyz=xyz[s * per_step:(s + 1) * per_step], **layer)
+    for _ in range(args.steps):
+        oracle.tier_b_grid(x=x, y=y, z=z, **layer)
     dt = (time.perf_counter() - t0) / args.steps
     value = per_step / dt
-    sample = f"{per_step} seeded samples of config 1 layer 0 per step (Tier A triple loop)"
+    cores = oracle.threads()
+    idx = si.sample_subset(cfg, per_step, 4096)
+    iz, iy, ix = np.unravel_index(idx, (cfg.planes, cfg.Ny, cfg.Nx))
+    na, ta = time_tier_a(layer, np.column_stack([x[ix], y[iy], z[iz]]), cores, 6.0)
+    sample = f"one full layer of config 1 per step ({per_step} samples), Tier B (factored, numpy complex128 + BLAS)"
     print(json.dumps(dict(impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
                           warmup=args.warmup, ms_per_step=dt * 1e3, higher_is_better=True, scaling="weak",
                           vs_baseline=None, dtype="f64", data="synthetic",
                           config=dict(workload="BASELINE.json configs[1] (33x33 frequencies, 4 layers x 64 planes, "
-                                      "256x256 grid); bounded sample per step", samples_per_step=per_step),
-                          cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample),
+                                      "256x256 grid); one of its four layers per step", samples_per_step=per_step),
+                          cpu_baseline=dict(value=value, unit=UNIT, cores=blas_threads(), kind="oracle",
+                                            tier="B (factored)", sample=sample,
+                                            definition=dict(value=na / ta, unit=UNIT, cores=cores, kind="oracle", tier="A",
+                                                            sample=f"{na} seeded samples of config 1 layer 0, {ta:.1f} s")),
                           e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
                           gpu_launches=0)))
 
@@ -425,7 +569,6 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--all", action="store_true", help="(default now) also time config 2, config 1 complex128, config 3'")
     ap.add_argument("--skip-large", action="store_true", help="skip config 2, config 1 complex128 and config 3' (extra)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--quick", action="store_true", help="only the resident-input step (for ncu captures)")

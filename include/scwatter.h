@@ -59,7 +59,15 @@ enum {
 enum { SCW_C64 = 0, SCW_C128 = 1 };
 
 /* Which kernels implement the two contractions (scw_set_option(ctx, SCW_OPT_PATH, v)). */
-enum { SCW_OPT_PATH = 1, SCW_OPT_PROFILE = 2 /* 0/1: record CUDA events around every kernel launch */ };
+enum {
+    SCW_OPT_PATH = 1,
+    SCW_OPT_PROFILE = 2,  /* 0/1: record CUDA events around every kernel launch */
+    SCW_OPT_CACHE = 3     /* 0/1: keep the twiddle tables F_x, F_y (step a-3; wavelength-free, eq. 6) in the workspace between
+                             consecutive scw_sweep_wavelengths / scw_sweep_intensity calls.  While it is 1 the caller promises
+                             that (i) the workspace is not written between those calls and (ii) the CONTENTS of x and y do not
+                             change while their pointers, Nx, Ny, U, Vn, X, Y stay the same; call scw_invalidate_cache() after
+                             changing coordinates in place.  Any other call on the ctx drops the cache.  Default 0. */
+};
 enum {
     SCW_PATH_AUTO = 0,    /* tcgen05 tensor-core kernels where shape/dtype allow, CUDA-core otherwise */
     SCW_PATH_SIMT = 1,    /* CUDA-core kernels only (fp32 FMA for C64, fp64 DFMA for C128) */
@@ -76,6 +84,7 @@ int32_t scw_set_stream(scw_ctx* ctx, void* cuda_stream);
 /* Register caller-owned device scratch (256-byte aligned).  May be (NULL, 0). */
 int32_t scw_set_workspace(scw_ctx* ctx, void* dev_ptr, size_t bytes);
 int32_t scw_set_option(scw_ctx* ctx, int32_t option, int64_t value);
+int32_t scw_invalidate_cache(scw_ctx* ctx);
 /* Message / raw cudaError_t / required workspace bytes of the last failing call on this ctx. */
 const char* scw_last_error(const scw_ctx* ctx);
 int32_t scw_last_cuda_error(const scw_ctx* ctx);
@@ -93,6 +102,11 @@ int32_t scw_profile_classes(void);
 const char* scw_profile_name(int32_t kernel_class);
 int32_t scw_profile_read(scw_ctx* ctx, int32_t kernel_class, double* ms_total, int64_t* launches);
 int32_t scw_profile_reset(scw_ctx* ctx);
+/* Timeline of the last tensor-core assembly launch (always recorded, four globaltimer reads per CTA): for each of its
+ * persistent CTAs the microseconds from the CTA's start to (0) its share of the mode weights written, (1) the weights of
+ * all CTAs visible, (2) its span of V streamed, (3) exit after the fix-up.  us: HOST [max_ctas][4]; *n_ctas (HOST) = CTAs of
+ * that launch (0 if none yet).  SYNCHRONISES the stream.  Errors: NULL, SHAPE (max_ctas too small), CUDA. */
+int32_t scw_profile_assembly(scw_ctx* ctx, int32_t max_ctas, double* us, int32_t* n_ctas);
 
 /* ---------------------------------------------------------------- descriptors (HOST PODs) */
 
@@ -138,9 +152,10 @@ typedef struct {
  *   P[:, i] = V . ( c o g(z_i) ),  g_j(z) = G(gamma_j, zref_j, z) = exp(i k gamma_j (z - zref_j))  (eq. 7)
  * z: [Fz] doubles (device).  P: [ldP x Fz] column-major complex<dtype>, ldP >= 3*U*Vn.
  * z outside [z_lo, z_hi] is evaluated as-is.  Workspace: see scw_assemble_workspace().
- * Domain: every phase gamma_j (z - zref_j) / lambda is reduced to a fraction of a turn in fp64 (rint) before the
- * trigonometric functions, for both dtypes: any finite z gives the correctly reduced phase (the fp64 product itself
- * carries 2^-53 |phase| turns of rounding, which is what limits complex128 beyond ~1e5 turns).
+ * Domain: every phase gamma_j (z - zref_j) / lambda is reduced to a fraction of a turn in fp64 before the trigonometric
+ * functions, for both dtypes (SCW_C128: rint; SCW_C64: the low word of the 64-bit integer nearest to phase * 2^32, valid
+ * for |phase| < 2^31 turns): any z of practical size gives the correctly reduced phase (the fp64 product itself carries
+ * 2^-53 |phase| turns of rounding, which is what limits complex128 beyond ~1e5 turns).
  */
 int32_t scw_assemble_spectra(scw_ctx* ctx, const scw_layer* layer, int64_t Fz, const double* z,
                              void* P, int64_t ldP);
@@ -186,6 +201,19 @@ int32_t scw_sweep_wavelengths(scw_ctx* ctx, int64_t n_inst, const scw_layer* ins
                               void* const* E, const int64_t* strides);
 int32_t scw_sweep_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz,
                             int64_t Nx, int64_t Ny, size_t* bytes);
+
+/*
+ * Calibrate the work split of the tensor-core assembly (step a-2) for this device and this workload: its persistent CTAs
+ * (one per SM) each stream a contiguous span of V, and the SMs do not all reach the same HBM rate (the same groups of SMs
+ * are slower in every run; by how much depends on what else the memory system is doing when the kernel starts).  Runs the
+ * given sweep -- arguments and outputs exactly as scw_sweep_wavelengths -- `reps` + 1 times per round for three rounds,
+ * measures every CTA of its assembly launch and makes the spans proportional to the measured rates for all later calls on
+ * this ctx (results change only in summation order).  SYNCHRONISES the stream.  A sweep that does not take the tensor-core
+ * assembly is accepted and leaves the equal split.  reps in [1, 64].  Errors: those of scw_sweep_wavelengths, VALUE (reps).
+ */
+int32_t scw_calibrate(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, const double* const* z,
+                      int64_t Nx, const double* x, int64_t Ny, const double* y, void* const* E, const int64_t* strides,
+                      int32_t reps);
 
 /*
  * Same as scw_sweep_wavelengths with every array in HOST memory (V, c, gamma, dir, z[i], x, y, E[i];

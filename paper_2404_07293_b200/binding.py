@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(HERE, "libscw.so")
 
 SCW_C64, SCW_C128 = 0, 1
 SCW_MODES_PLANEWAVE, SCW_MODES_DENSE = 0, 1
-SCW_OPT_PATH, SCW_OPT_PROFILE = 1, 2
+SCW_OPT_PATH, SCW_OPT_PROFILE, SCW_OPT_CACHE = 1, 2, 3
 SCW_PATH_AUTO, SCW_PATH_SIMT, SCW_PATH_TENSOR = 0, 1, 2
 STATUS = {0: "SCW_OK", 1: "SCW_ERR_NULL", 2: "SCW_ERR_SHAPE", 3: "SCW_ERR_DTYPE", 4: "SCW_ERR_ALIGN",
           5: "SCW_ERR_VALUE", 6: "SCW_ERR_WORKSPACE", 7: "SCW_ERR_CUDA", 8: "SCW_ERR_UNSUPPORTED"}
@@ -30,7 +30,7 @@ EXPORTS = [
     "scw_profile_classes", "scw_profile_name", "scw_profile_read", "scw_profile_reset",
     "scw_exterior_spectra", "scw_exterior_points", "scw_exterior_points_workspace",
     "scw_sweep_intensity", "scw_sweep_intensity_workspace",
-    "scw_measure_peak",
+    "scw_measure_peak", "scw_invalidate_cache", "scw_calibrate", "scw_profile_assembly",
 ]
 SCW_PEAKS = {"fp64_dmma_tflops": 0, "fp32_fma_tflops": 1, "mufu_gops": 2, "hbm_read_gbs": 3, "hbm_write_gbs": 4,
              "hbm_write_tma_gbs": 5}
@@ -113,6 +113,9 @@ def lib():
         L.scw_exterior_spectra.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, c_void_p, c_void_p, c_int64]
         L.scw_exterior_points.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, c_void_p, c_void_p]
         L.scw_exterior_points_workspace.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, POINTER(c_size_t)]
+        L.scw_invalidate_cache.argtypes = [c_void_p]
+        L.scw_profile_assembly.argtypes = [c_void_p, c_int32, POINTER(c_double), POINTER(c_int32)]
+        L.scw_calibrate.argtypes = L.scw_sweep_wavelengths.argtypes + [c_int32]
         L.scw_measure_peak.argtypes = [c_void_p, c_int32, c_void_p, c_size_t, c_int32, POINTER(c_double)]
         _LIB = L
     return _LIB
@@ -256,6 +259,13 @@ class Context:
     def set_path(self, path):
         self.check(self.L.scw_set_option(self._h, SCW_OPT_PATH, path))
 
+    def set_cache(self, on):
+        """SCW_OPT_CACHE: keep the twiddle tables in the workspace between consecutive sweep calls (see scwatter.h)."""
+        self.check(self.L.scw_set_option(self._h, SCW_OPT_CACHE, 1 if on else 0))
+
+    def invalidate_cache(self):
+        self.check(self.L.scw_invalidate_cache(self._h))
+
     def set_profile(self, on):
         self.check(self.L.scw_set_option(self._h, SCW_OPT_PROFILE, 1 if on else 0))
         self.check(self.L.scw_profile_reset(self._h))
@@ -279,6 +289,13 @@ class Context:
             self.check(self.L.scw_measure_peak(self._h, which, c_void_p(buf.data_ptr()), buf.numel(), reps, byref(v)))
             out[name] = v.value
         return out
+
+    def assembly_timeline(self):
+        """[(us to: own weights written, all weights seen, span streamed, exit)] per CTA of the last tcgen05 assembly."""
+        buf = (c_double * (256 * 4))()
+        n = c_int32()
+        self.check(self.L.scw_profile_assembly(self._h, 256, buf, byref(n)))
+        return [tuple(buf[4 * i:4 * i + 4]) for i in range(n.value)]
 
     def reserve(self, nbytes):
         """Grow the registered workspace to at least nbytes."""
@@ -384,6 +401,21 @@ def scw_sweep_wavelengths(ctx, layers, zs, x, y, out=None, strides=None):
     Ep = (c_void_p * max(n, 1))(*[e.data_ptr() for e in out])
     sarr = None if strides is None else (c_int64 * 4)(*strides)
     ctx.check(ctx.L.scw_sweep_wavelengths(ctx._h, n, inst, Fz, zp, Nx, _p(x), Ny, _p(y), Ep, sarr))
+    return out
+
+
+def scw_calibrate(ctx, layers, zs, x, y, out=None, strides=None, reps=5):
+    """Calibrate the stream-K split of the tensor-core assembly by running this sweep (synchronises); returns E."""
+    n, inst, Fz, zp = _sweep_args(layers, zs)
+    Nx, Ny = x.numel(), y.numel()
+    need = c_size_t()
+    ctx.check(ctx.L.scw_sweep_workspace(ctx._h, n, inst, Fz, Nx, Ny, byref(need)))
+    ctx.reserve(need.value)
+    if out is None:
+        out = [torch.empty((z.numel(), 3, Ny, Nx), dtype=l.V.dtype, device=ctx.device) for l, z in zip(layers, zs)]
+    Ep = (c_void_p * max(n, 1))(*[e.data_ptr() for e in out])
+    sarr = None if strides is None else (c_int64 * 4)(*strides)
+    ctx.check(ctx.L.scw_calibrate(ctx._h, n, inst, Fz, zp, Nx, _p(x), Ny, _p(y), Ep, sarr, reps))
     return out
 
 

@@ -1,5 +1,6 @@
 // C ABI of libscw: argument validation, workspace carving and kernel dispatch.
 // See include/scwatter.h for the contract of every entry point.
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -31,9 +32,15 @@ inline bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
 constexpr int64_t MAX_FREQ = 4096;        // per-axis frequency count
 constexpr int64_t MAX_GRID = 1 << 20;     // per-axis grid points
 
-int32_t check_ctx(scw_ctx* ctx)
+// sweep_call: only back-to-back sweep calls keep the cached twiddles / clean control block (any other call may carve
+// the same workspace bytes differently)
+int32_t check_ctx(scw_ctx* ctx, bool sweep_call = false)
 {
     if (!ctx) return SCW_ERR_NULL;
+    if (!sweep_call) {
+        ctx->tw_valid = false;
+        ctx->clean_ctl = nullptr;
+    }
     ctx->msg[0] = 0;
     ctx->cuda_err = 0;
     ctx->required_ws = 0;
@@ -110,7 +117,7 @@ bool use_dmma(const scw_ctx* ctx, int dtype) { return ctx->path != SCW_PATH_SIMT
 size_t assemble_ws(const scw_ctx* ctx, const scw_layer* L, int64_t Fz)
 {
     const int64_t R = 3LL * L->U * L->Vn;
-    if (use_tc_assemble(ctx, L, Fz)) return tc_assemble_scratch(R, L->J, Fz, 1, ctx->sm_count);
+    if (use_tc_assemble(ctx, L, Fz)) return tc_assemble_scratch(ctx, R, L->J, Fz, 1);
     if (use_dmma(ctx, L->dtype))
         return align_up((size_t)L->J * Fz * esize(L->dtype)) + dmma_assemble_scratch(R, L->J, Fz, ctx->sm_count);
     return align_up((size_t)L->J * Fz * esize(L->dtype)) + simt_assemble_scratch(L->dtype, R, L->J, Fz, ctx->sm_count);
@@ -120,7 +127,7 @@ void run_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z,
 {
     const int64_t R = 3LL * L->U * L->Vn;
     if (use_tc_assemble(ctx, L, Fz)) {
-        void* scratch = cv.take(tc_assemble_scratch(R, L->J, Fz, 1, ctx->sm_count));
+        void* scratch = cv.take(tc_assemble_scratch(ctx, R, L->J, Fz, 1));
         launch_tc_assemble(ctx, L, Fz, z, P, ldP, scratch);
         return;
     }
@@ -161,21 +168,39 @@ size_t synth_ws(const scw_ctx* ctx, int dtype, int U, int Vn, int64_t Fz, int64_
     return simt_synth_scratch(dtype, U, Fz, Ny);
 }
 
+// a-3.  With SCW_OPT_CACHE on, the tables of the previous call are reused when the key (coordinate pointers, sizes,
+// frequency grid, periods, location in the workspace) is unchanged.  zero / n_zero: ints the tensor-core twiddle kernel
+// clears on the way (control block of the assembly that follows); *zeroed tells whether that happened.
 Twiddles run_twiddles(scw_ctx* ctx, int dtype, int U, int Vn, double X, double Y, int64_t Nx, const double* x,
-                      int64_t Ny, const double* y, Carver& cv)
+                      int64_t Ny, const double* y, Carver& cv, int* zero = nullptr, size_t n_zero = 0, bool* zeroed = nullptr)
 {
     Twiddles t;
     t.tc = use_tc_synth(ctx, dtype, U, Vn);
+    if (zeroed) *zeroed = false;
     if (t.tc) {
         t.a = cv.take(tc_synth_twiddle_bytes(U, Vn, Nx, Ny));
         t.b = nullptr;
-        launch_tc_synth_twiddles(ctx, U, Vn, X, Y, Nx, x, Ny, y, t.a);
     } else {
         t.a = cv.take((size_t)U * Nx * esize(dtype));
         t.b = cv.take((size_t)Vn * Ny * esize(dtype));
+    }
+    scw_ctx::TwKey key;
+    key.x = x; key.y = y; key.where = t.a; key.Nx = Nx; key.Ny = Ny; key.U = U; key.Vn = Vn; key.dtype = dtype;
+    key.X = X; key.Y = Y; key.tc = t.tc;
+    const scw_ctx::TwKey& k0 = ctx->tw_key;
+    if (ctx->cache_on && ctx->tw_valid && k0.x == key.x && k0.y == key.y && k0.where == key.where && k0.Nx == key.Nx &&
+        k0.Ny == key.Ny && k0.U == key.U && k0.Vn == key.Vn && k0.dtype == key.dtype && k0.X == key.X && k0.Y == key.Y &&
+        k0.tc == key.tc)
+        return t;
+    if (t.tc) {
+        launch_tc_synth_twiddles(ctx, U, Vn, X, Y, Nx, x, Ny, y, t.a, zero, n_zero);
+        if (zeroed) *zeroed = zero != nullptr;
+    } else {
         launch_twiddles(ctx, dtype, U, Nx, x, X, t.a);
         launch_twiddles(ctx, dtype, Vn, Ny, y, Y, t.b);
     }
+    ctx->tw_key = key;
+    ctx->tw_valid = ctx->cache_on;
     return t;
 }
 
@@ -262,6 +287,16 @@ int32_t scw_set_workspace(scw_ctx* ctx, void* dev_ptr, size_t bytes)
     if (!aligned(dev_ptr, 256)) return fail(ctx, SCW_ERR_ALIGN, "workspace must be 256-byte aligned");
     ctx->ws = dev_ptr;
     ctx->ws_bytes = bytes;
+    ctx->tw_valid = false;
+    ctx->clean_ctl = nullptr;
+    return SCW_OK;
+}
+
+int32_t scw_invalidate_cache(scw_ctx* ctx)
+{
+    if (!ctx) return SCW_ERR_NULL;
+    ctx->tw_valid = false;
+    ctx->clean_ctl = nullptr;
     return SCW_OK;
 }
 
@@ -270,6 +305,13 @@ int32_t scw_set_option(scw_ctx* ctx, int32_t option, int64_t value)
     if (!ctx) return SCW_ERR_NULL;
     if (option == SCW_OPT_PATH && value >= SCW_PATH_AUTO && value <= SCW_PATH_TENSOR) {
         ctx->path = value;
+        ctx->tw_valid = false;
+        return SCW_OK;
+    }
+    if (option == SCW_OPT_CACHE && (value == 0 || value == 1)) {
+        ctx->cache_on = value != 0;
+        ctx->tw_valid = false;
+        ctx->clean_ctl = nullptr;
         return SCW_OK;
     }
     if (option == SCW_OPT_PROFILE && (value == 0 || value == 1)) {
@@ -433,8 +475,7 @@ static int sweep_group_size(const scw_ctx* ctx, int64_t n_inst, const scw_layer*
 static size_t sweep_group_ws(const scw_ctx* ctx, const scw_layer* L0, int64_t Fz, int group, int64_t Nx, int64_t Ny)
 {
     const int64_t R = 3LL * L0->U * L0->Vn;
-    return twiddle_ws(ctx, L0->dtype, L0->U, L0->Vn, Nx, Ny) + align_up((size_t)R * Fz * group * esize(L0->dtype)) +
-           align_up(tc_assemble_scratch(R, L0->J, Fz, group, ctx->sm_count)) +
+    return twiddle_ws(ctx, L0->dtype, L0->U, L0->Vn, Nx, Ny) + align_up(tc_assemble_scratch(ctx, R, L0->J, Fz, group)) +
            align_up(tc_synth_scratch(L0->U, L0->Vn, Fz * group));
 }
 
@@ -489,28 +530,38 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
     // intensity: E[i] are real buffers receiving sum_comp |E_comp|^2 at n*s4[1] + k*s4[2] + i*s4[3] (NEXT-3)
     const scw_layer& L0 = inst[0];
     const int64_t R = 3LL * L0.U * L0.Vn;
-    const Twiddles tw = run_twiddles(ctx, L0.dtype, L0.U, L0.Vn, L0.X, L0.Y, Nx, x, Ny, y, cv);
     const int group = sweep_group_size(ctx, n_inst, inst, Fz);
     if (group) {
-        // batched: all instances of a group share two assembly launches and two synthesis launches
-        void* P_all = cv.take((size_t)R * Fz[0] * group * esize(L0.dtype));
-        void* a_scr = cv.take(tc_assemble_scratch(R, L0.J, Fz[0], group, ctx->sm_count));
-        void* s_scr = cv.take(tc_synth_scratch(L0.U, L0.Vn, Fz[0] * group));
+        // batched: all instances of a group go through ONE assembly launch (weights + P = V W + fix-up that writes the
+        // synthesis kernel's spectrum images: P never goes to memory) and ONE synthesis launch; the twiddle launch, when
+        // it is not served from the cache, also clears the assembly's control block
+        Carver probe(cv.base);
+        probe.off = cv.off;
+        probe.take(tc_synth_twiddle_bytes(L0.U, L0.Vn, Nx, Ny));
+        void* a_scr = probe.take(tc_assemble_scratch(ctx, R, L0.J, Fz[0], group));
+        void* s_scr = probe.take(tc_synth_scratch(L0.U, L0.Vn, Fz[0] * group));
+        int* ctl = nullptr;
+        size_t n_ctl = 0;
+        tc_assemble_ctl(ctx, R, L0.J, Fz[0], group, a_scr, &ctl, &n_ctl);
+        bool clean = ctx->cache_on && ctx->clean_ctl == ctl && ctx->clean_ints >= n_ctl;
+        bool zeroed = false;
+        const Twiddles tw = run_twiddles(ctx, L0.dtype, L0.U, L0.Vn, L0.X, L0.Y, Nx, x, Ny, y, cv, clean ? nullptr : ctl,
+                                         n_ctl, &zeroed);
+        clean = clean || zeroed;
         for (int64_t i0 = 0; i0 < n_inst; i0 += group) {
             const int g = (int)(n_inst - i0 < group ? n_inst - i0 : group);
-            // the spectra go from the assembly's stream-K partial tiles straight into the synthesis images
-            TcPartials parts;
-            launch_tc_assemble_group_partials(ctx, g, inst + i0, Fz[0], z + i0, a_scr, &parts);
+            TcFixup fix = {};
+            int* sched = nullptr;
+            int n_sched = 0;
+            tc_synth_image_plan(L0.U, L0.Vn, Nx, Ny, s_scr, tw.a, &fix, &sched, &n_sched);
+            launch_tc_assemble_group(ctx, g, inst + i0, Fz[0], z + i0, fix, sched, n_sched, a_scr, clean);
             if (ctx->tc_error) return;
-            if (tc_synth_partials_supported(L0.U, L0.Vn, parts)) {
-                launch_tc_synth_group_partials(ctx, L0.U, L0.Vn, Fz[0], g, parts, Nx, Ny, tw.a, E + i0, s4, s_scr, intensity);
-            } else {
-                launch_tc_assemble_group(ctx, g, inst + i0, Fz[0], z + i0, P_all, R, R * Fz[0], a_scr);
-                launch_tc_synth_group(ctx, L0.U, L0.Vn, Fz[0], g, P_all, R, Nx, Ny, tw.a, E + i0, s4, s_scr, intensity);
-            }
+            clean = true;                               // the kernel leaves its control block zeroed
+            launch_tc_synth_group_images(ctx, L0.U, L0.Vn, Fz[0], g, Nx, Ny, tw.a, E + i0, s4, s_scr, intensity);
         }
         return;
     }
+    const Twiddles tw = run_twiddles(ctx, L0.dtype, L0.U, L0.Vn, L0.X, L0.Y, Nx, x, Ny, y, cv);
     void* P = cv.take((size_t)R * fz_max * esize(L0.dtype));
     const size_t asm_off = cv.off;
     cv.take(asm_max);
@@ -535,7 +586,7 @@ static int32_t sweep_impl(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, c
                           int64_t Nx, const double* x, int64_t Ny, const double* y, void* const* E, const int64_t* strides,
                           bool intensity, const char* who)
 {
-    if (int32_t s = check_ctx(ctx)) return s;
+    if (int32_t s = check_ctx(ctx, true)) return s;
     int64_t fz_max = 0;
     size_t asm_max = 0;
     if (int32_t s = check_sweep(ctx, n_inst, inst, Fz, Nx, Ny, who, &fz_max, &asm_max)) return s;
@@ -579,6 +630,84 @@ int32_t scw_sweep_intensity(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst,
                             void* const* I, const int64_t* strides)
 {
     return sweep_impl(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, I, strides, true, "scw_sweep_intensity");
+}
+
+int32_t scw_profile_assembly(scw_ctx* ctx, int32_t max_ctas, double* us, int32_t* n_ctas)
+{
+    if (!ctx || !us || !n_ctas) return SCW_ERR_NULL;
+    ctx->msg[0] = 0;
+    *n_ctas = 0;
+    const int G = ctx->last_asm_G;
+    if (G == 0 || !ctx->last_asm_ns) return SCW_OK;
+    if (max_ctas < G) return fail(ctx, SCW_ERR_SHAPE, "scw_profile_assembly: room for %d CTAs, %d needed", max_ctas, G);
+    std::vector<unsigned long long> ns((size_t)G * 4);
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpy(ns.data(), ctx->last_asm_ns, ns.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) {
+        ctx->cuda_err = (int32_t)e;
+        return fail(ctx, SCW_ERR_CUDA, "scw_profile_assembly: %s", cudaGetErrorString(e));
+    }
+    for (size_t i = 0; i < ns.size(); ++i) us[i] = (double)ns[i] * 1e-3;
+    *n_ctas = G;
+    return SCW_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// Stream-K split calibration: the persistent CTAs of the tcgen05 assembly do not all stream from HBM at the same rate
+// (the same groups of SMs are slower in every run, and how much depends on what the L2 is busy with when the kernel
+// starts), so equal spans leave a tail.  Runs the given sweep as the caller will run it, reads the per-CTA durations of
+// its assembly launch and sets every CTA's (= SM's) share proportional to its measured rate.
+int32_t scw_calibrate(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, const double* const* z,
+                      int64_t Nx, const double* x, int64_t Ny, const double* y, void* const* E, const int64_t* strides,
+                      int32_t reps)
+{
+    if (!ctx) return SCW_ERR_NULL;
+    if (reps < 1 || reps > 64) return fail(ctx, SCW_ERR_VALUE, "scw_calibrate: reps must be in [1, 64]");
+    ctx->split_w.clear();
+    std::vector<unsigned long long> ns(4 * 256);
+    for (int round = 0; round < 3; ++round) {
+        std::vector<std::vector<double>> samples;
+        int G = 0;
+        for (int r = 0; r <= reps; ++r) {           // the first sweep of a round is a warm-up
+            ctx->last_asm_G = 0;
+            if (int32_t s = sweep_impl(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, E, strides, false, "scw_calibrate")) {
+                ctx->split_w.clear();
+                return s;
+            }
+            G = ctx->last_asm_G;
+            if (G < 2) return SCW_OK;               // not on the tensor-core assembly: nothing to calibrate
+            cudaError_t e = cudaStreamSynchronize(ctx->stream);
+            if (e == cudaSuccess)
+                e = cudaMemcpy(ns.data(), ctx->last_asm_ns, (size_t)G * 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+            if (e != cudaSuccess) {
+                ctx->cuda_err = (int32_t)e;
+                ctx->split_w.clear();
+                return fail(ctx, SCW_ERR_CUDA, "scw_calibrate: %s", cudaGetErrorString(e));
+            }
+            if (r == 0) continue;
+            std::vector<double> rate(G);
+            for (int c = 0; c < G; ++c)
+                rate[c] = (double)(ctx->last_asm_span0[c + 1] - ctx->last_asm_span0[c]) /
+                          (double)(ns[4 * c + 2] > ns[4 * c + 1] ? ns[4 * c + 2] - ns[4 * c + 1] : 1);      // main loop only
+            samples.push_back(rate);
+        }
+        std::vector<double> w(G);
+        double mean = 0.0;
+        for (int c = 0; c < G; ++c) {               // median over the repetitions
+            std::vector<double> v;
+            for (auto& sm : samples) v.push_back(sm[c]);
+            std::sort(v.begin(), v.end());
+            w[c] = v[v.size() / 2];
+            mean += w[c] / G;
+        }
+        for (int c = 0; c < G; ++c) {               // clipped: no span beyond ~1.5x the mean (bounds the partial-tile slots)
+            w[c] /= mean;
+            if (!(w[c] > 0.6)) w[c] = 0.6;
+            if (w[c] > 1.5) w[c] = 1.5;
+        }
+        ctx->split_w = w;
+    }
+    return SCW_OK;
 }
 
 // ------------------------------------------------------------------------------------------

@@ -33,6 +33,18 @@ struct scw_ctx {
     char msg[256] = {0};
     bool profile = false;
     bool tc_error = false;          // a tensor map could not be encoded (reported by the entry point)
+    // stream-K split of the tcgen05 assembly: relative rate of every persistent CTA (scw_calibrate), empty = equal spans
+    std::vector<double> split_w;
+    int last_asm_G = 0;             // the last assembly launch: grid, spans, where its per-CTA nanoseconds are (device)
+    int64_t last_asm_span0[161] = {0};
+    const unsigned long long* last_asm_ns = nullptr;
+    // twiddle cache (SCW_OPT_CACHE): key of the twiddle images held in the workspace, and the control block known clean
+    bool cache_on = false;
+    struct TwKey { const void *x = nullptr, *y = nullptr, *where = nullptr; int64_t Nx = 0, Ny = 0; int U = 0, Vn = 0, dtype = -1;
+                   double X = 0, Y = 0; bool tc = false; } tw_key;
+    bool tw_valid = false;
+    const void* clean_ctl = nullptr;
+    size_t clean_ints = 0;
     cudaEvent_t prof_last = nullptr;   // profiling: end event of the previous kernel of this API call
     std::vector<scw::ProfRec> recs;
     double prof_ms[scw::KC_COUNT] = {0};
@@ -113,24 +125,26 @@ void launch_intensity(scw_ctx* ctx, int dtype, int64_t Fz, int64_t Ny, int64_t N
 // ---- scw_tc_assemble.cu: tcgen05 BF16x3 spectral assembly (complex64) ----------------------------
 bool tc_assemble_supported(int dtype, int64_t R, int64_t J, int64_t Fz, const void* V, int64_t ldV);
 int tc_assemble_max_group();
-size_t tc_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int n_inst, int sm_count);
-// n_inst <= tc_assemble_max_group() instances with equal U, Vn, J, Fz in three launches; instance i -> P_all + i*inst_stride
-void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
-                              void* P_all, int64_t ldP, int64_t inst_stride, void* scratch);
-// Where the stream-K partial tiles of a grouped assembly are: tile (inst, n_tile, m_tile) = rows_per_tile complex
-// rows x Fzt planes, fp32 [plane][2*rows_per_tile].  A tile is the sum of seg_count[tile] segments, segment i in slot
-// seg_slot[tile*max_segs + i] (the table is written by the assembly kernel, in CTA order: a fixed summation order).
-struct TcPartials {
-    const float* part;
-    const int* seg_count;
-    const int* seg_slot;
-    int Fzt, n_tiles, m_tiles, max_segs, rows_per_tile;
+size_t tc_assemble_scratch(const scw_ctx* ctx, int64_t R, int64_t J, int64_t Fz, int n_inst);
+// Where the control block (arrival counters, must be zero at launch) of an assembly over `scratch` lies.
+void tc_assemble_ctl(const scw_ctx* ctx, int64_t R, int64_t J, int64_t Fz, int n_inst, void* scratch, int** ctl, size_t* n_ints);
+// What the assembly kernel's fix-up writes once a tile is complete.
+enum { TC_FIX_P = 0, TC_FIX_IMAGES = 1, TC_FIX_NONE = 2 };
+struct TcFixup {
+    int mode;
+    int64_t R;                  // rows of P (3M), filled in by the launcher
+    // TC_FIX_P: instance i -> P + i*inst_stride, column-major [ldP x Fz] complex64
+    float2* P;
+    int64_t ldP, inst_stride;
+    // TC_FIX_IMAGES: spectrum images of k_tc_synth (scw_tc_synth.cu): image ((inst*Fz + n)*3 + comp, uc, vc), hi | lo,
+    // N1 rows x K1p, K-major core-matrix layout; chunks of Uc x Vc frequencies
+    uint8_t* img;
+    int U, Vn, Uc, Vc, nuc, nvc, K1p, N1;
 };
-// weights (a-1) + stream-K partial tiles of P = V W (a-2), WITHOUT the segment reduce: the consumer sums the segments
-// (launch_tc_synth_group_partials folds that into its spectrum-image pass, so P never goes to memory).
-void launch_tc_assemble_group_partials(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
-                                       void* scratch, TcPartials* out);
-// weights (a-1) + P = V W (a-2) + segment reduce; scratch from tc_assemble_scratch
+// weights (a-1) + P = V W (a-2) + fix-up, n_inst <= tc_assemble_max_group() instances with equal U, Vn, J, Fz in ONE launch;
+// sched/n_sched: plane counters of the synthesis that follows (zeroed by the kernel), may be NULL.
+void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
+                              const TcFixup& fix, int* sched, int n_sched, void* scratch, bool ctl_clean);
 void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z, void* P, int64_t ldP,
                         void* scratch);
 
@@ -138,19 +152,22 @@ void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const doub
 bool tc_synth_supported(int dtype, int U, int Vn);
 size_t tc_synth_twiddle_bytes(int U, int Vn, int64_t Nx, int64_t Ny);
 size_t tc_synth_scratch(int U, int Vn, int64_t Fz);
+// zero/n_zero: ints cleared by the same launch (the control block of the assembly that follows), may be NULL
 void launch_tc_synth_twiddles(scw_ctx* ctx, int U, int Vn, double X, double Y, int64_t Nx, const double* x, int64_t Ny,
-                              const double* y, void* tw);
+                              const double* y, void* tw, int* zero = nullptr, size_t n_zero = 0);
 int tc_synth_max_group();
+// Image layout of a synthesis over `scratch` (for the assembly's fix-up) and its plane counters inside the twiddle blob.
+void tc_synth_image_plan(int U, int Vn, int64_t Nx, int64_t Ny, void* scratch, const void* tw, TcFixup* fix, int** sched,
+                         int* n_sched);
 // n_inst instances with equal Fz, spectra back to back in P_all ([ldP x n_inst*Fz]); scratch = tc_synth_scratch(U, Vn, Fz*n_inst)
 // intensity: E[i] are float buffers receiving I = sum_comp |E_comp|^2 at z*strides[1] + y*strides[2] + x*strides[3]
 void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const void* P_all, int64_t ldP,
                            int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
                            void* scratch, bool intensity = false);
-// Same, reading the spectra as stream-K partial tiles (segment reduce fused into the image pass).
-bool tc_synth_partials_supported(int U, int Vn, const TcPartials& parts);
-void launch_tc_synth_group_partials(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const TcPartials& parts,
-                                    int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
-                                    void* scratch, bool intensity = false);
+// Same, with the spectrum images already in `scratch` and the plane counters zeroed (written by the assembly's fix-up).
+void launch_tc_synth_group_images(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, int64_t Nx, int64_t Ny,
+                                  const void* tw, void* const* E, const int64_t strides[4], void* scratch,
+                                  bool intensity = false);
 void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,
                      const void* tw, void* E, const int64_t strides[4], void* scratch);
 

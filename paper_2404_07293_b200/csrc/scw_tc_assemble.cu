@@ -9,21 +9,28 @@
 // (rows 2r / 2r+1 = Re / Im of complex row r); the small operand is laid out as [W_r | W_i] so that one
 // real GEMM yields all four real products, combined between adjacent TMEM lanes in the epilogue.
 //
-// Work decomposition ("stream-K"): the iteration space (instance, n_tile, m_tile, k_block) is cut into
-// equal contiguous spans, one per persistent CTA (one CTA per SM); every (CTA, tile) segment writes an
-// fp32 partial tile, k_tc_reduce sums the segments of each tile in a fixed order (deterministic).
+// ONE launch does steps a-1 and a-2 and hands the spectra to the consumer in its format:
+//  phase 0  every CTA computes its share of the mode weights W (a-1, eq. 7 / 30) as bf16 hi/lo UMMA images in
+//           global memory (L2-resident, re-read by all m-tiles), zero-fills the padding of the synthesis images and
+//           publishes a grid-wide counter; only the W loader warp waits for it, the V pipeline fills meanwhile.
+//  main     "stream-K": the iteration space (instance, n_tile, m_tile, k_block) is cut into contiguous spans, one per
+//           persistent CTA (one CTA per SM; equal spans, or spans weighted by the per-CTA rates of
+//           scw_calibrate()); every (CTA, tile) segment writes an fp32 partial tile.
+//  fix-up   the CTA that completes a tile LAST (per-tile arrival counter) sums the tile's segments in CTA order
+//           (deterministic) and writes either P (column-major complex64) or the synthesis kernel's spectrum images
+//           (bf16 hi/lo, "complex as real" rows) -- there is no separate reduce / image kernel, P never goes to memory
+//           inside a sweep.
 //
 // A tile is 128 complex rows (two 128-lane M blocks) x 32 modes per pipeline stage.  V reaches shared
 // memory through TMA: two tensor maps per instance describe the even and the odd columns of V (column
 // stride 2*ldV*8 bytes is a multiple of 16 for any ldV; for odd ldV the odd-column map starts one element
 // early with a 130-row box so that every box starts on a 16-byte boundary), so one elected thread issues two
-// 16 KB box copies per stage --
-// 1 KB contiguous per column, rows past R and columns past J arrive as zeros.
+// 16 KB box copies per stage -- 1 KB contiguous per column, rows past R and columns past J arrive as zeros.
 // Warp roles (768 threads): warps 0-15 (two groups of 8 on alternate stages) read their real row of the
 // staged fp32 tile, split it to bf16 hi/lo and write the A operand straight into TMEM (tcgen05.st); warp 16 =
-// TMA producer for V; warp 17 fetches the pre-formatted W tiles with bulk copies; warp 18 issues tcgen05.mma
+// TMA producer for V; warp 17 fetches the W tiles with bulk copies; warp 18 issues tcgen05.mma
 // (A from TMEM, B from shared memory); warps 20-23 drain the accumulators (tcgen05.ld), combine lanes with
-// one shuffle per element and store the partial tile.
+// one shuffle per element, store the partial tile and run the fix-up.
 #include <cuda.h>
 
 #include "scw_internal.h"
@@ -39,6 +46,7 @@ constexpr int TA_CONV_WARPS = 8;           // converter warp w of a group owns r
 constexpr int TA_CONV_GROUPS = 2;          // group g converts the CTA's iterations n = g, g+2, ... (two stages in flight)
 constexpr int TA_V_LOADER = 16, TA_W_LOADER = 17, TA_MMA_WARP = 18, TA_EPI_WARP0 = 20;
 constexpr int TA_THREADS = 24 * 32;
+constexpr int TA_P0_THREADS = TA_THREADS - 32;        // phase 0 runs on every warp but the V loader
 constexpr int TA_A_COL = 256;              // TMEM: A operand, per MMA stage and M block 16 columns hi + 16 columns lo
 constexpr int TA_STG_ODD = TA_ROWS * 8 * 16;          // fp32 staging slot: [16 even columns][128 rows] then the odd-column box
 constexpr int TA_STG_BYTES = TA_STG_ODD + 16 * (TA_ROWS + 2) * 8;   // odd-column box: up to 130 rows (odd ldV, see ta_make_map)
@@ -46,19 +54,33 @@ constexpr int TA_MMA_STAGES = 3;
 constexpr int TA_TMEM_COLS = 512;
 constexpr int TA_SMEM_LIMIT = 226 * 1024;
 constexpr int TA_MAX_STG = 5;
+constexpr int TA_MAX_CTAS = 160;           // span table size (>= SM count)
+constexpr int TA_CTL_CLAIM = 2;            // control block: [0] CTAs past phase 0, [1] CTAs out, [2..] span claimed, then tiles
+constexpr int TA_CTL_TILE = TA_CTL_CLAIM + TA_MAX_CTAS;
 
 constexpr int TA_MAX_INST = 64;            // instances (layers x wavelengths) per grouped launch
-
 
 struct TaParams {
     CUtensorMap tmap[TA_MAX_INST][2];   // [0]: even columns of V, [1]: odd columns; box = 128 rows x 16 columns of 8 bytes
     int xoff1[TA_MAX_INST];             // 1 when ldV is odd: odd-column box has 130 rows and starts one element early
+    // a-1 inputs per instance
+    const float2* c[TA_MAX_INST];
+    const double2* gamma[TA_MAX_INST];
+    const int8_t* dir[TA_MAX_INST];
+    const double* z[TA_MAX_INST];
+    double inv_lambda[TA_MAX_INST], z_lo[TA_MAX_INST], z_hi[TA_MAX_INST];
+    int64_t span0[TA_MAX_CTAS + 1];     // CTA c owns iterations [span0[c], span0[c+1])
     int n_inst;
-    const uint8_t* Wt;      // [inst][n_tile][k_block][hi | lo] K-major UMMA images of [W_r | W_i]
+    int64_t J, Fz;
+    uint8_t* Wt;            // [inst][n_tile][k_block][hi | lo] K-major UMMA images of [W_r | W_i]
     float* part;            // [slot][Fzt][256] fp32 partial tiles
-    int* seg_count;         // [tile] number of stream-K segments of the tile (written by the tile's first CTA)
-    int* seg_slot;          // [tile][max_segs] slot of every segment, in CTA order
-    int N2, Fzt, n_tiles, m_tiles, kblocks, S, stg_stages, nbuf, max_segs;
+    int* ctl;               // [0] CTAs past phase 0, [1] CTAs out, [TA_CTL_CLAIM + s] span s taken, [TA_CTL_TILE + tile] segments stored
+    unsigned long long* cta_ns;   // [CTA][4] ns since the CTA's prologue (globaltimer): phase 0 done, all weights seen,
+                                  // main loop done, exit (read by scw_calibrate / scw_profile_assembly)
+    int* sched;             // plane counters of the synthesis that follows (zeroed here), may be NULL
+    int n_sched;
+    int N2, Fzt, n_tiles, m_tiles, kblocks, S, stg_stages, nbuf;
+    TcFixup fix;
 };
 
 // Mode index of staging column kk (0..31) of k-block kb: even modes first, then odd modes.
@@ -67,75 +89,277 @@ __host__ __device__ __forceinline__ int64_t ta_mode(int kb, int kk)
     return (int64_t)kb * TA_BK + (kk < 16 ? 2 * kk : 2 * (kk - 16) + 1);
 }
 
-// ---- W~ in UMMA image form -----------------------------------------------------------------------
-// a-1 mode weights (eq. 7, 30): phase reduced in fp64 (turns), sincospi / exp in fp32 (the result is split to
+__device__ __forceinline__ int ld_acquire_gpu(const int* p)
+{
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned long long ta_now()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ void fence_proxy_async_global() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
+
+// ---- phase 0 ---------------------------------------------------------------------------------------
+// a-1 mode weights (eq. 7, 30): phase reduced in fp64 (turns), sin / cos / ex2 on the MUFU pipe (the result is split to
 // bf16 hi + lo, 2^-17 relative, so fp32 transcendentals lose nothing), written as the K-major no-swizzle
 // shared-memory image of every (n_tile, k_block) B tile: element (n, kk) at
 //   (kk/8)*(N2*16) + (n/8)*128 + (n%8)*16 + (kk%8)*2,  n < Fzt: Re W[j, i], n >= Fzt: Im W[j, i],  j = ta_mode(kb, kk).
-// One thread produces two consecutive kk (4 bytes of a 16-byte core-matrix row), for the Re and the Im row, hi and lo.
-struct TwGroup {
-    const float2* c[TA_MAX_INST];
-    const double2* gamma[TA_MAX_INST];
-    const int8_t* dir[TA_MAX_INST];
-    const double* z[TA_MAX_INST];
-    double inv_lambda[TA_MAX_INST], z_lo[TA_MAX_INST], z_hi[TA_MAX_INST];
-};
-
-__global__ void __launch_bounds__(256) k_tc_weights(int n_inst, int64_t J, int64_t Fz, int Fzt, int n_tiles, int kblocks,
-                                                    const __grid_constant__ TwGroup g_, uint8_t* __restrict__ Wt_all)
+// fp64 -> fp32 without the (slow) conversion instruction: truncates the mantissa, flushes |x| < 2^-126 to 0, saturates to
+// +-3.4e38-ish beyond the fp32 range (the value is a log2 amplitude: both ends mean 0 or inf after ex2 anyway).
+__device__ __forceinline__ float ta_f64_to_f32_trunc(double x)
 {
-    // block = one (inst, n_tile, k_block) tile; thread item = (k chunk c4, plane n, mode pair e2), e2 fastest: the four
-    // lanes of a pair group fill one 16-byte core-matrix row, a warp writes 128 contiguous bytes per store
-    const int kb = blockIdx.x, nt = blockIdx.y, inst = blockIdx.z;
-    const int64_t tile_id = ((int64_t)inst * n_tiles + nt) * kblocks + kb;
-    const float2* __restrict__ c = g_.c[inst];
-    const double2* __restrict__ gamma = g_.gamma[inst];
-    const int8_t* __restrict__ dir = g_.dir[inst];
-    const double inv_lambda = g_.inv_lambda[inst], z_lo = g_.z_lo[inst], z_hi = g_.z_hi[inst];
-    const int N2 = 2 * Fzt;
-    uint8_t* tile = Wt_all + (size_t)tile_id * (size_t)N2 * 128;
-    for (int rem = threadIdx.x; rem < 16 * Fzt; rem += blockDim.x) {
-    const int e2 = rem & 3, cn = rem >> 2;
-    const int c4 = cn / Fzt, n = cn - c4 * Fzt;                        // k chunk (8 modes), plane within the n tile
-    const int64_t i = (int64_t)nt * Fzt + n;
-    const double zi = i < Fz ? g_.z[inst][i] : 0.0;
-    float wr[2], wi[2];
+    const uint32_t hi = (uint32_t)__double2hiint(x), lo = (uint32_t)__double2loint(x);
+    const uint32_t sign = hi & 0x80000000u, mag = hi & 0x7fffffffu;
+    const uint32_t e11 = mag >> 20;                                  // biased fp64 exponent
+    uint32_t bits = ((mag - (896u << 20)) << 3) | (lo >> 29);        // rebias 1023 -> 127, 20 + 3 mantissa bits
+    if (e11 < 897u) bits = 0u;                                       // below the fp32 normal range
+    if (e11 > 1150u) bits = 0x7f000000u;                             // above: a huge finite number
+    return __uint_as_float(sign | bits);
+}
+
+// One warp produces an 8-mode k chunk c4 of a tile: lane = (mode pair e2, plane n % 8) writes two consecutive kk (4 bytes
+// of a 16-byte core-matrix row) for the Re and the Im row, hi and lo, and walks the plane octets -- the mode data (gamma,
+// c, dir) are loaded once per lane, a warp store covers 128 contiguous bytes.
+__device__ __forceinline__ void ta_weight_unit(const TaParams& p, int64_t tile_id, int c4, int lane)
+{
+    const int per_g = p.kblocks;
+    const int g = (int)(tile_id / per_g), kb = (int)(tile_id - (int64_t)g * per_g);
+    const int inst = g / p.n_tiles, nt = g - inst * p.n_tiles;
+    const float2* __restrict__ c = p.c[inst];
+    const double2* __restrict__ gamma = p.gamma[inst];
+    const int8_t* __restrict__ dir = p.dir[inst];
+    const double* __restrict__ z = p.z[inst];
+    const double inv_lambda = p.inv_lambda[inst];
+    const int Fzt = p.Fzt, N2 = p.N2;
+    uint8_t* tile = p.Wt + (size_t)tile_id * (size_t)N2 * 128;
+    const int e2 = lane & 3, nn = lane >> 2;
+    // per mode: phase (turns) = pa z + pb, log2 amplitude = ka z + kb  (fp64: z may be far from zref)
+    double pa[2], pb[2], ka[2], kb2[2];
+    float cr[2], ci[2];
+    bool live[2];
 #pragma unroll
     for (int e = 0; e < 2; ++e) {
         const int64_t j = ta_mode(kb, 8 * c4 + 2 * e2 + e);
-        wr[e] = 0.f;
-        wi[e] = 0.f;
-        if (j < J && i < Fz) {
-            const double2 g = gamma[j];
-            const int d = dir ? (dir[j] > 0 ? 1 : -1) : ((g.y > 0.0 || (g.y == 0.0 && g.x >= 0.0)) ? 1 : -1);
-            const double dz = (zi - (d > 0 ? z_lo : z_hi)) * inv_lambda;
-            // phase in turns, reduced in fp64 by the magic-constant trick: the low word of t + 1.5*2^20 is
-            // frac(t) * 2^32 (two's complement: an angle in [-pi, pi) after scaling), then the MUFU sin / cos / ex2
-            // (abs. error ~5e-7, below the 2^-17 of the bf16 hi/lo split that follows)
-            // (the product is reduced with rint first, so a thick layer with |gamma dz / lambda| >= 2^19 turns is fine)
-            const double tt = g.x * dz;
-            const int ph = __double2loint((tt - rint(tt)) + 1572864.0);
-            const float ang = __int2float_rn(ph) * 1.4629180792671596e-9f;           // 2 pi / 2^32
-            const float s = __sinf(ang), co = __cosf(ang);
-            const float a = exp2f((float)(-9.0647202836543876194 * g.y * dz));        // exp(-2 pi x) = 2^(-2 pi log2(e) x)
-            float cr = 1.f, ci = 0.f;
-            if (c) { cr = c[j].x; ci = c[j].y; }
-            const float ar = a * co, ai = a * s;
-            wr[e] = cr * ar - ci * ai;
-            wi[e] = cr * ai + ci * ar;
+        live[e] = j < p.J;
+        pa[e] = pb[e] = ka[e] = kb2[e] = 0.0;
+        cr[e] = 1.f;
+        ci[e] = 0.f;
+        if (live[e]) {
+            const double2 gm = gamma[j];
+            const int d = dir ? (dir[j] > 0 ? 1 : -1) : ((gm.y > 0.0 || (gm.y == 0.0 && gm.x >= 0.0)) ? 1 : -1);
+            const double zref = d > 0 ? p.z_lo[inst] : p.z_hi[inst];
+            pa[e] = gm.x * inv_lambda;
+            ka[e] = -9.0647202836543876194 * gm.y * inv_lambda;                    // exp(-2 pi x) = 2^(-2 pi log2(e) x)
+            pb[e] = -pa[e] * zref;
+            kb2[e] = -ka[e] * zref;
+            if (c) { cr[e] = c[j].x; ci[e] = c[j].y; }
         }
     }
-    uint32_t rh, rl, ih, il;
-    split_bf16x2(wr[0], wr[1], rh, rl);
-    split_bf16x2(wi[0], wi[1], ih, il);
-    const int n2 = n + Fzt;
-    const size_t off_r = (size_t)c4 * (N2 * 16) + (size_t)(n >> 3) * 128 + (n & 7) * 16 + e2 * 4;
-    const size_t off_i = (size_t)c4 * (N2 * 16) + (size_t)(n2 >> 3) * 128 + (n2 & 7) * 16 + e2 * 4;
     const size_t lo = (size_t)N2 * 64;
-    *reinterpret_cast<uint32_t*>(tile + off_r) = rh;
-    *reinterpret_cast<uint32_t*>(tile + off_i) = ih;
-    *reinterpret_cast<uint32_t*>(tile + lo + off_r) = rl;
-    *reinterpret_cast<uint32_t*>(tile + lo + off_i) = il;
+    uint8_t* lane_base = tile + (size_t)c4 * (N2 * 16) + nn * 16 + e2 * 4;
+    double zv[8];                                      // this lane's planes (Fzt <= 64), loaded up front: one round trip
+#pragma unroll
+    for (int o = 0; o < 8; ++o) {
+        const int64_t i = (int64_t)nt * Fzt + nn + 8 * o;
+        zv[o] = (nn + 8 * o < Fzt && i < p.Fz) ? z[i] : 0.0;
+    }
+    // Stage by stage over 4 planes x 2 modes, so that eight independent chains are in flight.  Only fp64 ADD / FMA and
+    // integer instructions touch the doubles: the fp64 CONVERSION instructions (FRND, F2F, F2I) run at a few lanes per
+    // clock and made this phase 3x longer.  The phase in turns is reduced for any layer thickness (|t| < 2^51): rint by
+    // adding and subtracting 1.5*2^52, then the low word of frac(t) + 1.5*2^20 is frac(t) * 2^32 in two's complement --
+    // an angle in [-pi, pi) after scaling; then MUFU sin / cos / ex2 (abs. error ~5e-7, below the 2^-17 of the bf16
+    // hi/lo split that follows).  The log2 amplitude goes from fp64 to fp32 by bit surgery (truncation, 2^-23 relative).
+#pragma unroll
+    for (int o0 = 0; o0 < 8; o0 += 4) {
+        if (nn + 8 * o0 >= Fzt) break;
+        int ph[4][2];
+        float ex[4][2];
+#pragma unroll
+        for (int o = 0; o < 4; ++o)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const double t = fma(pa[e], zv[o0 + o], pb[e]);
+                const double r = (t + 6755399441055744.0) - 6755399441055744.0;          // rint(t)
+                ph[o][e] = __double2loint((t - r) + 1572864.0);
+                ex[o][e] = ta_f64_to_f32_trunc(fma(ka[e], zv[o0 + o], kb2[e]));
+            }
+#pragma unroll
+        for (int o = 0; o < 4; ++o) {
+            const int n = nn + 8 * (o0 + o);
+            if (n >= Fzt) continue;
+            const bool in = (int64_t)nt * Fzt + n < p.Fz;
+            float wr[2], wi[2];
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const float ang = __int2float_rn(ph[o][e]) * 1.4629180792671596e-9f;     // 2 pi / 2^32
+                const float sn = __sinf(ang), co = __cosf(ang);
+                const float a = exp2f(ex[o][e]);
+                const float ar = a * co, ai = a * sn;
+                const bool on = live[e] && in;
+                wr[e] = on ? cr[e] * ar - ci[e] * ai : 0.f;
+                wi[e] = on ? cr[e] * ai + ci[e] * ar : 0.f;
+            }
+            uint32_t rh, rl, ih, il;
+            split_bf16x2(wr[0], wr[1], rh, rl);
+            split_bf16x2(wi[0], wi[1], ih, il);
+            // n = nn + 8 (o0 + o): core-matrix row nn of row group o0 + o; the Im row n + Fzt is Fzt/8 row groups on
+            uint8_t* dst = lane_base + (o0 + o) * 128;
+            *reinterpret_cast<uint32_t*>(dst) = rh;
+            *reinterpret_cast<uint32_t*>(dst + Fzt * 16) = ih;
+            *reinterpret_cast<uint32_t*>(dst + lo) = rl;
+            *reinterpret_cast<uint32_t*>(dst + lo + Fzt * 16) = il;
+        }
+    }
+}
+
+// Everything the main loop of ANY CTA depends on, spread over all CTAs: t = this thread's index among the
+// gridDim.x * TA_P0_THREADS phase-0 threads of the grid.
+__device__ __forceinline__ void ta_phase0(const TaParams& p, int64_t t, int64_t nthreads)
+{
+    // (1) weight images: warp units (tile, k chunk of 8 modes)
+    {
+        const int64_t n_units = (int64_t)p.n_inst * p.n_tiles * p.kblocks * (TA_BK / 8);
+        const int lane = (int)(t & 31);
+        // units are dealt round-robin over the CTAs (warp w of CTA b takes units w*G + b, ...): every SM gets its share
+        const int64_t first = (int64_t)((t % TA_P0_THREADS) >> 5) * gridDim.x + blockIdx.x;
+        for (int64_t unit = first; unit < n_units; unit += nthreads >> 5)
+            ta_weight_unit(p, unit >> 2, (int)(unit & 3), lane);
+    }
+    // (2) spectrum images of the synthesis: every 16-byte chunk that is not entirely spectrum data is zeroed (frequency
+    // and K padding; the chunks that straddle the edge get their data from the fix-up, which runs after phase 0 of all CTAs)
+    if (p.fix.mode == TC_FIX_IMAGES) {
+        const TcFixup& f = p.fix;
+        const int chunks_half = f.N1 * (f.K1p / 8);                      // chunk id within a hi or lo image = kc*N1 + row
+        const int n_half = (int)(p.n_inst * p.Fz * 3 * f.nuc * f.nvc * 2);   // (image, hi/lo) halves, < 2^31
+        const int per_image = f.nuc * f.nvc;                                 // <= 4 kinds of image (uc, vc)
+        for (int rem = (int)(t % TA_P0_THREADS); rem < chunks_half; rem += TA_P0_THREADS) {
+            // this thread's chunk of every image half.  MN-major image: chunk = rows 8*nb .. 8*nb+7 at one k,
+            // chunk id = (k/8)*N1 + nb*8 + k%8.  bit ci of `pad`: the chunk is not entirely spectrum data in images of kind ci
+            const int kblk = rem / f.N1, r2 = rem - kblk * f.N1;
+            const int nb = r2 >> 3, k = 8 * kblk + (r2 & 7);
+            unsigned pad = 0;
+            for (int ci = 0; ci < per_image; ++ci) {
+                const int uc = ci / f.nvc, vc = ci - uc * f.nvc;
+                const int ulen = min(f.Uc, f.U - uc * f.Uc), vlen = min(f.Vc, f.Vn - vc * f.Vc);
+                if (!(4 * nb + 3 < ulen && k < 2 * vlen)) pad |= 1u << ci;
+            }
+            if (pad == 0) continue;
+            uint4* dst = reinterpret_cast<uint4*>(f.img) + rem;
+            for (int half = blockIdx.x; half < n_half; half += gridDim.x) {
+                const int ci = per_image == 1 ? 0 : (half >> 1) % per_image;
+                if ((pad >> ci) & 1u) dst[(size_t)half * chunks_half] = make_uint4(0u, 0u, 0u, 0u);
+            }
+        }
+    }
+    // (3) plane counters of the synthesis kernel
+    for (int64_t i = t; i < p.n_sched; i += nthreads) p.sched[i] = 0;
+}
+
+// ---- fix-up: the last CTA to store a segment of a tile sums the tile and writes it in the consumer's format ----------
+// CTA that owns iteration i: the largest c with span0[c] <= i (empty spans are never picked for an existing iteration).
+__device__ __forceinline__ int ta_owner(const TaParams& p, int64_t i, int G)
+{
+    int lo = 0, hi = G - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (p.span0[mid] <= i) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
+// A crew of 128 * groups threads: thread (r, pg) owns complex row r of the tile and the planes pg, pg + groups, ... .
+// Segments are summed in CTA order (a fixed order: deterministic).  E planes per batch: the loads of the first two
+// segments of a batch are all in flight at once (one round trip for a tile of two segments), further segments follow.
+template <int E>
+__device__ __forceinline__ void ta_fixup(const TaParams& p, int64_t tile, int c_first, int c_last, int r, int pg, int groups)
+{
+    const TcFixup& f = p.fix;
+    const int gnt = (int)(tile / p.m_tiles), mt = (int)(tile - (int64_t)gnt * p.m_tiles);
+    const int inst = gnt / p.n_tiles, nt = gnt - inst * p.n_tiles;
+    const int64_t row = (int64_t)mt * TA_ROWS + r;
+    if (row >= f.R) return;
+    const int nv = (int)min((int64_t)p.Fzt, p.Fz - (int64_t)nt * p.Fzt);        // planes of this n tile that exist
+    const size_t tile_floats = (size_t)p.Fzt * 2 * TA_ROWS;
+    // image addressing (TC_FIX_IMAGES): row = comp*M + v*U + u -> image (plane, uc, vc), rows 2ul / 2ul+1, k = 2vl
+    uint8_t* ibase = nullptr;
+    size_t plane_stride = 0, img_bytes = 0;
+    if (f.mode == TC_FIX_IMAGES) {
+        const int M = f.U * f.Vn;
+        const int comp = (int)(row / M), m = (int)(row - (int64_t)comp * M);
+        const int v = m / f.U, u = m - v * f.U;
+        const int uc = u / f.Uc, ul = u - uc * f.Uc, vc = v / f.Vc, vl = v - vc * f.Vc;
+        img_bytes = (size_t)f.N1 * f.K1p * 2;
+        const size_t per_plane = (size_t)f.nuc * f.nvc * 2 * img_bytes;
+        plane_stride = 3 * per_plane;                                            // consecutive z planes of one component
+        const int k = 2 * vl, ri = 2 * ul;                                       // MN-major image (scw_tc_synth.cu)
+        ibase = f.img + ((size_t)((int64_t)inst * p.Fz + (int64_t)nt * p.Fzt) * 3 + comp) * per_plane +
+                ((size_t)uc * f.nvc + vc) * 2 * img_bytes + (size_t)(k >> 3) * (f.N1 * 16) + (size_t)(ri >> 3) * 128 +
+                (k & 7) * 16 + (ri & 7) * 2;
+    }
+    float2* pbase = f.mode == TC_FIX_P ? f.P + (int64_t)inst * f.inst_stride + row + (int64_t)nt * p.Fzt * f.ldP : nullptr;
+    auto seg_base = [&](int c) -> const float* {
+        const int seg = (int)(tile - p.span0[c] / p.kblocks);
+        return p.part + ((size_t)c * p.S + seg) * tile_floats + 2 * r;
+    };
+    int c1 = c_first + 1;                                                        // second non-empty segment, if any
+    while (c1 <= c_last && p.span0[c1] == p.span0[c1 + 1]) ++c1;
+    const float* s0 = seg_base(c_first);
+    const float* s1 = c1 <= c_last ? seg_base(c1) : nullptr;
+    for (int n0 = pg; n0 < nv; n0 += E * groups) {
+        float2 acc[E], t[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int n = n0 + e * groups;
+            acc[e] = n < nv ? __ldcg(reinterpret_cast<const float2*>(s0 + (size_t)n * (2 * TA_ROWS))) : make_float2(0.f, 0.f);
+        }
+        if (s1) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const int n = n0 + e * groups;
+                t[e] = n < nv ? __ldcg(reinterpret_cast<const float2*>(s1 + (size_t)n * (2 * TA_ROWS))) : make_float2(0.f, 0.f);
+            }
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                acc[e].x += t[e].x;
+                acc[e].y += t[e].y;
+            }
+        }
+        for (int c = c1 + 1; c <= c_last; ++c) {                                 // third and later segments: one at a time
+            if (p.span0[c] == p.span0[c + 1]) continue;
+            const float* sc = seg_base(c);
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const int n = n0 + e * groups;
+                t[e] = n < nv ? __ldcg(reinterpret_cast<const float2*>(sc + (size_t)n * (2 * TA_ROWS))) : make_float2(0.f, 0.f);
+            }
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                acc[e].x += t[e].x;
+                acc[e].y += t[e].y;
+            }
+        }
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int n = n0 + e * groups;
+            if (n >= nv) continue;
+            if (f.mode == TC_FIX_P) {
+                pbase[(int64_t)n * f.ldP] = acc[e];
+            } else {
+                // rows (u,Re), (u,Im) are adjacent in the MN-major image: word (P_r, P_i) at k, word (-P_i, P_r) at k + 1;
+                // consecutive rows r of the tile (consecutive u) write consecutive words: full 32-byte sectors per warp
+                uint32_t H, L;
+                split_bf16x2(acc[e].x, acc[e].y, H, L);
+                uint8_t* dst = ibase + (size_t)n * plane_stride;
+                *reinterpret_cast<uint32_t*>(dst) = H;
+                *reinterpret_cast<uint32_t*>(dst + 16) = __byte_perm(H, 0, 0x1032) ^ 0x00008000u;
+                *reinterpret_cast<uint32_t*>(dst + img_bytes) = L;
+                *reinterpret_cast<uint32_t*>(dst + img_bytes + 16) = __byte_perm(L, 0, 0x1032) ^ 0x00008000u;
+            }
+        }
     }
 }
 
@@ -181,6 +405,9 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
     uint64_t* stg_full = acc_empty + 2;               // TMA -> converters           [stg_stages]
     uint64_t* stg_empty = stg_full + TA_MAX_STG;      // converters -> TMA producer  [stg_stages]
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(stg_empty + TA_MAX_STG);
+    volatile int* fix_flag = reinterpret_cast<volatile int*>(tmem_slot + 1);
+    volatile int* fin = fix_flag + 1;                   // [3] tile, c_first, c_last of a fix-up left to the whole CTA
+    volatile int* cta_slot = fin + 3;                   // the span this CTA claimed
 
     if (tid == 0) {
         for (int s = 0; s < TA_MMA_STAGES; ++s) {
@@ -197,6 +424,14 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
             mbar_init(&stg_empty[s], TA_CONV_WARPS);
         }
         mbar_fence_init();
+        fin[0] = -1;
+        uint32_t smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        int slot = -1;
+        if (smid < gridDim.x && atomicCAS(&p.ctl[TA_CTL_CLAIM + smid], 0, 1) == 0) slot = (int)smid;
+        for (int i = 0; slot < 0 && i < (int)gridDim.x; ++i)
+            if (atomicCAS(&p.ctl[TA_CTL_CLAIM + i], 0, 1) == 0) slot = i;
+        *cta_slot = slot;
     }
     if (warp == TA_MMA_WARP) tmem_alloc(tmem_slot, TA_TMEM_COLS);
     tc_fence_before();
@@ -204,9 +439,26 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
-    const int64_t T = (int64_t)p.n_inst * p.n_tiles * p.m_tiles * p.kblocks;
-    const int64_t it0 = (int64_t)blockIdx.x * T / gridDim.x;
-    const int64_t it1 = (int64_t)(blockIdx.x + 1) * T / gridDim.x;
+    // Which span this CTA works on: the one of its SM (spans are sized per SM by scw_calibrate; with one CTA per SM and a
+    // grid of #SM CTAs every SM id shows up once), claimed with a CAS so that the CTA -> span map is a bijection whatever
+    // the placement turns out to be (a taken or out-of-range id falls back to the first free span).
+    const int cta = *cta_slot;
+    const int64_t it0 = p.span0[cta], it1 = p.span0[cta + 1];
+    const unsigned long long t_start_all = ta_now();
+
+    // phase 0 on every warp but the V loader, whose TMA pipeline fills meanwhile (phase 0 is bound by instruction issue,
+    // not by its few loads, and the early V requests start the write-back of whatever dirty lines the L2 still holds)
+    if (warp != TA_V_LOADER) {
+        const int t0 = tid - (warp > TA_V_LOADER ? 32 : 0);
+        ta_phase0(p, (int64_t)blockIdx.x * TA_P0_THREADS + t0, (int64_t)gridDim.x * TA_P0_THREADS);
+        named_bar_sync(15, TA_P0_THREADS);
+        if (t0 == 0) {                                     // release: this CTA's share is visible to the bulk copies of all
+            __threadfence();
+            fence_proxy_async_global();
+            atomicAdd(&p.ctl[0], 1);
+            p.cta_ns[cta * 4 + 0] = ta_now() - t_start_all;
+        }
+    }
 
     if (warp < TA_CONV_WARPS * TA_CONV_GROUPS) {
         // ===== converters: staged fp32 -> bf16 hi/lo A operand in TMEM =====
@@ -284,6 +536,15 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
             uint32_t phase = 0;
             const uint32_t bytes = (uint32_t)w_stage_bytes;
             TaPos q = ta_pos(p, it0);
+            if (it0 < it1) {                               // acquire: the weight images of every CTA are in memory
+                uint32_t spins = 0;
+                while (ld_acquire_gpu(&p.ctl[0]) < (int)gridDim.x) {
+                    __nanosleep(64);
+                    if (++spins > (1u << 24)) __trap();    // a CTA of the grid never ran (not co-resident): error, not a hang
+                }
+                fence_proxy_async_global();
+                p.cta_ns[cta * 4 + 1] = ta_now() - t_start_all;
+            }
             for (int64_t it = it0; it < it1; ++it) {
                 mbar_wait(&empty[stage], phase ^ 1);
                 mbar_expect_tx(&full_b[stage], bytes);
@@ -353,14 +614,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
             if (q == 0) mbar_wait(&acc_full[buf], (buf ? use1 : use0) & 1);
             named_bar_sync(10, 128);
             tc_fence_after();
-            if (q == 0 && lane == 0) {
-                // segment table: the CTAs whose spans meet this tile are c_first..c_last, this one is number c - c_first
-                const int64_t a = tile * p.kblocks, b = a + p.kblocks;
-                const int c_first = (int)(((a + 1) * gridDim.x + T - 1) / T) - 1;
-                p.seg_slot[tile * p.max_segs + ((int)blockIdx.x - c_first)] = (int)blockIdx.x * p.S + seg;
-                if ((int)blockIdx.x == c_first) p.seg_count[tile] = (int)((b * gridDim.x + T - 1) / T) - c_first;
-            }
-            float* out = p.part + ((size_t)blockIdx.x * p.S + seg) * ((size_t)p.Fzt * 2 * TA_ROWS) + 32 * q + lane;
+            float* out = p.part + ((size_t)cta * p.S + seg) * ((size_t)p.Fzt * 2 * TA_ROWS) + 32 * q + lane;
 #pragma unroll 1
             for (int b = 0; b < 2; ++b) {
                 const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(buf * 2 * p.N2 + b * p.N2);
@@ -391,9 +645,32 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
             }
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(&acc_empty[buf]);
+            if (lane == 0) mbar_arrive(&acc_empty[buf]);           // the MMA warp may start the next tile
             if (buf) ++use1; else ++use0;
             if (p.nbuf == 2) buf ^= 1;
+            // arrival: the CTAs whose spans meet this tile are c_first..c_last; the one that stores its segment last
+            // sums the tile (its own segment included, from memory: fixed order) and writes it out
+            const int64_t ta = tile * p.kblocks;
+            const int c_first = ta_owner(p, ta, (int)gridDim.x), c_last = ta_owner(p, ta + p.kblocks - 1, (int)gridDim.x);
+            int nseg = 0;
+            for (int c = c_first; c <= c_last; ++c) nseg += p.span0[c] != p.span0[c + 1];
+            __threadfence();
+            named_bar_sync(10, 128);
+            if (q == 0 && lane == 0) {
+                const int old = atomicAdd(&p.ctl[TA_CTL_TILE + tile], 1);
+                *fix_flag = old == nseg - 1;
+                if (old == nseg - 1) p.ctl[TA_CTL_TILE + tile] = 0;          // left clean for the next launch
+            }
+            named_bar_sync(10, 128);
+            if (*fix_flag && p.fix.mode != TC_FIX_NONE) {
+                if (seg_end == it1) {                              // last segment of the span: the whole CTA sums it below
+                    if (q == 0 && lane == 0) { fin[0] = (int)tile; fin[1] = c_first; fin[2] = c_last; }
+                } else {
+                    __threadfence();
+                    ta_fixup<8>(p, tile, c_first, c_last, 32 * q + lane, 0, 1);
+                }
+            }
+            named_bar_sync(10, 128);                               // fix_flag is rewritten by the next segment
             ++seg;
             it = seg_end;
         }
@@ -401,41 +678,35 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
     tc_fence_before();
     __syncthreads();
     if (warp == TA_MMA_WARP) tmem_dealloc(tmem_base, TA_TMEM_COLS);
-}
-
-// Sum the segments of every tile in CTA order: P[mt*128 + r, nt*Fzt + n] = sum_seg part[seg][n][2r..2r+1].
-__global__ void k_tc_reduce(int64_t R, int64_t Fz, int Fzt, int n_tiles, int m_tiles, int max_segs,
-                            const int* __restrict__ seg_count, const int* __restrict__ seg_slot,
-                            const float* __restrict__ part, float2* __restrict__ P_all, int64_t ldP, int64_t inst_stride)
-{
-    const int tile = blockIdx.x;                                 // global tile id: (inst, n_tile, m_tile)
-    const int n = blockIdx.y * blockDim.y + threadIdx.y;
-    const int r = threadIdx.x;                                   // complex row in tile, 0..127
-    const int gnt = tile / m_tiles, mt = tile - gnt * m_tiles;
-    const int inst = gnt / n_tiles, nt = gnt - inst * n_tiles;
-    float2* __restrict__ P = P_all + (int64_t)inst * inst_stride;
-    const int64_t row = (int64_t)mt * TA_ROWS + r, col = (int64_t)nt * Fzt + n;
-    if (n >= Fzt || row >= R || col >= Fz) return;
-    const int count = seg_count[tile];
-    const int* __restrict__ slots = seg_slot + (size_t)tile * max_segs;
-    float2 acc = make_float2(0.f, 0.f);
-    for (int i = 0; i < count; ++i) {
-        const float2 v = *reinterpret_cast<const float2*>(part + (size_t)slots[i] * ((size_t)Fzt * 2 * TA_ROWS) +
-                                                          (size_t)n * (2 * TA_ROWS) + 2 * r);
-        acc.x += v.x;
-        acc.y += v.y;
+    if (tid == 0) p.cta_ns[cta * 4 + 2] = ta_now() - t_start_all;
+    // Most tiles are completed by the LAST segment of some CTA (the head of a tile is the tail of a span), i.e. at the
+    // very end of the kernel, where every other role of the CTA is idle: all 24 warps sum that tile (6 plane groups).
+    if (fin[0] >= 0) {
+        __threadfence();
+        ta_fixup<11>(p, fin[0], fin[1], fin[2], tid & 127, tid >> 7, TA_THREADS / 128);
     }
-    P[row + col * ldP] = acc;
+    __syncthreads();
+    if (tid == 0) {                                                // the last CTA out leaves the counters clean
+        p.cta_ns[cta * 4 + 3] = ta_now() - t_start_all;
+        const int old = atomicAdd(&p.ctl[1], 1);
+        if (old == (int)gridDim.x - 1) {
+            p.ctl[0] = 0;
+            p.ctl[1] = 0;
+            for (int i = 0; i < (int)gridDim.x; ++i) p.ctl[TA_CTL_CLAIM + i] = 0;
+        }
+    }
 }
 
 // ---- host side -------------------------------------------------------------------------------------
 struct TaPlan {
-    int Fzt, N2, n_tiles, m_tiles, kblocks, G, S, stg_stages, nbuf, max_segs;
+    int Fzt, N2, n_tiles, m_tiles, kblocks, G, S, stg_stages, nbuf;
     int64_t T;
-    size_t wt_bytes, part_bytes, seg_bytes, smem_bytes;      // wt_bytes: W~ images of ONE instance
+    int64_t span0[TA_MAX_CTAS + 1];
+    size_t wt_bytes, part_bytes, ctl_ints, smem_bytes;       // wt_bytes: W~ images of ONE instance
 };
 
-static TaPlan ta_plan(int64_t R, int64_t J, int64_t Fz, int n_inst, int sm_count)
+// Spans of the persistent CTAs: equal, or proportional to the per-CTA rates of scw_calibrate (ctx->split_w).
+static TaPlan ta_plan(const scw_ctx* ctx, int64_t R, int64_t J, int64_t Fz, int n_inst)
 {
     TaPlan pl;
     int64_t fzt = (Fz + 7) / 8 * 8;
@@ -447,24 +718,47 @@ static TaPlan ta_plan(int64_t R, int64_t J, int64_t Fz, int n_inst, int sm_count
     pl.m_tiles = (int)((R + TA_ROWS - 1) / TA_ROWS);
     pl.kblocks = (int)((J + TA_BK - 1) / TA_BK);
     pl.T = (int64_t)n_inst * pl.n_tiles * pl.m_tiles * pl.kblocks;
-    pl.G = (int)(pl.T < sm_count ? pl.T : sm_count);
+    int sms = ctx->sm_count < TA_MAX_CTAS ? ctx->sm_count : TA_MAX_CTAS;
+    pl.G = (int)(pl.T < sms ? pl.T : sms);
+    const bool weighted = (int)ctx->split_w.size() == pl.G && pl.T >= 8LL * pl.G;
+    double total = 0.0, run = 0.0;
+    if (weighted) for (double w : ctx->split_w) total += w;
+    pl.span0[0] = 0;
+    for (int c = 0; c < pl.G; ++c) {
+        int64_t e;
+        if (weighted) {
+            run += ctx->split_w[c];
+            e = (int64_t)((double)pl.T * (run / total) + 0.5);
+            if (e < pl.span0[c]) e = pl.span0[c];
+            if (e > pl.T) e = pl.T;
+        } else {
+            e = (int64_t)(c + 1) * pl.T / pl.G;
+        }
+        pl.span0[c + 1] = c + 1 == pl.G ? pl.T : e;
+    }
     pl.S = 1;
     for (int c = 0; c < pl.G; ++c) {
-        const int64_t s = (int64_t)c * pl.T / pl.G, e = (int64_t)(c + 1) * pl.T / pl.G;
+        const int64_t s = pl.span0[c], e = pl.span0[c + 1];
         if (e > s) {
             const int span = (int)((e - 1) / pl.kblocks - s / pl.kblocks) + 1;
             if (span > pl.S) pl.S = span;
         }
     }
+    // partial-tile slots per CTA: fixed by the shape alone, so that the scratch size does not depend on the calibration
+    // (scw_calibrate clips the weights so that no span exceeds twice the mean; otherwise the equal split is used)
+    const int s_max = (int)((2 * (pl.T / pl.G + 1)) / pl.kblocks + 2);
+    if (pl.S > s_max) {
+        for (int c = 0; c <= pl.G; ++c) pl.span0[c] = (int64_t)c * pl.T / pl.G;
+        pl.S = s_max;
+    }
+    pl.S = s_max;
     const int w_bytes = TA_MMA_STAGES * (pl.N2 * 128);
     pl.stg_stages = (TA_SMEM_LIMIT - 256 - w_bytes) / TA_STG_BYTES;
     if (pl.stg_stages > TA_MAX_STG) pl.stg_stages = TA_MAX_STG;
     pl.smem_bytes = (size_t)w_bytes + (size_t)pl.stg_stages * TA_STG_BYTES + 256;
     pl.wt_bytes = (size_t)pl.n_tiles * pl.kblocks * pl.N2 * 128;
     pl.part_bytes = align_up((size_t)pl.G * pl.S * pl.Fzt * 2 * TA_ROWS * sizeof(float));
-    // a CTA span holds at least T/G iterations, so at most (kblocks-1)/(T/G) + 2 spans meet one tile
-    pl.max_segs = (int)((pl.kblocks - 1) / (pl.T / pl.G) + 2);
-    pl.seg_bytes = align_up((size_t)n_inst * pl.n_tiles * pl.m_tiles * (1 + pl.max_segs) * sizeof(int));
+    pl.ctl_ints = TA_CTL_TILE + (size_t)n_inst * pl.n_tiles * pl.m_tiles;
     return pl;
 }
 
@@ -520,52 +814,61 @@ bool tc_assemble_supported(int dtype, int64_t R, int64_t J, int64_t Fz, const vo
 
 int tc_assemble_max_group() { return TA_MAX_INST; }
 
-size_t tc_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int n_inst, int sm_count)
+// scratch layout: control block | weight images | partial tiles
+static size_t ta_ctl_bytes(const TaPlan& pl) { return align_up(pl.ctl_ints * sizeof(int) + 8 + (size_t)TA_MAX_CTAS * 4 * 8); }
+
+size_t tc_assemble_scratch(const scw_ctx* ctx, int64_t R, int64_t J, int64_t Fz, int n_inst)
 {
-    const TaPlan pl = ta_plan(R, J, Fz, n_inst, sm_count);
-    return align_up(pl.wt_bytes * n_inst) + pl.part_bytes + pl.seg_bytes;
+    const TaPlan pl = ta_plan(ctx, R, J, Fz, n_inst);
+    return ta_ctl_bytes(pl) + align_up(pl.wt_bytes * n_inst) + pl.part_bytes;
 }
 
-// weights (a-1) + the stream-K assembly kernel (a-2) of a group; the partial tiles end up in `part`.
-static bool ta_run(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z, void* scratch,
-                   TaPlan& pl, float*& part, int*& seg_count, int*& seg_slot)
+void tc_assemble_ctl(const scw_ctx* ctx, int64_t R, int64_t J, int64_t Fz, int n_inst, void* scratch, int** ctl, size_t* n_ints)
+{
+    const TaPlan pl = ta_plan(ctx, R, J, Fz, n_inst);
+    *ctl = static_cast<int*>(scratch);
+    *n_ints = pl.ctl_ints;
+}
+
+// weights (a-1) + stream-K assembly (a-2) + fix-up of a group of n_inst <= TA_MAX_INST instances with equal U, Vn, J, Fz:
+// ONE launch.  ctl_clean: the control block is known to hold zeros (a kernel launched before in this call zeroed it, or
+// the previous launch left it clean); otherwise it is cleared with a memset node first.
+void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
+                              const TcFixup& fix, int* sched, int n_sched, void* scratch, bool ctl_clean)
 {
     const scw_layer& L0 = inst[0];
     const int64_t R = 3LL * L0.U * L0.Vn;
-    pl = ta_plan(R, L0.J, Fz, n_inst, ctx->sm_count);
-    uint8_t* Wt = static_cast<uint8_t*>(scratch);
-    part = reinterpret_cast<float*>(Wt + align_up(pl.wt_bytes * n_inst));
-    seg_count = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(part) + pl.part_bytes);
-    seg_slot = seg_count + (size_t)n_inst * pl.n_tiles * pl.m_tiles;
-    TwGroup g;
-    static thread_local TaParams p;                 // 17 KB of kernel parameters: kept off the stack
+    const TaPlan pl = ta_plan(ctx, R, L0.J, Fz, n_inst);
+    int* ctl = static_cast<int*>(scratch);
+    uint8_t* Wt = static_cast<uint8_t*>(scratch) + ta_ctl_bytes(pl);
+    float* part = reinterpret_cast<float*>(Wt + align_up(pl.wt_bytes * n_inst));
+    static thread_local TaParams p;                 // ~22 KB of kernel parameters: kept off the stack
     bool maps_ok = true;
     for (int i = 0; i < n_inst; ++i) {
-        g.c[i] = (const float2*)inst[i].c;
-        g.gamma[i] = (const double2*)inst[i].gamma;
-        g.dir[i] = inst[i].dir;
-        g.z[i] = z[i];
-        g.inv_lambda[i] = 1.0 / inst[i].lambda;
-        g.z_lo[i] = inst[i].z_lo;
-        g.z_hi[i] = inst[i].z_hi;
+        p.c[i] = (const float2*)inst[i].c;
+        p.gamma[i] = (const double2*)inst[i].gamma;
+        p.dir[i] = inst[i].dir;
+        p.z[i] = z[i];
+        p.inv_lambda[i] = 1.0 / inst[i].lambda;
+        p.z_lo[i] = inst[i].z_lo;
+        p.z_hi[i] = inst[i].z_hi;
         maps_ok = maps_ok && ta_make_map(&p.tmap[i][0], inst[i].V, inst[i].ldV, R, L0.J, 0, nullptr) &&
                   ta_make_map(&p.tmap[i][1], inst[i].V, inst[i].ldV, R, L0.J, 1, &p.xoff1[i]);
     }
     if (!maps_ok) {                                 // reported by the entry point's check_launch
         ctx->tc_error = true;
-        return false;
+        return;
     }
-    {
-        KernelScope ks(ctx, KC_WEIGHTS);
-        const dim3 grid((unsigned)pl.kblocks, (unsigned)pl.n_tiles, (unsigned)n_inst);
-        k_tc_weights<<<grid, 256, 0, ctx->stream>>>(n_inst, L0.J, Fz, pl.Fzt, pl.n_tiles, pl.kblocks, g, Wt);
-    }
+    for (int c = 0; c <= pl.G; ++c) p.span0[c] = pl.span0[c];
     p.n_inst = n_inst;
+    p.J = L0.J;
+    p.Fz = Fz;
     p.Wt = Wt;
     p.part = part;
-    p.seg_count = seg_count;
-    p.seg_slot = seg_slot;
-    p.max_segs = pl.max_segs;
+    p.ctl = ctl;
+    p.cta_ns = reinterpret_cast<unsigned long long*>(reinterpret_cast<uint8_t*>(ctl) + align_up(pl.ctl_ints * sizeof(int), 8));
+    p.sched = sched;
+    p.n_sched = sched ? n_sched : 0;
     p.N2 = pl.N2;
     p.Fzt = pl.Fzt;
     p.n_tiles = pl.n_tiles;
@@ -574,54 +877,31 @@ static bool ta_run(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, 
     p.S = pl.S;
     p.stg_stages = pl.stg_stages;
     p.nbuf = pl.nbuf;
-    {
-        KernelScope ks(ctx, KC_ASSEMBLE_TC);
-        cudaFuncSetAttribute(k_tc_assemble, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes);
-        k_tc_assemble<<<pl.G, TA_THREADS, pl.smem_bytes, ctx->stream>>>(p);
-    }
-    return true;
-}
-
-void launch_tc_assemble_group_partials(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
-                                       void* scratch, TcPartials* out)
-{
-    TaPlan pl;
-    float* part = nullptr;
-    int *seg_count = nullptr, *seg_slot = nullptr;
-    out->part = nullptr;
-    if (!ta_run(ctx, n_inst, inst, Fz, z, scratch, pl, part, seg_count, seg_slot)) return;
-    out->part = part;
-    out->seg_count = seg_count;
-    out->seg_slot = seg_slot;
-    out->max_segs = pl.max_segs;
-    out->Fzt = pl.Fzt;
-    out->n_tiles = pl.n_tiles;
-    out->m_tiles = pl.m_tiles;
-    out->rows_per_tile = TA_ROWS;
-}
-
-// A group of n_inst <= TA_MAX_INST instances with the same U, Vn, J and Fz in three launches:
-// weights (a-1), P = V W over the concatenated iteration space (a-2), segment reduce.
-// Instance i writes P_all + i * inst_stride (column-major [ldP x Fz]).
-void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
-                              void* P_all, int64_t ldP, int64_t inst_stride, void* scratch)
-{
-    TaPlan pl;
-    float* part = nullptr;
-    int *seg_count = nullptr, *seg_slot = nullptr;
-    if (!ta_run(ctx, n_inst, inst, Fz, z, scratch, pl, part, seg_count, seg_slot)) return;
-    const int64_t R = 3LL * inst[0].U * inst[0].Vn;
-    KernelScope ks(ctx, KC_REDUCE);
-    dim3 block(TA_ROWS, 2);
-    dim3 grid((unsigned)(n_inst * pl.n_tiles * pl.m_tiles), (unsigned)((pl.Fzt + 1) / 2));
-    k_tc_reduce<<<grid, block, 0, ctx->stream>>>(R, Fz, pl.Fzt, pl.n_tiles, pl.m_tiles, pl.max_segs, seg_count, seg_slot,
-                                                 part, (float2*)P_all, ldP, inst_stride);
+    p.fix = fix;
+    p.fix.R = R;
+    // control block: zero at launch.  Zeroed by the caller's previous kernel (ctl_clean), left clean by the previous
+    // assembly launch over the same scratch (trusted only while SCW_OPT_CACHE promises an untouched workspace), else memset
+    const bool clean = ctl_clean || (ctx->cache_on && ctx->clean_ctl == ctl && ctx->clean_ints >= pl.ctl_ints);
+    if (!clean) cudaMemsetAsync(ctl, 0, pl.ctl_ints * sizeof(int), ctx->stream);
+    ctx->clean_ctl = ctl;
+    ctx->clean_ints = pl.ctl_ints;
+    KernelScope ks(ctx, KC_ASSEMBLE_TC);
+    cudaFuncSetAttribute(k_tc_assemble, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes);
+    k_tc_assemble<<<pl.G, TA_THREADS, pl.smem_bytes, ctx->stream>>>(p);
+    ctx->last_asm_G = pl.G;
+    ctx->last_asm_ns = p.cta_ns;
+    for (int c = 0; c <= pl.G; ++c) ctx->last_asm_span0[c] = pl.span0[c];
 }
 
 void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z, void* P, int64_t ldP,
                         void* scratch)
 {
-    launch_tc_assemble_group(ctx, 1, L, Fz, &z, P, ldP, 0, scratch);
+    TcFixup fix = {};
+    fix.mode = TC_FIX_P;
+    fix.P = static_cast<float2*>(P);
+    fix.ldP = ldP;
+    fix.inst_stride = 0;
+    launch_tc_assemble_group(ctx, 1, L, Fz, &z, fix, nullptr, 0, scratch, false);
 }
 
 }  // namespace scw

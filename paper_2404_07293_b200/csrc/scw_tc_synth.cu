@@ -39,7 +39,7 @@ constexpr int TS_MAX_INST = 64;            // instances per grouped launch
 struct TsParams {
     const uint8_t* A1;     // [ty][vc][hi|lo] images of (Fy_r, Fy_i): 128 rows x K1p, K-major, LBO = 2048, SBO = 128
     const uint32_t* A2;    // [tx][uc][row][hi K2p/2 | lo K2p/2] packed bf16 pairs (cos, sin) of Fx: TMEM A-operand rows
-    const uint8_t* B1;     // [plane][uc][vc][hi|lo] images: N1 rows x K1p, LBO = N1*16, SBO = 128
+    const uint8_t* B1;     // [plane][uc][vc][hi|lo] images: N1 rows x K1p, MN-major, LBO (k blocks) = N1*16, SBO (row blocks) = 128
     float2* E[TS_MAX_INST];   // output of every instance of the group
     int64_t s_comp, s_z, s_y, s_x;
     int64_t Nx, Ny;
@@ -74,8 +74,10 @@ __host__ __device__ inline TsChunks ts_chunks(int nfreq)
 // row = [hi: Kp/2 words | lo: Kp/2 words], word f = bf16 pair (cos, sin).
 struct TwAxis { int nfreq, nch, len, Kp, tiles; int64_t N; const double* coord; double inv_period; void* out; };
 
-__global__ void k_tc_synth_twiddles(const TwAxis ay, const TwAxis ax, int blocks_y)
+__global__ void k_tc_synth_twiddles(const TwAxis ay, const TwAxis ax, int blocks_y, int* __restrict__ zero, size_t n_zero)
 {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_zero; i += (size_t)gridDim.x * blockDim.x)
+        zero[i] = 0;                                                          // control block of the assembly that follows
     const bool is_y = (int)blockIdx.x < blocks_y;                            // one launch covers both axes
     const TwAxis& a = is_y ? ay : ax;
     const int64_t idx = (int64_t)(blockIdx.x - (is_y ? 0 : blocks_y)) * blockDim.x + threadIdx.x;   // (tile, chunk, r, f)
@@ -110,111 +112,48 @@ __global__ void k_tc_synth_twiddles(const TwAxis ay, const TwAxis ax, int blocks
     }
 }
 
-// Spectrum images: image (plane, uc, vc), plane = n*3 + comp, row = 2ul + c, k = 2vl + c'' with u = uc*Uc + ul,
-// v = vc*Vc + vl:   row (u,Re): (P_r, -P_i);  row (u,Im): (P_i, P_r)
-// so that  D1[y, (u,c)] = sum_v Fy[y,v] P[u,v]  in real arithmetic.
+// Spectrum images (GEMM1's B operand): image (plane, uc, vc), plane = n*3 + comp, row n' = 2ul + c, k = 2vl + c'' with
+// u = uc*Uc + ul, v = vc*Vc + vl:   row (u,Re): (P_r, -P_i) over (k, k+1);  row (u,Im): (P_i, P_r)
+// so that  D1[y, (u,c)] = sum_v Fy[y,v] P[u,v]  in real arithmetic.  The image is MN-MAJOR (no swizzle): element (n', k) at
+//   (k/8)*(N1*16) + (n'/8)*128 + (k%8)*16 + (n'%8)*2      [core matrix = 8 k-rows of 16 bytes, 8 rows n' contiguous]
+// so that consecutive u -- consecutive rows of P, which is what one thread block of the producer holds -- are contiguous
+// in memory: the word at k = 2vl is the bf16 pair (P_r, P_i), the word at k + 1 (16 bytes on) is (-P_i, P_r).
+__device__ __forceinline__ void ts_image_store(uint8_t* img_hi, size_t img_bytes, int N1, int ul, int vl, float pr, float pi)
+{
+    uint32_t H, L;
+    split_bf16x2(pr, pi, H, L);
+    const int k = 2 * vl, n = 2 * ul;
+    uint8_t* dst = img_hi + (size_t)(k >> 3) * (N1 * 16) + (size_t)(n >> 3) * 128 + (k & 7) * 16 + (n & 7) * 2;
+    *reinterpret_cast<uint32_t*>(dst) = H;
+    *reinterpret_cast<uint32_t*>(dst + 16) = __byte_perm(H, 0, 0x1032) ^ 0x00008000u;       // (-P_i, P_r)
+    *reinterpret_cast<uint32_t*>(dst + img_bytes) = L;
+    *reinterpret_cast<uint32_t*>(dst + img_bytes + 16) = __byte_perm(L, 0, 0x1032) ^ 0x00008000u;
+}
+
 __global__ void k_tc_synth_pimage(int U, int Vn, int Uc, int Vc, int nuc, int nvc, int K1p, int N1, int planes,
                                   const float2* __restrict__ P, int64_t ldP, uint8_t* __restrict__ img,
                                   int* __restrict__ sched, int n_sched)
 {
-    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;      // (image, row, kpair)
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;      // (image, vl, ul), ul fastest
     for (int64_t i = idx; i < n_sched; i += (int64_t)gridDim.x * blockDim.x) sched[i] = 0;   // plane counters of the synthesis that follows
-    const int kpairs = K1p / 2;
-    if (idx >= (int64_t)planes * nuc * nvc * N1 * kpairs) return;
-    const int vl = (int)(idx % kpairs);
-    const int64_t pr = idx / kpairs;
-    const int row = (int)(pr % N1);
-    const int64_t image = pr / N1;
+    const int half_n = N1 / 2, kpairs = K1p / 2;
+    if (idx >= (int64_t)planes * nuc * nvc * half_n * kpairs) return;
+    const int ul = (int)(idx % half_n);
+    const int64_t pr = idx / half_n;
+    const int vl = (int)(pr % kpairs);
+    const int64_t image = pr / kpairs;
     const int vc = (int)(image % nvc);
     const int uc = (int)((image / nvc) % nuc);
     const int64_t plane = image / (nvc * nuc);
-    const int ul = row >> 1, c = row & 1;
     const int u = uc * Uc + ul, v = vc * Vc + vl;
-    float a = 0.f, b = 0.f;
+    float2 p = make_float2(0.f, 0.f);                                         // padding entries are written as zeros
     if (ul < Uc && vl < Vc && u < U && v < Vn) {
         const int64_t n = plane / 3;
         const int comp = (int)(plane - n * 3);
-        const float2 p = P[n * ldP + (int64_t)comp * U * Vn + (int64_t)v * U + u];
-        a = c ? p.y : p.x;
-        b = c ? p.x : -p.y;
+        p = P[n * ldP + (int64_t)comp * U * Vn + (int64_t)v * U + u];
     }
-    uint32_t hi, lo;
-    split_bf16x2(a, b, hi, lo);
-    const int k = 2 * vl;
     const size_t img_bytes = (size_t)N1 * K1p * 2;
-    uint8_t* base = img + (size_t)image * 2 * img_bytes;
-    const size_t off = (size_t)(k >> 3) * (N1 * 16) + (size_t)(row >> 3) * 128 + (row & 7) * 16 + (k & 7) * 2;
-    *reinterpret_cast<uint32_t*>(base + off) = hi;
-    *reinterpret_cast<uint32_t*>(base + img_bytes + off) = lo;
-}
-
-// Spectrum images straight from the stream-K partial tiles of the assembly (TcPartials): thread = (image (plane, uc,
-// vc), 8-wide k chunk kc, local frequency ul) sums the segments of its four spectrum entries P[u, v0..v0+3] in the
-// table's fixed order (deterministic) and writes the 16-byte chunks of image rows (ul,Re) and (ul,Im), hi and lo --
-// P itself never goes to memory.  Lanes run along u: loads of one v are contiguous, a warp's stores cover 1 KB.
-constexpr int TS_PI_THREADS = 128;
-
-__global__ void __launch_bounds__(TS_PI_THREADS) k_tc_synth_pimage_partials(int U, int Vn, int Uc, int Vc, int nuc, int nvc,
-                                                                            int K1p, int N1, int Fz,
-                                                                            const __grid_constant__ TcPartials tp,
-                                                                            uint8_t* __restrict__ img,
-                                                                            int* __restrict__ sched, int n_sched)
-{
-    if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0)              // plane counters of the synthesis that follows
-        for (int i = threadIdx.x; i < n_sched; i += TS_PI_THREADS) sched[i] = 0;
-    // grid: x = (instance, z plane), y = item chunk, z = (u chunk, v chunk, component): few divisions, all but one uniform
-    constexpr int rpt = 128;                                      // rows per assembly tile (checked on the host)
-    const int pz = blockIdx.x;                                    // inst*Fz + n
-    const int item = blockIdx.y * TS_PI_THREADS + threadIdx.x;    // kc * (N1/2) + ul
-    const int half = N1 / 2, kchunks = K1p / 8;
-    if (item >= kchunks * half) return;
-    const int kc = item / half, ul = item - kc * half;
-    const int comp = blockIdx.z % 3, cc = blockIdx.z / 3;
-    const int vc = cc % nvc, uc = cc / nvc;
-    const int plane = pz * 3 + comp;
-    const int image = (plane * nuc + uc) * nvc + vc;
-    const int u = uc * Uc + ul;
-    const int M = U * Vn;
-    const int inst = pz / Fz, n = pz - inst * Fz;
-    const int nt = n / tp.Fzt, nn = n - nt * tp.Fzt;
-    const int tile_base = (inst * tp.n_tiles + nt) * tp.m_tiles;
-    const size_t tile_floats = (size_t)tp.Fzt * 2 * rpt;
-    float2 pv[4];
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-        const int vl = 4 * kc + e, v = vc * Vc + vl;
-        pv[e] = make_float2(0.f, 0.f);
-        if (ul < Uc && vl < Vc && u < U && v < Vn) {
-            const int row = comp * M + v * U + u;
-            const int mt = row / rpt, r = row % rpt;
-            const int tile = tile_base + mt;
-            const int cnt = tp.seg_count[tile];
-            const int* __restrict__ slots = tp.seg_slot + (size_t)tile * tp.max_segs;
-            const float* __restrict__ src = tp.part + (size_t)nn * (2 * rpt) + 2 * r;
-            for (int i = 0; i < cnt; ++i) {
-                const float2 t = *reinterpret_cast<const float2*>(src + (size_t)slots[i] * tile_floats);
-                pv[e].x += t.x;
-                pv[e].y += t.y;
-            }
-        }
-    }
-    // row (u,Re): (P_r, -P_i) per v;  row (u,Im): (P_i, P_r): one split per entry, the two rows by sign flip / half swap
-    uint32_t H[4], Lw[4];
-#pragma unroll
-    for (int e = 0; e < 4; ++e) split_bf16x2(pv[e].x, pv[e].y, H[e], Lw[e]);
-    const uint4 re_hi = make_uint4(H[0] ^ 0x80000000u, H[1] ^ 0x80000000u, H[2] ^ 0x80000000u, H[3] ^ 0x80000000u);
-    const uint4 re_lo = make_uint4(Lw[0] ^ 0x80000000u, Lw[1] ^ 0x80000000u, Lw[2] ^ 0x80000000u, Lw[3] ^ 0x80000000u);
-    const uint4 im_hi = make_uint4(__byte_perm(H[0], 0, 0x1032), __byte_perm(H[1], 0, 0x1032), __byte_perm(H[2], 0, 0x1032),
-                                   __byte_perm(H[3], 0, 0x1032));
-    const uint4 im_lo = make_uint4(__byte_perm(Lw[0], 0, 0x1032), __byte_perm(Lw[1], 0, 0x1032), __byte_perm(Lw[2], 0, 0x1032),
-                                   __byte_perm(Lw[3], 0, 0x1032));
-    const size_t img_bytes = (size_t)N1 * K1p * 2;
-    const int row = 2 * ul;                                       // rows 2ul and 2ul+1 sit in the same 8-row core matrix
-    uint8_t* dst = img + (size_t)image * 2 * img_bytes + (size_t)kc * (N1 * 16) + (size_t)(row >> 3) * 128 + (row & 7) * 16;
-    *reinterpret_cast<uint4*>(dst) = re_hi;
-    *reinterpret_cast<uint4*>(dst + 16) = im_hi;
-    *reinterpret_cast<uint4*>(dst + img_bytes) = re_lo;
-    *reinterpret_cast<uint4*>(dst + img_bytes + 16) = im_lo;
+    ts_image_store(img + (size_t)image * 2 * img_bytes, img_bytes, N1, ul, vl, p.x, p.y);
 }
 
 // ---- main kernel ------------------------------------------------------------------------------------
@@ -361,7 +300,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
     } else if (warp == 1) {
         // ===== MMA issuer: the whole warp runs the loop (warp-uniform control flow), one elected lane issues =====
         if (sched_get(0) >= 0) {
-            const uint32_t idesc1 = umma_idesc_bf16(TS_TILE, N1);
+            const uint32_t idesc1 = umma_idesc_bf16(TS_TILE, N1, false, true);    // B1 (spectrum images) is MN-major
             const uint32_t idesc2 = umma_idesc_bf16(TS_TILE, TS_TILE);
             const uint32_t a1 = smem_u32(sA1), b1 = smem_u32(sB1), b2 = smem_u32(sB2);
             const uint32_t d1 = tmem_base + TS_D1_COL;
@@ -591,7 +530,7 @@ size_t tc_synth_twiddle_bytes(int U, int Vn, int64_t Nx, int64_t Ny)
 size_t tc_synth_scratch(int U, int Vn, int64_t Fz) { return ts_plan(U, Vn, Fz, 1, 1).b1_bytes; }
 
 void launch_tc_synth_twiddles(scw_ctx* ctx, int U, int Vn, double X, double Y, int64_t Nx, const double* x, int64_t Ny,
-                              const double* y, void* tw)
+                              const double* y, void* tw, int* zero, size_t n_zero)
 {
     const TsPlan pl = ts_plan(U, Vn, 1, Nx, Ny);
     uint8_t* A1 = static_cast<uint8_t*>(tw);
@@ -602,7 +541,7 @@ void launch_tc_synth_twiddles(scw_ctx* ctx, int U, int Vn, double X, double Y, i
     const int64_t nx = (int64_t)pl.tiles_x * pl.cu.n * TS_TILE * (pl.K2p / 2);
     const int by = (int)((ny + 255) / 256), bx = (int)((nx + 255) / 256);
     KernelScope ks(ctx, KC_TWIDDLES);
-    k_tc_synth_twiddles<<<by + bx, 256, 0, ctx->stream>>>(ay, ax, by);
+    k_tc_synth_twiddles<<<by + bx, 256, 0, ctx->stream>>>(ay, ax, by, zero, zero ? n_zero : 0);
 }
 
 
@@ -670,7 +609,7 @@ void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, 
     uint8_t* B1 = static_cast<uint8_t*>(scratch);
     {
         KernelScope ks(ctx, KC_SYNTH_IMG);
-        const int64_t n = (int64_t)planes * pl.cu.n * pl.cv.n * pl.K2p * (pl.K1p / 2);
+        const int64_t n = (int64_t)planes * pl.cu.n * pl.cv.n * (pl.K2p / 2) * (pl.K1p / 2);
         k_tc_synth_pimage<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(U, Vn, pl.cu.len, pl.cv.len, pl.cu.n, pl.cv.n,
                                                                                 pl.K1p, pl.K2p, planes, (const float2*)P_all,
                                                                                 ldP, B1, ts_sched(pl, tw),
@@ -679,28 +618,29 @@ void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, 
     ts_launch_main(ctx, pl, Fz, n_inst, B1, Nx, Ny, tw, E, strides, intensity);
 }
 
-bool tc_synth_partials_supported(int U, int Vn, const TcPartials& parts)
+void tc_synth_image_plan(int U, int Vn, int64_t Nx, int64_t Ny, void* scratch, const void* tw, TcFixup* fix, int** sched,
+                         int* n_sched)
 {
-    return parts.part && parts.rows_per_tile == 128 && (int64_t)U * Vn * 3 < (1 << 30);
+    const TsPlan pl = ts_plan(U, Vn, 1, Nx, Ny);
+    fix->mode = TC_FIX_IMAGES;
+    fix->img = static_cast<uint8_t*>(scratch);
+    fix->U = U;
+    fix->Vn = Vn;
+    fix->Uc = pl.cu.len;
+    fix->Vc = pl.cv.len;
+    fix->nuc = pl.cu.n;
+    fix->nvc = pl.cv.n;
+    fix->K1p = pl.K1p;
+    fix->N1 = pl.K2p;
+    *sched = ts_sched(pl, tw);
+    *n_sched = pl.tiles_x * pl.tiles_y;
 }
 
-void launch_tc_synth_group_partials(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const TcPartials& parts,
-                                    int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
-                                    void* scratch, bool intensity)
+void launch_tc_synth_group_images(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, int64_t Nx, int64_t Ny,
+                                  const void* tw, void* const* E, const int64_t strides[4], void* scratch, bool intensity)
 {
     const TsPlan pl = ts_plan(U, Vn, Fz * n_inst, Nx, Ny);
-    const int planes = (int)(Fz * 3 * n_inst);
-    uint8_t* B1 = static_cast<uint8_t*>(scratch);
-    {
-        KernelScope ks(ctx, KC_SYNTH_IMG);
-        const int items = (pl.K1p / 8) * (pl.K2p / 2);
-        const dim3 grid((unsigned)(planes / 3), (unsigned)((items + TS_PI_THREADS - 1) / TS_PI_THREADS),
-                        (unsigned)(pl.cu.n * pl.cv.n * 3));
-        k_tc_synth_pimage_partials<<<grid, TS_PI_THREADS, 0, ctx->stream>>>(U, Vn, pl.cu.len, pl.cv.len, pl.cu.n, pl.cv.n,
-                                                                            pl.K1p, pl.K2p, (int)Fz, parts, B1,
-                                                                            ts_sched(pl, tw), pl.tiles_x * pl.tiles_y);
-    }
-    ts_launch_main(ctx, pl, Fz, n_inst, B1, Nx, Ny, tw, E, strides, intensity);
+    ts_launch_main(ctx, pl, Fz, n_inst, static_cast<const uint8_t*>(scratch), Nx, Ny, tw, E, strides, intensity);
 }
 
 void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,
