@@ -393,6 +393,13 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
         kI["tc_synth"]["binding"] = "tensor"
     extra["config4_sweep_intensity"] = dict(ms_per_call=ms_i, samples_per_s=n4 / (ms_i * 1e-3), kernels=kI,
                                             speedup_vs_complex_field=ms / ms_i)
+    # window sums only: the detector reading S(lambda, z) of a 192 x 192 window, no per-sample output at all
+    win = (32, 224, 32, 224)
+    outS = [torch.empty((c4.planes,), dtype=torch.float32, device=device) for _ in Ls]
+    detw = lambda: scw.scw_sweep_detector(ctx, Ls, zs, dx, dy, window=win, want_I=False, out_S=outS)
+    ms_w = time_steps(torch, detw, args.steps, args.warmup)
+    extra["config4_sweep_window_sums"] = dict(ms_per_call=ms_w, samples_per_s=n4 / (ms_w * 1e-3), window=win,
+                                              speedup_vs_complex_field=ms / ms_w)
     del Ls, zs, out, outI
     torch.cuda.empty_cache()
     # NEXT-1 exterior field (eq. 9-10): the paper's Table 2 shape (M = 2500 orders, one 256 x 256 plane below the

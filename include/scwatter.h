@@ -265,20 +265,43 @@ int32_t scw_exterior_spectra(scw_ctx* ctx, const scw_exterior* ext, int64_t Fz, 
 int32_t scw_exterior_points(scw_ctx* ctx, const scw_exterior* ext, int64_t N, const double* r, void* E);
 int32_t scw_exterior_points_workspace(scw_ctx* ctx, const scw_exterior* ext, int64_t N, size_t* bytes);
 
-/* ---------------------------------------------------------------- detector intensity
+/* ---------------------------------------------------------------- detector reductions
  *
- * scw_sweep_wavelengths followed by the detector reduction I(x, y, z) = sum_comp |E_comp(x, y, z)|^2 (the light intensity
- * the paper collects on a plane; reading c-18), with the complex field never written:
- * on the tensor-core path the reduction runs in the synthesis epilogue (4 bytes per sample leave the SM instead of 24).
+ * scw_sweep_wavelengths followed by what a detector records instead of the complex field (PAPER.md:422, 520-524, 544-546,
+ * 554; reading c-18), with the field never written: on the tensor-core path the reductions run in the synthesis
+ * epilogue.
+ *   I(x, y, z)  = sum_comp |E_comp(x, y, z)|^2                    intensity per sample (4 bytes leave the SM instead of 24)
+ *   S(z)        = sum_{(i, k) in window} I(x_i, y_k, z)           intensity collected by a detector window of the plane
+ *                                                                  (plain sum over grid samples; multiply by dx dy for an area integral)
+ *   A           = -log10(S / S_0)                                  absorbance against a reference sweep (scw_absorbance)
  * I: HOST array of device pointers, real (float for SCW_C64, double for SCW_C128), element (n, k, i) at
- * n*strides[0] + k*strides[1] + i*strides[2] elements; strides == NULL means [Fz][Ny][Nx], x fastest.
+ * n*strides[0] + k*strides[1] + i*strides[2] elements; strides == NULL means [Fz][Ny][Nx], x fastest.  I == NULL: no per-
+ * sample output.  S: HOST array of device pointers, real [Fz[i]] per instance; S == NULL: no window sums.  At least one of
+ * I, S.  window: HOST, grid-index box [ix0, ix1) x [iy0, iy1) of the (x, y) grid; NULL = the whole plane.
+ * Errors: those of scw_sweep_wavelengths; SHAPE for an empty window or one outside the grid.
  */
+typedef struct { int64_t ix0, ix1, iy0, iy1; } scw_window;
+int32_t scw_sweep_detector(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst,
+                           const int64_t* Fz, const double* const* z,
+                           int64_t Nx, const double* x, int64_t Ny, const double* y,
+                           void* const* I, const int64_t* strides, const scw_window* window, void* const* S);
+int32_t scw_sweep_detector_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz,
+                                     int64_t Nx, int64_t Ny, size_t* bytes);
+/* scw_sweep_detector with I only (whole plane, no window sums). */
 int32_t scw_sweep_intensity(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst,
                             const int64_t* Fz, const double* const* z,
                             int64_t Nx, const double* x, int64_t Ny, const double* y,
                             void* const* I, const int64_t* strides);
 int32_t scw_sweep_intensity_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz,
                                       int64_t Nx, int64_t Ny, size_t* bytes);
+/*
+ * Absorbance spectrum (Fig. 6): A[i] = -log10(S[i] / S0[i]) for n detector readings S (e.g. one per
+ * wavelength of a sweep) against the readings S0 of a reference sweep, and / or the absorbance of the whole band,
+ * band[0] = -log10( sum_i w_i S_i / sum_i w_i S0_i ) with spectral weights w (NULL = ones).  dtype SCW_C64: float arrays,
+ * SCW_C128: double.  All device pointers; A or band may be NULL (not both).  Errors: NULL, DTYPE, SHAPE, ALIGN, CUDA.
+ */
+int32_t scw_absorbance(scw_ctx* ctx, int32_t dtype, int64_t n, const void* S, const void* S0, const void* w, void* A,
+                       void* band);
 
 /* ---------------------------------------------------------------- roofline denominators (measurement helper)
  *

@@ -253,3 +253,25 @@ def intensity(E):
     collected on a plane; reading c-18)."""
     E = np.asarray(E)
     return (E.real ** 2 + E.imag ** 2).sum(axis=-3)
+
+
+def window_sum(I, window=None):
+    """Detector window: S = sum of the intensity over the grid samples ix0 <= i < ix1, iy0 <= k < iy1 of every plane
+    (plain sum over samples; "we detect the intensity of the transmission waves", 554).  I [..., Ny, Nx]."""
+    I = np.asarray(I, dtype=np.float64)
+    if window is None:
+        return I.sum(axis=(-2, -1))
+    ix0, ix1, iy0, iy1 = window
+    return I[..., iy0:iy1, ix0:ix1].sum(axis=(-2, -1))
+
+
+def absorbance(S, S0):
+    """A = -log10(S / S0): absorbance of a detector reading against a reference reading (Fig. 6)."""
+    return -np.log10(np.asarray(S, dtype=np.float64) / np.asarray(S0, dtype=np.float64))
+
+
+def band_absorbance(S, S0, w=None):
+    """Absorbance of a whole band: -log10(sum_i w_i S_i / sum_i w_i S0_i), spectral weights w (None = ones)."""
+    S, S0 = np.asarray(S, dtype=np.float64), np.asarray(S0, dtype=np.float64)
+    w = np.ones_like(S) if w is None else np.asarray(w, dtype=np.float64)
+    return float(-np.log10((w * S).sum() / (w * S0).sum()))

@@ -31,6 +31,7 @@ EXPORTS = [
     "scw_exterior_spectra", "scw_exterior_points", "scw_exterior_points_workspace",
     "scw_sweep_intensity", "scw_sweep_intensity_workspace",
     "scw_measure_peak", "scw_invalidate_cache", "scw_calibrate", "scw_profile_assembly",
+    "scw_sweep_detector", "scw_sweep_detector_workspace", "scw_absorbance",
 ]
 SCW_PEAKS = {"fp64_dmma_tflops": 0, "fp32_fma_tflops": 1, "mufu_gops": 2, "hbm_read_gbs": 3, "hbm_write_gbs": 4,
              "hbm_write_tma_gbs": 5}
@@ -41,6 +42,10 @@ class scw_exterior(Structure):
     _fields_ = [("struct_size", c_uint32), ("dtype", c_int32), ("side", c_int32), ("U", c_int32), ("Vn", c_int32),
                 ("X", c_double), ("Y", c_double), ("lambda_", c_double), ("n_re", c_double), ("n_im", c_double),
                 ("z_face", c_double), ("z_inc", c_double), ("p_face", c_void_p), ("p_inc", c_void_p)]
+
+
+class scw_window(Structure):
+    _fields_ = [("ix0", c_int64), ("ix1", c_int64), ("iy0", c_int64), ("iy1", c_int64)]
 
 
 class ScwError(RuntimeError):
@@ -113,6 +118,9 @@ def lib():
         L.scw_exterior_spectra.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, c_void_p, c_void_p, c_int64]
         L.scw_exterior_points.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, c_void_p, c_void_p]
         L.scw_exterior_points_workspace.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, POINTER(c_size_t)]
+        L.scw_sweep_detector.argtypes = L.scw_sweep_wavelengths.argtypes + [POINTER(scw_window), POINTER(c_void_p)]
+        L.scw_sweep_detector_workspace.argtypes = L.scw_sweep_workspace.argtypes
+        L.scw_absorbance.argtypes = [c_void_p, c_int32, c_int64, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
         L.scw_invalidate_cache.argtypes = [c_void_p]
         L.scw_profile_assembly.argtypes = [c_void_p, c_int32, POINTER(c_double), POINTER(c_int32)]
         L.scw_calibrate.argtypes = L.scw_sweep_wavelengths.argtypes + [c_int32]
@@ -433,6 +441,36 @@ def scw_sweep_intensity(ctx, layers, zs, x, y, out=None, strides=None):
     sarr = None if strides is None else (c_int64 * 3)(*strides)
     ctx.check(ctx.L.scw_sweep_intensity(ctx._h, n, inst, Fz, zp, Nx, _p(x), Ny, _p(y), Ip, sarr))
     return out
+
+
+def scw_sweep_detector(ctx, layers, zs, x, y, window=None, want_I=True, want_S=True, out_I=None, out_S=None, strides=None):
+    """Detector reductions of a sweep: (I list or None, S list or None).  I[i]: [Fz, Ny, Nx] intensity, S[i]: [Fz] sums
+    of I over the window (ix0, ix1, iy0, iy1) of grid indices (None = whole plane); the complex field is never stored."""
+    n, inst, Fz, zp = _sweep_args(layers, zs)
+    Nx, Ny = x.numel(), y.numel()
+    need = c_size_t()
+    ctx.check(ctx.L.scw_sweep_detector_workspace(ctx._h, n, inst, Fz, Nx, Ny, byref(need)))
+    ctx.reserve(need.value)
+    real = {torch.complex64: torch.float32, torch.complex128: torch.float64}
+    if want_I and out_I is None:
+        out_I = [torch.empty((z.numel(), Ny, Nx), dtype=real[l.V.dtype], device=ctx.device) for l, z in zip(layers, zs)]
+    if want_S and out_S is None:
+        out_S = [torch.empty((z.numel(),), dtype=real[l.V.dtype], device=ctx.device) for l, z in zip(layers, zs)]
+    Ip = (c_void_p * max(n, 1))(*[e.data_ptr() for e in out_I]) if want_I else None
+    Sp = (c_void_p * max(n, 1))(*[e.data_ptr() for e in out_S]) if want_S else None
+    sarr = None if strides is None else (c_int64 * 3)(*strides)
+    w = None if window is None else byref(scw_window(*[int(v) for v in window]))
+    ctx.check(ctx.L.scw_sweep_detector(ctx._h, n, inst, Fz, zp, Nx, _p(x), Ny, _p(y), Ip, sarr, w, Sp))
+    return (out_I if want_I else None), (out_S if want_S else None)
+
+
+def scw_absorbance(ctx, S, S0, w=None, want_band=False):
+    """A = -log10(S / S0) elementwise; with want_band also -log10(sum w S / sum w S0) as a 1-element tensor."""
+    dt = SCW_C64 if S.dtype == torch.float32 else SCW_C128
+    A = torch.empty_like(S)
+    band = torch.empty((1,), dtype=S.dtype, device=S.device) if want_band else None
+    ctx.check(ctx.L.scw_absorbance(ctx._h, dt, S.numel(), _p(S), _p(S0), _p(w), _p(A), _p(band)))
+    return (A, band) if want_band else A
 
 
 def scw_sweep_wavelengths_host(ctx, layers, zs, x, y, out=None):

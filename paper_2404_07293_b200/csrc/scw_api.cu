@@ -488,25 +488,33 @@ static size_t sweep_ws(const scw_ctx* ctx, const scw_layer* L0, int64_t fz_max, 
 }
 
 // workspace of a sweep; the general (non-grouped) detector path adds a planar E buffer for one instance
+// Detector reductions asked of a sweep (NEXT-3): per-sample intensity I and / or its sum S over a window of every plane.
+struct DetArgs {
+    void* const* I;
+    void* const* S;
+    int64_t win[4];     // ix0, ix1, iy0, iy1
+};
+
 static size_t sweep_need(const scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, int64_t fz_max,
-                         size_t asm_max, int64_t Nx, int64_t Ny, bool intensity)
+                         size_t asm_max, int64_t Nx, int64_t Ny, const DetArgs* det)
 {
     if (!n_inst || fz_max == 0) return 0;
     const int group = sweep_group_size(ctx, n_inst, inst, Fz);
-    if (group) return sweep_group_ws(ctx, &inst[0], Fz[0], group, Nx, Ny);
+    if (group) return sweep_group_ws(ctx, &inst[0], Fz[0], group, Nx, Ny) + (det ? tc_synth_wsum_bytes(Fz[0] * group, Nx, Ny) : 0);
     return sweep_ws(ctx, &inst[0], fz_max, asm_max, Nx, Ny) +
-           (intensity ? align_up((size_t)fz_max * 3 * Nx * Ny * esize(inst[0].dtype)) : 0);
+           (det ? align_up((size_t)fz_max * 3 * Nx * Ny * esize(inst[0].dtype)) : 0);
 }
 
 static int32_t sweep_workspace_impl(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, int64_t Nx,
-                                    int64_t Ny, size_t* bytes, bool intensity, const char* who)
+                                    int64_t Ny, size_t* bytes, bool detector, const char* who)
 {
     if (!ctx || !bytes) return SCW_ERR_NULL;
     ctx->msg[0] = 0;
     int64_t fz_max = 0;
     size_t asm_max = 0;
     if (int32_t s = check_sweep(ctx, n_inst, inst, Fz, Nx, Ny, who, &fz_max, &asm_max)) return s;
-    *bytes = sweep_need(ctx, n_inst, inst, Fz, fz_max, asm_max, Nx, Ny, intensity);
+    const DetArgs any = {};
+    *bytes = sweep_need(ctx, n_inst, inst, Fz, fz_max, asm_max, Nx, Ny, detector ? &any : nullptr);
     return SCW_OK;
 }
 
@@ -525,9 +533,10 @@ int32_t scw_sweep_intensity_workspace(scw_ctx* ctx, int64_t n_inst, const scw_la
 // Shared by the device- and host-buffer variants: everything after validation.
 static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, const double* const* z,
                       int64_t Nx, const double* x, int64_t Ny, const double* y, void* const* E, const int64_t s4[4],
-                      int64_t fz_max, size_t asm_max, Carver& cv, bool intensity = false)
+                      int64_t fz_max, size_t asm_max, Carver& cv, const DetArgs* det = nullptr)
 {
-    // intensity: E[i] are real buffers receiving sum_comp |E_comp|^2 at n*s4[1] + k*s4[2] + i*s4[3] (NEXT-3)
+    // det: no complex field; det->I[i] are real buffers receiving sum_comp |E_comp|^2 at n*s4[1] + k*s4[2] + i*s4[3], det->S[i]
+    // the window sums (NEXT-3)
     const scw_layer& L0 = inst[0];
     const int64_t R = 3LL * L0.U * L0.Vn;
     const int group = sweep_group_size(ctx, n_inst, inst, Fz);
@@ -540,6 +549,7 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
         probe.take(tc_synth_twiddle_bytes(L0.U, L0.Vn, Nx, Ny));
         void* a_scr = probe.take(tc_assemble_scratch(ctx, R, L0.J, Fz[0], group));
         void* s_scr = probe.take(tc_synth_scratch(L0.U, L0.Vn, Fz[0] * group));
+        void* w_scr = det ? probe.take(tc_synth_wsum_bytes(Fz[0] * group, Nx, Ny)) : nullptr;
         int* ctl = nullptr;
         size_t n_ctl = 0;
         tc_assemble_ctl(ctx, R, L0.J, Fz[0], group, a_scr, &ctl, &n_ctl);
@@ -557,7 +567,15 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
             launch_tc_assemble_group(ctx, g, inst + i0, Fz[0], z + i0, fix, sched, n_sched, a_scr, clean);
             if (ctx->tc_error) return;
             clean = true;                               // the kernel leaves its control block zeroed
-            launch_tc_synth_group_images(ctx, L0.U, L0.Vn, Fz[0], g, Nx, Ny, tw.a, E + i0, s4, s_scr, intensity);
+            TcDetector td;
+            if (det) {
+                td.I = det->I ? det->I + i0 : nullptr;
+                td.S = det->S ? det->S + i0 : nullptr;
+                memcpy(td.win, det->win, sizeof(td.win));
+                td.s_part = w_scr;
+            }
+            launch_tc_synth_group_images(ctx, L0.U, L0.Vn, Fz[0], g, Nx, Ny, tw.a, det ? nullptr : E + i0, s4, s_scr,
+                                         det ? &td : nullptr);
         }
         return;
     }
@@ -566,16 +584,17 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
     const size_t asm_off = cv.off;
     cv.take(asm_max);
     void* scratch = cv.take(synth_ws(ctx, L0.dtype, L0.U, L0.Vn, fz_max, Ny));
-    void* E_tmp = intensity ? cv.take((size_t)fz_max * 3 * Nx * Ny * esize(L0.dtype)) : nullptr;   // general detector path
+    void* E_tmp = det ? cv.take((size_t)fz_max * 3 * Nx * Ny * esize(L0.dtype)) : nullptr;   // general detector path
     int64_t planar[4];
     planar_strides(Nx, Ny, planar);
     for (int64_t i = 0; i < n_inst; ++i) {
         if (Fz[i] == 0) continue;
         Carver sub(cv.base ? cv.base + asm_off : nullptr);
         run_assemble(ctx, &inst[i], Fz[i], z[i], P, R, sub);
-        if (intensity) {
+        if (det) {
             run_synth(ctx, tw, L0.dtype, L0.U, L0.Vn, Fz[i], P, R, Nx, Ny, E_tmp, planar, scratch);
-            launch_intensity(ctx, L0.dtype, Fz[i], Ny, Nx, E_tmp, E[i], s4 + 1);
+            if (det->I) launch_intensity(ctx, L0.dtype, Fz[i], Ny, Nx, E_tmp, det->I[i], s4 + 1);
+            if (det->S) launch_window_sum(ctx, L0.dtype, Fz[i], Ny, Nx, E_tmp, det->win, det->S[i]);
         } else {
             run_synth(ctx, tw, L0.dtype, L0.U, L0.Vn, Fz[i], P, R, Nx, Ny, E[i], s4, scratch);
         }
@@ -584,7 +603,7 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
 
 static int32_t sweep_impl(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, const double* const* z,
                           int64_t Nx, const double* x, int64_t Ny, const double* y, void* const* E, const int64_t* strides,
-                          bool intensity, const char* who)
+                          const DetArgs* det, const char* who)
 {
     if (int32_t s = check_ctx(ctx, true)) return s;
     int64_t fz_max = 0;
@@ -592,16 +611,28 @@ static int32_t sweep_impl(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, c
     if (int32_t s = check_sweep(ctx, n_inst, inst, Fz, Nx, Ny, who, &fz_max, &asm_max)) return s;
     if (n_inst == 0 || fz_max == 0) return SCW_OK;
     if (int32_t s = check_grid(ctx, inst[0].dtype, inst[0].U, inst[0].Vn, inst[0].X, inst[0].Y, Nx, x, Ny, y, who)) return s;
-    if (!z || !E) return fail(ctx, SCW_ERR_NULL, "%s: z and the output array are required", who);
-    const size_t out_es = intensity ? esize(inst[0].dtype) / 2 : esize(inst[0].dtype);
+    if (!z) return fail(ctx, SCW_ERR_NULL, "%s: z is required", who);
+    if (!det && !E) return fail(ctx, SCW_ERR_NULL, "%s: the output array is required", who);
+    if (det && !det->I && !det->S) return fail(ctx, SCW_ERR_NULL, "%s: at least one of I and S is required", who);
+    if (det && (det->win[0] < 0 || det->win[1] > Nx || det->win[0] >= det->win[1] || det->win[2] < 0 || det->win[3] > Ny ||
+                det->win[2] >= det->win[3]))
+        return fail(ctx, SCW_ERR_SHAPE, "%s: window [%lld, %lld) x [%lld, %lld) is empty or outside the %lld x %lld grid", who,
+                    (long long)det->win[0], (long long)det->win[1], (long long)det->win[2], (long long)det->win[3],
+                    (long long)Nx, (long long)Ny);
+    const size_t out_es = det ? esize(inst[0].dtype) / 2 : esize(inst[0].dtype);
     for (int64_t i = 0; i < n_inst; ++i) {
         if (Fz[i] == 0) continue;
-        if (!z[i] || !E[i]) return fail(ctx, SCW_ERR_NULL, "%s: z[%lld] / output[%lld] is NULL", who, (long long)i, (long long)i);
-        if (!aligned(z[i], 8) || !aligned(E[i], out_es))
-            return fail(ctx, SCW_ERR_ALIGN, "%s: z[%lld] / output[%lld] misaligned", who, (long long)i, (long long)i);
+        if (!z[i] || !aligned(z[i], 8)) return fail(ctx, SCW_ERR_NULL, "%s: z[%lld] is NULL or misaligned", who, (long long)i);
+        void* outs[3] = {det ? nullptr : E[i], (det && det->I) ? det->I[i] : nullptr, (det && det->S) ? det->S[i] : nullptr};
+        const bool wanted[3] = {!det, det && det->I, det && det->S};
+        for (int k = 0; k < 3; ++k) {
+            if (!wanted[k]) continue;
+            if (!outs[k]) return fail(ctx, SCW_ERR_NULL, "%s: output[%lld] is NULL", who, (long long)i);
+            if (!aligned(outs[k], out_es)) return fail(ctx, SCW_ERR_ALIGN, "%s: output[%lld] misaligned", who, (long long)i);
+        }
     }
     int64_t s4[4];
-    if (intensity) {                                   // (z, y, x) strides in s4[1..3]; the component slot is unused
+    if (det) {                                         // (z, y, x) strides in s4[1..3]; the component slot is unused
         s4[0] = 0;
         if (strides) memcpy(s4 + 1, strides, 3 * sizeof(int64_t));
         else { s4[1] = Nx * Ny; s4[2] = Nx; s4[3] = 1; }
@@ -612,9 +643,9 @@ static int32_t sweep_impl(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, c
     }
     for (int i = 0; i < 4; ++i)
         if (s4[i] < 0) return fail(ctx, SCW_ERR_SHAPE, "%s: negative stride", who);
-    if (int32_t s = need_ws(ctx, sweep_need(ctx, n_inst, inst, Fz, fz_max, asm_max, Nx, Ny, intensity), who)) return s;
+    if (int32_t s = need_ws(ctx, sweep_need(ctx, n_inst, inst, Fz, fz_max, asm_max, Nx, Ny, det), who)) return s;
     Carver cv(ctx->ws);
-    run_sweep(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, E, s4, fz_max, asm_max, cv, intensity);
+    run_sweep(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, E, s4, fz_max, asm_max, cv, det);
     return check_launch(ctx, who);
 }
 
@@ -622,14 +653,50 @@ int32_t scw_sweep_wavelengths(scw_ctx* ctx, int64_t n_inst, const scw_layer* ins
                               const double* const* z, int64_t Nx, const double* x, int64_t Ny, const double* y,
                               void* const* E, const int64_t* strides)
 {
-    return sweep_impl(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, E, strides, false, "scw_sweep_wavelengths");
+    return sweep_impl(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, E, strides, nullptr, "scw_sweep_wavelengths");
+}
+
+int32_t scw_sweep_detector(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz,
+                           const double* const* z, int64_t Nx, const double* x, int64_t Ny, const double* y,
+                           void* const* I, const int64_t* strides, const scw_window* window, void* const* S)
+{
+    DetArgs det;
+    det.I = I;
+    det.S = S;
+    det.win[0] = window ? window->ix0 : 0;
+    det.win[1] = window ? window->ix1 : Nx;
+    det.win[2] = window ? window->iy0 : 0;
+    det.win[3] = window ? window->iy1 : Ny;
+    return sweep_impl(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, nullptr, strides, &det, "scw_sweep_detector");
+}
+
+int32_t scw_sweep_detector_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, int64_t Nx,
+                                     int64_t Ny, size_t* bytes)
+{
+    return sweep_workspace_impl(ctx, n_inst, inst, Fz, Nx, Ny, bytes, true, "scw_sweep_detector_workspace");
 }
 
 int32_t scw_sweep_intensity(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz,
                             const double* const* z, int64_t Nx, const double* x, int64_t Ny, const double* y,
                             void* const* I, const int64_t* strides)
 {
-    return sweep_impl(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, I, strides, true, "scw_sweep_intensity");
+    if (ctx && !I) return fail(ctx, SCW_ERR_NULL, "scw_sweep_intensity: the output array is required");
+    return scw_sweep_detector(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, I, strides, nullptr, nullptr);
+}
+
+int32_t scw_absorbance(scw_ctx* ctx, int32_t dtype, int64_t n, const void* S, const void* S0, const void* w, void* A,
+                       void* band)
+{
+    if (int32_t s = check_ctx(ctx)) return s;
+    if (dtype != SCW_C64 && dtype != SCW_C128) return fail(ctx, SCW_ERR_DTYPE, "scw_absorbance: bad dtype %d", dtype);
+    if (n < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_absorbance: n=%lld < 0", (long long)n);
+    if (n == 0) return SCW_OK;
+    if (!S || !S0 || (!A && !band)) return fail(ctx, SCW_ERR_NULL, "scw_absorbance: S, S0 and one of A, band are required");
+    const size_t es = esize(dtype) / 2;
+    if (!aligned(S, es) || !aligned(S0, es) || (w && !aligned(w, es)) || (A && !aligned(A, es)) || (band && !aligned(band, es)))
+        return fail(ctx, SCW_ERR_ALIGN, "scw_absorbance: misaligned array");
+    launch_absorbance(ctx, dtype, n, S, S0, w, A, band);
+    return check_launch(ctx, "scw_absorbance");
 }
 
 int32_t scw_profile_assembly(scw_ctx* ctx, int32_t max_ctas, double* us, int32_t* n_ctas)
@@ -670,7 +737,7 @@ int32_t scw_calibrate(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
         int G = 0;
         for (int r = 0; r <= reps; ++r) {           // the first sweep of a round is a warm-up
             ctx->last_asm_G = 0;
-            if (int32_t s = sweep_impl(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, E, strides, false, "scw_calibrate")) {
+            if (int32_t s = sweep_impl(ctx, n_inst, inst, Fz, z, Nx, x, Ny, y, E, strides, nullptr, "scw_calibrate")) {
                 ctx->split_w.clear();
                 return s;
             }

@@ -121,6 +121,10 @@ void launch_simt_synth(scw_ctx* ctx, int dtype, int U, int Vn, int64_t Fz, const
 // I[n][k][i] = sum_comp |E[n][comp][k][i]|^2, E planar, I at n*s3[0] + k*s3[1] + i*s3[2]
 void launch_intensity(scw_ctx* ctx, int dtype, int64_t Fz, int64_t Ny, int64_t Nx, const void* E, void* I,
                       const int64_t s3[3]);
+// S[n] = sum over the window (ix0, ix1, iy0, iy1; grid indices, half-open) and the components of |E[n][comp][k][i]|^2, E planar
+void launch_window_sum(scw_ctx* ctx, int dtype, int64_t Fz, int64_t Ny, int64_t Nx, const void* E, const int64_t win[4], void* S);
+// A[i] = -log10(S[i] / S0[i]); band (may be NULL): -log10(sum w S / sum w S0) over the n entries (w NULL = ones)
+void launch_absorbance(scw_ctx* ctx, int dtype, int64_t n, const void* S, const void* S0, const void* w, void* A, void* band);
 
 // ---- scw_tc_assemble.cu: tcgen05 BF16x3 spectral assembly (complex64) ----------------------------
 bool tc_assemble_supported(int dtype, int64_t R, int64_t J, int64_t Fz, const void* V, int64_t ldV);
@@ -148,6 +152,14 @@ void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, i
 void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z, void* P, int64_t ldP,
                         void* scratch);
 
+// Detector reductions of a sweep (NEXT-3): what leaves the synthesis instead of the complex field.
+struct TcDetector {
+    void* const* I;        // per instance: real [Fz][Ny][Nx] at s3 strides (passed as strides[1..3]), or NULL: not wanted
+    void* const* S;        // per instance: real [Fz] sums of I over the window, or NULL: not wanted
+    int64_t win[4];        // ix0, ix1, iy0, iy1 (grid indices, half-open)
+    void* s_part;          // scratch of tc_synth_wsum_bytes() for the fused kernel (when S is wanted)
+};
+
 // ---- scw_tc_synth.cu: tcgen05 BF16x3 separable synthesis (complex64, 2U and 2V <= 80) ---------------
 bool tc_synth_supported(int dtype, int U, int Vn);
 size_t tc_synth_twiddle_bytes(int U, int Vn, int64_t Nx, int64_t Ny);
@@ -160,14 +172,15 @@ int tc_synth_max_group();
 void tc_synth_image_plan(int U, int Vn, int64_t Nx, int64_t Ny, void* scratch, const void* tw, TcFixup* fix, int** sched,
                          int* n_sched);
 // n_inst instances with equal Fz, spectra back to back in P_all ([ldP x n_inst*Fz]); scratch = tc_synth_scratch(U, Vn, Fz*n_inst)
-// intensity: E[i] are float buffers receiving I = sum_comp |E_comp|^2 at z*strides[1] + y*strides[2] + x*strides[3]
+// det != NULL: detector mode (no complex field; I at z*strides[1] + y*strides[2] + x*strides[3] and / or window sums)
 void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const void* P_all, int64_t ldP,
                            int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
-                           void* scratch, bool intensity = false);
+                           void* scratch, const TcDetector* det = nullptr);
+size_t tc_synth_wsum_bytes(int64_t planes_z, int64_t Nx, int64_t Ny);
 // Same, with the spectrum images already in `scratch` and the plane counters zeroed (written by the assembly's fix-up).
 void launch_tc_synth_group_images(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, int64_t Nx, int64_t Ny,
                                   const void* tw, void* const* E, const int64_t strides[4], void* scratch,
-                                  bool intensity = false);
+                                  const TcDetector* det = nullptr);
 void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,
                      const void* tw, void* E, const int64_t strides[4], void* scratch);
 

@@ -378,4 +378,71 @@ void launch_intensity(scw_ctx* ctx, int dtype, int64_t Fz, int64_t Ny, int64_t N
                                                                                     s3[0], s3[1], s3[2]);
 }
 
+// NEXT-3 detector, general path: window sum of the intensity on a plane, one block per z plane, fixed reduction tree.
+template <typename T>
+__global__ void __launch_bounds__(256) k_window_sum(int64_t Ny, int64_t Nx, const typename C2<T>::type* __restrict__ E,
+                                                   int64_t x0, int64_t x1, int64_t y0, int64_t y1, T* __restrict__ S)
+{
+    __shared__ T red[256];
+    const int64_t n = blockIdx.x, plane = Nx * Ny;
+    const int64_t wx = x1 - x0, cnt = wx * (y1 - y0);
+    T acc = 0;
+    for (int64_t i = threadIdx.x; i < cnt; i += 256) {
+        const int64_t k = y0 + i / wx, ix = x0 + i % wx;
+#pragma unroll
+        for (int comp = 0; comp < 3; ++comp) {
+            const typename C2<T>::type e = E[(n * 3 + comp) * plane + k * Nx + ix];
+            acc += e.x * e.x + e.y * e.y;
+        }
+    }
+    red[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) S[n] = red[0];
+}
+
+void launch_window_sum(scw_ctx* ctx, int dtype, int64_t Fz, int64_t Ny, int64_t Nx, const void* E, const int64_t win[4], void* S)
+{
+    KernelScope ks(ctx, KC_MISC);
+    if (dtype == SCW_C64)
+        k_window_sum<float><<<(unsigned)Fz, 256, 0, ctx->stream>>>(Ny, Nx, (const float2*)E, win[0], win[1], win[2], win[3], (float*)S);
+    else
+        k_window_sum<double><<<(unsigned)Fz, 256, 0, ctx->stream>>>(Ny, Nx, (const double2*)E, win[0], win[1], win[2], win[3], (double*)S);
+}
+
+// Absorbance A = -log10(S / S0) per entry and, optionally, of the band: -log10(sum w S / sum w S0).
+template <typename T>
+__global__ void __launch_bounds__(256) k_absorbance(int64_t n, const T* __restrict__ S, const T* __restrict__ S0,
+                                                   const T* __restrict__ w, T* __restrict__ A, T* __restrict__ band)
+{
+    __shared__ double rs[256], r0[256];
+    double as = 0.0, a0 = 0.0;
+    for (int64_t i = threadIdx.x; i < n; i += 256) {
+        const double s = (double)S[i], s0 = (double)S0[i], wi = w ? (double)w[i] : 1.0;
+        if (A) A[i] = (T)(-log10(s / s0));
+        as += wi * s;
+        a0 += wi * s0;
+    }
+    rs[threadIdx.x] = as;
+    r0[threadIdx.x] = a0;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) { rs[threadIdx.x] += rs[threadIdx.x + o]; r0[threadIdx.x] += r0[threadIdx.x + o]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0 && band) band[0] = (T)(-log10(rs[0] / r0[0]));
+}
+
+void launch_absorbance(scw_ctx* ctx, int dtype, int64_t n, const void* S, const void* S0, const void* w, void* A, void* band)
+{
+    KernelScope ks(ctx, KC_MISC);
+    if (dtype == SCW_C64)
+        k_absorbance<float><<<1, 256, 0, ctx->stream>>>(n, (const float*)S, (const float*)S0, (const float*)w, (float*)A, (float*)band);
+    else
+        k_absorbance<double><<<1, 256, 0, ctx->stream>>>(n, (const double*)S, (const double*)S0, (const double*)w, (double*)A, (double*)band);
+}
+
 }  // namespace scw

@@ -36,6 +36,8 @@ constexpr int TS_MAX_INST = 64;            // instances per grouped launch
 #endif
 
 
+struct TsWsumOut { float* S[TS_MAX_INST]; };
+
 struct TsParams {
     const uint8_t* A1;     // [ty][vc][hi|lo] images of (Fy_r, Fy_i): 128 rows x K1p, K-major, LBO = 2048, SBO = 128
     const uint32_t* A2;    // [tx][uc][row][hi K2p/2 | lo K2p/2] packed bf16 pairs (cos, sin) of Fx: TMEM A-operand rows
@@ -49,9 +51,12 @@ struct TsParams {
     int nuc, nvc;          // frequency chunks along u and v
     int tiles_x, tiles_y, pair0, npairs;   // this launch covers tile pairs [pair0, pair0 + npairs)
     int* sched;            // [tile pair] next plane group to hand out (zeroed by the spectrum-image kernel)
-    int group;             // planes per drawn unit: 1, or 3 (the components of one z) in intensity mode
-    int intensity;         // 1: E[] point to float outputs I = sum_comp |E_comp|^2 (NEXT-3 detector), no complex field stored
-    int acc_col;           // detector: first of 128 TMEM columns holding the running sum, 0 = none (sum kept in the output)
+    int group;             // planes per drawn unit: 1, or 3 (the components of one z) when the detector writes I
+    // NEXT-3 detector (k_tc_synth<true>): no complex field is stored.
+    int want_I;            // E[] point to float outputs I = sum_comp |E_comp|^2
+    int acc_col;           // first of 128 TMEM columns holding the running sum over components, 0 = none (kept in the output)
+    float* s_part;         // window sums: [plane][tile][16] partial sums of |E_comp|^2 over the window, NULL = not wanted
+    int win_x0, win_x1, win_y0, win_y1;   // window (grid indices, half-open)
 };
 
 __host__ __device__ inline int ts_pad16(int v) { return (v + 15) / 16 * 16; }
@@ -427,41 +432,76 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                 tc_fence_after();
                 const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + TS_D2_COL + h * TS_TILE + 64 * cg;
                 if (INTENSITY) {
-                    // detector: I = |E_x|^2 + |E_y|^2 + |E_z|^2.  The three components of a z plane come to this CTA in
-                    // order (group = 3) and every (x, y) belongs to one thread.  The running sum lives in TMEM (128 spare
-                    // columns, lane = x, column = y) when they exist (p.acc_col; then only the third component writes the
-                    // output), else in the output itself (read-modify-write through L2).
-                    float* io = reinterpret_cast<float*>(Einst) + zi * p.s_z + x * p.s_x + y0 * p.s_y;
+                    // detector: |E_comp|^2 per sample, then (want_I) I = |E_x|^2 + |E_y|^2 + |E_z|^2 and / or (s_part) the
+                    // sum over a window of the plane.  D2[h] is released as soon as it is in registers, like the complex
+                    // path.  For I the three components of a z plane come to this CTA in order (group = 3) and every
+                    // (x, y) belongs to one thread: the running sum lives in 128 spare TMEM columns (lane = x, column = y)
+                    // when they exist (p.acc_col; only the third component writes the output), else in the output itself
+                    // (read-modify-write through L2).
+                    const bool tm_acc = p.want_I && p.acc_col;
                     const uint32_t acc = tmem_base + ((uint32_t)(32 * q) << 16) + p.acc_col + h * 64 + 32 * cg;
-                    if (p.acc_col && comp > 0) tmem_st_wait();     // the previous component's sums have landed
-#pragma unroll
-                    for (int j = 0; j < 2; ++j) {                  // 16 y at a time
-                        uint32_t v[32];
-                        float a[16];
-                        tmem_ld32_raw(taddr + 32 * j, v);
-                        if (p.acc_col && comp > 0) tmem_ld16(acc + 16 * j, a);
+                    float m2[32];
+                    {
+                        uint32_t v[2][32];
+                        tmem_ld32_raw(taddr, v[0]);
+                        tmem_ld32_raw(taddr + 32, v[1]);
                         tmem_ld_wait();
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(&d2_empty[h]);  // D2[h] is in registers now
 #pragma unroll
-                        for (int e = 0; e < 16; ++e) {
-                            const float re = __uint_as_float(v[2 * e]), im = __uint_as_float(v[2 * e + 1]);
-                            const float m2 = re * re + im * im;
-                            if (!p.acc_col && comp > 0 && x_ok && 16 * j + e < ny) a[e] = __ldcg(io + (16 * j + e) * p.s_y);
-                            a[e] = comp > 0 ? a[e] + m2 : m2;
-                        }
-                        if (p.acc_col && comp < 2) {
-                            uint32_t w[16];
-#pragma unroll
-                            for (int e = 0; e < 16; ++e) w[e] = __float_as_uint(a[e]);
-                            tmem_st16(acc + 16 * j, w);
-                        } else if (x_ok) {
-#pragma unroll
-                            for (int e = 0; e < 16; ++e)
-                                if (16 * j + e < ny) __stcg(io + (16 * j + e) * p.s_y, a[e]);
+                        for (int e = 0; e < 32; ++e) {
+                            const float re = __uint_as_float(v[e >> 4][(2 * e) & 31]), im = __uint_as_float(v[e >> 4][(2 * e + 1) & 31]);
+                            m2[e] = re * re + im * im;
                         }
                     }
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(&d2_empty[h]);      // D2[h] has been consumed
+                    if (p.s_part) {                                // window sum of this warp's 32 x 32 patch, fixed order
+                        float ws = 0.f;
+                        const bool xin = x >= p.win_x0 && x < p.win_x1;
+#pragma unroll
+                        for (int e = 0; e < 32; ++e)
+                            if (xin && y0 + e >= p.win_y0 && y0 + e < p.win_y1) ws += m2[e];
+#pragma unroll
+                        for (int o = 16; o > 0; o >>= 1) ws += __shfl_xor_sync(0xffffffffu, ws, o);
+                        if (lane == 0)
+                            p.s_part[((size_t)gplane * (p.tiles_x * p.tiles_y) + pair) * 16 + h * 8 + cg * 4 + q] = ws;
+                    }
+                    if (p.want_I) {
+                        float* io = reinterpret_cast<float*>(Einst) + zi * p.s_z + x * p.s_x + y0 * p.s_y;
+                        if (tm_acc) {
+                            if (comp > 0) {
+                                float a[2][16];
+                                tmem_st_wait();                    // the previous component's sums have landed
+                                tmem_ld16(acc, a[0]);
+                                tmem_ld16(acc + 16, a[1]);
+                                tmem_ld_wait();
+#pragma unroll
+                                for (int e = 0; e < 32; ++e) m2[e] += a[e >> 4][e & 15];
+                            }
+                            if (comp < 2) {
+                                uint32_t w0[16], w1[16];
+#pragma unroll
+                                for (int e = 0; e < 16; ++e) {
+                                    w0[e] = __float_as_uint(m2[e]);
+                                    w1[e] = __float_as_uint(m2[16 + e]);
+                                }
+                                tmem_st16(acc, w0);
+                                tmem_st16(acc + 16, w1);
+                            } else if (x_ok) {
+#pragma unroll
+                                for (int e = 0; e < 32; ++e)
+                                    if (e < ny) __stcg(io + e * p.s_y, m2[e]);
+                            }
+                        } else if (x_ok) {
+#pragma unroll
+                            for (int e = 0; e < 32; ++e) {
+                                if (e < ny) {
+                                    const float prev = comp > 0 ? __ldcg(io + e * p.s_y) : 0.f;
+                                    __stcg(io + e * p.s_y, prev + m2[e]);
+                                }
+                            }
+                        }
+                    }
                 } else {
                     uint32_t v[2][32];
                     tmem_ld32_raw(taddr, v[0]);
@@ -486,6 +526,19 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
     tc_fence_before();
     __syncthreads();
     if (warp == 1) tmem_dealloc(tmem_base, TS_TMEM_COLS);
+}
+
+// Window sums: S[inst][n] = sum over the three components, the output tiles and the 16 warp patches of a tile, in a fixed
+// order (deterministic), of the partial sums the detector epilogue left in s_part.
+__global__ void k_tc_synth_wsum(int n_inst, int Fz, int tiles, const float* __restrict__ s_part, const TsWsumOut out)
+{
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;           // (inst, n)
+    if (idx >= n_inst * Fz) return;
+    const int inst = idx / Fz, n = idx - inst * Fz;
+    const float* src = s_part + (size_t)idx * 3 * tiles * 16;         // plane (inst*Fz + n)*3 + comp, contiguous over comp
+    float acc = 0.f;
+    for (int i = 0; i < 3 * tiles * 16; ++i) acc += src[i];
+    out.S[inst][n] = acc;
 }
 
 // ---- host side -------------------------------------------------------------------------------------
@@ -554,15 +607,17 @@ static int* ts_sched(const TsPlan& pl, const void* tw)
 
 // The synthesis launches proper: B1 holds the spectrum images of all n_inst*Fz*3 planes.
 static void ts_launch_main(scw_ctx* ctx, const TsPlan& pl, int64_t Fz, int n_inst, const uint8_t* B1, int64_t Nx,
-                           int64_t Ny, const void* tw, void* const* E, const int64_t strides[4], bool intensity)
+                           int64_t Ny, const void* tw, void* const* E, const int64_t strides[4], const TcDetector* det)
 {
+    const bool intensity = det != nullptr;
+    const bool want_I = intensity && det->I != nullptr;
     static thread_local TsParams p;
     const int planes = (int)(Fz * 3 * n_inst);
     p.A1 = static_cast<const uint8_t*>(tw);
     p.A2 = reinterpret_cast<const uint32_t*>(p.A1 + pl.a1_bytes);
     p.B1 = B1;
     p.sched = ts_sched(pl, tw);
-    for (int i = 0; i < n_inst; ++i) p.E[i] = static_cast<float2*>(E[i]);
+    for (int i = 0; i < n_inst; ++i) p.E[i] = static_cast<float2*>(intensity ? (want_I ? det->I[i] : nullptr) : E[i]);
     p.s_comp = strides[0];
     p.s_z = strides[1];
     p.s_y = strides[2];
@@ -575,11 +630,15 @@ static void ts_launch_main(scw_ctx* ctx, const TsPlan& pl, int64_t Fz, int n_ins
     p.K2p = pl.K2p;
     p.nuc = pl.cu.n;
     p.nvc = pl.cv.n;
-    p.intensity = intensity ? 1 : 0;
-    p.group = intensity ? 3 : 1;
+    p.want_I = want_I ? 1 : 0;
+    p.group = want_I ? 3 : 1;
     {   // detector accumulators go behind D2 | D1 | A2 when 128 TMEM columns are left (U <= 32)
         const int used = TS_D1_COL + pl.K2p * (1 + pl.cu.n);
-        p.acc_col = (intensity && used + 128 <= TS_TMEM_COLS) ? used : 0;
+        p.acc_col = (want_I && used + 128 <= TS_TMEM_COLS) ? used : 0;
+    }
+    p.s_part = (intensity && det->S) ? static_cast<float*>(det->s_part) : nullptr;
+    if (intensity) {
+        p.win_x0 = (int)det->win[0]; p.win_x1 = (int)det->win[1]; p.win_y0 = (int)det->win[2]; p.win_y1 = (int)det->win[3];
     }
     const size_t smem_bytes = pl.smem_bytes;
     p.tiles_x = pl.tiles_x;
@@ -596,13 +655,26 @@ static void ts_launch_main(scw_ctx* ctx, const TsPlan& pl, int64_t Fz, int n_ins
         if (intensity) k_tc_synth<true><<<p.npairs * per_pair, TS_THREADS, smem_bytes, ctx->stream>>>(p);
         else k_tc_synth<false><<<p.npairs * per_pair, TS_THREADS, smem_bytes, ctx->stream>>>(p);
     }
+    if (p.s_part) {
+        TsWsumOut out;
+        for (int i = 0; i < n_inst; ++i) out.S[i] = static_cast<float*>(det->S[i]);
+        KernelScope ks(ctx, KC_MISC);
+        const int n = n_inst * (int)Fz;
+        k_tc_synth_wsum<<<(n + 127) / 128, 128, 0, ctx->stream>>>(n_inst, (int)Fz, total_pairs, p.s_part, out);
+    }
+}
+
+size_t tc_synth_wsum_bytes(int64_t planes_z, int64_t Nx, int64_t Ny)
+{
+    const int64_t tiles = ((Nx + TS_TILE - 1) / TS_TILE) * ((Ny + TS_TILE - 1) / TS_TILE);
+    return align_up((size_t)planes_z * 3 * tiles * 16 * sizeof(float));
 }
 
 // n_inst <= TS_MAX_INST instances with the same Fz whose spectra are stored back to back
 // (P_all is one column-major [ldP x n_inst*Fz] matrix): one image pre-kernel + one synthesis launch.
 void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, const void* P_all, int64_t ldP,
                            int64_t Nx, int64_t Ny, const void* tw, void* const* E, const int64_t strides[4],
-                           void* scratch, bool intensity)
+                           void* scratch, const TcDetector* det)
 {
     const TsPlan pl = ts_plan(U, Vn, Fz * n_inst, Nx, Ny);
     const int planes = (int)(Fz * 3 * n_inst);
@@ -615,7 +687,7 @@ void launch_tc_synth_group(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, 
                                                                                 ldP, B1, ts_sched(pl, tw),
                                                                                 pl.tiles_x * pl.tiles_y);
     }
-    ts_launch_main(ctx, pl, Fz, n_inst, B1, Nx, Ny, tw, E, strides, intensity);
+    ts_launch_main(ctx, pl, Fz, n_inst, B1, Nx, Ny, tw, E, strides, det);
 }
 
 void tc_synth_image_plan(int U, int Vn, int64_t Nx, int64_t Ny, void* scratch, const void* tw, TcFixup* fix, int** sched,
@@ -637,16 +709,17 @@ void tc_synth_image_plan(int U, int Vn, int64_t Nx, int64_t Ny, void* scratch, c
 }
 
 void launch_tc_synth_group_images(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n_inst, int64_t Nx, int64_t Ny,
-                                  const void* tw, void* const* E, const int64_t strides[4], void* scratch, bool intensity)
+                                  const void* tw, void* const* E, const int64_t strides[4], void* scratch,
+                                  const TcDetector* det)
 {
     const TsPlan pl = ts_plan(U, Vn, Fz * n_inst, Nx, Ny);
-    ts_launch_main(ctx, pl, Fz, n_inst, static_cast<const uint8_t*>(scratch), Nx, Ny, tw, E, strides, intensity);
+    ts_launch_main(ctx, pl, Fz, n_inst, static_cast<const uint8_t*>(scratch), Nx, Ny, tw, E, strides, det);
 }
 
 void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,
                      const void* tw, void* E, const int64_t strides[4], void* scratch)
 {
-    launch_tc_synth_group(ctx, U, Vn, Fz, 1, P, ldP, Nx, Ny, tw, &E, strides, scratch, false);
+    launch_tc_synth_group(ctx, U, Vn, Fz, 1, P, ldP, Nx, Ny, tw, &E, strides, scratch, nullptr);
 }
 
 }  // namespace scw

@@ -144,3 +144,98 @@ def test_intensity_wide_frequency_grids(scw, U, Vn):
             assert float((I - Ie).abs().max() / Ie.max()) <= 5e-6
     finally:
         ctx.close()
+
+
+# ------------------------------------------------------------------------------------------------ window sums, absorbance
+def test_window_sum_and_absorbance_closed_forms():
+    """Pins for the remaining detector reductions (CPU).  (i) One plane wave: I is flat, so the window sum is the number of
+    samples in the window times I.  (ii) Absorbing homogeneous slab, one "+" wave at normal incidence with gamma = n:
+    I(z) = I(z_lo) exp(-2 k Im(n) (z - z_lo)), so A = -log10(I(z_hi) / I(z_lo)) = 2 k Im(n) t log10(e) (Beer-Lambert).
+    (iii) Band absorbance of equal readings equals the single absorbance; weights act as a weighted mean of S, S0."""
+    cfg = si.CONFIGS[0]
+    lay = si.make_layer(cfg, dtype=np.complex128)
+    M = lay["U"] * lay["Vn"]
+    j, m = 6, 40
+    V1 = np.zeros_like(lay["V"])
+    for comp in range(3):
+        V1[j, comp * M + m] = lay["V"][j, comp * M + m]
+    one = dict(lay, V=V1)
+    x, y, z = np.arange(12) * 0.37, np.arange(9) * 0.51, np.array([0.4, 1.9])
+    I = oracle.intensity(oracle.layer_grid(x=x, y=y, z=z, **one))
+    S = oracle.window_sum(I, (2, 9, 1, 6))
+    assert np.allclose(S, 7 * 5 * I[:, 0, 0], rtol=1e-12)
+    assert np.allclose(oracle.window_sum(I), 12 * 9 * I[:, 0, 0], rtol=1e-12)
+    # Beer-Lambert slab
+    n_slab, lam, t = 1.45 + 0.03j, 0.8, 2.5
+    Vs = np.zeros((4, 3), dtype=np.complex128)
+    Vs[0, 0] = 1.0                                              # E_x, frequency (0, 0), "+" mode
+    slab = dict(U=1, Vn=1, X=3.0, Y=3.0, lam=lam, z_lo=0.0, z_hi=t, V=Vs, c=None,
+                gamma=np.array([n_slab, -n_slab, n_slab, -n_slab]), dir=np.array([1, -1, 1, -1], dtype=np.int8))
+    slab["c"] = np.array([1.0, 0, 0, 0], dtype=np.complex128)
+    Iz = oracle.intensity(oracle.layer_grid(x=np.array([0.3, 1.1]), y=np.array([0.2]), z=np.array([0.0, t]), **slab))
+    A = oracle.absorbance(oracle.window_sum(Iz)[1], oracle.window_sum(Iz)[0])
+    assert abs(A - 2 * (2 * np.pi / lam) * n_slab.imag * t * np.log10(np.e)) < 1e-12
+    assert abs(oracle.band_absorbance([3.0, 3.0], [6.0, 6.0]) - np.log10(2.0)) < 1e-15
+    assert abs(oracle.band_absorbance([1.0, 4.0], [2.0, 4.0], w=[1.0, 0.5]) + np.log10(3.0 / 4.0)) < 1e-15
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("dtype,tol", [(np.complex64, 4e-4), (np.complex128, 2e-10)])
+@pytest.mark.parametrize("want_I", [True, False])
+def test_detector_window_sums_and_absorbance(scw, dtype, tol, want_I):
+    """scw_sweep_detector: window sums (with and without the per-sample intensity) against oracle.window_sum of Tier A /
+    Tier B intensities, ragged grid spanning several output tiles, two instances; then scw_absorbance against the oracle."""
+    import torch
+    cfg = si.CONFIGS[0]
+    lays = [si.make_layer(cfg, dtype=dtype), si.make_layer(cfg, dtype=dtype, lam_index=0, layer=0)]
+    lays[1] = dict(lays[1], c=(lays[1]["c"] * 0.5).astype(dtype))
+    g = np.random.default_rng(3)
+    Nx, Ny, Fz = 150, 140, 3
+    x, y = np.sort(g.uniform(0, 8, Nx)), np.sort(g.uniform(0, 8, Ny))
+    zs = [np.linspace(0.1, 1.8, Fz), np.linspace(0.0, 2.0, Fz)]
+    win = (17, 141, 5, 133)
+    ctx = scw.Context(0)
+    try:
+        Ls = [scw.Layer.from_numpy(d, "cuda") for d in lays]
+        I, S = scw.scw_sweep_detector(ctx, Ls, [dev(z) for z in zs], dev(x), dev(y), window=win, want_I=want_I)
+        _, S_all = scw.scw_sweep_detector(ctx, Ls, [dev(z) for z in zs], dev(x), dev(y), want_I=False)
+        torch.cuda.synchronize()
+        assert (I is None) == (not want_I)
+        refs = []
+        for i in range(2):
+            Iref = oracle.intensity(oracle.tier_b_grid(x=x, y=y, z=zs[i], **lays[i]))
+            Sref, Sref_all = oracle.window_sum(Iref, win), oracle.window_sum(Iref)
+            refs.append(Sref)
+            assert np.abs(S[i].cpu().numpy() - Sref).max() / Sref.max() <= tol
+            assert np.abs(S_all[i].cpu().numpy() - Sref_all).max() / Sref_all.max() <= tol
+            if want_I:
+                assert np.abs(I[i].cpu().numpy() - Iref).max() / Iref.max() <= tol
+        w = torch.tensor([1.0, 0.5, 2.0], dtype=S[0].dtype, device="cuda")
+        A, band = scw.scw_absorbance(ctx, S[1], S[0], w=w, want_band=True)
+        torch.cuda.synchronize()
+        Aref = oracle.absorbance(refs[1], refs[0])
+        assert np.abs(A.cpu().numpy() - Aref).max() <= 10 * tol
+        assert abs(float(band) - oracle.band_absorbance(refs[1], refs[0], w=[1.0, 0.5, 2.0])) <= 10 * tol
+    finally:
+        ctx.close()
+
+
+@pytest.mark.gpu
+def test_detector_errors(scw):
+    import torch
+    cfg = si.CONFIGS[0]
+    lay = si.make_layer(cfg, dtype=np.complex64)
+    x, y, z = si.grid_coords(cfg, 0, planes=2, Nx=16, Ny=12)
+    ctx = scw.Context(0)
+    try:
+        L = scw.Layer.from_numpy(lay, "cuda")
+        for bad in [(0, 0, 0, 12), (0, 17, 0, 12), (-1, 4, 0, 12), (0, 16, 5, 5), (0, 16, 0, 13)]:
+            with pytest.raises(scw.ScwError) as e:
+                scw.scw_sweep_detector(ctx, [L], [dev(z)], dev(x), dev(y), window=bad)
+            assert e.value.status == 2
+        with pytest.raises(scw.ScwError) as e:
+            scw.scw_sweep_detector(ctx, [L], [dev(z)], dev(x), dev(y), want_I=False, want_S=False)
+        assert e.value.status == 1
+        torch.cuda.synchronize()
+    finally:
+        ctx.close()
