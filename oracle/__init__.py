@@ -275,3 +275,47 @@ def band_absorbance(S, S0, w=None):
     S, S0 = np.asarray(S, dtype=np.float64), np.asarray(S0, dtype=np.float64)
     w = np.ones_like(S) if w is None else np.asarray(w, dtype=np.float64)
     return float(-np.log10((w * S).sum() / (w * S0).sum()))
+
+
+# ----------------------------------------------------------------------------- V builder (NEXT-2, eq. 33)
+def wrap_index(U, Vn, m, mp):
+    """m (-) m': index of the frequency (u - u', v - v') wrapped back onto the U x Vn grid of eq. 6 (DESIGN.md reading
+    c-20: the "m - m'" of eq. 33 is a difference of frequency VECTORS, and the circulant of eq. 21, PAPER.md:198-212,
+    wraps it per axis -- a block-circulant matrix with circulant blocks)."""
+    u, v = index_map(U, Vn, m)
+    up, vp = index_map(U, Vn, mp)
+    du = (u - up + U // 2) % U - U // 2
+    dv = (v - vp + Vn // 2) % Vn - Vn // 2
+    return (dv + Vn // 2) * U + du + U // 2
+
+
+def build_V(*, U, Vn, X, Y, lam, Q, psi, alpha=None):
+    """V = T Q [diag(alpha)]: the map from the eigenvector matrix Q [J, ldQ >= 4M] (column-major
+    [4M x J], rows P_x, P_y, B_x, B_y in blocks of M, eq. 19-20) to the plane-wave amplitudes [P_x; P_y; P_z]:
+    the P_x, P_y rows are copied, and eq. 33 gives the z component,
+
+        [P_z]_m = + sum_{m'} psi_{m'} { [s_y]_{m-m'} [b_x]_{m-m'} - [s_x]_{m-m'} [b_y]_{m-m'} },
+
+    one (m, m') term at a time.  Sign: + (reading c-19: the printed minus comes from a curl written with the opposite sign
+    at PAPER.md:344 and breaks s.p = 0, eq. 14); psi_m are the Fourier-series coefficients of 1/n^2 on the grid of eq. 6,
+    1/n^2(r) = sum_m psi_m exp(ik s_m.r) (reading c-21), s_m = lam (u/X, v/Y).  Returns V [J, 3M] (column-major [3M x J])."""
+    M = U * Vn
+    Q = np.asarray(Q)
+    J = Q.shape[0]
+    psi = np.asarray(psi, dtype=np.complex128)
+    assert Q.shape[1] >= 4 * M and psi.shape == (M,)
+    Qc = Q[:, :4 * M].astype(np.complex128)
+    sx = np.empty(M)
+    sy = np.empty(M)
+    for m in range(M):
+        u, v = index_map(U, Vn, m)
+        sx[m], sy[m] = lam * u / X, lam * v / Y                      # eq. 6
+    q = sy[None, :] * Qc[:, 2 * M:3 * M] - sx[None, :] * Qc[:, 3 * M:4 * M]       # [J, M]: s_y b_x - s_x b_y per column
+    V = np.zeros((J, 3 * M), dtype=np.complex128)
+    V[:, :2 * M] = Qc[:, :2 * M]
+    for m in range(M):
+        for mp in range(M):
+            V[:, 2 * M + m] += psi[mp] * q[:, wrap_index(U, Vn, m, mp)]
+    if alpha is not None:
+        V *= np.asarray(alpha, dtype=np.complex128)[:, None]
+    return V
