@@ -424,6 +424,25 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
         ns = planes * cfgx.Nx * cfgx.Ny
         extra[name] = dict(ms_per_call=ms, samples_per_s=ns / (ms * 1e-3), orders=cfgx.U * cfgx.Vn, planes=planes,
                            hbm_write_frac=ns * 24 / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
+    # NEXT-2 V builder (eq. 33) at config-1 shape: V = T Q, an M x M by M x 4M complex GEMM (BF16x3 on tcgen05) + row copy
+    c1s = si.CONFIGS[1]
+    M1 = c1s.U * c1s.Vn
+    gq = torch.Generator(device=device).manual_seed(7293)
+    Qd = torch.view_as_complex(torch.randn((4 * M1, 4 * M1, 2), generator=gq, device=device) / (8 * M1) ** 0.5)
+    psid = torch.view_as_complex(torch.randn((M1, 2), generator=gq, device=device) / (2 * M1) ** 0.5)
+    Vout = torch.empty((4 * M1, 3 * M1), dtype=torch.complex64, device=device)
+    vb = lambda: scw.scw_build_V(ctx, U=c1s.U, Vn=c1s.Vn, X=c1s.L, Y=c1s.L, lam=1.0, Q=Qd, psi=psid, out=Vout)
+    ms = time_steps(torch, vb, args.steps, args.warmup)
+    useful = 8 * M1 * M1 * 4 * M1 / (ms * 1e-3) / 1e12
+    qbytes = (Qd.numel() + Vout.numel()) * 8
+    extra["vbuild_config1_shape"] = dict(
+        ms_per_call=ms, modes_per_s=4 * M1 / (ms * 1e-3),
+        roofline=dict(bound="tensor", achieved=3 * useful, peak=peaks["bf16_tflops_sustained"], unit="TFLOP/s executed (BF16x3)",
+                      frac=3 * useful / peaks["bf16_tflops_sustained"], useful_tflops=useful,
+                      hbm_frac=qbytes / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"], traffic=None,
+                      note="reads Q once (152 MB), writes V (114 MB); 41 GF useful"))
+    del Qd, psid, Vout
+    torch.cuda.empty_cache()
     if not args.skip_large:
         c1, layers, zs1, x1, y1 = config1_inputs(np.complex128)
         Ls = [scw.Layer.from_numpy(d, device) for d in layers]

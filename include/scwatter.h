@@ -303,6 +303,35 @@ int32_t scw_sweep_intensity_workspace(scw_ctx* ctx, int64_t n_inst, const scw_la
 int32_t scw_absorbance(scw_ctx* ctx, int32_t dtype, int64_t n, const void* S, const void* S0, const void* w, void* A,
                        void* band);
 
+/* ---------------------------------------------------------------- V builder
+ *
+ * The step upstream of the field evaluation: from the eigenvector matrix Q of a layer's property matrix (eq. 19-23,
+ * PAPER.md:184-246; rows [P_x; P_y; B_x; B_y] in blocks of M, one column per mode) to the matrix V = T Q [diag(alpha)]
+ * of scw_layer.  The P_x, P_y rows are copied; the P_z rows follow from eq. 33:
+ *     [P_z]_m = + sum_{m'} psi_{m'} { [s_y]_{m-m'} [b_x]_{m-m'} - [s_x]_{m-m'} [b_y]_{m-m'} },   s_m = lambda (u/X, v/Y),
+ * the 2-D circular convolution (per-axis wrap of the frequency difference onto the grid of eq. 6; the block-circulant
+ * form of the matrix printed as eq. 21) of q = s_y o B_x - s_x o B_y with the Fourier-series coefficients psi of 1/n^2,
+ * 1/n^2(r) = sum_m psi_m exp(ik s_m . r) (eq. 12 with that normalisation: a homogeneous layer has psi = delta_{(0,0)} / n^2).
+ * The sign is + : with B = s x P (eq. 15, and eq. 21's D) only this sign gives s . p = 0 (eq. 14); the minus printed in
+ * eq. 33 comes from the curl written with the opposite sign at PAPER.md:344 (readings c-19..c-21).
+ * Runs as an M x M by M x J complex GEMM on the tensor cores.  V: [ldV x J] column-major complex<dtype>, ldV >= 3M.
+ * Errors: NULL, SHAPE, DTYPE, ALIGN, VALUE, WORKSPACE, CUDA.
+ */
+typedef struct {
+    uint32_t struct_size;      /* = sizeof(scw_vbuild) */
+    int32_t dtype;             /* SCW_C64 | SCW_C128: element type of Q, psi, alpha, V */
+    int32_t U, Vn;             /* frequency grid (eq. 6) */
+    double X, Y;               /* patch size */
+    double lambda;             /* vacuum wavelength */
+    int64_t J;                 /* columns of Q (modes), normally 4*U*Vn */
+    const void* Q;             /* [ldQ x J] column-major complex<dtype>, rows [P_x; P_y; B_x; B_y] (eq. 19-20) */
+    int64_t ldQ;               /* >= 4*U*Vn */
+    const void* psi;           /* [M] complex<dtype>, index m of eq. 6 */
+    const void* alpha;         /* [J] complex<dtype> or NULL: fold diag(alpha) into V (then pass c = NULL to the evaluation) */
+} scw_vbuild;
+int32_t scw_build_V(scw_ctx* ctx, const scw_vbuild* vb, void* V, int64_t ldV);
+int32_t scw_build_V_workspace(scw_ctx* ctx, const scw_vbuild* vb, size_t* bytes);
+
 /* ---------------------------------------------------------------- roofline denominators (measurement helper)
  *
  * Runs a small microbenchmark of one hardware unit on the ctx stream and returns its measured rate (best of `reps`

@@ -31,7 +31,7 @@ EXPORTS = [
     "scw_exterior_spectra", "scw_exterior_points", "scw_exterior_points_workspace",
     "scw_sweep_intensity", "scw_sweep_intensity_workspace",
     "scw_measure_peak", "scw_invalidate_cache", "scw_calibrate", "scw_profile_assembly",
-    "scw_sweep_detector", "scw_sweep_detector_workspace", "scw_absorbance",
+    "scw_sweep_detector", "scw_sweep_detector_workspace", "scw_absorbance", "scw_build_V", "scw_build_V_workspace",
 ]
 SCW_PEAKS = {"fp64_dmma_tflops": 0, "fp32_fma_tflops": 1, "mufu_gops": 2, "hbm_read_gbs": 3, "hbm_write_gbs": 4,
              "hbm_write_tma_gbs": 5}
@@ -42,6 +42,12 @@ class scw_exterior(Structure):
     _fields_ = [("struct_size", c_uint32), ("dtype", c_int32), ("side", c_int32), ("U", c_int32), ("Vn", c_int32),
                 ("X", c_double), ("Y", c_double), ("lambda_", c_double), ("n_re", c_double), ("n_im", c_double),
                 ("z_face", c_double), ("z_inc", c_double), ("p_face", c_void_p), ("p_inc", c_void_p)]
+
+
+class scw_vbuild(Structure):
+    _fields_ = [("struct_size", c_uint32), ("dtype", c_int32), ("U", c_int32), ("Vn", c_int32), ("X", c_double),
+                ("Y", c_double), ("lambda_", c_double), ("J", c_int64), ("Q", c_void_p), ("ldQ", c_int64), ("psi", c_void_p),
+                ("alpha", c_void_p)]
 
 
 class scw_window(Structure):
@@ -121,6 +127,8 @@ def lib():
         L.scw_sweep_detector.argtypes = L.scw_sweep_wavelengths.argtypes + [POINTER(scw_window), POINTER(c_void_p)]
         L.scw_sweep_detector_workspace.argtypes = L.scw_sweep_workspace.argtypes
         L.scw_absorbance.argtypes = [c_void_p, c_int32, c_int64, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
+        L.scw_build_V.argtypes = [c_void_p, POINTER(scw_vbuild), c_void_p, c_int64]
+        L.scw_build_V_workspace.argtypes = [c_void_p, POINTER(scw_vbuild), POINTER(c_size_t)]
         L.scw_invalidate_cache.argtypes = [c_void_p]
         L.scw_profile_assembly.argtypes = [c_void_p, c_int32, POINTER(c_double), POINTER(c_int32)]
         L.scw_calibrate.argtypes = L.scw_sweep_wavelengths.argtypes + [c_int32]
@@ -471,6 +479,22 @@ def scw_absorbance(ctx, S, S0, w=None, want_band=False):
     band = torch.empty((1,), dtype=S.dtype, device=S.device) if want_band else None
     ctx.check(ctx.L.scw_absorbance(ctx._h, dt, S.numel(), _p(S), _p(S0), _p(w), _p(A), _p(band)))
     return (A, band) if want_band else A
+
+
+def scw_build_V(ctx, *, U, Vn, X, Y, lam, Q, psi, alpha=None, out=None, ldV=None):
+    """V = T Q [diag(alpha)] (eq. 33): Q (J, ldQ) complex (column-major [ldQ x J], rows P_x, P_y, B_x, B_y), psi (M,),
+    alpha (J,) or None.  Returns V as a (J, ldV) tensor (column-major [ldV x J])."""
+    J, ldQ = Q.shape
+    M = U * Vn
+    vb = scw_vbuild(ctypes.sizeof(scw_vbuild), _dt(Q), U, Vn, X, Y, lam, J, Q.data_ptr(), ldQ, psi.data_ptr(),
+                    None if alpha is None else alpha.data_ptr())
+    need = c_size_t()
+    ctx.check(ctx.L.scw_build_V_workspace(ctx._h, byref(vb), byref(need)))
+    ctx.reserve(need.value)
+    if out is None:
+        out = torch.zeros((J, 3 * M if ldV is None else ldV), dtype=Q.dtype, device=ctx.device)
+    ctx.check(ctx.L.scw_build_V(ctx._h, byref(vb), _p(out), out.shape[1]))
+    return out
 
 
 def scw_sweep_wavelengths_host(ctx, layers, zs, x, y, out=None):

@@ -328,7 +328,7 @@ const char* scw_profile_name(int32_t kc)
     static const char* names[KC_COUNT] = {"mode_weights", "twiddles", "simt_assemble", "reduce_splits", "simt_synth_a",
                                           "simt_synth_b", "points_table", "points_planewave", "point_synth", "misc",
                                           "tc_assemble", "tc_synth", "tc_synth_images", "dmma_assemble", "dmma_synth_a",
-                                          "dmma_synth_b", "exterior"};
+                                          "dmma_synth_b", "exterior", "vbuild_prepare"};
     return (kc >= 0 && kc < KC_COUNT) ? names[kc] : nullptr;
 }
 
@@ -1064,6 +1064,46 @@ int32_t scw_exterior_points(scw_ctx* ctx, const scw_exterior* ext, int64_t N, co
     if (int32_t s = need_ws(ctx, exterior_points_bytes(ext), "scw_exterior_points")) return s;
     launch_exterior_points(ctx, ext, N, r, E, ctx->ws);
     return check_launch(ctx, "scw_exterior_points");
+}
+
+// ------------------------------------------------------------------------------------------
+static int32_t check_vbuild(scw_ctx* ctx, const scw_vbuild* vb, const char* who)
+{
+    if (!vb) return fail(ctx, SCW_ERR_NULL, "%s: descriptor is NULL", who);
+    if (vb->struct_size != sizeof(scw_vbuild)) return fail(ctx, SCW_ERR_SHAPE, "%s: vbuild.struct_size mismatch", who);
+    if (vb->dtype != SCW_C64 && vb->dtype != SCW_C128) return fail(ctx, SCW_ERR_DTYPE, "%s: bad dtype %d", who, vb->dtype);
+    if (vb->U <= 0 || vb->Vn <= 0 || vb->U > MAX_FREQ || vb->Vn > MAX_FREQ)
+        return fail(ctx, SCW_ERR_SHAPE, "%s: U=%d Vn=%d out of range", who, vb->U, vb->Vn);
+    if (vb->J <= 0) return fail(ctx, SCW_ERR_SHAPE, "%s: J must be positive", who);
+    if (vb->ldQ < 4LL * vb->U * vb->Vn) return fail(ctx, SCW_ERR_SHAPE, "%s: ldQ=%lld < 4*U*Vn", who, (long long)vb->ldQ);
+    if (!finite_pos(vb->X) || !finite_pos(vb->Y) || !finite_pos(vb->lambda))
+        return fail(ctx, SCW_ERR_VALUE, "%s: X, Y and lambda must be finite and > 0", who);
+    if (!vb->Q || !vb->psi) return fail(ctx, SCW_ERR_NULL, "%s: Q and psi are required", who);
+    const size_t es = esize(vb->dtype);
+    if (!aligned(vb->Q, es) || !aligned(vb->psi, es) || (vb->alpha && !aligned(vb->alpha, es)))
+        return fail(ctx, SCW_ERR_ALIGN, "%s: Q/psi/alpha misaligned", who);
+    return SCW_OK;
+}
+
+int32_t scw_build_V_workspace(scw_ctx* ctx, const scw_vbuild* vb, size_t* bytes)
+{
+    if (!ctx || !bytes) return SCW_ERR_NULL;
+    ctx->msg[0] = 0;
+    if (int32_t s = check_vbuild(ctx, vb, "scw_build_V_workspace")) return s;
+    *bytes = vbuild_scratch(ctx, vb);
+    return SCW_OK;
+}
+
+int32_t scw_build_V(scw_ctx* ctx, const scw_vbuild* vb, void* V, int64_t ldV)
+{
+    if (int32_t s = check_ctx(ctx)) return s;
+    if (int32_t s = check_vbuild(ctx, vb, "scw_build_V")) return s;
+    if (!V) return fail(ctx, SCW_ERR_NULL, "scw_build_V: V is required");
+    if (ldV < 3LL * vb->U * vb->Vn) return fail(ctx, SCW_ERR_SHAPE, "scw_build_V: ldV=%lld < 3*U*Vn", (long long)ldV);
+    if (!aligned(V, esize(vb->dtype))) return fail(ctx, SCW_ERR_ALIGN, "scw_build_V: V misaligned");
+    if (int32_t s = need_ws(ctx, vbuild_scratch(ctx, vb), "scw_build_V")) return s;
+    launch_vbuild(ctx, vb, V, ldV, ctx->ws);
+    return check_launch(ctx, "scw_build_V");
 }
 
 }  // extern "C"

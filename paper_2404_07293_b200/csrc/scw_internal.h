@@ -10,7 +10,7 @@ namespace scw {
 // Kernel classes for launch accounting and the optional per-kernel CUDA-event timers.
 enum KernelClass {
     KC_WEIGHTS = 0, KC_TWIDDLES, KC_ASSEMBLE, KC_REDUCE, KC_SYNTH_A, KC_SYNTH_B, KC_POINTS_TABLE, KC_POINTS,
-    KC_POINT_SYNTH, KC_MISC, KC_ASSEMBLE_TC, KC_SYNTH_TC, KC_SYNTH_IMG, KC_ASSEMBLE_DMMA, KC_SYNTH_A_DMMA, KC_SYNTH_B_DMMA, KC_EXTERIOR, KC_COUNT
+    KC_POINT_SYNTH, KC_MISC, KC_ASSEMBLE_TC, KC_SYNTH_TC, KC_SYNTH_IMG, KC_ASSEMBLE_DMMA, KC_SYNTH_A_DMMA, KC_SYNTH_B_DMMA, KC_EXTERIOR, KC_VBUILD_PREP, KC_COUNT
 };
 struct ProfRec { cudaEvent_t a, b; int kc; bool owns_a; };
 }  // namespace scw
@@ -151,6 +151,14 @@ void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, i
                               const TcFixup& fix, int* sched, int n_sched, void* scratch, bool ctl_clean);
 void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z, void* P, int64_t ldP,
                         void* scratch);
+// Generic complex64 GEMM on the assembly kernel (BF16x3 tcgen05): C [ldC x N] col-major = A [ldA x K] col-major (R rows,
+// 16-byte aligned) . B [K x N] row-major; scratch = tc_assemble_scratch(ctx, R, K, N, 1).
+void launch_tc_gemm(scw_ctx* ctx, int64_t R, int64_t K, int64_t N, const void* A, int64_t ldA, const void* B, void* C,
+                    int64_t ldC, void* scratch);
+
+// ---- scw_vbuild.cu: V = T Q diag(alpha), eq. 33 (NEXT-2) -------------------------------------------------------
+size_t vbuild_scratch(const scw_ctx* ctx, const scw_vbuild* vb);
+void launch_vbuild(scw_ctx* ctx, const scw_vbuild* vb, void* V, int64_t ldV, void* scratch);
 
 // Detector reductions of a sweep (NEXT-3): what leaves the synthesis instead of the complex field.
 struct TcDetector {

@@ -69,6 +69,8 @@ struct TaParams {
     const int8_t* dir[TA_MAX_INST];
     const double* z[TA_MAX_INST];
     double inv_lambda[TA_MAX_INST], z_lo[TA_MAX_INST], z_hi[TA_MAX_INST];
+    const float2* wsrc;     // not NULL (single instance): the small operand is GIVEN, row-major [J x Fz] complex64, instead of
+                            // generated from gamma (generic complex GEMM C = V B; used by the V builder, eq. 33)
     int64_t span0[TA_MAX_CTAS + 1];     // CTA c owns iterations [span0[c], span0[c+1])
     int n_inst;
     int64_t J, Fz;
@@ -137,6 +139,26 @@ __device__ __forceinline__ void ta_weight_unit(const TaParams& p, int64_t tile_i
     const int Fzt = p.Fzt, N2 = p.N2;
     uint8_t* tile = p.Wt + (size_t)tile_id * (size_t)N2 * 128;
     const int e2 = lane & 3, nn = lane >> 2;
+    if (p.wsrc) {                                      // given operand: element (mode j, column i) = wsrc[j*Fz + i]
+        const size_t lo_ = (size_t)N2 * 64;
+        uint8_t* base_ = tile + (size_t)c4 * (N2 * 16) + nn * 16 + e2 * 4;
+        const int64_t j0 = ta_mode(kb, 8 * c4 + 2 * e2), j1 = ta_mode(kb, 8 * c4 + 2 * e2 + 1);
+        for (int o = 0; nn + 8 * o < Fzt; ++o) {
+            const int64_t i = (int64_t)nt * Fzt + nn + 8 * o;
+            const bool in = i < p.Fz;
+            const float2 w0 = (in && j0 < p.J) ? p.wsrc[j0 * p.Fz + i] : make_float2(0.f, 0.f);
+            const float2 w1 = (in && j1 < p.J) ? p.wsrc[j1 * p.Fz + i] : make_float2(0.f, 0.f);
+            uint32_t rh, rl, ih, il;
+            split_bf16x2(w0.x, w1.x, rh, rl);
+            split_bf16x2(w0.y, w1.y, ih, il);
+            uint8_t* dst = base_ + o * 128;
+            *reinterpret_cast<uint32_t*>(dst) = rh;
+            *reinterpret_cast<uint32_t*>(dst + Fzt * 16) = ih;
+            *reinterpret_cast<uint32_t*>(dst + lo_) = rl;
+            *reinterpret_cast<uint32_t*>(dst + lo_ + Fzt * 16) = il;
+        }
+        return;
+    }
     // per mode: phase (turns) = pa z + pb, log2 amplitude = ka z + kb  (fp64: z may be far from zref)
     double pa[2], pb[2], ka[2], kb2[2];
     float cr[2], ci[2];
@@ -833,12 +855,11 @@ void tc_assemble_ctl(const scw_ctx* ctx, int64_t R, int64_t J, int64_t Fz, int n
 // weights (a-1) + stream-K assembly (a-2) + fix-up of a group of n_inst <= TA_MAX_INST instances with equal U, Vn, J, Fz:
 // ONE launch.  ctl_clean: the control block is known to hold zeros (a kernel launched before in this call zeroed it, or
 // the previous launch left it clean); otherwise it is cleared with a memset node first.
-void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
-                              const TcFixup& fix, int* sched, int n_sched, void* scratch, bool ctl_clean)
+// Shared by the spectral assembly and the generic GEMM: everything but the per-instance operands.
+static void ta_launch(scw_ctx* ctx, int n_inst, int64_t R, int64_t J, int64_t Fz, const scw_layer* inst, const double* const* z,
+                      const float2* wsrc, const TcFixup& fix, int* sched, int n_sched, void* scratch, bool ctl_clean)
 {
-    const scw_layer& L0 = inst[0];
-    const int64_t R = 3LL * L0.U * L0.Vn;
-    const TaPlan pl = ta_plan(ctx, R, L0.J, Fz, n_inst);
+    const TaPlan pl = ta_plan(ctx, R, J, Fz, n_inst);
     int* ctl = static_cast<int*>(scratch);
     uint8_t* Wt = static_cast<uint8_t*>(scratch) + ta_ctl_bytes(pl);
     float* part = reinterpret_cast<float*>(Wt + align_up(pl.wt_bytes * n_inst));
@@ -848,20 +869,21 @@ void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, i
         p.c[i] = (const float2*)inst[i].c;
         p.gamma[i] = (const double2*)inst[i].gamma;
         p.dir[i] = inst[i].dir;
-        p.z[i] = z[i];
+        p.z[i] = z ? z[i] : nullptr;
         p.inv_lambda[i] = 1.0 / inst[i].lambda;
         p.z_lo[i] = inst[i].z_lo;
         p.z_hi[i] = inst[i].z_hi;
-        maps_ok = maps_ok && ta_make_map(&p.tmap[i][0], inst[i].V, inst[i].ldV, R, L0.J, 0, nullptr) &&
-                  ta_make_map(&p.tmap[i][1], inst[i].V, inst[i].ldV, R, L0.J, 1, &p.xoff1[i]);
+        maps_ok = maps_ok && ta_make_map(&p.tmap[i][0], inst[i].V, inst[i].ldV, R, J, 0, nullptr) &&
+                  ta_make_map(&p.tmap[i][1], inst[i].V, inst[i].ldV, R, J, 1, &p.xoff1[i]);
     }
     if (!maps_ok) {                                 // reported by the entry point's check_launch
         ctx->tc_error = true;
         return;
     }
+    p.wsrc = wsrc;
     for (int c = 0; c <= pl.G; ++c) p.span0[c] = pl.span0[c];
     p.n_inst = n_inst;
-    p.J = L0.J;
+    p.J = J;
     p.Fz = Fz;
     p.Wt = Wt;
     p.part = part;
@@ -891,6 +913,28 @@ void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, i
     ctx->last_asm_G = pl.G;
     ctx->last_asm_ns = p.cta_ns;
     for (int c = 0; c <= pl.G; ++c) ctx->last_asm_span0[c] = pl.span0[c];
+}
+
+void launch_tc_assemble_group(scw_ctx* ctx, int n_inst, const scw_layer* inst, int64_t Fz, const double* const* z,
+                              const TcFixup& fix, int* sched, int n_sched, void* scratch, bool ctl_clean)
+{
+    ta_launch(ctx, n_inst, 3LL * inst[0].U * inst[0].Vn, inst[0].J, Fz, inst, z, nullptr, fix, sched, n_sched, scratch, ctl_clean);
+}
+
+// Generic complex64 GEMM on the same kernel: C [ldC x N] (column-major) = A [ldA x K] (column-major, R rows) . B [K x N]
+// (row-major).  A must be 16-byte aligned; scratch = tc_assemble_scratch(ctx, R, K, N, 1).
+void launch_tc_gemm(scw_ctx* ctx, int64_t R, int64_t K, int64_t N, const void* A, int64_t ldA, const void* B, void* C,
+                    int64_t ldC, void* scratch)
+{
+    scw_layer L = {};
+    L.V = A;
+    L.ldV = ldA;
+    L.lambda = 1.0;
+    TcFixup fix = {};
+    fix.mode = TC_FIX_P;
+    fix.P = static_cast<float2*>(C);
+    fix.ldP = ldC;
+    ta_launch(ctx, 1, R, K, N, &L, nullptr, static_cast<const float2*>(B), fix, nullptr, 0, scratch, false);
 }
 
 void launch_tc_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z, void* P, int64_t ldP,

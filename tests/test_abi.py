@@ -21,7 +21,7 @@ def declared_symbols():
     for h in glob.glob(os.path.join(ROOT, "include", "*.h")):
         src = open(h).read()
         src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-        names |= set(re.findall(r"\b(scw_[a-z_0-9]+)\s*\(", src))
+        names |= set(re.findall(r"\b(scw_[A-Za-z_0-9]+)\s*\(", src))
     return sorted(names)
 
 

@@ -114,3 +114,70 @@ def test_bruteforce_pairs_on_3x3():
                         md, mp = (dv + 1) * 3 + du + 1, (vp + 1) * 3 + up + 1
                         acc += psi[mp] * (0.9 * dv / 2.5 * Q[j, 2 * M + md] - 0.9 * du / 2.0 * Q[j, 3 * M + md])
                 assert abs(V[j, 2 * M + (v + 1) * 3 + u + 1] - acc) < 1e-14
+
+
+# ------------------------------------------------------------------------------------------------ GPU
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("path", ["auto", "simt"])
+@pytest.mark.parametrize("dtype,tol", [(np.complex64, 2e-4), (np.complex128, 1e-10)])
+@pytest.mark.parametrize("U,Vn,J,pad,with_alpha", [(3, 3, 36, 0, False), (9, 9, 324, 3, True), (12, 7, 100, 1, True)])
+def test_build_V_every_entry(dtype, tol, U, Vn, J, pad, with_alpha, path):
+    """scw_build_V against oracle.build_V, every entry: odd / even grids, J != 4M, padded ldQ / ldV, alpha folded or not;
+    complex64 on the tcgen05 GEMM where a tile fits (M >= 64), complex128 on DMMA, both on CUDA cores ("simt")."""
+    import torch
+    import paper_2404_07293_b200 as scw
+    M = U * Vn
+    Q, psi = random_Q(U, Vn, J, seed=U * 10 + Vn, dtype=dtype, pad=pad)
+    g = np.random.default_rng(5)
+    alpha = ((g.standard_normal(J) + 1j * g.standard_normal(J)) / np.sqrt(2)).astype(dtype) if with_alpha else None
+    lam, X, Y = 0.8, 5.0, 4.0
+    ref = oracle.build_V(U=U, Vn=Vn, X=X, Y=Y, lam=lam, Q=Q, psi=psi, alpha=alpha)
+    ctx = scw.Context(0)
+    try:
+        if path == "simt":
+            ctx.set_path(scw.SCW_PATH_SIMT)
+        out = torch.full((J, 3 * M + pad), 7.0, dtype=dev(Q).dtype, device="cuda")
+        V = scw.scw_build_V(ctx, U=U, Vn=Vn, X=X, Y=Y, lam=lam, Q=dev(Q), psi=dev(psi),
+                            alpha=None if alpha is None else dev(alpha), out=out)
+        torch.cuda.synchronize()
+        got = V.cpu().numpy()
+        assert np.all(got[:, 3 * M:] == 7.0)                          # padding rows of V untouched
+        assert np.abs(got[:, :3 * M] - ref).max() / np.abs(ref).max() <= tol
+    finally:
+        ctx.close()
+
+
+@pytest.mark.gpu
+def test_build_V_feeds_the_field_evaluation():
+    """End to end at config-1 shape (33 x 33, J = 4356, complex64): V from scw_build_V (tcgen05 GEMM) equals the oracle's V on
+    sampled columns, and the field evaluated from it equals Tier B evaluated from the oracle's V."""
+    import torch
+    import paper_2404_07293_b200 as scw
+    cfg = si.CONFIGS[1]
+    U, Vn, M = cfg.U, cfg.Vn, cfg.U * cfg.Vn
+    J = 4 * M
+    Q, psi = random_Q(U, Vn, J, seed=77, dtype=np.complex64)
+    lay = si.make_layer(cfg, 0, dtype=np.complex64, with_V=False)
+    ctx = scw.Context(0)
+    try:
+        V = scw.scw_build_V(ctx, U=U, Vn=Vn, X=cfg.L, Y=cfg.L, lam=lay["lam"], Q=dev(Q), psi=dev(psi))
+        torch.cuda.synchronize()
+        cols = np.sort(np.random.default_rng(1).choice(J, 24, replace=False))
+        ref = oracle.build_V(U=U, Vn=Vn, X=cfg.L, Y=cfg.L, lam=lay["lam"], Q=Q[cols], psi=psi)
+        got = V.cpu().numpy()
+        assert np.abs(got[cols] - ref).max() / np.abs(ref).max() <= 2e-4
+        # the field from the built V
+        x, y, z = si.grid_coords(cfg, 0, planes=2, Nx=64, Ny=48)
+        L = scw.Layer(U=U, Vn=Vn, X=cfg.L, Y=cfg.L, lam=lay["lam"], z_lo=lay["z_lo"], z_hi=lay["z_hi"], V=V,
+                      gamma=dev(lay["gamma"]), c=dev(lay["c"]), dir=dev(lay["dir"]))
+        E = scw.scw_sweep_wavelengths(ctx, [L], [dev(z)], dev(x), dev(y))[0]
+        torch.cuda.synchronize()
+        Eref = oracle.tier_b_grid(x=x, y=y, z=z, **dict(lay, V=got))
+        assert np.abs(E.cpu().numpy() - Eref).max() / np.abs(Eref).max() <= 2e-4
+    finally:
+        ctx.close()
