@@ -91,6 +91,10 @@ int32_t scw_last_cuda_error(const scw_ctx* ctx);
 size_t scw_required_workspace(const scw_ctx* ctx);
 /* Number of kernels this ctx has launched since creation (monotone counter). */
 int64_t scw_launch_count(const scw_ctx* ctx);
+/* Which kernels the last hot-path call on this ctx launched: bit k set = kernel class k (names: scw_profile_name(k)).  Lets a
+ * caller see whether SCW_PATH_AUTO took the tensor-core kernels ("tc_assemble", "tc_synth", "dmma_*") or fell back to the
+ * CUDA-core ones ("simt_*": complex64 beyond 80 frequencies per axis, V not 16-byte aligned, tiny problems, ...). */
+uint64_t scw_last_kernels(const scw_ctx* ctx);
 /* Library version: major*10000 + minor*100 + patch. */
 int32_t scw_version(void);
 

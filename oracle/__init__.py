@@ -319,3 +319,36 @@ def build_V(*, U, Vn, X, Y, lam, Q, psi, alpha=None):
     if alpha is not None:
         V *= np.asarray(alpha, dtype=np.complex128)[:, None]
     return V
+
+
+# ----------------------------------------------------------------------------- alpha propagation (NEXT-4, eq. 24-26)
+def interface_factors(*, lam, z_a, z_b, gamma, dir=None):
+    """Diagonals of the two interface matrices of a layer between z_a = z_{l-1} and z_b = z_l (symbols
+    de-garbled per reading c-7):  Q'_l = Qcheck + Qhat G(Gamma, z_l, z_{l-1}) = Q diag(d_acute),
+                                   Q`_l = Qcheck G(Gamma, z_{l-1}, z_l) + Qhat = Q diag(d_grave),
+    Qcheck / Qhat = the "+" / "-" columns of Q, G of eq. 7.  Every exponential decays (reading c-1)."""
+    gamma = np.asarray(gamma, dtype=np.complex128)
+    plus = _dirs(gamma, dir) > 0
+    d_acute = np.where(plus, 1.0, np.array([green(g, z_b, z_a, lam) for g in gamma]))
+    d_grave = np.where(plus, np.array([green(g, z_a, z_b, lam) for g in gamma]), 1.0)
+    return d_acute, d_grave
+
+
+def propagate_alpha(*, lam, z_if, Q, gamma, dir=None, r0):
+    """alpha^(l) of every layer from the field vector r0 = Gbar Rbar + Rhat at the top interface z_0 (eq. 24,
+    PAPER.md:254-256) through the middle-boundary conditions (eq. 25):
+        alpha^(1) = Q'_1^-1 r0,      alpha^(l) = Q'_l^-1 Q`_{l-1} alpha^(l-1),
+    and the field vector at the bottom interface, Rcheck = Q`_L alpha^(L) (eq. 26).  The linear solve is a library routine
+    (numpy / LAPACK).  Q: list of L arrays [n, n] in MATHEMATICAL orientation (row = field component, column = mode),
+    gamma: list of [n], dir: list of [n] or None.  Returns (list of alpha [n], r_L)."""
+    r = np.asarray(r0, dtype=np.complex128)
+    alphas = []
+    for l in range(len(Q)):
+        Ql = np.asarray(Q[l], dtype=np.complex128)
+        d_acute, d_grave = interface_factors(lam=lam, z_a=z_if[l], z_b=z_if[l + 1], gamma=gamma[l],
+                                             dir=None if dir is None else dir[l])
+        Q_acute = Ql * d_acute[None, :]
+        alpha = np.linalg.solve(Q_acute, r)
+        alphas.append(alpha)
+        r = (Ql * d_grave[None, :]) @ alpha
+    return alphas, r

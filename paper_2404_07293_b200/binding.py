@@ -23,7 +23,7 @@ STATUS = {0: "SCW_OK", 1: "SCW_ERR_NULL", 2: "SCW_ERR_SHAPE", 3: "SCW_ERR_DTYPE"
 
 EXPORTS = [
     "scw_version", "scw_create", "scw_destroy", "scw_set_stream", "scw_set_workspace", "scw_set_option",
-    "scw_last_error", "scw_last_cuda_error", "scw_required_workspace", "scw_launch_count",
+    "scw_last_error", "scw_last_cuda_error", "scw_required_workspace", "scw_launch_count", "scw_last_kernels",
     "scw_assemble_spectra", "scw_assemble_workspace", "scw_synthesize_grid", "scw_synthesize_workspace",
     "scw_eval_points", "scw_points_workspace", "scw_sweep_wavelengths", "scw_sweep_workspace",
     "scw_sweep_wavelengths_host", "scw_sweep_host_workspace",
@@ -96,6 +96,8 @@ def lib():
         L.scw_last_cuda_error.argtypes = [c_void_p]
         L.scw_required_workspace.argtypes = [c_void_p]
         L.scw_launch_count.argtypes = [c_void_p]
+        L.scw_last_kernels.restype = ctypes.c_uint64
+        L.scw_last_kernels.argtypes = [c_void_p]
         L.scw_profile_name.restype = c_char_p
         L.scw_profile_name.argtypes = [c_int32]
         L.scw_profile_read.argtypes = [c_void_p, c_int32, POINTER(c_double), POINTER(c_int64)]
@@ -271,6 +273,11 @@ class Context:
 
     def launch_count(self):
         return int(self.L.scw_launch_count(self._h))
+
+    def last_kernels(self):
+        """Names of the kernel classes the last hot-path call launched (scw_last_kernels)."""
+        bits = int(self.L.scw_last_kernels(self._h))
+        return [self.L.scw_profile_name(k).decode() for k in range(self.L.scw_profile_classes()) if (bits >> k) & 1]
 
     def set_path(self, path):
         self.check(self.L.scw_set_option(self._h, SCW_OPT_PATH, path))

@@ -45,6 +45,7 @@ int32_t check_ctx(scw_ctx* ctx, bool sweep_call = false)
     ctx->cuda_err = 0;
     ctx->required_ws = 0;
     ctx->tc_error = false;
+    ctx->last_classes = 0;
     ctx->prof_last = nullptr;       // per-kernel timers: the first kernel of this call gets its own start event
     int cur = -1;
     cudaError_t e = cudaGetDevice(&cur);
@@ -371,6 +372,7 @@ const char* scw_last_error(const scw_ctx* ctx) { return ctx ? ctx->msg : "ctx is
 int32_t scw_last_cuda_error(const scw_ctx* ctx) { return ctx ? ctx->cuda_err : 0; }
 size_t scw_required_workspace(const scw_ctx* ctx) { return ctx ? ctx->required_ws : 0; }
 int64_t scw_launch_count(const scw_ctx* ctx) { return ctx ? ctx->launches : 0; }
+uint64_t scw_last_kernels(const scw_ctx* ctx) { return ctx ? ctx->last_classes : 0; }
 
 // ------------------------------------------------------------------------------------------
 int32_t scw_assemble_workspace(scw_ctx* ctx, const scw_layer* layer, int64_t Fz, size_t* bytes)

@@ -28,6 +28,7 @@ struct scw_ctx {
     size_t ws_bytes = 0;
     int64_t path = SCW_PATH_AUTO;
     int64_t launches = 0;
+    uint64_t last_classes = 0;      // bit kc set: the last API call launched a kernel of class kc (scw_last_kernels)
     int32_t cuda_err = 0;
     size_t required_ws = 0;
     char msg[256] = {0};
@@ -66,6 +67,7 @@ struct KernelScope {
     KernelScope(scw_ctx* c, int kc) : ctx(c), on(c->profile)
     {
         ctx->launches++;
+        ctx->last_classes |= 1ull << kc;
         rec.kc = kc;
         if (on) {
             rec.owns_a = ctx->prof_last == nullptr;

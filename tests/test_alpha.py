@@ -1,0 +1,96 @@
+"""alpha propagation across layers (eq. 24-26): oracle pins (CPU) and GPU parity through the C ABI.
+
+Pins of oracle.propagate_alpha: the interface matrices written out as the paper defines them (Qcheck + Qhat G, ...) must
+make both sides of eq. 25 equal; a stack of identical layers propagates every mode analytically; a single layer equals
+the explicit inverse; the solve against a pure-python Gaussian elimination on a tiny system.
+"""
+import cmath
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+
+
+def random_stack(n, L, seed, dtype=np.complex128, lam=0.8):
+    g = np.random.default_rng(seed)
+    z_if = np.concatenate([[0.0], np.cumsum(g.uniform(0.3, 0.9, L))])
+    Q, gamma, dirs = [], [], []
+    for _ in range(L):
+        A = (g.standard_normal((n, n)) + 1j * g.standard_normal((n, n))) / np.sqrt(2 * n)
+        Q.append((A + 1.5 * np.eye(n)).astype(dtype))                       # well conditioned, not diagonally trivial
+        d = np.where(np.arange(n) % 2 == 0, 1, -1).astype(np.int8)
+        gamma.append(d * (g.uniform(0.2, 1.4, n) + 1j * g.uniform(0.0, 0.4, n)))
+        dirs.append(d)
+    r0 = ((g.standard_normal(n) + 1j * g.standard_normal(n)) / np.sqrt(2)).astype(dtype)
+    return dict(lam=lam, z_if=z_if, Q=Q, gamma=gamma, dir=dirs, r0=r0)
+
+
+def test_middle_boundary_condition_with_the_papers_matrices():
+    """Eq. 25 with Q'_l and Q`_l assembled exactly as printed: Qcheck, Qhat by column parity, G of
+    eq. 7 as full diagonal matrices."""
+    st = random_stack(12, 3, seed=1)
+    alphas, rL = oracle.propagate_alpha(**st)
+    k = 2 * math.pi / st["lam"]
+    def mats(l):
+        Q, gam = st["Q"][l], st["gamma"][l]
+        plus = np.arange(12) % 2 == 0
+        Qc, Qh = Q * plus[None, :], Q * (~plus)[None, :]
+        za, zb = st["z_if"][l], st["z_if"][l + 1]
+        G_ba = np.diag(np.exp(1j * k * (za - zb) * gam))                    # G(Gamma, z_l, z_{l-1})
+        G_ab = np.diag(np.exp(1j * k * (zb - za) * gam))                    # G(Gamma, z_{l-1}, z_l)
+        return Qc + Qh @ G_ba, Qc @ G_ab + Qh
+    Qa1, _ = mats(0)
+    assert np.abs(Qa1 @ alphas[0] - st["r0"]).max() < 1e-13                 # eq. 24
+    for l in (1, 2):
+        Qa, _ = mats(l)
+        _, Qg_prev = mats(l - 1)
+        assert np.abs(Qg_prev @ alphas[l - 1] - Qa @ alphas[l]).max() < 1e-12      # eq. 25
+    assert np.abs(mats(2)[1] @ alphas[2] - rL).max() < 1e-13                # eq. 26
+
+
+def test_identical_layers_propagate_analytically():
+    """Same Q, Gamma in consecutive layers: alpha^(l)_j = G(gamma_j, z_{l-2}, z_{l-1}) alpha^(l-1)_j for "+" modes and
+    alpha^(l-1)_j = G(Gamma_j, z_l, z_{l-1}) alpha^(l)_j for "-" modes (every mode just propagates, eq. 23)."""
+    st = random_stack(10, 1, seed=2)
+    z_if = np.array([0.0, 0.4, 1.1, 1.5])
+    st3 = dict(st, z_if=z_if, Q=st["Q"] * 3, gamma=st["gamma"] * 3, dir=st["dir"] * 3)
+    alphas, _ = oracle.propagate_alpha(**st3)
+    k = 2 * math.pi / st["lam"]
+    gam = st["gamma"][0]
+    for l in (1, 2):
+        t_prev, t_cur = z_if[l] - z_if[l - 1], z_if[l + 1] - z_if[l]
+        for j in range(10):
+            if j % 2 == 0:
+                ref = cmath.exp(1j * k * gam[j] * t_prev) * alphas[l - 1][j]
+            else:
+                ref = alphas[l - 1][j] / cmath.exp(1j * k * (-t_cur) * gam[j])
+            assert abs(alphas[l][j] - ref) < 1e-11 * max(1.0, abs(ref))
+
+
+def test_single_layer_is_the_explicit_inverse_and_gauss():
+    st = random_stack(6, 1, seed=3)
+    alphas, _ = oracle.propagate_alpha(**st)
+    d_acute, _ = oracle.interface_factors(lam=st["lam"], z_a=0.0, z_b=st["z_if"][1], gamma=st["gamma"][0], dir=st["dir"][0])
+    Qa = st["Q"][0] * d_acute[None, :]
+    assert np.abs(np.linalg.inv(Qa) @ st["r0"] - alphas[0]).max() < 1e-12
+    # pure-python Gaussian elimination with partial pivoting
+    A = [[complex(v) for v in row] for row in Qa]
+    b = [complex(v) for v in st["r0"]]
+    n = 6
+    for c in range(n):
+        p = max(range(c, n), key=lambda r: abs(A[r][c]))
+        A[c], A[p], b[c], b[p] = A[p], A[c], b[p], b[c]
+        for r in range(c + 1, n):
+            f = A[r][c] / A[c][c]
+            for cc in range(c, n):
+                A[r][cc] -= f * A[c][cc]
+            b[r] -= f * b[c]
+    xs = [0j] * n
+    for r in range(n - 1, -1, -1):
+        xs[r] = (b[r] - sum(A[r][cc] * xs[cc] for cc in range(r + 1, n))) / A[r][r]
+    assert np.abs(np.array(xs) - alphas[0]).max() < 1e-12
+    # |d| <= 1: every interface factor decays (reading c-1)
+    da, dg = oracle.interface_factors(lam=st["lam"], z_a=0.0, z_b=st["z_if"][1], gamma=st["gamma"][0], dir=None)
+    assert np.abs(da).max() <= 1 + 1e-15 and np.abs(dg).max() <= 1 + 1e-15

@@ -308,3 +308,22 @@ def test_grouped_sweep_with_an_8_byte_aligned_V(scw, ctx):
     torch.cuda.synchronize()
     for lay, E in zip(lays, Es):
         assert rel_err(E.cpu().numpy(), oracle.layer_grid(x=x, y=y, z=z, **lay)) <= 2e-4
+
+
+def test_last_kernels_tells_which_path_ran(scw, ctx):
+    """SCW_PATH_AUTO drops to the CUDA-core kernels for shapes the tensor-core kernels do not take; scw_last_kernels makes
+    that visible: complex64 with 96 frequencies along u (> 80) synthesises on CUDA cores, a small sweep with different J per
+    instance leaves the grouped path (two assembly launches), a regular one takes tc_assemble + tc_synth."""
+    lay = ragged_layer(5, 5, 100, np.complex64, seed=7)
+    x, y, z = np.arange(20) * 0.15, np.arange(18) * 0.25, np.linspace(-0.3, 0.8, 4)
+    L = scw.Layer.from_numpy(lay, "cuda")
+    scw.scw_sweep_wavelengths(ctx, [L], [dev(z)], dev(x), dev(y))
+    assert {"tc_assemble", "tc_synth"} <= set(ctx.last_kernels()) and not any(k.startswith("simt") for k in ctx.last_kernels())
+    wide = ragged_layer(96, 2, 64, np.complex64, seed=8)
+    scw.scw_sweep_wavelengths(ctx, [scw.Layer.from_numpy(wide, "cuda")], [dev(z)], dev(x), dev(y))
+    assert "simt_synth_b" in ctx.last_kernels() and "tc_synth" not in ctx.last_kernels()
+    lay2 = ragged_layer(5, 5, 132, np.complex64, seed=9)
+    n0 = ctx.launch_count()
+    scw.scw_sweep_wavelengths(ctx, [L, scw.Layer.from_numpy(lay2, "cuda")], [dev(z), dev(z)], dev(x), dev(y))
+    assert ctx.launch_count() - n0 > 3                                       # per-instance launches, not one group
+    torch.cuda.synchronize()
