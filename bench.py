@@ -443,6 +443,23 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
                       note="reads Q once (152 MB), writes V (114 MB); 41 GF useful"))
     del Qd, psid, Vout
     torch.cuda.empty_cache()
+    # NEXT-4 alpha propagation (eq. 24-26) at config-1 size: one layer = one 4356 x 4356 complex128 LU + two triangular solves
+    n_a = 4 * M1
+    ga = torch.Generator(device=device).manual_seed(7294)
+    Qa = torch.view_as_complex(torch.randn((n_a, n_a, 2), generator=ga, device=device, dtype=torch.float64) / (2 * n_a) ** 0.5)
+    Qa = Qa + 1.5 * torch.eye(n_a, device=device, dtype=torch.complex128)
+    gma = torch.view_as_complex(torch.rand((n_a, 2), generator=ga, device=device, dtype=torch.float64))
+    r0a = torch.view_as_complex(torch.randn((n_a, 2), generator=ga, device=device, dtype=torch.float64))
+    al = lambda: scw.scw_propagate_alpha(ctx, lam=1.0, z_if=[0.0, 1.5], Q=[Qa], gamma=[gma], r0=r0a)
+    ms = time_steps(torch, al, 3, 1)
+    lu_tf = (8.0 / 3.0) * n_a ** 3 / (ms * 1e-3) / 1e12
+    extra["alpha_propagation_config1_size"] = dict(
+        ms_per_layer=ms, n=n_a,
+        roofline=dict(bound="tensor", achieved=lu_tf, peak=peaks.get("fp64_dmma_tflops"), unit="TFLOP/s (fp64, 8/3 n^3 for the complex LU)",
+                      frac=lu_tf / peaks["fp64_dmma_tflops"] if peaks.get("fp64_dmma_tflops") else None, traffic=None,
+                      note="bound by the 2 grid barriers per column of the cooperative panel kernel, not by the tensor cores"))
+    del Qa, gma, r0a
+    torch.cuda.empty_cache()
     if not args.skip_large:
         c1, layers, zs1, x1, y1 = config1_inputs(np.complex128)
         Ls = [scw.Layer.from_numpy(d, device) for d in layers]

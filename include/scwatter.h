@@ -336,6 +336,36 @@ typedef struct {
 int32_t scw_build_V(scw_ctx* ctx, const scw_vbuild* vb, void* V, int64_t ldV);
 int32_t scw_build_V_workspace(scw_ctx* ctx, const scw_vbuild* vb, size_t* bytes);
 
+/* ---------------------------------------------------------------- alpha propagation
+ *
+ * The coefficient vectors alpha^(l) of every layer of a stack from the field vector at its top interface, by the
+ * boundary conditions of PAPER.md:252-296 (eq. 24-26; interface matrices as de-garbled in DESIGN.md reading c-7):
+ *     alpha^(1) = Q'_1^-1 r_0                         r_0 = Gbar Rbar + Rhat, the field [P_x; P_y; B_x; B_y] at z_0   (eq. 24)
+ *     alpha^(l) = Q'_l^-1 Q`_{l-1} alpha^(l-1)                                                                      (eq. 25)
+ *     r_L       = Q`_L alpha^(L)                      the field at the bottom interface z_L                          (eq. 26)
+ *     Q'_l = Qcheck^(l) + Qhat^(l) G(Gamma^(l), z_l, z_{l-1}),   Q`_l = Qcheck^(l) G(Gamma^(l), z_{l-1}, z_l) + Qhat^(l)
+ * with Qcheck / Qhat the "+" / "-" columns of the eigenvector matrix Q^(l) (dir as in scw_layer) and G of eq. 7.  Per
+ * layer: one dense complex LU (partial pivoting, blocked, trailing updates on the FP64 tensor cores) and two triangular
+ * solves; all arithmetic in fp64, SCW_C64 inputs and outputs are widened / rounded at the boundary.
+ * r0, rL: [n] complex<dtype> (device); alpha: HOST array of n_layers device pointers [n]; rL may be NULL.
+ * A singular Q^(l) gives non-finite alpha (no error is raised: nothing is read back).
+ * Errors: NULL, SHAPE, DTYPE, ALIGN, VALUE, WORKSPACE, UNSUPPORTED (n > 128 x #SMs or > 25 600), CUDA.
+ */
+typedef struct {
+    uint32_t struct_size;          /* = sizeof(scw_stack) */
+    int32_t dtype;                 /* SCW_C64 | SCW_C128: element type of Q, r0, alpha, rL */
+    int32_t n_layers;              /* L */
+    int64_t n;                     /* order of Q: 4M */
+    double lambda;                 /* vacuum wavelength */
+    const double* z_if;            /* HOST [L + 1]: interfaces z_0 <= ... <= z_L */
+    const void* const* Q;          /* HOST [L] device pointers: Q^(l), [ldQ x n] column-major complex<dtype> */
+    int64_t ldQ;                   /* >= n */
+    const double* const* gamma;    /* HOST [L] device pointers: Gamma^(l), [n] complex128 signed (as scw_layer.gamma) */
+    const int8_t* const* dir;      /* HOST [L] device pointers [n] (+1 / -1), or NULL: derive from the sign of gamma */
+} scw_stack;
+int32_t scw_propagate_alpha(scw_ctx* ctx, const scw_stack* st, const void* r0, void* const* alpha, void* rL);
+int32_t scw_propagate_alpha_workspace(scw_ctx* ctx, const scw_stack* st, size_t* bytes);
+
 /* ---------------------------------------------------------------- roofline denominators (measurement helper)
  *
  * Runs a small microbenchmark of one hardware unit on the ctx stream and returns its measured rate (best of `reps`

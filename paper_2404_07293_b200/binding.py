@@ -31,7 +31,7 @@ EXPORTS = [
     "scw_exterior_spectra", "scw_exterior_points", "scw_exterior_points_workspace",
     "scw_sweep_intensity", "scw_sweep_intensity_workspace",
     "scw_measure_peak", "scw_invalidate_cache", "scw_calibrate", "scw_profile_assembly",
-    "scw_sweep_detector", "scw_sweep_detector_workspace", "scw_absorbance", "scw_build_V", "scw_build_V_workspace",
+    "scw_sweep_detector", "scw_sweep_detector_workspace", "scw_absorbance", "scw_build_V", "scw_build_V_workspace", "scw_propagate_alpha", "scw_propagate_alpha_workspace",
 ]
 SCW_PEAKS = {"fp64_dmma_tflops": 0, "fp32_fma_tflops": 1, "mufu_gops": 2, "hbm_read_gbs": 3, "hbm_write_gbs": 4,
              "hbm_write_tma_gbs": 5}
@@ -48,6 +48,12 @@ class scw_vbuild(Structure):
     _fields_ = [("struct_size", c_uint32), ("dtype", c_int32), ("U", c_int32), ("Vn", c_int32), ("X", c_double),
                 ("Y", c_double), ("lambda_", c_double), ("J", c_int64), ("Q", c_void_p), ("ldQ", c_int64), ("psi", c_void_p),
                 ("alpha", c_void_p)]
+
+
+class scw_stack(Structure):
+    _fields_ = [("struct_size", c_uint32), ("dtype", c_int32), ("n_layers", c_int32), ("n", c_int64), ("lambda_", c_double),
+                ("z_if", POINTER(c_double)), ("Q", POINTER(c_void_p)), ("ldQ", c_int64), ("gamma", POINTER(c_void_p)),
+                ("dir", POINTER(c_void_p))]
 
 
 class scw_window(Structure):
@@ -131,6 +137,8 @@ def lib():
         L.scw_absorbance.argtypes = [c_void_p, c_int32, c_int64, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
         L.scw_build_V.argtypes = [c_void_p, POINTER(scw_vbuild), c_void_p, c_int64]
         L.scw_build_V_workspace.argtypes = [c_void_p, POINTER(scw_vbuild), POINTER(c_size_t)]
+        L.scw_propagate_alpha.argtypes = [c_void_p, POINTER(scw_stack), c_void_p, POINTER(c_void_p), c_void_p]
+        L.scw_propagate_alpha_workspace.argtypes = [c_void_p, POINTER(scw_stack), POINTER(c_size_t)]
         L.scw_invalidate_cache.argtypes = [c_void_p]
         L.scw_profile_assembly.argtypes = [c_void_p, c_int32, POINTER(c_double), POINTER(c_int32)]
         L.scw_calibrate.argtypes = L.scw_sweep_wavelengths.argtypes + [c_int32]
@@ -502,6 +510,27 @@ def scw_build_V(ctx, *, U, Vn, X, Y, lam, Q, psi, alpha=None, out=None, ldV=None
         out = torch.zeros((J, 3 * M if ldV is None else ldV), dtype=Q.dtype, device=ctx.device)
     ctx.check(ctx.L.scw_build_V(ctx._h, byref(vb), _p(out), out.shape[1]))
     return out
+
+
+def scw_propagate_alpha(ctx, *, lam, z_if, Q, gamma, r0, dir=None, want_rL=True):
+    """alpha^(l) of every layer (eq. 24-26).  Q: list of (n, ldQ) complex device tensors (column-major [ldQ x n]: row j of
+    the tensor is column j = mode j of Q), gamma: list of (n,) complex128, dir: list of (n,) int8 or None, z_if: L + 1
+    floats (host), r0: (n,) field vector at z_0.  Returns (list of alpha tensors, r_L or None)."""
+    L_ = len(Q)
+    n, ldQ = Q[0].shape
+    zarr = (c_double * (L_ + 1))(*[float(v) for v in z_if])
+    Qp = (c_void_p * L_)(*[q.data_ptr() for q in Q])
+    gp = (c_void_p * L_)(*[g.data_ptr() for g in gamma])
+    dp = None if dir is None else (c_void_p * L_)(*[d.data_ptr() for d in dir])
+    st = scw_stack(ctypes.sizeof(scw_stack), _dt(Q[0]), L_, n, float(lam), zarr, Qp, ldQ, gp, dp)
+    need = c_size_t()
+    ctx.check(ctx.L.scw_propagate_alpha_workspace(ctx._h, byref(st), byref(need)))
+    ctx.reserve(need.value)
+    alphas = [torch.empty((n,), dtype=Q[0].dtype, device=ctx.device) for _ in range(L_)]
+    ap = (c_void_p * L_)(*[a.data_ptr() for a in alphas])
+    rL = torch.empty((n,), dtype=Q[0].dtype, device=ctx.device) if want_rL else None
+    ctx.check(ctx.L.scw_propagate_alpha(ctx._h, byref(st), _p(r0), ap, _p(rL)))
+    return alphas, rL
 
 
 def scw_sweep_wavelengths_host(ctx, layers, zs, x, y, out=None):

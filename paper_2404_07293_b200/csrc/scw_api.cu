@@ -329,7 +329,7 @@ const char* scw_profile_name(int32_t kc)
     static const char* names[KC_COUNT] = {"mode_weights", "twiddles", "simt_assemble", "reduce_splits", "simt_synth_a",
                                           "simt_synth_b", "points_table", "points_planewave", "point_synth", "misc",
                                           "tc_assemble", "tc_synth", "tc_synth_images", "dmma_assemble", "dmma_synth_a",
-                                          "dmma_synth_b", "exterior", "vbuild_prepare"};
+                                          "dmma_synth_b", "exterior", "vbuild_prepare", "alpha_misc", "alpha_lu"};
     return (kc >= 0 && kc < KC_COUNT) ? names[kc] : nullptr;
 }
 
@@ -1106,6 +1106,52 @@ int32_t scw_build_V(scw_ctx* ctx, const scw_vbuild* vb, void* V, int64_t ldV)
     if (int32_t s = need_ws(ctx, vbuild_scratch(ctx, vb), "scw_build_V")) return s;
     launch_vbuild(ctx, vb, V, ldV, ctx->ws);
     return check_launch(ctx, "scw_build_V");
+}
+
+// ------------------------------------------------------------------------------------------
+static int32_t check_stack(scw_ctx* ctx, const scw_stack* st, const char* who)
+{
+    if (!st) return fail(ctx, SCW_ERR_NULL, "%s: descriptor is NULL", who);
+    if (st->struct_size != sizeof(scw_stack)) return fail(ctx, SCW_ERR_SHAPE, "%s: stack.struct_size mismatch", who);
+    if (st->dtype != SCW_C64 && st->dtype != SCW_C128) return fail(ctx, SCW_ERR_DTYPE, "%s: bad dtype %d", who, st->dtype);
+    if (st->n_layers <= 0 || st->n <= 0) return fail(ctx, SCW_ERR_SHAPE, "%s: n_layers and n must be positive", who);
+    if (st->ldQ < st->n) return fail(ctx, SCW_ERR_SHAPE, "%s: ldQ=%lld < n=%lld", who, (long long)st->ldQ, (long long)st->n);
+    if (!finite_pos(st->lambda)) return fail(ctx, SCW_ERR_VALUE, "%s: lambda must be finite and > 0", who);
+    if (!st->z_if || !st->Q || !st->gamma) return fail(ctx, SCW_ERR_NULL, "%s: z_if, Q and gamma are required", who);
+    for (int l = 0; l <= st->n_layers; ++l)
+        if (!std::isfinite(st->z_if[l]) || (l > 0 && st->z_if[l] < st->z_if[l - 1]))
+            return fail(ctx, SCW_ERR_VALUE, "%s: interfaces must be finite and non-decreasing", who);
+    const size_t es = esize(st->dtype);
+    for (int l = 0; l < st->n_layers; ++l) {
+        if (!st->Q[l] || !st->gamma[l]) return fail(ctx, SCW_ERR_NULL, "%s: Q[%d] / gamma[%d] is NULL", who, l, l);
+        if (!aligned(st->Q[l], es) || !aligned(st->gamma[l], 16)) return fail(ctx, SCW_ERR_ALIGN, "%s: Q[%d] / gamma[%d] misaligned", who, l, l);
+    }
+    if (!alpha_supported(ctx, st->n))
+        return fail(ctx, SCW_ERR_UNSUPPORTED, "%s: n=%lld beyond the LU's limit on this device", who, (long long)st->n);
+    return SCW_OK;
+}
+
+int32_t scw_propagate_alpha_workspace(scw_ctx* ctx, const scw_stack* st, size_t* bytes)
+{
+    if (!ctx || !bytes) return SCW_ERR_NULL;
+    ctx->msg[0] = 0;
+    if (int32_t s = check_stack(ctx, st, "scw_propagate_alpha_workspace")) return s;
+    *bytes = alpha_scratch(ctx, st->n);
+    return SCW_OK;
+}
+
+int32_t scw_propagate_alpha(scw_ctx* ctx, const scw_stack* st, const void* r0, void* const* alpha, void* rL)
+{
+    if (int32_t s = check_ctx(ctx)) return s;
+    if (int32_t s = check_stack(ctx, st, "scw_propagate_alpha")) return s;
+    if (!r0 || !alpha) return fail(ctx, SCW_ERR_NULL, "scw_propagate_alpha: r0 and alpha are required");
+    const size_t es = esize(st->dtype);
+    if (!aligned(r0, es) || (rL && !aligned(rL, es))) return fail(ctx, SCW_ERR_ALIGN, "scw_propagate_alpha: r0 / rL misaligned");
+    for (int l = 0; l < st->n_layers; ++l)
+        if (!alpha[l] || !aligned(alpha[l], es)) return fail(ctx, SCW_ERR_NULL, "scw_propagate_alpha: alpha[%d] is NULL or misaligned", l);
+    if (int32_t s = need_ws(ctx, alpha_scratch(ctx, st->n), "scw_propagate_alpha")) return s;
+    launch_propagate_alpha(ctx, st, r0, alpha, rL, ctx->ws);
+    return check_launch(ctx, "scw_propagate_alpha");
 }
 
 }  // extern "C"

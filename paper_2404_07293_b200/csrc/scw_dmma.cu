@@ -32,6 +32,7 @@ struct DgParams {
     int64_t bA1, bA2, bB1, bB2, bC1, bC2;  // batch strides (complex elements)
     int nsplit; int64_t kchunk;            // split k: split s covers [s*kchunk, min(K, (s+1)*kchunk)), C += s*splitC
     int64_t splitC;
+    int sub;                               // 1: C -= A B (trailing update of the LU, scw_alpha.cu) instead of C = A B
 };
 
 __device__ __forceinline__ void cp_async16(void* dst_smem, const void* src, bool pred)
@@ -155,7 +156,15 @@ __global__ void __launch_bounds__(DG_THREADS, 2) k_dmma_cgemm(const DgParams p)
             for (int e = 0; e < 2; ++e) {
                 const int64_t n = n0 + wn * 32 + j * 8 + 2 * t + e;
                 const double t1 = acc[i][j][0][e], t2 = acc[i][j][1][e], t3 = acc[i][j][2][e];
-                if (n < p.N) C[m * p.sCm + n * p.sCn] = make_double2(t1 - t2, t3 - t1 - t2);
+                if (n < p.N) {
+                    double2* dst = C + m * p.sCm + n * p.sCn;
+                    if (p.sub) {
+                        const double2 old = *dst;
+                        *dst = make_double2(old.x - (t1 - t2), old.y - (t3 - t1 - t2));
+                    } else {
+                        *dst = make_double2(t1 - t2, t3 - t1 - t2);
+                    }
+                }
             }
         }
     }
@@ -190,6 +199,25 @@ static int dg_assemble_splits(int64_t R, int64_t J, int64_t Fz, int sm_count)
 }
 
 bool dmma_supported(int dtype) { return dtype == SCW_C128; }
+
+// C [ldC x N] -= A [ldA x K] (column-major, M rows) . B [K x N] (row-major, ldB): the trailing update of the blocked LU.
+void launch_dmma_gemm_sub(scw_ctx* ctx, int64_t M, int64_t N, int64_t K, const void* A, int64_t ldA, const void* B, int64_t ldB,
+                          void* C, int64_t ldC)
+{
+    DgParams p = {};
+    p.A = (const double2*)A;
+    p.B = (const double2*)B;
+    p.C = (double2*)C;
+    p.M = M; p.N = N; p.K = K;
+    p.sAk = ldA;
+    p.sBk = ldB;
+    p.sCm = 1; p.sCn = ldC;
+    p.nb2 = 1;
+    p.nsplit = 1;
+    p.kchunk = (K + DG_KB - 1) / DG_KB * DG_KB;
+    p.sub = 1;
+    dg_launch(ctx, KC_ALPHA_LU, p, 1);
+}
 
 size_t dmma_assemble_scratch(int64_t R, int64_t J, int64_t Fz, int sm_count)
 {

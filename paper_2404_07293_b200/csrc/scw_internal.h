@@ -10,7 +10,7 @@ namespace scw {
 // Kernel classes for launch accounting and the optional per-kernel CUDA-event timers.
 enum KernelClass {
     KC_WEIGHTS = 0, KC_TWIDDLES, KC_ASSEMBLE, KC_REDUCE, KC_SYNTH_A, KC_SYNTH_B, KC_POINTS_TABLE, KC_POINTS,
-    KC_POINT_SYNTH, KC_MISC, KC_ASSEMBLE_TC, KC_SYNTH_TC, KC_SYNTH_IMG, KC_ASSEMBLE_DMMA, KC_SYNTH_A_DMMA, KC_SYNTH_B_DMMA, KC_EXTERIOR, KC_VBUILD_PREP, KC_COUNT
+    KC_POINT_SYNTH, KC_MISC, KC_ASSEMBLE_TC, KC_SYNTH_TC, KC_SYNTH_IMG, KC_ASSEMBLE_DMMA, KC_SYNTH_A_DMMA, KC_SYNTH_B_DMMA, KC_EXTERIOR, KC_VBUILD_PREP, KC_ALPHA, KC_ALPHA_LU, KC_COUNT
 };
 struct ProfRec { cudaEvent_t a, b; int kc; bool owns_a; };
 }  // namespace scw
@@ -203,6 +203,14 @@ void launch_dmma_assemble(scw_ctx* ctx, int64_t R, int64_t J, int64_t Fz, const 
 // two-pass synthesis with the frequency-major tables of launch_twiddles; scratch = simt_synth_scratch(SCW_C128, ...)
 void launch_dmma_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, const void* FxT,
                        int64_t Ny, const void* FyT, void* E, const int64_t strides[4], void* scratch);
+
+void launch_dmma_gemm_sub(scw_ctx* ctx, int64_t M, int64_t N, int64_t K, const void* A, int64_t ldA, const void* B, int64_t ldB,
+                          void* C, int64_t ldC);
+
+// ---- scw_alpha.cu: alpha propagation across layers, eq. 24-26 (NEXT-4) -------------------------------------------
+bool alpha_supported(const scw_ctx* ctx, int64_t n);
+size_t alpha_scratch(const scw_ctx* ctx, int64_t n);
+void launch_propagate_alpha(scw_ctx* ctx, const scw_stack* st, const void* r0, void* const* alpha, void* rL, void* scratch);
 
 // ---- scw_exterior.cu: eq. 9 in the half-spaces above / below the sample (NEXT-1) -------------------------------
 void launch_exterior_spectra(scw_ctx* ctx, const scw_exterior* e, int64_t Fz, const double* z, void* P, int64_t ldP);

@@ -94,3 +94,54 @@ def test_single_layer_is_the_explicit_inverse_and_gauss():
     # |d| <= 1: every interface factor decays (reading c-1)
     da, dg = oracle.interface_factors(lam=st["lam"], z_a=0.0, z_b=st["z_if"][1], gamma=st["gamma"][0], dir=None)
     assert np.abs(da).max() <= 1 + 1e-15 and np.abs(dg).max() <= 1 + 1e-15
+
+
+# ------------------------------------------------------------------------------------------------ GPU
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("dtype,tol", [(np.complex64, 2e-4), (np.complex128, 1e-10)])
+@pytest.mark.parametrize("n,L,with_dir", [(4, 1, True), (36, 3, True), (100, 2, False), (324, 3, True), (517, 2, True)])
+def test_propagate_alpha_against_the_oracle(dtype, tol, n, L, with_dir):
+    """scw_propagate_alpha (blocked LU on the GPU) against oracle.propagate_alpha (LAPACK): every alpha of every layer and
+    the bottom field vector; n not a multiple of the 64-column panel, one to several panels, dir given or derived."""
+    import torch
+    import paper_2404_07293_b200 as scw
+    st = random_stack(n, L, seed=n + L, dtype=dtype)
+    ref_a, ref_r = oracle.propagate_alpha(lam=st["lam"], z_if=st["z_if"], Q=st["Q"], gamma=st["gamma"],
+                                          dir=st["dir"] if with_dir else None, r0=st["r0"])
+    ctx = scw.Context(0)
+    try:
+        # the C ABI takes column-major Q: tensor row j = column j of the mathematical matrix
+        Qd = [dev(np.ascontiguousarray(q.T)) for q in st["Q"]]
+        alphas, rL = scw.scw_propagate_alpha(ctx, lam=st["lam"], z_if=st["z_if"], Q=Qd, gamma=[dev(g) for g in st["gamma"]],
+                                             dir=[dev(d) for d in st["dir"]] if with_dir else None, r0=dev(st["r0"]))
+        torch.cuda.synchronize()
+        for l in range(L):
+            assert np.abs(alphas[l].cpu().numpy() - ref_a[l]).max() / np.abs(ref_a[l]).max() <= tol, l
+        assert np.abs(rL.cpu().numpy() - ref_r).max() / np.abs(ref_r).max() <= tol
+    finally:
+        ctx.close()
+
+
+@pytest.mark.gpu
+def test_propagate_alpha_config1_size():
+    """n = 4M = 4356 (config 1), two layers, complex128: 69 panels, trailing updates on the DMMA kernel."""
+    import torch
+    import paper_2404_07293_b200 as scw
+    st = random_stack(4356, 2, seed=5)
+    ref_a, ref_r = oracle.propagate_alpha(**st)
+    ctx = scw.Context(0)
+    try:
+        Qd = [dev(np.ascontiguousarray(q.T)) for q in st["Q"]]
+        alphas, rL = scw.scw_propagate_alpha(ctx, lam=st["lam"], z_if=st["z_if"], Q=Qd, gamma=[dev(g) for g in st["gamma"]],
+                                             dir=[dev(d) for d in st["dir"]], r0=dev(st["r0"]))
+        torch.cuda.synchronize()
+        for l in range(2):
+            assert np.abs(alphas[l].cpu().numpy() - ref_a[l]).max() / np.abs(ref_a[l]).max() <= 1e-10
+        assert np.abs(rL.cpu().numpy() - ref_r).max() / np.abs(ref_r).max() <= 1e-10
+    finally:
+        ctx.close()
