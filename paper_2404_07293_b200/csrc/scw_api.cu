@@ -40,6 +40,7 @@ int32_t check_ctx(scw_ctx* ctx, bool sweep_call = false)
     if (!sweep_call) {
         ctx->tw_valid = false;
         ctx->clean_ctl = nullptr;
+        ctx->clean_img = nullptr;
     }
     ctx->msg[0] = 0;
     ctx->cuda_err = 0;
@@ -290,6 +291,7 @@ int32_t scw_set_workspace(scw_ctx* ctx, void* dev_ptr, size_t bytes)
     ctx->ws_bytes = bytes;
     ctx->tw_valid = false;
     ctx->clean_ctl = nullptr;
+    ctx->clean_img = nullptr;
     return SCW_OK;
 }
 
@@ -298,6 +300,7 @@ int32_t scw_invalidate_cache(scw_ctx* ctx)
     if (!ctx) return SCW_ERR_NULL;
     ctx->tw_valid = false;
     ctx->clean_ctl = nullptr;
+    ctx->clean_img = nullptr;
     return SCW_OK;
 }
 
@@ -313,6 +316,7 @@ int32_t scw_set_option(scw_ctx* ctx, int32_t option, int64_t value)
         ctx->cache_on = value != 0;
         ctx->tw_valid = false;
         ctx->clean_ctl = nullptr;
+        ctx->clean_img = nullptr;
         return SCW_OK;
     }
     if (option == SCW_OPT_PROFILE && (value == 0 || value == 1)) {
@@ -566,6 +570,11 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
             int* sched = nullptr;
             int n_sched = 0;
             tc_synth_image_plan(L0.U, L0.Vn, Nx, Ny, s_scr, tw.a, &fix, &sched, &n_sched);
+            // image padding: zeroed by the kernel unless the previous sweep left this very buffer in the same layout
+            const int64_t planes = Fz[0] * 3 * g;
+            fix.skip_zero = ctx->cache_on && ctx->clean_img == s_scr && ctx->clean_img_U == L0.U && ctx->clean_img_Vn == L0.Vn &&
+                            ctx->clean_img_planes >= planes;
+            if (!fix.skip_zero) { ctx->clean_img = s_scr; ctx->clean_img_U = L0.U; ctx->clean_img_Vn = L0.Vn; ctx->clean_img_planes = planes; }
             launch_tc_assemble_group(ctx, g, inst + i0, Fz[0], z + i0, fix, sched, n_sched, a_scr, clean);
             if (ctx->tc_error) return;
             clean = true;                               // the kernel leaves its control block zeroed

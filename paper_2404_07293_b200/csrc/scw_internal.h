@@ -46,6 +46,10 @@ struct scw_ctx {
     bool tw_valid = false;
     const void* clean_ctl = nullptr;
     size_t clean_ints = 0;
+    // spectrum-image buffer whose padding is known to hold zeros (same promise): location, frequency grid, planes
+    const void* clean_img = nullptr;
+    int clean_img_U = 0, clean_img_Vn = 0;
+    int64_t clean_img_planes = 0;
     cudaEvent_t prof_last = nullptr;   // profiling: end event of the previous kernel of this API call
     std::vector<scw::ProfRec> recs;
     double prof_ms[scw::KC_COUNT] = {0};
@@ -146,6 +150,7 @@ struct TcFixup {
     // N1 rows x K1p, K-major core-matrix layout; chunks of Uc x Vc frequencies
     uint8_t* img;
     int U, Vn, Uc, Vc, nuc, nvc, K1p, N1;
+    int skip_zero;              // the padding of the images already holds zeros (left by the previous launch)
 };
 // weights (a-1) + P = V W (a-2) + fix-up, n_inst <= tc_assemble_max_group() instances with equal U, Vn, J, Fz in ONE launch;
 // sched/n_sched: plane counters of the synthesis that follows (zeroed by the kernel), may be NULL.

@@ -59,6 +59,9 @@ constexpr int TA_CTL_CLAIM = 2;            // control block: [0] CTAs past phase
 constexpr int TA_CTL_TILE = TA_CTL_CLAIM + TA_MAX_CTAS;
 
 constexpr int TA_MAX_INST = 64;            // instances (layers x wavelengths) per grouped launch
+#ifndef SCW_TA_L2PROMO
+#define SCW_TA_L2PROMO CU_TENSOR_MAP_L2_PROMOTION_L2_64B
+#endif
 
 struct TaParams {
     CUtensorMap tmap[TA_MAX_INST][2];   // [0]: even columns of V, [1]: odd columns; box = 128 rows x 16 columns of 8 bytes
@@ -253,7 +256,7 @@ __device__ __forceinline__ void ta_phase0(const TaParams& p, int64_t t, int64_t 
     }
     // (2) spectrum images of the synthesis: every 16-byte chunk that is not entirely spectrum data is zeroed (frequency
     // and K padding; the chunks that straddle the edge get their data from the fix-up, which runs after phase 0 of all CTAs)
-    if (p.fix.mode == TC_FIX_IMAGES) {
+    if (p.fix.mode == TC_FIX_IMAGES && !p.fix.skip_zero) {
         const TcFixup& f = p.fix;
         const int chunks_half = f.N1 * (f.K1p / 8);                      // chunk id within a hi or lo image = kc*N1 + row
         const int n_half = (int)(p.n_inst * p.Fz * 3 * f.nuc * f.nvc * 2);   // (image, hi/lo) halves, < 2^31
@@ -823,7 +826,7 @@ static bool ta_make_map(CUtensorMap* map, const void* V, int64_t ldV, int64_t R,
     const cuuint32_t estr[2] = {1, 1};
     if (xoff) *xoff = off;
     return enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT64, 2, const_cast<char*>(base), dims, strides, box, estr,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_64B,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, SCW_TA_L2PROMO,
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 

@@ -456,11 +456,15 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                         }
                     }
                     if (p.s_part) {                                // window sum of this warp's 32 x 32 patch, fixed order
+                        // bit e of ymask: (x, y0 + e) lies in the window (branch-free selects: a branch per sample costs more
+                        // than the whole epilogue)
+                        const int lo = (int)max((int64_t)0, (int64_t)p.win_y0 - y0), hi = (int)min((int64_t)32, (int64_t)p.win_y1 - y0);
+                        uint32_t ymask = 0u;
+                        if (x >= p.win_x0 && x < p.win_x1 && hi > lo)
+                            ymask = (hi >= 32 ? 0xffffffffu : ((1u << hi) - 1u)) & ~((1u << lo) - 1u);
                         float ws = 0.f;
-                        const bool xin = x >= p.win_x0 && x < p.win_x1;
 #pragma unroll
-                        for (int e = 0; e < 32; ++e)
-                            if (xin && y0 + e >= p.win_y0 && y0 + e < p.win_y1) ws += m2[e];
+                        for (int e = 0; e < 32; ++e) ws += ((ymask >> e) & 1u) ? m2[e] : 0.f;
 #pragma unroll
                         for (int o = 16; o > 0; o >>= 1) ws += __shfl_xor_sync(0xffffffffu, ws, o);
                         if (lane == 0)
@@ -530,15 +534,19 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
 
 // Window sums: S[inst][n] = sum over the three components, the output tiles and the 16 warp patches of a tile, in a fixed
 // order (deterministic), of the partial sums the detector epilogue left in s_part.
-__global__ void k_tc_synth_wsum(int n_inst, int Fz, int tiles, const float* __restrict__ s_part, const TsWsumOut out)
+__global__ void __launch_bounds__(128) k_tc_synth_wsum(int n_inst, int Fz, int tiles, const float* __restrict__ s_part,
+                                                       const TsWsumOut out)
 {
-    const int idx = blockIdx.x * blockDim.x + threadIdx.x;           // (inst, n)
+    const int idx = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;      // one warp per (inst, n)
     if (idx >= n_inst * Fz) return;
     const int inst = idx / Fz, n = idx - inst * Fz;
-    const float* src = s_part + (size_t)idx * 3 * tiles * 16;         // plane (inst*Fz + n)*3 + comp, contiguous over comp
+    const int cnt = 3 * tiles * 16;
+    const float* src = s_part + (size_t)idx * cnt;                    // plane (inst*Fz + n)*3 + comp, contiguous over comp
     float acc = 0.f;
-    for (int i = 0; i < 3 * tiles * 16; ++i) acc += src[i];
-    out.S[inst][n] = acc;
+    for (int i = lane; i < cnt; i += 32) acc += src[i];               // fixed order per lane, then a fixed tree
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) out.S[inst][n] = acc;
 }
 
 // ---- host side -------------------------------------------------------------------------------------
@@ -660,7 +668,7 @@ static void ts_launch_main(scw_ctx* ctx, const TsPlan& pl, int64_t Fz, int n_ins
         for (int i = 0; i < n_inst; ++i) out.S[i] = static_cast<float*>(det->S[i]);
         KernelScope ks(ctx, KC_MISC);
         const int n = n_inst * (int)Fz;
-        k_tc_synth_wsum<<<(n + 127) / 128, 128, 0, ctx->stream>>>(n_inst, (int)Fz, total_pairs, p.s_part, out);
+        k_tc_synth_wsum<<<(n + 3) / 4, 128, 0, ctx->stream>>>(n_inst, (int)Fz, total_pairs, p.s_part, out);
     }
 }
 

@@ -327,3 +327,54 @@ def test_last_kernels_tells_which_path_ran(scw, ctx):
     scw.scw_sweep_wavelengths(ctx, [L, scw.Layer.from_numpy(lay2, "cuda")], [dev(z), dev(z)], dev(x), dev(y))
     assert ctx.launch_count() - n0 > 3                                       # per-instance launches, not one group
     torch.cuda.synchronize()
+
+
+def test_twiddle_cache_and_calibration(scw):
+    """SCW_OPT_CACHE: consecutive sweeps reuse the twiddle tables, the clean control block and the zeroed image padding (two
+    launches instead of three); results stay those of the oracle; scw_invalidate_cache picks up coordinates changed in
+    place; a different call in between drops the cache; scw_calibrate changes the split, not the values."""
+    c = scw.Context(0)
+    try:
+        c.set_cache(True)
+        lays = [ragged_layer(9, 7, 252, np.complex64, seed=60 + i) for i in range(3)]
+        x = np.arange(150) * 3.0 / 150
+        y = np.arange(140) * 4.5 / 140
+        z = np.linspace(-0.2, 0.8, 5)
+        Ls = [scw.Layer.from_numpy(l, "cuda") for l in lays]
+        dx, dy, dzs = dev(x), dev(y), [dev(z)] * 3
+        refs = [oracle.tier_b_grid(x=x, y=y, z=z, **l) for l in lays]
+        n0 = c.launch_count()
+        E1 = [e.clone() for e in scw.scw_sweep_wavelengths(c, Ls, dzs, dx, dy)]
+        n1 = c.launch_count()
+        E2 = scw.scw_sweep_wavelengths(c, Ls, dzs, dx, dy)
+        n2 = c.launch_count()
+        torch.cuda.synchronize()
+        assert n1 - n0 == 3 and n2 - n1 == 2                               # the second call skips the twiddle kernel
+        for a, b, r in zip(E1, E2, refs):
+            assert torch.equal(a, b)
+            assert rel_err(b.cpu().numpy(), r) <= 2e-4
+        I = scw.scw_sweep_intensity(c, Ls, dzs, dx, dy)                     # same workspace layout family: still cached
+        torch.cuda.synchronize()
+        assert np.abs(I[0].cpu().numpy() - oracle.intensity(refs[0])).max() / oracle.intensity(refs[0]).max() <= 4e-4
+        # coordinates changed in place: stale until invalidated
+        dx.mul_(0.5)
+        c.invalidate_cache()
+        E3 = scw.scw_sweep_wavelengths(c, Ls, dzs, dx, dy)
+        torch.cuda.synchronize()
+        assert rel_err(E3[1].cpu().numpy(), oracle.tier_b_grid(x=0.5 * x, y=y, z=z, **lays[1])) <= 2e-4
+        # another kind of call carves the workspace differently: the next sweep must not trust the cache
+        scw.scw_assemble_spectra(c, Ls[0], dzs[0])
+        n3 = c.launch_count()
+        E4 = scw.scw_sweep_wavelengths(c, Ls, dzs, dx, dy)
+        torch.cuda.synchronize()
+        assert c.launch_count() - n3 == 3 and torch.equal(E4[2], E3[2])
+        # calibration: same values up to the summation order of the stream-K split
+        E5 = scw.scw_calibrate(c, Ls, dzs, dx, dy, reps=2)
+        E6 = scw.scw_sweep_wavelengths(c, Ls, dzs, dx, dy)
+        torch.cuda.synchronize()
+        for a, b in zip(E5, E6):
+            assert float((a - E3[0].new_tensor(0) - b).abs().max()) == 0.0     # same split after calibration: identical
+        assert float((E6[0] - E3[0]).abs().max() / E3[0].abs().max()) <= 2e-5
+        assert len(c.assembly_timeline()) >= 1
+    finally:
+        c.close()
