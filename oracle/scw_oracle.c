@@ -19,7 +19,8 @@
  * Pins (tests/test_oracle_pins.py): eq. 2 special cases, eq. 6 index map,
  * eq. 7 semigroup, |w|<=1 reference-plane invariant, single-mode closed
  * form, ifft2 on commensurate grids, Parseval, periodicity, homogeneous-layer
- * TE/TM plane waves with s.p=0 (eq. 14), brute-force DFT on 3x3 toys.
+ * TE/TM plane waves with s.p=0 (eq. 14), brute-force DFT on 3x3 toys; the dir == NULL branch (scwo_dir) against the
+ * hand-derived table tests/golden/dir_cases.txt through the single-mode closed form.
  * Parity unpinned: the statistical content of the synthetic V, c, gamma
  * (synthetic by construction) -- see DESIGN.md.
  */
