@@ -55,6 +55,8 @@ struct TsParams {
     // NEXT-3 detector (k_tc_synth<true>): no complex field is stored.
     int want_I;            // E[] point to float outputs I = sum_comp |E_comp|^2
     int acc_col;           // first of 128 TMEM columns holding the running sum over components, 0 = none (kept in the output)
+    int d2_single;         // detector with 33..40 frequencies along u (one u chunk): D2 is ONE 128-column buffer shared by the two y halves
+                           // (released as soon as it is in registers), its second half holds the running sum
     float* s_part;         // window sums: [plane][tile][16] partial sums of |E_comp|^2 over the window, NULL = not wanted
     int win_x0, win_x1, win_y0, win_y1;   // window (grid indices, half-open)
 };
@@ -329,14 +331,16 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                 const int n = i / nuc, uc = i - n * nuc;
                 if (i == 0 && h == 0) mbar_wait(a2_full, 0);
                 mbar_wait(&b2_full[h], i & 1);
-                if (uc == 0) mbar_wait(&d2_empty[h], (n & 1) ^ 1);
+                const int hb = p.d2_single ? 0 : h;                       // D2 buffer of this half, and how often it was used
+                const int use = p.d2_single ? 2 * n + h : n;
+                if (uc == 0) mbar_wait(&d2_empty[hb], (use & 1) ^ 1);
                 tc_fence_after();
                 const uint32_t ta = tmem_base + a2_col + uc * K2p;
                 if (elect_one()) {
-                    ts_mma3_ts(tmem_base + TS_D2_COL + h * TS_TILE, ta, ta + K2p / 2, b2 + h * 2 * b2_img,
+                    ts_mma3_ts(tmem_base + TS_D2_COL + hb * TS_TILE, ta, ta + K2p / 2, b2 + h * 2 * b2_img,
                                b2 + h * 2 * b2_img + b2_img, 2048, K2p, idesc2, uc > 0 ? 1u : 0u);
                     umma_commit(&b2_empty[h]);
-                    if (uc == nuc - 1) umma_commit(&d2_full[h]);
+                    if (uc == nuc - 1) umma_commit(&d2_full[hb]);
                 }
                 __syncwarp();
             };
@@ -428,17 +432,19 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
             for (int h = 0; h < 2; ++h) {
                 const int64_t y0 = (int64_t)ty * TS_TILE + 64 * h + 32 * cg;
                 const int ny = (int)min((int64_t)32, p.Ny - y0);   // may be <= 0
-                mbar_wait(&d2_full[h], n & 1);
+                const int hb = p.d2_single ? 0 : h;
+                mbar_wait(&d2_full[hb], (p.d2_single ? 2 * n + h : n) & 1);
                 tc_fence_after();
-                const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + TS_D2_COL + h * TS_TILE + 64 * cg;
+                const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + TS_D2_COL + hb * TS_TILE + 64 * cg;
                 if (INTENSITY) {
                     // detector: |E_comp|^2 per sample, then (want_I) I = |E_x|^2 + |E_y|^2 + |E_z|^2 and / or (s_part) the
                     // sum over a window of the plane.  D2[h] is released as soon as it is in registers, like the complex
                     // path.  For I the three components of a z plane come to this CTA in order (group = 3) and every
-                    // (x, y) belongs to one thread: the running sum lives in 128 spare TMEM columns (lane = x, column = y)
-                    // when they exist (p.acc_col; only the third component writes the output), else in the output itself
-                    // (read-modify-write through L2).
-                    const bool tm_acc = p.want_I && p.acc_col;
+                    // (x, y) belongs to one thread: the running sum lives in 128 TMEM columns (lane = x, column = y) at
+                    // p.acc_col -- spare columns behind A2 (U <= 32), or the second half of D2 when D2 is single-buffered
+                    // (d2_single, 32 < U <= 40) -- and only the third component writes the output; with two u chunks
+                    // (U > 40) GEMM2 accumulates both y halves across the chunks, D2 cannot shrink and the sum is kept in
+                    // the output itself (read-modify-write through L2).
                     const uint32_t acc = tmem_base + ((uint32_t)(32 * q) << 16) + p.acc_col + h * 64 + 32 * cg;
                     float m2[32];
                     {
@@ -448,7 +454,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                         tmem_ld_wait();
                         tc_fence_before();
                         __syncwarp();
-                        if (lane == 0) mbar_arrive(&d2_empty[h]);  // D2[h] is in registers now
+                        if (lane == 0) mbar_arrive(&d2_empty[hb]); // D2 is in registers now
 #pragma unroll
                         for (int e = 0; e < 32; ++e) {
                             const float re = __uint_as_float(v[e >> 4][(2 * e) & 31]), im = __uint_as_float(v[e >> 4][(2 * e + 1) & 31]);
@@ -472,7 +478,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                     }
                     if (p.want_I) {
                         float* io = reinterpret_cast<float*>(Einst) + zi * p.s_z + x * p.s_x + y0 * p.s_y;
-                        if (tm_acc) {
+                        if (p.acc_col) {
                             if (comp > 0) {
                                 float a[2][16];
                                 tmem_st_wait();                    // the previous component's sums have landed
@@ -496,7 +502,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                                 for (int e = 0; e < 32; ++e)
                                     if (e < ny) __stcg(io + e * p.s_y, m2[e]);
                             }
-                        } else if (x_ok) {
+                        } else if (x_ok) {                         // no TMEM room (two u chunks, U > 40): sum kept in the output
 #pragma unroll
                             for (int e = 0; e < 32; ++e) {
                                 if (e < ny) {
@@ -513,7 +519,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                     tmem_ld_wait();
                     tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(&d2_empty[h]);      // D2[h] is in registers now
+                    if (lane == 0) mbar_arrive(&d2_empty[hb]);     // D2[h] is in registers now
                     float2* out = Einst + comp * p.s_comp + zi * p.s_z + x * p.s_x + y0 * p.s_y;
                     if (x_ok) {
 #pragma unroll
@@ -640,9 +646,12 @@ static void ts_launch_main(scw_ctx* ctx, const TsPlan& pl, int64_t Fz, int n_ins
     p.nvc = pl.cv.n;
     p.want_I = want_I ? 1 : 0;
     p.group = want_I ? 3 : 1;
-    {   // detector accumulators go behind D2 | D1 | A2 when 128 TMEM columns are left (U <= 32)
+    {   // detector accumulators (128 columns): behind D2 | D1 | A2 when they fit (U <= 32); else D2 shrinks to one
+        // 128-column buffer shared by the two y halves and the sum takes the columns of its second half
         const int used = TS_D1_COL + pl.K2p * (1 + pl.cu.n);
-        p.acc_col = (want_I && used + 128 <= TS_TMEM_COLS) ? used : 0;
+        const bool fits = used + 128 <= TS_TMEM_COLS;
+        p.d2_single = (want_I && !fits && pl.cu.n == 1) ? 1 : 0;
+        p.acc_col = !want_I ? 0 : (fits ? used : (p.d2_single ? TS_TILE : 0));
     }
     p.s_part = (intensity && det->S) ? static_cast<float*>(det->s_part) : nullptr;
     if (intensity) {
