@@ -94,6 +94,24 @@ struct KernelScope {
     }
 };
 
+// Launch with programmatic stream serialization (PDL): the kernel's prologue -- everything before its pdl_wait() -- may
+// overlap the tail of the previous kernel of the stream.
+template <typename P>
+inline void launch_pdl(void (*kernel)(P), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, const P& params)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kernel, params);
+}
+
 // Bump allocator over the caller's workspace.
 struct Carver {
     char* base;

@@ -243,17 +243,22 @@ __device__ __forceinline__ void ta_weight_unit(const TaParams& p, int64_t tile_i
 
 // Everything the main loop of ANY CTA depends on, spread over all CTAs: t = this thread's index among the
 // gridDim.x * TA_P0_THREADS phase-0 threads of the grid.
-__device__ __forceinline__ void ta_phase0(const TaParams& p, int64_t t, int64_t nthreads)
+// (1) weight images: warp units (tile, k chunk of 8 modes), on all 24 warps before the roles split.
+__device__ __forceinline__ void ta_phase0_weights(const TaParams& p, int64_t t, int64_t nthreads, int threads_per_cta)
 {
-    // (1) weight images: warp units (tile, k chunk of 8 modes)
     {
         const int64_t n_units = (int64_t)p.n_inst * p.n_tiles * p.kblocks * (TA_BK / 8);
         const int lane = (int)(t & 31);
         // units are dealt round-robin over the CTAs (warp w of CTA b takes units w*G + b, ...): every SM gets its share
-        const int64_t first = (int64_t)((t % TA_P0_THREADS) >> 5) * gridDim.x + blockIdx.x;
+        const int64_t first = (int64_t)((t % threads_per_cta) >> 5) * gridDim.x + blockIdx.x;
         for (int64_t unit = first; unit < n_units; unit += nthreads >> 5)
             ta_weight_unit(p, unit >> 2, (int)(unit & 3), lane);
     }
+}
+
+// (2), (3): image padding and plane counters, on every warp but the V loader.
+__device__ __forceinline__ void ta_phase0(const TaParams& p, int64_t t, int64_t nthreads)
+{
     // (2) spectrum images of the synthesis: every 16-byte chunk that is not entirely spectrum data is zeroed (frequency
     // and K padding; the chunks that straddle the edge get their data from the fix-up, which runs after phase 0 of all CTAs)
     if (p.fix.mode == TC_FIX_IMAGES && !p.fix.skip_zero) {
@@ -450,6 +455,15 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
         }
         mbar_fence_init();
         fin[0] = -1;
+    }
+    if (warp == TA_MMA_WARP) tmem_alloc(tmem_slot, TA_TMEM_COLS);
+    // PDL: only the set-up above overlaps the tail of the previous kernel of the stream.  The weights read the caller's
+    // inputs (gamma, c, z, ...), which the kernel just before this one in the caller's stream may have produced, so even
+    // they wait for it.
+    pdl_wait();
+    pdl_launch_dependents();
+    ta_phase0_weights(p, (int64_t)blockIdx.x * TA_THREADS + tid, (int64_t)gridDim.x * TA_THREADS, TA_THREADS);
+    if (tid == 0) {
         uint32_t smid;
         asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
         int slot = -1;
@@ -458,7 +472,6 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
             if (atomicCAS(&p.ctl[TA_CTL_CLAIM + i], 0, 1) == 0) slot = i;
         *cta_slot = slot;
     }
-    if (warp == TA_MMA_WARP) tmem_alloc(tmem_slot, TA_TMEM_COLS);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -471,8 +484,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
     const int64_t it0 = p.span0[cta], it1 = p.span0[cta + 1];
     const unsigned long long t_start_all = ta_now();
 
-    // phase 0 on every warp but the V loader, whose TMA pipeline fills meanwhile (phase 0 is bound by instruction issue,
-    // not by its few loads, and the early V requests start the write-back of whatever dirty lines the L2 still holds)
+    // rest of phase 0 (image padding, plane counters) on every warp but the V loader, whose TMA pipeline fills meanwhile
     if (warp != TA_V_LOADER) {
         const int t0 = tid - (warp > TA_V_LOADER ? 32 : 0);
         ta_phase0(p, (int64_t)blockIdx.x * TA_P0_THREADS + t0, (int64_t)gridDim.x * TA_P0_THREADS);
@@ -912,7 +924,7 @@ static void ta_launch(scw_ctx* ctx, int n_inst, int64_t R, int64_t J, int64_t Fz
     ctx->clean_ints = pl.ctl_ints;
     KernelScope ks(ctx, KC_ASSEMBLE_TC);
     cudaFuncSetAttribute(k_tc_assemble, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes);
-    k_tc_assemble<<<pl.G, TA_THREADS, pl.smem_bytes, ctx->stream>>>(p);
+    launch_pdl(k_tc_assemble, dim3(pl.G), dim3(TA_THREADS), pl.smem_bytes, ctx->stream, p);
     ctx->last_asm_G = pl.G;
     ctx->last_asm_ns = p.cta_ns;
     for (int c = 0; c <= pl.G; ++c) ctx->last_asm_span0[c] = pl.span0[c];

@@ -267,7 +267,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                                                               kg * half);
             const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + a2_col + uc * K2p + kg * half;
             for (int c8 = 0; c8 < half / 8; ++c8) {
-                const uint4 v0 = src[2 * c8], v1 = src[2 * c8 + 1];
+                const uint4 v0 = __ldcg(src + 2 * c8), v1 = __ldcg(src + 2 * c8 + 1);      // L2: this runs before pdl_wait()
                 const uint32_t r[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
                 tmem_st8(taddr + 8 * c8, r);
             }
@@ -277,6 +277,12 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
         __syncwarp();
         if (lane == 0) mbar_arrive(a2_full);           // only GEMM2 needs A2: the other roles do not wait for it
     }
+
+    // Everything above (barriers, TMEM, the x twiddles -- written by the twiddle kernel, which the assembly before this
+    // kernel has already waited for) predates the assembly that feeds this kernel; the spectrum images and the plane
+    // counters are its output: wait for it here (PDL), then let the next kernel's prologue start.
+    pdl_wait();
+    pdl_launch_dependents();
 
     if (warp == 0) {
         // ===== loader: draws the planes; y twiddle images once, then the nuc*nvc spectrum images of every plane =====
@@ -669,8 +675,8 @@ static void ts_launch_main(scw_ctx* ctx, const TsPlan& pl, int64_t Fz, int n_ins
         int per_pair = ctx->sm_count / p.npairs;
         if (per_pair > planes) per_pair = planes;
         KernelScope ks(ctx, KC_SYNTH_TC);
-        if (intensity) k_tc_synth<true><<<p.npairs * per_pair, TS_THREADS, smem_bytes, ctx->stream>>>(p);
-        else k_tc_synth<false><<<p.npairs * per_pair, TS_THREADS, smem_bytes, ctx->stream>>>(p);
+        if (intensity) launch_pdl(k_tc_synth<true>, dim3(p.npairs * per_pair), dim3(TS_THREADS), smem_bytes, ctx->stream, p);
+        else launch_pdl(k_tc_synth<false>, dim3(p.npairs * per_pair), dim3(TS_THREADS), smem_bytes, ctx->stream, p);
     }
     if (p.s_part) {
         TsWsumOut out;
