@@ -210,9 +210,10 @@ int32_t scw_sweep_workspace(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst,
  * Calibrate the work split of the tensor-core assembly (step a-2) for this device and this workload: its persistent CTAs
  * (one per SM) each stream a contiguous span of V, and the SMs do not all reach the same HBM rate (the same groups of SMs
  * are slower in every run; by how much depends on what else the memory system is doing when the kernel starts).  Runs the
- * given sweep -- arguments and outputs exactly as scw_sweep_wavelengths -- `reps` + 1 times per round for three rounds,
- * measures every CTA of its assembly launch and makes the spans proportional to the measured rates for all later calls on
- * this ctx (results change only in summation order).  SYNCHRONISES the stream.  A sweep that does not take the tensor-core
+ * given sweep -- arguments and outputs exactly as scw_sweep_wavelengths -- `reps` + 1 times per round for nine rounds,
+ * measures every CTA of its assembly launch, moves the spans half way towards the measured relative rates after each round
+ * and keeps, for all later calls on this ctx, the split whose assembly finished earliest (the equal split if none beat it;
+ * results change only in summation order).  SYNCHRONISES the stream.  A sweep that does not take the tensor-core
  * assembly is accepted and leaves the equal split.  reps in [1, 64].  Errors: those of scw_sweep_wavelengths, VALUE (reps).
  */
 int32_t scw_calibrate(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz, const double* const* z,

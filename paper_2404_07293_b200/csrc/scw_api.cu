@@ -743,8 +743,12 @@ int32_t scw_calibrate(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
     if (reps < 1 || reps > 64) return fail(ctx, SCW_ERR_VALUE, "scw_calibrate: reps must be in [1, 64]");
     ctx->split_w.clear();
     std::vector<unsigned long long> ns(4 * 256);
-    for (int round = 0; round < 3; ++round) {
+    std::vector<double> best_w;                     // the split with the shortest assembly seen so far (empty = equal)
+    double best_us = 1e30;
+    const int rounds = 8;
+    for (int round = 0; round <= rounds; ++round) { // the last round only scores the last update
         std::vector<std::vector<double>> samples;
+        std::vector<double> kernel_us;
         int G = 0;
         for (int r = 0; r <= reps; ++r) {           // the first sweep of a round is a warm-up
             ctx->last_asm_G = 0;
@@ -768,7 +772,14 @@ int32_t scw_calibrate(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
                 rate[c] = (double)(ctx->last_asm_span0[c + 1] - ctx->last_asm_span0[c]) /
                           (double)(ns[4 * c + 2] > ns[4 * c + 1] ? ns[4 * c + 2] - ns[4 * c + 1] : 1);      // main loop only
             samples.push_back(rate);
+            double last_exit = 0.0;
+            for (int c = 0; c < G; ++c) last_exit = std::max(last_exit, (double)ns[4 * c + 3] * 1e-3);
+            kernel_us.push_back(last_exit);
         }
+        std::sort(kernel_us.begin(), kernel_us.end());
+        const double score = kernel_us[kernel_us.size() / 2];        // median over the repetitions of the slowest CTA's exit
+        if (score < best_us) { best_us = score; best_w = ctx->split_w; }
+        if (round == rounds) break;
         std::vector<double> w(G);
         double mean = 0.0;
         for (int c = 0; c < G; ++c) {               // median over the repetitions
@@ -778,13 +789,20 @@ int32_t scw_calibrate(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
             w[c] = v[v.size() / 2];
             mean += w[c] / G;
         }
-        for (int c = 0; c < G; ++c) {               // clipped: no span beyond ~1.5x the mean (bounds the partial-tile slots)
-            w[c] /= mean;
-            if (!(w[c] > 0.6)) w[c] = 0.6;
+        // damped update towards the measured relative rate: a CTA's time is not proportional to its span (what one CTA
+        // gives up, its neighbours on the same memory paths pick up), the undamped update oscillates
+        const bool first = (int)ctx->split_w.size() != G;
+        for (int c = 0; c < G; ++c) {
+            const double old = first ? 1.0 : ctx->split_w[c];
+            const double rel = w[c] / mean;                      // measured rate relative to the mean
+            const double cur = old;                               // share it ran with
+            w[c] = cur * (1.0 + 0.5 * (rel / cur - 1.0));         // half way from the current share to the measured rate
+            if (!(w[c] > 0.6)) w[c] = 0.6;                        // clipped: no span beyond ~1.5x the mean (bounds the partial-tile slots)
             if (w[c] > 1.5) w[c] = 1.5;
         }
         ctx->split_w = w;
     }
+    ctx->split_w = best_w;
     return SCW_OK;
 }
 
