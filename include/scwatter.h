@@ -195,7 +195,10 @@ int32_t scw_points_workspace(scw_ctx* ctx, const scw_modes* modes, int64_t N, si
 /*
  * Batched grid evaluation: assembly + synthesis for every (wavelength, layer) instance in one
  * call (spectroscopy sweep).  All instances share U, Vn, X, Y, dtype and the
- * x/y grid (the twiddles are wavelength-free: k s_m . r = 2 pi (u x/X + v y/Y), eq. 6).
+ * x/y grid (the twiddles are wavelength-free: k s_m . r = 2 pi (u x/X + v y/Y), eq. 6).  J and Fz may differ between
+ * instances: consecutive instances with the same J and Fz (up to 64) form a run that is evaluated by ONE assembly launch and
+ * ONE synthesis launch; an instance the tensor-core kernels cannot take (see scw_last_kernels) puts the whole call on the
+ * per-instance path.
  * inst: HOST [n_inst].  Fz: HOST [n_inst].  z: HOST array of device pointers.  E: HOST array of
  * device pointers, each laid out by `strides` as in scw_synthesize_grid.
  */

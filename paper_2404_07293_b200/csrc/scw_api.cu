@@ -468,21 +468,24 @@ static int32_t check_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, 
 }
 
 // Grouped (batched) sweep: every instance on the tensor-core kernels with the same J and Fz.
-static int sweep_group_size(const scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz)
-{
-    if (n_inst < 1 || Fz[0] <= 0) return 0;
-    if (!use_tc_assemble(ctx, &inst[0], Fz[0]) || !use_tc_synth(ctx, inst[0].dtype, inst[0].U, inst[0].Vn)) return 0;
-    for (int64_t i = 1; i < n_inst; ++i)        // every instance must be able to take the TMA path (16-byte aligned V, ...)
-        if (inst[i].J != inst[0].J || Fz[i] != Fz[0] || !use_tc_assemble(ctx, &inst[i], Fz[i])) return 0;
-    int g = tc_assemble_max_group() < tc_synth_max_group() ? tc_assemble_max_group() : tc_synth_max_group();
-    return (int)(n_inst < g ? n_inst : g);
-}
+// Grouped (batched) sweep: every instance on the tensor-core kernels.  The instances are cut into runs of consecutive
+// instances with the same J and Fz (at most 64 per run): each run is ONE assembly launch and ONE synthesis launch.
+// Empty = the sweep takes the per-instance path (some instance cannot run on the tensor-core kernels, or has Fz = 0).
+struct SweepRun { int64_t i0; int n; };
 
-static size_t sweep_group_ws(const scw_ctx* ctx, const scw_layer* L0, int64_t Fz, int group, int64_t Nx, int64_t Ny)
+static std::vector<SweepRun> sweep_runs(const scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const int64_t* Fz)
 {
-    const int64_t R = 3LL * L0->U * L0->Vn;
-    return twiddle_ws(ctx, L0->dtype, L0->U, L0->Vn, Nx, Ny) + align_up(tc_assemble_scratch(ctx, R, L0->J, Fz, group)) +
-           align_up(tc_synth_scratch(L0->U, L0->Vn, Fz * group));
+    std::vector<SweepRun> runs;
+    if (n_inst < 1 || !use_tc_synth(ctx, inst[0].dtype, inst[0].U, inst[0].Vn)) return runs;
+    const int gmax = tc_assemble_max_group() < tc_synth_max_group() ? tc_assemble_max_group() : tc_synth_max_group();
+    for (int64_t i = 0; i < n_inst; ++i) {          // every instance must be able to take the TMA path (16-byte aligned V, ...)
+        if (Fz[i] <= 0 || !use_tc_assemble(ctx, &inst[i], Fz[i])) return std::vector<SweepRun>();
+        if (!runs.empty() && runs.back().n < gmax && inst[i].J == inst[runs.back().i0].J && Fz[i] == Fz[runs.back().i0])
+            runs.back().n++;
+        else
+            runs.push_back(SweepRun{i, 1});
+    }
+    return runs;
 }
 
 static size_t sweep_ws(const scw_ctx* ctx, const scw_layer* L0, int64_t fz_max, size_t asm_max, int64_t Nx, int64_t Ny)
@@ -505,8 +508,17 @@ static size_t sweep_need(const scw_ctx* ctx, int64_t n_inst, const scw_layer* in
                          size_t asm_max, int64_t Nx, int64_t Ny, const DetArgs* det)
 {
     if (!n_inst || fz_max == 0) return 0;
-    const int group = sweep_group_size(ctx, n_inst, inst, Fz);
-    if (group) return sweep_group_ws(ctx, &inst[0], Fz[0], group, Nx, Ny) + (det ? tc_synth_wsum_bytes(Fz[0] * group, Nx, Ny) : 0);
+    const std::vector<SweepRun> runs = sweep_runs(ctx, n_inst, inst, Fz);
+    if (!runs.empty()) {                            // twiddles | assembly scratch | images | window partials, each sized for the largest run
+        size_t a = 0, sy = 0, w = 0;
+        const int64_t R = 3LL * inst[0].U * inst[0].Vn;
+        for (const SweepRun& r : runs) {
+            a = std::max(a, align_up(tc_assemble_scratch(ctx, R, inst[r.i0].J, Fz[r.i0], r.n)));
+            sy = std::max(sy, align_up(tc_synth_scratch(inst[0].U, inst[0].Vn, Fz[r.i0] * r.n)));
+            if (det) w = std::max(w, tc_synth_wsum_bytes(Fz[r.i0] * r.n, Nx, Ny));
+        }
+        return twiddle_ws(ctx, inst[0].dtype, inst[0].U, inst[0].Vn, Nx, Ny) + a + sy + w;
+    }
     return sweep_ws(ctx, &inst[0], fz_max, asm_max, Nx, Ny) +
            (det ? align_up((size_t)fz_max * 3 * Nx * Ny * esize(inst[0].dtype)) : 0);
 }
@@ -545,39 +557,54 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
     // the window sums (NEXT-3)
     const scw_layer& L0 = inst[0];
     const int64_t R = 3LL * L0.U * L0.Vn;
-    const int group = sweep_group_size(ctx, n_inst, inst, Fz);
-    if (group) {
-        // batched: all instances of a group go through ONE assembly launch (weights + P = V W + fix-up that writes the
+    const std::vector<SweepRun> runs = sweep_runs(ctx, n_inst, inst, Fz);
+    if (!runs.empty()) {
+        // batched: all instances of a run go through ONE assembly launch (weights + P = V W + fix-up that writes the
         // synthesis kernel's spectrum images: P never goes to memory) and ONE synthesis launch; the twiddle launch, when
         // it is not served from the cache, also clears the assembly's control block
+        size_t a_max = 0, s_max = 0, w_max = 0;
+        for (const SweepRun& r : runs) {
+            a_max = std::max(a_max, align_up(tc_assemble_scratch(ctx, R, inst[r.i0].J, Fz[r.i0], r.n)));
+            s_max = std::max(s_max, align_up(tc_synth_scratch(L0.U, L0.Vn, Fz[r.i0] * r.n)));
+            if (det) w_max = std::max(w_max, tc_synth_wsum_bytes(Fz[r.i0] * r.n, Nx, Ny));
+        }
         Carver probe(cv.base);
         probe.off = cv.off;
         probe.take(tc_synth_twiddle_bytes(L0.U, L0.Vn, Nx, Ny));
-        void* a_scr = probe.take(tc_assemble_scratch(ctx, R, L0.J, Fz[0], group));
-        void* s_scr = probe.take(tc_synth_scratch(L0.U, L0.Vn, Fz[0] * group));
-        void* w_scr = det ? probe.take(tc_synth_wsum_bytes(Fz[0] * group, Nx, Ny)) : nullptr;
+        void* a_scr = probe.take(a_max);
+        void* s_scr = probe.take(s_max);
+        void* w_scr = det ? probe.take(w_max) : nullptr;
         int* ctl = nullptr;
-        size_t n_ctl = 0;
-        tc_assemble_ctl(ctx, R, L0.J, Fz[0], group, a_scr, &ctl, &n_ctl);
+        size_t n_ctl = 0;                           // the control block starts the assembly scratch; sized for the largest run
+        for (const SweepRun& r : runs) {
+            size_t n = 0;
+            tc_assemble_ctl(ctx, R, inst[r.i0].J, Fz[r.i0], r.n, a_scr, &ctl, &n);
+            n_ctl = std::max(n_ctl, n);
+        }
         bool clean = ctx->cache_on && ctx->clean_ctl == ctl && ctx->clean_ints >= n_ctl;
         bool zeroed = false;
         const Twiddles tw = run_twiddles(ctx, L0.dtype, L0.U, L0.Vn, L0.X, L0.Y, Nx, x, Ny, y, cv, clean ? nullptr : ctl,
                                          n_ctl, &zeroed);
         clean = clean || zeroed;
-        for (int64_t i0 = 0; i0 < n_inst; i0 += group) {
-            const int g = (int)(n_inst - i0 < group ? n_inst - i0 : group);
+        if (!clean) {                               // cached twiddles but an unknown control block: clear all of it once
+            cudaMemsetAsync(ctl, 0, n_ctl * sizeof(int), ctx->stream);
+            clean = true;
+        }
+        for (const SweepRun& r : runs) {
+            const int64_t i0 = r.i0, fz = Fz[i0];
+            const int g = r.n;
             TcFixup fix = {};
             int* sched = nullptr;
             int n_sched = 0;
             tc_synth_image_plan(L0.U, L0.Vn, Nx, Ny, s_scr, tw.a, &fix, &sched, &n_sched);
-            // image padding: zeroed by the kernel unless the previous sweep left this very buffer in the same layout
-            const int64_t planes = Fz[0] * 3 * g;
-            fix.skip_zero = ctx->cache_on && ctx->clean_img == s_scr && ctx->clean_img_U == L0.U && ctx->clean_img_Vn == L0.Vn &&
-                            ctx->clean_img_planes >= planes;
+            // image padding: zeroed by the kernel unless an earlier launch left this very buffer in the same layout
+            const int64_t planes = fz * 3 * g;
+            fix.skip_zero = (ctx->cache_on || i0 > 0) && ctx->clean_img == s_scr && ctx->clean_img_U == L0.U &&
+                            ctx->clean_img_Vn == L0.Vn && ctx->clean_img_planes >= planes;
             if (!fix.skip_zero) { ctx->clean_img = s_scr; ctx->clean_img_U = L0.U; ctx->clean_img_Vn = L0.Vn; ctx->clean_img_planes = planes; }
-            launch_tc_assemble_group(ctx, g, inst + i0, Fz[0], z + i0, fix, sched, n_sched, a_scr, clean);
+            launch_tc_assemble_group(ctx, g, inst + i0, fz, z + i0, fix, sched, n_sched, a_scr, clean);
             if (ctx->tc_error) return;
-            clean = true;                               // the kernel leaves its control block zeroed
+            clean = true;                               // the kernel leaves its control block zeroed (n_ctl ints were clean before)
             TcDetector td;
             if (det) {
                 td.I = det->I ? det->I + i0 : nullptr;
@@ -585,9 +612,11 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
                 memcpy(td.win, det->win, sizeof(td.win));
                 td.s_part = w_scr;
             }
-            launch_tc_synth_group_images(ctx, L0.U, L0.Vn, Fz[0], g, Nx, Ny, tw.a, det ? nullptr : E + i0, s4, s_scr,
+            launch_tc_synth_group_images(ctx, L0.U, L0.Vn, fz, g, Nx, Ny, tw.a, det ? nullptr : E + i0, s4, s_scr,
                                          det ? &td : nullptr);
         }
+        if (!ctx->cache_on) ctx->clean_img = nullptr;   // trusted across calls only under SCW_OPT_CACHE
+        ctx->clean_ints = n_ctl;
         return;
     }
     const Twiddles tw = run_twiddles(ctx, L0.dtype, L0.U, L0.Vn, L0.X, L0.Y, Nx, x, Ny, y, cv);

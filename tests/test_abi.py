@@ -58,6 +58,18 @@ def test_binding_structs_match_header_layout(libscw, tmp_path):
     assert int(out[5]) == ctypes.sizeof(binding.scw_exterior)
     assert int(out[6]) == binding.scw_exterior.n_re.offset
     assert int(out[7]) == binding.scw_exterior.p_inc.offset
+    # the round-2 descriptors
+    src2 = tmp_path / "sz2.c"
+    src2.write_text('#include "scwatter.h"\n#include <stdio.h>\n#include <stddef.h>\n'
+                    'int main(void){printf("%zu %zu %zu %zu %zu %zu %zu\\n", sizeof(scw_window), sizeof(scw_vbuild),'
+                    ' offsetof(scw_vbuild, psi), sizeof(scw_stack), offsetof(scw_stack, z_if), offsetof(scw_stack, gamma),'
+                    ' offsetof(scw_stack, dir));return 0;}\n')
+    exe2 = tmp_path / "sz2"
+    subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(src2), "-o", str(exe2)], check=True)
+    o2 = [int(v) for v in subprocess.run([str(exe2)], capture_output=True, text=True, check=True).stdout.split()]
+    assert o2 == [ctypes.sizeof(binding.scw_window), ctypes.sizeof(binding.scw_vbuild), binding.scw_vbuild.psi.offset,
+                  ctypes.sizeof(binding.scw_stack), binding.scw_stack.z_if.offset, binding.scw_stack.gamma.offset,
+                  binding.scw_stack.dir.offset]
     assert set(binding.EXPORTS) == set(declared_symbols())
 
 

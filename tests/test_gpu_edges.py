@@ -312,8 +312,8 @@ def test_grouped_sweep_with_an_8_byte_aligned_V(scw, ctx):
 
 def test_last_kernels_tells_which_path_ran(scw, ctx):
     """SCW_PATH_AUTO drops to the CUDA-core kernels for shapes the tensor-core kernels do not take; scw_last_kernels makes
-    that visible: complex64 with 96 frequencies along u (> 80) synthesises on CUDA cores, a small sweep with different J per
-    instance leaves the grouped path (two assembly launches), a regular one takes tc_assemble + tc_synth."""
+    that visible: complex64 with 96 frequencies along u (> 80) synthesises on CUDA cores, a sweep whose instances differ in J
+    is cut into runs of equal shape (one assembly + one synthesis launch each), a regular one takes tc_assemble + tc_synth."""
     lay = ragged_layer(5, 5, 100, np.complex64, seed=7)
     x, y, z = np.arange(20) * 0.15, np.arange(18) * 0.25, np.linspace(-0.3, 0.8, 4)
     L = scw.Layer.from_numpy(lay, "cuda")
@@ -325,8 +325,9 @@ def test_last_kernels_tells_which_path_ran(scw, ctx):
     lay2 = ragged_layer(5, 5, 132, np.complex64, seed=9)
     n0 = ctx.launch_count()
     scw.scw_sweep_wavelengths(ctx, [L, scw.Layer.from_numpy(lay2, "cuda")], [dev(z), dev(z)], dev(x), dev(y))
-    assert ctx.launch_count() - n0 > 3                                       # per-instance launches, not one group
     torch.cuda.synchronize()
+    assert ctx.launch_count() - n0 == 5                                      # twiddles + two runs (J differs) x (assembly, synthesis)
+    assert not any(k.startswith("simt") for k in ctx.last_kernels())
 
 
 def test_twiddle_cache_and_calibration(scw):
@@ -378,3 +379,23 @@ def test_twiddle_cache_and_calibration(scw):
         assert len(c.assembly_timeline()) >= 1
     finally:
         c.close()
+
+
+def test_sweep_with_mixed_shapes_runs_grouped(scw, ctx):
+    """Instances that differ in J and in Fz: consecutive instances of equal shape form a run (one assembly + one synthesis
+    launch per run, all on the tensor-core kernels); every sample of every instance against Tier B."""
+    shapes = [(100, 4), (100, 4), (132, 4), (132, 7), (132, 7), (100, 4)]
+    lays = [ragged_layer(5, 5, J, np.complex64, seed=120 + i) for i, (J, _) in enumerate(shapes)]
+    zs = [np.linspace(-0.3, 0.8, fz) for _, fz in shapes]
+    x, y = np.arange(150) * 3.0 / 150, np.arange(40) * 4.5 / 40
+    Ls = [scw.Layer.from_numpy(l, "cuda") for l in lays]
+    n0 = ctx.launch_count()
+    Es = scw.scw_sweep_wavelengths(ctx, Ls, [dev(z) for z in zs], dev(x), dev(y))
+    S = scw.scw_sweep_detector(ctx, Ls, [dev(z) for z in zs], dev(x), dev(y), window=(3, 140, 2, 33), want_I=False)[1]
+    torch.cuda.synchronize()
+    for lay, z, E, s in zip(lays, zs, Es, S):
+        ref = oracle.tier_b_grid(x=x, y=y, z=z, **lay)
+        assert rel_err(E.cpu().numpy(), ref) <= 2e-4
+        sref = oracle.window_sum(oracle.intensity(ref), (3, 140, 2, 33))
+        assert np.abs(s.cpu().numpy() - sref).max() / sref.max() <= 4e-4
+    assert not any(k.startswith("simt") for k in ctx.last_kernels())
