@@ -268,6 +268,14 @@ typedef struct {
  * No workspace.  Errors: NULL, SHAPE, DTYPE, ALIGN, VALUE, CUDA. */
 int32_t scw_exterior_spectra(scw_ctx* ctx, const scw_exterior* ext, int64_t Fz, const double* z, void* P, int64_t ldP);
 
+/* eq. 9 followed by eq. 10 on a rectilinear grid in ONE call: E as in scw_synthesize_grid (strides, planar default).  For
+ * SCW_C64 with at most 80 frequencies per axis eq. 9 is evaluated straight into the synthesis kernel's operand (P is never
+ * written) and the twiddle tables are kept under SCW_OPT_CACHE like a sweep's; otherwise it is scw_exterior_spectra into
+ * the workspace + the synthesis.  Errors: as scw_exterior_spectra and scw_synthesize_grid, WORKSPACE. */
+int32_t scw_exterior_grid(scw_ctx* ctx, const scw_exterior* ext, int64_t Fz, const double* z,
+                          int64_t Nx, const double* x, int64_t Ny, const double* y, void* E, const int64_t* strides);
+int32_t scw_exterior_grid_workspace(scw_ctx* ctx, const scw_exterior* ext, int64_t Fz, int64_t Nx, int64_t Ny, size_t* bytes);
+
 /* eq. 9-10 at scattered points: the M (below) or 2M (above) plane waves are tabulated in the workspace and summed by
  * the direct plane-wave kernels of scw_eval_points.  r: [N x 3] doubles, E: [N x 3] complex<dtype>, comp fastest. */
 int32_t scw_exterior_points(scw_ctx* ctx, const scw_exterior* ext, int64_t N, const double* r, void* E);

@@ -28,7 +28,8 @@ EXPORTS = [
     "scw_eval_points", "scw_points_workspace", "scw_sweep_wavelengths", "scw_sweep_workspace",
     "scw_sweep_wavelengths_host", "scw_sweep_host_workspace",
     "scw_profile_classes", "scw_profile_name", "scw_profile_read", "scw_profile_reset",
-    "scw_exterior_spectra", "scw_exterior_points", "scw_exterior_points_workspace",
+    "scw_exterior_spectra", "scw_exterior_points", "scw_exterior_points_workspace", "scw_exterior_grid",
+    "scw_exterior_grid_workspace",
     "scw_sweep_intensity", "scw_sweep_intensity_workspace",
     "scw_measure_peak", "scw_invalidate_cache", "scw_calibrate", "scw_profile_assembly",
     "scw_sweep_detector", "scw_sweep_detector_workspace", "scw_absorbance", "scw_build_V", "scw_build_V_workspace", "scw_propagate_alpha", "scw_propagate_alpha_workspace",
@@ -130,6 +131,9 @@ def lib():
         L.scw_sweep_intensity.argtypes = L.scw_sweep_wavelengths.argtypes
         L.scw_sweep_intensity_workspace.argtypes = L.scw_sweep_workspace.argtypes
         L.scw_exterior_spectra.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, c_void_p, c_void_p, c_int64]
+        L.scw_exterior_grid.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, c_void_p, c_int64, c_void_p, c_int64, c_void_p,
+                                        c_void_p, POINTER(c_int64)]
+        L.scw_exterior_grid_workspace.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, c_int64, c_int64, POINTER(c_size_t)]
         L.scw_exterior_points.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, c_void_p, c_void_p]
         L.scw_exterior_points_workspace.argtypes = [c_void_p, POINTER(scw_exterior), c_int64, POINTER(c_size_t)]
         L.scw_sweep_detector.argtypes = L.scw_sweep_wavelengths.argtypes + [POINTER(scw_window), POINTER(c_void_p)]
@@ -396,6 +400,20 @@ def scw_exterior_spectra(ctx, ext, z, out=None):
     if out is None:
         out = torch.empty((Fz, R), dtype=ext.p_face.dtype, device=ctx.device)
     ctx.check(ctx.L.scw_exterior_spectra(ctx._h, byref(st), Fz, _p(z), _p(out), out.shape[1] if Fz else R))
+    return out
+
+
+def scw_exterior_grid(ctx, ext, z, x, y, out=None, strides=None):
+    """eq. 9-10 on a rectilinear grid in one call: E (Fz, 3, Ny, Nx)."""
+    Fz, Nx, Ny = z.numel(), x.numel(), y.numel()
+    st = ext.struct()
+    need = c_size_t()
+    ctx.check(ctx.L.scw_exterior_grid_workspace(ctx._h, byref(st), Fz, Nx, Ny, byref(need)))
+    ctx.reserve(need.value)
+    if out is None:
+        out = torch.empty((Fz, 3, Ny, Nx), dtype=ext.p_face.dtype, device=ctx.device)
+    sarr = None if strides is None else (c_int64 * 4)(*strides)
+    ctx.check(ctx.L.scw_exterior_grid(ctx._h, byref(st), Fz, _p(z), Nx, _p(x), Ny, _p(y), _p(out), sarr))
     return out
 
 

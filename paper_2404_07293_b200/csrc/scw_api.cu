@@ -1101,6 +1101,57 @@ int32_t scw_exterior_spectra(scw_ctx* ctx, const scw_exterior* ext, int64_t Fz, 
     return check_launch(ctx, "scw_exterior_spectra");
 }
 
+// eq. 9 + eq. 10 on a rectilinear grid in one call.  complex64 within the tensor-core synthesis' reach: twiddles (kept under
+// SCW_OPT_CACHE), eq. 9 straight into the spectrum images, synthesis -- 3 launches, 2 cached, P never in memory; otherwise
+// scw_exterior_spectra into the workspace followed by the synthesis of scw_synthesize_grid.
+static size_t exterior_grid_ws(const scw_ctx* ctx, const scw_exterior* e, int64_t Fz, int64_t Nx, int64_t Ny)
+{
+    const size_t tw = twiddle_ws(ctx, e->dtype, e->U, e->Vn, Nx, Ny), sy = synth_ws(ctx, e->dtype, e->U, e->Vn, Fz, Ny);
+    if (use_tc_synth(ctx, e->dtype, e->U, e->Vn)) return tw + sy;
+    return tw + sy + align_up((size_t)3 * e->U * e->Vn * Fz * esize(e->dtype));
+}
+
+int32_t scw_exterior_grid_workspace(scw_ctx* ctx, const scw_exterior* ext, int64_t Fz, int64_t Nx, int64_t Ny, size_t* bytes)
+{
+    if (!ctx || !bytes) return SCW_ERR_NULL;
+    ctx->msg[0] = 0;
+    if (int32_t s = check_exterior(ctx, ext, "scw_exterior_grid_workspace")) return s;
+    if (Fz < 0 || Nx <= 0 || Ny <= 0) return fail(ctx, SCW_ERR_SHAPE, "scw_exterior_grid_workspace: bad dimensions");
+    *bytes = Fz ? exterior_grid_ws(ctx, ext, Fz, Nx, Ny) : 0;
+    return SCW_OK;
+}
+
+int32_t scw_exterior_grid(scw_ctx* ctx, const scw_exterior* ext, int64_t Fz, const double* z, int64_t Nx, const double* x,
+                          int64_t Ny, const double* y, void* E, const int64_t* strides)
+{
+    if (int32_t s = check_ctx(ctx, true)) return s;           // keeps the twiddle cache (same place in the workspace as a sweep's)
+    ctx->clean_ctl = nullptr;                                  // ... but a sweep's control block and images may be overwritten
+    ctx->clean_img = nullptr;
+    if (int32_t s = check_exterior(ctx, ext, "scw_exterior_grid")) return s;
+    if (int32_t s = check_grid(ctx, ext->dtype, ext->U, ext->Vn, ext->X, ext->Y, Nx, x, Ny, y, "scw_exterior_grid")) return s;
+    if (Fz < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_exterior_grid: Fz=%lld < 0", (long long)Fz);
+    if (Fz == 0) return SCW_OK;
+    if (!z || !E) return fail(ctx, SCW_ERR_NULL, "scw_exterior_grid: z and E are required");
+    if (!aligned(z, 8) || !aligned(E, esize(ext->dtype))) return fail(ctx, SCW_ERR_ALIGN, "scw_exterior_grid: z/E misaligned");
+    int64_t s4[4];
+    if (strides) memcpy(s4, strides, sizeof(s4)); else planar_strides(Nx, Ny, s4);
+    for (int i = 0; i < 4; ++i)
+        if (s4[i] < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_exterior_grid: negative stride");
+    if (int32_t s = need_ws(ctx, exterior_grid_ws(ctx, ext, Fz, Nx, Ny), "scw_exterior_grid")) return s;
+    Carver cv(ctx->ws);
+    const Twiddles tw = run_twiddles(ctx, ext->dtype, ext->U, ext->Vn, ext->X, ext->Y, Nx, x, Ny, y, cv);
+    void* scratch = cv.take(synth_ws(ctx, ext->dtype, ext->U, ext->Vn, Fz, Ny));
+    if (tw.tc) {
+        launch_tc_synth_exterior(ctx, ext, Fz, z, Nx, Ny, tw.a, E, s4, scratch);
+    } else {
+        const int64_t R = 3LL * ext->U * ext->Vn;
+        void* P = cv.take((size_t)R * Fz * esize(ext->dtype));
+        launch_exterior_spectra(ctx, ext, Fz, z, P, R);
+        run_synth(ctx, tw, ext->dtype, ext->U, ext->Vn, Fz, P, R, Nx, Ny, E, s4, scratch);
+    }
+    return check_launch(ctx, "scw_exterior_grid");
+}
+
 int32_t scw_exterior_points_workspace(scw_ctx* ctx, const scw_exterior* ext, int64_t N, size_t* bytes)
 {
     if (!ctx || !bytes) return SCW_ERR_NULL;

@@ -216,6 +216,9 @@ void launch_tc_synth_group_images(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n
                                   const TcDetector* det = nullptr);
 void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,
                      const void* tw, void* E, const int64_t strides[4], void* scratch);
+// Exterior field (eq. 9-10) on a grid, complex64: spectrum images from eq. 9 directly, then the synthesis; scratch = tc_synth_scratch(U, Vn, Fz)
+void launch_tc_synth_exterior(scw_ctx* ctx, const scw_exterior* e, int64_t Fz, const double* z, int64_t Nx, int64_t Ny,
+                              const void* tw, void* E, const int64_t strides[4], void* scratch);
 
 // ---- scw_dmma.cu: FP64 tensor-core (DMMA mma.sync) batched complex GEMM for the complex128 contractions -----------
 bool dmma_supported(int dtype);

@@ -18,6 +18,7 @@
 // produced by two small pre-kernels and fetched with bulk async copies.
 #include "scw_internal.h"
 #include "scw_tc_common.cuh"
+#include "scw_exterior.cuh"
 
 namespace scw {
 
@@ -161,6 +162,64 @@ __global__ void k_tc_synth_pimage(int U, int Vn, int Uc, int Vc, int nuc, int nv
     }
     const size_t img_bytes = (size_t)N1 * K1p * 2;
     ts_image_store(img + (size_t)image * 2 * img_bytes, img_bytes, N1, ul, vl, p.x, p.y);
+}
+
+// Exterior field straight into the spectrum images (eq. 9, then eq. 10 by the synthesis kernel): thread =
+// (z plane, image (uc, vc), vl, ul) evaluates p_comp(s_m, z) = p_inc G[s_z, z_inc, z] + p_face G[-/+ s_z, z_face, z] for the
+// three components (one s_z, two propagators) and writes their image entries; P never goes to memory.
+struct TsExterior {
+    int side;
+    double lam_over_X, lam_over_Y, inv_lambda, n_re, n_im, z_face, z_inc;
+    const float2* p_face;
+    const float2* p_inc;
+};
+
+__global__ void k_tc_synth_exterior_images(int U, int Vn, int Uc, int Vc, int nuc, int nvc, int K1p, int N1, int Fz,
+                                           const TsExterior e, const double* __restrict__ z, uint8_t* __restrict__ img,
+                                           int* __restrict__ sched, int n_sched)
+{
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;      // (plane n, uc, vc, vl, ul), ul fastest
+    for (int64_t i = idx; i < n_sched; i += (int64_t)gridDim.x * blockDim.x) sched[i] = 0;
+    const int half_n = N1 / 2, kpairs = K1p / 2;
+    if (idx >= (int64_t)Fz * nuc * nvc * half_n * kpairs) return;
+    const int ul = (int)(idx % half_n);
+    int64_t rest = idx / half_n;
+    const int vl = (int)(rest % kpairs);
+    rest /= kpairs;
+    const int vc = (int)(rest % nvc);
+    rest /= nvc;
+    const int uc = (int)(rest % nuc);
+    const int64_t n = rest / nuc;
+    const int u = uc * Uc + ul, v = vc * Vc + vl;
+    const bool real = ul < Uc && vl < Vc && u < U && v < Vn;
+    float2 p[3] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};      // padding entries: zeros
+    if (real) {
+        const int m = v * U + u;
+        const double sx = (double)(u - U / 2) * e.lam_over_X, sy = (double)(v - Vn / 2) * e.lam_over_Y;
+        const double2 sz = ext_sz(e.n_re, e.n_im, sx, sy);
+        const double zi = z[n];
+        const double2 gf = e.side == SCW_SIDE_BELOW ? sz : make_double2(-sz.x, -sz.y);
+        const double2 wf = ext_green(gf, (zi - e.z_face) * e.inv_lambda);
+        const bool inc = e.side == SCW_SIDE_ABOVE && e.p_inc != nullptr;
+        const double2 wi = inc ? ext_green(sz, (zi - e.z_inc) * e.inv_lambda) : make_double2(0.0, 0.0);
+#pragma unroll
+        for (int comp = 0; comp < 3; ++comp) {
+            const float2 a = e.p_face[3 * m + comp];
+            double er = (double)a.x * wf.x - (double)a.y * wf.y, ei = (double)a.x * wf.y + (double)a.y * wf.x;
+            if (inc) {
+                const float2 b = e.p_inc[3 * m + comp];
+                er += (double)b.x * wi.x - (double)b.y * wi.y;
+                ei += (double)b.x * wi.y + (double)b.y * wi.x;
+            }
+            p[comp] = make_float2((float)er, (float)ei);
+        }
+    }
+    const size_t img_bytes = (size_t)N1 * K1p * 2;
+#pragma unroll
+    for (int comp = 0; comp < 3; ++comp) {
+        const int64_t image = ((n * 3 + comp) * nuc + uc) * nvc + vc;
+        ts_image_store(img + (size_t)image * 2 * img_bytes, img_bytes, N1, ul, vl, p[comp].x, p[comp].y);
+    }
 }
 
 // ---- main kernel ------------------------------------------------------------------------------------
@@ -737,6 +796,33 @@ void launch_tc_synth_group_images(scw_ctx* ctx, int U, int Vn, int64_t Fz, int n
 {
     const TsPlan pl = ts_plan(U, Vn, Fz * n_inst, Nx, Ny);
     ts_launch_main(ctx, pl, Fz, n_inst, static_cast<const uint8_t*>(scratch), Nx, Ny, tw, E, strides, det);
+}
+
+// Exterior field on a grid in two launches: eq. 9 into the spectrum images, then the synthesis (eq. 10).
+void launch_tc_synth_exterior(scw_ctx* ctx, const scw_exterior* e, int64_t Fz, const double* z, int64_t Nx, int64_t Ny,
+                              const void* tw, void* E, const int64_t strides[4], void* scratch)
+{
+    const TsPlan pl = ts_plan(e->U, e->Vn, Fz, Nx, Ny);
+    uint8_t* B1 = static_cast<uint8_t*>(scratch);
+    TsExterior te;
+    te.side = e->side;
+    te.lam_over_X = e->lambda / e->X;
+    te.lam_over_Y = e->lambda / e->Y;
+    te.inv_lambda = 1.0 / e->lambda;
+    te.n_re = e->n_re;
+    te.n_im = e->n_im;
+    te.z_face = e->z_face;
+    te.z_inc = e->z_inc;
+    te.p_face = static_cast<const float2*>(e->p_face);
+    te.p_inc = static_cast<const float2*>(e->p_inc);
+    {
+        KernelScope ks(ctx, KC_EXTERIOR);
+        const int64_t n = Fz * pl.cu.n * pl.cv.n * (pl.K2p / 2) * (pl.K1p / 2);
+        k_tc_synth_exterior_images<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(
+            e->U, e->Vn, pl.cu.len, pl.cv.len, pl.cu.n, pl.cv.n, pl.K1p, pl.K2p, (int)Fz, te, z, B1, ts_sched(pl, tw),
+            pl.tiles_x * pl.tiles_y);
+    }
+    ts_launch_main(ctx, pl, Fz, 1, B1, Nx, Ny, tw, &E, strides, nullptr);
 }
 
 void launch_tc_synth(scw_ctx* ctx, int U, int Vn, int64_t Fz, const void* P, int64_t ldP, int64_t Nx, int64_t Ny,

@@ -102,3 +102,41 @@ def test_exterior_edges_and_errors(scw, ctx):
     with pytest.raises(scw.ScwError) as e:
         scw.scw_exterior_spectra(ctx, scw.Exterior.from_numpy(dict(ext, lam=-1.0), "cuda"), dev(z))
     assert e.value.status == 5
+
+
+@pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 2e-4)])
+@pytest.mark.parametrize("side", [0, 1])
+@pytest.mark.parametrize("U,Vn", [(9, 9), (45, 12)])
+def test_exterior_grid_one_call(scw, dtype, tol, side, U, Vn):
+    """scw_exterior_grid (eq. 9 straight into the synthesis operand for complex64; spectra + synthesis for complex128):
+    every sample against the eq. 9-10 oracle, ragged grid, two frequency chunks along u, custom strides, twice with the
+    twiddle cache on (the second call reuses the tables), then with other planes."""
+    cfg = si.Config(6, "exterior grid", U, Vn, 8.0, (1.0,), 1, 1, 0, 0, (dtype,))
+    ext = si.make_exterior(cfg, side, dtype=dtype)
+    g = np.random.default_rng(U + side)
+    x, y = np.sort(g.uniform(0, 8, 150)), np.sort(g.uniform(0, 8, 37))
+    z = ext_z(ext, 5, ext["lam"])
+    ref = oracle.exterior_grid(x=x, y=y, z=z, **ext)
+    c = scw.Context(0)
+    try:
+        c.set_cache(True)
+        X = scw.Exterior.from_numpy(ext, "cuda")
+        dx, dy = dev(x), dev(y)
+        n0 = c.launch_count()
+        E1 = scw.scw_exterior_grid(c, X, dev(z), dx, dy).clone()
+        n1 = c.launch_count()
+        out = torch.zeros((5, 37, 150, 3), dtype=E1.dtype, device="cuda")             # [z][y][x][comp]
+        scw.scw_exterior_grid(c, X, dev(z), dx, dy, out=out, strides=(1, 37 * 150 * 3, 150 * 3, 3))
+        n2 = c.launch_count()
+        z2 = ext_z(ext, 3, 0.5 * ext["lam"])
+        E3 = scw.scw_exterior_grid(c, X, dev(z2), dx, dy)
+        torch.cuda.synchronize()
+        scale = np.abs(ref).max()
+        assert np.abs(E1.cpu().numpy() - ref).max() / scale <= tol
+        assert torch.equal(out.permute(0, 3, 1, 2), E1)
+        assert np.abs(E3.cpu().numpy() - oracle.exterior_grid(x=x, y=y, z=z2, **ext)).max() / scale <= tol
+        if dtype == np.complex64:
+            assert n1 - n0 == 3 and n2 - n1 == 2                   # twiddles + images + synthesis, then cached twiddles
+            assert "tc_synth" in c.last_kernels()
+    finally:
+        c.close()
