@@ -459,7 +459,7 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
         ms_per_layer=ms, n=n_a,
         roofline=dict(bound="tensor", achieved=lu_tf, peak=peaks.get("fp64_dmma_tflops"), unit="TFLOP/s (fp64, 8/3 n^3 for the complex LU)",
                       frac=lu_tf / peaks["fp64_dmma_tflops"] if peaks.get("fp64_dmma_tflops") else None, traffic=None,
-                      note="bound by the 2 grid barriers per column of the cooperative panel kernel, not by the tensor cores"))
+                      note="bound by the grid barrier per column of the cooperative panel kernel (half of the time) and by K = 64 trailing GEMMs, not by the tensor-core rate"))
     del Qa, gma, r0a
     torch.cuda.empty_cache()
     if not args.skip_large:

@@ -8,8 +8,8 @@
 // Everything runs in fp64 (complex64 inputs are widened; a 4356 x 4356 LU in fp32 would lose the 2e-4 bar):
 //   LU      blocked right-looking with partial pivoting, panels of 64 columns:
 //             k_lu_panel   one cooperative launch per panel; the panel's rows are spread over the CTAs (in shared memory),
-//                          per column: local |.|_1 maximum -> grid barrier -> pivot row exchanged through global memory
-//                          -> grid barrier -> scale + rank-1 update
+//                          per column: local |.|_1 maximum, candidate row and diagonal row published -> ONE grid
+//                          barrier -> pivot chosen, rows interchanged, scale + rank-1 update
 //             k_lu_laswp   the panel's row interchanges applied to the columns outside the panel
 //             k_lu_trsm    U12 = L11^-1 A12, one warp per column (also written row-major for the GEMM)
 //             k_dmma_cgemm A22 -= L21 U12 on the FP64 tensor cores (scw_dmma.cu, 3M complex product)
@@ -23,6 +23,9 @@ namespace scw {
 constexpr int LU_NB = 64;                  // panel width
 constexpr int LU_RPC = 128;                // max panel rows per CTA (shared memory: 128 x 64 x 16 B = 128 KB)
 constexpr int LU_THREADS = 256;
+#ifndef LU_ROWS_WANTED
+#define LU_ROWS_WANTED 32                   // panel rows per CTA aimed at (32, 64, 96, 128 measured: 32 is the fastest)
+#endif
 
 __device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 __device__ __forceinline__ double2 cdiv(double2 a, double2 b)
@@ -45,7 +48,7 @@ struct LuPanel {
     unsigned* bar;         // grid barrier counter (zero at launch)
     double* slot_val;      // [2][grid] local maxima
     int* slot_row;         // [2][grid]
-    double2* rowbuf;       // [2][2][LU_NB]: pivot row, diagonal row of the current column (double-buffered by column parity)
+    double2* rowbuf;       // [2][grid + 1][LU_NB]: every CTA's candidate row, then the diagonal row (double-buffered by column parity)
     int* info;             // set to column + 1 on an exactly zero pivot (first one wins)
 };
 
@@ -72,7 +75,7 @@ __global__ void __launch_bounds__(LU_THREADS, 1) k_lu_panel(const LuPanel p)
     __shared__ double2 pr[LU_NB];                                 // pivot row of the current column
     __shared__ double red_v[LU_THREADS / 32];
     __shared__ int red_r[LU_THREADS / 32];
-    __shared__ int s_piv;
+    __shared__ int s_piv, s_win;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nb = p.nb, rpc = p.rpc;
     const int64_t row0 = p.k0 + (int64_t)blockIdx.x * rpc;        // first global row of this CTA
@@ -88,7 +91,9 @@ __global__ void __launch_bounds__(LU_THREADS, 1) k_lu_panel(const LuPanel p)
     for (int j = 0; j < nb; ++j) {
         const int par = j & 1;
         const int64_t gj = p.k0 + j;                              // global row / column of the diagonal
-        // ---- 1. local maximum of |re| + |im| over this CTA's rows >= gj (ties: the smaller row)
+        // ---- 1. local maximum of |re| + |im| over this CTA's rows >= gj (ties: the smaller row); the candidate row itself
+        // (all nb entries) is published with it, and the owner of the diagonal row publishes that row: ONE grid barrier per
+        // column instead of two
         double bv = -1.0;
         int br = 0x7fffffff;
         for (int r = tid; r < rows; r += LU_THREADS) {
@@ -111,25 +116,37 @@ __global__ void __launch_bounds__(LU_THREADS, 1) k_lu_panel(const LuPanel p)
                 if (red_v[w] > bv || (red_v[w] == bv && red_r[w] < br)) { bv = red_v[w]; br = red_r[w]; }
             p.slot_val[par * gridDim.x + blockIdx.x] = bv;
             p.slot_row[par * gridDim.x + blockIdx.x] = br;
+            s_piv = br;                                            // local candidate (0x7fffffff: none)
+        }
+        __syncthreads();
+        double2* rows_par = p.rowbuf + (size_t)par * (gridDim.x + 1) * LU_NB;
+        {
+            const int lb = s_piv;
+            if (lb != 0x7fffffff)
+                for (int c = tid; c < nb; c += LU_THREADS) rows_par[(size_t)blockIdx.x * LU_NB + c] = a[c * rpc + (lb - (int)row0)];
+            if (gj >= row0 && gj < row0 + rows)
+                for (int c = tid; c < nb; c += LU_THREADS) rows_par[(size_t)gridDim.x * LU_NB + c] = a[c * rpc + (int)(gj - row0)];
         }
         lu_grid_sync(p.bar, target);
-        // ---- 2. global pivot; its row and the diagonal row go through global memory
+        // ---- 2. global pivot = the best candidate; interchange with the diagonal row
         if (warp == 0) {
             double gv = -1.0;
-            int gr = 0x7fffffff;
+            int gr = 0x7fffffff, gc = 0;
             for (int c = lane; c < (int)gridDim.x; c += 32) {
                 const double v = __ldcg(&p.slot_val[par * gridDim.x + c]);       // written by other SMs: L2, not L1
                 const int r = __ldcg(&p.slot_row[par * gridDim.x + c]);
-                if (v > gv || (v == gv && r < gr)) { gv = v; gr = r; }
+                if (v > gv || (v == gv && r < gr)) { gv = v; gr = r; gc = c; }
             }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
                 const double ov = __shfl_xor_sync(0xffffffffu, gv, o);
                 const int orow = __shfl_xor_sync(0xffffffffu, gr, o);
-                if (ov > gv || (ov == gv && orow < gr)) { gv = ov; gr = orow; }
+                const int oc = __shfl_xor_sync(0xffffffffu, gc, o);
+                if (ov > gv || (ov == gv && orow < gr)) { gv = ov; gr = orow; gc = oc; }
             }
             if (lane == 0) {
                 s_piv = gr;
+                s_win = gc;
                 if (blockIdx.x == 0) {
                     p.piv[gj] = gr;
                     if (!(gv > 0.0)) atomicCAS(p.info, 0, (int)gj + 1);
@@ -138,19 +155,12 @@ __global__ void __launch_bounds__(LU_THREADS, 1) k_lu_panel(const LuPanel p)
         }
         __syncthreads();
         const int64_t pv = s_piv;
-        double2* buf = p.rowbuf + (size_t)par * 2 * LU_NB;
-        if (pv >= row0 && pv < row0 + rows)
-            for (int c = tid; c < nb; c += LU_THREADS) buf[c] = a[c * rpc + (int)(pv - row0)];
-        if (pv != gj && gj >= row0 && gj < row0 + rows)
-            for (int c = tid; c < nb; c += LU_THREADS) buf[LU_NB + c] = a[c * rpc + (int)(gj - row0)];
-        lu_grid_sync(p.bar, target);
-        // ---- 3. interchange, scale, rank-1 update
-        for (int c = tid; c < nb; c += LU_THREADS) pr[c] = __ldcg(&buf[c]);
+        for (int c = tid; c < nb; c += LU_THREADS) pr[c] = __ldcg(&rows_par[(size_t)s_win * LU_NB + c]);
         if (pv != gj) {
             if (pv >= row0 && pv < row0 + rows)
-                for (int c = tid; c < nb; c += LU_THREADS) a[c * rpc + (int)(pv - row0)] = __ldcg(&buf[LU_NB + c]);
+                for (int c = tid; c < nb; c += LU_THREADS) a[c * rpc + (int)(pv - row0)] = __ldcg(&rows_par[(size_t)gridDim.x * LU_NB + c]);
             if (gj >= row0 && gj < row0 + rows)
-                for (int c = tid; c < nb; c += LU_THREADS) a[c * rpc + (int)(gj - row0)] = __ldcg(&buf[c]);
+                for (int c = tid; c < nb; c += LU_THREADS) a[c * rpc + (int)(gj - row0)] = __ldcg(&rows_par[(size_t)s_win * LU_NB + c]);
         }
         __syncthreads();
         const double2 pivot = pr[j];
@@ -243,19 +253,25 @@ __global__ void __launch_bounds__(256) k_lu_apply_piv(int64_t n, const int* __re
     for (int64_t i = threadIdx.x; i < n; i += 256) dst[i] = src[perm[i]];
 }
 
-// Diagonal block [k0, k0 + nb) of the forward (unit lower) or backward (upper) substitution: one warp.
-__global__ void __launch_bounds__(32) k_trsv_block(const double2* __restrict__ A, int64_t ld, int64_t k0, int nb, int upper,
-                                                   double2* __restrict__ x)
+// Diagonal block [k0, k0 + nb) of the forward (unit lower) or backward (upper) substitution: the nb x nb block is staged in
+// shared memory by the whole CTA (the substitution itself is a chain of nb dependent steps: it must not wait on global
+// memory at every step), then one warp solves.
+__global__ void __launch_bounds__(256) k_trsv_block(const double2* __restrict__ A, int64_t ld, int64_t k0, int nb, int upper,
+                                                    double2* __restrict__ x)
 {
+    extern __shared__ __align__(16) unsigned char trsv_smem[];
+    double2* T = reinterpret_cast<double2*>(trsv_smem);            // column-major nb x nb
     __shared__ double2 xs[LU_NB];
+    for (int idx = threadIdx.x; idx < nb * nb; idx += 256) T[idx] = A[(k0 + idx / nb) * ld + k0 + idx % nb];
+    for (int i = threadIdx.x; i < nb; i += 256) xs[i] = x[k0 + i];
+    __syncthreads();
+    if (threadIdx.x >= 32) return;
     const int lane = threadIdx.x;
-    for (int i = lane; i < nb; i += 32) xs[i] = x[k0 + i];
-    __syncwarp();
     if (!upper) {
         for (int k = 0; k < nb; ++k) {
             const double2 xk = xs[k];
             for (int i = k + 1 + lane; i < nb; i += 32) {
-                const double2 l = A[(k0 + k) * ld + k0 + i];
+                const double2 l = T[k * nb + i];
                 xs[i].x -= l.x * xk.x - l.y * xk.y;
                 xs[i].y -= l.x * xk.y + l.y * xk.x;
             }
@@ -263,11 +279,11 @@ __global__ void __launch_bounds__(32) k_trsv_block(const double2* __restrict__ A
         }
     } else {
         for (int k = nb - 1; k >= 0; --k) {
-            if (lane == 0) xs[k] = cdiv(xs[k], A[(k0 + k) * ld + k0 + k]);
+            if (lane == 0) xs[k] = cdiv(xs[k], T[k * nb + k]);
             __syncwarp();
             const double2 xk = xs[k];
             for (int i = lane; i < k; i += 32) {
-                const double2 u = A[(k0 + k) * ld + k0 + i];
+                const double2 u = T[k * nb + i];
                 xs[i].x -= u.x * xk.x - u.y * xk.y;
                 xs[i].y -= u.x * xk.y + u.y * xk.x;
             }
@@ -348,20 +364,22 @@ __global__ void k_alpha_scale(int64_t n, double t_over_lambda, const double2* __
     w[j] = wj;
 }
 
-// r = Q w with the caller's Q (either dtype), fp64 accumulation: one warp per 32 rows x a slice of columns would need a
-// second pass; one thread per row with coalesced reads along rows is enough for a matrix-vector product.
+// r = Q w with the caller's Q (either dtype), fp64 accumulation.  grid = (row blocks, MV_SLICES column slices): every CTA
+// writes the partial sums of its slice, k_alpha_matvec_sum adds the slices in a fixed order (deterministic).
+constexpr int MV_SLICES = 16;
 template <typename T2>
 __global__ void __launch_bounds__(256) k_alpha_matvec(int64_t n, int64_t ldQ, const T2* __restrict__ Q, const double2* __restrict__ w,
-                                                     double2* __restrict__ r)
+                                                     double2* __restrict__ part)
 {
     __shared__ double2 ws[256];
     const int64_t row = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    const int64_t per = (n + MV_SLICES - 1) / MV_SLICES, c_begin = blockIdx.y * per, c_end = min(n, c_begin + per);
     double2 acc = make_double2(0.0, 0.0);
-    for (int64_t c0 = 0; c0 < n; c0 += 256) {
+    for (int64_t c0 = c_begin; c0 < c_end; c0 += 256) {
         __syncthreads();
-        if (c0 + threadIdx.x < n) ws[threadIdx.x] = w[c0 + threadIdx.x];
+        if (c0 + threadIdx.x < c_end) ws[threadIdx.x] = w[c0 + threadIdx.x];
         __syncthreads();
-        const int cn = (int)min((int64_t)256, n - c0);
+        const int cn = (int)min((int64_t)256, c_end - c0);
         if (row < n)
             for (int c = 0; c < cn; ++c) {
                 const T2 q = Q[(c0 + c) * ldQ + row];
@@ -369,7 +387,19 @@ __global__ void __launch_bounds__(256) k_alpha_matvec(int64_t n, int64_t ldQ, co
                 acc.y += (double)q.x * ws[c].y + (double)q.y * ws[c].x;
             }
     }
-    if (row < n) r[row] = acc;
+    if (row < n) part[(int64_t)blockIdx.y * n + row] = acc;
+}
+
+__global__ void k_alpha_matvec_sum(int64_t n, const double2* __restrict__ part, double2* __restrict__ r)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double2 acc = make_double2(0.0, 0.0);
+    for (int s = 0; s < MV_SLICES; ++s) {
+        acc.x += part[(int64_t)s * n + i].x;
+        acc.y += part[(int64_t)s * n + i].y;
+    }
+    r[i] = acc;
 }
 
 template <typename T2>
@@ -387,7 +417,7 @@ __global__ void k_alpha_vec_out(int64_t n, const double2* __restrict__ src, T2* 
 static int lu_grid(const scw_ctx* ctx, int64_t rows, int* rpc)
 {
     int g = (int)((rows + LU_RPC - 1) / LU_RPC);
-    const int want = (int)std::min<int64_t>(ctx->sm_count, (rows + 31) / 32);     // >= 32 rows per CTA when possible
+    const int want = (int)std::min<int64_t>(ctx->sm_count, (rows + LU_ROWS_WANTED - 1) / LU_ROWS_WANTED);
     if (g < want) g = want;
     if (g < 1) g = 1;
     *rpc = (int)((rows + g - 1) / g);
@@ -395,6 +425,11 @@ static int lu_grid(const scw_ctx* ctx, int64_t rows, int* rpc)
 }
 
 // rows of a panel per CTA <= LU_RPC (shared memory) and the interchange replay holds 8 n bytes of shared memory
+static size_t lu_misc_bytes(const scw_ctx* ctx)
+{
+    return 64 + align_up((size_t)2 * ctx->sm_count * 12, 64) + (size_t)2 * (ctx->sm_count + 1) * LU_NB * 16;
+}
+
 bool alpha_supported(const scw_ctx* ctx, int64_t n)
 {
     return n >= 1 && (n + ctx->sm_count - 1) / ctx->sm_count <= LU_RPC && n * 8 <= 200 * 1024;
@@ -403,7 +438,7 @@ bool alpha_supported(const scw_ctx* ctx, int64_t n)
 size_t alpha_scratch(const scw_ctx* ctx, int64_t n)
 {
     return align_up((size_t)n * n * 16) + align_up((size_t)LU_NB * n * 16) + 3 * align_up((size_t)n * 16) + align_up((size_t)n * 4) +
-           align_up(4096 + (size_t)4 * ctx->sm_count * 12);
+           align_up(lu_misc_bytes(ctx));
 }
 
 void launch_propagate_alpha(scw_ctx* ctx, const scw_stack* st, const void* r0, void* const* alpha, void* rL, void* scratch)
@@ -417,12 +452,12 @@ void launch_propagate_alpha(scw_ctx* ctx, const scw_stack* st, const void* r0, v
     double2* y = (double2*)cv.take((size_t)n * 16);
     double2* w = (double2*)cv.take((size_t)n * 16);
     int* piv = (int*)cv.take((size_t)n * 4);
-    char* misc = (char*)cv.take(4096 + (size_t)4 * ctx->sm_count * 12);
+    char* misc = (char*)cv.take(lu_misc_bytes(ctx));
     unsigned* bar = (unsigned*)misc;                       // [0]: barrier counter, [1]: info
     int* info = (int*)(misc + 4);
-    double2* rowbuf = (double2*)(misc + 64);               // 4 * 64 * 16 = 4096 - 64 ... keep inside the first 4 KB + slots
-    double* slot_val = (double*)(misc + 64 + 4 * LU_NB * 16);
-    int* slot_row = (int*)(slot_val + 2 * ctx->sm_count);
+    double* slot_val = (double*)(misc + 64);               // [2][#SM]
+    int* slot_row = (int*)(slot_val + 2 * ctx->sm_count);  // [2][#SM]
+    double2* rowbuf = (double2*)(misc + 64 + align_up((size_t)2 * ctx->sm_count * 12, 64));   // [2][#SM + 1][LU_NB]
     const unsigned vb = (unsigned)((n + 255) / 256);
     {
         KernelScope ks(ctx, KC_ALPHA);
@@ -431,6 +466,7 @@ void launch_propagate_alpha(scw_ctx* ctx, const scw_stack* st, const void* r0, v
     }
     cudaFuncSetAttribute(k_lu_panel, cudaFuncAttributeMaxDynamicSharedMemorySize, LU_RPC * LU_NB * 16);
     cudaFuncSetAttribute(k_lu_trsm, cudaFuncAttributeMaxDynamicSharedMemorySize, LU_NB * LU_NB * 16);
+    cudaFuncSetAttribute(k_trsv_block, cudaFuncAttributeMaxDynamicSharedMemorySize, LU_NB * LU_NB * 16);
     cudaFuncSetAttribute(k_lu_apply_piv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(n * 8));
     cudaMemsetAsync(misc, 0, 64, ctx->stream);
     for (int l = 0; l < st->n_layers; ++l) {
@@ -450,7 +486,7 @@ void launch_propagate_alpha(scw_ctx* ctx, const scw_stack* st, const void* r0, v
             const int grid = lu_grid(ctx, n - k0, &p.rpc);
             cudaMemsetAsync(bar, 0, 4, ctx->stream);
             {
-                KernelScope ks(ctx, KC_ALPHA_LU);
+                KernelScope ks(ctx, KC_ALPHA_PANEL);
                 void* args[] = {&p};
                 cudaLaunchCooperativeKernel((const void*)k_lu_panel, dim3(grid), dim3(LU_THREADS), args,
                                             (size_t)p.rpc * nb * 16, ctx->stream);
@@ -477,14 +513,14 @@ void launch_propagate_alpha(scw_ctx* ctx, const scw_stack* st, const void* r0, v
         for (int64_t k0 = 0; k0 < n; k0 += LU_NB) {
             const int nb = (int)std::min<int64_t>(LU_NB, n - k0);
             KernelScope ks(ctx, KC_ALPHA);
-            k_trsv_block<<<1, 32, 0, ctx->stream>>>(A, n, k0, nb, 0, y);
+            k_trsv_block<<<1, 256, LU_NB * LU_NB * 16, ctx->stream>>>(A, n, k0, nb, 0, y);
             if (k0 + nb < n)
                 k_trsv_update<<<(unsigned)((n - k0 - nb + 255) / 256), 256, 0, ctx->stream>>>(A, n, k0, nb, k0 + nb, n, y);
         }
         for (int64_t k0 = (n - 1) / LU_NB * LU_NB; k0 >= 0; k0 -= LU_NB) {
             const int nb = (int)std::min<int64_t>(LU_NB, n - k0);
             KernelScope ks(ctx, KC_ALPHA);
-            k_trsv_block<<<1, 32, 0, ctx->stream>>>(A, n, k0, nb, 1, y);
+            k_trsv_block<<<1, 256, LU_NB * LU_NB * 16, ctx->stream>>>(A, n, k0, nb, 1, y);
             if (k0 > 0) k_trsv_update<<<(unsigned)((k0 + 255) / 256), 256, 0, ctx->stream>>>(A, n, k0, nb, 0, k0, y);
         }
         // ---- alpha = y / d', r = Q (d` o alpha)
@@ -499,8 +535,10 @@ void launch_propagate_alpha(scw_ctx* ctx, const scw_stack* st, const void* r0, v
         }
         {
             KernelScope ks(ctx, KC_ALPHA);
-            if (f32) k_alpha_matvec<float2><<<vb, 256, 0, ctx->stream>>>(n, st->ldQ, (const float2*)st->Q[l], w, r);
-            else k_alpha_matvec<double2><<<vb, 256, 0, ctx->stream>>>(n, st->ldQ, (const double2*)st->Q[l], w, r);
+            const dim3 mv(vb, MV_SLICES);                  // the slice partials go to the U12 buffer (free outside the LU)
+            if (f32) k_alpha_matvec<float2><<<mv, 256, 0, ctx->stream>>>(n, st->ldQ, (const float2*)st->Q[l], w, Ut);
+            else k_alpha_matvec<double2><<<mv, 256, 0, ctx->stream>>>(n, st->ldQ, (const double2*)st->Q[l], w, Ut);
+            k_alpha_matvec_sum<<<vb, 256, 0, ctx->stream>>>(n, Ut, r);
         }
     }
     if (rL) {

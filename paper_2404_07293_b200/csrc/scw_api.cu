@@ -333,7 +333,7 @@ const char* scw_profile_name(int32_t kc)
     static const char* names[KC_COUNT] = {"mode_weights", "twiddles", "simt_assemble", "reduce_splits", "simt_synth_a",
                                           "simt_synth_b", "points_table", "points_planewave", "point_synth", "misc",
                                           "tc_assemble", "tc_synth", "tc_synth_images", "dmma_assemble", "dmma_synth_a",
-                                          "dmma_synth_b", "exterior", "vbuild_prepare", "alpha_misc", "alpha_lu"};
+                                          "dmma_synth_b", "exterior", "vbuild_prepare", "alpha_misc", "alpha_lu_update", "alpha_lu_panel"};
     return (kc >= 0 && kc < KC_COUNT) ? names[kc] : nullptr;
 }
 

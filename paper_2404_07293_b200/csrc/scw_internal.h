@@ -10,7 +10,7 @@ namespace scw {
 // Kernel classes for launch accounting and the optional per-kernel CUDA-event timers.
 enum KernelClass {
     KC_WEIGHTS = 0, KC_TWIDDLES, KC_ASSEMBLE, KC_REDUCE, KC_SYNTH_A, KC_SYNTH_B, KC_POINTS_TABLE, KC_POINTS,
-    KC_POINT_SYNTH, KC_MISC, KC_ASSEMBLE_TC, KC_SYNTH_TC, KC_SYNTH_IMG, KC_ASSEMBLE_DMMA, KC_SYNTH_A_DMMA, KC_SYNTH_B_DMMA, KC_EXTERIOR, KC_VBUILD_PREP, KC_ALPHA, KC_ALPHA_LU, KC_COUNT
+    KC_POINT_SYNTH, KC_MISC, KC_ASSEMBLE_TC, KC_SYNTH_TC, KC_SYNTH_IMG, KC_ASSEMBLE_DMMA, KC_SYNTH_A_DMMA, KC_SYNTH_B_DMMA, KC_EXTERIOR, KC_VBUILD_PREP, KC_ALPHA, KC_ALPHA_LU, KC_ALPHA_PANEL, KC_COUNT
 };
 struct ProfRec { cudaEvent_t a, b; int kc; bool owns_a; };
 }  // namespace scw
