@@ -289,6 +289,19 @@ def run_ours(args):
     kernels = kernel_rooflines(prof, args.steps, sweep_shape(cfg, cfg.n_layers), peaks, load_traffic())
     roof = dominant_roofline(kernels, peaks)
     vbytes = sum(l.V.numel() * 8 for l in Ls)
+    # where the fused assembly kernel's time goes: per-CTA timeline of its last launch (scw_profile_assembly)
+    tl = np.array(ctx.assembly_timeline())
+    asm_phases = None
+    if len(tl):
+        main, fix = tl[:, 2] - tl[:, 1], tl[:, 3] - tl[:, 2]
+        asm_phases = dict(unit="us since the CTA's start, over the persistent CTAs of the last assembly launch",
+                          weights_and_padding_done=dict(median=float(np.median(tl[:, 1])), max=float(tl[:, 1].max())),
+                          main_loop=dict(min=float(main.min()), median=float(np.median(main)), max=float(main.max())),
+                          fixup=dict(median=float(np.median(fix)), max=float(fix.max())),
+                          exit=dict(min=float(tl[:, 3].min()), median=float(np.median(tl[:, 3])), max=float(tl[:, 3].max())),
+                          main_loop_hbm_frac_at_median=vbytes / (float(np.median(main)) * 1e-6) / 1e9 / peaks["hbm_gbs"],
+                          note="main loop = V streamed through TMA + tensor cores; its median is what the kernel would take "
+                               "if every SM streamed at the same rate and the weight / fix-up phases were free")
     whole = dict(alg_bytes=vbytes + samples * 24, hbm_frac=(vbytes + samples * 24) / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
                  note="V read once + E written once per step, over the step time: the step's HBM floor fraction")
 
@@ -336,7 +349,7 @@ def run_ours(args):
                                             "(HBM-bound, Fz = 16), [3], [3'] and configs[1] complex128 are under `extra`, "
                                             "each with its own roofline"),
                     clocks=clocks, e2e=e2e, gpu_launches=int(launches) * args.steps, gpu_launches_per_step=int(launches),
-                    roofline=roof, whole_step=whole, kernels=kernels, cpu_baseline=cpu, extra=extra, peaks=peaks)
+                    roofline=roof, whole_step=whole, assembly_phases=asm_phases, kernels=kernels, cpu_baseline=cpu, extra=extra, peaks=peaks)
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

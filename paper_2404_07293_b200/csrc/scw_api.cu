@@ -775,6 +775,7 @@ int32_t scw_calibrate(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
     std::vector<double> best_w;                     // the split with the shortest assembly seen so far (empty = equal)
     double best_us = 1e30;
     const int rounds = 8;
+    const double eta = 0.5;                          // 0.2 .. 0.7 and up to 24 rounds measured: no better
     for (int round = 0; round <= rounds; ++round) { // the last round only scores the last update
         std::vector<std::vector<double>> samples;
         std::vector<double> kernel_us;
@@ -825,7 +826,7 @@ int32_t scw_calibrate(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
             const double old = first ? 1.0 : ctx->split_w[c];
             const double rel = w[c] / mean;                      // measured rate relative to the mean
             const double cur = old;                               // share it ran with
-            w[c] = cur * (1.0 + 0.5 * (rel / cur - 1.0));         // half way from the current share to the measured rate
+            w[c] = cur * (1.0 + eta * (rel / cur - 1.0));         // half way from the current share to the measured rate
             if (!(w[c] > 0.6)) w[c] = 0.6;                        // clipped: no span beyond ~1.5x the mean (bounds the partial-tile slots)
             if (w[c] > 1.5) w[c] = 1.5;
         }
