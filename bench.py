@@ -221,8 +221,10 @@ def dominant_roofline(kernels, peaks):
     return roof
 
 
-def profile_sweep(torch, ctx, step, steps):
-    """Per-kernel device milliseconds over `steps` further calls (the library's CUDA-event timers)."""
+def profile_sweep_events(torch, ctx, step, steps):
+    """Per-kernel device milliseconds over `steps` further calls with a CUDA event between consecutive kernels (the
+    library's event timers).  The events serialise the launches: the programmatic overlap of a kernel's prologue with its
+    predecessor's tail is lost, so these intervals add up to MORE than the plain step."""
     ctx.set_profile(True)
     for _ in range(steps):
         step()
@@ -230,6 +232,30 @@ def profile_sweep(torch, ctx, step, steps):
     prof = ctx.profile()
     ctx.set_profile(False)
     return prof
+
+
+def profile_sweep(torch, ctx, step, steps):
+    """{kernel: (ms over the steps, launches)} inside `steps` PLAIN back-to-back calls, from the GPU's own clock: every
+    tensor-core sweep kernel leaves the globaltimer of its last CTA's exit in a ring (scw_profile_timeline); a kernel's
+    interval runs from the end of its predecessor in the stream to its own end, so the intervals add up to the CUDA-event
+    time of the steps and nothing sits between the kernels."""
+    for _ in range(2):
+        step()
+    torch.cuda.synchronize()
+    for _ in range(steps):
+        step()
+    torch.cuda.synchronize()
+    tl = ctx.kernel_timeline()
+    names = [name for _, name in tl]
+    last = [i for i, nm in enumerate(names) if nm == names[-1]]   # a step's launches end with its last synthesis launch
+    per_step = names[:last[-1] + 1][::-1].index("tc_assemble") + 1 if "tc_assemble" in names else len(names)
+    use = min(steps, (len(tl) - 1) // per_step) * per_step
+    prof = {}
+    for i in range(len(tl) - use, len(tl)):
+        ms = (tl[i][0] - tl[i - 1][0]) * 1e-6
+        a = prof.get(tl[i][1], (0.0, 0))
+        prof[tl[i][1]] = (a[0] + ms, a[1] + 1)
+    return prof, use // per_step
 
 
 def load_traffic():
@@ -256,7 +282,14 @@ def run_ours(args):
     dz, dx, dy = [dev(z) for z in zs], dev(x), dev(y)
     out = [torch.empty((cfg.planes, 3, cfg.Ny, cfg.Nx), dtype=torch.complex64, device=device) for _ in Ls]
     samples = cfg.n_layers * cfg.planes * cfg.Nx * cfg.Ny
-    step = lambda: scw.scw_sweep_wavelengths(ctx, Ls, dz, dx, dy, out=out)
+    # two output sets used alternately: a step never overwrites lines of its predecessor that are still dirty in the
+    # 126 MB L2 (re-using one set would let those lines be overwritten in place and never reach the DRAM)
+    outs = (out, [torch.empty_like(o) for o in out])
+    n_calls = [0]
+
+    def step():
+        n_calls[0] += 1
+        return scw.scw_sweep_wavelengths(ctx, Ls, dz, dx, dy, out=outs[n_calls[0] & 1])
 
     # ---- set-up (untimed, once per context): twiddle cache on (x, y do not change between steps) and the stream-K split
     # of the assembly calibrated on this very sweep (scw_calibrate: 3 rounds of 6 sweeps)
@@ -285,9 +318,16 @@ def run_ours(args):
     value = world * samples / (ms * 1e-3)
 
     # ---- per-kernel device timers over a second pass of the same K steps
-    prof = profile_sweep(torch, ctx, step, args.steps)
-    kernels = kernel_rooflines(prof, args.steps, sweep_shape(cfg, cfg.n_layers), peaks, load_traffic())
+    # plain steps, device clock (sums to the step time); then the same with a CUDA event between the kernels
+    prof, nsteps = profile_sweep(torch, ctx, step, args.steps)
+    kernels = kernel_rooflines(prof, nsteps, sweep_shape(cfg, cfg.n_layers), peaks, load_traffic())
     roof = dominant_roofline(kernels, peaks)
+    roof["timing"] = ("device clock inside plain back-to-back steps: interval from the previous kernel's end to this "
+                      "kernel's end (scw_profile_timeline); `kernels_cuda_events` holds the same with a CUDA event "
+                      "between the kernels, which removes their programmatic overlap")
+    ev = profile_sweep_events(torch, ctx, step, args.steps)
+    kernels_ev = {k: dict(ms_per_launch=v["ms_per_launch"], hbm_frac=v.get("hbm_frac"))
+                  for k, v in kernel_rooflines(ev, args.steps, sweep_shape(cfg, cfg.n_layers), peaks).items()}
     vbytes = sum(l.V.numel() * 8 for l in Ls)
     # where the fused assembly kernel's time goes: per-CTA timeline of its last launch (scw_profile_assembly)
     tl = np.array(ctx.assembly_timeline())
@@ -341,7 +381,7 @@ def run_ours(args):
                     config=dict(workload="BASELINE.json configs[1]: 33x33 frequencies (M=1089, J=4356), 4 layers x 64 "
                                 "planes, 256x256 grid, complex64, one scw_sweep_wavelengths call per step",
                                 samples_per_step=samples, parallelism=f"replicas x{world}",
-                                cache="inputs (457 MB of V) + outputs (403 MB) per step exceed the 126 MB L2",
+                                cache="inputs (457 MB of V) + outputs (403 MB) per step exceed the 126 MB L2; outputs alternate between two buffer sets",
                                 setup="untimed, once: SCW_OPT_CACHE=1 (twiddle tables kept between steps, step a-3 'cached in ctx') "
                                       "and scw_calibrate (per-SM stream-K split of the assembly)",
                                 why_config1="configs[1] is the largest config that runs in BOTH dtypes and the only one "
@@ -349,7 +389,8 @@ def run_ours(args):
                                             "(HBM-bound, Fz = 16), [3], [3'] and configs[1] complex128 are under `extra`, "
                                             "each with its own roofline"),
                     clocks=clocks, e2e=e2e, gpu_launches=int(launches) * args.steps, gpu_launches_per_step=int(launches),
-                    roofline=roof, whole_step=whole, assembly_phases=asm_phases, kernels=kernels, cpu_baseline=cpu, extra=extra, peaks=peaks)
+                    roofline=roof, whole_step=whole, assembly_phases=asm_phases, kernels=kernels,
+                    kernels_cuda_events=kernels_ev, cpu_baseline=cpu, extra=extra, peaks=peaks)
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
@@ -391,14 +432,14 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
     ms = time_steps(torch, sweep4, args.steps, args.warmup)
     n4 = len(Ls) * c4.planes * c4.Nx * c4.Ny
     vbytes = sum(l.V.numel() * 8 for l in Ls)
-    k4 = kernel_rooflines(profile_sweep(torch, ctx, sweep4, args.steps), args.steps, sweep_shape(c4, len(Ls)), peaks)
+    k4 = kernel_rooflines(*profile_sweep(torch, ctx, sweep4, args.steps), sweep_shape(c4, len(Ls)), peaks)
     extra["config4_sweep"] = dict(ms_per_call=ms, samples_per_s=n4 / (ms * 1e-3), kernels=k4,
                                   hbm_frac_V_plus_E=(vbytes + n4 * 24) / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
     # NEXT-3 detector: the same sweep with I = sum_comp |E_comp|^2 reduced in the synthesis epilogue (E never written)
     outI = [torch.empty((c4.planes, c4.Ny, c4.Nx), dtype=torch.float32, device=device) for _ in Ls]
     det4 = lambda: scw.scw_sweep_intensity(ctx, Ls, zs, dx, dy, out=outI)
     ms_i = time_steps(torch, det4, args.steps, args.warmup)
-    kI = kernel_rooflines(profile_sweep(torch, ctx, det4, args.steps), args.steps, sweep_shape(c4, len(Ls)), peaks)
+    kI = kernel_rooflines(*profile_sweep(torch, ctx, det4, args.steps), sweep_shape(c4, len(Ls)), peaks)
     if "tc_synth" in kI:                                     # detector: 4 bytes per sample leave the SM instead of 24
         kI["tc_synth"]["alg_bytes"] = n4 * 4
         kI["tc_synth"]["hbm_gbs"] = n4 * 4 / (kI["tc_synth"]["ms_per_launch"] * 1e-3) / 1e9
@@ -503,7 +544,7 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
         ms = time_steps(torch, sweep2, max(2, args.steps // 2), 2)
         n2 = c2.n_layers * c2.planes * c2.Nx * c2.Ny
         vbytes = sum(l.V.numel() * 8 for l in Ls)
-        k2 = kernel_rooflines(profile_sweep(torch, ctx, sweep2, 4), 4, sweep_shape(c2, len(Ls)), peaks, traffic.get("config2"))
+        k2 = kernel_rooflines(*profile_sweep(torch, ctx, sweep2, 4), sweep_shape(c2, len(Ls)), peaks, traffic.get("config2"))
         extra["config2_large"] = dict(ms_per_call=ms, samples_per_s=n2 / (ms * 1e-3), kernels=k2,
                                       hbm_frac_V_plus_E=(vbytes + n2 * 24) / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
         del Ls, out

@@ -111,6 +111,14 @@ int32_t scw_profile_reset(scw_ctx* ctx);
  * all CTAs visible, (2) its span of V streamed, (3) exit after the fix-up.  us: HOST [max_ctas][4]; *n_ctas (HOST) = CTAs of
  * that launch (0 if none yet).  SYNCHRONISES the stream.  Errors: NULL, SHAPE (max_ctas too small), CUDA. */
 int32_t scw_profile_assembly(scw_ctx* ctx, int32_t max_ctas, double* us, int32_t* n_ctas);
+/* Device-clock timeline of the tensor-core sweep kernels (always recorded, one atomicMax per CTA): the last CTA of every
+ * tcgen05 assembly / synthesis launch of a grouped sweep leaves the GPU's globaltimer (ns) at its exit in a ring of 128
+ * slots inside the workspace.  Unlike the CUDA-event timers above this does not put anything between the kernels, so the
+ * programmatic overlap of consecutive launches stays as in a plain run: the difference of two consecutive entries is the
+ * time the later kernel added to the stream.  Returns the last min(max_n, 128, launches so far) launches, oldest first:
+ * exit_ns[i] (HOST), kernel_class[i] (HOST; an index for scw_profile_name), *n (HOST).  Valid while the workspace of the
+ * sweeps is untouched.  SYNCHRONISES the stream.  Errors: NULL, CUDA. */
+int32_t scw_profile_timeline(scw_ctx* ctx, int32_t max_n, uint64_t* exit_ns, int32_t* kernel_class, int32_t* n);
 
 /* ---------------------------------------------------------------- descriptors (HOST PODs) */
 

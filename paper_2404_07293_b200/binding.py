@@ -31,7 +31,7 @@ EXPORTS = [
     "scw_exterior_spectra", "scw_exterior_points", "scw_exterior_points_workspace", "scw_exterior_grid",
     "scw_exterior_grid_workspace",
     "scw_sweep_intensity", "scw_sweep_intensity_workspace",
-    "scw_measure_peak", "scw_invalidate_cache", "scw_calibrate", "scw_profile_assembly",
+    "scw_measure_peak", "scw_invalidate_cache", "scw_calibrate", "scw_profile_assembly", "scw_profile_timeline",
     "scw_sweep_detector", "scw_sweep_detector_workspace", "scw_absorbance", "scw_build_V", "scw_build_V_workspace", "scw_propagate_alpha", "scw_propagate_alpha_workspace",
 ]
 SCW_PEAKS = {"fp64_dmma_tflops": 0, "fp32_fma_tflops": 1, "mufu_gops": 2, "hbm_read_gbs": 3, "hbm_write_gbs": 4,
@@ -145,6 +145,7 @@ def lib():
         L.scw_propagate_alpha_workspace.argtypes = [c_void_p, POINTER(scw_stack), POINTER(c_size_t)]
         L.scw_invalidate_cache.argtypes = [c_void_p]
         L.scw_profile_assembly.argtypes = [c_void_p, c_int32, POINTER(c_double), POINTER(c_int32)]
+        L.scw_profile_timeline.argtypes = [c_void_p, c_int32, POINTER(ctypes.c_uint64), POINTER(c_int32), POINTER(c_int32)]
         L.scw_calibrate.argtypes = L.scw_sweep_wavelengths.argtypes + [c_int32]
         L.scw_measure_peak.argtypes = [c_void_p, c_int32, c_void_p, c_size_t, c_int32, POINTER(c_double)]
         _LIB = L
@@ -331,6 +332,14 @@ class Context:
         n = c_int32()
         self.check(self.L.scw_profile_assembly(self._h, 256, buf, byref(n)))
         return [tuple(buf[4 * i:4 * i + 4]) for i in range(n.value)]
+
+    def kernel_timeline(self, max_n=128):
+        """[(exit_ns, kernel class name)] of the last tensor-core sweep launches, oldest first (scw_profile_timeline)."""
+        ns = (ctypes.c_uint64 * max_n)()
+        kc = (c_int32 * max_n)()
+        n = c_int32()
+        self.check(self.L.scw_profile_timeline(self._h, max_n, ns, kc, byref(n)))
+        return [(int(ns[i]), self.L.scw_profile_name(kc[i]).decode()) for i in range(n.value)]
 
     def reserve(self, nbytes):
         """Grow the registered workspace to at least nbytes."""

@@ -48,6 +48,7 @@ int32_t check_ctx(scw_ctx* ctx, bool sweep_call = false)
     ctx->tc_error = false;
     ctx->last_classes = 0;
     ctx->prof_last = nullptr;       // per-kernel timers: the first kernel of this call gets its own start event
+    ctx->tl_ring = nullptr;         // timeline ring: set by the assembly launch of this call, if any
     int cur = -1;
     cudaError_t e = cudaGetDevice(&cur);
     if (e == cudaSuccess && cur != ctx->device) e = cudaSetDevice(ctx->device);
@@ -756,6 +757,30 @@ int32_t scw_profile_assembly(scw_ctx* ctx, int32_t max_ctas, double* us, int32_t
     }
     for (size_t i = 0; i < ns.size(); ++i) us[i] = (double)ns[i] * 1e-3;
     *n_ctas = G;
+    return SCW_OK;
+}
+
+int32_t scw_profile_timeline(scw_ctx* ctx, int32_t max_n, uint64_t* exit_ns, int32_t* kernel_class, int32_t* n)
+{
+    if (!ctx || !exit_ns || !kernel_class || !n) return SCW_ERR_NULL;
+    ctx->msg[0] = 0;
+    *n = 0;
+    if (!ctx->tl_last_ring || ctx->tl_seq == 0 || max_n < 1) return SCW_OK;
+    unsigned long long ring[TL_RING];
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpy(ring, ctx->tl_last_ring, sizeof(ring), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) {
+        ctx->cuda_err = (int32_t)e;
+        return fail(ctx, SCW_ERR_CUDA, "scw_profile_timeline: %s", cudaGetErrorString(e));
+    }
+    int64_t cnt = ctx->tl_seq < TL_RING ? ctx->tl_seq : TL_RING;
+    if (cnt > max_n) cnt = max_n;
+    for (int64_t i = 0; i < cnt; ++i) {                 // oldest first
+        const int slot = (int)((ctx->tl_seq - cnt + i) % TL_RING);
+        exit_ns[i] = ring[slot];
+        kernel_class[i] = ctx->tl_class[slot];
+    }
+    *n = (int32_t)cnt;
     return SCW_OK;
 }
 

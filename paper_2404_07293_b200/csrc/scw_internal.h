@@ -50,6 +50,13 @@ struct scw_ctx {
     const void* clean_img = nullptr;
     int clean_img_U = 0, clean_img_Vn = 0;
     int64_t clean_img_planes = 0;
+    // device-clock timeline of the tensor-core sweep kernels (scw_profile_timeline): every such launch leaves the
+    // globaltimer value of its last CTA's exit in slot (tl_seq % TL_RING) of a ring that lives in the assembly's control
+    // block (caller's workspace); tl_ring is only valid inside the API call that set it (reset by check_ctx)
+    unsigned long long* tl_ring = nullptr;
+    const unsigned long long* tl_last_ring = nullptr;   // where the ring of the last sweep is (read back on request)
+    int64_t tl_seq = 0;
+    int tl_class[128] = {0};
     cudaEvent_t prof_last = nullptr;   // profiling: end event of the previous kernel of this API call
     std::vector<scw::ProfRec> recs;
     double prof_ms[scw::KC_COUNT] = {0};
@@ -59,6 +66,17 @@ struct scw_ctx {
 namespace scw {
 
 inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+// Timeline ring (see scw_ctx::tl_ring): the slot the next launch of class kc stamps its exit time into, NULL if no ring.
+constexpr int TL_RING = 128;
+inline unsigned long long* tl_next(scw_ctx* ctx, int kc)
+{
+    if (!ctx->tl_ring) return nullptr;
+    const int slot = (int)(ctx->tl_seq % TL_RING);
+    ctx->tl_class[slot] = kc;
+    ctx->tl_seq++;
+    return ctx->tl_ring + slot;
+}
 
 // Brackets one kernel launch: counts it and, when profiling is on, times it with CUDA events on the ctx stream (read
 // back by scw_profile_read).  A kernel's interval runs from the end event of the previous kernel of the same API call
