@@ -914,9 +914,13 @@ static void ta_launch(scw_ctx* ctx, int n_inst, int64_t R, int64_t J, int64_t Fz
     p.part = part;
     p.ctl = ctl;
     p.cta_ns = reinterpret_cast<unsigned long long*>(reinterpret_cast<uint8_t*>(ctl) + align_up(pl.ctl_ints * sizeof(int), 8));
-    ctx->tl_ring = p.cta_ns + TA_MAX_CTAS * 4;
-    ctx->tl_last_ring = ctx->tl_ring;
-    p.tl_slot = tl_next(ctx, KC_ASSEMBLE_TC);
+    p.tl_slot = nullptr;
+    if (fix.mode == TC_FIX_IMAGES) {                // a sweep: this launch and the synthesis that follows stamp the timeline
+        ctx->tl_ring = p.cta_ns + TA_MAX_CTAS * 4;
+        if (ctx->tl_last_ring != ctx->tl_ring) ctx->tl_seq = 0;     // the ring moved (other workspace layout): start over
+        ctx->tl_last_ring = ctx->tl_ring;
+        p.tl_slot = tl_next(ctx, KC_ASSEMBLE_TC);
+    }
     p.sched = sched;
     p.n_sched = sched ? n_sched : 0;
     p.N2 = pl.N2;

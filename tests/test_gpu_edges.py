@@ -381,6 +381,34 @@ def test_twiddle_cache_and_calibration(scw):
         c.close()
 
 
+def test_kernel_timeline_of_the_sweep_kernels(scw):
+    """scw_profile_timeline: every tensor-core sweep launch leaves its exit time on the device clock; entries come oldest
+    first, alternate assembly / synthesis, never decrease, and a call that is not a sweep leaves them alone."""
+    c = scw.Context(0)
+    try:
+        assert c.kernel_timeline() == []
+        c.set_cache(True)
+        lay = ragged_layer(9, 7, 252, np.complex64, seed=77)
+        L = scw.Layer.from_numpy(lay, "cuda")
+        x, y, z = dev(np.arange(150) * 3.0 / 150), dev(np.arange(140) * 4.5 / 140), dev(np.linspace(0.1, 0.7, 5))
+        for _ in range(4):
+            scw.scw_sweep_wavelengths(c, [L, L], [z, z], x, y)
+        tl = c.kernel_timeline()
+        assert [k for _, k in tl] == ["tc_assemble", "tc_synth"] * 4
+        t = [ns for ns, _ in tl]
+        assert all(b > a for a, b in zip(t, t[1:])) and t[-1] - t[0] < 1e9      # strictly later, all within a second
+        assert c.kernel_timeline(3) == tl[-3:]
+        scw.scw_assemble_spectra(c, L, z)                                     # its own launch is not part of the ring's order
+        for _ in range(70):                                                   # more launches than the ring holds
+            scw.scw_sweep_wavelengths(c, [L, L], [z, z], x, y)
+        tl = c.kernel_timeline()
+        assert len(tl) == 128 and [k for _, k in tl] == ["tc_assemble", "tc_synth"] * 64
+        t = [ns for ns, _ in tl]
+        assert all(b > a for a, b in zip(t, t[1:]))
+    finally:
+        c.close()
+
+
 def test_sweep_with_mixed_shapes_runs_grouped(scw, ctx):
     """Instances that differ in J and in Fz: consecutive instances of equal shape form a run (one assembly + one synthesis
     launch per run, all on the tensor-core kernels); every sample of every instance against Tier B."""
