@@ -234,21 +234,17 @@ def profile_sweep_events(torch, ctx, step, steps):
     return prof
 
 
-def profile_sweep(torch, ctx, step, steps):
-    """{kernel: (ms over the steps, launches)} inside `steps` PLAIN back-to-back calls, from the GPU's own clock: every
-    tensor-core sweep kernel leaves the globaltimer of its last CTA's exit in a ring (scw_profile_timeline); a kernel's
-    interval runs from the end of its predecessor in the stream to its own end, so the intervals add up to the CUDA-event
-    time of the steps and nothing sits between the kernels."""
-    for _ in range(2):
-        step()
-    torch.cuda.synchronize()
-    for _ in range(steps):
-        step()
-    torch.cuda.synchronize()
+def profile_from_ring(ctx, steps):
+    """{kernel: (ms over the steps, launches)}, steps covered: the device-clock intervals of the LAST `steps` sweep calls,
+    read from the ring every tensor-core sweep kernel stamps with the globaltimer of its last CTA's exit
+    (scw_profile_timeline).  A kernel's interval runs from the end of its predecessor in the stream to its own end, so the
+    intervals add up to the CUDA-event time of the same steps, and nothing sits between the kernels (a CUDA event between
+    two launches would undo their programmatic overlap).  Call it right after the timed loop: it reads, it runs nothing."""
     tl = ctx.kernel_timeline()
     names = [name for _, name in tl]
-    last = [i for i, nm in enumerate(names) if nm == names[-1]]   # a step's launches end with its last synthesis launch
-    per_step = names[:last[-1] + 1][::-1].index("tc_assemble") + 1 if "tc_assemble" in names else len(names)
+    if "tc_assemble" not in names:
+        return {}, 0
+    per_step = names[::-1].index("tc_assemble") + 1               # a step's launches: from its assembly to its last synthesis
     use = min(steps, (len(tl) - 1) // per_step) * per_step
     prof = {}
     for i in range(len(tl) - use, len(tl)):
@@ -306,6 +302,8 @@ def run_ours(args):
     while not sampler.rows and time.perf_counter() - t_wait < 3.0:   # nvidia-smi needs ~0.3 s to start
         time.sleep(0.05)
     ms = time_steps(torch, step, args.steps, args.warmup, dist)
+    prof, nsteps = profile_from_ring(ctx, min(args.steps, 60) - 1)  # the kernels of these timed steps (bar the first, whose
+                                                                     # assembly interval holds the host's launch latency)
     launches = (ctx.launch_count() - n0) // (args.steps + args.warmup)
     each = time_each(torch, step, max(20, args.steps))
     # the timed region lasts a few ms: keep the identical step running ~0.7 s so the 100 ms sampler sees it
@@ -318,13 +316,14 @@ def run_ours(args):
     value = world * samples / (ms * 1e-3)
 
     # ---- per-kernel device timers over a second pass of the same K steps
-    # plain steps, device clock (sums to the step time); then the same with a CUDA event between the kernels
-    prof, nsteps = profile_sweep(torch, ctx, step, args.steps)
+    # per kernel: device clock inside the timed steps above (sums to their CUDA-event time); then a further pass with a
+    # CUDA event between the kernels
     kernels = kernel_rooflines(prof, nsteps, sweep_shape(cfg, cfg.n_layers), peaks, load_traffic())
     roof = dominant_roofline(kernels, peaks)
-    roof["timing"] = ("device clock inside plain back-to-back steps: interval from the previous kernel's end to this "
-                      "kernel's end (scw_profile_timeline); `kernels_cuda_events` holds the same with a CUDA event "
-                      "between the kernels, which removes their programmatic overlap")
+    roof["timing"] = ("device clock (globaltimer) inside the timed steps themselves: interval from the previous kernel's end "
+                      "to this kernel's end (scw_profile_timeline), the intervals add up to ms_per_step; "
+                      "`kernels_cuda_events` = a further pass with a CUDA event between the kernels, which removes their "
+                      "programmatic overlap")
     ev = profile_sweep_events(torch, ctx, step, args.steps)
     kernels_ev = {k: dict(ms_per_launch=v["ms_per_launch"], hbm_frac=v.get("hbm_frac"))
                   for k, v in kernel_rooflines(ev, args.steps, sweep_shape(cfg, cfg.n_layers), peaks).items()}
@@ -432,14 +431,14 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
     ms = time_steps(torch, sweep4, args.steps, args.warmup)
     n4 = len(Ls) * c4.planes * c4.Nx * c4.Ny
     vbytes = sum(l.V.numel() * 8 for l in Ls)
-    k4 = kernel_rooflines(*profile_sweep(torch, ctx, sweep4, args.steps), sweep_shape(c4, len(Ls)), peaks)
+    k4 = kernel_rooflines(*profile_from_ring(ctx, args.steps - 1), sweep_shape(c4, len(Ls)), peaks)   # of the steps just timed
     extra["config4_sweep"] = dict(ms_per_call=ms, samples_per_s=n4 / (ms * 1e-3), kernels=k4,
                                   hbm_frac_V_plus_E=(vbytes + n4 * 24) / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
     # NEXT-3 detector: the same sweep with I = sum_comp |E_comp|^2 reduced in the synthesis epilogue (E never written)
     outI = [torch.empty((c4.planes, c4.Ny, c4.Nx), dtype=torch.float32, device=device) for _ in Ls]
     det4 = lambda: scw.scw_sweep_intensity(ctx, Ls, zs, dx, dy, out=outI)
     ms_i = time_steps(torch, det4, args.steps, args.warmup)
-    kI = kernel_rooflines(*profile_sweep(torch, ctx, det4, args.steps), sweep_shape(c4, len(Ls)), peaks)
+    kI = kernel_rooflines(*profile_from_ring(ctx, args.steps - 1), sweep_shape(c4, len(Ls)), peaks)
     if "tc_synth" in kI:                                     # detector: 4 bytes per sample leave the SM instead of 24
         kI["tc_synth"]["alg_bytes"] = n4 * 4
         kI["tc_synth"]["hbm_gbs"] = n4 * 4 / (kI["tc_synth"]["ms_per_launch"] * 1e-3) / 1e9
@@ -544,7 +543,7 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
         ms = time_steps(torch, sweep2, max(2, args.steps // 2), 2)
         n2 = c2.n_layers * c2.planes * c2.Nx * c2.Ny
         vbytes = sum(l.V.numel() * 8 for l in Ls)
-        k2 = kernel_rooflines(*profile_sweep(torch, ctx, sweep2, 4), sweep_shape(c2, len(Ls)), peaks, traffic.get("config2"))
+        k2 = kernel_rooflines(*profile_from_ring(ctx, max(2, args.steps // 2) - 1), sweep_shape(c2, len(Ls)), peaks, traffic.get("config2"))
         extra["config2_large"] = dict(ms_per_call=ms, samples_per_s=n2 / (ms * 1e-3), kernels=k2,
                                       hbm_frac_V_plus_E=(vbytes + n2 * 24) / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
         del Ls, out

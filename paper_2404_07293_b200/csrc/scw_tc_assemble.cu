@@ -557,10 +557,11 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
             int ss = 0;
             uint32_t ps = 0;
             TaPos q = ta_pos(p, it0);
-            // V is read once: evict-first in L2, so that the stream replaces its own lines instead of forcing out the dirty
-            // output lines the previous synthesis left there (their write-back, interleaved with these reads, cost 6 % of the
-            // config-1 step and most of the SM-to-SM imbalance of this loop)
-            const uint64_t pol = l2_policy_evict_first();
+            // Inside a sweep V is read once: evict-first in L2, so that the stream replaces its own lines instead of forcing
+            // out the dirty output lines the previous synthesis left there (their write-back, interleaved with these reads,
+            // cost 6 % of the config-1 step and most of the SM-to-SM imbalance of this loop).  Other callers may come back to
+            // the same V (the dense point path re-reads it once per chunk of points, mostly from L2): normal priority.
+            const uint64_t pol = p.fix.mode == TC_FIX_IMAGES ? l2_policy_evict_first() : l2_policy_evict_normal();
             for (int64_t it = it0; it < it1; ++it) {
                 const int inst = q.inst;
                 uint8_t* dst = stg_base + (size_t)ss * TA_STG_BYTES;
