@@ -302,7 +302,7 @@ def run_ours(args):
     while not sampler.rows and time.perf_counter() - t_wait < 3.0:   # nvidia-smi needs ~0.3 s to start
         time.sleep(0.05)
     ms = time_steps(torch, step, args.steps, args.warmup, dist)
-    prof, nsteps = profile_from_ring(ctx, min(args.steps, 60) - 1)  # the kernels of these timed steps (bar the first, whose
+    prof, nsteps = profile_from_ring(ctx, max(1, min(args.steps, 60) - 1))  # the kernels of these timed steps (bar the first, whose
                                                                      # assembly interval holds the host's launch latency)
     launches = (ctx.launch_count() - n0) // (args.steps + args.warmup)
     each = time_each(torch, step, max(20, args.steps))
@@ -431,14 +431,14 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
     ms = time_steps(torch, sweep4, args.steps, args.warmup)
     n4 = len(Ls) * c4.planes * c4.Nx * c4.Ny
     vbytes = sum(l.V.numel() * 8 for l in Ls)
-    k4 = kernel_rooflines(*profile_from_ring(ctx, args.steps - 1), sweep_shape(c4, len(Ls)), peaks)   # of the steps just timed
+    k4 = kernel_rooflines(*profile_from_ring(ctx, max(1, args.steps - 1)), sweep_shape(c4, len(Ls)), peaks)   # of the steps just timed
     extra["config4_sweep"] = dict(ms_per_call=ms, samples_per_s=n4 / (ms * 1e-3), kernels=k4,
                                   hbm_frac_V_plus_E=(vbytes + n4 * 24) / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
     # NEXT-3 detector: the same sweep with I = sum_comp |E_comp|^2 reduced in the synthesis epilogue (E never written)
     outI = [torch.empty((c4.planes, c4.Ny, c4.Nx), dtype=torch.float32, device=device) for _ in Ls]
     det4 = lambda: scw.scw_sweep_intensity(ctx, Ls, zs, dx, dy, out=outI)
     ms_i = time_steps(torch, det4, args.steps, args.warmup)
-    kI = kernel_rooflines(*profile_from_ring(ctx, args.steps - 1), sweep_shape(c4, len(Ls)), peaks)
+    kI = kernel_rooflines(*profile_from_ring(ctx, max(1, args.steps - 1)), sweep_shape(c4, len(Ls)), peaks)
     if "tc_synth" in kI:                                     # detector: 4 bytes per sample leave the SM instead of 24
         kI["tc_synth"]["alg_bytes"] = n4 * 4
         kI["tc_synth"]["hbm_gbs"] = n4 * 4 / (kI["tc_synth"]["ms_per_launch"] * 1e-3) / 1e9
@@ -543,7 +543,7 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
         ms = time_steps(torch, sweep2, max(2, args.steps // 2), 2)
         n2 = c2.n_layers * c2.planes * c2.Nx * c2.Ny
         vbytes = sum(l.V.numel() * 8 for l in Ls)
-        k2 = kernel_rooflines(*profile_from_ring(ctx, max(2, args.steps // 2) - 1), sweep_shape(c2, len(Ls)), peaks, traffic.get("config2"))
+        k2 = kernel_rooflines(*profile_from_ring(ctx, max(1, max(2, args.steps // 2) - 1)), sweep_shape(c2, len(Ls)), peaks, traffic.get("config2"))
         extra["config2_large"] = dict(ms_per_call=ms, samples_per_s=n2 / (ms * 1e-3), kernels=k2,
                                       hbm_frac_V_plus_E=(vbytes + n2 * 24) / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
         del Ls, out
