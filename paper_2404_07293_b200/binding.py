@@ -175,6 +175,7 @@ class Layer:
         self.U, self.Vn, self.X, self.Y, self.lam = int(U), int(Vn), float(X), float(Y), float(lam)
         self.z_lo, self.z_hi = float(z_lo), float(z_hi)
         self.V, self.c, self.gamma, self.dir = V, c, gamma, dir
+        self._struct = None
         assert V.dim() == 2 and V.is_contiguous() and gamma.dtype == torch.complex128
         assert c is None or c.dtype == V.dtype
         assert dir is None or dir.dtype == torch.int8
@@ -188,10 +189,13 @@ class Layer:
         return 3 * self.U * self.Vn
 
     def struct(self):
-        return scw_layer(ctypes.sizeof(scw_layer), _dt(self.V), self.U, self.Vn, self.X, self.Y, self.lam,
-                         self.z_lo, self.z_hi, self.V.shape[0], self.V.data_ptr(), self.V.shape[1],
-                         None if self.c is None else self.c.data_ptr(), self.gamma.data_ptr(),
-                         None if self.dir is None else self.dir.data_ptr())
+        """The scw_layer descriptor (built once: a Layer is not modified after construction)."""
+        if self._struct is None:
+            self._struct = scw_layer(ctypes.sizeof(scw_layer), _dt(self.V), self.U, self.Vn, self.X, self.Y, self.lam,
+                                     self.z_lo, self.z_hi, self.V.shape[0], self.V.data_ptr(), self.V.shape[1],
+                                     None if self.c is None else self.c.data_ptr(), self.gamma.data_ptr(),
+                                     None if self.dir is None else self.dir.data_ptr())
+        return self._struct
 
     @staticmethod
     def from_numpy(d, device):

@@ -461,8 +461,14 @@ static int32_t check_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, 
         if (Fz[i] < 0) return fail(ctx, SCW_ERR_SHAPE, "%s: Fz[%lld] < 0", who, (long long)i);
         if (Fz[i] > *fz_max) *fz_max = Fz[i];
         if (Fz[i] > 0) {
-            const size_t a = assemble_ws(ctx, &inst[i], Fz[i]);
-            if (a > *asm_max) *asm_max = a;
+            // the scratch size is a function of (J, Fz, path eligibility) once U, Vn, dtype are equal: instances of a sweep
+            // mostly repeat the previous one's shape, and planning the stream-K split 64 times per call showed on the host
+            const bool tc = use_tc_assemble(ctx, &inst[i], Fz[i]);
+            if (i == 0 || inst[i].J != inst[i - 1].J || Fz[i] != Fz[i - 1] || Fz[i - 1] <= 0 ||
+                tc != use_tc_assemble(ctx, &inst[i - 1], Fz[i - 1])) {
+                const size_t a = assemble_ws(ctx, &inst[i], Fz[i]);
+                if (a > *asm_max) *asm_max = a;
+            }
         }
     }
     return SCW_OK;

@@ -891,6 +891,10 @@ static void ta_launch(scw_ctx* ctx, int n_inst, int64_t R, int64_t J, int64_t Fz
     float* part = reinterpret_cast<float*>(Wt + align_up(pl.wt_bytes * n_inst));
     static thread_local TaParams p;                 // ~22 KB of kernel parameters: kept off the stack
     bool maps_ok = true;
+    // Tensor maps are pure functions of (V, ldV, R, J): a sweep that comes back with the same matrices (every step of a
+    // time loop, every call of a calibrated bench) re-uses the encoded maps (128 driver calls per 64-instance sweep otherwise).
+    struct MapEntry { const void* V; int64_t ldV, R, J; CUtensorMap m[2]; int xoff; };
+    static thread_local MapEntry map_cache[256] = {};
     for (int i = 0; i < n_inst; ++i) {
         p.c[i] = (const float2*)inst[i].c;
         p.gamma[i] = (const double2*)inst[i].gamma;
@@ -899,8 +903,22 @@ static void ta_launch(scw_ctx* ctx, int n_inst, int64_t R, int64_t J, int64_t Fz
         p.inv_lambda[i] = 1.0 / inst[i].lambda;
         p.z_lo[i] = inst[i].z_lo;
         p.z_hi[i] = inst[i].z_hi;
-        maps_ok = maps_ok && ta_make_map(&p.tmap[i][0], inst[i].V, inst[i].ldV, R, J, 0, nullptr) &&
-                  ta_make_map(&p.tmap[i][1], inst[i].V, inst[i].ldV, R, J, 1, &p.xoff1[i]);
+        MapEntry& ce = map_cache[(reinterpret_cast<uintptr_t>(inst[i].V) >> 8) & 255];
+        if (ce.V != inst[i].V || ce.ldV != inst[i].ldV || ce.R != R || ce.J != J) {
+            ce.V = nullptr;
+            if (ta_make_map(&ce.m[0], inst[i].V, inst[i].ldV, R, J, 0, nullptr) &&
+                ta_make_map(&ce.m[1], inst[i].V, inst[i].ldV, R, J, 1, &ce.xoff)) {
+                ce.V = inst[i].V;
+                ce.ldV = inst[i].ldV;
+                ce.R = R;
+                ce.J = J;
+            } else {
+                maps_ok = false;
+            }
+        }
+        p.tmap[i][0] = ce.m[0];
+        p.tmap[i][1] = ce.m[1];
+        p.xoff1[i] = ce.xoff;
     }
     if (!maps_ok) {                                 // reported by the entry point's check_launch
         ctx->tc_error = true;

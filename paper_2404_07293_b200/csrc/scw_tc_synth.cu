@@ -58,6 +58,7 @@ struct TsParams {
     int acc_col;           // first of 128 TMEM columns holding the running sum over components, 0 = none (kept in the output)
     int d2_single;         // detector with 33..40 frequencies along u (one u chunk): D2 is ONE 128-column buffer shared by the two y halves
                            // (released as soon as it is in registers), its second half holds the running sum
+    int b2_stages;         // 1, or 2 when shared memory holds two B2 buffers: the converters fill one while GEMM2 reads the other
     float* s_part;         // window sums: [plane][tile][16] partial sums of |E_comp|^2 over the window, NULL = not wanted
     int win_x0, win_x1, win_y0, win_y1;   // window (grid indices, half-open)
     unsigned long long* tl_slot;          // timeline ring slot of this launch (scw_profile_timeline), may be NULL
@@ -267,8 +268,8 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
     const uint32_t b1_img = (uint32_t)N1 * K1p * 2, b2_img = TS_TILE * K2p * 2;
     uint8_t* sA1 = smem;                              // nvc x (hi | lo)
     uint8_t* sB1 = sA1 + (size_t)nvc * 2 * a1_img;    // 2 stages x (hi | lo)
-    uint8_t* sB2 = sB1 + 4 * b1_img;                  // 2 halves x (hi | lo)
-    uint64_t* bars = reinterpret_cast<uint64_t*>(sB2 + 4 * b2_img);
+    uint8_t* sB2 = sB1 + 4 * b1_img;                  // b2_stages x 2 halves x (hi | lo)
+    uint64_t* bars = reinterpret_cast<uint64_t*>(sB2 + (size_t)p.b2_stages * 4 * b2_img);
     uint64_t* tw_full = bars;            // [1]
     uint64_t* b1_full = bars + 1;        // [2]
     uint64_t* b1_empty = bars + 3;       // [2]
@@ -282,6 +283,9 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
     int* s_plane = reinterpret_cast<int*>(bars + 23);               // [8]
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 27);
     uint64_t* a2_full = bars + 28;       // [1] x twiddles are in TMEM (converter warps -> MMA warp)
+    uint64_t* b2_full_s1 = bars + 29;    // [2] second B2 stage (b2_stages == 2)
+    uint64_t* b2_empty_s1 = bars + 31;   // [2]
+    const int b2s = p.b2_stages;
 
     if (tid == 0) {
         if (blockIdx.x == 0 && p.tl_slot) *p.tl_slot = 0ull;   // this launch's timeline slot (atomicMax at the CTAs' exits)
@@ -293,6 +297,8 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
             mbar_init(&b1_empty[s], 1);
             mbar_init(&b2_full[s], 4);
             mbar_init(&b2_empty[s], 1);
+            mbar_init(&b2_full_s1[s], 4);
+            mbar_init(&b2_empty_s1[s], 1);
             mbar_init(&d2_full[s], 1);
             mbar_init(&d2_empty[s], 8);
         }
@@ -397,16 +403,19 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
             auto issue_gemm2 = [&](int i, int h) {     // D2[h] (+)= A2[uc] B2[h]; complete after the last u chunk
                 const int n = i / nuc, uc = i - n * nuc;
                 if (i == 0 && h == 0) mbar_wait(a2_full, 0);
-                mbar_wait(&b2_full[h], i & 1);
+                const int st = b2s == 2 ? (i & 1) : 0;                    // B2 stage of this item and how often it was used
+                const int su = b2s == 2 ? (i >> 1) : i;
+                mbar_wait(st ? &b2_full_s1[h] : &b2_full[h], su & 1);
                 const int hb = p.d2_single ? 0 : h;                       // D2 buffer of this half, and how often it was used
                 const int use = p.d2_single ? 2 * n + h : n;
                 if (uc == 0) mbar_wait(&d2_empty[hb], (use & 1) ^ 1);
                 tc_fence_after();
                 const uint32_t ta = tmem_base + a2_col + uc * K2p;
                 if (elect_one()) {
-                    ts_mma3_ts(tmem_base + TS_D2_COL + hb * TS_TILE, ta, ta + K2p / 2, b2 + h * 2 * b2_img,
-                               b2 + h * 2 * b2_img + b2_img, 2048, K2p, idesc2, uc > 0 ? 1u : 0u);
-                    umma_commit(&b2_empty[h]);
+                    const uint32_t b2h = b2 + (uint32_t)(st * 4 + h * 2) * b2_img;
+                    ts_mma3_ts(tmem_base + TS_D2_COL + hb * TS_TILE, ta, ta + K2p / 2, b2h, b2h + b2_img, 2048, K2p, idesc2,
+                               uc > 0 ? 1u : 0u);
+                    umma_commit(st ? &b2_empty_s1[h] : &b2_empty[h]);
                     if (uc == nuc - 1) umma_commit(&d2_full[hb]);
                 }
                 __syncwarp();
@@ -435,7 +444,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
         const int kg = (warp - 2) >> 2;              // chunk parity handled by this warp
         const int h = q >> 1;                        // which half of the tile this y belongs to
         const int yy = 32 * (q & 1) + lane;          // y within the half
-        uint8_t* row = sB2 + (size_t)h * 2 * b2_img + yy * 32;
+        uint8_t* row0 = sB2 + (size_t)h * 2 * b2_img + yy * 32;
         const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + TS_D1_COL;
         const int nchunks = K2p / 8;                 // <= 10
         for (int n = 0;; ++n) {                      // n = item (plane, u chunk)
@@ -450,7 +459,9 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(d1_empty);    // D1 may be overwritten by the next plane's GEMM1
-            mbar_wait(&b2_empty[h], (n & 1) ^ 1);
+            const int st = b2s == 2 ? (n & 1) : 0, su = b2s == 2 ? (n >> 1) : n;
+            uint8_t* row = row0 + (size_t)st * 4 * b2_img;
+            mbar_wait(st ? &b2_empty_s1[h] : &b2_empty[h], (su & 1) ^ 1);
 #pragma unroll
             for (int i = 0; i < 5; ++i) {
                 const int c = 2 * i + kg;
@@ -479,7 +490,7 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
             }
             fence_proxy_async();
             __syncwarp();
-            if (lane == 0) mbar_arrive(&b2_full[h]);
+            if (lane == 0) mbar_arrive(st ? &b2_full_s1[h] : &b2_full[h]);
         }
     } else {
         // ===== epilogue: D2 (lane = x, columns = (y, Re/Im)) -> E.  Two warps per lane quarter, 32 y each. =====
@@ -634,6 +645,7 @@ struct TsPlan {
     TsChunks cu, cv;          // frequency chunks along u (GEMM2's K) and v (GEMM1's K)
     int K1p, K2p, tiles_x, tiles_y;
     size_t a1_bytes, a2_bytes, sched_bytes, b1_bytes, smem_bytes;
+    int b2_stages;
 };
 
 static TsPlan ts_plan(int U, int Vn, int64_t Fz, int64_t Nx, int64_t Ny)
@@ -649,8 +661,13 @@ static TsPlan ts_plan(int U, int Vn, int64_t Fz, int64_t Nx, int64_t Ny)
     pl.a2_bytes = align_up((size_t)pl.tiles_x * pl.cu.n * TS_TILE * pl.K2p * 4);
     pl.sched_bytes = align_up((size_t)pl.tiles_x * pl.tiles_y * sizeof(int));
     pl.b1_bytes = align_up((size_t)Fz * 3 * pl.cu.n * pl.cv.n * 2 * pl.K2p * pl.K1p * 2);
-    pl.smem_bytes = (size_t)pl.cv.n * 2 * TS_TILE * pl.K1p * 2 + (size_t)4 * pl.K2p * pl.K1p * 2 +
-                    (size_t)4 * TS_TILE * pl.K2p * 2 + 256;
+    const size_t b2_bytes = (size_t)4 * TS_TILE * pl.K2p * 2;                  // one B2 buffer: 2 halves x (hi | lo)
+    pl.smem_bytes = (size_t)pl.cv.n * 2 * TS_TILE * pl.K1p * 2 + (size_t)4 * pl.K2p * pl.K1p * 2 + b2_bytes + 512;
+    // a second B2 buffer when it fits (up to 24 frequencies along u): the converters then split plane i + 1 while GEMM2 still
+    // reads plane i (with one buffer GEMM2 -> converters -> GEMM2 is a serial chain: 2.1 us per plane at 17 x 17 frequencies
+    // against 1.1 us of MMA issue)
+    pl.b2_stages = pl.smem_bytes + b2_bytes <= 227 * 1024 ? 2 : 1;
+    if (pl.b2_stages == 2) pl.smem_bytes += b2_bytes;
     return pl;
 }
 
@@ -727,6 +744,7 @@ static void ts_launch_main(scw_ctx* ctx, const TsPlan& pl, int64_t Fz, int n_ins
         p.d2_single = (want_I && !fits && pl.cu.n == 1) ? 1 : 0;
         p.acc_col = !want_I ? 0 : (fits ? used : (p.d2_single ? TS_TILE : 0));
     }
+    p.b2_stages = pl.b2_stages;
     p.s_part = (intensity && det->S) ? static_cast<float*>(det->s_part) : nullptr;
     if (intensity) {
         p.win_x0 = (int)det->win[0]; p.win_x1 = (int)det->win[1]; p.win_y0 = (int)det->win[2]; p.win_y1 = (int)det->win[3];
