@@ -189,12 +189,17 @@ class Layer:
         return 3 * self.U * self.Vn
 
     def struct(self):
-        """The scw_layer descriptor (built once: a Layer is not modified after construction)."""
+        """A fresh scw_layer descriptor of this layer (the caller may edit it)."""
+        return scw_layer(ctypes.sizeof(scw_layer), _dt(self.V), self.U, self.Vn, self.X, self.Y, self.lam,
+                         self.z_lo, self.z_hi, self.V.shape[0], self.V.data_ptr(), self.V.shape[1],
+                         None if self.c is None else self.c.data_ptr(), self.gamma.data_ptr(),
+                         None if self.dir is None else self.dir.data_ptr())
+
+    def _cached_struct(self):
+        """The descriptor built once, for the sweep calls that marshal many layers per call (a Layer is not modified after
+        construction; never handed out)."""
         if self._struct is None:
-            self._struct = scw_layer(ctypes.sizeof(scw_layer), _dt(self.V), self.U, self.Vn, self.X, self.Y, self.lam,
-                                     self.z_lo, self.z_hi, self.V.shape[0], self.V.data_ptr(), self.V.shape[1],
-                                     None if self.c is None else self.c.data_ptr(), self.gamma.data_ptr(),
-                                     None if self.dir is None else self.dir.data_ptr())
+            self._struct = self.struct()
         return self._struct
 
     @staticmethod
@@ -445,7 +450,7 @@ def scw_exterior_points(ctx, ext, r, out=None):
 
 def _sweep_args(layers, zs):
     n = len(layers)
-    inst = (scw_layer * max(n, 1))(*[l.struct() for l in layers])
+    inst = (scw_layer * max(n, 1))(*[l._cached_struct() for l in layers])
     Fz = (c_int64 * max(n, 1))(*[z.numel() for z in zs])
     zp = (c_void_p * max(n, 1))(*[z.data_ptr() for z in zs])
     return n, inst, Fz, zp

@@ -27,14 +27,12 @@ using namespace tc;
 constexpr int TS_TILE = 128;               // output tile edge (x and y)
 constexpr int TS_KMAX = 80;                // max padded K per chunk (= 2*chunk rounded up to 16)
 constexpr int TS_FMAX = 80;                // max frequencies per axis (two chunks)
-constexpr int TS_THREADS = 18 * 32;        // loader, MMA, 8 converter warps, 8 epilogue warps
+constexpr int TS_THREADS = 19 * 32;        // loader, GEMM2 issuer, 8 converter warps, 8 epilogue warps, GEMM1 issuer
+constexpr int TS_GEMM1_WARP = 18;
 constexpr int TS_TMEM_COLS = 512;
 constexpr int TS_D2_COL = 0;               // D2[h] at columns h*128
 constexpr int TS_D1_COL = 256;             // D1 at columns 256..256+N1, then A2 (per u chunk: hi K2p/2 | lo K2p/2 columns)
 constexpr int TS_MAX_INST = 64;            // instances per grouped launch
-#ifndef SCW_TS_ORDER
-#define SCW_TS_ORDER 0                     // 0: GEMM1(next item) before GEMM2 of this item (measured best with dynamic planes)
-#endif
 
 
 struct TsWsumOut { float* S[TS_MAX_INST]; };
@@ -377,14 +375,18 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                     }
             }
         }
-    } else if (warp == 1) {
-        // ===== MMA issuer: the whole warp runs the loop (warp-uniform control flow), one elected lane issues =====
+    } else if (warp == 1 || warp == TS_GEMM1_WARP) {
+        // ===== MMA issuers: GEMM1 (warp 18) and GEMM2 (warp 1) are issued by different warps.  One thread needs ~100 cycles
+        // per tcgen05.mma it issues (descriptor arithmetic, the instruction itself, the barriers around a GEMM) and a plane
+        // takes 27 (17 x 17 frequencies) to 45 (33 x 33) of them: with a single issuer the detector mode, which stores
+        // almost nothing, ran at the issue rate (2.1 us per plane), not at the tensor pipe's.  The two chains only meet
+        // through D1 (d1_full / d1_empty via the converters), which the mbarriers already order.  The whole warp runs the
+        // loop (warp-uniform control flow), one elected lane issues. =====
         if (sched_get(0) >= 0) {
             const uint32_t idesc1 = umma_idesc_bf16(TS_TILE, N1, false, true);    // B1 (spectrum images) is MN-major
             const uint32_t idesc2 = umma_idesc_bf16(TS_TILE, TS_TILE);
             const uint32_t a1 = smem_u32(sA1), b1 = smem_u32(sB1), b2 = smem_u32(sB2);
             const uint32_t d1 = tmem_base + TS_D1_COL;
-            mbar_wait(tw_full, 0);
             auto issue_gemm1 = [&](int i) {            // D1 = sum over the v chunks of item i
                 for (int vc = 0; vc < nvc; ++vc) {
                     const int q = i * nvc + vc, s = q & 1;
@@ -420,21 +422,16 @@ __global__ void __launch_bounds__(TS_THREADS, 1) k_tc_synth(const __grid_constan
                 }
                 __syncwarp();
             };
-            // GEMM1 of the next item goes first: it only needs D1 back from the converters (a TMEM load after d1_full) and
-            // then runs on the tensor pipe while they split and store this item's B2
-            issue_gemm1(0);
-            for (int i = 0;; ++i) {
+            if (warp == TS_GEMM1_WARP) mbar_wait(tw_full, 0);              // the y twiddle images (A1) are in shared memory
+            for (int i = 0;; ++i) {                                        // item i = (plane n, u chunk uc)
                 const int n = i / nuc, uc = i - n * nuc;
-                const bool next = (uc + 1 < nuc) || sched_get(n + 1) >= 0;
-#if SCW_TS_ORDER == 0
-                if (next) issue_gemm1(i + 1);
-                issue_gemm2(i, 0);
-#else
-                issue_gemm2(i, 0);
-                if (next) issue_gemm1(i + 1);
-#endif
-                issue_gemm2(i, 1);
-                if (!next) break;
+                if (uc == 0 && i > 0 && sched_get(n) < 0) break;
+                if (warp == TS_GEMM1_WARP) {
+                    issue_gemm1(i);
+                } else {
+                    issue_gemm2(i, 0);
+                    issue_gemm2(i, 1);
+                }
             }
         }
     } else if (warp < 10) {
