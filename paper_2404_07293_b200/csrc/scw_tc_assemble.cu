@@ -459,20 +459,47 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
         fin[0] = -1;
     }
     if (warp == TA_MMA_WARP) tmem_alloc(tmem_slot, TA_TMEM_COLS);
+    __syncthreads();                                     // the barriers are initialised for the V loader below
     // PDL: only the set-up above overlaps the tail of the previous kernel of the stream.  The weights read the caller's
     // inputs (gamma, c, z, ...), which the kernel just before this one in the caller's stream may have produced, so even
     // they wait for it.
     pdl_wait();
     pdl_launch_dependents();
-    ta_phase0_weights(p, (int64_t)blockIdx.x * TA_THREADS + tid, (int64_t)gridDim.x * TA_THREADS, TA_THREADS);
-    if (tid == 0) {
-        uint32_t smid;
-        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-        int slot = -1;
-        if (smid < gridDim.x && atomicCAS(&p.ctl[TA_CTL_CLAIM + smid], 0, 1) == 0) slot = (int)smid;
-        for (int i = 0; slot < 0 && i < (int)gridDim.x; ++i)
-            if (atomicCAS(&p.ctl[TA_CTL_CLAIM + i], 0, 1) == 0) slot = i;
-        *cta_slot = slot;
+    // The V loader does not compute weights: its lane claims the CTA's span and fills the staging ring at once, so that the
+    // DRAM works while the other 23 warps are busy with phase 0 (the first stg_stages loads need no free slot).
+    int ld_ss = 0;                                       // loader state carried into its role below
+    uint32_t ld_ps = 0;
+    int64_t ld_it = 0;
+    TaPos ld_q = {};
+    uint64_t ld_pol = 0;
+    if (warp == TA_V_LOADER) {
+        if (lane == 0) {
+            uint32_t smid;
+            asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+            int slot = -1;
+            if (smid < gridDim.x && atomicCAS(&p.ctl[TA_CTL_CLAIM + smid], 0, 1) == 0) slot = (int)smid;
+            for (int i = 0; slot < 0 && i < (int)gridDim.x; ++i)
+                if (atomicCAS(&p.ctl[TA_CTL_CLAIM + i], 0, 1) == 0) slot = i;
+            *cta_slot = slot;
+            // Inside a sweep V is read once: evict-first in L2, so that the stream replaces its own lines instead of forcing
+            // out the dirty output lines the previous synthesis left there (their write-back, interleaved with these reads,
+            // cost 6 % of the config-1 step and most of the SM-to-SM imbalance of this loop).  Other callers may come back to
+            // the same V (the dense point path re-reads it once per chunk of points, mostly from L2): normal priority.
+            ld_pol = p.fix.mode == TC_FIX_IMAGES ? l2_policy_evict_first() : l2_policy_evict_normal();
+            const int64_t a = p.span0[slot], b = min(p.span0[slot + 1], a + p.stg_stages);
+            ld_q = ta_pos(p, a);
+            for (ld_it = a; ld_it < b; ++ld_it) {
+                uint8_t* dst = stg_base + (size_t)ld_ss * TA_STG_BYTES;
+                mbar_expect_tx(&stg_full[ld_ss], TA_STG_ODD + 16 * (TA_ROWS + 2 * p.xoff1[ld_q.inst]) * 8);
+                tma_load_2d_hint(dst, &p.tmap[ld_q.inst][0], ld_q.mt * TA_ROWS, ld_q.kb * 16, &stg_full[ld_ss], ld_pol);
+                tma_load_2d_hint(dst + TA_STG_ODD, &p.tmap[ld_q.inst][1], ld_q.mt * TA_ROWS, ld_q.kb * 16, &stg_full[ld_ss], ld_pol);
+                ta_next(p, ld_q);
+                if (++ld_ss == p.stg_stages) { ld_ss = 0; ld_ps ^= 1; }
+            }
+        }
+    } else {
+        const int t0 = tid - (warp > TA_V_LOADER ? 32 : 0);
+        ta_phase0_weights(p, (int64_t)blockIdx.x * TA_P0_THREADS + t0, (int64_t)gridDim.x * TA_P0_THREADS, TA_P0_THREADS);
     }
     tc_fence_before();
     __syncthreads();
@@ -553,16 +580,12 @@ __global__ void __launch_bounds__(TA_THREADS, 1) k_tc_assemble(const __grid_cons
         }
     } else if (warp == TA_V_LOADER) {
         // ===== TMA producer: two 128-row x 16-column boxes (even / odd modes) per stage =====
-        if (lane == 0) {
-            int ss = 0;
-            uint32_t ps = 0;
-            TaPos q = ta_pos(p, it0);
-            // Inside a sweep V is read once: evict-first in L2, so that the stream replaces its own lines instead of forcing
-            // out the dirty output lines the previous synthesis left there (their write-back, interleaved with these reads,
-            // cost 6 % of the config-1 step and most of the SM-to-SM imbalance of this loop).  Other callers may come back to
-            // the same V (the dense point path re-reads it once per chunk of points, mostly from L2): normal priority.
-            const uint64_t pol = p.fix.mode == TC_FIX_IMAGES ? l2_policy_evict_first() : l2_policy_evict_normal();
-            for (int64_t it = it0; it < it1; ++it) {
+        if (lane == 0) {                                   // continues after the stages issued before phase 0
+            int ss = ld_ss;
+            uint32_t ps = ld_ps;
+            TaPos q = ld_q;
+            const uint64_t pol = ld_pol;
+            for (int64_t it = ld_it; it < it1; ++it) {
                 const int inst = q.inst;
                 uint8_t* dst = stg_base + (size_t)ss * TA_STG_BYTES;
                 mbar_wait(&stg_empty[ss], ps ^ 1);
