@@ -414,6 +414,9 @@ def extra_workloads(torch, scw, ctx, device, args, peaks):
                                    roofline=dict(bound="alu", achieved=gterm, peak=mufu / 3,
                                                  unit="Gterm/s (3 MUFU per term: sin, cos, ex2; peak = measured MUFU rate / 3)",
                                                  frac=gterm / (mufu / 3), traffic=None,
+                                                 note="the XU floor is the demanding bound; what binds in practice is the "
+                                                      "issue port (FFMA2 and DFMA hold it 2 cycles each: ~28.5 issue cycles "
+                                                      "per warp-term against 24 XU cycles, DESIGN.md 5.3)",
                                                  fp32_fma_frac=gterm * 28 / 1e3 / peaks.get("fp32_fma_tflops", 70.7)))
     del pts, outp
     # config 4: 32 wavelengths x 2 layers, one call

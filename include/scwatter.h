@@ -392,12 +392,13 @@ int32_t scw_propagate_alpha_workspace(scw_ctx* ctx, const scw_stack* st, size_t*
  * launches, CUDA events).  Unlike every other call this one SYNCHRONISES the stream.  buf: device scratch of `bytes`
  * bytes (contents destroyed); the HBM units stream through all of it -- pass >= 1 GiB so that it exceeds the L2;
  * the arithmetic units need 256 bytes.  value (HOST): TFLOP/s for FP64_DMMA (mma.sync.m8n8k4.f64, the complex128
- * contractions) and FP32_FMA, Gop/s for MUFU (ex2.approx: the pipe of the point path's sin / cos / ex2), GB/s for
+ * contractions) and FP32_FMA, Gop/s for MUFU (ex2.approx: the pipe of the point path's sin / cos / ex2) and MUFU_MIX (one
+ * sin.approx, one cos.approx and one ex2.approx per term, the point kernel's own mix: 3 ops per term), GB/s for
  * HBM_READ (16-byte loads), HBM_WRITE (16-byte st.global) and HBM_WRITE_TMA (16 KB cp.async.bulk shared -> global).
  * Errors: NULL, VALUE (unknown unit, reps < 1), CUDA.
  */
 enum { SCW_PEAK_FP64_DMMA = 0, SCW_PEAK_FP32_FMA = 1, SCW_PEAK_MUFU = 2, SCW_PEAK_HBM_READ = 3, SCW_PEAK_HBM_WRITE = 4,
-       SCW_PEAK_HBM_WRITE_TMA = 5 };
+       SCW_PEAK_HBM_WRITE_TMA = 5, SCW_PEAK_MUFU_MIX = 6 };
 int32_t scw_measure_peak(scw_ctx* ctx, int32_t which, void* buf, size_t bytes, int32_t reps, double* value);
 
 #ifdef __cplusplus

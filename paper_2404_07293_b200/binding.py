@@ -35,7 +35,7 @@ EXPORTS = [
     "scw_sweep_detector", "scw_sweep_detector_workspace", "scw_absorbance", "scw_build_V", "scw_build_V_workspace", "scw_propagate_alpha", "scw_propagate_alpha_workspace",
 ]
 SCW_PEAKS = {"fp64_dmma_tflops": 0, "fp32_fma_tflops": 1, "mufu_gops": 2, "hbm_read_gbs": 3, "hbm_write_gbs": 4,
-             "hbm_write_tma_gbs": 5}
+             "hbm_write_tma_gbs": 5, "mufu_sincosex2_gops": 6}
 SCW_SIDE_ABOVE, SCW_SIDE_BELOW = 0, 1
 
 

@@ -62,6 +62,29 @@ __global__ void __launch_bounds__(256) k_peak_mufu(int iters, float* __restrict_
     if (s == 123.456f) sink[0] = s;
 }
 
+// ---- MUFU mix of the point path: one sin, one cos and one ex2 per term on independent chains (sin / cos also cost their
+// range pre-scale FMUL on the FMA pipe, as in the kernel).  Tells whether SIN / COS issue at the EX2 rate.
+__global__ void __launch_bounds__(256) k_peak_mufu_mix(int iters, float* __restrict__ sink)
+{
+    float v[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = 1e-3f * (threadIdx.x + i + 1);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            float a, b, c;
+            asm volatile("sin.approx.ftz.f32 %0, %1;" : "=f"(a) : "f"(v[i]));
+            asm volatile("cos.approx.ftz.f32 %0, %1;" : "=f"(b) : "f"(v[i]));
+            asm volatile("ex2.approx.ftz.f32 %0, %1;" : "=f"(c) : "f"(-v[i]));
+            v[i] = a * b + c;
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += v[i];
+    if (s == 123.456f) sink[0] = s;
+}
+
 // ---- HBM read: every thread streams 16-byte loads, grid-stride, four loads in flight -----------------------------------
 __global__ void __launch_bounds__(512) k_peak_read(const uint4* __restrict__ src, size_t n16, unsigned* __restrict__ sink)
 {
@@ -119,11 +142,11 @@ extern "C" int32_t scw_measure_peak(scw_ctx* ctx, int32_t which, void* buf, size
     if (!ctx || !value) return SCW_ERR_NULL;
     ctx->msg[0] = 0;
     *value = 0.0;
-    if (which < SCW_PEAK_FP64_DMMA || which > SCW_PEAK_HBM_WRITE_TMA || reps < 1) {
+    if (which < SCW_PEAK_FP64_DMMA || which > SCW_PEAK_MUFU_MIX || reps < 1) {
         snprintf(ctx->msg, sizeof(ctx->msg), "scw_measure_peak: unknown unit %d or reps < 1", which);
         return SCW_ERR_VALUE;
     }
-    const bool mem = which >= SCW_PEAK_HBM_READ;
+    const bool mem = which >= SCW_PEAK_HBM_READ && which <= SCW_PEAK_HBM_WRITE_TMA;
     if (!buf || bytes < 256) {
         snprintf(ctx->msg, sizeof(ctx->msg), "scw_measure_peak: a device buffer is required (%s)",
                  mem ? ">= 1 GiB recommended: larger than L2" : "256 bytes");
@@ -139,6 +162,7 @@ extern "C" int32_t scw_measure_peak(scw_ctx* ctx, int32_t which, void* buf, size
             case SCW_PEAK_FP64_DMMA: k_peak_dmma<<<sms * 8, 256, 0, ctx->stream>>>(iters, (double*)buf); break;
             case SCW_PEAK_FP32_FMA: k_peak_ffma<<<sms * 8, 256, 0, ctx->stream>>>(iters, (float*)buf); break;
             case SCW_PEAK_MUFU: k_peak_mufu<<<sms * 8, 256, 0, ctx->stream>>>(iters, (float*)buf); break;
+            case SCW_PEAK_MUFU_MIX: k_peak_mufu_mix<<<sms * 8, 256, 0, ctx->stream>>>(iters, (float*)buf); break;
             case SCW_PEAK_HBM_READ: k_peak_read<<<sms * 4, 512, 0, ctx->stream>>>((const uint4*)buf, n16, (unsigned*)buf); break;
             case SCW_PEAK_HBM_WRITE: k_peak_write<<<sms * 4, 512, 0, ctx->stream>>>((uint4*)buf, n16); break;
             default: k_peak_write_tma<<<sms * 4, 128, 2 * PEAK_TMA_CHUNK, ctx->stream>>>((uint8_t*)buf, n_chunks); break;
@@ -172,6 +196,7 @@ extern "C" int32_t scw_measure_peak(scw_ctx* ctx, int32_t which, void* buf, size
         case SCW_PEAK_FP64_DMMA: *value = threads / 32 * iters * 8.0 * (2.0 * 8 * 8 * 4) / s / 1e12; break;   // TFLOP/s
         case SCW_PEAK_FP32_FMA: *value = threads * iters * 16.0 * 2.0 / s / 1e12; break;                      // TFLOP/s
         case SCW_PEAK_MUFU: *value = threads * iters * 8.0 / s / 1e9; break;                                  // Gop/s
+        case SCW_PEAK_MUFU_MIX: *value = threads * iters * 8.0 * 3.0 / s / 1e9; break;                        // Gop/s (3 per term)
         case SCW_PEAK_HBM_WRITE_TMA: *value = (double)n_chunks * PEAK_TMA_CHUNK / s / 1e9; break;             // GB/s
         default: *value = (double)n16 * 16.0 / s / 1e9; break;                                                // GB/s
     }
