@@ -381,6 +381,25 @@ def test_twiddle_cache_and_calibration(scw):
         c.close()
 
 
+def test_measure_peak_units_and_errors(scw, ctx):
+    """scw_measure_peak: every unit returns a rate in a sane range for a B200 (an order of magnitude either side of the
+    nominal figures), the sin + cos + ex2 mix runs on the same pipe as the ex2 chain, unknown units are refused."""
+    from paper_2404_07293_b200 import binding as b
+    peaks = ctx.measure_peaks(reps=2, hbm_bytes=1 << 28)
+    assert set(peaks) == set(b.SCW_PEAKS)
+    assert 10.0 < peaks["fp64_dmma_tflops"] < 100.0 and 20.0 < peaks["fp32_fma_tflops"] < 200.0
+    assert 1000.0 < peaks["mufu_gops"] < 10000.0
+    assert 0.8 < peaks["mufu_sincosex2_gops"] / peaks["mufu_gops"] < 1.2
+    for k in ("hbm_read_gbs", "hbm_write_gbs", "hbm_write_tma_gbs"):
+        assert 2000.0 < peaks[k] < 12000.0, (k, peaks[k])
+    buf = torch.empty(1 << 20, dtype=torch.uint8, device="cuda")
+    v = ctypes.c_double()
+    rc = ctx.L.scw_measure_peak(ctx._h, 99, ctypes.c_void_p(buf.data_ptr()), buf.numel(), 1, ctypes.byref(v))
+    assert rc == 5 and v.value == 0.0                                        # SCW_ERR_VALUE
+    rc = ctx.L.scw_measure_peak(ctx._h, 2, None, 0, 1, ctypes.byref(v))
+    assert rc == 1                                                           # SCW_ERR_NULL
+
+
 def test_kernel_timeline_of_the_sweep_kernels(scw):
     """scw_profile_timeline: every tensor-core sweep launch leaves its exit time on the device clock; entries come oldest
     first, alternate assembly / synthesis, never decrease, and a call that is not a sweep leaves them alone."""
