@@ -186,17 +186,49 @@ __global__ void __launch_bounds__(LU_THREADS, 1) k_lu_panel(const LuPanel p)
     }
 }
 
-// Row interchanges of panel [k0, k0 + nb) applied, in order, to every column outside the panel: one thread per column.
-__global__ void k_lu_laswp(double2* __restrict__ A, int64_t n, int64_t ld, int64_t k0, int nb, const int* __restrict__ piv)
+// Row interchanges of panel [k0, k0 + nb) applied, in order, to every column outside the panel.  A thread per column
+// replaying the nb interchanges one after the other is a chain of nb dependent round trips to memory (47 us per panel at
+// n = 4356).  Instead every block replays them once on an index array in shared memory (idx[r] = the row whose content ends
+// up in row r), which leaves at most 2 nb rows to move (the diagonal rows and the pivot rows); thread = (move, half of the
+// block's LSW_COLS columns) then loads its values -- all independent --, the block synchronises, and the values are stored:
+// two round trips.  Shared memory: n ints.
+constexpr int LSW_COLS = 32;                                       // columns per block
+__global__ void __launch_bounds__(256) k_lu_laswp(double2* __restrict__ A, int64_t n, int64_t ld, int64_t k0, int nb,
+                                                  const int* __restrict__ piv)
 {
-    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= n - nb) return;
-    if (c >= k0) c += nb;                                         // skip the panel's own columns
-    double2* col = A + c * ld;
-    for (int j = 0; j < nb; ++j) {
-        const int64_t r = k0 + j, q = piv[r];
-        if (q != r) { const double2 t = col[r]; col[r] = col[q]; col[q] = t; }
+    extern __shared__ int lsw_idx[];
+    const int tid = threadIdx.x;
+    for (int64_t i = tid; i < n; i += 256) lsw_idx[i] = (int)i;
+    __syncthreads();
+    if (tid == 0)
+        for (int j = 0; j < nb; ++j) {
+            const int r = (int)k0 + j, q = piv[r];
+            if (q != r) { const int t = lsw_idx[r]; lsw_idx[r] = lsw_idx[q]; lsw_idx[q] = t; }
+        }
+    __syncthreads();
+    const int m = tid & 127, half = tid >> 7;                      // LU_NB <= 64: at most 128 rows change
+    int dst = -1;
+    if (m < nb) dst = (int)k0 + m;
+    else if (m < 2 * nb) {
+        dst = piv[k0 + m - nb];
+        if (dst < k0 + nb) dst = -1;                               // a pivot inside the diagonal block: covered by m < nb
     }
+    const int src = dst >= 0 ? lsw_idx[dst] : -1;
+    const bool active = dst >= 0 && src != dst;                    // (the same pivot row twice: two threads move the same value)
+    constexpr int PER = LSW_COLS / 2;
+    double2 v[PER];
+    int64_t col[PER];
+#pragma unroll
+    for (int e = 0; e < PER; ++e) {
+        int64_t c = (int64_t)blockIdx.x * LSW_COLS + half * PER + e;
+        if (c >= k0) c += nb;                                      // skip the panel's own columns
+        col[e] = c < n ? c : -1;
+        if (active && col[e] >= 0) v[e] = A[col[e] * ld + src];
+    }
+    __syncthreads();                                               // every value of the block's columns is read before any is written
+#pragma unroll
+    for (int e = 0; e < PER; ++e)
+        if (active && col[e] >= 0) A[col[e] * ld + dst] = v[e];
 }
 
 // U12 = L11^-1 A12 (L11 unit lower, nb x nb): one warp per column of A12, lane l holds rows l and l + 32.
@@ -262,7 +294,19 @@ __global__ void __launch_bounds__(256) k_trsv_block(const double2* __restrict__ 
     extern __shared__ __align__(16) unsigned char trsv_smem[];
     double2* T = reinterpret_cast<double2*>(trsv_smem);            // column-major nb x nb
     __shared__ double2 xs[LU_NB];
-    for (int idx = threadIdx.x; idx < nb * nb; idx += 256) T[idx] = A[(k0 + idx / nb) * ld + k0 + idx % nb];
+    for (int i0 = 0; i0 < nb * nb; i0 += 256 * 8) {     // eight independent loads per thread in flight
+        double2 v[8];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+            const int idx = i0 + e * 256 + threadIdx.x;
+            if (idx < nb * nb) v[e] = A[(k0 + idx / nb) * ld + k0 + idx % nb];
+        }
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+            const int idx = i0 + e * 256 + threadIdx.x;
+            if (idx < nb * nb) T[idx] = v[e];
+        }
+    }
     for (int i = threadIdx.x; i < nb; i += 256) xs[i] = x[k0 + i];
     __syncthreads();
     if (threadIdx.x >= 32) return;
@@ -303,7 +347,18 @@ __global__ void __launch_bounds__(256) k_trsv_update(const double2* __restrict__
     const int64_t r = r0 + (int64_t)blockIdx.x * 256 + threadIdx.x;
     if (r >= r1) return;
     double2 acc = x[r];
-    for (int k = 0; k < nb; ++k) {
+    int k = 0;
+    for (; k + 8 <= nb; k += 8) {                       // eight independent loads in flight (one per round trip otherwise)
+        double2 a[8];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) a[e] = A[(k0 + k + e) * ld + r];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+            acc.x -= a[e].x * xk[k + e].x - a[e].y * xk[k + e].y;
+            acc.y -= a[e].x * xk[k + e].y + a[e].y * xk[k + e].x;
+        }
+    }
+    for (; k < nb; ++k) {
         const double2 a = A[(k0 + k) * ld + r];
         acc.x -= a.x * xk[k].x - a.y * xk[k].y;
         acc.y -= a.x * xk[k].y + a.y * xk[k].x;
@@ -468,6 +523,7 @@ void launch_propagate_alpha(scw_ctx* ctx, const scw_stack* st, const void* r0, v
     cudaFuncSetAttribute(k_lu_trsm, cudaFuncAttributeMaxDynamicSharedMemorySize, LU_NB * LU_NB * 16);
     cudaFuncSetAttribute(k_trsv_block, cudaFuncAttributeMaxDynamicSharedMemorySize, LU_NB * LU_NB * 16);
     cudaFuncSetAttribute(k_lu_apply_piv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(n * 8));
+    cudaFuncSetAttribute(k_lu_laswp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(n * 4));
     cudaMemsetAsync(misc, 0, 64, ctx->stream);
     for (int l = 0; l < st->n_layers; ++l) {
         const double t_over_lambda = (st->z_if[l + 1] - st->z_if[l]) / st->lambda;
@@ -493,7 +549,7 @@ void launch_propagate_alpha(scw_ctx* ctx, const scw_stack* st, const void* r0, v
             }
             if (n > nb) {
                 KernelScope ks(ctx, KC_ALPHA_LU);
-                k_lu_laswp<<<(unsigned)((n - nb + 255) / 256), 256, 0, ctx->stream>>>(A, n, n, k0, nb, piv);
+                k_lu_laswp<<<(unsigned)((n - nb + LSW_COLS - 1) / LSW_COLS), 256, (size_t)n * 4, ctx->stream>>>(A, n, n, k0, nb, piv);
             }
             const int64_t rest = n - k0 - nb;
             if (rest > 0) {
