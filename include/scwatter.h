@@ -19,9 +19,10 @@
  *  - Ownership: the caller owns every input, output and workspace buffer.  The library never
  *    allocates or frees device memory and keeps no caller pointer past the call, except the
  *    workspace registered with scw_set_workspace(), which it uses as scratch during calls.
- *  - Asynchrony: all work is enqueued on the ctx's CUDA stream; no call synchronises.  Outputs
+ *  - Asynchrony: all work is enqueued on the ctx's CUDA stream; no call synchronises (the few that do say so).  Outputs
  *    are valid once the caller has synchronised that stream.  Descriptor structs are HOST memory
- *    and are copied by value during the call.
+ *    and are copied by value during the call.  The device-buffer calls may be captured into a CUDA graph (stream
+ *    capture) once the workspace has its final size; inputs and outputs of one call must not overlap.
  *  - One ctx per host thread.  There is no CPU fallback: scw_create fails with
  *    SCW_ERR_UNSUPPORTED on a device that is not compute capability 10.x.
  *

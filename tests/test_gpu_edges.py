@@ -381,6 +381,36 @@ def test_twiddle_cache_and_calibration(scw):
         c.close()
 
 
+def test_sweep_captured_in_a_cuda_graph(scw):
+    """The library only enqueues work on the ctx stream (no synchronisation, no allocation): a cached sweep can be captured
+    into a CUDA graph and replayed; the replay writes what the plain call writes."""
+    s = torch.cuda.Stream()
+    c = scw.Context(0, stream=s)
+    try:
+        c.set_cache(True)
+        lays = [ragged_layer(9, 7, 252, np.complex64, seed=90 + i) for i in range(3)]
+        Ls = [scw.Layer.from_numpy(l, "cuda") for l in lays]
+        x, y, z = dev(np.arange(150) * 3.0 / 150), dev(np.arange(140) * 4.5 / 140), dev(np.linspace(-0.2, 0.8, 5))
+        out = [torch.empty((5, 3, 140, 150), dtype=torch.complex64, device="cuda") for _ in Ls]
+        with torch.cuda.stream(s):
+            for _ in range(2):                                              # warm: workspace sized, twiddles cached
+                scw.scw_sweep_wavelengths(c, Ls, [z] * 3, x, y, out=out)
+            s.synchronize()
+            ref = [o.clone() for o in out]
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=s):
+                scw.scw_sweep_wavelengths(c, Ls, [z] * 3, x, y, out=out)
+            for o in out:
+                o.zero_()
+            g.replay()
+            s.synchronize()
+        for a, b, l in zip(out, ref, lays):
+            assert torch.equal(a, b)
+            assert rel_err(a.cpu().numpy(), oracle.tier_b_grid(x=x.cpu().numpy(), y=y.cpu().numpy(), z=z.cpu().numpy(), **l)) <= 2e-4
+    finally:
+        c.close()
+
+
 def test_measure_peak_units_and_errors(scw, ctx):
     """scw_measure_peak: every unit returns a rate in a sane range for a B200 (an order of magnitude either side of the
     nominal figures), the sin + cos + ex2 mix runs on the same pipe as the ex2 chain, unknown units are refused."""
