@@ -69,6 +69,7 @@ inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 // Timeline ring (see scw_ctx::tl_ring): the slot the next launch of class kc stamps its exit time into, NULL if no ring.
 constexpr int TL_RING = 128;
+static_assert(sizeof(((scw_ctx*)nullptr)->tl_class) / sizeof(int) == TL_RING, "scw_ctx::tl_class holds one class per ring slot");
 inline unsigned long long* tl_next(scw_ctx* ctx, int kc)
 {
     if (!ctx->tl_ring) return nullptr;
