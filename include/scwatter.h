@@ -202,6 +202,43 @@ int32_t scw_eval_points(scw_ctx* ctx, const scw_modes* modes, int64_t N, const d
 int32_t scw_points_workspace(scw_ctx* ctx, const scw_modes* modes, int64_t N, size_t* bytes);
 
 /*
+ * scw_eval_points for callers that cannot hand the library any scratch memory.
+ *
+ * Who this is for: code that runs where device memory can no longer be obtained -- a plug-in called from inside a host
+ * application whose memory pool already owns the whole GPU, a real-time loop that has promised not to touch the allocator
+ * after start-up (cudaMalloc takes a process-wide lock and may synchronise the device), or an out-of-memory handler that
+ * still wants one last field evaluation.  Such a caller cannot cudaMalloc a workspace for
+ * scw_set_workspace, and scw_eval_points needs one for complex64 plane-wave tables (it tabulates the J waves there
+ * before summing them).
+ *
+ * This call needs none and allocates nothing: no cudaMalloc / cudaFree, no event or stream creation, no workspace.
+ * Its table lives in a fixed array compiled into libscw.so (SCW_POINTS_NOALLOC_MAX_J entries of 96 bytes plus a
+ * 256-byte header, 768.25 KiB); every GPU that loads the library carries that array until the process exits, whether
+ * or not this function is ever called.  Only the SCW_MODES_PLANEWAVE kind is served (the dense kind needs scratch that
+ * grows with M * N).  modes, N, r, E: exactly as scw_eval_points; inputs and outputs stay the caller's.  The registered
+ * workspace, if any, is neither needed nor touched.  The arithmetic is that of scw_eval_points (same kernels, same
+ * domain notes): for equal inputs the two calls return equal fields.
+ *
+ * Limit: J <= SCW_POINTS_NOALLOC_MAX_J for SCW_C64; a larger table is refused with SCW_ERR_SHAPE before anything is
+ * enqueued (scw_last_error names the limit).  SCW_C128 tables use no scratch and are accepted at any J.
+ *
+ * First call on a device: it looks up where that GPU keeps the array (once per device per process, under a lock; this
+ * may make the CUDA runtime load the library's kernels on that GPU).  Make that first call during start-up, before any
+ * stream capture begins; later calls only enqueue one 24-byte memset and two kernels on the ctx stream.  A
+ * cudaDeviceReset() invalidates the looked-up address: do not reset a device this function has been used on.
+ *
+ * Sharing: there is ONE array per GPU, shared by every ctx, stream and host thread of the process, and it keeps what the
+ * last call left in it.  The call rewrites what it reads (the header is cleared, the J table entries are rebuilt) in
+ * stream order, so back-to-back calls on one stream are safe.  Two calls that can overlap on the same GPU -- different
+ * streams, different ctxs, different threads -- race on the table and return garbage: order them yourself (one stream,
+ * or an event between them).
+ * Errors: NULL, SHAPE (N < 0, J <= 0, J above the limit, wrong struct_size), DTYPE, ALIGN, VALUE,
+ * UNSUPPORTED (SCW_MODES_DENSE), CUDA (address look-up or launch failed; see scw_last_cuda_error).
+ */
+#define SCW_POINTS_NOALLOC_MAX_J 8192
+int32_t scw_eval_points_noalloc(scw_ctx* ctx, const scw_modes* modes, int64_t N, const double* r, void* E);
+
+/*
  * Batched grid evaluation: assembly + synthesis for every (wavelength, layer) instance in one
  * call (spectroscopy sweep).  All instances share U, Vn, X, Y, dtype and the
  * x/y grid (the twiddles are wavelength-free: k s_m . r = 2 pi (u x/X + v y/Y), eq. 6).  J and Fz may differ between

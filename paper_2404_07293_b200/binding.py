@@ -25,7 +25,7 @@ EXPORTS = [
     "scw_version", "scw_create", "scw_destroy", "scw_set_stream", "scw_set_workspace", "scw_set_option",
     "scw_last_error", "scw_last_cuda_error", "scw_required_workspace", "scw_launch_count", "scw_last_kernels",
     "scw_assemble_spectra", "scw_assemble_workspace", "scw_synthesize_grid", "scw_synthesize_workspace",
-    "scw_eval_points", "scw_points_workspace", "scw_sweep_wavelengths", "scw_sweep_workspace",
+    "scw_eval_points", "scw_points_workspace", "scw_eval_points_noalloc", "scw_sweep_wavelengths", "scw_sweep_workspace",
     "scw_sweep_wavelengths_host", "scw_sweep_host_workspace",
     "scw_profile_classes", "scw_profile_name", "scw_profile_read", "scw_profile_reset",
     "scw_exterior_spectra", "scw_exterior_points", "scw_exterior_points_workspace", "scw_exterior_grid",
@@ -118,6 +118,7 @@ def lib():
                                                POINTER(c_size_t)]
         L.scw_eval_points.argtypes = [c_void_p, POINTER(scw_modes), c_int64, c_void_p, c_void_p]
         L.scw_points_workspace.argtypes = [c_void_p, POINTER(scw_modes), c_int64, POINTER(c_size_t)]
+        L.scw_eval_points_noalloc.argtypes = [c_void_p, POINTER(scw_modes), c_int64, c_void_p, c_void_p]
         L.scw_sweep_wavelengths.argtypes = [c_void_p, c_int64, POINTER(scw_layer), POINTER(c_int64),
                                             POINTER(c_void_p), c_int64, c_void_p, c_int64, c_void_p,
                                             POINTER(c_void_p), POINTER(c_int64)]
@@ -408,6 +409,25 @@ def scw_eval_points(ctx, modes, r, out=None):
     if out is None:
         out = torch.empty((N, 3), dtype=dtype, device=ctx.device)
     ctx.check(ctx.L.scw_eval_points(ctx._h, byref(m), N, _p(r), _p(out)))
+    return out
+
+
+SCW_POINTS_NOALLOC_MAX_J = 8192
+
+
+def scw_eval_points_noalloc(ctx, modes, r, out):
+    """scw_eval_points for a caller that cannot allocate GPU memory (a plug-in inside an application whose pool owns the
+    whole device, a real-time loop that must stay off the allocator, an out-of-memory handler): the plane-wave table
+    goes into an array built into libscw.so instead of a workspace, so neither the library nor this wrapper allocates
+    anything -- `out` (N, 3) is required and must be the caller's own tensor.  modes: a PlaneWaves table with at most
+    SCW_POINTS_NOALLOC_MAX_J waves for complex64 (more is refused with ScwError, status 2).  All callers on one GPU share
+    that array: do not let two of these calls overlap on the device.  Make the first call per device at start-up."""
+    if isinstance(modes, Layer):
+        raise ScwError(8, "scw_eval_points_noalloc takes a PlaneWaves table, not a Layer")
+    if out is None:
+        raise ScwError(1, "scw_eval_points_noalloc: pass the output tensor (this call allocates nothing)")
+    m = modes.struct()
+    ctx.check(ctx.L.scw_eval_points_noalloc(ctx._h, byref(m), r.shape[0], _p(r), _p(out)))
     return out
 
 

@@ -1099,6 +1099,32 @@ int32_t scw_eval_points(scw_ctx* ctx, const scw_modes* modes, int64_t N, const d
     return check_launch(ctx, "scw_eval_points");
 }
 
+// No-allocation variant of the plane-wave point path: see include/scwatter.h.  Everything is checked before the first
+// CUDA call that enqueues work; the table limit is a property of the library image, not of the ctx.
+int32_t scw_eval_points_noalloc(scw_ctx* ctx, const scw_modes* modes, int64_t N, const double* r, void* E)
+{
+    if (int32_t s = check_ctx(ctx)) return s;
+    if (int32_t s = check_modes(ctx, modes, "scw_eval_points_noalloc")) return s;
+    if (modes->kind != SCW_MODES_PLANEWAVE)
+        return fail(ctx, SCW_ERR_UNSUPPORTED, "scw_eval_points_noalloc: only SCW_MODES_PLANEWAVE tables (the dense kind needs "
+                                              "scratch that grows with the problem: use scw_eval_points with a workspace)");
+    if (N < 0) return fail(ctx, SCW_ERR_SHAPE, "scw_eval_points_noalloc: N=%lld < 0", (long long)N);
+    if (modes->dtype == SCW_C64 && modes->J > (int64_t)SCW_POINTS_NOALLOC_MAX_J)
+        return fail(ctx, SCW_ERR_SHAPE, "scw_eval_points_noalloc: J=%lld plane waves exceed the built-in table of "
+                                        "SCW_POINTS_NOALLOC_MAX_J=%d entries; split the table or use scw_eval_points",
+                    (long long)modes->J, (int)SCW_POINTS_NOALLOC_MAX_J);
+    if (N == 0) return SCW_OK;
+    if (!r || !E) return fail(ctx, SCW_ERR_NULL, "scw_eval_points_noalloc: r and E are required");
+    if (!aligned(r, 8) || !aligned(E, esize(modes->dtype)))
+        return fail(ctx, SCW_ERR_ALIGN, "scw_eval_points_noalloc: r/E misaligned");
+    const cudaError_t e = launch_points_planewave_noalloc(ctx, modes, N, r, E);
+    if (e != cudaSuccess) {
+        ctx->cuda_err = (int32_t)e;
+        return fail(ctx, SCW_ERR_CUDA, "scw_eval_points_noalloc: %s", cudaGetErrorString(e));
+    }
+    return check_launch(ctx, "scw_eval_points_noalloc");
+}
+
 // ------------------------------------------------------------------------------------------
 static int32_t check_exterior(scw_ctx* ctx, const scw_exterior* e, const char* who)
 {

@@ -267,6 +267,9 @@ struct PwTableInfo { size_t bytes; };
 size_t points_table_bytes(int dtype, int64_t J);
 void launch_points_planewave(scw_ctx* ctx, const scw_modes* m, int64_t N, const double* r, void* E,
                              void* table);
+// same sum with the table in the library's built-in array (scw_eval_points_noalloc): allocates nothing; returns the CUDA
+// error of the address look-up / memset, launch errors are left for cudaGetLastError
+cudaError_t launch_points_planewave_noalloc(scw_ctx* ctx, const scw_modes* m, int64_t N, const double* r, void* E);
 // dense form, per-point synthesis: E[p,comp] = sum_m P[comp*M+m, p] exp(i 2 pi (u x_p/X + v y_p/Y))
 void launch_point_synth(scw_ctx* ctx, int dtype, int U, int Vn, double X, double Y, int64_t n,
                         const double* r, const void* P, int64_t ldP, void* E);

@@ -12,6 +12,8 @@
 // and folded into c0), so the limit applies to the EXTENT of the point cloud, not to its distance from the origin;
 // a block that holds a point whose bound |a|_max . |r - r_0| reaches 2^19 turns takes a second loop that reduces every
 // term with rint first (any finite coordinate is then evaluated correctly, at ~1.3x the cost for that block).
+#include <mutex>
+
 #include "scw_internal.h"
 
 namespace scw {
@@ -255,6 +257,68 @@ void launch_points_planewave(scw_ctx* ctx, const scw_modes* m, int64_t N, const 
             m->J, N, 1.0 / m->lambda, r, m->sx, m->sy, (const double2*)m->gamma, m->zref,
             (const double2*)m->p, (double2*)E);
     }
+}
+
+// ------------------------------------------------------------------------------------------
+// scw_eval_points_noalloc (include/scwatter.h): the same two complex64 kernels with the mode table in an array that is
+// part of the library image instead of the caller's workspace, for callers that cannot allocate device memory.
+//
+// g_pw_noalloc is a __device__ variable.  Inside kernels of THIS file its name is the array; in host code the name only
+// stands for the symbol (taking its address on the host gives a host address that no kernel may be handed), so the host
+// asks the runtime where the current device keeps it -- cudaGetSymbolAddress -- and passes that pointer to the kernels
+// like any other scratch buffer.  Every device has its own copy at its own address: the look-up is done once per device,
+// with that device current, and remembered in g_pw_noalloc_addr.
+constexpr size_t PW_NOALLOC_BYTES = PW_HEADER_BYTES + (size_t)SCW_POINTS_NOALLOC_MAX_J * sizeof(PwMode);
+static __device__ __align__(256) unsigned char g_pw_noalloc[PW_NOALLOC_BYTES];
+
+constexpr int PW_NOALLOC_MAX_DEV = 64;              // devices whose address is remembered; beyond: looked up every call
+static std::mutex g_pw_noalloc_mu;
+static void* g_pw_noalloc_addr[PW_NOALLOC_MAX_DEV]; // device address of g_pw_noalloc on device d, NULL = not looked up yet
+
+// Device address of the built-in table on `device`, which the caller has made current.  No allocation.
+static cudaError_t pw_noalloc_scratch(int device, void** out)
+{
+    std::lock_guard<std::mutex> lk(g_pw_noalloc_mu);
+    const bool slot = device >= 0 && device < PW_NOALLOC_MAX_DEV;
+    if (slot && g_pw_noalloc_addr[device]) {
+        *out = g_pw_noalloc_addr[device];
+        return cudaSuccess;
+    }
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_pw_noalloc);
+    if (e != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    if (slot) g_pw_noalloc_addr[device] = p;
+    *out = p;
+    return cudaSuccess;
+}
+
+// Enqueues header clear + table + sum on the ctx stream (SCW_C64, J <= SCW_POINTS_NOALLOC_MAX_J, checked by the entry
+// point).  Launch accounting without KernelScope: its profiling branch creates CUDA events, which this path must not.
+cudaError_t launch_points_planewave_noalloc(scw_ctx* ctx, const scw_modes* m, int64_t N, const double* r, void* E)
+{
+    if (m->dtype != SCW_C64) {                      // complex128: no table at all, the plain kernel
+        ctx->launches++;
+        ctx->last_classes |= 1ull << KC_POINTS;
+        k_points_pw_c128<<<(unsigned)((N + 127) / 128), 128, 0, ctx->stream>>>(
+            m->J, N, 1.0 / m->lambda, r, m->sx, m->sy, (const double2*)m->gamma, m->zref, (const double2*)m->p, (double2*)E);
+        return cudaSuccess;
+    }
+    void* scratch = nullptr;
+    if (cudaError_t e = pw_noalloc_scratch(ctx->device, &scratch)) return e;
+    PwHeader* hdr = static_cast<PwHeader*>(scratch);
+    PwMode* modes = reinterpret_cast<PwMode*>(static_cast<char*>(scratch) + PW_HEADER_BYTES);
+    // the array still holds the previous call's maxima and table: the maxima must start at zero (atomicMax), the J
+    // entries the sum reads are all rewritten by the table kernel
+    if (cudaError_t e = cudaMemsetAsync(hdr, 0, sizeof(PwHeader), ctx->stream)) return e;
+    ctx->launches += 2;
+    ctx->last_classes |= (1ull << KC_POINTS_TABLE) | (1ull << KC_POINTS);
+    k_points_table<float2><<<(unsigned)((m->J + 127) / 128), 128, 0, ctx->stream>>>(
+        m->J, 1.0 / m->lambda, m->sx, m->sy, (const double2*)m->gamma, m->zref, (const float2*)m->p, r, hdr, modes);
+    const int64_t per_block = PW_THREADS * PW_PPT;
+    k_points_pw_c64<<<(unsigned)((N + per_block - 1) / per_block), PW_THREADS, 0, ctx->stream>>>(
+        m->J, N, r, hdr, modes, (float2*)E);
+    return cudaSuccess;
 }
 
 // ------------------------------------------------------------------------------------------
