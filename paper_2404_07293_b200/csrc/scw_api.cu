@@ -597,9 +597,17 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
             cudaMemsetAsync(ctl, 0, n_ctl * sizeof(int), ctx->stream);
             clean = true;
         }
+        // ints [0, clean_upto) of the control block hold zeros at this point of the stream.  Every run lays its per-CTA
+        // timers, timeline ring, weight images and partial tiles out right behind ITS OWN counters, so after a run only its
+        // own counters are known clean: a larger run that follows gets its counters cleared first.
+        size_t clean_upto = n_ctl;
         for (const SweepRun& r : runs) {
             const int64_t i0 = r.i0, fz = Fz[i0];
             const int g = r.n;
+            size_t n_run = 0;
+            tc_assemble_ctl(ctx, R, inst[i0].J, fz, g, a_scr, &ctl, &n_run);
+            if (n_run > clean_upto) cudaMemsetAsync(ctl, 0, n_run * sizeof(int), ctx->stream);
+            clean_upto = n_run;
             TcFixup fix = {};
             int* sched = nullptr;
             int n_sched = 0;
@@ -623,7 +631,7 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
                                          det ? &td : nullptr);
         }
         if (!ctx->cache_on) ctx->clean_img = nullptr;   // trusted across calls only under SCW_OPT_CACHE
-        ctx->clean_ints = n_ctl;
+        ctx->clean_ints = clean_upto;                   // what the LAST run left clean, not the largest run's block
         return;
     }
     const Twiddles tw = run_twiddles(ctx, L0.dtype, L0.U, L0.Vn, L0.X, L0.Y, Nx, x, Ny, y, cv);

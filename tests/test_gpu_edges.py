@@ -476,3 +476,33 @@ def test_sweep_with_mixed_shapes_runs_grouped(scw, ctx):
         sref = oracle.window_sum(oracle.intensity(ref), (3, 140, 2, 33))
         assert np.abs(s.cpu().numpy() - sref).max() / sref.max() <= 4e-4
     assert not any(k.startswith("simt") for k in ctx.last_kernels())
+
+
+def test_sweep_small_run_before_a_large_one(scw):
+    """Runs of different size share one assembly scratch, and each run keeps its per-CTA timers and weight images right
+    behind its own tile counters: a 1-instance run followed by a 6-instance run (2 m-tiles each) must not leave the
+    larger run's counters dirty (its fix-up would be skipped and the spectrum images stay stale).  Every sample against
+    Tier B; then the same with SCW_OPT_CACHE on and the inputs exchanged between two calls (large run first, so that the
+    LAST run of the call is the small one and the next call may not trust the largest run's control block)."""
+    x, y = np.arange(150) * 3.0 / 150, np.arange(40) * 4.5 / 40
+    z = np.linspace(-0.3, 0.8, 4)
+    dx, dy = dev(x), dev(y)
+
+    def check(c, shapes, seed0):
+        lays = [ragged_layer(9, 7, J, np.complex64, seed=seed0 + i) for i, J in enumerate(shapes)]
+        Es = scw.scw_sweep_wavelengths(c, [scw.Layer.from_numpy(l, "cuda") for l in lays], [dev(z)] * len(lays), dx, dy)
+        torch.cuda.synchronize()
+        assert not any(k.startswith("simt") for k in c.last_kernels())
+        for i, (lay, E) in enumerate(zip(lays, Es)):
+            assert rel_err(E.cpu().numpy(), oracle.tier_b_grid(x=x, y=y, z=z, **lay)) <= 2e-4, i
+
+    c = scw.Context(0)
+    try:
+        check(c, [100] + [132] * 6, 300)
+        check(c, [100, 100] + [132] * 3 + [100] + [132] * 5, 320)
+        c.set_cache(True)
+        check(c, [132] * 6 + [100] * 2, 340)
+        check(c, [132] * 6 + [100] * 2, 360)           # same shapes, new inputs: stale images would be call 1's fields
+        check(c, [100] + [132] * 6, 380)
+    finally:
+        c.close()
