@@ -134,6 +134,9 @@ void run_assemble(scw_ctx* ctx, const scw_layer* L, int64_t Fz, const double* z,
         launch_tc_assemble(ctx, L, Fz, z, P, ldP, scratch);
         return;
     }
+    // the weights and the scratch of these paths go where a tensor-core assembly over the same carver keeps its control
+    // block (per-instance sweeps alternate between them): that block is no longer known clean
+    ctx->clean_ctl = nullptr;
     void* W = cv.take((size_t)L->J * Fz * esize(L->dtype));
     if (use_dmma(ctx, L->dtype)) {
         void* scratch = cv.take(dmma_assemble_scratch(R, L->J, Fz, ctx->sm_count));
@@ -311,6 +314,8 @@ int32_t scw_set_option(scw_ctx* ctx, int32_t option, int64_t value)
     if (option == SCW_OPT_PATH && value >= SCW_PATH_AUTO && value <= SCW_PATH_TENSOR) {
         ctx->path = value;
         ctx->tw_valid = false;
+        ctx->clean_ctl = nullptr;       // the other path carves the same workspace bytes differently
+        ctx->clean_img = nullptr;
         return SCW_OK;
     }
     if (option == SCW_OPT_CACHE && (value == 0 || value == 1)) {
@@ -634,6 +639,10 @@ static void run_sweep(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
         ctx->clean_ints = clean_upto;                   // what the LAST run left clean, not the largest run's block
         return;
     }
+    // per-instance path: its P, assembly scratch and synthesis buffers overlay the grouped layout's control block and
+    // spectrum images, so a later grouped sweep must not trust either (SCW_OPT_CACHE)
+    ctx->clean_ctl = nullptr;
+    ctx->clean_img = nullptr;
     const Twiddles tw = run_twiddles(ctx, L0.dtype, L0.U, L0.Vn, L0.X, L0.Y, Nx, x, Ny, y, cv);
     void* P = cv.take((size_t)R * fz_max * esize(L0.dtype));
     const size_t asm_off = cv.off;

@@ -506,3 +506,39 @@ def test_sweep_small_run_before_a_large_one(scw):
         check(c, [100] + [132] * 6, 380)
     finally:
         c.close()
+
+
+def test_cache_survives_alternating_paths_and_layouts(scw):
+    """SCW_OPT_CACHE on: a grouped tensor-core sweep, then a sweep that carves the same workspace differently (the
+    CUDA-core path; a sweep with an instance the grouped kernels cannot take, here J = 1), then the grouped sweep again.
+    The middle sweeps overwrite the grouped layout's control block and image padding: the last sweep must clear them
+    again instead of trusting the cache.  Every sample of every sweep against Tier B."""
+    x, y = np.arange(150) * 3.0 / 150, np.arange(140) * 4.5 / 140
+    z = np.linspace(-0.2, 0.8, 5)
+    dx, dy = dev(x), dev(y)
+
+    def sweep(c, lays):
+        Es = scw.scw_sweep_wavelengths(c, [scw.Layer.from_numpy(l, "cuda") for l in lays], [dev(z)] * len(lays), dx, dy)
+        torch.cuda.synchronize()
+        for i, (lay, E) in enumerate(zip(lays, Es)):
+            assert rel_err(E.cpu().numpy(), oracle.tier_b_grid(x=x, y=y, z=z, **lay)) <= 2e-4, i
+        return c.last_kernels()
+
+    c = scw.Context(0)
+    try:
+        c.set_cache(True)
+        grouped = [ragged_layer(9, 7, 252, np.complex64, seed=400 + i) for i in range(4)]
+        assert not any(k.startswith("simt") for k in sweep(c, grouped))
+        c.set_path(scw.SCW_PATH_SIMT)
+        assert not any(k.startswith("tc_") for k in sweep(c, grouped))
+        c.set_path(scw.SCW_PATH_AUTO)
+        assert not any(k.startswith("simt") for k in sweep(c, grouped))
+        # per-instance layout in the middle: one instance with a single mode
+        mixed = [ragged_layer(9, 7, 252, np.complex64, seed=410), ragged_layer(9, 7, 1, np.complex64, seed=411),
+                 ragged_layer(9, 7, 252, np.complex64, seed=412)]
+        sweep(c, mixed)
+        assert not any(k.startswith("simt") for k in sweep(c, grouped))
+        sweep(c, mixed)
+        sweep(c, [ragged_layer(9, 7, 252, np.complex64, seed=420 + i) for i in range(4)])
+    finally:
+        c.close()
