@@ -406,7 +406,10 @@ int32_t scw_build_V_workspace(scw_ctx* ctx, const scw_vbuild* vb, size_t* bytes)
  * layer: one dense complex LU (partial pivoting, blocked, trailing updates on the FP64 tensor cores) and two triangular
  * solves; all arithmetic in fp64, SCW_C64 inputs and outputs are widened / rounded at the boundary.
  * r0, rL: [n] complex<dtype> (device); alpha: HOST array of n_layers device pointers [n]; rL may be NULL.
- * A singular Q^(l) gives non-finite alpha (no error is raised: nothing is read back).
+ * Pivoting: the pivot of column k is the entry of largest |re| + |im| at or below the diagonal (LAPACK's izamax measure);
+ * among equal candidates the one in the smallest row wins, so the factorisation does not depend on the launch geometry.
+ * A singular Q^(l), or one that holds NaN, gives non-finite alpha (no error is raised: nothing is read back); the ctx
+ * and the device stay usable.
  * Errors: NULL, SHAPE, DTYPE, ALIGN, VALUE, WORKSPACE, UNSUPPORTED (n > 128 x #SMs or > 25 600), CUDA.
  */
 typedef struct {

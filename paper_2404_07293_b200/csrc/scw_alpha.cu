@@ -145,6 +145,10 @@ __global__ void __launch_bounds__(LU_THREADS, 1) k_lu_panel(const LuPanel p)
                 if (ov > gv || (ov == gv && orow < gr)) { gv = ov; gr = orow; gc = oc; }
             }
             if (lane == 0) {
+                // no candidate at all: every entry at or below the diagonal is NaN (`m > bv` is false for NaN), the normal
+                // state of the columns after an exactly zero pivot (0/0) or of a Q that holds NaN.  Keep the diagonal row
+                // (published in slot gridDim.x) so that the NaNs simply propagate into alpha, as the header promises.
+                if (gr == 0x7fffffff) { gr = (int)gj; gc = (int)gridDim.x; }
                 s_piv = gr;
                 s_win = gc;
                 if (blockIdx.x == 0) {
@@ -203,7 +207,7 @@ __global__ void __launch_bounds__(256) k_lu_laswp(double2* __restrict__ A, int64
     if (tid == 0)
         for (int j = 0; j < nb; ++j) {
             const int r = (int)k0 + j, q = piv[r];
-            if (q != r) { const int t = lsw_idx[r]; lsw_idx[r] = lsw_idx[q]; lsw_idx[q] = t; }
+            if (q != r && q >= 0 && q < n) { const int t = lsw_idx[r]; lsw_idx[r] = lsw_idx[q]; lsw_idx[q] = t; }
         }
     __syncthreads();
     const int m = tid & 127, half = tid >> 7;                      // LU_NB <= 64: at most 128 rows change
@@ -211,7 +215,7 @@ __global__ void __launch_bounds__(256) k_lu_laswp(double2* __restrict__ A, int64
     if (m < nb) dst = (int)k0 + m;
     else if (m < 2 * nb) {
         dst = piv[k0 + m - nb];
-        if (dst < k0 + nb) dst = -1;                               // a pivot inside the diagonal block: covered by m < nb
+        if (dst < k0 + nb || dst >= n) dst = -1;                   // a pivot inside the diagonal block: covered by m < nb
     }
     const int src = dst >= 0 ? lsw_idx[dst] : -1;
     const bool active = dst >= 0 && src != dst;                    // (the same pivot row twice: two threads move the same value)
@@ -279,7 +283,7 @@ __global__ void __launch_bounds__(256) k_lu_apply_piv(int64_t n, const int* __re
     if (threadIdx.x == 0)
         for (int64_t r = 0; r < n; ++r) {
             const int q = pv[r];
-            if (q != r) { const int t = perm[r]; perm[r] = perm[q]; perm[q] = t; }
+            if (q != r && q >= 0 && q < n) { const int t = perm[r]; perm[r] = perm[q]; perm[q] = t; }
         }
     __syncthreads();
     for (int64_t i = threadIdx.x; i < n; i += 256) dst[i] = src[perm[i]];

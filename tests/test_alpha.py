@@ -145,3 +145,133 @@ def test_propagate_alpha_config1_size():
         assert np.abs(rL.cpu().numpy() - ref_r).max() / np.abs(ref_r).max() <= 1e-10
     finally:
         ctx.close()
+
+
+# ------------------------------------------------------------------------------------------------ pivoting
+def rows_moved(A):
+    """How many rows LAPACK's partial pivoting (same |re| + |im| measure as the GPU kernel) exchanges on A."""
+    import scipy.linalg
+    _, piv = scipy.linalg.lu_factor(A)
+    return int((piv != np.arange(len(piv))).sum())
+
+
+def pivoting_stack(kind, n, L, seed, dtype):
+    """Stacks whose Q'_l = Q diag(d_acute) are NOT diagonally dominant (an eigenvector matrix is not), so
+    the LU of eq. 24-25 has to exchange rows:
+      gauss  -- plain complex Gaussian Q, no dominant diagonal at all;
+      perm   -- the well-conditioned stack of random_stack with its rows permuted;
+      last   -- 1.5 x (cyclic shift by n - 8 rows) + noise: the largest entry of every column sits in the last 8 rows of the
+                matrix for every column, i.e. always in the rows of the last CTA of the panel kernel;
+      ties   -- gauss with pairs of candidates of exactly equal |re| + |im| in many columns (3 and 3i; 2 + 1i and 1 + 2i)."""
+    st = random_stack(n, L, seed, dtype=dtype)
+    g = np.random.default_rng(seed + 1000)
+    for l in range(L):
+        if kind in ("gauss", "ties"):
+            A = (g.standard_normal((n, n)) + 1j * g.standard_normal((n, n))) / np.sqrt(2)
+            if kind == "ties":
+                for c in range(0, n, 3):
+                    r1, r2 = g.choice(n, 2, replace=False)
+                    A[r1, c], A[r2, c] = (3.0, 3.0j) if c % 2 else (2.0 + 1.0j, 1.0 + 2.0j)
+        elif kind == "perm":
+            A = st["Q"][l].astype(np.complex128)[g.permutation(n)]
+        elif kind == "last":
+            A = (g.standard_normal((n, n)) + 1j * g.standard_normal((n, n))) / np.sqrt(2 * n)
+            s = n - min(8, n // 2)
+            A[(np.arange(n) + s) % n, np.arange(n)] += 1.5
+        st["Q"][l] = A.astype(dtype)
+    return st
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("dtype,tol", [(np.complex64, 2e-4), (np.complex128, 1e-10)])
+@pytest.mark.parametrize("kind,n,L", [("gauss", 36, 3), ("gauss", 324, 2), ("gauss", 517, 2), ("perm", 324, 3), ("perm", 517, 2),
+                                      ("last", 100, 2), ("last", 517, 2), ("ties", 36, 2), ("ties", 324, 2)])
+def test_propagate_alpha_with_row_exchanges(kind, dtype, tol, n, L):
+    """The LU behind eq. 24-25 on matrices that need partial pivoting: LAPACK exchanges more
+    than a quarter of the rows on every Q'_l here (asserted), so the cross-CTA pivot search, the candidate-row exchange,
+    k_lu_laswp and k_lu_apply_piv all run.  The SOLUTION is compared, not the permutation.  Tolerance: the usual
+    1e-10 / 2e-4 of max|alpha|, not widened: both sides solve in fp64 from the same rounded inputs with the same pivoting
+    measure, and the measured differences stay below 1e-12 up to prod_l cond_2(Q'_l) = 2e7 (asserted < 1e8 here so that
+    eps cond stays well inside the tolerance)."""
+    import torch
+    import paper_2404_07293_b200 as scw
+    st = pivoting_stack(kind, n, L, seed=7 * n + L, dtype=dtype)
+    ref_a, ref_r = oracle.propagate_alpha(**st)
+    cond = 1.0
+    for l in range(L):
+        d_acute, _ = oracle.interface_factors(lam=st["lam"], z_a=st["z_if"][l], z_b=st["z_if"][l + 1], gamma=st["gamma"][l],
+                                              dir=st["dir"][l])
+        Qa = st["Q"][l].astype(np.complex128) * d_acute[None, :]
+        assert rows_moved(Qa) > n // 4, (kind, l)
+        cond *= np.linalg.cond(Qa)
+    assert cond < 1e8
+    ctx = scw.Context(0)
+    try:
+        Qd = [dev(np.ascontiguousarray(q.T)) for q in st["Q"]]
+        alphas, rL = scw.scw_propagate_alpha(ctx, lam=st["lam"], z_if=st["z_if"], Q=Qd, gamma=[dev(g) for g in st["gamma"]],
+                                             dir=[dev(d) for d in st["dir"]], r0=dev(st["r0"]))
+        torch.cuda.synchronize()
+        for l in range(L):
+            assert np.abs(alphas[l].cpu().numpy() - ref_a[l]).max() / np.abs(ref_a[l]).max() <= tol, (l, cond)
+        assert np.abs(rL.cpu().numpy() - ref_r).max() / np.abs(ref_r).max() <= tol
+    finally:
+        ctx.close()
+
+
+@pytest.mark.gpu
+def test_propagate_alpha_config1_size_with_row_exchanges():
+    """n = 4356 (config 1), complex128, plain Gaussian Q: 69 panels that all pivot across CTAs."""
+    import torch
+    import paper_2404_07293_b200 as scw
+    n = 4356
+    st = pivoting_stack("gauss", n, 1, seed=11, dtype=np.complex128)
+    ref_a, ref_r = oracle.propagate_alpha(**st)
+    d_acute, _ = oracle.interface_factors(lam=st["lam"], z_a=st["z_if"][0], z_b=st["z_if"][1], gamma=st["gamma"][0], dir=st["dir"][0])
+    Qa = st["Q"][0] * d_acute[None, :]
+    assert rows_moved(Qa) > n // 4
+    tol = 1e-10
+    ctx = scw.Context(0)
+    try:
+        alphas, rL = scw.scw_propagate_alpha(ctx, lam=st["lam"], z_if=st["z_if"], Q=[dev(np.ascontiguousarray(st["Q"][0].T))],
+                                             gamma=[dev(st["gamma"][0])], dir=[dev(st["dir"][0])], r0=dev(st["r0"]))
+        torch.cuda.synchronize()
+        err = np.abs(alphas[0].cpu().numpy() - ref_a[0]).max() / np.abs(ref_a[0]).max()
+        assert err <= tol, (err, tol)
+        assert np.abs(rL.cpu().numpy() - ref_r).max() / np.abs(ref_r).max() <= tol
+    finally:
+        ctx.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("kind", ["zero_column", "nan_entry", "zero_matrix"])
+def test_propagate_alpha_singular_or_nan_Q_gives_non_finite_alpha_and_a_healthy_ctx(kind):
+    """An exactly singular Q (a zero column: a zero pivot, then 0/0 = NaN below it, then columns without any finite pivot
+    candidate) or a Q holding NaN: alpha comes back non-finite, no error, no fault -- and the same ctx then solves a
+    regular stack correctly (include/scwatter.h: 'the ctx and the device stay usable')."""
+    import torch
+    import paper_2404_07293_b200 as scw
+    n = 200
+    st = random_stack(n, 2, seed=21)
+    bad = dict(st, Q=[q.copy() for q in st["Q"]])
+    if kind == "zero_column":
+        bad["Q"][0][:, 70] = 0.0
+    elif kind == "nan_entry":
+        bad["Q"][0][130, 5] = np.nan
+    else:
+        bad["Q"][0][:] = 0.0
+    ctx = scw.Context(0)
+    try:
+        def run(s):
+            out = scw.scw_propagate_alpha(ctx, lam=s["lam"], z_if=s["z_if"], Q=[dev(np.ascontiguousarray(q.T)) for q in s["Q"]],
+                                          gamma=[dev(g) for g in s["gamma"]], dir=[dev(d) for d in s["dir"]], r0=dev(s["r0"]))
+            torch.cuda.synchronize()
+            return out
+        alphas, _ = run(bad)
+        assert not np.isfinite(alphas[0].cpu().numpy()).all()
+        ref_a, ref_r = oracle.propagate_alpha(**st)
+        alphas, rL = run(st)
+        for l in range(2):
+            assert np.abs(alphas[l].cpu().numpy() - ref_a[l]).max() / np.abs(ref_a[l]).max() <= 1e-10
+        assert np.abs(rL.cpu().numpy() - ref_r).max() / np.abs(ref_r).max() <= 1e-10
+    finally:
+        ctx.close()
