@@ -296,6 +296,13 @@ int32_t scw_set_workspace(scw_ctx* ctx, void* dev_ptr, size_t bytes)
     ctx->tw_valid = false;
     ctx->clean_ctl = nullptr;
     ctx->clean_img = nullptr;
+    // the per-CTA timers and the timeline ring of the last assembly lived in the previous workspace, which the caller may
+    // free now: scw_profile_assembly / scw_profile_timeline report "nothing recorded" until the next launch
+    ctx->last_asm_ns = nullptr;
+    ctx->last_asm_G = 0;
+    ctx->tl_last_ring = nullptr;
+    ctx->tl_ring = nullptr;
+    ctx->tl_seq = 0;
     return SCW_OK;
 }
 
@@ -819,7 +826,7 @@ int32_t scw_calibrate(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
     if (!ctx) return SCW_ERR_NULL;
     if (reps < 1 || reps > 64) return fail(ctx, SCW_ERR_VALUE, "scw_calibrate: reps must be in [1, 64]");
     ctx->split_w.clear();
-    std::vector<unsigned long long> ns(4 * 256);
+    std::vector<unsigned long long> ns;             // [G][4] per-CTA nanoseconds of one assembly launch, sized once G is known
     std::vector<double> best_w;                     // the split with the shortest assembly seen so far (empty = equal)
     double best_us = 1e30;
     const int rounds = 8;
@@ -836,6 +843,7 @@ int32_t scw_calibrate(scw_ctx* ctx, int64_t n_inst, const scw_layer* inst, const
             }
             G = ctx->last_asm_G;
             if (G < 2) return SCW_OK;               // not on the tensor-core assembly: nothing to calibrate
+            if (ns.size() < (size_t)G * 4) ns.resize((size_t)G * 4);
             cudaError_t e = cudaStreamSynchronize(ctx->stream);
             if (e == cudaSuccess)
                 e = cudaMemcpy(ns.data(), ctx->last_asm_ns, (size_t)G * 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost);

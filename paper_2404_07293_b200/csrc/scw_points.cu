@@ -49,8 +49,11 @@ __global__ void k_points_table(int64_t J, double inv_lambda, const double* __res
                                const double* __restrict__ zref, const T2* __restrict__ p,
                                const double* __restrict__ r, PwHeader* __restrict__ hdr, PwMode* __restrict__ table)
 {
-    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= J) return;
+    // every lane stays alive for the warp reduction at the end: lanes past J redo mode J - 1 and only skip the store
+    // (their maxima equal that mode's, so the reduction is unchanged)
+    const int64_t j_raw = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = j_raw < J;
+    const int64_t j = live ? j_raw : J - 1;
     const double x0 = r[0], y0 = r[1], z0 = r[2];                 // phase origin: the first point of the call
     const double2 g = gamma[j];
     PwMode m;
@@ -76,7 +79,7 @@ __global__ void k_points_table(int64_t J, double inv_lambda, const double* __res
         m.prr[c][0] = m.prr[c][1] = (float)v.x;
         m.pii[c][0] = m.pii[c][1] = (float)v.y;
     }
-    table[j] = m;
+    if (live) table[j] = m;
     // per-axis maxima for the domain check of the fast loop: one atomic per warp and axis
     double a3[3] = {fabs(m.ax), fabs(m.ay), fabs(m.az)};
 #pragma unroll
@@ -84,7 +87,7 @@ __global__ void k_points_table(int64_t J, double inv_lambda, const double* __res
         unsigned long long b = (unsigned long long)__double_as_longlong(a3[k]);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
-            const unsigned long long other = __shfl_xor_sync(__activemask(), b, o);
+            const unsigned long long other = __shfl_xor_sync(0xffffffffu, b, o);
             b = other > b ? other : b;
         }
         if ((threadIdx.x & 31) == 0) atomicMax(&hdr->max_a[k], b);

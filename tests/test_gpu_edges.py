@@ -542,3 +542,23 @@ def test_cache_survives_alternating_paths_and_layouts(scw):
         sweep(c, [ragged_layer(9, 7, 252, np.complex64, seed=420 + i) for i in range(4)])
     finally:
         c.close()
+
+
+def test_profile_readers_forget_a_replaced_workspace(scw):
+    """The per-CTA timers and the timeline ring of a sweep live in the workspace.  After the caller registers another
+    workspace (the old one may be freed) the readers must report 'nothing recorded' instead of copying from the old
+    address; the next sweep records again."""
+    c = scw.Context(0)
+    try:
+        lays = [ragged_layer(9, 7, 252, np.complex64, seed=500 + i) for i in range(2)]
+        x, y, z = np.arange(150) * 3.0 / 150, np.arange(140) * 4.5 / 140, np.linspace(-0.2, 0.8, 5)
+        Ls = [scw.Layer.from_numpy(l, "cuda") for l in lays]
+        scw.scw_sweep_wavelengths(c, Ls, [dev(z)] * 2, dev(x), dev(y))
+        assert len(c.assembly_timeline()) >= 1 and len(c.kernel_timeline()) == 2
+        c.reserve(c.workspace_bytes() + (1 << 20))               # a new, larger buffer: scw_set_workspace
+        torch.cuda.empty_cache()                                 # the old one really goes back to the driver
+        assert c.assembly_timeline() == [] and c.kernel_timeline() == []
+        scw.scw_sweep_wavelengths(c, Ls, [dev(z)] * 2, dev(x), dev(y))
+        assert len(c.assembly_timeline()) >= 1 and len(c.kernel_timeline()) == 2
+    finally:
+        c.close()
