@@ -562,3 +562,41 @@ def test_profile_readers_forget_a_replaced_workspace(scw):
         assert len(c.assembly_timeline()) >= 1 and len(c.kernel_timeline()) == 2
     finally:
         c.close()
+
+
+@pytest.mark.parametrize("Nx,Ny", [(1, 150), (150, 1), (1, 1)])
+@pytest.mark.parametrize("U,Vn,J,Fz", [(7, 9, 250, 20), (45, 50, 64, 4)])
+def test_xz_and_yz_planes(scw, Nx, Ny, U, Vn, J, Fz):
+    """x-z and y-z planes ('The same goes for x-z and y-z planes'): the separable synthesis with ONE
+    coordinate along an axis -- a 1-wide axis through the 128 x 128 output tiles of the forced tcgen05 path (complex64),
+    through the DMMA path (complex128) and through the fused detector epilogue; every sample against Tier A."""
+    g = np.random.default_rng(1000 * Nx + Ny)
+    x = np.sort(g.uniform(-2, 5, Nx))
+    y = np.sort(g.uniform(-2, 5, Ny))
+    z = np.linspace(-0.4, 0.9, Fz)
+    for dtype, tol, path in ((np.complex64, 2e-4, "tensor"), (np.complex128, 1e-10, "auto")):
+        lay = ragged_layer(U, Vn, J, dtype, seed=70 + U + Nx)
+        ref = oracle.layer_grid(x=x, y=y, z=z, **lay)
+        c = scw.Context(0)
+        try:
+            if path == "tensor":
+                c.set_path(scw.SCW_PATH_TENSOR)
+            L = scw.Layer.from_numpy(lay, "cuda")
+            E = scw.scw_sweep_wavelengths(c, [L], [dev(z)], dev(x), dev(y))[0]
+            torch.cuda.synchronize()
+            assert E.shape == (Fz, 3, Ny, Nx)
+            assert rel_err(E.cpu().numpy(), ref) <= tol
+            kinds = c.last_kernels()
+            assert any(k.startswith("tc_") for k in kinds) if path == "tensor" else any(k.startswith("dmma") for k in kinds)
+            P = scw.scw_assemble_spectra(c, L, dev(z))
+            E2 = scw.scw_synthesize_grid(c, U=U, Vn=Vn, X=lay["X"], Y=lay["Y"], P=P, x=dev(x), y=dev(y))
+            torch.cuda.synchronize()
+            assert rel_err(E2.cpu().numpy(), ref) <= tol
+            I, S = scw.scw_sweep_detector(c, [L], [dev(z)], dev(x), dev(y))
+            torch.cuda.synchronize()
+            Iref = oracle.intensity(ref)
+            assert np.abs(I[0].cpu().numpy() - Iref).max() / Iref.max() <= 2 * tol
+            sref = oracle.window_sum(Iref, (0, Nx, 0, Ny))
+            assert np.abs(S[0].cpu().numpy() - sref).max() / sref.max() <= 2 * tol
+        finally:
+            c.close()

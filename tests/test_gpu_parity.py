@@ -216,12 +216,14 @@ def test_config4_sweep_full_size(scw, ctx):
         # the BF16x3 rounding level (each is ~1e-5 from the oracle), not bit for bit
         err_one = rel_err(one.cpu().numpy(), Es[i].cpu().numpy().astype(np.complex128))
         assert err_one <= 5e-5, err_one
-    for i in range(0, 64, 7):
+    # every one of the 64 instances against the plain definition (Tier A): 32 seeded samples each = 2048
+    for i in range(64):
         idx = si.sample_subset(cfg, 16 * 256 * 256, 32, lam_index=i // 2, layer=i % 2)
         iz, iy, ix = np.unravel_index(idx, (16, 256, 256))
         ref_a = oracle.layer_samples(xyz=np.column_stack([x[ix], y[iy], zs[i][iz]]), **insts[i])
-        E = Es[i].cpu().numpy()
-        assert np.abs(E[iz, :, iy, ix] - ref_a).max() / np.abs(E).max() <= 2e-4
+        tz, ty, tx = (torch.from_numpy(v).cuda() for v in (iz, iy, ix))
+        got = Es[i][tz, :, ty, tx].cpu().numpy()
+        assert np.abs(got - ref_a).max() / float(Es[i].abs().max()) <= 2e-4, i
 
 
 def test_sweep_host_buffers_match_device_call(scw, ctx):

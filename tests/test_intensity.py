@@ -92,6 +92,14 @@ def test_config4_intensity_full_size_fused(scw):
         for i in (0, 1, 37, 63):
             ref = oracle.intensity(oracle.tier_b_grid(x=x, y=y, z=zs[i], **lays[i]))
             assert np.abs(I[i].cpu().numpy() - ref).max() / ref.max() <= 4e-4
+        # every one of the 64 instances against the plain definition (Tier A): 32 seeded samples each
+        for i in range(len(Ls)):
+            idx = si.sample_subset(c4, 16 * 256 * 256, 32, lam_index=i // 2, layer=i % 2)
+            iz, iy, ix = np.unravel_index(idx, (16, 256, 256))
+            Ea = oracle.layer_samples(xyz=np.column_stack([x[ix], y[iy], zs[i][iz]]), **lays[i])
+            Ia = (np.abs(Ea) ** 2).sum(axis=1)
+            got = I[i][torch.from_numpy(iz).cuda(), torch.from_numpy(iy).cuda(), torch.from_numpy(ix).cuda()].cpu().numpy()
+            assert np.abs(got - Ia).max() / float(I[i].max()) <= 4e-4, i
         E = scw.scw_sweep_wavelengths(ctx, Ls, dz, dx, dy)
         torch.cuda.synchronize()
         for i in range(len(Ls)):
